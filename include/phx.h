@@ -1,0 +1,220 @@
+/*
+ * phx.h — C ABI of the PHOENIX in-memory optimizer-state checkpoint hot path on B200 (sm_100a).
+ *
+ * What it is: the per-iteration replication of a data-parallel rank's sharded optimizer
+ * state (fp32 master weights, Adam first/second moments, step count) taken INSIDE the
+ * distributed-optimizer AdamW update, and the restore of a lost shard from that replica.
+ * Paper: /root/reference/PAPER.md §V-B "Asynchronous Offload Pipeline" (lines 143-154),
+ * §VI-A "In-Memory State Protection" (208-226), §V-C recovery stage 3 (171),
+ * §VI-E/F restoration and resume (248-254).  The peer node's memory of the paper is stood
+ * in for by a pinned host replica on the same box (BASELINE.json:north_star).
+ *
+ * General conventions
+ *   - Every function returns int: PHX_OK (0) or a negative PHX_ERR_*.  No exceptions, no
+ *     aborts, nothing is printed.
+ *   - Pointers named d_* are DEVICE pointers (HBM of the current CUDA device), h_* are HOST
+ *     pointers.  Replica memory must be pinned (page-locked) and mapped: the restore kernel
+ *     reads it directly over the host link.  All buffers are owned by the caller (allocate
+ *     them with any CUDA allocator, e.g. torch); the library never frees them and only owns
+ *     small internals (events, a few hundred bytes of device scratch).
+ *   - Streams are cudaStream_t passed as void*.  Calls that take a stream only ENQUEUE work;
+ *     they never block the host on the device unless stated (phx_snapshot_wait, phx_restore's
+ *     host-side slot validation).  Ordering between the compute stream and the flush stream
+ *     is by library-owned events.  One host thread uses a handle at a time.
+ *   - There is deliberately no fallback: a device that is not compute capability 10.x gives
+ *     PHX_ERR_UNSUPPORTED_DEVICE at phx_shard_bind.
+ *
+ * Memory layout (all little-endian, unit-stride)
+ *   live state   d_p, d_m, d_v : float[n_padded]; d_p_bf16 : bf16[n_padded];
+ *                d_grads_bf16  : bf16[n_padded] (read-only).  Lanes [n, n_padded) are padding:
+ *                they must be zero in p, m, v and grads and the update keeps them exactly zero.
+ *                Bases must be 256-byte aligned.
+ *   snapshot     one packed contiguous buffer of snapshot_bytes =
+ *                256 + 12*n_padded bytes:   header[256] ‖ p[n_padded] ‖ m[n_padded] ‖ v[n_padded]
+ *   staging      d_staging : staging_depth snapshot slots, slot s at byte s*slot_stride
+ *                (slot_stride = snapshot_bytes rounded up to 256).  Step k writes slot k mod depth.
+ *   replica      h_replica : 2 snapshot slots at the same stride (ping-pong):
+ *                the snapshot of step k lands in host slot k mod 2.
+ *   header       phx_snapshot_header_t below — the paper's "metadata envelope (step index,
+ *                parallelism configuration, RNG states)".
+ */
+#ifndef PHX_H
+#define PHX_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PHX_API __attribute__((visibility("default")))
+
+/* ---- errors ---------------------------------------------------------------------------- */
+enum {
+    PHX_OK = 0,
+    PHX_ERR_INVALID_ARG = -1,
+    PHX_ERR_ALIGNMENT = -2,           /* a bound pointer is not 256-byte aligned                 */
+    PHX_ERR_NOT_BOUND = -3,           /* phx_shard_bind has not been called                      */
+    PHX_ERR_STEP_ORDER = -4,          /* step != last_step + 1 (I4 step atomicity) */
+    PHX_ERR_NO_FLUSH_PENDING = -5,    /* flush requested but no un-flushed snapshot exists       */
+    PHX_ERR_NO_COMMITTED_SNAPSHOT = -6,
+    PHX_ERR_LAYOUT_MISMATCH = -7,     /* replica belongs to another logical shard */
+    PHX_ERR_CORRUPT_SLOT = -8,        /* reserved: both slots carry a header that fails checks   */
+    PHX_ERR_CUDA = -9,                /* see phx_last_cuda_error                                  */
+    PHX_ERR_UNSUPPORTED_DEVICE = -10, /* not compute capability 10.x; there is no fallback       */
+    PHX_ERR_SNAPSHOT_DISABLED = -11,  /* flush/restore asked of a shard created with snapshots off */
+    PHX_ERR_NOMEM = -12
+};
+
+/* ---- types ----------------------------------------------------------------------------- */
+typedef struct phx_shard phx_shard_t; /* opaque */
+
+/* One entry per tensor the rank holds after TP/PP slicing, in flattening order. */
+typedef struct {
+    uint64_t numel;
+    uint32_t tensor_id;
+    uint32_t flags; /* reserved (per-tensor no-decay groups); hashed into the layout hash */
+} phx_tensor_desc_t;
+
+enum { PHX_SYNC_STRICT = 0, PHX_SYNC_RELAXED = 1 };
+enum { PHX_RESTORE_BULK_KERNEL = 0, PHX_RESTORE_COPY_ENGINE = 1 };
+
+/* Any field left 0 takes its default; cfg == NULL means all defaults. */
+typedef struct {
+    uint32_t tp_size, tp_rank, pp_size, pp_rank; /* logical identity only; sizes default 1      */
+    uint32_t staging_depth;   /* 1..4 device staging slots; default 2                            */
+    uint32_t sync_mode;       /* PHX_SYNC_STRICT (default): step k+1 waits for commit(k) — the
+                                 paper's single sync point, replay <= 1 step.
+                                 PHX_SYNC_RELAXED: step k+1 waits only until staging slot
+                                 (k+1) mod depth has been drained, replay <= depth steps.        */
+    uint64_t chunk_bytes;     /* D2H chunk size, 4 MiB..256 MiB (rounded to 256 B); default 64 MiB */
+    uint32_t snapshot_disabled; /* 1: plain AdamW + bf16 copy, no staging stores (the paper's
+                                 "mechanism disabled" baseline)                     */
+    uint32_t restore_mode;    /* PHX_RESTORE_BULK_KERNEL (default) | PHX_RESTORE_COPY_ENGINE      */
+    float max_grad_norm;      /* > 0: clip by the shard-local gradient norm before the step       */
+    uint32_t reserved[5];
+} phx_config_t;
+
+typedef struct {
+    uint64_t n;              /* real fp32 elements owned by this rank                             */
+    uint64_t n_padded;       /* plane length: total padded to a multiple of 64*dp_size, / dp_size */
+    uint64_t total_numel;    /* sum of layout numel                                               */
+    uint64_t shard_begin;    /* dp_rank * n_padded: start of the rank's range in the flat space   */
+    uint64_t layout_hash;    /* FNV-1a 64 over the tensor descriptors and dp/tp/pp sizes+tp/pp rank */
+    uint64_t snapshot_bytes; /* 256 + 12*n_padded                                                 */
+    uint64_t slot_stride;    /* snapshot_bytes rounded up to 256                                  */
+    uint32_t n_segments, staging_depth;
+    uint32_t dp_size, dp_rank;
+} phx_shard_info_t;
+
+/* The 256-byte metadata envelope at the front of every snapshot slot. */
+typedef struct {
+    uint8_t magic[8];       /* "PHXSNAP1"                                                         */
+    uint32_t version;       /* 1                                                                  */
+    uint32_t header_bytes;  /* 256                                                                */
+    uint64_t seq_begin;     /* == step                                                            */
+    uint64_t step;          /* state in this slot is the state AFTER optimizer step `step`        */
+    uint64_t n, n_padded, total_numel, shard_begin, layout_hash;
+    uint32_t dp_size, dp_rank, tp_size, tp_rank, pp_size, pp_rank;
+    uint64_t chunk_bytes;
+    uint32_t user_len;      /* bytes used of user[]                                               */
+    uint32_t reserved;
+    uint8_t user[128];      /* opaque caller blob (RNG states...), restored bit-exactly           */
+    uint64_t header_hash;   /* FNV-1a 64 of bytes [0, 240)                                        */
+    uint64_t seq_end;       /* == seq_begin once the slot is committed; written last              */
+} phx_snapshot_header_t;
+
+/* ---- a0: shard definition (host only; works without a GPU) -------------------------------
+ * Flatten the tensor list in order, pad the total up to a multiple of 64*dp_size, cut dp_size
+ * equal contiguous ranges; this rank owns [dp_rank*L, (dp_rank+1)*L) ("sharded model and
+ * optimizer states"; ZeRO-2 distributed optimizer).  A tensor may
+ * straddle ranks; the segment table records the pieces.  layout is copied. */
+PHX_API int phx_shard_create(const phx_tensor_desc_t *layout, size_t n_tensors, uint32_t dp_size,
+                             uint32_t dp_rank, const phx_config_t *cfg, phx_shard_t **out);
+PHX_API int phx_shard_destroy(phx_shard_t *s); /* waits for in-flight flushes, frees internals */
+PHX_API int phx_shard_info(const phx_shard_t *s, phx_shard_info_t *out);
+/* Fills up to cap entries (all four arrays have cap entries); entry i is the i-th piece of
+ * the rank's range: tensor_id, offset inside that tensor, offset inside the shard, length. */
+PHX_API int phx_shard_segments(const phx_shard_t *s, uint32_t *tensor_id, uint64_t *off_in_tensor,
+                               uint64_t *off_in_shard, uint64_t *len, uint32_t cap);
+
+/* ---- binding memory -----------------------------------------------------------------------
+ * d_staging: staging_depth * slot_stride bytes of device memory (may be NULL iff snapshots are
+ * disabled).  h_replica: 2 * slot_stride bytes of pinned, mapped host memory (may be NULL iff
+ * snapshots are disabled).  Requires a CUDA device of compute capability 10.x. */
+PHX_API int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p_bf16,
+                           void *d_staging, void *h_replica);
+/* Declare the bound p, m, v to be the state after optimizer step `step` (0 at initialisation)
+ * and regenerate d_p_bf16 = RNE_bf16(p) on `stream`. */
+PHX_API int phx_shard_set_state(phx_shard_t *s, uint64_t step, void *stream);
+/* Opaque blob (<= 128 bytes) copied into the header of every later snapshot. */
+PHX_API int phx_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len);
+
+/* ---- a1+a2+a3: fused AdamW step + snapshot -------------------------------------------------
+ * Enqueues on `stream`:
+ *   a1 (only if max_grad_norm > 0): S = sum g^2 in fp64 by a fixed two-stage tree, clip
+ *      coefficient c = fp32(min(1, max_grad_norm / (sqrt(S) + 1e-6))) left in device memory;
+ *   a2: wait (stream-side, not host-side) until the previous snapshot is committed (strict) or
+ *      the staging slot about to be written has been drained (relaxed) — PAPER.md:226;
+ *   a3: ONE kernel making one pass over the shard.  Per element, in fp32 with every operation
+ *      individually rounded (no FMA contraction, no flush-to-zero, IEEE sqrt and divide):
+ *        g = widen(g_bf16) * c;  p1 = p * decay;  m' = beta1*m + omb1*g;
+ *        v' = beta2*v + omb2*(g*g);  d = sqrt(v')/sbc2 + eps;  p' = p1 - ss*(m'/d)
+ *      with decay = 1 - lr*wd, omb1 = 1 - beta1, omb2 = 1 - beta2, ss = lr/(1 - beta1^step),
+ *      sbc2 = sqrt(1 - beta2^step) computed on the host in double and rounded once to fp32.
+ *      It writes p', m', v' to the live arrays, RNE_bf16(p') to d_p_bf16, and the same p', m',
+ *      v' bits plus the header into staging slot `step mod depth` ("packed into a contiguous
+ *      buffer") — the snapshot costs no extra read pass and no extra kernel.
+ * `step` is the 1-based index of the update and must equal last_step + 1.
+ * Traffic: reads 14 B/element, writes 26 B/element (14 with snapshots disabled). */
+PHX_API int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads_bf16, float lr, float beta1,
+                                  float beta2, float eps, float wd, uint64_t step, void *stream);
+
+/* ---- a4+a5: asynchronous chunked flush of the newest staged snapshot ------------------------
+ * Enqueues on `side_stream` (a copy-engine stream, "dedicated CUDA stream"):
+ * wait for the step's kernel; invalidate the host slot's header; copy the payload in
+ * chunk_bytes pieces; copy the header last (= commit: seq_end lands last).  The other host
+ * slot keeps the previous committed snapshot throughout. */
+PHX_API int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream);
+/* Host-blocking wait until the snapshot of `step` is committed (tests, shutdown). */
+PHX_API int phx_snapshot_wait(phx_shard_t *s, uint64_t step);
+/* Non-blocking: newest snapshot known committed (by completed flush events); *slot = host slot
+ * index, or PHX_ERR_NO_COMMITTED_SNAPSHOT. */
+PHX_API int phx_snapshot_query(phx_shard_t *s, uint64_t *newest_committed_step, int *slot);
+/* Fault injection for tests: the NEXT flush copies only `payload_chunks` payload
+ * chunks and never commits; the slot stays torn.  payload_chunks < 0 clears the hook. */
+PHX_API int phx_fault_inject_torn_flush(phx_shard_t *s, int64_t payload_chunks);
+
+/* ---- a6: restore ---------------------------------------------------------------------------
+ * Waits (host side) for in-flight flushes, then chooses between the two host slots the valid
+ * one (magic, version, header hash, seq_begin == seq_end) with the largest step, refuses it if
+ * its logical identity (layout hash, dp/tp/pp coordinates, n) differs from this shard's, and
+ * enqueues on `stream` the rebuild of the live shard: p, m, v from the slot and d_p_bf16 =
+ * RNE_bf16(p).  PHX_RESTORE_BULK_KERNEL: one kernel pulls the replica straight from mapped host
+ * memory with 1-D bulk async (TMA) loads into shared memory and writes all four arrays;
+ * PHX_RESTORE_COPY_ENGINE: three H2D copies plus a bf16 regeneration kernel.  Depends on
+ * nothing in device memory.  Afterwards last_step = header.step, so the caller re-issues step
+ * last_step + 1 with the same gradients (recompute of the in-flight step).
+ * A fresh handle created with the same layout/coordinates and bound to the same replica can
+ * restore too (a replacement rank assuming the failed rank's role). */
+PHX_API int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step);
+/* Copies the user blob of the slot the last phx_restore used. */
+PHX_API int phx_restored_user_metadata(const phx_shard_t *s, void *blob, uint32_t cap, uint32_t *len);
+
+/* ---- introspection ---------------------------------------------------------------------- */
+PHX_API int phx_last_step(const phx_shard_t *s, uint64_t *step);
+/* Host-blocking: clip coefficient and sum of squares of the last step (1.0 / 0 if clip is off). */
+PHX_API int phx_last_clip(phx_shard_t *s, float *coef, double *sumsq);
+/* Number of kernels the library has launched on this handle (bench.py's gpu_launches). */
+PHX_API int phx_kernel_launches(const phx_shard_t *s, uint64_t *count);
+/* Selects a kernel variant of the fused step (0 = default); for tuning/benchmarks only. */
+PHX_API int phx_set_kernel_variant(phx_shard_t *s, uint32_t variant);
+PHX_API const char *phx_strerror(int err);
+PHX_API int phx_last_cuda_error(const phx_shard_t *s);
+PHX_API uint32_t phx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PHX_H */

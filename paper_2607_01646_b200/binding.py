@@ -1,0 +1,249 @@
+"""Thin ctypes binding of libphx.so — same names as include/phx.h, argument marshalling only.
+
+Every step of the hot path runs inside the library's kernels / copy engines; nothing here
+computes.  There is no CPU fallback: if libphx.so is missing this module raises on first use
+(build it with `python -m paper_2607_01646_b200.build`), and every compute entry point needs a
+compute-capability-10.x GPU (PHX_ERR_UNSUPPORTED_DEVICE otherwise).
+
+PyTorch is used by callers for device memory and streams only; pointers cross this boundary as
+plain integers (`tensor.data_ptr()`, `stream.cuda_stream`).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import List, Optional, Sequence, Tuple
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libphx.so")
+
+PHX_OK = 0
+PHX_ERR_INVALID_ARG = -1
+PHX_ERR_ALIGNMENT = -2
+PHX_ERR_NOT_BOUND = -3
+PHX_ERR_STEP_ORDER = -4
+PHX_ERR_NO_FLUSH_PENDING = -5
+PHX_ERR_NO_COMMITTED_SNAPSHOT = -6
+PHX_ERR_LAYOUT_MISMATCH = -7
+PHX_ERR_CORRUPT_SLOT = -8
+PHX_ERR_CUDA = -9
+PHX_ERR_UNSUPPORTED_DEVICE = -10
+PHX_ERR_SNAPSHOT_DISABLED = -11
+PHX_ERR_NOMEM = -12
+
+PHX_SYNC_STRICT, PHX_SYNC_RELAXED = 0, 1
+PHX_RESTORE_BULK_KERNEL, PHX_RESTORE_COPY_ENGINE = 0, 1
+
+
+class phx_tensor_desc_t(C.Structure):
+    _fields_ = [("numel", C.c_uint64), ("tensor_id", C.c_uint32), ("flags", C.c_uint32)]
+
+
+class phx_config_t(C.Structure):
+    _fields_ = [("tp_size", C.c_uint32), ("tp_rank", C.c_uint32), ("pp_size", C.c_uint32),
+                ("pp_rank", C.c_uint32), ("staging_depth", C.c_uint32), ("sync_mode", C.c_uint32),
+                ("chunk_bytes", C.c_uint64), ("snapshot_disabled", C.c_uint32),
+                ("restore_mode", C.c_uint32), ("max_grad_norm", C.c_float),
+                ("reserved", C.c_uint32 * 5)]
+
+
+class phx_shard_info_t(C.Structure):
+    _fields_ = [("n", C.c_uint64), ("n_padded", C.c_uint64), ("total_numel", C.c_uint64),
+                ("shard_begin", C.c_uint64), ("layout_hash", C.c_uint64),
+                ("snapshot_bytes", C.c_uint64), ("slot_stride", C.c_uint64),
+                ("n_segments", C.c_uint32), ("staging_depth", C.c_uint32),
+                ("dp_size", C.c_uint32), ("dp_rank", C.c_uint32)]
+
+
+class PhxError(RuntimeError):
+    def __init__(self, code: int, where: str, cuda: int = 0):
+        self.code, self.cuda = code, cuda
+        msg = lib().phx_strerror(code).decode()
+        super().__init__(f"{where}: {msg} ({code})" + (f", cudaError {cuda}" if cuda else ""))
+
+
+_lib = None
+
+# name -> (restype, argtypes); the CPU test tier checks that libphx.so exports every one of them
+PROTOTYPES = {
+    "phx_version": (C.c_uint32, []),
+    "phx_strerror": (C.c_char_p, [C.c_int]),
+    "phx_last_cuda_error": (C.c_int, [C.c_void_p]),
+    "phx_shard_create": (C.c_int, [C.POINTER(phx_tensor_desc_t), C.c_size_t, C.c_uint32, C.c_uint32,
+                                   C.POINTER(phx_config_t), C.POINTER(C.c_void_p)]),
+    "phx_shard_destroy": (C.c_int, [C.c_void_p]),
+    "phx_shard_info": (C.c_int, [C.c_void_p, C.POINTER(phx_shard_info_t)]),
+    "phx_shard_segments": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint32), C.POINTER(C.c_uint64),
+                                     C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.c_uint32]),
+    "phx_shard_bind": (C.c_int, [C.c_void_p] * 7),
+    "phx_shard_set_state": (C.c_int, [C.c_void_p, C.c_uint64, C.c_void_p]),
+    "phx_set_user_metadata": (C.c_int, [C.c_void_p, C.c_char_p, C.c_uint32]),
+    "phx_step_and_snapshot": (C.c_int, [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float,
+                                        C.c_float, C.c_float, C.c_uint64, C.c_void_p]),
+    "phx_snapshot_flush_async": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "phx_snapshot_wait": (C.c_int, [C.c_void_p, C.c_uint64]),
+    "phx_snapshot_query": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64), C.POINTER(C.c_int)]),
+    "phx_fault_inject_torn_flush": (C.c_int, [C.c_void_p, C.c_int64]),
+    "phx_restore": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(C.c_uint64)]),
+    "phx_restored_user_metadata": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(C.c_uint32)]),
+    "phx_last_step": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
+    "phx_last_clip": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)]),
+    "phx_kernel_launches": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
+    "phx_set_kernel_variant": (C.c_int, [C.c_void_p, C.c_uint32]),
+}
+
+
+def lib() -> C.CDLL:
+    """Load libphx.so (fails loudly if it has not been built)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_2607_01646_b200.build` "
+                "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in PROTOTYPES.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _ck(rc: int, where: str, handle=None):
+    if rc != PHX_OK:
+        cuda = lib().phx_last_cuda_error(handle) if (handle and rc == PHX_ERR_CUDA) else 0
+        raise PhxError(rc, where, cuda)
+
+
+def _ptr(x) -> int:
+    """tensor -> data_ptr(), stream -> cuda_stream, int/None pass through."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "cuda_stream"):
+        return x.cuda_stream
+    raise TypeError(type(x))
+
+
+# ---- the calls of include/phx.h, same names -------------------------------------------------
+
+
+def phx_shard_create(layout: Sequence[Tuple[int, int]], dp_size: int, dp_rank: int, *, tp=(1, 0),
+                     pp=(1, 0), staging_depth=0, sync_mode=PHX_SYNC_STRICT, chunk_bytes=0,
+                     snapshot_disabled=False, restore_mode=PHX_RESTORE_BULK_KERNEL,
+                     max_grad_norm=0.0, flags: Optional[Sequence[int]] = None) -> int:
+    """layout = [(numel, tensor_id)] in flattening order.  Returns the opaque handle."""
+    n = len(layout)
+    arr = (phx_tensor_desc_t * max(n, 1))()
+    for i, (numel, tid) in enumerate(layout):
+        arr[i].numel, arr[i].tensor_id = int(numel), int(tid)
+        arr[i].flags = int(flags[i]) if flags is not None else 0
+    cfg = phx_config_t(tp_size=tp[0], tp_rank=tp[1], pp_size=pp[0], pp_rank=pp[1],
+                       staging_depth=staging_depth, sync_mode=sync_mode, chunk_bytes=chunk_bytes,
+                       snapshot_disabled=1 if snapshot_disabled else 0, restore_mode=restore_mode,
+                       max_grad_norm=max_grad_norm)
+    h = C.c_void_p()
+    _ck(lib().phx_shard_create(arr, n, dp_size, dp_rank, C.byref(cfg), C.byref(h)), "phx_shard_create")
+    return h.value
+
+
+def phx_shard_destroy(h: int) -> None:
+    _ck(lib().phx_shard_destroy(h), "phx_shard_destroy")
+
+
+def phx_shard_info(h: int) -> phx_shard_info_t:
+    info = phx_shard_info_t()
+    _ck(lib().phx_shard_info(h, C.byref(info)), "phx_shard_info")
+    return info
+
+
+def phx_shard_segments(h: int) -> List[Tuple[int, int, int, int]]:
+    """[(tensor_id, off_in_tensor, off_in_shard, len)]"""
+    k = phx_shard_info(h).n_segments
+    tid = (C.c_uint32 * max(k, 1))()
+    a, b, c = ((C.c_uint64 * max(k, 1))() for _ in range(3))
+    _ck(lib().phx_shard_segments(h, tid, a, b, c, k), "phx_shard_segments")
+    return [(tid[i], a[i], b[i], c[i]) for i in range(k)]
+
+
+def phx_shard_bind(h: int, d_p, d_m, d_v, d_p_bf16, d_staging, h_replica) -> None:
+    _ck(lib().phx_shard_bind(h, _ptr(d_p), _ptr(d_m), _ptr(d_v), _ptr(d_p_bf16), _ptr(d_staging),
+                             _ptr(h_replica)), "phx_shard_bind", h)
+
+
+def phx_shard_set_state(h: int, step: int, stream=None) -> None:
+    _ck(lib().phx_shard_set_state(h, step, _ptr(stream)), "phx_shard_set_state", h)
+
+
+def phx_set_user_metadata(h: int, blob: bytes) -> None:
+    _ck(lib().phx_set_user_metadata(h, blob, len(blob)), "phx_set_user_metadata", h)
+
+
+def phx_step_and_snapshot(h: int, d_grads_bf16, lr: float, beta1: float, beta2: float, eps: float,
+                          wd: float, step: int, stream=None) -> None:
+    _ck(lib().phx_step_and_snapshot(h, _ptr(d_grads_bf16), lr, beta1, beta2, eps, wd, step,
+                                    _ptr(stream)), "phx_step_and_snapshot", h)
+
+
+def phx_snapshot_flush_async(h: int, side_stream=None) -> None:
+    _ck(lib().phx_snapshot_flush_async(h, _ptr(side_stream)), "phx_snapshot_flush_async", h)
+
+
+def phx_snapshot_wait(h: int, step: int) -> None:
+    _ck(lib().phx_snapshot_wait(h, step), "phx_snapshot_wait", h)
+
+
+def phx_snapshot_query(h: int) -> Optional[Tuple[int, int]]:
+    """(newest committed step, host slot) or None."""
+    st, slot = C.c_uint64(), C.c_int()
+    rc = lib().phx_snapshot_query(h, C.byref(st), C.byref(slot))
+    if rc == PHX_ERR_NO_COMMITTED_SNAPSHOT:
+        return None
+    _ck(rc, "phx_snapshot_query", h)
+    return st.value, slot.value
+
+
+def phx_fault_inject_torn_flush(h: int, payload_chunks: int) -> None:
+    _ck(lib().phx_fault_inject_torn_flush(h, payload_chunks), "phx_fault_inject_torn_flush", h)
+
+
+def phx_restore(h: int, stream=None) -> int:
+    st = C.c_uint64()
+    _ck(lib().phx_restore(h, _ptr(stream), C.byref(st)), "phx_restore", h)
+    return st.value
+
+
+def phx_restored_user_metadata(h: int) -> bytes:
+    buf = C.create_string_buffer(128)
+    n = C.c_uint32()
+    _ck(lib().phx_restored_user_metadata(h, buf, 128, C.byref(n)), "phx_restored_user_metadata", h)
+    return buf.raw[:n.value]
+
+
+def phx_last_step(h: int) -> int:
+    st = C.c_uint64()
+    _ck(lib().phx_last_step(h, C.byref(st)), "phx_last_step", h)
+    return st.value
+
+
+def phx_last_clip(h: int) -> Tuple[float, float]:
+    c, q = C.c_float(), C.c_double()
+    _ck(lib().phx_last_clip(h, C.byref(c), C.byref(q)), "phx_last_clip", h)
+    return c.value, q.value
+
+
+def phx_kernel_launches(h: int) -> int:
+    n = C.c_uint64()
+    _ck(lib().phx_kernel_launches(h, C.byref(n)), "phx_kernel_launches", h)
+    return n.value
+
+
+def phx_set_kernel_variant(h: int, variant: int) -> None:
+    _ck(lib().phx_set_kernel_variant(h, variant), "phx_set_kernel_variant", h)
+
+
+def phx_version() -> int:
+    return lib().phx_version()

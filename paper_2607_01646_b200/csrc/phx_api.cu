@@ -1,0 +1,622 @@
+// phx_api.cu — the C-ABI boundary (include/phx.h): shard definition, envelope, staging ring,
+// chunked D2H flush with ping-pong host slots and DMA-ordered commit, restore.  Host logic only;
+// every byte of the hot path is moved by the kernels in phx_kernels.cu or by the copy engines.
+#include "../../include/phx.h"
+#include "phx_kernels.cuh"
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace {
+
+constexpr uint64_t kPadUnit = 64;      // elements; every rank's range is a multiple of 64
+constexpr uint64_t kHeaderBytes = 256;
+constexpr uint32_t kVersion = 1;
+constexpr int kMaxDepth = 4;
+
+struct Segment {
+    uint32_t tensor_id;
+    uint64_t off_in_tensor, off_in_shard, len;
+};
+
+enum SlotState { SLOT_EMPTY = 0, SLOT_INFLIGHT, SLOT_COMMITTED, SLOT_TORN_INFLIGHT, SLOT_TORN };
+
+struct HostSlot {
+    uint64_t step = 0;
+    SlotState state = SLOT_EMPTY;
+};
+
+// device scratch layout (bytes)
+constexpr size_t kScrZeroHdr = 0;      // 256 zero bytes: invalidates a host slot header
+constexpr size_t kScrOne = 256;        // float 1.0f: clip coefficient when clipping is off
+constexpr size_t kScrCoef = 260;       // float: clip coefficient of the current step
+constexpr size_t kScrSumsq = 264;      // double
+constexpr size_t kScrPartials = 512;   // kSumsqMaxBlocks doubles
+constexpr size_t kScrBytes = kScrPartials + phx::kSumsqMaxBlocks * sizeof(double);
+
+uint64_t fnv1a64(const void *data, size_t len, uint64_t h = 0xCBF29CE484222325ull)
+{
+    const uint8_t *b = static_cast<const uint8_t *>(data);
+    for (size_t i = 0; i < len; ++i) {
+        h ^= b[i];
+        h *= 0x100000001B3ull;
+    }
+    return h;
+}
+
+double pow_sqmul(double b, uint64_t t)  // LSB-first square-and-multiply, no libm pow
+{
+    double r = 1.0;
+    while (t) {
+        if (t & 1) r = r * b;
+        b = b * b;
+        t >>= 1;
+    }
+    return r;
+}
+
+inline bool aligned256(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 255u) == 0; }
+
+}  // namespace
+
+struct phx_shard {
+    std::vector<phx_tensor_desc_t> layout;
+    std::vector<Segment> segments;
+    phx_config_t cfg{};
+    phx_shard_info_t info{};
+    // bound memory
+    bool bound = false;
+    float *d_p = nullptr, *d_m = nullptr, *d_v = nullptr;
+    void *d_p16 = nullptr;
+    uint8_t *d_staging = nullptr;
+    uint8_t *h_replica = nullptr;
+    uint8_t *d_replica = nullptr;  // device view of h_replica
+    uint8_t *d_scratch = nullptr;
+    int sm_count = 148;
+    // state
+    uint64_t last_step = 0;
+    uint8_t user[128] = {0};
+    uint32_t user_len = 0;
+    uint8_t restored_user[128] = {0};
+    uint32_t restored_user_len = 0;
+    // staging ring / flush bookkeeping
+    cudaEvent_t ev_step[kMaxDepth] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev_flush[kMaxDepth] = {nullptr, nullptr, nullptr, nullptr};
+    bool flush_valid[kMaxDepth] = {false, false, false, false};
+    cudaEvent_t ev_host[2] = {nullptr, nullptr};
+    HostSlot host[2];
+    int last_flush_slot = -1;  // staging slot whose ev_flush is the newest flush event
+    int pending_slot = -1;     // staging slot holding a snapshot that has not been flushed
+    uint64_t pending_step = 0;
+    int64_t torn_chunks = -1;
+    // misc
+    int last_cuda_error = 0;
+    uint64_t launches = 0;
+    uint32_t variant = 0;
+    bool clip_valid = false;
+};
+
+#define PHX_CK(call)                                  \
+    do {                                              \
+        cudaError_t e__ = (call);                     \
+        if (e__ != cudaSuccess) {                     \
+            s->last_cuda_error = (int)e__;            \
+            return PHX_ERR_CUDA;                      \
+        }                                             \
+    } while (0)
+
+namespace {
+
+void build_header(const phx_shard *s, uint64_t step, bool committed, phx_snapshot_header_t *h)
+{
+    static_assert(sizeof(phx_snapshot_header_t) == 256, "envelope must be 256 bytes");
+    std::memset(h, 0, sizeof(*h));
+    std::memcpy(h->magic, "PHXSNAP1", 8);
+    h->version = kVersion;
+    h->header_bytes = (uint32_t)kHeaderBytes;
+    h->seq_begin = step;
+    h->step = step;
+    h->n = s->info.n;
+    h->n_padded = s->info.n_padded;
+    h->total_numel = s->info.total_numel;
+    h->shard_begin = s->info.shard_begin;
+    h->layout_hash = s->info.layout_hash;
+    h->dp_size = s->info.dp_size;
+    h->dp_rank = s->info.dp_rank;
+    h->tp_size = s->cfg.tp_size;
+    h->tp_rank = s->cfg.tp_rank;
+    h->pp_size = s->cfg.pp_size;
+    h->pp_rank = s->cfg.pp_rank;
+    h->chunk_bytes = s->cfg.chunk_bytes;
+    h->user_len = s->user_len;
+    std::memcpy(h->user, s->user, s->user_len);
+    h->header_hash = fnv1a64(h, 240);
+    h->seq_end = committed ? step : 0;
+}
+
+// commit rule: magic/version/size right, header hash matches, seq_begin == seq_end
+bool header_valid(const phx_snapshot_header_t *h)
+{
+    if (std::memcmp(h->magic, "PHXSNAP1", 8) != 0) return false;
+    if (h->version != kVersion || h->header_bytes != kHeaderBytes) return false;
+    if (h->header_hash != fnv1a64(h, 240)) return false;
+    return h->seq_begin == h->seq_end && h->seq_begin == h->step;
+}
+
+bool header_matches(const phx_shard *s, const phx_snapshot_header_t *h)
+{
+    return h->layout_hash == s->info.layout_hash && h->n == s->info.n && h->n_padded == s->info.n_padded &&
+           h->total_numel == s->info.total_numel && h->shard_begin == s->info.shard_begin &&
+           h->dp_size == s->info.dp_size && h->dp_rank == s->info.dp_rank && h->tp_size == s->cfg.tp_size &&
+           h->tp_rank == s->cfg.tp_rank && h->pp_size == s->cfg.pp_size && h->pp_rank == s->cfg.pp_rank;
+}
+
+bool snapshots_on(const phx_shard *s) { return s->cfg.snapshot_disabled == 0; }
+
+// settle the bookkeeping of host slots whose flush event has completed (block=true waits for it)
+int settle_host_slots(phx_shard *s, bool block)
+{
+    for (int i = 0; i < 2; ++i) {
+        HostSlot &h = s->host[i];
+        if (h.state != SLOT_INFLIGHT && h.state != SLOT_TORN_INFLIGHT) continue;
+        cudaError_t e = block ? cudaEventSynchronize(s->ev_host[i]) : cudaEventQuery(s->ev_host[i]);
+        if (e == cudaErrorNotReady) continue;
+        if (e != cudaSuccess) {
+            s->last_cuda_error = (int)e;
+            return PHX_ERR_CUDA;
+        }
+        h.state = h.state == SLOT_INFLIGHT ? SLOT_COMMITTED : SLOT_TORN;
+    }
+    return PHX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+uint32_t phx_version(void) { return 0x00010000u; }
+
+const char *phx_strerror(int err)
+{
+    switch (err) {
+    case PHX_OK: return "ok";
+    case PHX_ERR_INVALID_ARG: return "invalid argument";
+    case PHX_ERR_ALIGNMENT: return "pointer not 256-byte aligned";
+    case PHX_ERR_NOT_BOUND: return "shard memory not bound";
+    case PHX_ERR_STEP_ORDER: return "step is not last_step + 1";
+    case PHX_ERR_NO_FLUSH_PENDING: return "no un-flushed snapshot";
+    case PHX_ERR_NO_COMMITTED_SNAPSHOT: return "no committed snapshot in the replica";
+    case PHX_ERR_LAYOUT_MISMATCH: return "replica belongs to a different logical shard";
+    case PHX_ERR_CORRUPT_SLOT: return "replica slot is torn or corrupt";
+    case PHX_ERR_CUDA: return "CUDA error (see phx_last_cuda_error)";
+    case PHX_ERR_UNSUPPORTED_DEVICE: return "device is not compute capability 10.x";
+    case PHX_ERR_SNAPSHOT_DISABLED: return "snapshots are disabled on this shard";
+    case PHX_ERR_NOMEM: return "out of memory";
+    default: return "unknown error";
+    }
+}
+
+int phx_last_cuda_error(const phx_shard_t *s) { return s ? s->last_cuda_error : 0; }
+
+// ---- a0 -------------------------------------------------------------------------------------
+int phx_shard_create(const phx_tensor_desc_t *layout, size_t n_tensors, uint32_t dp_size, uint32_t dp_rank,
+                     const phx_config_t *cfg, phx_shard_t **out)
+{
+    if (!out) return PHX_ERR_INVALID_ARG;
+    *out = nullptr;
+    if ((!layout && n_tensors) || dp_size == 0 || dp_rank >= dp_size) return PHX_ERR_INVALID_ARG;
+    phx_shard *s = new (std::nothrow) phx_shard();
+    if (!s) return PHX_ERR_NOMEM;
+    if (cfg) s->cfg = *cfg;
+    phx_config_t &c = s->cfg;
+    if (c.tp_size == 0) c.tp_size = 1;
+    if (c.pp_size == 0) c.pp_size = 1;
+    if (c.staging_depth == 0) c.staging_depth = 2;
+    if (c.chunk_bytes == 0) c.chunk_bytes = 64ull << 20;
+    c.chunk_bytes = (c.chunk_bytes + 255) & ~255ull;
+    if (c.tp_rank >= c.tp_size || c.pp_rank >= c.pp_size || c.staging_depth > kMaxDepth ||
+        c.sync_mode > PHX_SYNC_RELAXED || c.restore_mode > PHX_RESTORE_COPY_ENGINE || !(c.max_grad_norm == c.max_grad_norm)) {
+        delete s;
+        return PHX_ERR_INVALID_ARG;
+    }
+    s->layout.assign(layout, layout + n_tensors);
+
+    uint64_t total = 0;
+    for (const auto &t : s->layout) total += t.numel;
+    const uint64_t unit = kPadUnit * dp_size;
+    const uint64_t L = ((total + unit - 1) / unit) * kPadUnit;
+    const uint64_t begin = (uint64_t)dp_rank * L, end = begin + L;
+    uint64_t n = total > begin ? total - begin : 0;
+    if (n > L) n = L;
+
+    uint64_t t0 = 0;
+    for (const auto &t : s->layout) {
+        const uint64_t t1 = t0 + t.numel;
+        const uint64_t lo = t0 > begin ? t0 : begin, hi = t1 < end ? t1 : end;
+        if (hi > lo) s->segments.push_back(Segment{t.tensor_id, lo - t0, lo - begin, hi - lo});
+        t0 = t1;
+    }
+    // layout hash: per tensor (numel u64, tensor_id u32, flags u32), then dp_size, tp_size, tp_rank, pp_size, pp_rank
+    uint64_t h = 0xCBF29CE484222325ull;
+    for (const auto &t : s->layout) {
+        uint8_t rec[16];
+        std::memcpy(rec, &t.numel, 8);
+        std::memcpy(rec + 8, &t.tensor_id, 4);
+        std::memcpy(rec + 12, &t.flags, 4);
+        h = fnv1a64(rec, 16, h);
+    }
+    const uint32_t coords[5] = {dp_size, c.tp_size, c.tp_rank, c.pp_size, c.pp_rank};
+    h = fnv1a64(coords, sizeof(coords), h);
+
+    phx_shard_info_t &i = s->info;
+    i.n = n;
+    i.n_padded = L;
+    i.total_numel = total;
+    i.shard_begin = begin;
+    i.layout_hash = h;
+    i.snapshot_bytes = kHeaderBytes + 12 * L;
+    i.slot_stride = (i.snapshot_bytes + 255) & ~255ull;
+    i.n_segments = (uint32_t)s->segments.size();
+    i.staging_depth = c.staging_depth;
+    i.dp_size = dp_size;
+    i.dp_rank = dp_rank;
+    *out = s;
+    return PHX_OK;
+}
+
+int phx_shard_destroy(phx_shard_t *s)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (s->bound) {
+        settle_host_slots(s, true);
+        for (int k = 0; k < kMaxDepth; ++k) {
+            if (s->ev_step[k]) cudaEventSynchronize(s->ev_step[k]), cudaEventDestroy(s->ev_step[k]);
+            if (s->ev_flush[k]) cudaEventSynchronize(s->ev_flush[k]), cudaEventDestroy(s->ev_flush[k]);
+        }
+        for (int k = 0; k < 2; ++k)
+            if (s->ev_host[k]) cudaEventDestroy(s->ev_host[k]);
+        if (s->d_scratch) cudaFree(s->d_scratch);
+    }
+    delete s;
+    return PHX_OK;
+}
+
+int phx_shard_info(const phx_shard_t *s, phx_shard_info_t *out)
+{
+    if (!s || !out) return PHX_ERR_INVALID_ARG;
+    *out = s->info;
+    return PHX_OK;
+}
+
+int phx_shard_segments(const phx_shard_t *s, uint32_t *tensor_id, uint64_t *off_in_tensor, uint64_t *off_in_shard,
+                       uint64_t *len, uint32_t cap)
+{
+    if (!s || (cap && (!tensor_id || !off_in_tensor || !off_in_shard || !len))) return PHX_ERR_INVALID_ARG;
+    for (uint32_t k = 0; k < cap && k < s->segments.size(); ++k) {
+        tensor_id[k] = s->segments[k].tensor_id;
+        off_in_tensor[k] = s->segments[k].off_in_tensor;
+        off_in_shard[k] = s->segments[k].off_in_shard;
+        len[k] = s->segments[k].len;
+    }
+    return PHX_OK;
+}
+
+// ---- binding ----------------------------------------------------------------------------------
+int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p_bf16, void *d_staging,
+                   void *h_replica)
+{
+    if (!s || !d_p || !d_m || !d_v || !d_p_bf16) return PHX_ERR_INVALID_ARG;
+    if (snapshots_on(s) && (!d_staging || !h_replica)) return PHX_ERR_INVALID_ARG;
+    if (!aligned256(d_p) || !aligned256(d_m) || !aligned256(d_v) || !aligned256(d_p_bf16) || !aligned256(d_staging) ||
+        !aligned256(h_replica))
+        return PHX_ERR_ALIGNMENT;
+    if (s->bound) return PHX_ERR_INVALID_ARG;
+
+    int dev = 0, major = 0;
+    PHX_CK(cudaGetDevice(&dev));
+    PHX_CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return PHX_ERR_UNSUPPORTED_DEVICE;  // sm_100a only; deliberately no fallback
+    PHX_CK(cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, dev));
+
+    if (snapshots_on(s)) {
+        void *dview = nullptr;
+        cudaError_t e = cudaHostGetDevicePointer(&dview, h_replica, 0);
+        if (e != cudaSuccess) {  // not pinned/mapped host memory
+            s->last_cuda_error = (int)e;
+            (void)cudaGetLastError();
+            return PHX_ERR_INVALID_ARG;
+        }
+        s->d_replica = static_cast<uint8_t *>(dview);
+    }
+    PHX_CK(cudaMalloc(reinterpret_cast<void **>(&s->d_scratch), kScrBytes));
+    PHX_CK(cudaMemset(s->d_scratch, 0, kScrBytes));
+    const float one = 1.0f;
+    PHX_CK(cudaMemcpy(s->d_scratch + kScrOne, &one, 4, cudaMemcpyHostToDevice));
+    PHX_CK(cudaMemcpy(s->d_scratch + kScrCoef, &one, 4, cudaMemcpyHostToDevice));
+    for (uint32_t k = 0; k < s->cfg.staging_depth; ++k) {
+        PHX_CK(cudaEventCreateWithFlags(&s->ev_step[k], cudaEventDisableTiming));
+        PHX_CK(cudaEventCreateWithFlags(&s->ev_flush[k], cudaEventDisableTiming));
+    }
+    for (int k = 0; k < 2; ++k) PHX_CK(cudaEventCreateWithFlags(&s->ev_host[k], cudaEventDisableTiming));
+
+    s->d_p = d_p;
+    s->d_m = d_m;
+    s->d_v = d_v;
+    s->d_p16 = d_p_bf16;
+    s->d_staging = static_cast<uint8_t *>(d_staging);
+    s->h_replica = static_cast<uint8_t *>(h_replica);
+    s->bound = true;
+    return PHX_OK;
+}
+
+int phx_shard_set_state(phx_shard_t *s, uint64_t step, void *stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    PHX_CK(phx::launch_regen_bf16(s->d_p, s->d_p16, s->info.n_padded, static_cast<cudaStream_t>(stream)));
+    s->launches += s->info.n_padded ? 1 : 0;
+    s->last_step = step;
+    s->pending_slot = -1;
+    return PHX_OK;
+}
+
+int phx_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len)
+{
+    if (!s || len > 128 || (len && !blob)) return PHX_ERR_INVALID_ARG;
+    std::memset(s->user, 0, sizeof(s->user));
+    if (len) std::memcpy(s->user, blob, len);
+    s->user_len = len;
+    return PHX_OK;
+}
+
+// ---- a1 + a2 + a3 --------------------------------------------------------------------------------
+int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads_bf16, float lr, float beta1, float beta2, float eps,
+                          float wd, uint64_t step, void *stream)
+{
+    if (!s || !d_grads_bf16) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!aligned256(d_grads_bf16)) return PHX_ERR_ALIGNMENT;
+    if (step != s->last_step + 1) return PHX_ERR_STEP_ORDER;  // I4 step atomicity
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const bool snap = snapshots_on(s);
+
+    phx::StepArgs a;
+    std::memset(&a, 0, sizeof(a));
+    // derived scalars: double on the host, rounded once to fp32 (include/phx.h a3)
+    const double dlr = lr, db1 = beta1, db2 = beta2, dwd = wd;
+    a.sc.beta1 = beta1;
+    a.sc.beta2 = beta2;
+    a.sc.eps = eps;
+    a.sc.decay = (float)(1.0 - dlr * dwd);
+    a.sc.omb1 = (float)(1.0 - db1);
+    a.sc.omb2 = (float)(1.0 - db2);
+    a.sc.ss = (float)(dlr / (1.0 - pow_sqmul(db1, step)));
+    a.sc.sbc2 = (float)std::sqrt(1.0 - pow_sqmul(db2, step));
+
+    // a1: optional clip by the shard-local gradient norm
+    a.coef = reinterpret_cast<const float *>(s->d_scratch + kScrOne);
+    s->clip_valid = false;
+    if (s->cfg.max_grad_norm > 0.0f) {
+        int nl = 0;
+        PHX_CK(phx::launch_sumsq_clip(d_grads_bf16, s->info.n_padded, s->cfg.max_grad_norm,
+                                      reinterpret_cast<double *>(s->d_scratch + kScrPartials),
+                                      reinterpret_cast<double *>(s->d_scratch + kScrSumsq),
+                                      reinterpret_cast<float *>(s->d_scratch + kScrCoef), st, &nl));
+        s->launches += nl;
+        a.coef = reinterpret_cast<const float *>(s->d_scratch + kScrCoef);
+        s->clip_valid = true;
+    }
+
+    int slot = -1;
+    if (snap) {
+        slot = (int)(step % s->cfg.staging_depth);
+        // a2: the single sync point — stream-side wait, the host never blocks
+        if (s->cfg.sync_mode == PHX_SYNC_STRICT) {
+            if (s->last_flush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[s->last_flush_slot], 0));
+        } else if (s->flush_valid[slot]) {
+            PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[slot], 0));
+        }
+        uint8_t *base = s->d_staging + (uint64_t)slot * s->info.slot_stride;
+        a.shdr = base;
+        a.sp = reinterpret_cast<float *>(base + kHeaderBytes);
+        a.sm = a.sp + s->info.n_padded;
+        a.sv = a.sm + s->info.n_padded;
+        phx_snapshot_header_t hdr;
+        build_header(s, step, true, &hdr);
+        std::memcpy(&a.hdr, &hdr, sizeof(hdr));
+    }
+    a.p = s->d_p;
+    a.m = s->d_m;
+    a.v = s->d_v;
+    a.g = d_grads_bf16;
+    a.p16 = s->d_p16;
+    a.n_padded = s->info.n_padded;
+
+    // a3: one kernel, one pass
+    PHX_CK(phx::launch_step(a, snap, s->variant, st));
+    s->launches += s->info.n_padded ? 1 : 0;
+    if (snap) {
+        PHX_CK(cudaEventRecord(s->ev_step[slot], st));
+        s->pending_slot = slot;
+        s->pending_step = step;
+    }
+    s->last_step = step;
+    return PHX_OK;
+}
+
+// ---- a4 + a5 -------------------------------------------------------------------------------------
+int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
+    if (s->pending_slot < 0) return PHX_ERR_NO_FLUSH_PENDING;
+    cudaStream_t st = static_cast<cudaStream_t>(side_stream);
+    const int slot = s->pending_slot;
+    const uint64_t step = s->pending_step;
+    const int hs = (int)(step & 1);  // ping-pong
+    const uint8_t *src = s->d_staging + (uint64_t)slot * s->info.slot_stride;
+    uint8_t *dst = s->h_replica + (uint64_t)hs * s->info.slot_stride;
+
+    PHX_CK(cudaStreamWaitEvent(st, s->ev_step[slot], 0));  // the step's kernel has written the slot
+    if (s->last_flush_slot >= 0)                            // flushes are serialised whatever stream they use
+        PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[s->last_flush_slot], 0));
+
+    const bool torn = s->torn_chunks >= 0;
+    s->host[hs].step = step;
+    s->host[hs].state = torn ? SLOT_TORN_INFLIGHT : SLOT_INFLIGHT;
+    // 1. invalidate the target slot's header; the OTHER slot keeps the previous committed snapshot
+    PHX_CK(cudaMemcpyAsync(dst, s->d_scratch + kScrZeroHdr, kHeaderBytes, cudaMemcpyDeviceToHost, st));
+    // 2. payload in chunk_bytes pieces ("chunked")
+    const uint64_t payload = s->info.snapshot_bytes - kHeaderBytes;
+    const uint64_t chunk = s->cfg.chunk_bytes;
+    uint64_t done_chunks = 0;
+    for (uint64_t off = 0; off < payload; off += chunk, ++done_chunks) {
+        if (torn && (int64_t)done_chunks >= s->torn_chunks) break;
+        const uint64_t len = payload - off < chunk ? payload - off : chunk;
+        PHX_CK(cudaMemcpyAsync(dst + kHeaderBytes + off, src + kHeaderBytes + off, len, cudaMemcpyDeviceToHost, st));
+    }
+    // 3. commit: the valid header (seq_end == seq_begin) lands last
+    if (!torn) PHX_CK(cudaMemcpyAsync(dst, src, kHeaderBytes, cudaMemcpyDeviceToHost, st));
+    PHX_CK(cudaEventRecord(s->ev_flush[slot], st));
+    PHX_CK(cudaEventRecord(s->ev_host[hs], st));
+    s->flush_valid[slot] = true;
+    s->last_flush_slot = slot;
+    s->pending_slot = -1;
+    s->torn_chunks = -1;
+    return PHX_OK;
+}
+
+int phx_snapshot_wait(phx_shard_t *s, uint64_t step)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    const int hs = (int)(step & 1);
+    if (s->host[hs].state == SLOT_EMPTY || s->host[hs].step != step) return PHX_ERR_NO_COMMITTED_SNAPSHOT;
+    int rc = settle_host_slots(s, true);
+    if (rc != PHX_OK) return rc;
+    return s->host[hs].state == SLOT_COMMITTED ? PHX_OK : PHX_ERR_CORRUPT_SLOT;
+}
+
+int phx_snapshot_query(phx_shard_t *s, uint64_t *newest_committed_step, int *slot)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    int rc = settle_host_slots(s, false);
+    if (rc != PHX_OK) return rc;
+    int best = -1;
+    for (int i = 0; i < 2; ++i)
+        if (s->host[i].state == SLOT_COMMITTED && (best < 0 || s->host[i].step > s->host[best].step)) best = i;
+    if (best < 0) return PHX_ERR_NO_COMMITTED_SNAPSHOT;
+    if (newest_committed_step) *newest_committed_step = s->host[best].step;
+    if (slot) *slot = best;
+    return PHX_OK;
+}
+
+int phx_fault_inject_torn_flush(phx_shard_t *s, int64_t payload_chunks)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    s->torn_chunks = payload_chunks < 0 ? -1 : payload_chunks;
+    return PHX_OK;
+}
+
+// ---- a6 ------------------------------------------------------------------------------------------
+int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // in-flight flushes must land (or be known torn) before the host reads the headers
+    int rc = settle_host_slots(s, true);
+    if (rc != PHX_OK) return rc;
+
+    // Selection depends only on what is IN the replica: a fresh handle can restore.
+    int best = -1;
+    bool any_valid = false;
+    phx_snapshot_header_t hdr[2];
+    for (int i = 0; i < 2; ++i) {
+        std::memcpy(&hdr[i], s->h_replica + (uint64_t)i * s->info.slot_stride, sizeof(hdr[i]));
+        if (!header_valid(&hdr[i])) continue;
+        any_valid = true;
+        if (!header_matches(s, &hdr[i])) continue;
+        if (best < 0 || hdr[i].step > hdr[best].step) best = i;
+    }
+    if (best < 0) return any_valid ? PHX_ERR_LAYOUT_MISMATCH : PHX_ERR_NO_COMMITTED_SNAPSHOT;
+
+    const uint64_t N = s->info.n_padded;
+    const uint64_t off = (uint64_t)best * s->info.slot_stride + kHeaderBytes;
+    if (s->cfg.restore_mode == PHX_RESTORE_BULK_KERNEL) {
+        PHX_CK(phx::launch_restore_bulk(s->d_replica + off, s->d_p, s->d_m, s->d_v, s->d_p16, N, s->sm_count, st));
+        s->launches += N ? 1 : 0;
+    } else {
+        const uint8_t *src = s->h_replica + off;
+        PHX_CK(cudaMemcpyAsync(s->d_p, src, 4 * N, cudaMemcpyHostToDevice, st));
+        PHX_CK(cudaMemcpyAsync(s->d_m, src + 4 * N, 4 * N, cudaMemcpyHostToDevice, st));
+        PHX_CK(cudaMemcpyAsync(s->d_v, src + 8 * N, 4 * N, cudaMemcpyHostToDevice, st));
+        PHX_CK(phx::launch_regen_bf16(s->d_p, s->d_p16, N, st));
+        s->launches += N ? 1 : 0;
+    }
+    s->last_step = hdr[best].step;
+    s->pending_slot = -1;
+    s->restored_user_len = hdr[best].user_len <= 128 ? hdr[best].user_len : 128;
+    std::memcpy(s->restored_user, hdr[best].user, 128);
+    for (int i = 0; i < 2; ++i) {
+        const bool ok = header_valid(&hdr[i]) && header_matches(s, &hdr[i]);
+        s->host[i].state = ok ? SLOT_COMMITTED : (s->host[i].state == SLOT_EMPTY ? SLOT_EMPTY : SLOT_TORN);
+        if (ok) s->host[i].step = hdr[i].step;
+    }
+    if (restored_step) *restored_step = s->last_step;
+    return PHX_OK;
+}
+
+int phx_restored_user_metadata(const phx_shard_t *s, void *blob, uint32_t cap, uint32_t *len)
+{
+    if (!s || (cap && !blob)) return PHX_ERR_INVALID_ARG;
+    const uint32_t k = s->restored_user_len < cap ? s->restored_user_len : cap;
+    if (k) std::memcpy(blob, s->restored_user, k);
+    if (len) *len = s->restored_user_len;
+    return PHX_OK;
+}
+
+// ---- introspection -----------------------------------------------------------------------------
+int phx_last_step(const phx_shard_t *s, uint64_t *step)
+{
+    if (!s || !step) return PHX_ERR_INVALID_ARG;
+    *step = s->last_step;
+    return PHX_OK;
+}
+
+int phx_last_clip(phx_shard_t *s, float *coef, double *sumsq)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    float c = 1.0f;
+    double q = 0.0;
+    if (s->clip_valid) {
+        PHX_CK(cudaDeviceSynchronize());
+        PHX_CK(cudaMemcpy(&c, s->d_scratch + kScrCoef, 4, cudaMemcpyDeviceToHost));
+        PHX_CK(cudaMemcpy(&q, s->d_scratch + kScrSumsq, 8, cudaMemcpyDeviceToHost));
+    }
+    if (coef) *coef = c;
+    if (sumsq) *sumsq = q;
+    return PHX_OK;
+}
+
+int phx_kernel_launches(const phx_shard_t *s, uint64_t *count)
+{
+    if (!s || !count) return PHX_ERR_INVALID_ARG;
+    *count = s->launches;
+    return PHX_OK;
+}
+
+int phx_set_kernel_variant(phx_shard_t *s, uint32_t variant)
+{
+    if (!s || variant >= phx::kNumStepVariants) return PHX_ERR_INVALID_ARG;
+    s->variant = variant;
+    return PHX_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,547 @@
+// phx_kernels.cu — hand-written sm_100a kernels of the phx hot path.
+//
+//   k_step8 / k_step4 : a3, fused AdamW step + bf16 copy + packed snapshot (include/phx.h).
+//                       Pure HBM streaming: 14 B/element read, 26 B/element written, one pass,
+//                       256-bit (LDG.E.256 / STG.E.256, new on sm_100) or 128-bit vectors,
+//                       streaming cache hints, no shared memory, no tensor cores (no contraction).
+//   k_sumsq_*         : a1, deterministic fp64 sum of squares + clip coefficient.
+//   k_regen_bf16      : p16 = RNE_bf16(p).
+//   k_restore_bulk    : a6, pulls the replica from mapped pinned host memory with 1-D bulk
+//                       async copies (TMA, cp.async.bulk + mbarrier) into shared memory, writes
+//                       p, m, v back with bulk stores and regenerates the bf16 copy.
+//
+// Arithmetic contract (include/phx.h a3): every fp32 operation individually rounded —
+// __fmul_rn/__fadd_rn/__fsub_rn never fuse into FMA, __fdiv_rn/__fsqrt_rn are IEEE — and the
+// file must be compiled WITHOUT --use_fast_math and with the default -ftz=false.
+#include "phx_kernels.cuh"
+
+#include <cuda_bf16.h>
+
+namespace phx {
+
+// ------------------------------------------------------------------------------------------
+// vector memory helpers.  HINT: 0 plain, 1 L1::no_allocate (+L2::evict_first on loads),
+// 2 .cs (cache-streaming) both ways, 3 like 1 with L2::evict_first on stores as well.
+// p/m/v are read then overwritten by the same thread, so the non-coherent (.nc) path is used
+// only for the gradients.
+// ------------------------------------------------------------------------------------------
+struct F8 {
+    float x[8];
+};
+struct F4 {
+    float x[4];
+};
+
+#define PHX_LD256(QUAL)                                                                              \
+    asm volatile("ld.global" QUAL ".v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"                          \
+                 : "=f"(r.x[0]), "=f"(r.x[1]), "=f"(r.x[2]), "=f"(r.x[3]), "=f"(r.x[4]), "=f"(r.x[5]), \
+                   "=f"(r.x[6]), "=f"(r.x[7])                                                         \
+                 : "l"(ptr))
+#define PHX_ST256(QUAL)                                                                              \
+    asm volatile("st.global" QUAL ".v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(ptr), "f"(r.x[0]), \
+                 "f"(r.x[1]), "f"(r.x[2]), "f"(r.x[3]), "f"(r.x[4]), "f"(r.x[5]), "f"(r.x[6]),        \
+                 "f"(r.x[7])                                                                          \
+                 : "memory")
+#define PHX_LD128F(QUAL)                                                   \
+    asm volatile("ld.global" QUAL ".v4.f32 {%0,%1,%2,%3}, [%4];"            \
+                 : "=f"(r.x[0]), "=f"(r.x[1]), "=f"(r.x[2]), "=f"(r.x[3])   \
+                 : "l"(ptr))
+#define PHX_ST128F(QUAL)                                                                          \
+    asm volatile("st.global" QUAL ".v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(ptr), "f"(r.x[0]), "f"(r.x[1]), \
+                 "f"(r.x[2]), "f"(r.x[3])                                                          \
+                 : "memory")
+
+template <int HINT>
+__device__ __forceinline__ F8 ld256(const float *ptr)
+{
+    F8 r;
+    if (HINT == 0) PHX_LD256("");
+    else if (HINT == 2) PHX_LD256(".cs");
+    else PHX_LD256(".L1::no_allocate.L2::evict_first");
+    return r;
+}
+template <int HINT>
+__device__ __forceinline__ void st256(float *ptr, const F8 &r)
+{
+    if (HINT == 0) PHX_ST256("");
+    else if (HINT == 2) PHX_ST256(".cs");
+    else if (HINT == 3) PHX_ST256(".L1::no_allocate.L2::evict_first");
+    else PHX_ST256(".L1::no_allocate");
+}
+template <int HINT>
+__device__ __forceinline__ F4 ld128f(const float *ptr)
+{
+    F4 r;
+    if (HINT == 0) PHX_LD128F("");
+    else if (HINT == 2) PHX_LD128F(".cs");
+    else PHX_LD128F(".L1::no_allocate");  // ptxas: L2::evict_first needs a 256-bit type
+    return r;
+}
+template <int HINT>
+__device__ __forceinline__ void st128f(float *ptr, const F4 &r)
+{
+    if (HINT == 0) PHX_ST128F("");
+    else if (HINT == 2) PHX_ST128F(".cs");
+    else if (HINT == 3) PHX_ST128F(".L1::no_allocate.L2::evict_first");
+    else PHX_ST128F(".L1::no_allocate");
+}
+// gradients: read-only for the whole kernel -> non-coherent path, never allocate in L1
+__device__ __forceinline__ uint4 ldg128_stream(const void *ptr)
+{
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(ptr));
+    return r;
+}
+__device__ __forceinline__ uint2 ldg64_stream(const void *ptr)
+{
+    uint2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];"
+                 : "=r"(r.x), "=r"(r.y)
+                 : "l"(ptr));
+    return r;
+}
+template <int HINT>
+__device__ __forceinline__ void st128u(void *ptr, const uint4 &r)
+{
+    if (HINT == 0)
+        asm volatile("st.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(ptr), "r"(r.x), "r"(r.y), "r"(r.z), "r"(r.w) : "memory");
+    else if (HINT == 2)
+        asm volatile("st.global.cs.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(ptr), "r"(r.x), "r"(r.y), "r"(r.z), "r"(r.w) : "memory");
+    else
+        asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(ptr), "r"(r.x), "r"(r.y), "r"(r.z), "r"(r.w) : "memory");
+}
+template <int HINT>
+__device__ __forceinline__ void st64u(void *ptr, const uint2 &r)
+{
+    if (HINT == 0)
+        asm volatile("st.global.v2.u32 [%0], {%1,%2};" ::"l"(ptr), "r"(r.x), "r"(r.y) : "memory");
+    else if (HINT == 2)
+        asm volatile("st.global.cs.v2.u32 [%0], {%1,%2};" ::"l"(ptr), "r"(r.x), "r"(r.y) : "memory");
+    else
+        asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};" ::"l"(ptr), "r"(r.x), "r"(r.y) : "memory");
+}
+
+// ------------------------------------------------------------------------------------------
+// element arithmetic
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ float bf16lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16hi(uint32_t w) { return __uint_as_float(w & 0xFFFF0000u); }
+
+// two fp32 -> packed bf16x2, round-to-nearest-even (cvt.rn.bf16x2.f32; lo in bits [0,16))
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi)
+{
+    __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t *>(&h);
+}
+
+// One element of the canonical AdamW sequence (include/phx.h a3).  Each intrinsic is one
+// IEEE-754 binary32 operation, round-to-nearest-even; none can be contracted into an FMA.
+__device__ __forceinline__ void adamw_element(float &p, float &m, float &v, float g, float coef,
+                                              const AdamScalars &sc)
+{
+    g = __fmul_rn(g, coef);
+    const float p1 = __fmul_rn(p, sc.decay);
+    const float mn = __fadd_rn(__fmul_rn(sc.beta1, m), __fmul_rn(sc.omb1, g));
+    const float vn = __fadd_rn(__fmul_rn(sc.beta2, v), __fmul_rn(sc.omb2, __fmul_rn(g, g)));
+    const float d = __fadd_rn(__fdiv_rn(__fsqrt_rn(vn), sc.sbc2), sc.eps);
+    p = __fsub_rn(p1, __fmul_rn(sc.ss, __fdiv_rn(mn, d)));
+    m = mn;
+    v = vn;
+}
+
+// ------------------------------------------------------------------------------------------
+// a3: fused step + snapshot, 8 elements per thread-group, 256-bit vectors
+// ------------------------------------------------------------------------------------------
+constexpr int kStepThreads = 256;
+
+template <int HINT, int U, bool SNAP>
+__global__ void __launch_bounds__(kStepThreads) k_step8(const __grid_constant__ StepArgs a)
+{
+    const uint64_t ngroups = a.n_padded >> 3;
+    const uint64_t base = (uint64_t)blockIdx.x * (kStepThreads * U) + threadIdx.x;
+    if (SNAP && blockIdx.x == 0 && threadIdx.x < 16)
+        reinterpret_cast<uint4 *>(a.shdr)[threadIdx.x] = a.hdr.q[threadIdx.x];
+    const float coef = __ldg(a.coef);
+
+    F8 P[U], M[U], V[U];
+    uint4 G[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const uint64_t gi = base + (uint64_t)u * kStepThreads;
+        if (gi < ngroups) {
+            const uint64_t e = gi << 3;
+            G[u] = ldg128_stream(reinterpret_cast<const uint16_t *>(a.g) + e);
+            P[u] = ld256<HINT>(a.p + e);
+            M[u] = ld256<HINT>(a.m + e);
+            V[u] = ld256<HINT>(a.v + e);
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const uint64_t gi = base + (uint64_t)u * kStepThreads;
+        if (gi < ngroups) {
+            const uint64_t e = gi << 3;
+            const uint32_t gw[4] = {G[u].x, G[u].y, G[u].z, G[u].w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                adamw_element(P[u].x[2 * j], M[u].x[2 * j], V[u].x[2 * j], bf16lo(gw[j]), coef, a.sc);
+                adamw_element(P[u].x[2 * j + 1], M[u].x[2 * j + 1], V[u].x[2 * j + 1], bf16hi(gw[j]), coef, a.sc);
+            }
+            uint4 h;
+            h.x = pack_bf16x2(P[u].x[0], P[u].x[1]);
+            h.y = pack_bf16x2(P[u].x[2], P[u].x[3]);
+            h.z = pack_bf16x2(P[u].x[4], P[u].x[5]);
+            h.w = pack_bf16x2(P[u].x[6], P[u].x[7]);
+            st256<HINT>(a.p + e, P[u]);
+            st256<HINT>(a.m + e, M[u]);
+            st256<HINT>(a.v + e, V[u]);
+            st128u<HINT>(reinterpret_cast<uint16_t *>(a.p16) + e, h);
+            if (SNAP) {
+                st256<HINT>(a.sp + e, P[u]);
+                st256<HINT>(a.sm + e, M[u]);
+                st256<HINT>(a.sv + e, V[u]);
+            }
+        }
+    }
+}
+
+// 128-bit flavour: 4 elements per thread-group (classic float4 streaming)
+template <int HINT, int U, bool SNAP>
+__global__ void __launch_bounds__(kStepThreads) k_step4(const __grid_constant__ StepArgs a)
+{
+    const uint64_t ngroups = a.n_padded >> 2;
+    const uint64_t base = (uint64_t)blockIdx.x * (kStepThreads * U) + threadIdx.x;
+    if (SNAP && blockIdx.x == 0 && threadIdx.x < 16)
+        reinterpret_cast<uint4 *>(a.shdr)[threadIdx.x] = a.hdr.q[threadIdx.x];
+    const float coef = __ldg(a.coef);
+
+    F4 P[U], M[U], V[U];
+    uint2 G[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const uint64_t gi = base + (uint64_t)u * kStepThreads;
+        if (gi < ngroups) {
+            const uint64_t e = gi << 2;
+            G[u] = ldg64_stream(reinterpret_cast<const uint16_t *>(a.g) + e);
+            P[u] = ld128f<HINT>(a.p + e);
+            M[u] = ld128f<HINT>(a.m + e);
+            V[u] = ld128f<HINT>(a.v + e);
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const uint64_t gi = base + (uint64_t)u * kStepThreads;
+        if (gi < ngroups) {
+            const uint64_t e = gi << 2;
+            const uint32_t gw[2] = {G[u].x, G[u].y};
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                adamw_element(P[u].x[2 * j], M[u].x[2 * j], V[u].x[2 * j], bf16lo(gw[j]), coef, a.sc);
+                adamw_element(P[u].x[2 * j + 1], M[u].x[2 * j + 1], V[u].x[2 * j + 1], bf16hi(gw[j]), coef, a.sc);
+            }
+            uint2 h;
+            h.x = pack_bf16x2(P[u].x[0], P[u].x[1]);
+            h.y = pack_bf16x2(P[u].x[2], P[u].x[3]);
+            st128f<HINT>(a.p + e, P[u]);
+            st128f<HINT>(a.m + e, M[u]);
+            st128f<HINT>(a.v + e, V[u]);
+            st64u<HINT>(reinterpret_cast<uint16_t *>(a.p16) + e, h);
+            if (SNAP) {
+                st128f<HINT>(a.sp + e, P[u]);
+                st128f<HINT>(a.sm + e, M[u]);
+                st128f<HINT>(a.sv + e, V[u]);
+            }
+        }
+    }
+}
+
+template <int HINT, int U>
+static cudaError_t launch8(const StepArgs &a, bool snapshot, cudaStream_t st)
+{
+    const uint64_t ngroups = a.n_padded >> 3;
+    const uint64_t per_block = (uint64_t)kStepThreads * U;
+    const unsigned grid = (unsigned)((ngroups + per_block - 1) / per_block);
+    if (grid == 0) return cudaSuccess;
+    if (snapshot) k_step8<HINT, U, true><<<grid, kStepThreads, 0, st>>>(a);
+    else k_step8<HINT, U, false><<<grid, kStepThreads, 0, st>>>(a);
+    return cudaGetLastError();
+}
+template <int HINT, int U>
+static cudaError_t launch4(const StepArgs &a, bool snapshot, cudaStream_t st)
+{
+    const uint64_t ngroups = a.n_padded >> 2;
+    const uint64_t per_block = (uint64_t)kStepThreads * U;
+    const unsigned grid = (unsigned)((ngroups + per_block - 1) / per_block);
+    if (grid == 0) return cudaSuccess;
+    if (snapshot) k_step4<HINT, U, true><<<grid, kStepThreads, 0, st>>>(a);
+    else k_step4<HINT, U, false><<<grid, kStepThreads, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, cudaStream_t st)
+{
+    switch (variant) {
+    case 0: return launch8<1, 1>(a, snapshot, st);  // 256-bit, streaming hints (default)
+    case 1: return launch8<0, 1>(a, snapshot, st);  // 256-bit, no hints
+    case 2: return launch8<1, 2>(a, snapshot, st);  // 256-bit, two groups in flight per thread
+    case 3: return launch4<1, 2>(a, snapshot, st);  // 128-bit, two groups per thread
+    case 4: return launch8<2, 1>(a, snapshot, st);  // 256-bit, .cs both ways
+    case 5: return launch8<3, 1>(a, snapshot, st);  // 256-bit, evict_first on stores too
+    case 6: return launch4<1, 4>(a, snapshot, st);  // 128-bit, four groups per thread
+    case 7: return launch4<0, 2>(a, snapshot, st);  // 128-bit, no hints
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a1: sum of squares (fp64, fixed two-stage tree => deterministic run to run) + clip coefficient
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double sq_acc(double acc, uint32_t w)
+{
+    const float lo = bf16lo(w), hi = bf16hi(w);
+    acc += (double)__fmul_rn(lo, lo);  // the square of a bf16 value is exact in fp32
+    acc += (double)__fmul_rn(hi, hi);
+    return acc;
+}
+
+__global__ void __launch_bounds__(256) k_sumsq_partial(const uint4 *__restrict__ g, uint64_t ngroups,
+                                                       double *__restrict__ partials)
+{
+    double acc = 0.0;
+    const uint64_t stride = (uint64_t)gridDim.x * 256;
+    uint64_t gi = (uint64_t)blockIdx.x * 256 + threadIdx.x;
+    for (; gi + 3 * stride < ngroups; gi += 4 * stride) {
+        uint4 w[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) w[k] = ldg128_stream(g + gi + k * stride);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            acc = sq_acc(acc, w[k].x);
+            acc = sq_acc(acc, w[k].y);
+            acc = sq_acc(acc, w[k].z);
+            acc = sq_acc(acc, w[k].w);
+        }
+    }
+    for (; gi < ngroups; gi += stride) {
+        const uint4 w = ldg128_stream(g + gi);
+        acc = sq_acc(acc, w.x);
+        acc = sq_acc(acc, w.y);
+        acc = sq_acc(acc, w.z);
+        acc = sq_acc(acc, w.w);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+    __shared__ double wsum[8];
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = wsum[0];
+#pragma unroll
+        for (int k = 1; k < 8; ++k) s += wsum[k];
+        partials[blockIdx.x] = s;
+    }
+}
+
+__global__ void __launch_bounds__(kSumsqMaxBlocks) k_sumsq_final(const double *__restrict__ partials, int nblocks,
+                                                                 float max_norm, double *__restrict__ out_sumsq,
+                                                                 float *__restrict__ out_coef)
+{
+    __shared__ double sh[kSumsqMaxBlocks];
+    sh[threadIdx.x] = (int)threadIdx.x < nblocks ? partials[threadIdx.x] : 0.0;
+    __syncthreads();
+    for (int o = kSumsqMaxBlocks / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const double S = sh[0];
+        double c = (double)max_norm / (sqrt(S) + 1e-6);  // IEEE double sqrt and divide
+        if (c > 1.0) c = 1.0;
+        *out_sumsq = S;
+        *out_coef = (float)c;  // cvt.rn.f32.f64
+    }
+}
+
+cudaError_t launch_sumsq_clip(const void *g_bf16, uint64_t n_padded, float max_norm, double *partials,
+                              double *out_sumsq, float *out_coef, cudaStream_t st, int *n_launches)
+{
+    const uint64_t ngroups = n_padded >> 3;
+    uint64_t want = (ngroups + 255) / 256;
+    int nblocks = (int)(want < 592 ? want : 592);  // 148 SMs x 4; fixed by n alone
+    if (nblocks < 1) nblocks = 1;
+    k_sumsq_partial<<<nblocks, 256, 0, st>>>(reinterpret_cast<const uint4 *>(g_bf16), ngroups, partials);
+    k_sumsq_final<<<1, kSumsqMaxBlocks, 0, st>>>(partials, nblocks, max_norm, out_sumsq, out_coef);
+    if (n_launches) *n_launches = 2;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// p16 = RNE_bf16(p)
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_regen_bf16(const float *__restrict__ p, void *__restrict__ p16, uint64_t ngroups)
+{
+    const uint64_t gi = (uint64_t)blockIdx.x * 256 + threadIdx.x;
+    if (gi >= ngroups) return;
+    const F8 P = ld256<1>(p + (gi << 3));
+    uint4 h;
+    h.x = pack_bf16x2(P.x[0], P.x[1]);
+    h.y = pack_bf16x2(P.x[2], P.x[3]);
+    h.z = pack_bf16x2(P.x[4], P.x[5]);
+    h.w = pack_bf16x2(P.x[6], P.x[7]);
+    st128u<1>(reinterpret_cast<uint16_t *>(p16) + (gi << 3), h);
+}
+
+cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cudaStream_t st)
+{
+    const uint64_t ngroups = n_padded >> 3;
+    if (ngroups == 0) return cudaSuccess;
+    k_regen_bf16<<<(unsigned)((ngroups + 255) / 256), 256, 0, st>>>(p, p16, ngroups);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// a6: restore from the mapped pinned host replica with 1-D bulk async copies (TMA).
+//   Per CTA: kStages shared-memory stages of 3 x kTile fp32 (p, m, v tiles).  One elected
+//   thread arms an mbarrier with the byte count and issues three cp.async.bulk loads
+//   host -> smem per tile; when they land it issues three cp.async.bulk stores smem -> live
+//   p, m, v (no register traffic), while all threads read the p tile from smem, convert to
+//   bf16 and store the copy.  The host link (PCIe) is the bound; the deep pipeline keeps
+//   148 x 2 x kStages x 24 KB of reads in flight.
+// ------------------------------------------------------------------------------------------
+constexpr int kTile = 2048;  // elements per plane per tile (8 KB)
+constexpr int kStages = 4;
+constexpr int kRestoreThreads = 256;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {  // try_wait suspends the thread in hardware for a bounded time; loop until the phase flips
+        asm volatile(
+            "{\n"
+            ".reg .pred P1;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, P1;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void *gdst, const void *smem_src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+__global__ void __launch_bounds__(kRestoreThreads) k_restore_bulk(const float *__restrict__ src, float *__restrict__ p,
+                                                                  float *__restrict__ m, float *__restrict__ v,
+                                                                  void *__restrict__ p16, uint64_t n_padded)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float *tiles = reinterpret_cast<float *>(smem_raw);  // [kStages][3][kTile]
+    __shared__ __align__(8) uint64_t full[kStages];
+
+    const uint64_t ntiles = (n_padded + kTile - 1) / kTile;
+    const uint64_t my_first = blockIdx.x;
+    const uint64_t stride = gridDim.x;
+    const uint64_t my_count = my_first < ntiles ? (ntiles - my_first + stride - 1) / stride : 0;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    auto issue = [&](uint64_t it) {  // thread 0 only
+        const int s = (int)(it % kStages);
+        const uint64_t t = my_first + it * stride;
+        const uint64_t e0 = t * kTile;
+        const uint32_t cnt = (uint32_t)((n_padded - e0) < (uint64_t)kTile ? (n_padded - e0) : kTile);
+        const uint32_t bytes = cnt * 4u;
+        float *dst = tiles + (size_t)s * 3 * kTile;
+        mbar_expect_tx(&full[s], 3u * bytes);
+        bulk_g2s(dst, src + e0, bytes, &full[s]);
+        bulk_g2s(dst + kTile, src + n_padded + e0, bytes, &full[s]);
+        bulk_g2s(dst + 2 * kTile, src + 2 * n_padded + e0, bytes, &full[s]);
+    };
+
+    if (threadIdx.x == 0)
+        for (uint64_t it = 0; it < my_count && it < (uint64_t)kStages; ++it) issue(it);
+
+    for (uint64_t it = 0; it < my_count; ++it) {
+        const int s = (int)(it % kStages);
+        const uint32_t parity = (uint32_t)((it / kStages) & 1);
+        const uint64_t t = my_first + it * stride;
+        const uint64_t e0 = t * kTile;
+        const uint32_t cnt = (uint32_t)((n_padded - e0) < (uint64_t)kTile ? (n_padded - e0) : kTile);
+        float *tp = tiles + (size_t)s * 3 * kTile;
+        mbar_wait(&full[s], parity);
+        if (threadIdx.x == 0) {
+            bulk_s2g(p + e0, tp, cnt * 4u);
+            bulk_s2g(m + e0, tp + kTile, cnt * 4u);
+            bulk_s2g(v + e0, tp + 2 * kTile, cnt * 4u);
+            bulk_commit();
+        }
+        // bf16 copy: 8 elements per thread, conflict-free 128-bit shared loads
+        const uint32_t e = threadIdx.x * 8;
+        if (e < cnt) {
+            const float4 a = *reinterpret_cast<const float4 *>(tp + e);
+            const float4 b = *reinterpret_cast<const float4 *>(tp + e + 4);
+            uint4 h;
+            h.x = pack_bf16x2(a.x, a.y);
+            h.y = pack_bf16x2(a.z, a.w);
+            h.z = pack_bf16x2(b.x, b.y);
+            h.w = pack_bf16x2(b.z, b.w);
+            st128u<1>(reinterpret_cast<uint16_t *>(p16) + e0 + e, h);
+        }
+        __syncthreads();  // everyone is done reading stage s
+        if (threadIdx.x == 0) {
+            bulk_wait_read0();  // the bulk stores have finished reading stage s
+            if (it + kStages < my_count) issue(it + kStages);
+        }
+    }
+    if (threadIdx.x == 0) bulk_wait_all0();  // stores globally complete before the CTA exits
+}
+
+cudaError_t launch_restore_bulk(const void *src_payload, float *p, float *m, float *v, void *p16,
+                                uint64_t n_padded, int sm_count, cudaStream_t st)
+{
+    if (n_padded == 0) return cudaSuccess;
+    const size_t smem = (size_t)kStages * 3 * kTile * sizeof(float);  // 96 KB
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_restore_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const uint64_t ntiles = (n_padded + kTile - 1) / kTile;
+    uint64_t grid = (uint64_t)sm_count * 2;
+    if (grid > ntiles) grid = ntiles;
+    k_restore_bulk<<<(unsigned)grid, kRestoreThreads, smem, st>>>(reinterpret_cast<const float *>(src_payload), p, m, v,
+                                                                   p16, n_padded);
+    return cudaGetLastError();
+}
+
+}  // namespace phx

@@ -1,0 +1,49 @@
+// phx_kernels.cuh — internal launch interface between the C-ABI layer (phx_api.cu) and the
+// sm_100a kernels (phx_kernels.cu).  Not part of the public boundary (include/phx.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace phx {
+
+// Derived AdamW scalars, computed on the host in double and rounded once (include/phx.h, a3).
+struct AdamScalars {
+    float beta1, beta2, eps, decay, omb1, omb2, ss, sbc2;
+};
+
+// 256-byte envelope passed by value as a kernel parameter; block 0 stores it in front of the
+// staging slot so that the packed snapshot (header ‖ p ‖ m ‖ v) is produced by ONE kernel.
+struct alignas(16) HeaderBlob {
+    uint4 q[16];
+};
+
+struct StepArgs {
+    float *p, *m, *v;            // live planes, n_padded each
+    const void *g;               // bf16 grads
+    void *p16;                   // bf16 param copy
+    float *sp, *sm, *sv;         // staging planes of the slot being written (null if !snapshot)
+    void *shdr;                  // staging slot header (256 B) (null if !snapshot)
+    const float *coef;           // device scalar: clip coefficient (1.0f when clipping is off)
+    uint64_t n_padded;           // multiple of 64
+    AdamScalars sc;
+    HeaderBlob hdr;
+};
+
+enum { kNumStepVariants = 8 };
+
+// a3.  variant selects the kernel flavour (see phx_kernels.cu); snapshot=false drops the staging stores.
+cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, cudaStream_t st);
+
+// a1.  partials: >= kSumsqMaxBlocks doubles of device scratch; out_sumsq/out_coef device scalars.
+enum { kSumsqMaxBlocks = 1024 };
+cudaError_t launch_sumsq_clip(const void *g_bf16, uint64_t n_padded, float max_norm, double *partials,
+                              double *out_sumsq, float *out_coef, cudaStream_t st, int *n_launches);
+
+// p16 = RNE_bf16(p)
+cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cudaStream_t st);
+
+// a6, bulk-kernel mode: src_payload = device-visible address of the host slot's payload (p ‖ m ‖ v).
+cudaError_t launch_restore_bulk(const void *src_payload, float *p, float *m, float *v, void *p16,
+                                uint64_t n_padded, int sm_count, cudaStream_t st);
+
+}  // namespace phx

@@ -1,0 +1,93 @@
+"""Device/pinned memory plumbing for one shard: torch allocates, libphx computes.
+
+`Shard` owns the torch tensors the C library is bound to (live p/m/v/bf16 copy, the device
+staging ring, the pinned host replica) and forwards the hot-path calls to `binding`.  It holds no
+arithmetic and no fallback.
+"""
+from __future__ import annotations
+
+from typing import Optional
+
+import torch
+
+from . import binding as B
+from .workloads import Hyper, Workload
+
+
+class Shard:
+    def __init__(self, wl: Workload, *, device="cuda:0", staging_depth=2, sync_mode=B.PHX_SYNC_STRICT,
+                 chunk_bytes=64 << 20, snapshot=True, restore_mode=B.PHX_RESTORE_BULK_KERNEL,
+                 max_grad_norm: Optional[float] = None, replica: Optional[torch.Tensor] = None):
+        self.wl = wl
+        self.device = torch.device(device)
+        self.hyper: Hyper = wl.hyper
+        mgn = wl.hyper.max_grad_norm if max_grad_norm is None else max_grad_norm
+        self.h = B.phx_shard_create(
+            wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank), pp=(wl.pp_size, wl.pp_rank),
+            staging_depth=staging_depth, sync_mode=sync_mode, chunk_bytes=chunk_bytes,
+            snapshot_disabled=not snapshot, restore_mode=restore_mode, max_grad_norm=mgn)
+        self.info = B.phx_shard_info(self.h)
+        self.n, self.n_padded = self.info.n, self.info.n_padded
+        self.segments = [(tid, off_s, ln) for tid, _, off_s, ln in B.phx_shard_segments(self.h)]
+        N = self.n_padded
+        with torch.cuda.device(self.device):
+            self.p = torch.zeros(N, dtype=torch.float32, device=self.device)
+            self.m = torch.zeros(N, dtype=torch.float32, device=self.device)
+            self.v = torch.zeros(N, dtype=torch.float32, device=self.device)
+            self.p16 = torch.zeros(N, dtype=torch.bfloat16, device=self.device)
+            self.staging = None
+            self.replica = None
+            if snapshot:
+                self.staging = torch.zeros(self.info.staging_depth * self.info.slot_stride,
+                                           dtype=torch.uint8, device=self.device)
+                if replica is None:
+                    replica = torch.zeros(2 * self.info.slot_stride, dtype=torch.uint8).pin_memory()
+                assert replica.is_pinned() and replica.numel() >= 2 * self.info.slot_stride
+                self.replica = replica
+            B.phx_shard_bind(self.h, self.p, self.m, self.v, self.p16, self.staging, self.replica)
+
+    # -- thin forwards -----------------------------------------------------------------
+    def set_state(self, step: int = 0, stream=None):
+        B.phx_shard_set_state(self.h, step, stream or torch.cuda.current_stream(self.device))
+
+    def step_and_snapshot(self, grads: torch.Tensor, step: int, stream=None, hyper: Optional[Hyper] = None):
+        hp = hyper or self.hyper
+        assert grads.dtype == torch.bfloat16 and grads.numel() == self.n_padded and grads.is_cuda
+        B.phx_step_and_snapshot(self.h, grads, hp.lr, hp.beta1, hp.beta2, hp.eps, hp.wd, step,
+                                stream or torch.cuda.current_stream(self.device))
+
+    def flush_async(self, side_stream):
+        B.phx_snapshot_flush_async(self.h, side_stream)
+
+    def wait(self, step: int):
+        B.phx_snapshot_wait(self.h, step)
+
+    def restore(self, stream=None) -> int:
+        return B.phx_restore(self.h, stream or torch.cuda.current_stream(self.device))
+
+    def staging_slot(self, step: int) -> torch.Tensor:
+        k = step % self.info.staging_depth
+        return self.staging[k * self.info.slot_stride: k * self.info.slot_stride + self.info.snapshot_bytes]
+
+    def replica_slot(self, step: int) -> torch.Tensor:
+        k = step % 2
+        return self.replica[k * self.info.slot_stride: k * self.info.slot_stride + self.info.snapshot_bytes]
+
+    def drop_live(self):
+        """'Drop the live shard' (BASELINE.json:configs[3]): zero p, m, v, bf16 copy and scribble
+        over the device staging ring — restore must not depend on anything device-resident."""
+        for t in (self.p, self.m, self.v, self.p16):
+            t.zero_()
+        if self.staging is not None:
+            self.staging.fill_(0xA5)
+
+    def close(self):
+        if self.h:
+            B.phx_shard_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

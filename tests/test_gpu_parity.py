@@ -1,0 +1,386 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the CPU oracle on the same
+seeded inputs, element by element.
+
+Bars (BASELINE.json:north_star):
+  * snapshot and restore bytes: bit-exact;
+  * fp32 state p, m, v: the primary criterion is 0 ulp (both sides execute the same
+    individually-rounded IEEE sequence); the stated tolerance — max relative error 1e-6 per step,
+    1e-5 after 10 steps, under the floor-normalised metric of reading R22 — is asserted as well;
+  * bf16 copy: within 1 bf16 ulp (0 expected and asserted).
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2607_01646_b200 import binding as B
+from paper_2607_01646_b200 import workloads as W
+from paper_2607_01646_b200.shard import Shard
+
+from gpu_util import DEV, assert_state_equal, bits16, hp_of, make_pair, metric_ii
+
+pytestmark = pytest.mark.gpu
+
+
+def side_stream():
+    return torch.cuda.Stream(device=DEV)
+
+
+# ------------------------------------------------------------------------------------------------
+# config c1: 10 steps, snapshot after every step, restore and compare, fault at 5 and resume
+# ------------------------------------------------------------------------------------------------
+
+
+def test_c1_ten_steps_snapshot_restore_bit_exact():
+    wl = W.CONFIGS["c1"]
+    s, o, gdev, gbits = make_pair(wl, steps=10, chunk_bytes=4 << 20, user=b"rng:\x01\x02\x03")
+    hp = hp_of(wl)
+    side = side_stream()
+    for t in range(1, 11):
+        s.step_and_snapshot(gdev[t - 1], t)
+        s.flush_async(side)
+        o.step(gbits[t - 1], **hp, step=t, nthreads=4)
+        o.snapshot()
+        assert_state_equal(s, o, f"step {t}")
+        # tolerance form of the bar (trivially met when the bits agree)
+        lim = 1e-6 if t < 10 else 1e-5
+        for a, b in ((s.p, o.p), (s.m, o.m), (s.v, o.v)):
+            assert metric_ii(a.cpu().numpy(), b) <= lim
+        d16 = np.abs(bits16(s.p16).astype(np.int32) - o.p16.astype(np.int32))
+        assert d16.max() <= 1
+        # the packed snapshot in the device staging slot == the oracle's packed buffer
+        assert np.array_equal(s.staging_slot(t).cpu().numpy(), o.packed_snapshot()), t
+        # ... and the committed host replica slot too (header included)
+        s.wait(t)
+        assert B.phx_snapshot_query(s.h) == (t, t % 2)
+        assert np.array_equal(s.replica_slot(t).numpy(), o.replica[t % 2]), t
+        # restore(snapshot(s)) == s
+        s.drop_live()
+        assert s.restore() == t
+        assert B.phx_restored_user_metadata(s.h) == b"rng:\x01\x02\x03"
+        assert_state_equal(s, o, f"restore after step {t}")
+    s.close()
+
+
+def test_c1_fault_at_step_5_and_resume_matches_uninterrupted():
+    wl = W.CONFIGS["c1"]
+    hp = hp_of(wl)
+    ref, o, gdev, gbits = make_pair(wl, steps=10)
+    for t in range(1, 11):
+        ref.step_and_snapshot(gdev[t - 1], t)
+        o.step(gbits[t - 1], **hp, step=t, nthreads=4)
+    assert_state_equal(ref, o, "uninterrupted")
+    s, _, _, _ = make_pair(wl, steps=0)
+    side = side_stream()
+    for t in range(1, 5):
+        s.step_and_snapshot(gdev[t - 1], t)
+        s.flush_async(side)
+    s.step_and_snapshot(gdev[4], 5)          # step 5 in flight: launched, never flushed
+    s.drop_live()
+    assert s.restore() == 4                  # replay <= 1 step
+    for t in range(5, 11):
+        s.step_and_snapshot(gdev[t - 1], t)
+        s.flush_async(side)
+    torch.cuda.synchronize()
+    for a, b in ((s.p, ref.p), (s.m, ref.m), (s.v, ref.v), (s.p16, ref.p16)):
+        assert torch.equal(a, b)             # GPU vs GPU
+    assert_state_equal(s, o, "resumed")      # GPU vs oracle
+    s.close(); ref.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# sizes: several blocks + ragged tail, tiny, padding, every kernel variant
+# ------------------------------------------------------------------------------------------------
+
+SIZES = [[1], [64], [70], [2047, 1], [2048 * 3 + 64], [256 * 8 * 5 + 192, 33, 1000], [300_000, 77, 12_345]]
+
+
+@pytest.mark.parametrize("numels", SIZES)
+@pytest.mark.parametrize("dp", [1, 3])
+def test_sizes_and_ragged_tails(numels, dp):
+    wl = W.tiny_workload(numels, dp_size=dp, dp_rank=dp - 1)   # the last rank holds the padding
+    s, o, gdev, gbits = make_pair(wl, steps=3, chunk_bytes=4096, init_mv=True)
+    side = side_stream()
+    for t in range(1, 4):
+        s.step_and_snapshot(gdev[t - 1], t)
+        s.flush_async(side)
+        o.step(gbits[t - 1], **hp_of(wl), step=t)
+        o.snapshot()
+        assert_state_equal(s, o, f"{numels} dp{dp} step {t}")
+        s.wait(t)
+        assert np.array_equal(s.replica_slot(t).numpy(), o.replica[t % 2])
+    # pad lanes stay exactly zero
+    if s.n < s.n_padded:
+        for a in (s.p, s.m, s.v):
+            assert not a[s.n:].cpu().numpy().view(np.uint32).any()
+        assert not bits16(s.p16[s.n:]).any()
+    s.drop_live()
+    assert s.restore() == 3
+    assert_state_equal(s, o, "restore")
+    s.close()
+
+
+@pytest.mark.parametrize("variant", range(8))
+def test_every_kernel_variant_is_bit_identical(variant):
+    wl = W.tiny_workload([256 * 8 * 7 + 64 * 5, 999], dp_size=1, grad_kind="heavy_tail")
+    s, o, gdev, gbits = make_pair(wl, steps=4, init_mv=True)
+    B.phx_set_kernel_variant(s.h, variant)
+    for t in range(1, 5):
+        s.step_and_snapshot(gdev[t - 1], t)
+        o.step(gbits[t - 1], **hp_of(wl), step=t)
+        assert_state_equal(s, o, f"variant {variant} step {t}")
+        assert np.array_equal(s.staging_slot(t).cpu().numpy(), o.packed_snapshot())
+    s.close()
+
+
+def test_extreme_values_denormals_and_zeros():
+    n = 64 * 1000
+    wl = W.tiny_workload([n], dp_size=1)
+    rng = np.random.default_rng(5)
+    grads = []
+    for t in range(6):
+        scale = rng.choice([1e-38, 1e-30, 1e-20, 1e-12, 1e-3, 1.0, 1e4, 1e15], n)
+        g = torch.from_numpy((rng.standard_t(3, n) * scale).astype(np.float32)).to(torch.bfloat16)
+        g[::97] = 0
+        g[1::97] = -0.0
+        grads.append(g)
+    s, o, gdev, gbits = make_pair(wl, steps=6, grads=grads)
+    p0 = s.p.cpu()
+    p0[:50] = 0
+    p0[50:60] = 1e-42            # denormal parameters
+    s.p.copy_(p0); s.set_state(0); o.set_state(p0.numpy())
+    for t in range(1, 7):
+        s.step_and_snapshot(gdev[t - 1], t)
+        o.step(gbits[t - 1], **hp_of(wl), step=t)
+        assert_state_equal(s, o, f"extremes step {t}")
+    assert np.isfinite(o.p).all()
+    s.close()
+
+
+def test_snapshot_off_variant_gives_identical_live_bits():
+    wl = W.tiny_workload([100_000, 31], dp_size=2, dp_rank=0)
+    a, o, gdev, gbits = make_pair(wl, steps=3)
+    b, _, _, _ = make_pair(wl, steps=0, snapshot=False)
+    for t in range(1, 4):
+        a.step_and_snapshot(gdev[t - 1], t)
+        b.step_and_snapshot(gdev[t - 1], t)
+        o.step(gbits[t - 1], **hp_of(wl), step=t)
+    assert_state_equal(a, o, "snapshot on")
+    assert_state_equal(b, o, "snapshot off")
+    with pytest.raises(B.PhxError) as e:
+        b.flush_async(side_stream())
+    assert e.value.code == B.PHX_ERR_SNAPSHOT_DISABLED
+    a.close(); b.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# clip (a1)
+# ------------------------------------------------------------------------------------------------
+
+
+@pytest.mark.parametrize("n,max_norm", [(64, 1e-3), (5000, 0.01), (1_000_000, 0.5), (1_000_000, 1e6)])
+def test_clip_coefficient_and_clipped_step(n, max_norm):
+    wl = W.tiny_workload([n], dp_size=1, grad_kind="heavy_tail", hyper=W.Hyper(max_grad_norm=max_norm))
+    s, o, gdev, gbits = make_pair(wl, steps=3)
+    for t in range(1, 4):
+        s.step_and_snapshot(gdev[t - 1], t)
+        o.step(gbits[t - 1], **hp_of(wl), step=t)
+        coef, S = B.phx_last_clip(s.h)
+        So = O.sumsq(gbits[t - 1])
+        assert abs(S - So) <= 4e-15 * So                        # fp64 tree vs long-double sequential sum
+        # the fp32 coefficient is the decision both sides take in double; a different summation
+        # order can flip its last bit with probability ~1e-8 per step (reading R7)
+        assert np.float32(coef) == o.last_coef, (coef, o.last_coef)
+        if max_norm >= 1e6:
+            assert coef == 1.0
+        else:
+            assert coef < 1.0
+        assert_state_equal(s, o, f"clip step {t}")
+    s.close()
+
+
+def test_clip_hand_computable():
+    wl = W.tiny_workload([64], dp_size=1, hyper=W.Hyper(max_grad_norm=1e-3))
+    g = torch.zeros(64)
+    g[0], g[1] = 3 * 2.0 ** -10, 4 * 2.0 ** -10
+    s, o, gdev, gbits = make_pair(wl, steps=1, grads=[g.to(torch.bfloat16)])
+    s.step_and_snapshot(gdev[0], 1)
+    coef, S = B.phx_last_clip(s.h)
+    assert S == 25 * 2.0 ** -20
+    assert np.float32(coef) == np.float32(float(np.float32(1e-3)) / (5 * 2.0 ** -10 + 1e-6))
+    s.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# replica engine: ping-pong, torn flush, sync modes, depth, restore modes, identity
+# ------------------------------------------------------------------------------------------------
+
+
+@pytest.mark.parametrize("mode", [B.PHX_SYNC_STRICT, B.PHX_SYNC_RELAXED])
+@pytest.mark.parametrize("depth", [1, 2, 3, 4])
+def test_depth_and_sync_modes(mode, depth):
+    wl = W.tiny_workload([400_000, 1234], dp_size=1)
+    s, o, gdev, gbits = make_pair(wl, steps=9, chunk_bytes=256 << 10, staging_depth=depth, sync_mode=mode)
+    side = side_stream()
+    for t in range(1, 10):
+        s.step_and_snapshot(gdev[t - 1], t)
+        s.flush_async(side)
+        o.step(gbits[t - 1], **hp_of(wl), step=t)
+        o.snapshot()
+    s.wait(9)
+    assert_state_equal(s, o, "end")
+    for t in (8, 9):
+        assert np.array_equal(s.replica_slot(t).numpy(), o.replica[t % 2]), (t, mode, depth)
+    s.close()
+
+
+@pytest.mark.parametrize("rmode", [B.PHX_RESTORE_BULK_KERNEL, B.PHX_RESTORE_COPY_ENGINE])
+def test_torn_flush_is_never_chosen(rmode):
+    wl = W.tiny_workload([300_000], dp_size=1)
+    s, o, gdev, gbits = make_pair(wl, steps=4, chunk_bytes=128 << 10, restore_mode=rmode,
+                                  sync_mode=B.PHX_SYNC_RELAXED)
+    side = side_stream()
+    hp = hp_of(wl)
+    for t in (1, 2):
+        s.step_and_snapshot(gdev[t - 1], t); s.flush_async(side)
+        o.step(gbits[t - 1], **hp, step=t); o.snapshot()
+    s.step_and_snapshot(gdev[2], 3)
+    o.step(gbits[2], **hp, step=3)
+    B.phx_fault_inject_torn_flush(s.h, 5)        # flush(3) dies after 5 of 28 payload chunks
+    s.flush_async(side)
+    o.snapshot(abort_after_chunks=5)
+    with pytest.raises(B.PhxError) as e:
+        s.wait(3)
+    assert e.value.code == B.PHX_ERR_CORRUPT_SLOT
+    assert B.phx_snapshot_query(s.h) == (2, 0)
+    assert np.array_equal(s.replica_slot(3).numpy(), o.replica[1])     # torn slot: same bytes, no header
+    assert not s.replica_slot(3)[:256].numpy().any()
+    s.step_and_snapshot(gdev[3], 4)              # step 4 in flight when the fault hits
+    s.drop_live(); o.drop_live()
+    assert s.restore() == 2 and o.restore() == 2
+    assert_state_equal(s, o, "restored from the surviving slot")
+    for t in (3, 4):                             # replay 3..4
+        s.step_and_snapshot(gdev[t - 1], t); s.flush_async(side)
+        o.step(gbits[t - 1], **hp, step=t); o.snapshot()
+    s.wait(4)
+    assert_state_equal(s, o, "replayed")
+    assert np.array_equal(s.replica_slot(4).numpy(), o.replica[0])
+    s.close()
+
+
+@pytest.mark.parametrize("rmode", [B.PHX_RESTORE_BULK_KERNEL, B.PHX_RESTORE_COPY_ENGINE])
+@pytest.mark.parametrize("numels", [[64], [2048 * 9 + 64 * 3], [1_000_000, 17]])
+def test_restore_modes_and_replacement_rank(rmode, numels):
+    wl = W.tiny_workload(numels, dp_size=2, dp_rank=1, tp_size=2, tp_rank=1)
+    s, o, gdev, gbits = make_pair(wl, steps=2, restore_mode=rmode, user=b"seed=7")
+    side = side_stream()
+    for t in (1, 2):
+        s.step_and_snapshot(gdev[t - 1], t); s.flush_async(side)
+        o.step(gbits[t - 1], **hp_of(wl), step=t); o.snapshot()
+    s.wait(2)
+    # a replacement rank: a FRESH handle with fresh device memory, bound to the surviving replica
+    r = Shard(wl, device=DEV, restore_mode=rmode, replica=s.replica)
+    assert r.restore() == 2
+    assert B.phx_restored_user_metadata(r.h) == b"seed=7"
+    assert_state_equal(r, o, "replacement rank")
+    # a rank with another logical identity must refuse the replica
+    other = W.tiny_workload(numels, dp_size=2, dp_rank=0, tp_size=2, tp_rank=1)
+    x = Shard(other, device=DEV, replica=s.replica)
+    if x.info.snapshot_bytes == s.info.snapshot_bytes:
+        with pytest.raises(B.PhxError) as e:
+            x.restore()
+        assert e.value.code == B.PHX_ERR_LAYOUT_MISMATCH
+    x.close(); r.close(); s.close()
+
+
+def test_protocol_errors_on_device():
+    wl = W.tiny_workload([1000], dp_size=1)
+    s, o, gdev, _ = make_pair(wl, steps=2)
+    with pytest.raises(B.PhxError) as e:
+        s.restore()
+    assert e.value.code == B.PHX_ERR_NO_COMMITTED_SNAPSHOT
+    with pytest.raises(B.PhxError) as e:
+        s.flush_async(side_stream())
+    assert e.value.code == B.PHX_ERR_NO_FLUSH_PENDING
+    with pytest.raises(B.PhxError) as e:
+        s.step_and_snapshot(gdev[0], 2)
+    assert e.value.code == B.PHX_ERR_STEP_ORDER
+    s.step_and_snapshot(gdev[0], 1)
+    with pytest.raises(B.PhxError) as e:
+        s.step_and_snapshot(gdev[0], 1)
+    assert e.value.code == B.PHX_ERR_STEP_ORDER
+    with pytest.raises(B.PhxError) as e:
+        B.phx_step_and_snapshot(s.h, gdev[1].data_ptr() + 2, 1e-3, 0.9, 0.95, 1e-8, 0.1, 2, None)
+    assert e.value.code == B.PHX_ERR_ALIGNMENT
+    assert B.phx_kernel_launches(s.h) == 2      # set_state's bf16 regeneration + one fused step
+    s.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# full size, in the launch configuration bench.py times: sampled element-by-element parity and
+# properties that hold at any size
+# ------------------------------------------------------------------------------------------------
+
+
+def _sample_windows(n_padded, rng, k=48, w=4096):
+    starts = [0, max(0, n_padded - w)] + [int(x) // 64 * 64 for x in rng.integers(0, max(1, n_padded - w), k)]
+    return [(a, min(a + w, n_padded)) for a in starts]
+
+
+@pytest.mark.parametrize("key", ["c2", "c3"])
+def test_full_size_sampled_parity(key):
+    wl = W.CONFIGS[key]
+    free, _ = torch.cuda.mem_get_info()
+    s = Shard(wl, device=DEV)
+    N = s.n_padded
+    s.p.copy_(W.init_params(s.n, N, wl.seed, device=DEV))
+    s.set_state(0)
+    rng = np.random.default_rng(11)
+    wins = _sample_windows(N, rng)
+    idx = torch.cat([torch.arange(a, b) for a, b in wins]).to(DEV)
+    ref = dict(p=s.p[idx].cpu().numpy().copy(), m=np.zeros(idx.numel(), np.float32),
+               v=np.zeros(idx.numel(), np.float32), h=np.zeros(idx.numel(), np.uint16))
+    side = side_stream()
+    hp = hp_of(wl)
+    for t in range(1, 4):
+        g = W.gen_grads(wl, s.segments, N, t, wl.seed, device=DEV)
+        s.step_and_snapshot(g, t)
+        s.flush_async(side)
+        coef = 1.0
+        if wl.hyper.max_grad_norm > 0:
+            coef, S = B.phx_last_clip(s.h)
+            # full-size sum of squares against an independent fp64 reduction (torch), then the
+            # oracle's coefficient formula on the oracle's own sum over the full gradient
+            gb = bits16(g)
+            So = O.sumsq(gb)
+            assert abs(S - So) <= 1e-13 * So
+            assert np.float32(coef) == O.clip_coef(So, wl.hyper.max_grad_norm)
+            assert 0.02 < coef < 0.2          # clip always active at c3 statistics (~0.048)
+        gs = bits16(g[idx]).copy()
+        O.adamw_step(ref["p"], ref["m"], ref["v"], gs, ref["h"], **hp, step=t, coef=float(coef), nthreads=4)
+        torch.cuda.synchronize()
+        assert np.array_equal(s.p[idx].cpu().numpy().view(np.uint32), ref["p"].view(np.uint32)), t
+        assert np.array_equal(s.m[idx].cpu().numpy().view(np.uint32), ref["m"].view(np.uint32)), t
+        assert np.array_equal(s.v[idx].cpu().numpy().view(np.uint32), ref["v"].view(np.uint32)), t
+        assert np.array_equal(bits16(s.p16[idx]), ref["h"]), t
+        # properties at full size: staging planes == live planes; bf16 copy == RNE(p); replica == staging
+        st = s.staging_slot(t)
+        assert torch.equal(st[256:256 + 4 * N].view(torch.float32), s.p)
+        assert torch.equal(st[256 + 4 * N:256 + 8 * N].view(torch.float32), s.m)
+        assert torch.equal(st[256 + 8 * N:].view(torch.float32), s.v)
+        assert torch.equal(s.p.to(torch.bfloat16), s.p16)
+        del g
+    s.wait(3)
+    rep = s.replica_slot(3)
+    CH = 1 << 28
+    for off in range(0, rep.numel(), CH):
+        assert torch.equal(rep[off:off + CH].to(DEV), s.staging_slot(3)[off:off + CH])
+    hdr = O.parse_header(rep[:256].numpy().tobytes())
+    assert hdr is not None and hdr["step"] == 3 and hdr["n"] == wl.n_expected
+    before = [x.clone() for x in (s.p, s.m, s.v, s.p16)]
+    s.drop_live()
+    assert s.restore() == 3
+    torch.cuda.synchronize()
+    for a, b in zip((s.p, s.m, s.v, s.p16), before):
+        assert torch.equal(a, b)
+    s.close()
