@@ -52,7 +52,7 @@ def parse_args():
     ap.add_argument("--config", default="c2", help="workload key (c1, c2, c3, c4a, c4b, c5)")
     ap.add_argument("--variant", type=int, default=0, help="fused-kernel variant (tuning)")
     ap.add_argument("--depth", type=int, default=2)
-    ap.add_argument("--chunk-mib", type=int, default=64)
+    ap.add_argument("--chunk-mib", type=int, default=8)
     ap.add_argument("--sync", default="strict", choices=["strict", "relaxed"])
     ap.add_argument("--gemms", type=int, default=0, help="GEMMs per overlapped iteration (0 = auto: T_c >= 4 T_D2H)")
     ap.add_argument("--overlap-iters", type=int, default=20)
@@ -60,6 +60,19 @@ def parse_args():
     ap.add_argument("--no-overlap", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=0, help="elements of the shard the oracle is timed on (0 = auto)")
+    ap.add_argument("--mode", default="headline",
+                    choices=["headline", "configs", "overlap-curve", "sweep", "hotswap"],
+                    help="headline: the ONE contract line (default).  The others print one JSON line per "
+                         "measurement: configs = every config's kernel/flush/restore; overlap-curve = exposed ms vs G; "
+                         "sweep = chunk x depth x sync-mode grid (BASELINE.json:configs[4]); hotswap = configs[3]")
+    ap.add_argument("--overlap-reps", type=int, default=2, help="ABAB alternations of the overlap arms")
+    ap.add_argument("--source", default="staged", choices=["staged", "direct"],
+                    help="snapshot source: staged = fused kernel also writes the staging slot (40 B/elem, north_star); "
+                         "direct = flush DMAs the live planes under the strict sync point (28 B/elem)")
+    ap.add_argument("--restore-mode", default="copy", choices=["bulk", "copy"])
+    ap.add_argument("--chunks", default="4,8,16,32,64,128,256", help="chunk sizes (MiB) of --mode sweep")
+    ap.add_argument("--depths", default="1,2,3,4", help="staging depths of --mode sweep")
+    ap.add_argument("--syncs", default="strict,relaxed", help="sync modes of --mode sweep")
     return ap.parse_args()
 
 
@@ -253,6 +266,259 @@ def run_reference(args):
 # ----------------------------------------------------------------------------------------------
 
 
+class Rig:
+    """One shard on one GPU plus everything the measurements need around it: gradients resident in HBM
+    and in pinned host memory, a flush stream, the GEMM operands of the stand-in compute window."""
+
+    def __init__(self, args, key, rank=0, world=1, local_rank=0, depth=None, chunk_mib=None, sync=None,
+                 replica=None, host_grads=True, restore_mode=None, source=None):
+        import dataclasses
+        import torch
+        from paper_2607_01646_b200 import binding as B
+        from paper_2607_01646_b200 import workloads as W
+        from paper_2607_01646_b200.shard import Shard
+        self.torch, self.B, self.W, self.Shard, self.args = torch, B, W, Shard, args
+        self.device = torch.device(f"cuda:{local_rank}")
+        base = W.CONFIGS[key]
+        # weak scaling: every rank owns one DP shard of the same model (its own dp_rank); no data-path collective
+        self.wl = dataclasses.replace(base, dp_rank=rank % base.dp_size)
+        self.depth = depth or args.depth
+        self.chunk_mib = chunk_mib or args.chunk_mib
+        self.sync_name = sync or args.sync
+        sync_mode = B.PHX_SYNC_STRICT if self.sync_name == "strict" else B.PHX_SYNC_RELAXED
+        self.source_name = source or args.source
+        self.source = B.PHX_SNAPSHOT_DIRECT if self.source_name == "direct" else B.PHX_SNAPSHOT_STAGED
+        self.bytes_per_elem = BYTES_PER_ELEM_OFF if self.source_name == "direct" else BYTES_PER_ELEM
+        if restore_mode is None:
+            restore_mode = B.PHX_RESTORE_COPY_ENGINE if args.restore_mode == "copy" else B.PHX_RESTORE_BULK_KERNEL
+        self.restore_mode_name = "copy_engine" if restore_mode == B.PHX_RESTORE_COPY_ENGINE else "bulk_kernel"
+        self.s = Shard(self.wl, device=self.device, staging_depth=self.depth, sync_mode=sync_mode,
+                       chunk_bytes=self.chunk_mib << 20, replica=replica, restore_mode=restore_mode,
+                       snapshot_source=self.source)
+        B.phx_set_kernel_variant(self.s.h, args.variant)
+        self.N = self.s.n_padded
+        self.s.p.copy_(W.init_params(self.s.n, self.N, self.wl.seed, device=self.device))
+        self.s.set_state(0)
+        self.grads = [W.gen_grads(self.wl, self.s.segments, self.N, t, self.wl.seed, device=self.device) for t in (1, 2)]
+        self.hgrads = [g.cpu().pin_memory() for g in self.grads] if host_grads else None
+        torch.cuda.synchronize()
+        self.cur = torch.cuda.current_stream(self.device)
+        self.side = torch.cuda.Stream(device=self.device)
+        self.step = 0
+        self.s_off = None
+        self.off_step = 0
+        self._gemm = None
+        self.gemm_ms = None
+
+    # -- the hot path -------------------------------------------------------------------------------
+    def do_step(self):
+        self.step += 1
+        self.s.step_and_snapshot(self.grads[self.step & 1], self.step)
+
+    def time_steps(self, K, Wm):
+        """K back-to-back a1..a3 passes after Wm warm-ups; CUDA events on the launching stream."""
+        torch, B = self.torch, self.B
+        for _ in range(Wm):
+            self.do_step()
+        torch.cuda.synchronize()
+        l0 = B.phx_kernel_launches(self.s.h)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+        ev[0].record(self.cur)
+        for k in range(K):
+            self.do_step()
+            ev[k + 1].record(self.cur)
+        torch.cuda.synchronize()
+        per = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
+        return ev[0].elapsed_time(ev[K]), per, B.phx_kernel_launches(self.s.h) - l0
+
+    def time_fused_kernel_alone(self, K):
+        """The dominant kernel without the clip kernels: a second handle with clipping off bound to the same memory."""
+        torch, B, wl = self.torch, self.B, self.wl
+        h0 = B.phx_shard_create(wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank),
+                                pp=(wl.pp_size, wl.pp_rank), staging_depth=self.depth, max_grad_norm=0.0,
+                                snapshot_source=self.source)
+        B.phx_shard_bind(h0, self.s.p, self.s.m, self.s.v, self.s.p16, self.s.staging, self.s.replica)
+        B.phx_shard_set_state(h0, 0, self.cur)
+        B.phx_set_kernel_variant(h0, self.args.variant)
+        hp = wl.hyper
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for k in range(3 + K):
+            if k == 3:
+                e0.record(self.cur)
+            B.phx_step_and_snapshot(h0, self.grads[k & 1], hp.lr, hp.beta1, hp.beta2, hp.eps, hp.wd, k + 1, self.cur)
+        e1.record(self.cur)
+        torch.cuda.synchronize()
+        B.phx_shard_destroy(h0)
+        return e0.elapsed_time(e1) / K
+
+    def off_shard(self):
+        """Snapshot-disabled handle (the paper's 'mechanism disabled' baseline) bound to the same live arrays."""
+        if self.s_off is None:
+            B, wl = self.B, self.wl
+            h = B.phx_shard_create(wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank),
+                                   pp=(wl.pp_size, wl.pp_rank), snapshot_disabled=True,
+                                   max_grad_norm=wl.hyper.max_grad_norm)
+            B.phx_shard_bind(h, self.s.p, self.s.m, self.s.v, self.s.p16, None, None)
+            B.phx_shard_set_state(h, 0, self.cur)
+            B.phx_set_kernel_variant(h, self.args.variant)
+            self.s_off = h
+        return self.s_off
+
+    def do_step_off(self):
+        hp = self.wl.hyper
+        self.off_step += 1
+        self.B.phx_step_and_snapshot(self.off_shard(), self.grads[self.off_step & 1], hp.lr, hp.beta1, hp.beta2,
+                                     hp.eps, hp.wd, self.off_step, self.cur)
+
+    def time_steps_off(self, K, Wm=3):
+        torch = self.torch
+        for _ in range(Wm):
+            self.do_step_off()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(self.cur)
+        for _ in range(K):
+            self.do_step_off()
+        e1.record(self.cur)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / K
+
+    def time_flush(self):
+        """One a4+a5 flush alone, timed on the side stream."""
+        torch = self.torch
+        self.do_step()
+        torch.cuda.synchronize()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record(self.side)
+        self.s.flush_async(self.side)
+        f1.record(self.side)
+        self.s.wait(self.step)
+        torch.cuda.synchronize()
+        return f0.elapsed_time(f1)
+
+    def e2e(self, Ke, world=1):
+        """Host buffers in, host replica out, through the same C-ABI calls."""
+        torch = self.torch
+
+        def loop(k_steps):
+            for _ in range(k_steps):
+                self.step += 1
+                g = self.grads[self.step & 1]
+                g.copy_(self.hgrads[self.step & 1], non_blocking=True)   # H2D of this step's inputs
+                self.s.step_and_snapshot(g, self.step)
+                self.s.flush_async(self.side)                            # D2H of this step's result (a4 + a5)
+            self.s.wait(self.step)
+        loop(2)
+        torch.cuda.synchronize()
+        barrier(world)
+        t0 = time.perf_counter()
+        loop(Ke)
+        torch.cuda.synchronize()
+        barrier(world)
+        return (time.perf_counter() - t0) * 1e3 / Ke
+
+    def restore_timing(self):
+        """Drop the live shard, restore from the host replica, recompute the in-flight step."""
+        torch = self.torch
+        torch.cuda.synchronize()
+        self.s.drop_live()
+        torch.cuda.synchronize()
+        r0, r1, r2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        r0.record(self.cur)
+        back = self.s.restore()
+        r1.record(self.cur)
+        self.step = back
+        self.do_step()
+        r2.record(self.cur)
+        torch.cuda.synchronize()
+        return back, r0.elapsed_time(r1), r1.elapsed_time(r2)
+
+    # -- the stand-in compute window ----------------------------------------------------------------
+    def gemm_setup(self):
+        torch = self.torch
+        if self._gemm is None:
+            a = torch.randn(4096, 4096, device=self.device, dtype=torch.bfloat16)
+            b = torch.randn(4096, 4096, device=self.device, dtype=torch.bfloat16)
+            c = torch.empty(4096, 4096, device=self.device, dtype=torch.bfloat16)
+            self._gemm = (a, b, c)
+            for _ in range(20):
+                torch.matmul(a, b, out=c)
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record(self.cur)
+            for _ in range(200):
+                torch.matmul(a, b, out=c)
+            g1.record(self.cur)
+            torch.cuda.synchronize()
+            self.gemm_ms = g0.elapsed_time(g1) / 200
+        return self.gemm_ms
+
+    def headline_gemms(self, flush_ms, factor=4.0):
+        """R21: smallest power of two G with T_c >= factor x T_D2H."""
+        gm = self.gemm_setup()
+        G = 64
+        while G * gm < factor * flush_ms:
+            G *= 2
+        return G
+
+    def overlap(self, G, iters, reps, arms=("off", "staged", "on"), warm=2):
+        """Iterations of G GEMMs + the hot path, three arms alternated `reps` times (ABCABC) to average
+        out clock drift:
+          off    — snapshot-disabled kernel, no flush (the paper's baseline run);
+          staged — snapshot-on kernel (writes the staging slot), no flush;
+          on     — snapshot-on kernel + flush on the side stream (PHOENIX enabled).
+        Per-iteration times from CUDA events on the compute stream; PAPER.md:283 trimming."""
+        torch = self.torch
+        self.gemm_setup()
+        a, b, c = self._gemm
+        it_ms = {k: [] for k in arms}
+        hp_ms = {k: [] for k in arms}
+        for _ in range(reps):
+            for arm in arms:
+                evs, kevs = [], []
+                for it in range(warm + iters):
+                    e0 = torch.cuda.Event(enable_timing=True)
+                    e0.record(self.cur)
+                    for _ in range(G):
+                        torch.matmul(a, b, out=c)
+                    k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    k0.record(self.cur)
+                    if arm == "off":
+                        self.do_step_off()
+                    else:
+                        self.do_step()
+                    k1.record(self.cur)
+                    if arm == "on":
+                        self.s.flush_async(self.side)
+                    evs.append(e0)
+                    kevs.append((k0, k1))
+                end = torch.cuda.Event(enable_timing=True)
+                end.record(self.cur)
+                torch.cuda.synchronize()
+                if arm == "on":
+                    self.s.wait(self.step)
+                evs.append(end)
+                it_ms[arm] += [evs[i].elapsed_time(evs[i + 1]) for i in range(warm, warm + iters)]
+                hp_ms[arm] += [x.elapsed_time(y) for x, y in kevs[warm:]]
+        t = {k: trimmed_mean(v) for k, v in it_ms.items()}
+        out = {"gemms_per_iter": G, "gemm_ms": self.gemm_ms, "compute_window_ms": G * self.gemm_ms,
+               "iters_per_arm": iters * reps, "reps": reps,
+               "protocol": "PAPER.md:283: warm-up dropped, slowest 5% dropped, mean of the rest; arms alternated"}
+        for k in arms:
+            out[f"iter_ms_{k}"] = t[k]
+            out[f"hot_path_ms_in_loop_{k}"] = trimmed_mean(hp_ms[k])
+        if "on" in t and "off" in t:
+            out["exposed_ms"] = t["on"] - t["off"]
+            out["exposed_frac_of_compute_step"] = (t["on"] - t["off"]) / t["off"]
+        if "staged" in t and "off" in t:
+            out["exposed_ms_kernel_only"] = t["staged"] - t["off"]
+        return out
+
+    def close(self):
+        if self.s_off is not None:
+            self.B.phx_shard_destroy(self.s_off)
+            self.s_off = None
+        self.s.close()
+
+
 def measure_host_link(torch, device, nbytes=1 << 30, reps=5):
     """Measured pinned-copy peak of the host link, each direction (north_star)."""
     h = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
@@ -272,183 +538,96 @@ def measure_host_link(torch, device, nbytes=1 << 30, reps=5):
     return out
 
 
-def run_phx(args):
+def gpu_setup():
     import torch
     rank, world, local_rank = rank_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --impl phx needs a B200: there is no CPU fallback")
-    device = torch.device(f"cuda:{local_rank}")
-    torch.cuda.set_device(device)
+    torch.cuda.set_device(local_rank)
     dist_init(world, True)
+    return torch, rank, world, local_rank
 
-    from paper_2607_01646_b200 import binding as B
-    from paper_2607_01646_b200 import workloads as W
-    from paper_2607_01646_b200.shard import Shard
-    import dataclasses
 
-    base = W.CONFIGS[args.config]
-    # weak scaling: every rank owns one DP shard of the same model (its own dp_rank), no data-path collective
-    wl = dataclasses.replace(base, dp_rank=rank % base.dp_size)
-    sync = B.PHX_SYNC_STRICT if args.sync == "strict" else B.PHX_SYNC_RELAXED
-    chunk = args.chunk_mib << 20
+def run_headline(args):
+    torch, rank, world, local_rank = gpu_setup()
+    rig = Rig(args, args.config, rank, world, local_rank)
+    device, N, wl, B = rig.device, rig.N, rig.wl, rig.B
     K, Wm = args.steps, max(args.warmup, 3)
-
-    s = Shard(wl, device=device, staging_depth=args.depth, sync_mode=sync, chunk_bytes=chunk)
-    B.phx_set_kernel_variant(s.h, args.variant)
-    N = s.n_padded
-    s.p.copy_(W.init_params(s.n, N, wl.seed, device=device))
-    s.set_state(0)
-    grads = [W.gen_grads(wl, s.segments, N, t, wl.seed, device=device) for t in (1, 2)]
-    hgrads = [g.cpu().pin_memory() for g in grads]       # e2e: the step's inputs live in pinned host memory
-    torch.cuda.synchronize()
-    cur = torch.cuda.current_stream(device)
-    side = torch.cuda.Stream(device=device)
-    step = 0
-
     link = measure_host_link(torch, device) if rank == 0 else {}
 
     # ---- value: K back-to-back a1..a3 passes, inputs resident in HBM ---------------------------------
     for _ in range(Wm):
-        step += 1
-        s.step_and_snapshot(grads[step & 1], step)
+        rig.do_step()
     torch.cuda.synchronize()
     barrier(world)
     clocks = ClockSampler(local_rank) if rank == 0 else None
-    l0 = B.phx_kernel_launches(s.h)
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
-    ev[0].record(cur)
-    for k in range(K):
-        step += 1
-        s.step_and_snapshot(grads[step & 1], step)
-        ev[k + 1].record(cur)
-    torch.cuda.synchronize()
+    total_ms, per, launches = rig.time_steps(K, 0)
     barrier(world)
-    launches = B.phx_kernel_launches(s.h) - l0
-    total_ms = ev[0].elapsed_time(ev[K])
     clk = clocks.stop() if clocks else None
-    per = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
     total_ms = max_over_ranks(total_ms, world, device)
     ms_per_step = total_ms / K
     units = sum_over_ranks(float(N), world, device)            # elements all ranks processed per step
-    value = BYTES_PER_ELEM * units / (ms_per_step * 1e-3) / 1e9
+    BPE = rig.bytes_per_elem                                   # 40 staged (north_star), 28 direct
+    value = BPE * units / (ms_per_step * 1e-3) / 1e9
 
-    # dominant kernel alone (differs from the step only when the clip kernels run): a handle with
-    # clipping off bound to the same memory
-    kern_ms = ms_per_step
-    if wl.hyper.max_grad_norm > 0:
-        cfg0 = dataclasses.replace(wl, hyper=dataclasses.replace(wl.hyper, max_grad_norm=0.0))
-        h0 = B.phx_shard_create(cfg0.layout(), cfg0.dp_size, cfg0.dp_rank, tp=(cfg0.tp_size, cfg0.tp_rank),
-                                pp=(cfg0.pp_size, cfg0.pp_rank), staging_depth=args.depth, sync_mode=sync,
-                                chunk_bytes=chunk)
-        B.phx_shard_bind(h0, s.p, s.m, s.v, s.p16, s.staging, s.replica)
-        B.phx_shard_set_state(h0, 0, cur)
-        hp = wl.hyper
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        for k in range(3):
-            B.phx_step_and_snapshot(h0, grads[k & 1], hp.lr, hp.beta1, hp.beta2, hp.eps, hp.wd, k + 1, cur)
-        e0.record(cur)
-        for k in range(3, 3 + K):
-            B.phx_step_and_snapshot(h0, grads[k & 1], hp.lr, hp.beta1, hp.beta2, hp.eps, hp.wd, k + 1, cur)
-        e1.record(cur)
-        torch.cuda.synchronize()
-        kern_ms = e0.elapsed_time(e1) / K
-        B.phx_shard_destroy(h0)
+    kern_ms = rig.time_fused_kernel_alone(K) if wl.hyper.max_grad_norm > 0 else ms_per_step
+    off_ms = rig.time_steps_off(min(K, 50))
     peak, peak_src = measured_peaks()
-    achieved = BYTES_PER_ELEM * N / (kern_ms * 1e-3) / 1e9
+    achieved = BPE * N / (kern_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": committed_traffic(args.config), "peak_source": peak_src,
-                "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS, "kernel": "phx::k_step8<1,1,true>",
-                "kernel_ms": kern_ms, "algorithmic_bytes_per_launch": BYTES_PER_ELEM * N}
+                "traffic": committed_traffic(args.config if rig.source_name == "staged" else args.config + "-direct"),
+                "peak_source": peak_src, "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS,
+                "kernel": "phx::k_step8<1,1,%s>" % ("true" if rig.source_name == "staged" else "false"),
+                "kernel_ms": kern_ms, "algorithmic_bytes_per_launch": BPE * N, "bytes_per_element": BPE,
+                "snapshot_off_step_ms": off_ms,
+                "snapshot_off_gbs": BYTES_PER_ELEM_OFF * N / (off_ms * 1e-3) / 1e9}
 
-    # ---- e2e: host buffers in, host replica out, through the same C-ABI calls ------------------------
-    Ke = args.e2e_steps
-    def e2e_loop(k_steps):
-        nonlocal step
-        for _ in range(k_steps):
-            step += 1
-            g = grads[step & 1]
-            g.copy_(hgrads[step & 1], non_blocking=True)          # H2D of this step's inputs
-            s.step_and_snapshot(g, step)
-            s.flush_async(side)                                   # D2H of this step's result (a4 + a5)
-        s.wait(step)
-    e2e_loop(2)
-    torch.cuda.synchronize()
-    barrier(world)
-    t0 = time.perf_counter()
-    e2e_loop(Ke)
-    torch.cuda.synchronize()
-    barrier(world)
-    e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3 / Ke, world, device)
-    e2e_val = BYTES_PER_ELEM * units / (e2e_ms * 1e-3) / 1e9
-    d2h_bytes = int(s.info.snapshot_bytes)
-    e2e = {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(2 * N), "d2h_bytes_per_step": d2h_bytes,
-           "ms_per_step": e2e_ms, "steps": Ke,
+    # ---- e2e -----------------------------------------------------------------------------------------
+    e2e_ms = max_over_ranks(rig.e2e(args.e2e_steps, world), world, device)
+    d2h_bytes = int(rig.s.info.snapshot_bytes)
+    e2e = {"value": BPE * units / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
+           "h2d_bytes_per_step": int(2 * N), "d2h_bytes_per_step": d2h_bytes, "ms_per_step": e2e_ms,
+           "steps": args.e2e_steps,
            "note": "H2D grads from pinned host + fused step + chunked D2H of the packed snapshot + commit, per step"}
 
-    # flush alone (a4+a5) against the measured pinned-copy peak
-    host_link = None
+    host_link = overlap = restore = cpu = None
     if rank == 0:
-        step += 1
-        s.step_and_snapshot(grads[step & 1], step)
-        torch.cuda.synchronize()
-        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        f0.record(side)
-        s.flush_async(side)
-        f1.record(side)
-        s.wait(step)
-        torch.cuda.synchronize()
-        flush_ms = f0.elapsed_time(f1)
+        # flush alone (a4+a5) against the measured pinned-copy peak
+        flush_ms = rig.time_flush()
         ach = d2h_bytes / (flush_ms * 1e-3) / 1e9
         host_link = {"bound": "host_link", "achieved": ach, "peak": link["d2h_gbs"], "unit": "GB/s",
-                     "frac": ach / link["d2h_gbs"], "flush_ms": flush_ms, "chunk_mib": args.chunk_mib,
+                     "frac": ach / link["d2h_gbs"], "flush_ms": flush_ms, "chunk_mib": rig.chunk_mib,
                      "h2d_peak_gbs": link["h2d_gbs"]}
-
-    # ---- overlap: exposed checkpoint ms/iteration (PAPER.md:283 protocol) -----------------------------
-    overlap = None
-    if not args.no_overlap and rank == 0:
-        overlap = measure_overlap(torch, B, W, Shard, s, wl, grads, args, device, side, step,
-                                  host_link["flush_ms"])
-        step = overlap.pop("_step")
-
-    # ---- restore + recompute (a6, a7) -------------------------------------------------------------------
-    restore = None
-    if rank == 0:
-        torch.cuda.synchronize()          # every flush issued so far has been waited for above
-        s.drop_live()
-        torch.cuda.synchronize()
-        r0, r1, r2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
-        r0.record(cur)
-        back = s.restore()
-        r1.record(cur)
-        s.step_and_snapshot(grads[(back + 1) & 1], back + 1)
-        r2.record(cur)
-        torch.cuda.synchronize()
-        rms = r0.elapsed_time(r1)
-        restore = {"restore_ms": rms, "recompute_ms": r1.elapsed_time(r2), "mode": "bulk_kernel",
+        # overlap: exposed checkpoint ms/iteration (PAPER.md:283 protocol)
+        if not args.no_overlap:
+            G = args.gemms if args.gemms > 0 else rig.headline_gemms(flush_ms)
+            overlap = rig.overlap(G, args.overlap_iters, args.overlap_reps)
+            overlap["flush_ms"] = flush_ms
+            overlap["rule"] = "G = smallest power of two with T_c >= 4 x T_D2H" if args.gemms <= 0 else "G given"
+        # restore + recompute (a6, a7)
+        back, rms, cms = rig.restore_timing()
+        restore = {"restore_ms": rms, "recompute_ms": cms, "mode": rig.restore_mode_name, "restored_step": back,
                    "host_link_gbs": 12 * N / (rms * 1e-3) / 1e9,
                    "frac_of_h2d_peak": 12 * N / (rms * 1e-3) / 1e9 / link["h2d_gbs"]}
-
-    # ---- cpu baseline: the oracle on the host cores (rank 0, N == 1 only) ------------------------------
-    cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cores = len(os.sched_getaffinity(0))
-        sample = args.cpu_sample or min(N, 1 << 28)
-        n_s, times = time_oracle(wl, sample, 3, 1, cores)
-        t = sum(times) / len(times)
-        n_1, times1 = time_oracle(wl, min(sample, 1 << 25), 2, 1, 1)
-        t1 = sum(times1) / len(times1)
-        cpu = {"value": BYTES_PER_ELEM * n_s / t / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"first {n_s} of {N} elements of the shard, 3 steps after 1 warm-up",
-               "elements_per_s": n_s / t, "single_thread_elements_per_s": n_1 / t1}
-
-    if rank == 0:
+        # cpu baseline: the oracle on the host cores (rank 0, N == 1 only)
+        if world == 1 and not args.no_cpu_baseline:
+            cores = len(os.sched_getaffinity(0))
+            sample = args.cpu_sample or min(N, 1 << 28)
+            n_s, times = time_oracle(wl, sample, 3, 1, cores)
+            t = sum(times) / len(times)
+            n_1, times1 = time_oracle(wl, min(sample, 1 << 25), 2, 1, 1)
+            t1 = sum(times1) / len(times1)
+            cpu = {"value": BYTES_PER_ELEM * n_s / t / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+                   "sample": f"first {n_s} of {N} elements of the shard, 3 steps after 1 warm-up",
+                   "elements_per_s": n_s / t, "single_thread_elements_per_s": n_1 / t1}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{wl.key}: {wl.title}", "elements_per_shard": int(N),
-                       "state_bytes": int(12 * N), "staging_depth": args.depth, "chunk_mib": args.chunk_mib,
-                       "sync_mode": args.sync, "kernel_variant": args.variant,
+                       "state_bytes": int(12 * N), "staging_depth": rig.depth, "chunk_mib": rig.chunk_mib,
+                       "sync_mode": rig.sync_name, "kernel_variant": args.variant, "snapshot_source": rig.source_name,
+                       "bytes_per_element": BPE,
                        "l2": "inputs larger than L2 (working set %.2f GB per step >> 126 MB)" % (BYTES_PER_ELEM * N / 1e9),
                        "timed_region": "K x phx_step_and_snapshot (a1 clip if configured, a2 sync-point wait, a3 fused "
                                        "AdamW+bf16 copy+packed snapshot); a4/a5 host flush is in e2e and overlap",
@@ -460,90 +639,205 @@ def run_phx(args):
             "step_ms_min_max": [min(per), max(per)],
         }
         print(json.dumps(line), flush=True)
-    s.close()
+    rig.close()
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
     return 0
 
 
-def measure_overlap(torch, B, W, Shard, s_on, wl, grads, args, device, side, step, flush_ms):
-    """Iterations of G GEMMs + hot path (snapshot on, flush on the side stream) versus the same
-    loop with the snapshot-off kernel and no flush; per-iteration times from CUDA events on the
-    compute stream; trimmed means per PAPER.md:283."""
-    cur = torch.cuda.current_stream(device)
-    a = torch.randn(4096, 4096, device=device, dtype=torch.bfloat16)
-    b = torch.randn(4096, 4096, device=device, dtype=torch.bfloat16)
-    c = torch.empty(4096, 4096, device=device, dtype=torch.bfloat16)
-    for _ in range(20):
-        torch.matmul(a, b, out=c)
-    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    g0.record(cur)
-    for _ in range(200):
-        torch.matmul(a, b, out=c)
-    g1.record(cur)
-    torch.cuda.synchronize()
-    gemm_ms = g0.elapsed_time(g1) / 200
-    G = args.gemms
-    if G <= 0:
-        G = 64
-        while G * gemm_ms < 4.0 * flush_ms:      # headline rule: smallest power of two with T_c >= 4 T_D2H
-            G *= 2
-    iters, warm = args.overlap_iters, 3
+# ----------------------------------------------------------------------------------------------
+# the other measurement rows of SURVEY.md §8(d): one JSON line per measurement
+# ----------------------------------------------------------------------------------------------
 
-    s_off = Shard(wl, device=device, snapshot=False)
-    s_off.p.copy_(s_on.p)
-    s_off.set_state(0)
 
-    def loop(shard, flush, first_step):
-        st = first_step
-        evs = []
-        kevs = []
-        for it in range(warm + iters):
-            e0 = torch.cuda.Event(enable_timing=True)
-            e0.record(cur)
-            for _ in range(G):
-                torch.matmul(a, b, out=c)
-            k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            k0.record(cur)
-            st += 1
-            shard.step_and_snapshot(grads[st & 1], st)
-            k1.record(cur)
-            if flush:
-                shard.flush_async(side)
-            evs.append(e0)
-            kevs.append((k0, k1))
-        end = torch.cuda.Event(enable_timing=True)
-        end.record(cur)
+def emit(**kw):
+    print(json.dumps(kw), flush=True)
+
+
+def run_configs(args):
+    """Every config's kernel, snapshot-off kernel, clip pass, flush, both restore modes."""
+    torch, rank, world, local_rank = gpu_setup()
+    keys = [args.config] if args.config != "c2" else ["c1", "c2", "c3", "c4a", "c4b", "c5"]
+    link = measure_host_link(torch, torch.device(f"cuda:{local_rank}"))
+    peak, _ = measured_peaks()
+    for key in keys:
+        rig = Rig(args, key, host_grads=False)
+        N = rig.N
+        total_ms, per, _ = rig.time_steps(args.steps, max(args.warmup, 3))
+        step_ms = total_ms / args.steps
+        kern_ms = rig.time_fused_kernel_alone(args.steps) if rig.wl.hyper.max_grad_norm > 0 else step_ms
+        off_ms = rig.time_steps_off(args.steps)
+        flush_ms = rig.time_flush()
+        _, r_bulk, rec = rig.restore_timing()
+        B = rig.B
+        replica, back_step = rig.s.replica, rig.step
+        rig.close()
+        # copy-engine restore on a fresh handle bound to the same replica (a replacement rank)
+        r2 = rig.Shard(rig.wl, device=rig.device, restore_mode=B.PHX_RESTORE_COPY_ENGINE, replica=replica)
         torch.cuda.synchronize()
-        evs.append(end)
-        it_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(warm, warm + iters)]
-        k_ms = [x.elapsed_time(y) for x, y in kevs[warm:]]
-        return st, it_ms, k_ms
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        r2.restore()
+        e1.record()
+        torch.cuda.synchronize()
+        r_ce = e0.elapsed_time(e1)
+        r2.close()
+        gbs = BYTES_PER_ELEM * N / (kern_ms * 1e-3) / 1e9
+        emit(mode="configs", config=key, elements=int(N), step_ms=step_ms, fused_kernel_ms=kern_ms,
+             fused_gbs=gbs, frac_of_measured_peak=gbs / peak, frac_of_nominal=gbs / NOMINAL_HBM_GBS,
+             elements_per_s=N / (step_ms * 1e-3), snapshot_off_step_ms=off_ms,
+             snapshot_extra_ms=step_ms - off_ms, flush_ms=flush_ms,
+             flush_gbs=rig_bytes(N) / (flush_ms * 1e-3) / 1e9, d2h_peak_gbs=link["d2h_gbs"],
+             restore_bulk_ms=r_bulk, restore_bulk_gbs=12 * N / (r_bulk * 1e-3) / 1e9,
+             restore_copy_engine_ms=r_ce, restore_copy_engine_gbs=12 * N / (r_ce * 1e-3) / 1e9,
+             h2d_peak_gbs=link["h2d_gbs"], recompute_ms=rec,
+             note="c1 fits in L2: reported, not an HBM figure" if key == "c1" else "")
+        del rig, r2, replica
+        torch.cuda.empty_cache()
+    return 0
 
-    # interleave on/off/on/off halves to average out slow clock drift
-    step, on1, kon1 = loop(s_on, True, step)
-    _, off1, koff1 = loop(s_off, False, 0)
-    s_on.wait(step)
-    on, off, kon, koff = on1, off1, kon1, koff1
-    t_on, t_off = trimmed_mean(on), trimmed_mean(off)
-    out = {
-        "gemms_per_iter": G, "gemm_ms": gemm_ms, "compute_window_ms": G * gemm_ms, "iters": iters,
-        "iter_ms_snapshot_on": t_on, "iter_ms_snapshot_off": t_off, "exposed_ms": t_on - t_off,
-        "exposed_frac_of_compute_step": (t_on - t_off) / t_off,
-        "hot_path_ms_in_loop_on": trimmed_mean(kon), "hot_path_ms_in_loop_off": trimmed_mean(koff),
-        "flush_ms": flush_ms, "protocol": "PAPER.md:283: warm-up dropped, slowest 5% dropped, mean of the rest",
-        "_step": step,
-    }
-    s_off.close()
-    return out
+
+def rig_bytes(N):
+    return 256 + 12 * N
+
+
+def run_overlap_curve(args):
+    """Exposed checkpoint ms/iteration against the length of the compute window (R21)."""
+    torch, rank, world, local_rank = gpu_setup()
+    rig = Rig(args, args.config, host_grads=False)
+    flush_ms = rig.time_flush()
+    gm = rig.gemm_setup()
+    Gs = [int(x) for x in str(args.gemms).split(",")] if args.gemms > 0 else [64, 256, 1024, 4096, 16384]
+    head = rig.headline_gemms(flush_ms)
+    for G in sorted(set(Gs + [head])):
+        t_iter = G * gm * 1.2 + 1.0
+        iters = max(5, min(20, int(3000.0 / t_iter)))
+        o = rig.overlap(G, iters, args.overlap_reps)
+        emit(mode="overlap-curve", config=args.config, elements=int(rig.N), flush_ms=flush_ms, headline=(G == head),
+             knee_gemms=flush_ms / gm, sync_mode=rig.sync_name, depth=rig.depth, chunk_mib=rig.chunk_mib, **o)
+    rig.close()
+    return 0
+
+
+def run_sweep(args):
+    """BASELINE.json:configs[4]: D2H chunk size 4..256 MiB x staging depth 1..4 (x sync mode), reporting exposed
+    checkpoint ms/iteration and host-link GB/s.  Run at a TIGHT compute window (T_c = 1.25 x T_D2H, where depth and
+    chunking can matter) and, on a reduced grid, at the headline window (T_c >= 4 x T_D2H)."""
+    torch, rank, world, local_rank = gpu_setup()
+    key = args.config if args.config != "c2" else "c5"
+    device = torch.device(f"cuda:{local_rank}")
+    link = measure_host_link(torch, device)
+    probe = Rig(args, key, host_grads=False)
+    replica = probe.s.replica                        # pin once, reuse for every grid point
+    flush_ref = probe.time_flush()
+    gm = probe.gemm_setup()
+    G_tight = max(1, int(round(1.25 * flush_ref / gm)))
+    G_head = probe.headline_gemms(flush_ref)
+    base = probe.overlap(G_tight, args.overlap_iters, 1, arms=("off",))
+    base_head = probe.overlap(G_head, max(5, args.overlap_iters // 2), 1, arms=("off",))
+    probe.close()
+    del probe
+    torch.cuda.empty_cache()
+    chunks = [int(x) for x in args.chunks.split(",")]
+    for sync in args.syncs.split(","):
+        for depth in [int(x) for x in args.depths.split(",")]:
+            for chunk in chunks:
+                rig = Rig(args, key, depth=depth, chunk_mib=chunk, sync=sync, replica=replica, host_grads=False)
+                flush_ms = rig.time_flush()
+                o = rig.overlap(G_tight, args.overlap_iters, 1, arms=("on",))
+                row = dict(mode="sweep", window="tight(1.25xT_D2H)", config=key, elements=int(rig.N), sync_mode=sync,
+                           depth=depth, chunk_mib=chunk, flush_ms=flush_ms,
+                           host_link_gbs=rig_bytes(rig.N) / (flush_ms * 1e-3) / 1e9, d2h_peak_gbs=link["d2h_gbs"],
+                           gemms_per_iter=G_tight, iter_ms_on=o["iter_ms_on"], iter_ms_off=base["iter_ms_off"],
+                           exposed_ms=o["iter_ms_on"] - base["iter_ms_off"],
+                           exposed_frac=(o["iter_ms_on"] - base["iter_ms_off"]) / base["iter_ms_off"],
+                           hot_path_ms_in_loop_on=o["hot_path_ms_in_loop_on"])
+                emit(**row)
+                if depth in (1, 2) and chunk in (chunks[0], 64, 256):
+                    o = rig.overlap(G_head, max(5, args.overlap_iters // 2), 1, arms=("on",))
+                    emit(mode="sweep", window="headline(>=4xT_D2H)", config=key, elements=int(rig.N), sync_mode=sync,
+                         depth=depth, chunk_mib=chunk, flush_ms=flush_ms, gemms_per_iter=G_head,
+                         iter_ms_on=o["iter_ms_on"], iter_ms_off=base_head["iter_ms_off"],
+                         exposed_ms=o["iter_ms_on"] - base_head["iter_ms_off"],
+                         exposed_frac=(o["iter_ms_on"] - base_head["iter_ms_off"]) / base_head["iter_ms_off"],
+                         hot_path_ms_in_loop_on=o["hot_path_ms_in_loop_on"])
+                rig.close()
+                del rig
+                torch.cuda.empty_cache()
+    return 0
+
+
+def run_hotswap(args):
+    """BASELINE.json:configs[3]: 20 steps with snapshots, drop the live shard while step 21 is in flight, restore
+    from the pinned host replica, recompute step 21, run 22..25; time restore + recompute and check the trajectory
+    bit-exactly against an uninterrupted run (GPU vs GPU; GPU vs oracle is in tests/)."""
+    torch, rank, world, local_rank = gpu_setup()
+    keys = [args.config] if args.config != "c2" else ["c4a", "c4b"]
+    for key in keys:
+        for rmode_name in ("bulk_kernel", "copy_engine"):
+            from paper_2607_01646_b200 import binding as B
+            rmode = B.PHX_RESTORE_BULK_KERNEL if rmode_name == "bulk_kernel" else B.PHX_RESTORE_COPY_ENGINE
+            rig = Rig(args, key, host_grads=False, restore_mode=rmode)
+            W, wl, N = rig.W, rig.wl, rig.N
+            G = rig.headline_gemms(rig.time_flush(), factor=1.25)
+            rig.s.p.copy_(W.init_params(rig.s.n, N, wl.seed, device=rig.device))
+            rig.s.m.zero_(); rig.s.v.zero_()
+            rig.s.set_state(0)
+            rig.step = 0
+            a, b, c = rig._gemm
+            # uninterrupted reference trajectory first (snapshot-off handle on its own arrays)
+            ref = rig.Shard(wl, device=rig.device, snapshot=False)
+            ref.p.copy_(rig.s.p); ref.set_state(0)
+            for t in range(1, 26):
+                ref.step_and_snapshot(rig.grads[t & 1], t)
+            torch.cuda.synchronize()
+            for t in range(1, 21):                       # 20 steps, snapshot + flush every step, overlapped
+                for _ in range(G):
+                    torch.matmul(a, b, out=c)
+                rig.do_step()
+                rig.s.flush_async(rig.side)
+            rig.do_step()                                # step 21 launched: in flight when the fault hits
+            torch.cuda.synchronize()
+            rig.s.drop_live()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            r0, r1, r2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            r0.record(rig.cur)
+            back = rig.s.restore()
+            r1.record(rig.cur)
+            rig.step = back
+            rig.do_step()                                # recompute of the in-flight step (a7)
+            r2.record(rig.cur)
+            torch.cuda.synchronize()
+            wall_ms = (time.perf_counter() - t0) * 1e3
+            for t in range(22, 26):
+                rig.do_step()
+                rig.s.flush_async(rig.side)
+            rig.s.wait(25)
+            torch.cuda.synchronize()
+            same = all(torch.equal(x, y) for x, y in ((rig.s.p, ref.p), (rig.s.m, ref.m), (rig.s.v, ref.v),
+                                                      (rig.s.p16, ref.p16)))
+            rms = r0.elapsed_time(r1)
+            emit(mode="hotswap", config=key, elements=int(N), restore_mode=rmode_name, restored_step=int(back),
+                 restore_ms=rms, recompute_ms=r1.elapsed_time(r2), restore_plus_recompute_wall_ms=wall_ms,
+                 host_link_gbs=12 * N / (rms * 1e-3) / 1e9, trajectory_bit_exact_vs_uninterrupted=bool(same),
+                 steps_before_fault=20, steps_after=5, gemms_per_iter=G)
+            ref.close()
+            rig.close()
+            del rig, ref
+            torch.cuda.empty_cache()
+            if not same:
+                return 1
+    return 0
 
 
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
-    return run_phx(args)
+    return {"headline": run_headline, "configs": run_configs, "overlap-curve": run_overlap_curve,
+            "sweep": run_sweep, "hotswap": run_hotswap}[args.mode](args)
 
 
 if __name__ == "__main__":

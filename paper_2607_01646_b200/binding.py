@@ -32,7 +32,8 @@ PHX_ERR_SNAPSHOT_DISABLED = -11
 PHX_ERR_NOMEM = -12
 
 PHX_SYNC_STRICT, PHX_SYNC_RELAXED = 0, 1
-PHX_RESTORE_BULK_KERNEL, PHX_RESTORE_COPY_ENGINE = 0, 1
+PHX_RESTORE_COPY_ENGINE, PHX_RESTORE_BULK_KERNEL = 0, 1
+PHX_SNAPSHOT_STAGED, PHX_SNAPSHOT_DIRECT = 0, 1
 
 
 class phx_tensor_desc_t(C.Structure):
@@ -44,7 +45,7 @@ class phx_config_t(C.Structure):
                 ("pp_rank", C.c_uint32), ("staging_depth", C.c_uint32), ("sync_mode", C.c_uint32),
                 ("chunk_bytes", C.c_uint64), ("snapshot_disabled", C.c_uint32),
                 ("restore_mode", C.c_uint32), ("max_grad_norm", C.c_float),
-                ("reserved", C.c_uint32 * 5)]
+                ("snapshot_source", C.c_uint32), ("reserved", C.c_uint32 * 4)]
 
 
 class phx_shard_info_t(C.Structure):
@@ -133,8 +134,9 @@ def _ptr(x) -> int:
 
 def phx_shard_create(layout: Sequence[Tuple[int, int]], dp_size: int, dp_rank: int, *, tp=(1, 0),
                      pp=(1, 0), staging_depth=0, sync_mode=PHX_SYNC_STRICT, chunk_bytes=0,
-                     snapshot_disabled=False, restore_mode=PHX_RESTORE_BULK_KERNEL,
-                     max_grad_norm=0.0, flags: Optional[Sequence[int]] = None) -> int:
+                     snapshot_disabled=False, restore_mode=PHX_RESTORE_COPY_ENGINE,
+                     max_grad_norm=0.0, snapshot_source=PHX_SNAPSHOT_STAGED,
+                     flags: Optional[Sequence[int]] = None) -> int:
     """layout = [(numel, tensor_id)] in flattening order.  Returns the opaque handle."""
     n = len(layout)
     arr = (phx_tensor_desc_t * max(n, 1))()
@@ -144,7 +146,7 @@ def phx_shard_create(layout: Sequence[Tuple[int, int]], dp_size: int, dp_rank: i
     cfg = phx_config_t(tp_size=tp[0], tp_rank=tp[1], pp_size=pp[0], pp_rank=pp[1],
                        staging_depth=staging_depth, sync_mode=sync_mode, chunk_bytes=chunk_bytes,
                        snapshot_disabled=1 if snapshot_disabled else 0, restore_mode=restore_mode,
-                       max_grad_norm=max_grad_norm)
+                       max_grad_norm=max_grad_norm, snapshot_source=snapshot_source)
     h = C.c_void_p()
     _ck(lib().phx_shard_create(arr, n, dp_size, dp_rank, C.byref(cfg), C.byref(h)), "phx_shard_create")
     return h.value

@@ -34,7 +34,8 @@ constexpr size_t kScrOne = 256;        // float 1.0f: clip coefficient when clip
 constexpr size_t kScrCoef = 260;       // float: clip coefficient of the current step
 constexpr size_t kScrSumsq = 264;      // double
 constexpr size_t kScrPartials = 512;   // kSumsqMaxBlocks doubles
-constexpr size_t kScrBytes = kScrPartials + phx::kSumsqMaxBlocks * sizeof(double);
+constexpr size_t kScrHdr = kScrPartials + phx::kSumsqMaxBlocks * sizeof(double);  // 2 x 256 B headers (direct mode)
+constexpr size_t kScrBytes = kScrHdr + 2 * 256;
 
 uint64_t fnv1a64(const void *data, size_t len, uint64_t h = 0xCBF29CE484222325ull)
 {
@@ -154,6 +155,9 @@ bool header_matches(const phx_shard *s, const phx_snapshot_header_t *h)
 }
 
 bool snapshots_on(const phx_shard *s) { return s->cfg.snapshot_disabled == 0; }
+bool direct_mode(const phx_shard *s) { return s->cfg.snapshot_source == PHX_SNAPSHOT_DIRECT; }
+// number of ring positions the bookkeeping cycles through (direct mode: two header slots)
+uint32_t ring_depth(const phx_shard *s) { return direct_mode(s) ? 2u : s->cfg.staging_depth; }
 
 // settle the bookkeeping of host slots whose flush event has completed (block=true waits for it)
 int settle_host_slots(phx_shard *s, bool block)
@@ -214,10 +218,12 @@ int phx_shard_create(const phx_tensor_desc_t *layout, size_t n_tensors, uint32_t
     if (c.tp_size == 0) c.tp_size = 1;
     if (c.pp_size == 0) c.pp_size = 1;
     if (c.staging_depth == 0) c.staging_depth = 2;
-    if (c.chunk_bytes == 0) c.chunk_bytes = 64ull << 20;
+    if (c.chunk_bytes == 0) c.chunk_bytes = 8ull << 20;
     c.chunk_bytes = (c.chunk_bytes + 255) & ~255ull;
     if (c.tp_rank >= c.tp_size || c.pp_rank >= c.pp_size || c.staging_depth > kMaxDepth ||
-        c.sync_mode > PHX_SYNC_RELAXED || c.restore_mode > PHX_RESTORE_COPY_ENGINE || !(c.max_grad_norm == c.max_grad_norm)) {
+        c.sync_mode > PHX_SYNC_RELAXED || c.restore_mode > PHX_RESTORE_BULK_KERNEL || !(c.max_grad_norm == c.max_grad_norm) ||
+        c.snapshot_source > PHX_SNAPSHOT_DIRECT ||
+        (c.snapshot_source == PHX_SNAPSHOT_DIRECT && c.sync_mode != PHX_SYNC_STRICT)) {
         delete s;
         return PHX_ERR_INVALID_ARG;
     }
@@ -259,7 +265,7 @@ int phx_shard_create(const phx_tensor_desc_t *layout, size_t n_tensors, uint32_t
     i.snapshot_bytes = kHeaderBytes + 12 * L;
     i.slot_stride = (i.snapshot_bytes + 255) & ~255ull;
     i.n_segments = (uint32_t)s->segments.size();
-    i.staging_depth = c.staging_depth;
+    i.staging_depth = c.snapshot_source == PHX_SNAPSHOT_DIRECT ? 0 : c.staging_depth;
     i.dp_size = dp_size;
     i.dp_rank = dp_rank;
     *out = s;
@@ -308,7 +314,7 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
                    void *h_replica)
 {
     if (!s || !d_p || !d_m || !d_v || !d_p_bf16) return PHX_ERR_INVALID_ARG;
-    if (snapshots_on(s) && (!d_staging || !h_replica)) return PHX_ERR_INVALID_ARG;
+    if (snapshots_on(s) && (!h_replica || (!d_staging && !direct_mode(s)))) return PHX_ERR_INVALID_ARG;
     if (!aligned256(d_p) || !aligned256(d_m) || !aligned256(d_v) || !aligned256(d_p_bf16) || !aligned256(d_staging) ||
         !aligned256(h_replica))
         return PHX_ERR_ALIGNMENT;
@@ -335,7 +341,7 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
     const float one = 1.0f;
     PHX_CK(cudaMemcpy(s->d_scratch + kScrOne, &one, 4, cudaMemcpyHostToDevice));
     PHX_CK(cudaMemcpy(s->d_scratch + kScrCoef, &one, 4, cudaMemcpyHostToDevice));
-    for (uint32_t k = 0; k < s->cfg.staging_depth; ++k) {
+    for (uint32_t k = 0; k < ring_depth(s); ++k) {
         PHX_CK(cudaEventCreateWithFlags(&s->ev_step[k], cudaEventDisableTiming));
         PHX_CK(cudaEventCreateWithFlags(&s->ev_flush[k], cudaEventDisableTiming));
     }
@@ -411,18 +417,22 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads_bf16, float lr, fl
 
     int slot = -1;
     if (snap) {
-        slot = (int)(step % s->cfg.staging_depth);
+        slot = (int)(step % ring_depth(s));
         // a2: the single sync point — stream-side wait, the host never blocks
         if (s->cfg.sync_mode == PHX_SYNC_STRICT) {
             if (s->last_flush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[s->last_flush_slot], 0));
         } else if (s->flush_valid[slot]) {
             PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[slot], 0));
         }
-        uint8_t *base = s->d_staging + (uint64_t)slot * s->info.slot_stride;
-        a.shdr = base;
-        a.sp = reinterpret_cast<float *>(base + kHeaderBytes);
-        a.sm = a.sp + s->info.n_padded;
-        a.sv = a.sm + s->info.n_padded;
+        if (direct_mode(s)) {
+            a.shdr = s->d_scratch + kScrHdr + (size_t)slot * kHeaderBytes;  // header only; planes stay live
+        } else {
+            uint8_t *base = s->d_staging + (uint64_t)slot * s->info.slot_stride;
+            a.shdr = base;
+            a.sp = reinterpret_cast<float *>(base + kHeaderBytes);
+            a.sm = a.sp + s->info.n_padded;
+            a.sv = a.sm + s->info.n_padded;
+        }
         phx_snapshot_header_t hdr;
         build_header(s, step, true, &hdr);
         std::memcpy(&a.hdr, &hdr, sizeof(hdr));
@@ -435,7 +445,7 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads_bf16, float lr, fl
     a.n_padded = s->info.n_padded;
 
     // a3: one kernel, one pass
-    PHX_CK(phx::launch_step(a, snap, s->variant, st));
+    PHX_CK(phx::launch_step(a, snap && !direct_mode(s), s->variant, st));
     s->launches += s->info.n_padded ? 1 : 0;
     if (snap) {
         PHX_CK(cudaEventRecord(s->ev_step[slot], st));
@@ -457,7 +467,9 @@ int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream)
     const int slot = s->pending_slot;
     const uint64_t step = s->pending_step;
     const int hs = (int)(step & 1);  // ping-pong
-    const uint8_t *src = s->d_staging + (uint64_t)slot * s->info.slot_stride;
+    const bool direct = direct_mode(s);
+    const uint8_t *src = direct ? nullptr : s->d_staging + (uint64_t)slot * s->info.slot_stride;
+    const uint8_t *src_hdr = direct ? s->d_scratch + kScrHdr + (size_t)slot * kHeaderBytes : src;
     uint8_t *dst = s->h_replica + (uint64_t)hs * s->info.slot_stride;
 
     PHX_CK(cudaStreamWaitEvent(st, s->ev_step[slot], 0));  // the step's kernel has written the slot
@@ -476,10 +488,26 @@ int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream)
     for (uint64_t off = 0; off < payload; off += chunk, ++done_chunks) {
         if (torn && (int64_t)done_chunks >= s->torn_chunks) break;
         const uint64_t len = payload - off < chunk ? payload - off : chunk;
-        PHX_CK(cudaMemcpyAsync(dst + kHeaderBytes + off, src + kHeaderBytes + off, len, cudaMemcpyDeviceToHost, st));
+        if (!direct) {
+            PHX_CK(cudaMemcpyAsync(dst + kHeaderBytes + off, src + kHeaderBytes + off, len, cudaMemcpyDeviceToHost, st));
+        } else {
+            // the chunk [off, off+len) of the packed payload p ‖ m ‖ v comes straight from the live planes;
+            // a chunk that straddles a plane boundary is split there
+            const uint64_t plane = 4 * s->info.n_padded;
+            const uint8_t *planes[3] = {reinterpret_cast<const uint8_t *>(s->d_p), reinterpret_cast<const uint8_t *>(s->d_m),
+                                        reinterpret_cast<const uint8_t *>(s->d_v)};
+            uint64_t o = off, left = len;
+            while (left) {
+                const uint64_t pi = o / plane, po = o % plane;
+                const uint64_t l = left < plane - po ? left : plane - po;
+                PHX_CK(cudaMemcpyAsync(dst + kHeaderBytes + o, planes[pi] + po, l, cudaMemcpyDeviceToHost, st));
+                o += l;
+                left -= l;
+            }
+        }
     }
     // 3. commit: the valid header (seq_end == seq_begin) lands last
-    if (!torn) PHX_CK(cudaMemcpyAsync(dst, src, kHeaderBytes, cudaMemcpyDeviceToHost, st));
+    if (!torn) PHX_CK(cudaMemcpyAsync(dst, src_hdr, kHeaderBytes, cudaMemcpyDeviceToHost, st));
     PHX_CK(cudaEventRecord(s->ev_flush[slot], st));
     PHX_CK(cudaEventRecord(s->ev_host[hs], st));
     s->flush_valid[slot] = true;

@@ -152,6 +152,54 @@ __device__ __forceinline__ void adamw_element(float &p, float &m, float &v, floa
 }
 
 // ------------------------------------------------------------------------------------------
+// 1-D bulk async copy (TMA) + mbarrier helpers (shared by the TMA step kernel and the restore kernel)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {  // try_wait suspends the thread in hardware for a bounded time; loop until the phase flips
+        asm volatile(
+            "{\n"
+            ".reg .pred P1;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, P1;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void *gdst, const void *smem_src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+__device__ __forceinline__ void bulk_wait_read1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
+// make this thread's generic-proxy shared-memory writes visible to the async proxy (bulk stores)
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// ------------------------------------------------------------------------------------------
 // a3: fused step + snapshot, 8 elements per thread-group, 256-bit vectors
 // ------------------------------------------------------------------------------------------
 constexpr int kStepThreads = 256;
@@ -161,7 +209,7 @@ __global__ void __launch_bounds__(kStepThreads) k_step8(const __grid_constant__ 
 {
     const uint64_t ngroups = a.n_padded >> 3;
     const uint64_t base = (uint64_t)blockIdx.x * (kStepThreads * U) + threadIdx.x;
-    if (SNAP && blockIdx.x == 0 && threadIdx.x < 16)
+    if (a.shdr != nullptr && blockIdx.x == 0 && threadIdx.x < 16)
         reinterpret_cast<uint4 *>(a.shdr)[threadIdx.x] = a.hdr.q[threadIdx.x];
     const float coef = __ldg(a.coef);
 
@@ -213,7 +261,7 @@ __global__ void __launch_bounds__(kStepThreads) k_step4(const __grid_constant__ 
 {
     const uint64_t ngroups = a.n_padded >> 2;
     const uint64_t base = (uint64_t)blockIdx.x * (kStepThreads * U) + threadIdx.x;
-    if (SNAP && blockIdx.x == 0 && threadIdx.x < 16)
+    if (a.shdr != nullptr && blockIdx.x == 0 && threadIdx.x < 16)
         reinterpret_cast<uint4 *>(a.shdr)[threadIdx.x] = a.hdr.q[threadIdx.x];
     const float coef = __ldg(a.coef);
 
@@ -280,6 +328,144 @@ static cudaError_t launch4(const StepArgs &a, bool snapshot, cudaStream_t st)
     return cudaGetLastError();
 }
 
+
+// ------------------------------------------------------------------------------------------
+// a3, TMA flavour: persistent CTAs, STAGES shared-memory stages of one TT-element tile each.
+//   producer (thread 0): cp.async.bulk loads of the p, m, v, g tiles, completion on an mbarrier;
+//   all threads: canonical AdamW in place in shared memory (conflict-free 128-bit accesses),
+//                bf16 copy into the stage's h tile;
+//   thread 0: cp.async.bulk stores of the SAME shared tiles to the live planes AND to the staging
+//             planes — the snapshot costs no extra SM instruction at all, only the extra bulk store.
+// ------------------------------------------------------------------------------------------
+template <int TT>
+struct alignas(128) StepTile {
+    float p[TT], m[TT], v[TT];
+    uint16_t g[TT], h[TT];
+};
+
+template <int TT, int STAGES, bool SNAP>
+__global__ void __launch_bounds__(kStepThreads) k_step_tma(const __grid_constant__ StepArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    StepTile<TT> *tiles = reinterpret_cast<StepTile<TT> *>(smem_raw);
+    __shared__ __align__(8) uint64_t full[STAGES];
+    constexpr int kHalves = TT / (kStepThreads * 4);
+
+    const uint64_t N = a.n_padded;
+    const uint64_t ntiles = (N + TT - 1) / TT;
+    const uint64_t first = blockIdx.x, stride = gridDim.x;
+    const uint64_t my_count = first < ntiles ? (ntiles - first + stride - 1) / stride : 0;
+
+    if (a.shdr != nullptr && blockIdx.x == 0 && threadIdx.x < 16)
+        reinterpret_cast<uint4 *>(a.shdr)[threadIdx.x] = a.hdr.q[threadIdx.x];
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const float coef = __ldg(a.coef);
+    const uint16_t *g16 = reinterpret_cast<const uint16_t *>(a.g);
+    uint16_t *p16 = reinterpret_cast<uint16_t *>(a.p16);
+
+    auto tile_cnt = [&](uint64_t it) -> uint32_t {
+        const uint64_t e0 = (first + it * stride) * TT;
+        return (uint32_t)((N - e0) < (uint64_t)TT ? (N - e0) : TT);
+    };
+    auto issue_loads = [&](uint64_t it) {  // thread 0
+        const int s = (int)(it % STAGES);
+        const uint64_t e0 = (first + it * stride) * TT;
+        const uint32_t cnt = tile_cnt(it);
+        StepTile<TT> &t = tiles[s];
+        mbar_expect_tx(&full[s], cnt * 14u);
+        bulk_g2s(t.p, a.p + e0, cnt * 4u, &full[s]);
+        bulk_g2s(t.m, a.m + e0, cnt * 4u, &full[s]);
+        bulk_g2s(t.v, a.v + e0, cnt * 4u, &full[s]);
+        bulk_g2s(t.g, g16 + e0, cnt * 2u, &full[s]);
+    };
+
+    if (threadIdx.x == 0)
+        for (uint64_t it = 0; it < my_count && it < (uint64_t)STAGES; ++it) issue_loads(it);
+
+    for (uint64_t it = 0; it < my_count; ++it) {
+        const int s = (int)(it % STAGES);
+        const uint32_t parity = (uint32_t)((it / STAGES) & 1);
+        const uint64_t e0 = (first + it * stride) * TT;
+        const uint32_t cnt = tile_cnt(it);
+        StepTile<TT> &t = tiles[s];
+        mbar_wait(&full[s], parity);
+#pragma unroll
+        for (int hf = 0; hf < kHalves; ++hf) {
+            const uint32_t e = hf * (kStepThreads * 4) + threadIdx.x * 4;
+            if (e < cnt) {
+                float4 P = *reinterpret_cast<float4 *>(t.p + e);
+                float4 M = *reinterpret_cast<float4 *>(t.m + e);
+                float4 V = *reinterpret_cast<float4 *>(t.v + e);
+                const uint2 G = *reinterpret_cast<const uint2 *>(t.g + e);
+                adamw_element(P.x, M.x, V.x, bf16lo(G.x), coef, a.sc);
+                adamw_element(P.y, M.y, V.y, bf16hi(G.x), coef, a.sc);
+                adamw_element(P.z, M.z, V.z, bf16lo(G.y), coef, a.sc);
+                adamw_element(P.w, M.w, V.w, bf16hi(G.y), coef, a.sc);
+                *reinterpret_cast<float4 *>(t.p + e) = P;
+                *reinterpret_cast<float4 *>(t.m + e) = M;
+                *reinterpret_cast<float4 *>(t.v + e) = V;
+                uint2 H;
+                H.x = pack_bf16x2(P.x, P.y);
+                H.y = pack_bf16x2(P.z, P.w);
+                *reinterpret_cast<uint2 *>(t.h + e) = H;
+            }
+        }
+        fence_proxy_async_smem();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            bulk_s2g(a.p + e0, t.p, cnt * 4u);
+            bulk_s2g(a.m + e0, t.m, cnt * 4u);
+            bulk_s2g(a.v + e0, t.v, cnt * 4u);
+            bulk_s2g(p16 + e0, t.h, cnt * 2u);
+            if (SNAP) {
+                bulk_s2g(a.sp + e0, t.p, cnt * 4u);
+                bulk_s2g(a.sm + e0, t.m, cnt * 4u);
+                bulk_s2g(a.sv + e0, t.v, cnt * 4u);
+            }
+            bulk_commit();
+            // refill the stage used one iteration ago: its stores must have finished READING smem
+            if (it >= 1 && it - 1 + STAGES < my_count) {
+                bulk_wait_read1();
+                issue_loads(it - 1 + STAGES);
+            }
+        }
+    }
+    if (threadIdx.x == 0) bulk_wait_all0();
+}
+
+template <int TT, int STAGES>
+static cudaError_t launch_tma(const StepArgs &a, bool snapshot, cudaStream_t st)
+{
+    if (a.n_padded == 0) return cudaSuccess;
+    const size_t smem = sizeof(StepTile<TT>) * STAGES;
+    static int sm_count = 0;
+    static int ctas_per_sm = 0;
+    if (sm_count == 0) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(k_step_tma<TT, STAGES, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(k_step_tma<TT, STAGES, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        ctas_per_sm = (int)((227u * 1024u) / (smem + 1024));
+        if (ctas_per_sm < 1) ctas_per_sm = 1;
+        if (ctas_per_sm > 8) ctas_per_sm = 8;
+    }
+    const uint64_t ntiles = (a.n_padded + TT - 1) / TT;
+    uint64_t grid = (uint64_t)sm_count * ctas_per_sm;
+    if (grid > ntiles) grid = ntiles;
+    if (snapshot) k_step_tma<TT, STAGES, true><<<(unsigned)grid, kStepThreads, smem, st>>>(a);
+    else k_step_tma<TT, STAGES, false><<<(unsigned)grid, kStepThreads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, cudaStream_t st)
 {
     switch (variant) {
@@ -291,6 +477,10 @@ cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, cuda
     case 5: return launch8<3, 1>(a, snapshot, st);  // 256-bit, evict_first on stores too
     case 6: return launch4<1, 4>(a, snapshot, st);  // 128-bit, four groups per thread
     case 7: return launch4<0, 2>(a, snapshot, st);  // 128-bit, no hints
+    case 8: return launch_tma<2048, 3>(a, snapshot, st);   // TMA pipeline, 32 KB stages x3, 2 CTAs/SM
+    case 9: return launch_tma<4096, 3>(a, snapshot, st);   // TMA pipeline, 64 KB stages x3, 1 CTA/SM
+    case 10: return launch_tma<1024, 4>(a, snapshot, st);  // TMA pipeline, 16 KB stages x4, 3 CTAs/SM
+    case 11: return launch_tma<2048, 2>(a, snapshot, st);  // TMA pipeline, 32 KB stages x2, 3 CTAs/SM
     default: return cudaErrorInvalidValue;
     }
 }
@@ -413,47 +603,6 @@ cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cuda
 constexpr int kTile = 2048;  // elements per plane per tile (8 KB)
 constexpr int kStages = 4;
 constexpr int kRestoreThreads = 256;
-
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t ok;
-    do {  // try_wait suspends the thread in hardware for a bounded time; loop until the phase flips
-        asm volatile(
-            "{\n"
-            ".reg .pred P1;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, P1;\n"
-            "}\n"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(smem_dst)),
-                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_s2g(void *gdst, const void *smem_src, uint32_t bytes)
-{
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)),
-                 "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 __global__ void __launch_bounds__(kRestoreThreads) k_restore_bulk(const float *__restrict__ src, float *__restrict__ p,
                                                                   float *__restrict__ m, float *__restrict__ v,

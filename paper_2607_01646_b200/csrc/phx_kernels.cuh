@@ -22,14 +22,14 @@ struct StepArgs {
     const void *g;               // bf16 grads
     void *p16;                   // bf16 param copy
     float *sp, *sm, *sv;         // staging planes of the slot being written (null if !snapshot)
-    void *shdr;                  // staging slot header (256 B) (null if !snapshot)
+    void *shdr;                  // where block 0 stores the 256-B header (null: no header)
     const float *coef;           // device scalar: clip coefficient (1.0f when clipping is off)
     uint64_t n_padded;           // multiple of 64
     AdamScalars sc;
     HeaderBlob hdr;
 };
 
-enum { kNumStepVariants = 8 };
+enum { kNumStepVariants = 12 };
 
 // a3.  variant selects the kernel flavour (see phx_kernels.cu); snapshot=false drops the staging stores.
 cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, cudaStream_t st);

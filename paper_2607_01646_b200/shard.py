@@ -16,8 +16,9 @@ from .workloads import Hyper, Workload
 
 class Shard:
     def __init__(self, wl: Workload, *, device="cuda:0", staging_depth=2, sync_mode=B.PHX_SYNC_STRICT,
-                 chunk_bytes=64 << 20, snapshot=True, restore_mode=B.PHX_RESTORE_BULK_KERNEL,
-                 max_grad_norm: Optional[float] = None, replica: Optional[torch.Tensor] = None):
+                 chunk_bytes=0, snapshot=True, restore_mode=B.PHX_RESTORE_COPY_ENGINE,
+                 max_grad_norm: Optional[float] = None, replica: Optional[torch.Tensor] = None,
+                 snapshot_source=B.PHX_SNAPSHOT_STAGED):
         self.wl = wl
         self.device = torch.device(device)
         self.hyper: Hyper = wl.hyper
@@ -25,7 +26,8 @@ class Shard:
         self.h = B.phx_shard_create(
             wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank), pp=(wl.pp_size, wl.pp_rank),
             staging_depth=staging_depth, sync_mode=sync_mode, chunk_bytes=chunk_bytes,
-            snapshot_disabled=not snapshot, restore_mode=restore_mode, max_grad_norm=mgn)
+            snapshot_disabled=not snapshot, restore_mode=restore_mode, max_grad_norm=mgn,
+            snapshot_source=snapshot_source)
         self.info = B.phx_shard_info(self.h)
         self.n, self.n_padded = self.info.n, self.info.n_padded
         self.segments = [(tid, off_s, ln) for tid, _, off_s, ln in B.phx_shard_segments(self.h)]
@@ -38,8 +40,9 @@ class Shard:
             self.staging = None
             self.replica = None
             if snapshot:
-                self.staging = torch.zeros(self.info.staging_depth * self.info.slot_stride,
-                                           dtype=torch.uint8, device=self.device)
+                if self.info.staging_depth > 0:     # PHX_SNAPSHOT_DIRECT needs no staging ring
+                    self.staging = torch.zeros(self.info.staging_depth * self.info.slot_stride,
+                                               dtype=torch.uint8, device=self.device)
                 if replica is None:
                     replica = torch.zeros(2 * self.info.slot_stride, dtype=torch.uint8).pin_memory()
                 assert replica.is_pinned() and replica.numel() >= 2 * self.info.slot_stride

@@ -17,7 +17,7 @@ def bits16(t: torch.Tensor) -> np.ndarray:
     return t.detach().cpu().view(torch.int16).numpy().view(np.uint16)
 
 
-def make_pair(wl, *, steps, grads=None, chunk_bytes=64 << 20, user=b"", init_mv=False, **shard_kw):
+def make_pair(wl, *, steps, grads=None, chunk_bytes=8 << 20, user=b"", init_mv=False, **shard_kw):
     """(Shard, OracleShard, [grad tensors on GPU], [grad bits for the oracle]) with equal initial state."""
     s = Shard(wl, device=DEV, chunk_bytes=chunk_bytes, **shard_kw)
     mgn = shard_kw.get("max_grad_norm", None)

@@ -83,7 +83,8 @@ def test_argument_and_state_errors_without_a_gpu():
         B.phx_shard_create([(10, 0)], 0, 0)
     assert e.value.code == B.PHX_ERR_INVALID_ARG
     for kw in (dict(dp_rank=2), dict(staging_depth=5), dict(tp=(2, 2)), dict(pp=(1, 1)), dict(sync_mode=2),
-               dict(restore_mode=2), dict(max_grad_norm=float("nan"))):
+               dict(restore_mode=2), dict(max_grad_norm=float("nan")), dict(snapshot_source=2),
+               dict(snapshot_source=B.PHX_SNAPSHOT_DIRECT, sync_mode=B.PHX_SYNC_RELAXED)):
         args = dict(dp_size=2, dp_rank=0)
         args.update(kw)
         with pytest.raises(B.PhxError) as e:

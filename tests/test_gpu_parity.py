@@ -120,7 +120,7 @@ def test_sizes_and_ragged_tails(numels, dp):
     s.close()
 
 
-@pytest.mark.parametrize("variant", range(8))
+@pytest.mark.parametrize("variant", range(12))
 def test_every_kernel_variant_is_bit_identical(variant):
     wl = W.tiny_workload([256 * 8 * 7 + 64 * 5, 999], dp_size=1, grad_kind="heavy_tail")
     s, o, gdev, gbits = make_pair(wl, steps=4, init_mv=True)
@@ -384,3 +384,107 @@ def test_full_size_sampled_parity(key):
     for a, b in zip((s.p, s.m, s.v, s.p16), before):
         assert torch.equal(a, b)
     s.close()
+
+
+def test_c4a_hot_swap_recovery_trajectory_bit_exact():
+    """BASELINE.json:configs[3] at the stated size (~200M elements): 20 steps with snapshots, the live shard is
+    dropped while step 21 is in flight, restore from the pinned host replica, recompute 21, run 22..25.  The
+    result equals the uninterrupted trajectory bit for bit — GPU vs GPU on every element, GPU vs oracle on
+    sampled windows the oracle advances through all 25 steps."""
+    wl = W.CONFIGS["c4a"]
+    hp = hp_of(wl)
+    s = Shard(wl, device=DEV)
+    N = s.n_padded
+    assert N == 203_379_200
+    p0 = W.init_params(s.n, N, wl.seed, device=DEV)
+    s.p.copy_(p0); s.set_state(0)
+    ref = Shard(wl, device=DEV, snapshot=False)
+    ref.p.copy_(p0); ref.set_state(0)
+    grads = [W.gen_grads(wl, s.segments, N, t, wl.seed, device=DEV) for t in (1, 2, 3)]
+    rng = np.random.default_rng(21)
+    idx = torch.cat([torch.arange(a, b) for a, b in _sample_windows(N, rng, k=24)]).to(DEV)
+    o = dict(p=p0[idx].cpu().numpy().copy(), m=np.zeros(idx.numel(), np.float32),
+             v=np.zeros(idx.numel(), np.float32), h=np.zeros(idx.numel(), np.uint16))
+    gs = [bits16(g[idx]).copy() for g in grads]
+    for t in range(1, 26):
+        ref.step_and_snapshot(grads[t % 3], t)
+        O.adamw_step(o["p"], o["m"], o["v"], gs[t % 3], o["h"], **hp, step=t, nthreads=4)
+    side = side_stream()
+    for t in range(1, 21):
+        s.step_and_snapshot(grads[t % 3], t)
+        s.flush_async(side)
+    s.step_and_snapshot(grads[21 % 3], 21)          # in flight
+    s.drop_live()
+    assert s.restore() == 20                        # at most one step of re-execution (PAPER.md:133)
+    for t in range(21, 26):
+        s.step_and_snapshot(grads[t % 3], t)
+        s.flush_async(side)
+    s.wait(25)
+    torch.cuda.synchronize()
+    for a, b in ((s.p, ref.p), (s.m, ref.m), (s.v, ref.v), (s.p16, ref.p16)):
+        assert torch.equal(a, b)
+    assert np.array_equal(s.p[idx].cpu().numpy().view(np.uint32), o["p"].view(np.uint32))
+    assert np.array_equal(s.m[idx].cpu().numpy().view(np.uint32), o["m"].view(np.uint32))
+    assert np.array_equal(s.v[idx].cpu().numpy().view(np.uint32), o["v"].view(np.uint32))
+    assert np.array_equal(bits16(s.p16[idx]), o["h"])
+    hdr = O.parse_header(s.replica_slot(25)[:256].numpy().tobytes())
+    assert hdr["step"] == 25 and hdr["tp"] == (2, 0) and hdr["pp"] == (2, 0) and hdr["dp"] == (16, 0)
+    s.close(); ref.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# PHX_SNAPSHOT_DIRECT: no staging ring, the flush DMAs the live planes (strict sync protects them)
+# ------------------------------------------------------------------------------------------------
+
+
+@pytest.mark.parametrize("numels,chunk", [([64], 4096), ([2048 * 3 + 64], 1000), ([300_000, 77, 12_345], 1 << 20),
+                                          ([300_000, 77, 12_345], 999_936)])
+def test_direct_source_replica_bytes_and_restore(numels, chunk):
+    wl = W.tiny_workload(numels, dp_size=1, hyper=W.Hyper(max_grad_norm=0.02))
+    s, o, gdev, gbits = make_pair(wl, steps=5, chunk_bytes=chunk, snapshot_source=B.PHX_SNAPSHOT_DIRECT,
+                                  user=b"direct")
+    assert s.staging is None and s.info.staging_depth == 0
+    side = side_stream()
+    hp = hp_of(wl)
+    for t in range(1, 5):
+        s.step_and_snapshot(gdev[t - 1], t)
+        s.flush_async(side)          # chunks straddle the p|m|v plane boundaries of the packed layout
+        o.step(gbits[t - 1], **hp, step=t)
+        o.snapshot()
+    s.wait(4)
+    assert_state_equal(s, o, "direct, 4 steps")
+    for t in (3, 4):
+        assert np.array_equal(s.replica_slot(t).numpy(), o.replica[t % 2]), t
+    s.step_and_snapshot(gdev[4], 5)   # in flight, never flushed
+    s.drop_live()
+    assert s.restore() == 4 and B.phx_restored_user_metadata(s.h) == b"direct"
+    assert_state_equal(s, o, "direct restore")
+    s.close()
+
+
+def test_direct_source_waits_for_commit_before_mutating_live_state():
+    """The hazard PHX_SNAPSHOT_DIRECT must exclude: step k+1's kernel overwriting live planes while
+    flush(k) still reads them.  Many back-to-back steps with a slow (tiny-chunk) flush in between:
+    every committed replica must equal the oracle's snapshot of exactly that step."""
+    wl = W.tiny_workload([1_500_000], dp_size=1)
+    s, o, gdev, gbits = make_pair(wl, steps=8, chunk_bytes=16 << 10, snapshot_source=B.PHX_SNAPSHOT_DIRECT)
+    side = side_stream()
+    snaps = {}
+    for t in range(1, 9):
+        s.step_and_snapshot(gdev[t - 1], t)
+        s.flush_async(side)           # ~1100 small copies; the next kernel is enqueued immediately
+        o.step(gbits[t - 1], **hp_of(wl), step=t)
+        o.snapshot()
+        snaps[t] = o.replica[t % 2].copy()
+    s.wait(8)
+    torch.cuda.synchronize()
+    assert np.array_equal(s.replica_slot(8).numpy(), snaps[8])
+    assert np.array_equal(s.replica_slot(7).numpy(), snaps[7])
+    assert_state_equal(s, o, "direct back-to-back")
+    s.close()
+
+
+def test_direct_source_requires_strict_sync():
+    with pytest.raises(B.PhxError) as e:
+        B.phx_shard_create([(1000, 0)], 1, 0, snapshot_source=B.PHX_SNAPSHOT_DIRECT, sync_mode=B.PHX_SYNC_RELAXED)
+    assert e.value.code == B.PHX_ERR_INVALID_ARG
