@@ -50,6 +50,12 @@ def lib() -> ctypes.CDLL:
         L.phx_oracle_clip_coef.restype = ctypes.c_float
         L.phx_oracle_regen_bf16.argtypes = [f32p, u16p, ctypes.c_size_t]
         L.phx_oracle_regen_bf16.restype = None
+        u8p = ctypes.POINTER(ctypes.c_uint8)
+        L.phx_oracle_adamw_step_ex.argtypes = [f32p, f32p, f32p, u16p, f32p, u16p, u8p, ctypes.c_size_t] + \
+            [ctypes.c_float] * 5 + [ctypes.c_uint64, ctypes.c_float, ctypes.c_int]
+        L.phx_oracle_adamw_step_ex.restype = None
+        L.phx_oracle_sumsq_f32.argtypes = [f32p, ctypes.c_size_t]
+        L.phx_oracle_sumsq_f32.restype = ctypes.c_double
         _lib = L
     return _lib
 
@@ -79,8 +85,29 @@ def adamw_step(p, m, v, g_bits, p16, lr, beta1, beta2, eps, wd, step, coef=1.0, 
                                 lr, beta1, beta2, eps, wd, int(step), coef, int(nthreads))
 
 
-def sumsq(g_bits: np.ndarray) -> float:
-    return float(lib().phx_oracle_sumsq(_u16p(g_bits), g_bits.shape[0]))
+def adamw_step_ex(p, m, v, g, p16, no_decay, lr, beta1, beta2, eps, wd, step, coef=1.0, nthreads=1):
+    """In-place step of the general routine: `g` is uint16 bf16 bits or
+    float32 gradients, `p16` may be None (no bf16 copy), `no_decay` may be None
+    or a uint8 mask, one byte per element (reading R5b)."""
+    n = p.shape[0]
+    assert m.shape[0] == n and v.shape[0] == n and g.shape[0] == n
+    null16 = ctypes.POINTER(ctypes.c_uint16)()
+    null32 = ctypes.POINTER(ctypes.c_float)()
+    g16, g32 = (_u16p(g), null32) if g.dtype == np.uint16 else (null16, _f32p(g))
+    nd = ctypes.POINTER(ctypes.c_uint8)()
+    if no_decay is not None:
+        assert no_decay.dtype == np.uint8 and no_decay.shape[0] == n and no_decay.flags.c_contiguous
+        nd = no_decay.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8))
+    lib().phx_oracle_adamw_step_ex(_f32p(p), _f32p(m), _f32p(v), g16, g32,
+                                   null16 if p16 is None else _u16p(p16), nd, n,
+                                   lr, beta1, beta2, eps, wd, int(step), coef, int(nthreads))
+
+
+def sumsq(g: np.ndarray) -> float:
+    """Sum of squares of the gradients (bf16 bits or float32), a1 / reading R7."""
+    if g.dtype == np.float32:
+        return float(lib().phx_oracle_sumsq_f32(_f32p(g), g.shape[0]))
+    return float(lib().phx_oracle_sumsq(_u16p(g), g.shape[0]))
 
 
 def clip_coef(sumsq_value: float, max_norm: float) -> np.float32:
@@ -101,6 +128,7 @@ def rne_bf16(x: np.ndarray) -> np.ndarray:
 # PAPER.md:27; ZeRO-2)
 # ----------------------------------------------------------------------------
 
+TENSOR_NO_DECAY = 1  # phx_tensor_desc_t.flags bit: the tensor takes weight decay 0 (reading R5b)
 PAD_UNIT = 64  # elements: every rank's range is a multiple of 64 (256 B of fp32, 128 B of bf16)
 HEADER_BYTES = 256
 MAGIC = b"PHXSNAP1"
@@ -197,10 +225,12 @@ class OracleShard:
     replica slots each `header ‖ p ‖ m ‖ v` (ping-pong)."""
 
     def __init__(self, layout, dp_size, dp_rank, tp=(1, 0), pp=(1, 0),
-                 chunk_bytes=64 << 20, max_grad_norm=0.0, user=b""):
+                 chunk_bytes=64 << 20, max_grad_norm=0.0, user=b"", flags=None, precision="bf16"):
+        assert precision in ("bf16", "fp32")
         self.layout = [(int(a), int(b)) for a, b in layout]
         self.dp, self.tp, self.pp = (dp_size, dp_rank), tuple(tp), tuple(pp)
-        d = define_shard(self.layout, dp_size, dp_rank, tp, pp)
+        self.precision = precision  # "fp32": binary32 gradients, no bf16 copy (PAPER.md:270; SURVEY §8(f2))
+        d = define_shard(self.layout, dp_size, dp_rank, tp, pp, flags)
         self.n, self.n_padded = d["n"], d["n_padded"]
         self.total_numel, self.shard_begin = d["total_numel"], d["shard_begin"]
         self.segments, self.layout_hash = d["segments"], d["layout_hash"]
@@ -216,6 +246,14 @@ class OracleShard:
         self.snapshot_bytes = HEADER_BYTES + 12 * N
         self.replica = [np.zeros(self.snapshot_bytes, np.uint8) for _ in range(2)]
         self.last_coef = np.float32(1.0)
+        # decay groups (reading R5b): one byte per element, 1 where the owning tensor is flagged no-decay
+        self.no_decay = None
+        if flags is not None and any(int(f) & TENSOR_NO_DECAY for f in flags):
+            by_id = {tid: int(f) for (_, tid), f in zip(self.layout, flags)}
+            self.no_decay = np.zeros(N, np.uint8)
+            for tid, _, off, ln in self.segments:
+                if by_id[tid] & TENSOR_NO_DECAY:
+                    self.no_decay[off:off + ln] = 1
 
     # -- state ---------------------------------------------------------------
     def set_state(self, p, m=None, v=None, step=0):
@@ -223,7 +261,7 @@ class OracleShard:
         self.p[:] = p
         self.m[:] = 0 if m is None else m
         self.v[:] = 0 if v is None else v
-        self.p16[:] = rne_bf16(self.p)
+        self.p16[:] = rne_bf16(self.p) if self.precision == "bf16" else 0
         self.last_step = int(step)
 
     # -- a1 + a3 ---------------------------------------------------------------
@@ -232,13 +270,17 @@ class OracleShard:
         atomicity; reading R3)."""
         if int(step) != self.last_step + 1:
             raise OracleError("step order")
-        g_bits = np.ascontiguousarray(g_bits, dtype=np.uint16)
+        g_bits = np.ascontiguousarray(g_bits, dtype=np.uint16 if self.precision == "bf16" else np.float32)
         coef = np.float32(1.0)
         if self.max_grad_norm > 0.0:
             coef = clip_coef(sumsq(g_bits), self.max_grad_norm)
         self.last_coef = coef
-        adamw_step(self.p, self.m, self.v, g_bits, self.p16, lr, beta1, beta2, eps, wd,
-                   step, float(coef), nthreads)
+        if self.precision == "bf16" and self.no_decay is None:
+            adamw_step(self.p, self.m, self.v, g_bits, self.p16, lr, beta1, beta2, eps, wd,
+                       step, float(coef), nthreads)
+        else:  # SURVEY §8(f2): fp32 gradients / no bf16 copy / decay groups
+            adamw_step_ex(self.p, self.m, self.v, g_bits, self.p16 if self.precision == "bf16" else None,
+                          self.no_decay, lr, beta1, beta2, eps, wd, step, float(coef), nthreads)
         self.last_step = int(step)
 
     # -- a4/a5: snapshot = byte copy of (header, p, m, v) after the step --------
@@ -306,7 +348,7 @@ class OracleShard:
         self.p[:] = raw[HEADER_BYTES:HEADER_BYTES + N4].view(np.float32)
         self.m[:] = raw[HEADER_BYTES + N4:HEADER_BYTES + 2 * N4].view(np.float32)
         self.v[:] = raw[HEADER_BYTES + 2 * N4:].view(np.float32)
-        self.p16[:] = rne_bf16(self.p)
+        self.p16[:] = rne_bf16(self.p) if self.precision == "bf16" else 0
         self.last_step = h["step"]
         self.restored_user = h["user"]
         return self.last_step

@@ -151,3 +151,65 @@ void phx_oracle_regen_bf16(const float *p, uint16_t *p16, size_t n)
     for (size_t i = 0; i < n; ++i)
         p16[i] = phx_oracle_rne_bf16(p[i]);
 }
+
+/* ==== SURVEY.md §8(f2): the paper's own precision and per-tensor decay groups ====
+ *
+ * "all parameters, main gradients and optimizer states (Adam moments together with the
+ * FP32 master copy) use torch.float32 ... BF16 and FP16 disabled": the
+ * gradients arrive as binary32 and there is no bf16 model-parameter copy.  The sequence
+ * is reading R1 unchanged except for its first line (g = g_f32 * coef, no widening) and
+ * its last (no RNE_bf16).  g*g is now a rounded binary32 product (24-bit significands).
+ *
+ * Decay groups (reading R5b): a tensor flagged "no decay" (biases, norm
+ * weights — the usual AdamW parameter groups) takes weight decay 0, i.e. decay = 1.0f
+ * for its elements; p * 1.0f is exact, so its trajectory is bit-identical to a wd = 0 run.
+ *
+ * One general routine: exactly one of g_bf16 / g_f32 is non-NULL; p16 may be NULL (no
+ * bf16 copy); no_decay may be NULL (uniform decay), else one byte per element. */
+void phx_oracle_adamw_step_ex(float *p, float *m, float *v, const uint16_t *g_bf16,
+                              const float *g_f32, uint16_t *p16, const uint8_t *no_decay,
+                              size_t n, float lr, float beta1, float beta2, float eps,
+                              float wd, uint64_t t, float coef, int nthreads)
+{
+    float sc[5];
+    phx_oracle_scalars(lr, beta1, beta2, eps, wd, t, sc);
+    const float decay = sc[0], omb1 = sc[1], omb2 = sc[2], ss = sc[3], sbc2 = sc[4];
+    (void)nthreads;
+#pragma omp parallel for schedule(static) num_threads(nthreads > 0 ? nthreads : 1)
+    for (ptrdiff_t i = 0; i < (ptrdiff_t)n; ++i) {
+        float g = g_f32 ? g_f32[i] : widen_bf16(g_bf16[i]);
+        g = g * coef;
+        float dk = (no_decay && no_decay[i]) ? 1.0f : decay;
+        float p1 = p[i] * dk;
+        float a = beta1 * m[i];
+        float b = omb1 * g;
+        float mn = a + b;
+        float gg = g * g;
+        float c = beta2 * v[i];
+        float e = omb2 * gg;
+        float vn = c + e;
+        float s = sqrtf(vn);
+        float q = s / sbc2;
+        float d = q + eps;
+        float r = mn / d;
+        float u = ss * r;
+        float pn = p1 - u;
+        p[i] = pn;
+        m[i] = mn;
+        v[i] = vn;
+        if (p16)
+            p16[i] = phx_oracle_rne_bf16(pn);
+    }
+}
+
+/* Sum of squares of binary32 gradients: each square is exact in double (48 significant
+ * bits); the running sum is long double, rounded to double once (as phx_oracle_sumsq). */
+double phx_oracle_sumsq_f32(const float *g, size_t n)
+{
+    long double s = 0.0L;
+    for (size_t i = 0; i < n; ++i) {
+        double x = (double)g[i];
+        s += (long double)(x * x);
+    }
+    return (double)s;
+}

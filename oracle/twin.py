@@ -65,6 +65,32 @@ def adamw_step_numpy(p, m, v, g_bits, lr, beta1, beta2, eps, wd, t, coef=1.0):
     return pn, mn, vn, rne_bf16_numpy(pn)
 
 
+def adamw_step_numpy_ex(p, m, v, g, lr, beta1, beta2, eps, wd, t, coef=1.0, no_decay=None, bf16_copy=True):
+    """The general routine of SURVEY.md §8(f2) as numpy float32 array operations: `g` is uint16
+    bf16 bits (widened exactly) or float32 gradients; `no_decay` is an optional
+    boolean/uint8 mask (reading R5b: decay 1.0f on flagged elements).  Returns (p', m', v', p16|None)."""
+    decay, omb1, omb2, ss, sbc2 = scalars_f32(lr, beta1, beta2, eps, wd, t)
+    b1, b2, e = f32(beta1), f32(beta2), f32(eps)
+    with np.errstate(all="ignore"):
+        gw = widen(g) if g.dtype == np.uint16 else g
+        gw = gw * f32(coef)
+        dk = decay if no_decay is None else np.where(np.asarray(no_decay) != 0, f32(1.0), decay).astype(np.float32)
+        p1 = p * dk
+        mn = (b1 * m) + (omb1 * gw)
+        vn = (b2 * v) + (omb2 * (gw * gw))
+        d = (np.sqrt(vn) / sbc2) + e
+        pn = p1 - (ss * (mn / d))
+    for a in (gw, p1, mn, vn, d, pn):
+        assert a.dtype == np.float32
+    return pn, mn, vn, (rne_bf16_numpy(pn) if bf16_copy else None)
+
+
+def sumsq_exact_f32(g: np.ndarray) -> float:
+    """math.fsum of the exact squares of binary32 gradients (each square is exact in double)."""
+    x = np.asarray(g, dtype=np.float32).astype(np.float64)
+    return math.fsum((x * x).tolist())
+
+
 def adamw_step_f64(p, m, v, g, lr, beta1, beta2, eps, wd, t):
     """float64 shadow: textbook AdamW (decoupled decay, bias-corrected, eps outside the
     square root after bias-correcting v) on float64 arrays; hyperparameters are the
