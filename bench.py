@@ -70,6 +70,11 @@ def parse_args():
                     help="snapshot source: staged = fused kernel also writes the staging slot (40 B/elem, north_star); "
                          "direct = flush DMAs the live planes under the strict sync point (28 B/elem)")
     ap.add_argument("--restore-mode", default="copy", choices=["bulk", "copy"])
+    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp32"],
+                    help="bf16 = fp32 state + bf16 grads + bf16 copy (north_star, default); fp32 = the paper's own "
+                         "all-FP32 setting (PAPER.md:270; SURVEY 8(f2)): fp32 grads, no bf16 copy, 16 B read + 24 B written")
+    ap.add_argument("--decay-groups", action="store_true",
+                    help="flag biases and norm weights no-decay (per-tensor AdamW parameter groups, SURVEY 8(f2))")
     ap.add_argument("--chunks", default="4,8,16,32,64,128,256", help="chunk sizes (MiB) of --mode sweep")
     ap.add_argument("--depths", default="1,2,3,4", help="staging depths of --mode sweep")
     ap.add_argument("--syncs", default="strict,relaxed", help="sync modes of --mode sweep")
@@ -203,13 +208,21 @@ def barrier(world):
 # ----------------------------------------------------------------------------------------------
 
 
+def workload_of(args, key):
+    """BASELINE.json config `key`, in the precision / decay-group variant the flags ask for."""
+    import dataclasses
+    from paper_2607_01646_b200 import workloads as W
+    return dataclasses.replace(W.CONFIGS[key], precision=args.precision, decay_groups=bool(args.decay_groups))
+
+
 def time_oracle(wl, sample, steps, warmup, nthreads):
     """Oracle AdamW step (phx_oracle.c, as it stands) on the first `sample` elements of the shard."""
     import numpy as np
     import torch
     from oracle import oracle as O
     from paper_2607_01646_b200 import workloads as W
-    d = O.define_shard(wl.layout(), wl.dp_size, wl.dp_rank, (wl.tp_size, wl.tp_rank), (wl.pp_size, wl.pp_rank))
+    fp32 = wl.precision == "fp32"
+    d = O.define_shard(wl.layout(), wl.dp_size, wl.dp_rank, (wl.tp_size, wl.tp_rank), (wl.pp_size, wl.pp_rank), wl.flags())
     n = min(sample, d["n_padded"])
     segs = []
     for tid, _, off, ln in d["segments"]:
@@ -219,7 +232,17 @@ def time_oracle(wl, sample, steps, warmup, nthreads):
     m = np.zeros(n, np.float32)
     v = np.zeros(n, np.float32)
     p16 = np.zeros(n, np.uint16)
-    g = W.gen_grads(wl, segs, n, 1, wl.seed).view(torch.int16).numpy().view(np.uint16)
+    if fp32:
+        g = W.gen_grads(wl, segs, n, 1, wl.seed, dtype=torch.float32).numpy()
+    else:
+        g = W.gen_grads(wl, segs, n, 1, wl.seed).view(torch.int16).numpy().view(np.uint16)
+    mask = None
+    if any(wl.flags()):
+        mask = np.zeros(n, np.uint8)
+        fl = wl.flags()
+        for tid, off, ln in segs:
+            if fl[tid] & 1:
+                mask[off:off + ln] = 1
     h = wl.hyper
     times = []
     for t in range(1, warmup + steps + 1):
@@ -227,7 +250,10 @@ def time_oracle(wl, sample, steps, warmup, nthreads):
         t0 = time.perf_counter()
         if h.max_grad_norm > 0:
             coef = float(O.clip_coef(O.sumsq(g), h.max_grad_norm))
-        O.adamw_step(p, m, v, g, p16, h.lr, h.beta1, h.beta2, h.eps, h.wd, t, coef, nthreads)
+        if fp32 or mask is not None:
+            O.adamw_step_ex(p, m, v, g, None if fp32 else p16, mask, h.lr, h.beta1, h.beta2, h.eps, h.wd, t, coef, nthreads)
+        else:
+            O.adamw_step(p, m, v, g, p16, h.lr, h.beta1, h.beta2, h.eps, h.wd, t, coef, nthreads)
         dt = time.perf_counter() - t0
         if t > warmup:
             times.append(dt)
@@ -238,8 +264,7 @@ def run_reference(args):
     rank, world, _ = rank_env()
     if rank != 0:
         return 0
-    from paper_2607_01646_b200 import workloads as W
-    wl = W.CONFIGS[args.config]
+    wl = workload_of(args, args.config)
     cores = len(os.sched_getaffinity(0))
     sample = args.cpu_sample or (1 << 24)
     n, times = time_oracle(wl, sample, args.steps, args.warmup, cores)
@@ -279,7 +304,7 @@ class Rig:
         from paper_2607_01646_b200.shard import Shard
         self.torch, self.B, self.W, self.Shard, self.args = torch, B, W, Shard, args
         self.device = torch.device(f"cuda:{local_rank}")
-        base = W.CONFIGS[key]
+        base = workload_of(args, key)
         # weak scaling: every rank owns one DP shard of the same model (its own dp_rank); no data-path collective
         self.wl = dataclasses.replace(base, dp_rank=rank % base.dp_size)
         self.depth = depth or args.depth
@@ -299,7 +324,11 @@ class Rig:
         self.N = self.s.n_padded
         self.s.p.copy_(W.init_params(self.s.n, self.N, self.wl.seed, device=self.device))
         self.s.set_state(0)
-        self.grads = [W.gen_grads(self.wl, self.s.segments, self.N, t, self.wl.seed, device=self.device) for t in (1, 2)]
+        self.fp32 = self.wl.precision == "fp32"
+        self.grad_bytes = 4 if self.fp32 else 2
+        gdt = torch.float32 if self.fp32 else torch.bfloat16
+        self.grads = [W.gen_grads(self.wl, self.s.segments, self.N, t, self.wl.seed, device=self.device, dtype=gdt)
+                      for t in (1, 2)]
         self.hgrads = [g.cpu().pin_memory() for g in self.grads] if host_grads else None
         torch.cuda.synchronize()
         self.cur = torch.cuda.current_stream(self.device)
@@ -309,6 +338,13 @@ class Rig:
         self.off_step = 0
         self._gemm = None
         self.gemm_ms = None
+
+    def precision_code(self):
+        return self.B.PHX_PRECISION_FP32 if self.fp32 else self.B.PHX_PRECISION_BF16_GRADS
+
+    def kernel_name(self):
+        mode = (1 if self.fp32 else 0) | (2 if any(self.wl.flags()) else 0)
+        return "phx::k_step8<1,1,%s,%d>" % ("true" if self.source_name == "staged" else "false", mode)
 
     # -- the hot path -------------------------------------------------------------------------------
     def do_step(self):
@@ -336,7 +372,7 @@ class Rig:
         torch, B, wl = self.torch, self.B, self.wl
         h0 = B.phx_shard_create(wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank),
                                 pp=(wl.pp_size, wl.pp_rank), staging_depth=self.depth, max_grad_norm=0.0,
-                                snapshot_source=self.source)
+                                snapshot_source=self.source, flags=wl.flags(), precision=self.precision_code())
         B.phx_shard_bind(h0, self.s.p, self.s.m, self.s.v, self.s.p16, self.s.staging, self.s.replica)
         B.phx_shard_set_state(h0, 0, self.cur)
         B.phx_set_kernel_variant(h0, self.args.variant)
@@ -357,7 +393,8 @@ class Rig:
             B, wl = self.B, self.wl
             h = B.phx_shard_create(wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank),
                                    pp=(wl.pp_size, wl.pp_rank), snapshot_disabled=True,
-                                   max_grad_norm=wl.hyper.max_grad_norm)
+                                   max_grad_norm=wl.hyper.max_grad_norm, flags=wl.flags(),
+                                   precision=self.precision_code())
             B.phx_shard_bind(h, self.s.p, self.s.m, self.s.v, self.s.p16, None, None)
             B.phx_shard_set_state(h, 0, self.cur)
             B.phx_set_kernel_variant(h, self.args.variant)
@@ -575,9 +612,10 @@ def run_headline(args):
     peak, peak_src = measured_peaks()
     achieved = BPE * N / (kern_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": committed_traffic(args.config if rig.source_name == "staged" else args.config + "-direct"),
+                "traffic": committed_traffic(args.config + ("" if rig.source_name == "staged" else "-direct")
+                                             + ("-fp32" if rig.fp32 else "") + ("-groups" if args.decay_groups else "")),
                 "peak_source": peak_src, "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS,
-                "kernel": "phx::k_step8<1,1,%s>" % ("true" if rig.source_name == "staged" else "false"),
+                "kernel": rig.kernel_name(),
                 "kernel_ms": kern_ms, "algorithmic_bytes_per_launch": BPE * N, "bytes_per_element": BPE,
                 "snapshot_off_step_ms": off_ms,
                 "snapshot_off_gbs": BYTES_PER_ELEM_OFF * N / (off_ms * 1e-3) / 1e9}
@@ -586,7 +624,7 @@ def run_headline(args):
     e2e_ms = max_over_ranks(rig.e2e(args.e2e_steps, world), world, device)
     d2h_bytes = int(rig.s.info.snapshot_bytes)
     e2e = {"value": BPE * units / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
-           "h2d_bytes_per_step": int(2 * N), "d2h_bytes_per_step": d2h_bytes, "ms_per_step": e2e_ms,
+           "h2d_bytes_per_step": int(rig.grad_bytes * N), "d2h_bytes_per_step": d2h_bytes, "ms_per_step": e2e_ms,
            "steps": args.e2e_steps,
            "note": "H2D grads from pinned host + fused step + chunked D2H of the packed snapshot + commit, per step"}
 
@@ -628,6 +666,9 @@ def run_headline(args):
                        "state_bytes": int(12 * N), "staging_depth": rig.depth, "chunk_mib": rig.chunk_mib,
                        "sync_mode": rig.sync_name, "kernel_variant": args.variant, "snapshot_source": rig.source_name,
                        "bytes_per_element": BPE,
+                       "precision": ("fp32 state + fp32 grads, no bf16 copy (PAPER.md:270): 16 B read + 24 B written"
+                                     if rig.fp32 else "fp32 state + bf16 grads + bf16 copy (north_star): 14 B read + 26 B written"),
+                       "decay_groups": bool(args.decay_groups),
                        "l2": "inputs larger than L2 (working set %.2f GB per step >> 126 MB)" % (BYTES_PER_ELEM * N / 1e9),
                        "timed_region": "K x phx_step_and_snapshot (a1 clip if configured, a2 sync-point wait, a3 fused "
                                        "AdamW+bf16 copy+packed snapshot); a4/a5 host flush is in e2e and overlap",

@@ -74,12 +74,22 @@ typedef struct phx_shard phx_shard_t; /* opaque */
 typedef struct {
     uint64_t numel;
     uint32_t tensor_id;
-    uint32_t flags; /* reserved (per-tensor no-decay groups); hashed into the layout hash */
+    uint32_t flags; /* PHX_TENSOR_* bits; hashed into the layout hash */
 } phx_tensor_desc_t;
+/* Decay groups (reading R5b): a tensor flagged PHX_TENSOR_NO_DECAY (biases,
+ * norm weights — the usual AdamW parameter groups) takes weight decay 0: decay = 1.0f for its elements,
+ * so its trajectory equals a wd = 0 run bit for bit.  All other bits are reserved (must be 0). */
+enum { PHX_TENSOR_NO_DECAY = 1u };
 
 enum { PHX_SYNC_STRICT = 0, PHX_SYNC_RELAXED = 1 };
 enum { PHX_RESTORE_COPY_ENGINE = 0, PHX_RESTORE_BULK_KERNEL = 1 };
 enum { PHX_SNAPSHOT_STAGED = 0, PHX_SNAPSHOT_DIRECT = 1 };
+/* PHX_PRECISION_BF16_GRADS (default, BASELINE.json:north_star): fp32 state, bf16 gradients, bf16 model-param
+ * copy.  PHX_PRECISION_FP32: the precision the paper evaluates — "all parameters, main
+ * gradients and optimizer states ... use torch.float32 ... BF16 and FP16 disabled": the
+ * gradients are float[n_padded], there is no bf16 copy (d_p_bf16 may be NULL) and the fused kernel moves
+ * 16 B read + 24 B written per element (12 written with snapshots off). */
+enum { PHX_PRECISION_BF16_GRADS = 0, PHX_PRECISION_FP32 = 1 };
 
 /* Any field left 0 takes its default; cfg == NULL means all defaults. */
 typedef struct {
@@ -104,7 +114,8 @@ typedef struct {
                                  next step's kernel waits for commit(k) before it mutates the protected state
                                  (exactly the paper's sync point); requires PHX_SYNC_STRICT.
                                  The kernel then moves 28 B/element instead of 40.                           */
-    uint32_t reserved[4];
+    uint32_t precision;       /* PHX_PRECISION_BF16_GRADS (default) | PHX_PRECISION_FP32                   */
+    uint32_t reserved[3];
 } phx_config_t;
 
 typedef struct {
@@ -154,6 +165,7 @@ PHX_API int phx_shard_segments(const phx_shard_t *s, uint32_t *tensor_id, uint64
  * d_staging: staging_depth * slot_stride bytes of device memory (may be NULL iff snapshots are
  * disabled or snapshot_source is PHX_SNAPSHOT_DIRECT).  h_replica: 2 * slot_stride bytes of pinned, mapped host memory (may be NULL iff
  * snapshots are disabled).  Requires a CUDA device of compute capability 10.x. */
+/* d_p_bf16 may be NULL iff precision is PHX_PRECISION_FP32. */
 PHX_API int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p_bf16,
                            void *d_staging, void *h_replica);
 /* Declare the bound p, m, v to be the state after optimizer step `step` (0 at initialisation)
@@ -178,8 +190,11 @@ PHX_API int phx_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len
  *      v' bits plus the header into staging slot `step mod depth` ("packed into a contiguous
  *      buffer") — the snapshot costs no extra read pass and no extra kernel.
  * `step` is the 1-based index of the update and must equal last_step + 1.
- * Traffic: reads 14 B/element, writes 26 B/element (14 with snapshots disabled). */
-PHX_API int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads_bf16, float lr, float beta1,
+ * d_grads: bf16[n_padded] (PHX_PRECISION_BF16_GRADS) or float[n_padded] (PHX_PRECISION_FP32: first line
+ * g = g_f32 * c, no bf16 copy is written, the sum of squares uses exact fp64 squares of the fp32 values).
+ * Elements of tensors flagged PHX_TENSOR_NO_DECAY use decay = 1.0f.
+ * Traffic: reads 14 B/element, writes 26 B/element (14 with snapshots disabled); FP32: 16 + 24 (12). */
+PHX_API int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float beta1,
                                   float beta2, float eps, float wd, uint64_t step, void *stream);
 
 /* ---- a4+a5: asynchronous chunked flush of the newest staged snapshot ------------------------
@@ -222,7 +237,8 @@ PHX_API int phx_last_step(const phx_shard_t *s, uint64_t *step);
 PHX_API int phx_last_clip(phx_shard_t *s, float *coef, double *sumsq);
 /* Number of kernels the library has launched on this handle (bench.py's gpu_launches). */
 PHX_API int phx_kernel_launches(const phx_shard_t *s, uint64_t *count);
-/* Selects a kernel variant of the fused step (0 = default); for tuning/benchmarks only. */
+/* Selects a kernel variant of the fused step (0 = default); for tuning/benchmarks only.  Shards with
+ * PHX_PRECISION_FP32 or decay groups accept variant 0 only. */
 PHX_API int phx_set_kernel_variant(phx_shard_t *s, uint32_t variant);
 PHX_API const char *phx_strerror(int err);
 PHX_API int phx_last_cuda_error(const phx_shard_t *s);

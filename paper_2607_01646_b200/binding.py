@@ -34,6 +34,8 @@ PHX_ERR_NOMEM = -12
 PHX_SYNC_STRICT, PHX_SYNC_RELAXED = 0, 1
 PHX_RESTORE_COPY_ENGINE, PHX_RESTORE_BULK_KERNEL = 0, 1
 PHX_SNAPSHOT_STAGED, PHX_SNAPSHOT_DIRECT = 0, 1
+PHX_PRECISION_BF16_GRADS, PHX_PRECISION_FP32 = 0, 1
+PHX_TENSOR_NO_DECAY = 1
 
 
 class phx_tensor_desc_t(C.Structure):
@@ -45,7 +47,7 @@ class phx_config_t(C.Structure):
                 ("pp_rank", C.c_uint32), ("staging_depth", C.c_uint32), ("sync_mode", C.c_uint32),
                 ("chunk_bytes", C.c_uint64), ("snapshot_disabled", C.c_uint32),
                 ("restore_mode", C.c_uint32), ("max_grad_norm", C.c_float),
-                ("snapshot_source", C.c_uint32), ("reserved", C.c_uint32 * 4)]
+                ("snapshot_source", C.c_uint32), ("precision", C.c_uint32), ("reserved", C.c_uint32 * 3)]
 
 
 class phx_shard_info_t(C.Structure):
@@ -136,7 +138,7 @@ def phx_shard_create(layout: Sequence[Tuple[int, int]], dp_size: int, dp_rank: i
                      pp=(1, 0), staging_depth=0, sync_mode=PHX_SYNC_STRICT, chunk_bytes=0,
                      snapshot_disabled=False, restore_mode=PHX_RESTORE_COPY_ENGINE,
                      max_grad_norm=0.0, snapshot_source=PHX_SNAPSHOT_STAGED,
-                     flags: Optional[Sequence[int]] = None) -> int:
+                     flags: Optional[Sequence[int]] = None, precision=PHX_PRECISION_BF16_GRADS) -> int:
     """layout = [(numel, tensor_id)] in flattening order.  Returns the opaque handle."""
     n = len(layout)
     arr = (phx_tensor_desc_t * max(n, 1))()
@@ -146,7 +148,7 @@ def phx_shard_create(layout: Sequence[Tuple[int, int]], dp_size: int, dp_rank: i
     cfg = phx_config_t(tp_size=tp[0], tp_rank=tp[1], pp_size=pp[0], pp_rank=pp[1],
                        staging_depth=staging_depth, sync_mode=sync_mode, chunk_bytes=chunk_bytes,
                        snapshot_disabled=1 if snapshot_disabled else 0, restore_mode=restore_mode,
-                       max_grad_norm=max_grad_norm, snapshot_source=snapshot_source)
+                       max_grad_norm=max_grad_norm, snapshot_source=snapshot_source, precision=precision)
     h = C.c_void_p()
     _ck(lib().phx_shard_create(arr, n, dp_size, dp_rank, C.byref(cfg), C.byref(h)), "phx_shard_create")
     return h.value
@@ -184,9 +186,9 @@ def phx_set_user_metadata(h: int, blob: bytes) -> None:
     _ck(lib().phx_set_user_metadata(h, blob, len(blob)), "phx_set_user_metadata", h)
 
 
-def phx_step_and_snapshot(h: int, d_grads_bf16, lr: float, beta1: float, beta2: float, eps: float,
+def phx_step_and_snapshot(h: int, d_grads, lr: float, beta1: float, beta2: float, eps: float,
                           wd: float, step: int, stream=None) -> None:
-    _ck(lib().phx_step_and_snapshot(h, _ptr(d_grads_bf16), lr, beta1, beta2, eps, wd, step,
+    _ck(lib().phx_step_and_snapshot(h, _ptr(d_grads), lr, beta1, beta2, eps, wd, step,
                                     _ptr(stream)), "phx_step_and_snapshot", h)
 
 

@@ -19,6 +19,7 @@ constexpr int kMaxDepth = 4;
 struct Segment {
     uint32_t tensor_id;
     uint64_t off_in_tensor, off_in_shard, len;
+    uint32_t flags;
 };
 
 enum SlotState { SLOT_EMPTY = 0, SLOT_INFLIGHT, SLOT_COMMITTED, SLOT_TORN_INFLIGHT, SLOT_TORN };
@@ -76,6 +77,12 @@ struct phx_shard {
     uint8_t *d_replica = nullptr;  // device view of h_replica
     uint8_t *d_scratch = nullptr;
     int sm_count = 148;
+    // decay groups: class per 2048-element tile and the offsets where the flag toggles
+    std::vector<uint8_t> decay_cls;
+    std::vector<uint64_t> decay_bnd;
+    uint32_t first_nodecay = 0;
+    bool has_groups = false;
+    uint8_t *d_decay = nullptr;  // device copy: toggles (8-byte aligned) then classes
     // state
     uint64_t last_step = 0;
     uint8_t user[128] = {0};
@@ -155,6 +162,52 @@ bool header_matches(const phx_shard *s, const phx_snapshot_header_t *h)
 }
 
 bool snapshots_on(const phx_shard *s) { return s->cfg.snapshot_disabled == 0; }
+bool fp32_mode(const phx_shard *s) { return s->cfg.precision == PHX_PRECISION_FP32; }
+uint32_t step_mode(const phx_shard *s)
+{
+    return (fp32_mode(s) ? (uint32_t)phx::kModeF32 : 0u) | (s->has_groups ? (uint32_t)phx::kModeGroups : 0u);
+}
+
+// Decay groups: walk the rank's segments in shard order, record the offsets at which the no-decay flag
+// toggles and classify every 2048-element tile as all-decay (0), all-no-decay (1) or mixed (2).  Pad
+// lanes behind the last segment count as decayed (they hold zeros either way).
+void build_decay_groups(phx_shard *s)
+{
+    const uint64_t L = s->info.n_padded;
+    const uint64_t tile = 1ull << phx::kDecayTileShift;
+    bool any = false;
+    for (const auto &g : s->segments) any = any || (g.flags & PHX_TENSOR_NO_DECAY);
+    s->has_groups = any;
+    if (!any) return;
+    s->first_nodecay = (!s->segments.empty() && s->segments[0].off_in_shard == 0 &&
+                        (s->segments[0].flags & PHX_TENSOR_NO_DECAY)) ? 1u : 0u;
+    uint32_t cur = s->first_nodecay;
+    uint64_t pos = 0;
+    auto toggle_to = [&](uint32_t f, uint64_t at) {
+        if (f != cur && at < L) {
+            s->decay_bnd.push_back(at);
+            cur = f;
+        }
+    };
+    for (const auto &g : s->segments) {
+        if (g.len == 0) continue;
+        toggle_to((g.flags & PHX_TENSOR_NO_DECAY) ? 1u : 0u, g.off_in_shard);
+        pos = g.off_in_shard + g.len;
+    }
+    toggle_to(0u, pos);  // padding
+    s->decay_cls.assign((size_t)((L + tile - 1) / tile), 0);
+    size_t k = 0;        // toggles consumed so far
+    uint32_t f = s->first_nodecay;
+    for (size_t t = 0; t < s->decay_cls.size(); ++t) {
+        const uint64_t lo = (uint64_t)t * tile, hi = lo + tile < L ? lo + tile : L;
+        while (k < s->decay_bnd.size() && s->decay_bnd[k] <= lo) {
+            f ^= 1u;
+            ++k;
+        }
+        const bool mixed = k < s->decay_bnd.size() && s->decay_bnd[k] < hi;
+        s->decay_cls[t] = mixed ? 2 : (uint8_t)f;
+    }
+}
 bool direct_mode(const phx_shard *s) { return s->cfg.snapshot_source == PHX_SNAPSHOT_DIRECT; }
 // number of ring positions the bookkeeping cycles through (direct mode: two header slots)
 uint32_t ring_depth(const phx_shard *s) { return direct_mode(s) ? 2u : s->cfg.staging_depth; }
@@ -222,7 +275,7 @@ int phx_shard_create(const phx_tensor_desc_t *layout, size_t n_tensors, uint32_t
     c.chunk_bytes = (c.chunk_bytes + 255) & ~255ull;
     if (c.tp_rank >= c.tp_size || c.pp_rank >= c.pp_size || c.staging_depth > kMaxDepth ||
         c.sync_mode > PHX_SYNC_RELAXED || c.restore_mode > PHX_RESTORE_BULK_KERNEL || !(c.max_grad_norm == c.max_grad_norm) ||
-        c.snapshot_source > PHX_SNAPSHOT_DIRECT ||
+        c.snapshot_source > PHX_SNAPSHOT_DIRECT || c.precision > PHX_PRECISION_FP32 ||
         (c.snapshot_source == PHX_SNAPSHOT_DIRECT && c.sync_mode != PHX_SYNC_STRICT)) {
         delete s;
         return PHX_ERR_INVALID_ARG;
@@ -241,7 +294,7 @@ int phx_shard_create(const phx_tensor_desc_t *layout, size_t n_tensors, uint32_t
     for (const auto &t : s->layout) {
         const uint64_t t1 = t0 + t.numel;
         const uint64_t lo = t0 > begin ? t0 : begin, hi = t1 < end ? t1 : end;
-        if (hi > lo) s->segments.push_back(Segment{t.tensor_id, lo - t0, lo - begin, hi - lo});
+        if (hi > lo) s->segments.push_back(Segment{t.tensor_id, lo - t0, lo - begin, hi - lo, t.flags});
         t0 = t1;
     }
     // layout hash: per tensor (numel u64, tensor_id u32, flags u32), then dp_size, tp_size, tp_rank, pp_size, pp_rank
@@ -268,6 +321,7 @@ int phx_shard_create(const phx_tensor_desc_t *layout, size_t n_tensors, uint32_t
     i.staging_depth = c.snapshot_source == PHX_SNAPSHOT_DIRECT ? 0 : c.staging_depth;
     i.dp_size = dp_size;
     i.dp_rank = dp_rank;
+    build_decay_groups(s);
     *out = s;
     return PHX_OK;
 }
@@ -284,6 +338,7 @@ int phx_shard_destroy(phx_shard_t *s)
         for (int k = 0; k < 2; ++k)
             if (s->ev_host[k]) cudaEventDestroy(s->ev_host[k]);
         if (s->d_scratch) cudaFree(s->d_scratch);
+        if (s->d_decay) cudaFree(s->d_decay);
     }
     delete s;
     return PHX_OK;
@@ -313,7 +368,7 @@ int phx_shard_segments(const phx_shard_t *s, uint32_t *tensor_id, uint64_t *off_
 int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p_bf16, void *d_staging,
                    void *h_replica)
 {
-    if (!s || !d_p || !d_m || !d_v || !d_p_bf16) return PHX_ERR_INVALID_ARG;
+    if (!s || !d_p || !d_m || !d_v || (!d_p_bf16 && !fp32_mode(s))) return PHX_ERR_INVALID_ARG;
     if (snapshots_on(s) && (!h_replica || (!d_staging && !direct_mode(s)))) return PHX_ERR_INVALID_ARG;
     if (!aligned256(d_p) || !aligned256(d_m) || !aligned256(d_v) || !aligned256(d_p_bf16) || !aligned256(d_staging) ||
         !aligned256(h_replica))
@@ -346,6 +401,12 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
         PHX_CK(cudaEventCreateWithFlags(&s->ev_flush[k], cudaEventDisableTiming));
     }
     for (int k = 0; k < 2; ++k) PHX_CK(cudaEventCreateWithFlags(&s->ev_host[k], cudaEventDisableTiming));
+    if (s->has_groups) {
+        const size_t nb = s->decay_bnd.size() * sizeof(uint64_t);
+        PHX_CK(cudaMalloc(reinterpret_cast<void **>(&s->d_decay), nb + s->decay_cls.size() + 8));
+        if (nb) PHX_CK(cudaMemcpy(s->d_decay, s->decay_bnd.data(), nb, cudaMemcpyHostToDevice));
+        PHX_CK(cudaMemcpy(s->d_decay + nb, s->decay_cls.data(), s->decay_cls.size(), cudaMemcpyHostToDevice));
+    }
 
     s->d_p = d_p;
     s->d_m = d_m;
@@ -361,8 +422,10 @@ int phx_shard_set_state(phx_shard_t *s, uint64_t step, void *stream)
 {
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound) return PHX_ERR_NOT_BOUND;
-    PHX_CK(phx::launch_regen_bf16(s->d_p, s->d_p16, s->info.n_padded, static_cast<cudaStream_t>(stream)));
-    s->launches += s->info.n_padded ? 1 : 0;
+    if (!fp32_mode(s)) {
+        PHX_CK(phx::launch_regen_bf16(s->d_p, s->d_p16, s->info.n_padded, static_cast<cudaStream_t>(stream)));
+        s->launches += s->info.n_padded ? 1 : 0;
+    }
     s->last_step = step;
     s->pending_slot = -1;
     return PHX_OK;
@@ -378,12 +441,12 @@ int phx_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len)
 }
 
 // ---- a1 + a2 + a3 --------------------------------------------------------------------------------
-int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads_bf16, float lr, float beta1, float beta2, float eps,
+int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float beta1, float beta2, float eps,
                           float wd, uint64_t step, void *stream)
 {
-    if (!s || !d_grads_bf16) return PHX_ERR_INVALID_ARG;
+    if (!s || !d_grads) return PHX_ERR_INVALID_ARG;
     if (!s->bound) return PHX_ERR_NOT_BOUND;
-    if (!aligned256(d_grads_bf16)) return PHX_ERR_ALIGNMENT;
+    if (!aligned256(d_grads)) return PHX_ERR_ALIGNMENT;
     if (step != s->last_step + 1) return PHX_ERR_STEP_ORDER;  // I4 step atomicity
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const bool snap = snapshots_on(s);
@@ -406,7 +469,7 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads_bf16, float lr, fl
     s->clip_valid = false;
     if (s->cfg.max_grad_norm > 0.0f) {
         int nl = 0;
-        PHX_CK(phx::launch_sumsq_clip(d_grads_bf16, s->info.n_padded, s->cfg.max_grad_norm,
+        PHX_CK(phx::launch_sumsq_clip(d_grads, fp32_mode(s), s->info.n_padded, s->cfg.max_grad_norm,
                                       reinterpret_cast<double *>(s->d_scratch + kScrPartials),
                                       reinterpret_cast<double *>(s->d_scratch + kScrSumsq),
                                       reinterpret_cast<float *>(s->d_scratch + kScrCoef), st, &nl));
@@ -440,12 +503,18 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads_bf16, float lr, fl
     a.p = s->d_p;
     a.m = s->d_m;
     a.v = s->d_v;
-    a.g = d_grads_bf16;
+    a.g = d_grads;
     a.p16 = s->d_p16;
     a.n_padded = s->info.n_padded;
+    if (s->has_groups) {
+        a.decay_bnd = reinterpret_cast<const uint64_t *>(s->d_decay);
+        a.decay_cls = s->d_decay + s->decay_bnd.size() * sizeof(uint64_t);
+        a.n_bnd = (uint32_t)s->decay_bnd.size();
+        a.first_nodecay = s->first_nodecay;
+    }
 
     // a3: one kernel, one pass
-    PHX_CK(phx::launch_step(a, snap && !direct_mode(s), s->variant, st));
+    PHX_CK(phx::launch_step(a, snap && !direct_mode(s), s->variant, step_mode(s), st));
     s->launches += s->info.n_padded ? 1 : 0;
     if (snap) {
         PHX_CK(cudaEventRecord(s->ev_step[slot], st));
@@ -577,15 +646,18 @@ int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
     const uint64_t N = s->info.n_padded;
     const uint64_t off = (uint64_t)best * s->info.slot_stride + kHeaderBytes;
     if (s->cfg.restore_mode == PHX_RESTORE_BULK_KERNEL) {
-        PHX_CK(phx::launch_restore_bulk(s->d_replica + off, s->d_p, s->d_m, s->d_v, s->d_p16, N, s->sm_count, st));
+        PHX_CK(phx::launch_restore_bulk(s->d_replica + off, s->d_p, s->d_m, s->d_v, fp32_mode(s) ? nullptr : s->d_p16, N,
+                                        s->sm_count, st));
         s->launches += N ? 1 : 0;
     } else {
         const uint8_t *src = s->h_replica + off;
         PHX_CK(cudaMemcpyAsync(s->d_p, src, 4 * N, cudaMemcpyHostToDevice, st));
         PHX_CK(cudaMemcpyAsync(s->d_m, src + 4 * N, 4 * N, cudaMemcpyHostToDevice, st));
         PHX_CK(cudaMemcpyAsync(s->d_v, src + 8 * N, 4 * N, cudaMemcpyHostToDevice, st));
-        PHX_CK(phx::launch_regen_bf16(s->d_p, s->d_p16, N, st));
-        s->launches += N ? 1 : 0;
+        if (!fp32_mode(s)) {
+            PHX_CK(phx::launch_regen_bf16(s->d_p, s->d_p16, N, st));
+            s->launches += N ? 1 : 0;
+        }
     }
     s->last_step = hdr[best].step;
     s->pending_slot = -1;
@@ -643,6 +715,7 @@ int phx_kernel_launches(const phx_shard_t *s, uint64_t *count)
 int phx_set_kernel_variant(phx_shard_t *s, uint32_t variant)
 {
     if (!s || variant >= phx::kNumStepVariants) return PHX_ERR_INVALID_ARG;
+    if (variant != 0 && step_mode(s) != 0) return PHX_ERR_INVALID_ARG;  // §8(f2) modes: default flavour only
     s->variant = variant;
     return PHX_OK;
 }

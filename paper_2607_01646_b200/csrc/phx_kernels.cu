@@ -4,6 +4,9 @@
 //                       Pure HBM streaming: 14 B/element read, 26 B/element written, one pass,
 //                       256-bit (LDG.E.256 / STG.E.256, new on sm_100) or 128-bit vectors,
 //                       streaming cache hints, no shared memory, no tensor cores (no contraction).
+//                       k_step8 MODE bits: kModeF32 = binary32 gradients and no bf16
+//                       copy (the paper's precision; 16 B read + 24 B written);
+//                       kModeGroups = per-tensor decay groups (no-decay tensors take decay 1.0f).
 //   k_sumsq_*         : a1, deterministic fp64 sum of squares + clip coefficient.
 //   k_regen_bf16      : p16 = RNE_bf16(p).
 //   k_restore_bulk    : a6, pulls the replica from mapped pinned host memory with 1-D bulk
@@ -94,6 +97,12 @@ __device__ __forceinline__ uint4 ldg128_stream(const void *ptr)
                  : "l"(ptr));
     return r;
 }
+__device__ __forceinline__ F8 ldg256_stream(const float *ptr)
+{
+    F8 r;
+    PHX_LD256(".nc.L1::no_allocate.L2::evict_first");
+    return r;
+}
 __device__ __forceinline__ uint2 ldg64_stream(const void *ptr)
 {
     uint2 r;
@@ -139,10 +148,10 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi)
 // One element of the canonical AdamW sequence (include/phx.h a3).  Each intrinsic is one
 // IEEE-754 binary32 operation, round-to-nearest-even; none can be contracted into an FMA.
 __device__ __forceinline__ void adamw_element(float &p, float &m, float &v, float g, float coef,
-                                              const AdamScalars &sc)
+                                              const AdamScalars &sc, float decay)
 {
     g = __fmul_rn(g, coef);
-    const float p1 = __fmul_rn(p, sc.decay);
+    const float p1 = __fmul_rn(p, decay);
     const float mn = __fadd_rn(__fmul_rn(sc.beta1, m), __fmul_rn(sc.omb1, g));
     const float vn = __fadd_rn(__fmul_rn(sc.beta2, v), __fmul_rn(sc.omb2, __fmul_rn(g, g)));
     const float d = __fadd_rn(__fdiv_rn(__fsqrt_rn(vn), sc.sbc2), sc.eps);
@@ -204,9 +213,25 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // ------------------------------------------------------------------------------------------
 constexpr int kStepThreads = 256;
 
-template <int HINT, int U, bool SNAP>
+// Decay groups (include/phx.h "decay groups"): cls[e >> kDecayTileShift] says whether the 2048-element
+// tile holding e is all-decay (0), all-no-decay (1) or mixed (2); in a mixed tile the flag of element
+// e is first_nodecay XOR (number of toggle offsets <= e), found by binary search.  Mixed tiles are
+// the few that contain a tensor boundary between a decayed and a no-decay tensor.
+__device__ __forceinline__ bool nodecay_at(uint64_t e, const uint64_t *__restrict__ bnd, uint32_t nb, uint32_t first)
+{
+    uint32_t lo = 0, hi = nb;
+    while (lo < hi) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (__ldg(bnd + mid) <= e) lo = mid + 1;
+        else hi = mid;
+    }
+    return ((first ^ lo) & 1u) != 0;
+}
+
+template <int HINT, int U, bool SNAP, int MODE>
 __global__ void __launch_bounds__(kStepThreads) k_step8(const __grid_constant__ StepArgs a)
 {
+    constexpr bool GF32 = (MODE & kModeF32) != 0, GROUPS = (MODE & kModeGroups) != 0;
     const uint64_t ngroups = a.n_padded >> 3;
     const uint64_t base = (uint64_t)blockIdx.x * (kStepThreads * U) + threadIdx.x;
     if (a.shdr != nullptr && blockIdx.x == 0 && threadIdx.x < 16)
@@ -215,12 +240,14 @@ __global__ void __launch_bounds__(kStepThreads) k_step8(const __grid_constant__ 
 
     F8 P[U], M[U], V[U];
     uint4 G[U];
+    F8 GF[GF32 ? U : 1];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
         const uint64_t gi = base + (uint64_t)u * kStepThreads;
         if (gi < ngroups) {
             const uint64_t e = gi << 3;
-            G[u] = ldg128_stream(reinterpret_cast<const uint16_t *>(a.g) + e);
+            if (GF32) GF[GF32 ? u : 0] = ldg256_stream(reinterpret_cast<const float *>(a.g) + e);
+            else G[u] = ldg128_stream(reinterpret_cast<const uint16_t *>(a.g) + e);
             P[u] = ld256<HINT>(a.p + e);
             M[u] = ld256<HINT>(a.m + e);
             V[u] = ld256<HINT>(a.v + e);
@@ -231,21 +258,42 @@ __global__ void __launch_bounds__(kStepThreads) k_step8(const __grid_constant__ 
         const uint64_t gi = base + (uint64_t)u * kStepThreads;
         if (gi < ngroups) {
             const uint64_t e = gi << 3;
-            const uint32_t gw[4] = {G[u].x, G[u].y, G[u].z, G[u].w};
+            float gv[8];
+            if (GF32) {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                adamw_element(P[u].x[2 * j], M[u].x[2 * j], V[u].x[2 * j], bf16lo(gw[j]), coef, a.sc);
-                adamw_element(P[u].x[2 * j + 1], M[u].x[2 * j + 1], V[u].x[2 * j + 1], bf16hi(gw[j]), coef, a.sc);
+                for (int j = 0; j < 8; ++j) gv[j] = GF[GF32 ? u : 0].x[j];
+            } else {
+                const uint32_t gw[4] = {G[u].x, G[u].y, G[u].z, G[u].w};
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    gv[2 * j] = bf16lo(gw[j]);
+                    gv[2 * j + 1] = bf16hi(gw[j]);
+                }
             }
-            uint4 h;
-            h.x = pack_bf16x2(P[u].x[0], P[u].x[1]);
-            h.y = pack_bf16x2(P[u].x[2], P[u].x[3]);
-            h.z = pack_bf16x2(P[u].x[4], P[u].x[5]);
-            h.w = pack_bf16x2(P[u].x[6], P[u].x[7]);
+            uint32_t cls = 0;
+            if (GROUPS) cls = __ldg(a.decay_cls + (e >> kDecayTileShift));
+            if (!GROUPS || cls != 2) {
+                const float decay = (GROUPS && cls == 1) ? 1.0f : a.sc.decay;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) adamw_element(P[u].x[j], M[u].x[j], V[u].x[j], gv[j], coef, a.sc, decay);
+            } else {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const float decay = nodecay_at(e + j, a.decay_bnd, a.n_bnd, a.first_nodecay) ? 1.0f : a.sc.decay;
+                    adamw_element(P[u].x[j], M[u].x[j], V[u].x[j], gv[j], coef, a.sc, decay);
+                }
+            }
             st256<HINT>(a.p + e, P[u]);
             st256<HINT>(a.m + e, M[u]);
             st256<HINT>(a.v + e, V[u]);
-            st128u<HINT>(reinterpret_cast<uint16_t *>(a.p16) + e, h);
+            if (!GF32) {
+                uint4 h;
+                h.x = pack_bf16x2(P[u].x[0], P[u].x[1]);
+                h.y = pack_bf16x2(P[u].x[2], P[u].x[3]);
+                h.z = pack_bf16x2(P[u].x[4], P[u].x[5]);
+                h.w = pack_bf16x2(P[u].x[6], P[u].x[7]);
+                st128u<HINT>(reinterpret_cast<uint16_t *>(a.p16) + e, h);
+            }
             if (SNAP) {
                 st256<HINT>(a.sp + e, P[u]);
                 st256<HINT>(a.sm + e, M[u]);
@@ -286,8 +334,8 @@ __global__ void __launch_bounds__(kStepThreads) k_step4(const __grid_constant__ 
             const uint32_t gw[2] = {G[u].x, G[u].y};
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-                adamw_element(P[u].x[2 * j], M[u].x[2 * j], V[u].x[2 * j], bf16lo(gw[j]), coef, a.sc);
-                adamw_element(P[u].x[2 * j + 1], M[u].x[2 * j + 1], V[u].x[2 * j + 1], bf16hi(gw[j]), coef, a.sc);
+                adamw_element(P[u].x[2 * j], M[u].x[2 * j], V[u].x[2 * j], bf16lo(gw[j]), coef, a.sc, a.sc.decay);
+                adamw_element(P[u].x[2 * j + 1], M[u].x[2 * j + 1], V[u].x[2 * j + 1], bf16hi(gw[j]), coef, a.sc, a.sc.decay);
             }
             uint2 h;
             h.x = pack_bf16x2(P[u].x[0], P[u].x[1]);
@@ -305,15 +353,15 @@ __global__ void __launch_bounds__(kStepThreads) k_step4(const __grid_constant__ 
     }
 }
 
-template <int HINT, int U>
+template <int HINT, int U, int MODE = 0>
 static cudaError_t launch8(const StepArgs &a, bool snapshot, cudaStream_t st)
 {
     const uint64_t ngroups = a.n_padded >> 3;
     const uint64_t per_block = (uint64_t)kStepThreads * U;
     const unsigned grid = (unsigned)((ngroups + per_block - 1) / per_block);
     if (grid == 0) return cudaSuccess;
-    if (snapshot) k_step8<HINT, U, true><<<grid, kStepThreads, 0, st>>>(a);
-    else k_step8<HINT, U, false><<<grid, kStepThreads, 0, st>>>(a);
+    if (snapshot) k_step8<HINT, U, true, MODE><<<grid, kStepThreads, 0, st>>>(a);
+    else k_step8<HINT, U, false, MODE><<<grid, kStepThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 template <int HINT, int U>
@@ -401,10 +449,10 @@ __global__ void __launch_bounds__(kStepThreads) k_step_tma(const __grid_constant
                 float4 M = *reinterpret_cast<float4 *>(t.m + e);
                 float4 V = *reinterpret_cast<float4 *>(t.v + e);
                 const uint2 G = *reinterpret_cast<const uint2 *>(t.g + e);
-                adamw_element(P.x, M.x, V.x, bf16lo(G.x), coef, a.sc);
-                adamw_element(P.y, M.y, V.y, bf16hi(G.x), coef, a.sc);
-                adamw_element(P.z, M.z, V.z, bf16lo(G.y), coef, a.sc);
-                adamw_element(P.w, M.w, V.w, bf16hi(G.y), coef, a.sc);
+                adamw_element(P.x, M.x, V.x, bf16lo(G.x), coef, a.sc, a.sc.decay);
+                adamw_element(P.y, M.y, V.y, bf16hi(G.x), coef, a.sc, a.sc.decay);
+                adamw_element(P.z, M.z, V.z, bf16lo(G.y), coef, a.sc, a.sc.decay);
+                adamw_element(P.w, M.w, V.w, bf16hi(G.y), coef, a.sc, a.sc.decay);
                 *reinterpret_cast<float4 *>(t.p + e) = P;
                 *reinterpret_cast<float4 *>(t.m + e) = M;
                 *reinterpret_cast<float4 *>(t.v + e) = V;
@@ -466,8 +514,17 @@ static cudaError_t launch_tma(const StepArgs &a, bool snapshot, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, cudaStream_t st)
+cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, uint32_t mode, cudaStream_t st)
 {
+    if (mode != 0) {  // §8(f2) modes exist for the default flavour only
+        if (variant != 0) return cudaErrorInvalidValue;
+        switch (mode) {
+        case kModeF32: return launch8<1, 1, kModeF32>(a, snapshot, st);
+        case kModeGroups: return launch8<1, 1, kModeGroups>(a, snapshot, st);
+        case kModeF32 | kModeGroups: return launch8<1, 1, kModeF32 | kModeGroups>(a, snapshot, st);
+        default: return cudaErrorInvalidValue;
+        }
+    }
     switch (variant) {
     case 0: return launch8<1, 1>(a, snapshot, st);  // 256-bit, streaming hints (default)
     case 1: return launch8<0, 1>(a, snapshot, st);  // 256-bit, no hints
@@ -534,6 +591,47 @@ __global__ void __launch_bounds__(256) k_sumsq_partial(const uint4 *__restrict__
     }
 }
 
+// binary32 gradients: the square of a widened fp32 value is exact in fp64 (48 bits),
+// so fma(x, x, acc) rounds exactly once, like a separate exact multiply and an add.
+__device__ __forceinline__ double sq_acc_f32(double acc, float g)
+{
+    const double x = (double)g;
+    return acc + x * x;
+}
+
+__global__ void __launch_bounds__(256) k_sumsq_partial_f32(const float *__restrict__ g, uint64_t ngroups,
+                                                           double *__restrict__ partials)
+{
+    double acc = 0.0;
+    const uint64_t stride = (uint64_t)gridDim.x * 256;
+    uint64_t gi = (uint64_t)blockIdx.x * 256 + threadIdx.x;
+    for (; gi + stride < ngroups; gi += 2 * stride) {
+        F8 w[2];
+#pragma unroll
+        for (int k = 0; k < 2; ++k) w[k] = ldg256_stream(g + ((gi + k * stride) << 3));
+#pragma unroll
+        for (int k = 0; k < 2; ++k)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) acc = sq_acc_f32(acc, w[k].x[j]);
+    }
+    for (; gi < ngroups; gi += stride) {
+        const F8 w = ldg256_stream(g + (gi << 3));
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc = sq_acc_f32(acc, w.x[j]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+    __shared__ double wsum[8];
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = wsum[0];
+#pragma unroll
+        for (int k = 1; k < 8; ++k) s += wsum[k];
+        partials[blockIdx.x] = s;
+    }
+}
+
 __global__ void __launch_bounds__(kSumsqMaxBlocks) k_sumsq_final(const double *__restrict__ partials, int nblocks,
                                                                  float max_norm, double *__restrict__ out_sumsq,
                                                                  float *__restrict__ out_coef)
@@ -554,14 +652,15 @@ __global__ void __launch_bounds__(kSumsqMaxBlocks) k_sumsq_final(const double *_
     }
 }
 
-cudaError_t launch_sumsq_clip(const void *g_bf16, uint64_t n_padded, float max_norm, double *partials,
+cudaError_t launch_sumsq_clip(const void *g, bool grads_f32, uint64_t n_padded, float max_norm, double *partials,
                               double *out_sumsq, float *out_coef, cudaStream_t st, int *n_launches)
 {
     const uint64_t ngroups = n_padded >> 3;
     uint64_t want = (ngroups + 255) / 256;
     int nblocks = (int)(want < 592 ? want : 592);  // 148 SMs x 4; fixed by n alone
     if (nblocks < 1) nblocks = 1;
-    k_sumsq_partial<<<nblocks, 256, 0, st>>>(reinterpret_cast<const uint4 *>(g_bf16), ngroups, partials);
+    if (grads_f32) k_sumsq_partial_f32<<<nblocks, 256, 0, st>>>(reinterpret_cast<const float *>(g), ngroups, partials);
+    else k_sumsq_partial<<<nblocks, 256, 0, st>>>(reinterpret_cast<const uint4 *>(g), ngroups, partials);
     k_sumsq_final<<<1, kSumsqMaxBlocks, 0, st>>>(partials, nblocks, max_norm, out_sumsq, out_coef);
     if (n_launches) *n_launches = 2;
     return cudaGetLastError();
@@ -655,7 +754,7 @@ __global__ void __launch_bounds__(kRestoreThreads) k_restore_bulk(const float *_
         }
         // bf16 copy: 8 elements per thread, conflict-free 128-bit shared loads
         const uint32_t e = threadIdx.x * 8;
-        if (e < cnt) {
+        if (p16 != nullptr && e < cnt) {
             const float4 a = *reinterpret_cast<const float4 *>(tp + e);
             const float4 b = *reinterpret_cast<const float4 *>(tp + e + 4);
             uint4 h;

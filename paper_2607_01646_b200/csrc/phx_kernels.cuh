@@ -19,30 +19,39 @@ struct alignas(16) HeaderBlob {
 
 struct StepArgs {
     float *p, *m, *v;            // live planes, n_padded each
-    const void *g;               // bf16 grads
-    void *p16;                   // bf16 param copy
+    const void *g;               // bf16 grads (float grads under kModeF32)
+    void *p16;                   // bf16 param copy (unused under kModeF32)
     float *sp, *sm, *sv;         // staging planes of the slot being written (null if !snapshot)
     void *shdr;                  // where block 0 stores the 256-B header (null: no header)
     const float *coef;           // device scalar: clip coefficient (1.0f when clipping is off)
     uint64_t n_padded;           // multiple of 64
+    // decay groups (kModeGroups): class per 2048-element tile, toggle offsets, flag before the first toggle
+    const uint8_t *decay_cls;
+    const uint64_t *decay_bnd;
+    uint32_t n_bnd, first_nodecay;
     AdamScalars sc;
     HeaderBlob hdr;
 };
 
 enum { kNumStepVariants = 12 };
+// SURVEY §8(f2) modes of the fused step (default flavour only): binary32 gradients without a bf16
+// copy (the paper's precision) and per-tensor decay groups.
+enum { kModeF32 = 1, kModeGroups = 2 };
+enum { kDecayTileShift = 11 };  // decay_cls granularity: 2048 elements
 
 // a3.  variant selects the kernel flavour (see phx_kernels.cu); snapshot=false drops the staging stores.
-cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, cudaStream_t st);
+cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, uint32_t mode, cudaStream_t st);
 
 // a1.  partials: >= kSumsqMaxBlocks doubles of device scratch; out_sumsq/out_coef device scalars.
 enum { kSumsqMaxBlocks = 1024 };
-cudaError_t launch_sumsq_clip(const void *g_bf16, uint64_t n_padded, float max_norm, double *partials,
+cudaError_t launch_sumsq_clip(const void *g, bool grads_f32, uint64_t n_padded, float max_norm, double *partials,
                               double *out_sumsq, float *out_coef, cudaStream_t st, int *n_launches);
 
 // p16 = RNE_bf16(p)
 cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cudaStream_t st);
 
-// a6, bulk-kernel mode: src_payload = device-visible address of the host slot's payload (p ‖ m ‖ v).
+// a6, bulk-kernel mode: src_payload = device-visible address of the host slot's payload (p ‖ m ‖ v);
+// p16 == nullptr skips the bf16 regeneration (kModeF32 shards have no bf16 copy).
 cudaError_t launch_restore_bulk(const void *src_payload, float *p, float *m, float *v, void *p16,
                                 uint64_t n_padded, int sm_count, cudaStream_t st);
 

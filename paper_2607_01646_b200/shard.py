@@ -27,7 +27,9 @@ class Shard:
             wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank), pp=(wl.pp_size, wl.pp_rank),
             staging_depth=staging_depth, sync_mode=sync_mode, chunk_bytes=chunk_bytes,
             snapshot_disabled=not snapshot, restore_mode=restore_mode, max_grad_norm=mgn,
-            snapshot_source=snapshot_source)
+            snapshot_source=snapshot_source, flags=wl.flags(),
+            precision=B.PHX_PRECISION_FP32 if wl.precision == "fp32" else B.PHX_PRECISION_BF16_GRADS)
+        self.fp32 = wl.precision == "fp32"
         self.info = B.phx_shard_info(self.h)
         self.n, self.n_padded = self.info.n, self.info.n_padded
         self.segments = [(tid, off_s, ln) for tid, _, off_s, ln in B.phx_shard_segments(self.h)]
@@ -36,7 +38,8 @@ class Shard:
             self.p = torch.zeros(N, dtype=torch.float32, device=self.device)
             self.m = torch.zeros(N, dtype=torch.float32, device=self.device)
             self.v = torch.zeros(N, dtype=torch.float32, device=self.device)
-            self.p16 = torch.zeros(N, dtype=torch.bfloat16, device=self.device)
+            # no bf16 model-param copy in the all-FP32 precision
+            self.p16 = None if self.fp32 else torch.zeros(N, dtype=torch.bfloat16, device=self.device)
             self.staging = None
             self.replica = None
             if snapshot:
@@ -55,7 +58,8 @@ class Shard:
 
     def step_and_snapshot(self, grads: torch.Tensor, step: int, stream=None, hyper: Optional[Hyper] = None):
         hp = hyper or self.hyper
-        assert grads.dtype == torch.bfloat16 and grads.numel() == self.n_padded and grads.is_cuda
+        assert grads.dtype == (torch.float32 if self.fp32 else torch.bfloat16)
+        assert grads.numel() == self.n_padded and grads.is_cuda
         B.phx_step_and_snapshot(self.h, grads, hp.lr, hp.beta1, hp.beta2, hp.eps, hp.wd, step,
                                 stream or torch.cuda.current_stream(self.device))
 
@@ -80,7 +84,8 @@ class Shard:
         """'Drop the live shard' (BASELINE.json:configs[3]): zero p, m, v, bf16 copy and scribble
         over the device staging ring — restore must not depend on anything device-resident."""
         for t in (self.p, self.m, self.v, self.p16):
-            t.zero_()
+            if t is not None:
+                t.zero_()
         if self.staging is not None:
             self.staging.fill_(0xA5)
 

@@ -143,6 +143,9 @@ class Workload:
     scale_per: str = "group"   # "tensor" | "group" : granularity of the U[0.5,2] scale
     n_expected: int = 0        # per-rank fp32 elements the config text / Appendix C states
     seed: int = 0
+    decay_groups: bool = False  # biases and norm weights are flagged no-decay
+    precision: str = "bf16"     # "bf16": bf16 grads + bf16 copy (north_star); "fp32": the paper's
+    no_decay_ids: Tuple[int, ...] = ()  # extra tensor indices flagged no-decay (ad-hoc test workloads)
 
     @property
     def total_numel(self) -> int:
@@ -151,6 +154,13 @@ class Workload:
     def layout(self) -> List[Tuple[int, int]]:
         """[(numel, tensor_id)] in list order — the argument of phx_shard_create / the oracle's a0."""
         return [(t.numel, i) for i, t in enumerate(self.tensors)]
+
+    def flags(self) -> List[int]:
+        """Per-tensor flags for phx_tensor_desc_t.flags / the oracle's a0: bit 0 (no decay) on biases
+        and normalisation weights when decay_groups is on (the usual AdamW parameter groups)."""
+        nd = ("bias", "ln1.", "ln2.", "final_ln.", "norm.") if self.decay_groups else ()
+        return [1 if (i in self.no_decay_ids or any(k in t.name for k in nd)) else 0
+                for i, t in enumerate(self.tensors)]
 
 
 def _mk() -> dict:
@@ -234,8 +244,10 @@ def gen_grads(
     seed: int = 0,
     device="cpu",
     chunk: int = 1 << 26,
+    dtype: torch.dtype = torch.bfloat16,
 ) -> torch.Tensor:
-    """bf16 gradients for one step, already reduce-scattered to this rank's shard.
+    """Gradients for one step, already reduce-scattered to this rank's shard: bf16 (default) or
+    float32 (`dtype`, the paper's all-FP32 setting, PAPER.md:270 — the same draws, not cast down).
 
     'normal'     : N(0, 1e-3) times the tensor's U[0.5,2] scale.
     'heavy_tail' : the same, except a Bernoulli(0.01) subset is 1e-3 * Student-t(df=3)
@@ -245,7 +257,7 @@ def gen_grads(
     """
     scales = group_scales(wl, seed)
     gen = _gen(seed * 2_654_435_761 + 1_000_000_007 * (step + 1), device)
-    out = torch.zeros(n_padded, dtype=torch.bfloat16, device=device)
+    out = torch.zeros(n_padded, dtype=dtype, device=device)
     for tid, off, length in segments:
         s = 1e-3 * scales[tid]
         for c0 in range(0, length, chunk):
@@ -259,5 +271,5 @@ def gen_grads(
                     chi = torch.randn(3, k, generator=gen, dtype=torch.float32, device=device)
                     den = torch.sqrt((chi * chi).sum(0) / 3.0)
                     z[mask] = num / den
-            out[off + c0: off + c0 + c] = (z * s).to(torch.bfloat16)
+            out[off + c0: off + c0 + c] = (z * s).to(dtype)
     return out

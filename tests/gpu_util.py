@@ -17,13 +17,19 @@ def bits16(t: torch.Tensor) -> np.ndarray:
     return t.detach().cpu().view(torch.int16).numpy().view(np.uint16)
 
 
+def grad_record(g: torch.Tensor) -> np.ndarray:
+    """The oracle's view of a gradient tensor: bf16 bits, or the float32 values themselves."""
+    return g.detach().cpu().numpy().copy() if g.dtype == torch.float32 else bits16(g).copy()
+
+
 def make_pair(wl, *, steps, grads=None, chunk_bytes=8 << 20, user=b"", init_mv=False, **shard_kw):
     """(Shard, OracleShard, [grad tensors on GPU], [grad bits for the oracle]) with equal initial state."""
     s = Shard(wl, device=DEV, chunk_bytes=chunk_bytes, **shard_kw)
     mgn = shard_kw.get("max_grad_norm", None)
     o = O.OracleShard(wl.layout(), wl.dp_size, wl.dp_rank, (wl.tp_size, wl.tp_rank), (wl.pp_size, wl.pp_rank),
                       chunk_bytes=(chunk_bytes + 255) & ~255,  # the library rounds chunks up to 256 B
-                      max_grad_norm=wl.hyper.max_grad_norm if mgn is None else mgn, user=user)
+                      max_grad_norm=wl.hyper.max_grad_norm if mgn is None else mgn, user=user,
+                      flags=wl.flags(), precision=wl.precision)
     assert (o.n, o.n_padded) == (s.n, s.n_padded)
     osegs = [(tid, off, ln) for tid, _, off, ln in o.segments]
     assert osegs == s.segments
@@ -43,9 +49,10 @@ def make_pair(wl, *, steps, grads=None, chunk_bytes=8 << 20, user=b"", init_mv=F
     if user:
         B.phx_set_user_metadata(s.h, user)
     if grads is None:
-        grads = [W.gen_grads(wl, osegs, s.n_padded, t, wl.seed) for t in range(1, steps + 1)]
+        gdt = torch.float32 if wl.precision == "fp32" else torch.bfloat16
+        grads = [W.gen_grads(wl, osegs, s.n_padded, t, wl.seed, dtype=gdt) for t in range(1, steps + 1)]
     gdev = [g.to(DEV) for g in grads]
-    gbits = [bits16(g).copy() for g in grads]
+    gbits = [grad_record(g) for g in grads]
     torch.cuda.synchronize()
     return s, o, gdev, gbits
 
@@ -59,10 +66,11 @@ def assert_state_equal(s: Shard, o: O.OracleShard, what=""):
             bad = np.flatnonzero(got != exp)
             raise AssertionError(f"{what}: {name} differs at {bad.size} of {exp.size} lanes, first {bad[:5]}: "
                                  f"{got[bad[:3]]} vs {exp[bad[:3]]}")
-    got = bits16(s.p16)
-    if not np.array_equal(got, o.p16):
-        bad = np.flatnonzero(got != o.p16)
-        raise AssertionError(f"{what}: p16 differs at {bad.size} lanes, first {bad[:5]}")
+    if s.p16 is not None:
+        got = bits16(s.p16)
+        if not np.array_equal(got, o.p16):
+            bad = np.flatnonzero(got != o.p16)
+            raise AssertionError(f"{what}: p16 differs at {bad.size} lanes, first {bad[:5]}")
     assert B.phx_last_step(s.h) == o.last_step, what
 
 
