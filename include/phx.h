@@ -163,8 +163,10 @@ PHX_API int phx_shard_segments(const phx_shard_t *s, uint32_t *tensor_id, uint64
 
 /* ---- binding memory -----------------------------------------------------------------------
  * d_staging: staging_depth * slot_stride bytes of device memory (may be NULL iff snapshots are
- * disabled or snapshot_source is PHX_SNAPSHOT_DIRECT).  h_replica: 2 * slot_stride bytes of pinned, mapped host memory (may be NULL iff
- * snapshots are disabled).  Requires a CUDA device of compute capability 10.x. */
+ * disabled or snapshot_source is PHX_SNAPSHOT_DIRECT).  h_replica: 2 * slot_stride bytes of pinned, mapped
+ * host memory (may be NULL if snapshots are disabled or only peer replicas are used, see
+ * phx_shard_bind_peers; phx_snapshot_flush_async / phx_restore then return PHX_ERR_NOT_BOUND).
+ * Requires a CUDA device of compute capability 10.x. */
 /* d_p_bf16 may be NULL iff precision is PHX_PRECISION_FP32. */
 PHX_API int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p_bf16,
                            void *d_staging, void *h_replica);
@@ -230,6 +232,59 @@ PHX_API int phx_fault_inject_torn_flush(phx_shard_t *s, int64_t payload_chunks);
 PHX_API int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step);
 /* Copies the user blob of the slot the last phx_restore used. */
 PHX_API int phx_restored_user_metadata(const phx_shard_t *s, void *blob, uint32_t cap, uint32_t *len);
+
+/* ---- peer replication around the data-parallel ring ------------------------
+ * The paper's H2H phase: the packed optimizer snapshot (envelope ‖ p ‖ m ‖ v — no
+ * model parameters) is sent to the ring peer, "the rank sharing the same
+ * tensor-parallel and pipeline-parallel positions but with a different data-parallel index"; with
+ * multi-peer replication to k distinct DP peers.  On a B200 NVLink 5 / NVSwitch box the
+ * peer's memory is reached directly: the peer process allocates a RECEIVED BUFFER (two snapshot slots at
+ * slot_stride, "committed / receiving", Fig. 5, 224) in its GPU's HBM, exports it over CUDA
+ * IPC, and the owner's copy engine writes the staging slot (or, in PHX_SNAPSHOT_DIRECT, the live planes)
+ * into it over NVLink on a dedicated stream — same protocol as the local pair: header invalidated,
+ * payload in chunk_bytes pieces, valid header last, slot = step mod 2.  No SM is involved and nothing is
+ * added to the critical path; pushing the snapshot stores themselves over NVLink from the fused kernel
+ * would put 12 B/element at ~0.9 TB/s (2.2 ms at c2) on it instead of 0.3 ms.
+ * The sync point of phx_step_and_snapshot (a2) also waits for the peer flush: "guarantees the
+ * peer-resident replica is fully committed before the optimizer mutates the protected state"
+ * (PAPER.md:226). */
+#define PHX_MAX_PEERS 4
+#define PHX_IPC_HANDLE_BYTES 64
+/* Ring peer j of rank r: (r + j) mod dp_size; j = 1..k are the ranks that hold r's replicas, j = -1..-k the
+ * ranks whose replicas r holds.  |j| must be in [1, dp_size - 1] (k distinct peers need k <= D - 1). */
+PHX_API int phx_ring_peer(uint32_t dp_size, uint32_t dp_rank, int32_t j, uint32_t *peer);
+/* Received-buffer memory: a zeroed device allocation of its own (cudaMalloc), so that it can be exported
+ * over CUDA IPC; owned by the caller, freed with phx_peer_buffer_free. */
+PHX_API int phx_peer_buffer_alloc(uint64_t bytes, void **d_buf);
+PHX_API int phx_peer_buffer_free(void *d_buf);
+/* CUDA IPC plumbing (cudaIpcGetMemHandle / cudaIpcOpenMemHandle with lazy peer access / Close): export a
+ * buffer allocated with phx_peer_buffer_alloc; open it in ANOTHER process of the same node. */
+PHX_API int phx_ipc_export(void *d_buf, uint8_t handle[PHX_IPC_HANDLE_BYTES]);
+PHX_API int phx_ipc_open(const uint8_t handle[PHX_IPC_HANDLE_BYTES], void **d_buf);
+PHX_API int phx_ipc_close(void *d_buf);
+/* d_peer_replicas[j-1]: device-addressable address of the received buffer (2 * slot_stride bytes) that ring
+ * peer j keeps for this rank; k <= min(PHX_MAX_PEERS, dp_size - 1) distinct buffers; k = 0 unbinds.
+ * h_replica of phx_shard_bind may be NULL when only peers are used. */
+PHX_API int phx_shard_bind_peers(phx_shard_t *s, void *const *d_peer_replicas, uint32_t k);
+/* Enqueues on `peer_stream` the replication of the newest snapshot to all k peers (one after the other: the
+ * source GPU's NVLink egress is the shared limit).  Independent of phx_snapshot_flush_async: either or both
+ * may be called after a step, on different streams, and overlap (PCIe and NVLink are separate links). */
+PHX_API int phx_snapshot_flush_peers_async(phx_shard_t *s, void *peer_stream);
+/* Host-blocking wait until the peer replication of `step` is committed on every peer. */
+PHX_API int phx_snapshot_wait_peers(phx_shard_t *s, uint64_t step);
+/* Fault injection: the NEXT replication to ring peer `peer_j` (1-based) stops after
+ * `payload_chunks` payload chunks and never commits. */
+PHX_API int phx_fault_inject_torn_peer_flush(phx_shard_t *s, uint32_t peer_j, int64_t payload_chunks);
+/* What a replica buffer (device, peer-mapped or pinned host memory) holds: both headers and whether each
+ * passes the commit rule.  Host-blocking.  A holder uses it to answer "which logical shard, which step"
+ * when sources and replacements are matched by logical shard identity. */
+PHX_API int phx_replica_inspect(const void *replica, uint64_t slot_stride, phx_snapshot_header_t out[2], int valid[2]);
+/* a6 from a replica held elsewhere (recovery stage 3: "optimizer state is restored from
+ * in-memory replicas"): `replica` is any device-accessible address of two snapshot slots — the surviving
+ * holder's received buffer opened over IPC, a device buffer, or pinned mapped host memory.  Same slot
+ * selection, identity check, restore modes and postconditions as phx_restore; reads the two headers with a
+ * blocking copy. */
+PHX_API int phx_restore_from(phx_shard_t *s, const void *replica, void *stream, uint64_t *restored_step);
 
 /* ---- introspection ---------------------------------------------------------------------- */
 PHX_API int phx_last_step(const phx_shard_t *s, uint64_t *step);

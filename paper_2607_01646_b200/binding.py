@@ -58,6 +58,20 @@ class phx_shard_info_t(C.Structure):
                 ("dp_size", C.c_uint32), ("dp_rank", C.c_uint32)]
 
 
+class phx_snapshot_header_t(C.Structure):
+    _fields_ = [("magic", C.c_uint8 * 8), ("version", C.c_uint32), ("header_bytes", C.c_uint32),
+                ("seq_begin", C.c_uint64), ("step", C.c_uint64), ("n", C.c_uint64), ("n_padded", C.c_uint64),
+                ("total_numel", C.c_uint64), ("shard_begin", C.c_uint64), ("layout_hash", C.c_uint64),
+                ("dp_size", C.c_uint32), ("dp_rank", C.c_uint32), ("tp_size", C.c_uint32), ("tp_rank", C.c_uint32),
+                ("pp_size", C.c_uint32), ("pp_rank", C.c_uint32), ("chunk_bytes", C.c_uint64),
+                ("user_len", C.c_uint32), ("reserved", C.c_uint32), ("user", C.c_uint8 * 128),
+                ("header_hash", C.c_uint64), ("seq_end", C.c_uint64)]
+
+
+PHX_MAX_PEERS = 4
+PHX_IPC_HANDLE_BYTES = 64
+
+
 class PhxError(RuntimeError):
     def __init__(self, code: int, where: str, cuda: int = 0):
         self.code, self.cuda = code, cuda
@@ -93,6 +107,18 @@ PROTOTYPES = {
     "phx_last_clip": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)]),
     "phx_kernel_launches": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_set_kernel_variant": (C.c_int, [C.c_void_p, C.c_uint32]),
+    "phx_ring_peer": (C.c_int, [C.c_uint32, C.c_uint32, C.c_int32, C.POINTER(C.c_uint32)]),
+    "phx_peer_buffer_alloc": (C.c_int, [C.c_uint64, C.POINTER(C.c_void_p)]),
+    "phx_peer_buffer_free": (C.c_int, [C.c_void_p]),
+    "phx_ipc_export": (C.c_int, [C.c_void_p, C.c_char_p]),
+    "phx_ipc_open": (C.c_int, [C.c_char_p, C.POINTER(C.c_void_p)]),
+    "phx_ipc_close": (C.c_int, [C.c_void_p]),
+    "phx_shard_bind_peers": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.c_uint32]),
+    "phx_snapshot_flush_peers_async": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "phx_snapshot_wait_peers": (C.c_int, [C.c_void_p, C.c_uint64]),
+    "phx_fault_inject_torn_peer_flush": (C.c_int, [C.c_void_p, C.c_uint32, C.c_int64]),
+    "phx_replica_inspect": (C.c_int, [C.c_void_p, C.c_uint64, C.POINTER(phx_snapshot_header_t), C.POINTER(C.c_int)]),
+    "phx_restore_from": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_uint64)]),
 }
 
 
@@ -251,3 +277,71 @@ def phx_set_kernel_variant(h: int, variant: int) -> None:
 
 def phx_version() -> int:
     return lib().phx_version()
+
+
+# ---- SURVEY.md §8(f1): peer replication ------------------------------------------------------
+
+
+def phx_ring_peer(dp_size: int, dp_rank: int, j: int) -> int:
+    out = C.c_uint32()
+    _ck(lib().phx_ring_peer(dp_size, dp_rank, j, C.byref(out)), "phx_ring_peer")
+    return out.value
+
+
+def phx_peer_buffer_alloc(nbytes: int) -> int:
+    p = C.c_void_p()
+    _ck(lib().phx_peer_buffer_alloc(nbytes, C.byref(p)), "phx_peer_buffer_alloc")
+    return p.value
+
+
+def phx_peer_buffer_free(d_buf: int) -> None:
+    _ck(lib().phx_peer_buffer_free(d_buf), "phx_peer_buffer_free")
+
+
+def phx_ipc_export(d_buf: int) -> bytes:
+    buf = C.create_string_buffer(PHX_IPC_HANDLE_BYTES)
+    _ck(lib().phx_ipc_export(d_buf, buf), "phx_ipc_export")
+    return buf.raw
+
+
+def phx_ipc_open(handle: bytes) -> int:
+    assert len(handle) == PHX_IPC_HANDLE_BYTES
+    p = C.c_void_p()
+    _ck(lib().phx_ipc_open(handle, C.byref(p)), "phx_ipc_open")
+    return p.value
+
+
+def phx_ipc_close(d_buf: int) -> None:
+    _ck(lib().phx_ipc_close(d_buf), "phx_ipc_close")
+
+
+def phx_shard_bind_peers(h: int, d_peer_replicas: Sequence) -> None:
+    k = len(d_peer_replicas)
+    arr = (C.c_void_p * max(k, 1))(*[_ptr(x) for x in d_peer_replicas])
+    _ck(lib().phx_shard_bind_peers(h, arr, k), "phx_shard_bind_peers", h)
+
+
+def phx_snapshot_flush_peers_async(h: int, peer_stream=None) -> None:
+    _ck(lib().phx_snapshot_flush_peers_async(h, _ptr(peer_stream)), "phx_snapshot_flush_peers_async", h)
+
+
+def phx_snapshot_wait_peers(h: int, step: int) -> None:
+    _ck(lib().phx_snapshot_wait_peers(h, step), "phx_snapshot_wait_peers", h)
+
+
+def phx_fault_inject_torn_peer_flush(h: int, peer_j: int, payload_chunks: int) -> None:
+    _ck(lib().phx_fault_inject_torn_peer_flush(h, peer_j, payload_chunks), "phx_fault_inject_torn_peer_flush", h)
+
+
+def phx_replica_inspect(replica, slot_stride: int):
+    """[(header, valid)] for the two slots of a replica buffer (device, peer-mapped or pinned host)."""
+    hdr = (phx_snapshot_header_t * 2)()
+    valid = (C.c_int * 2)()
+    _ck(lib().phx_replica_inspect(_ptr(replica), slot_stride, hdr, valid), "phx_replica_inspect")
+    return [(hdr[i], bool(valid[i])) for i in range(2)]
+
+
+def phx_restore_from(h: int, replica, stream=None) -> int:
+    st = C.c_uint64()
+    _ck(lib().phx_restore_from(h, _ptr(replica), _ptr(stream), C.byref(st)), "phx_restore_from", h)
+    return st.value

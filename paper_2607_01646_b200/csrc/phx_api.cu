@@ -89,6 +89,7 @@ struct phx_shard {
     uint32_t user_len = 0;
     uint8_t restored_user[128] = {0};
     uint32_t restored_user_len = 0;
+    uint64_t restore_hdr_step[2] = {0, 0};
     // staging ring / flush bookkeeping
     cudaEvent_t ev_step[kMaxDepth] = {nullptr, nullptr, nullptr, nullptr};
     cudaEvent_t ev_flush[kMaxDepth] = {nullptr, nullptr, nullptr, nullptr};
@@ -99,6 +100,17 @@ struct phx_shard {
     int pending_slot = -1;     // staging slot holding a snapshot that has not been flushed
     uint64_t pending_step = 0;
     int64_t torn_chunks = -1;
+    // §8(f1) peer replication: k device-addressable received buffers on the ring successors
+    uint32_t n_peers = 0;
+    uint8_t *d_peer[PHX_MAX_PEERS] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev_pflush[kMaxDepth] = {nullptr, nullptr, nullptr, nullptr};
+    bool pflush_valid[kMaxDepth] = {false, false, false, false};
+    cudaEvent_t ev_peer[2] = {nullptr, nullptr};
+    HostSlot peer[2];              // bookkeeping of the peers' slot `step mod 2` (all k peers as one unit)
+    int last_pflush_slot = -1;
+    int pending_peer_slot = -1;
+    uint64_t pending_peer_step = 0;
+    int64_t torn_peer_chunks[PHX_MAX_PEERS] = {-1, -1, -1, -1};
     // misc
     int last_cuda_error = 0;
     uint64_t launches = 0;
@@ -213,12 +225,12 @@ bool direct_mode(const phx_shard *s) { return s->cfg.snapshot_source == PHX_SNAP
 uint32_t ring_depth(const phx_shard *s) { return direct_mode(s) ? 2u : s->cfg.staging_depth; }
 
 // settle the bookkeeping of host slots whose flush event has completed (block=true waits for it)
-int settle_host_slots(phx_shard *s, bool block)
+int settle_slots(phx_shard *s, HostSlot *slots, cudaEvent_t *evs, bool block)
 {
     for (int i = 0; i < 2; ++i) {
-        HostSlot &h = s->host[i];
+        HostSlot &h = slots[i];
         if (h.state != SLOT_INFLIGHT && h.state != SLOT_TORN_INFLIGHT) continue;
-        cudaError_t e = block ? cudaEventSynchronize(s->ev_host[i]) : cudaEventQuery(s->ev_host[i]);
+        cudaError_t e = block ? cudaEventSynchronize(evs[i]) : cudaEventQuery(evs[i]);
         if (e == cudaErrorNotReady) continue;
         if (e != cudaSuccess) {
             s->last_cuda_error = (int)e;
@@ -226,6 +238,50 @@ int settle_host_slots(phx_shard *s, bool block)
         }
         h.state = h.state == SLOT_INFLIGHT ? SLOT_COMMITTED : SLOT_TORN;
     }
+    return PHX_OK;
+}
+int settle_host_slots(phx_shard *s, bool block) { return settle_slots(s, s->host, s->ev_host, block); }
+int settle_peer_slots(phx_shard *s, bool block) { return settle_slots(s, s->peer, s->ev_peer, block); }
+
+// a4 + a5 for one destination slot (pinned host memory or a peer's received buffer): invalidate the
+// destination header, copy the payload in chunk_bytes pieces (from the staging slot, or from the live
+// planes in direct mode), copy the valid header last.  torn_chunks >= 0: stop after that many payload
+// chunks and never commit (fault injection).
+int enqueue_snapshot_copy(phx_shard *s, cudaStream_t st, uint8_t *dst, cudaMemcpyKind kind, int slot, int64_t torn_chunks)
+{
+    const bool direct = direct_mode(s);
+    const uint8_t *src = direct ? nullptr : s->d_staging + (uint64_t)slot * s->info.slot_stride;
+    const uint8_t *src_hdr = direct ? s->d_scratch + kScrHdr + (size_t)slot * kHeaderBytes : src;
+    const bool torn = torn_chunks >= 0;
+    // 1. invalidate the target slot's header; the OTHER slot keeps the previous committed snapshot
+    PHX_CK(cudaMemcpyAsync(dst, s->d_scratch + kScrZeroHdr, kHeaderBytes, kind, st));
+    // 2. payload in chunk_bytes pieces (PAPER.md:152 "chunked")
+    const uint64_t payload = s->info.snapshot_bytes - kHeaderBytes;
+    const uint64_t chunk = s->cfg.chunk_bytes;
+    uint64_t done_chunks = 0;
+    for (uint64_t off = 0; off < payload; off += chunk, ++done_chunks) {
+        if (torn && (int64_t)done_chunks >= torn_chunks) break;
+        const uint64_t len = payload - off < chunk ? payload - off : chunk;
+        if (!direct) {
+            PHX_CK(cudaMemcpyAsync(dst + kHeaderBytes + off, src + kHeaderBytes + off, len, kind, st));
+        } else {
+            // the chunk [off, off+len) of the packed payload p ‖ m ‖ v comes straight from the live planes;
+            // a chunk that straddles a plane boundary is split there
+            const uint64_t plane = 4 * s->info.n_padded;
+            const uint8_t *planes[3] = {reinterpret_cast<const uint8_t *>(s->d_p), reinterpret_cast<const uint8_t *>(s->d_m),
+                                        reinterpret_cast<const uint8_t *>(s->d_v)};
+            uint64_t o = off, left = len;
+            while (left) {
+                const uint64_t pi = o / plane, po = o % plane;
+                const uint64_t l = left < plane - po ? left : plane - po;
+                PHX_CK(cudaMemcpyAsync(dst + kHeaderBytes + o, planes[pi] + po, l, kind, st));
+                o += l;
+                left -= l;
+            }
+        }
+    }
+    // 3. commit: the valid header (seq_end == seq_begin) lands last
+    if (!torn) PHX_CK(cudaMemcpyAsync(dst, src_hdr, kHeaderBytes, kind, st));
     return PHX_OK;
 }
 
@@ -335,8 +391,13 @@ int phx_shard_destroy(phx_shard_t *s)
             if (s->ev_step[k]) cudaEventSynchronize(s->ev_step[k]), cudaEventDestroy(s->ev_step[k]);
             if (s->ev_flush[k]) cudaEventSynchronize(s->ev_flush[k]), cudaEventDestroy(s->ev_flush[k]);
         }
-        for (int k = 0; k < 2; ++k)
+        settle_peer_slots(s, true);
+        for (int k = 0; k < kMaxDepth; ++k)
+            if (s->ev_pflush[k]) cudaEventSynchronize(s->ev_pflush[k]), cudaEventDestroy(s->ev_pflush[k]);
+        for (int k = 0; k < 2; ++k) {
             if (s->ev_host[k]) cudaEventDestroy(s->ev_host[k]);
+            if (s->ev_peer[k]) cudaEventDestroy(s->ev_peer[k]);
+        }
         if (s->d_scratch) cudaFree(s->d_scratch);
         if (s->d_decay) cudaFree(s->d_decay);
     }
@@ -369,7 +430,7 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
                    void *h_replica)
 {
     if (!s || !d_p || !d_m || !d_v || (!d_p_bf16 && !fp32_mode(s))) return PHX_ERR_INVALID_ARG;
-    if (snapshots_on(s) && (!h_replica || (!d_staging && !direct_mode(s)))) return PHX_ERR_INVALID_ARG;
+    if (snapshots_on(s) && !d_staging && !direct_mode(s)) return PHX_ERR_INVALID_ARG;
     if (!aligned256(d_p) || !aligned256(d_m) || !aligned256(d_v) || !aligned256(d_p_bf16) || !aligned256(d_staging) ||
         !aligned256(h_replica))
         return PHX_ERR_ALIGNMENT;
@@ -381,7 +442,7 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
     if (major != 10) return PHX_ERR_UNSUPPORTED_DEVICE;  // sm_100a only; deliberately no fallback
     PHX_CK(cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, dev));
 
-    if (snapshots_on(s)) {
+    if (snapshots_on(s) && h_replica) {
         void *dview = nullptr;
         cudaError_t e = cudaHostGetDevicePointer(&dview, h_replica, 0);
         if (e != cudaSuccess) {  // not pinned/mapped host memory
@@ -399,8 +460,12 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
     for (uint32_t k = 0; k < ring_depth(s); ++k) {
         PHX_CK(cudaEventCreateWithFlags(&s->ev_step[k], cudaEventDisableTiming));
         PHX_CK(cudaEventCreateWithFlags(&s->ev_flush[k], cudaEventDisableTiming));
+        PHX_CK(cudaEventCreateWithFlags(&s->ev_pflush[k], cudaEventDisableTiming));
     }
-    for (int k = 0; k < 2; ++k) PHX_CK(cudaEventCreateWithFlags(&s->ev_host[k], cudaEventDisableTiming));
+    for (int k = 0; k < 2; ++k) {
+        PHX_CK(cudaEventCreateWithFlags(&s->ev_host[k], cudaEventDisableTiming));
+        PHX_CK(cudaEventCreateWithFlags(&s->ev_peer[k], cudaEventDisableTiming));
+    }
     if (s->has_groups) {
         const size_t nb = s->decay_bnd.size() * sizeof(uint64_t);
         PHX_CK(cudaMalloc(reinterpret_cast<void **>(&s->d_decay), nb + s->decay_cls.size() + 8));
@@ -428,6 +493,7 @@ int phx_shard_set_state(phx_shard_t *s, uint64_t step, void *stream)
     }
     s->last_step = step;
     s->pending_slot = -1;
+    s->pending_peer_slot = -1;
     return PHX_OK;
 }
 
@@ -482,10 +548,13 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
     if (snap) {
         slot = (int)(step % ring_depth(s));
         // a2: the single sync point — stream-side wait, the host never blocks
+        // ("guarantees the peer-resident replica is fully committed before the optimizer mutates the protected state")
         if (s->cfg.sync_mode == PHX_SYNC_STRICT) {
             if (s->last_flush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[s->last_flush_slot], 0));
-        } else if (s->flush_valid[slot]) {
-            PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[slot], 0));
+            if (s->last_pflush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_pflush[s->last_pflush_slot], 0));
+        } else {
+            if (s->flush_valid[slot]) PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[slot], 0));
+            if (s->pflush_valid[slot]) PHX_CK(cudaStreamWaitEvent(st, s->ev_pflush[slot], 0));
         }
         if (direct_mode(s)) {
             a.shdr = s->d_scratch + kScrHdr + (size_t)slot * kHeaderBytes;  // header only; planes stay live
@@ -520,6 +589,8 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
         PHX_CK(cudaEventRecord(s->ev_step[slot], st));
         s->pending_slot = slot;
         s->pending_step = step;
+        s->pending_peer_slot = slot;
+        s->pending_peer_step = step;
     }
     s->last_step = step;
     return PHX_OK;
@@ -529,16 +600,13 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
 int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream)
 {
     if (!s) return PHX_ERR_INVALID_ARG;
-    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!s->bound || (snapshots_on(s) && !s->h_replica)) return PHX_ERR_NOT_BOUND;
     if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
     if (s->pending_slot < 0) return PHX_ERR_NO_FLUSH_PENDING;
     cudaStream_t st = static_cast<cudaStream_t>(side_stream);
     const int slot = s->pending_slot;
     const uint64_t step = s->pending_step;
     const int hs = (int)(step & 1);  // ping-pong
-    const bool direct = direct_mode(s);
-    const uint8_t *src = direct ? nullptr : s->d_staging + (uint64_t)slot * s->info.slot_stride;
-    const uint8_t *src_hdr = direct ? s->d_scratch + kScrHdr + (size_t)slot * kHeaderBytes : src;
     uint8_t *dst = s->h_replica + (uint64_t)hs * s->info.slot_stride;
 
     PHX_CK(cudaStreamWaitEvent(st, s->ev_step[slot], 0));  // the step's kernel has written the slot
@@ -548,35 +616,8 @@ int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream)
     const bool torn = s->torn_chunks >= 0;
     s->host[hs].step = step;
     s->host[hs].state = torn ? SLOT_TORN_INFLIGHT : SLOT_INFLIGHT;
-    // 1. invalidate the target slot's header; the OTHER slot keeps the previous committed snapshot
-    PHX_CK(cudaMemcpyAsync(dst, s->d_scratch + kScrZeroHdr, kHeaderBytes, cudaMemcpyDeviceToHost, st));
-    // 2. payload in chunk_bytes pieces (PAPER.md:152 "chunked")
-    const uint64_t payload = s->info.snapshot_bytes - kHeaderBytes;
-    const uint64_t chunk = s->cfg.chunk_bytes;
-    uint64_t done_chunks = 0;
-    for (uint64_t off = 0; off < payload; off += chunk, ++done_chunks) {
-        if (torn && (int64_t)done_chunks >= s->torn_chunks) break;
-        const uint64_t len = payload - off < chunk ? payload - off : chunk;
-        if (!direct) {
-            PHX_CK(cudaMemcpyAsync(dst + kHeaderBytes + off, src + kHeaderBytes + off, len, cudaMemcpyDeviceToHost, st));
-        } else {
-            // the chunk [off, off+len) of the packed payload p ‖ m ‖ v comes straight from the live planes;
-            // a chunk that straddles a plane boundary is split there
-            const uint64_t plane = 4 * s->info.n_padded;
-            const uint8_t *planes[3] = {reinterpret_cast<const uint8_t *>(s->d_p), reinterpret_cast<const uint8_t *>(s->d_m),
-                                        reinterpret_cast<const uint8_t *>(s->d_v)};
-            uint64_t o = off, left = len;
-            while (left) {
-                const uint64_t pi = o / plane, po = o % plane;
-                const uint64_t l = left < plane - po ? left : plane - po;
-                PHX_CK(cudaMemcpyAsync(dst + kHeaderBytes + o, planes[pi] + po, l, cudaMemcpyDeviceToHost, st));
-                o += l;
-                left -= l;
-            }
-        }
-    }
-    // 3. commit: the valid header (seq_end == seq_begin) lands last
-    if (!torn) PHX_CK(cudaMemcpyAsync(dst, src_hdr, kHeaderBytes, cudaMemcpyDeviceToHost, st));
+    int rc = enqueue_snapshot_copy(s, st, dst, cudaMemcpyDeviceToHost, slot, s->torn_chunks);
+    if (rc != PHX_OK) return rc;
     PHX_CK(cudaEventRecord(s->ev_flush[slot], st));
     PHX_CK(cudaEventRecord(s->ev_host[hs], st));
     s->flush_valid[slot] = true;
@@ -620,22 +661,21 @@ int phx_fault_inject_torn_flush(phx_shard_t *s, int64_t payload_chunks)
 }
 
 // ---- a6 ------------------------------------------------------------------------------------------
-int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
-{
-    if (!s) return PHX_ERR_INVALID_ARG;
-    if (!s->bound) return PHX_ERR_NOT_BOUND;
-    if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    // in-flight flushes must land (or be known torn) before the host reads the headers
-    int rc = settle_host_slots(s, true);
-    if (rc != PHX_OK) return rc;
+namespace {
 
-    // Selection depends only on what is IN the replica: a fresh handle can restore.
+// Rebuild the live shard from `replica` (two slots at slot_stride).  hdr_src: where the host can read the
+// two headers with a blocking copy; copy_src: address for copy-engine copies; kern_src: device-visible
+// address for the bulk kernel.  Selection depends only on what is IN the replica.
+int restore_impl(phx_shard *s, const uint8_t *hdr_src, const uint8_t *copy_src, const uint8_t *kern_src,
+                 bool hdr_on_host, cudaStream_t st, uint64_t *restored_step, bool *valid_out)
+{
     int best = -1;
     bool any_valid = false;
     phx_snapshot_header_t hdr[2];
     for (int i = 0; i < 2; ++i) {
-        std::memcpy(&hdr[i], s->h_replica + (uint64_t)i * s->info.slot_stride, sizeof(hdr[i]));
+        const uint8_t *hp = hdr_src + (uint64_t)i * s->info.slot_stride;
+        if (hdr_on_host) std::memcpy(&hdr[i], hp, sizeof(hdr[i]));
+        else PHX_CK(cudaMemcpy(&hdr[i], hp, sizeof(hdr[i]), cudaMemcpyDefault));
         if (!header_valid(&hdr[i])) continue;
         any_valid = true;
         if (!header_matches(s, &hdr[i])) continue;
@@ -646,14 +686,14 @@ int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
     const uint64_t N = s->info.n_padded;
     const uint64_t off = (uint64_t)best * s->info.slot_stride + kHeaderBytes;
     if (s->cfg.restore_mode == PHX_RESTORE_BULK_KERNEL) {
-        PHX_CK(phx::launch_restore_bulk(s->d_replica + off, s->d_p, s->d_m, s->d_v, fp32_mode(s) ? nullptr : s->d_p16, N,
+        PHX_CK(phx::launch_restore_bulk(kern_src + off, s->d_p, s->d_m, s->d_v, fp32_mode(s) ? nullptr : s->d_p16, N,
                                         s->sm_count, st));
         s->launches += N ? 1 : 0;
     } else {
-        const uint8_t *src = s->h_replica + off;
-        PHX_CK(cudaMemcpyAsync(s->d_p, src, 4 * N, cudaMemcpyHostToDevice, st));
-        PHX_CK(cudaMemcpyAsync(s->d_m, src + 4 * N, 4 * N, cudaMemcpyHostToDevice, st));
-        PHX_CK(cudaMemcpyAsync(s->d_v, src + 8 * N, 4 * N, cudaMemcpyHostToDevice, st));
+        const uint8_t *src = copy_src + off;
+        PHX_CK(cudaMemcpyAsync(s->d_p, src, 4 * N, cudaMemcpyDefault, st));
+        PHX_CK(cudaMemcpyAsync(s->d_m, src + 4 * N, 4 * N, cudaMemcpyDefault, st));
+        PHX_CK(cudaMemcpyAsync(s->d_v, src + 8 * N, 4 * N, cudaMemcpyDefault, st));
         if (!fp32_mode(s)) {
             PHX_CK(phx::launch_regen_bf16(s->d_p, s->d_p16, N, st));
             s->launches += N ? 1 : 0;
@@ -661,15 +701,54 @@ int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
     }
     s->last_step = hdr[best].step;
     s->pending_slot = -1;
+    s->pending_peer_slot = -1;
     s->restored_user_len = hdr[best].user_len <= 128 ? hdr[best].user_len : 128;
     std::memcpy(s->restored_user, hdr[best].user, 128);
-    for (int i = 0; i < 2; ++i) {
-        const bool ok = header_valid(&hdr[i]) && header_matches(s, &hdr[i]);
-        s->host[i].state = ok ? SLOT_COMMITTED : (s->host[i].state == SLOT_EMPTY ? SLOT_EMPTY : SLOT_TORN);
-        if (ok) s->host[i].step = hdr[i].step;
-    }
+    for (int i = 0; i < 2; ++i) valid_out[i] = header_valid(&hdr[i]) && header_matches(s, &hdr[i]);
     if (restored_step) *restored_step = s->last_step;
+    // the slots' steps, for the caller's own slot bookkeeping
+    s->restore_hdr_step[0] = hdr[0].step;
+    s->restore_hdr_step[1] = hdr[1].step;
     return PHX_OK;
+}
+
+}  // namespace
+
+int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound || (snapshots_on(s) && !s->h_replica)) return PHX_ERR_NOT_BOUND;
+    if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
+    // in-flight flushes must land (or be known torn) before the host reads the headers
+    int rc = settle_host_slots(s, true);
+    if (rc != PHX_OK) return rc;
+    bool ok[2] = {false, false};
+    rc = restore_impl(s, s->h_replica, s->h_replica, s->d_replica, true, static_cast<cudaStream_t>(stream), restored_step, ok);
+    if (rc != PHX_OK) return rc;
+    for (int i = 0; i < 2; ++i) {
+        s->host[i].state = ok[i] ? SLOT_COMMITTED : (s->host[i].state == SLOT_EMPTY ? SLOT_EMPTY : SLOT_TORN);
+        if (ok[i]) s->host[i].step = s->restore_hdr_step[i];
+    }
+    return PHX_OK;
+}
+
+// §8(f1): restore from a replica held elsewhere — a peer's received buffer mapped into this process
+// (PAPER.md:171 stage 3, 248-250), a device buffer, or pinned host memory.
+int phx_restore_from(phx_shard_t *s, const void *replica, void *stream, uint64_t *restored_step)
+{
+    if (!s || !replica) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!aligned256(replica)) return PHX_ERR_ALIGNMENT;
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, replica);
+    if (e != cudaSuccess || (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeHost) || !at.devicePointer) {
+        (void)cudaGetLastError();
+        return PHX_ERR_INVALID_ARG;  // pageable host memory or an unknown address
+    }
+    const uint8_t *r = static_cast<const uint8_t *>(replica);
+    bool ok[2];
+    return restore_impl(s, r, r, static_cast<const uint8_t *>(at.devicePointer), false, static_cast<cudaStream_t>(stream),
+                        restored_step, ok);
 }
 
 int phx_restored_user_metadata(const phx_shard_t *s, void *blob, uint32_t cap, uint32_t *len)
@@ -678,6 +757,155 @@ int phx_restored_user_metadata(const phx_shard_t *s, void *blob, uint32_t cap, u
     const uint32_t k = s->restored_user_len < cap ? s->restored_user_len : cap;
     if (k) std::memcpy(blob, s->restored_user, k);
     if (len) *len = s->restored_user_len;
+    return PHX_OK;
+}
+
+// ---- §8(f1): peer replication around the DP ring ----------------------------------------------------
+int phx_ring_peer(uint32_t dp_size, uint32_t dp_rank, int32_t j, uint32_t *peer)
+{
+    if (!peer || dp_size == 0 || dp_rank >= dp_size || j == 0) return PHX_ERR_INVALID_ARG;
+    const int64_t a = j < 0 ? -(int64_t)j : (int64_t)j;
+    if (a > (int64_t)dp_size - 1) return PHX_ERR_INVALID_ARG;  // k distinct peers need k <= D - 1
+    const int64_t D = dp_size;
+    *peer = (uint32_t)((((int64_t)dp_rank + j) % D + D) % D);
+    return PHX_OK;
+}
+
+int phx_peer_buffer_alloc(uint64_t bytes, void **d_buf)
+{
+    if (!d_buf || bytes == 0) return PHX_ERR_INVALID_ARG;
+    *d_buf = nullptr;
+    void *p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return PHX_ERR_NOMEM;
+    }
+    if (cudaMemset(p, 0, bytes) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) {
+        cudaFree(p);
+        return PHX_ERR_CUDA;
+    }
+    *d_buf = p;
+    return PHX_OK;
+}
+
+int phx_peer_buffer_free(void *d_buf)
+{
+    if (!d_buf) return PHX_ERR_INVALID_ARG;
+    return cudaFree(d_buf) == cudaSuccess ? PHX_OK : PHX_ERR_CUDA;
+}
+
+int phx_ipc_export(void *d_buf, uint8_t handle[PHX_IPC_HANDLE_BYTES])
+{
+    static_assert(sizeof(cudaIpcMemHandle_t) == PHX_IPC_HANDLE_BYTES, "IPC handle size");
+    if (!d_buf || !handle) return PHX_ERR_INVALID_ARG;
+    cudaIpcMemHandle_t h;
+    if (cudaIpcGetMemHandle(&h, d_buf) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return PHX_ERR_CUDA;
+    }
+    std::memcpy(handle, &h, sizeof(h));
+    return PHX_OK;
+}
+
+int phx_ipc_open(const uint8_t handle[PHX_IPC_HANDLE_BYTES], void **d_buf)
+{
+    if (!handle || !d_buf) return PHX_ERR_INVALID_ARG;
+    cudaIpcMemHandle_t h;
+    std::memcpy(&h, handle, sizeof(h));
+    void *p = nullptr;
+    if (cudaIpcOpenMemHandle(&p, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return PHX_ERR_CUDA;
+    }
+    *d_buf = p;
+    return PHX_OK;
+}
+
+int phx_ipc_close(void *d_buf)
+{
+    if (!d_buf) return PHX_ERR_INVALID_ARG;
+    return cudaIpcCloseMemHandle(d_buf) == cudaSuccess ? PHX_OK : PHX_ERR_CUDA;
+}
+
+int phx_shard_bind_peers(phx_shard_t *s, void *const *d_peer_replicas, uint32_t k)
+{
+    if (!s || (k && !d_peer_replicas) || k > PHX_MAX_PEERS) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
+    if (k > s->info.dp_size - 1) return PHX_ERR_INVALID_ARG;  // k distinct ring successors need k <= D - 1
+    for (uint32_t j = 0; j < k; ++j) {
+        if (!d_peer_replicas[j]) return PHX_ERR_INVALID_ARG;
+        if (!aligned256(d_peer_replicas[j])) return PHX_ERR_ALIGNMENT;
+        for (uint32_t i = 0; i < j; ++i)
+            if (d_peer_replicas[i] == d_peer_replicas[j]) return PHX_ERR_INVALID_ARG;  // k DISTINCT peers
+    }
+    int rc = settle_peer_slots(s, true);
+    if (rc != PHX_OK) return rc;
+    for (uint32_t j = 0; j < PHX_MAX_PEERS; ++j) s->d_peer[j] = j < k ? static_cast<uint8_t *>(d_peer_replicas[j]) : nullptr;
+    s->n_peers = k;
+    return PHX_OK;
+}
+
+int phx_snapshot_flush_peers_async(phx_shard_t *s, void *peer_stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound || s->n_peers == 0) return PHX_ERR_NOT_BOUND;
+    if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
+    if (s->pending_peer_slot < 0) return PHX_ERR_NO_FLUSH_PENDING;
+    cudaStream_t st = static_cast<cudaStream_t>(peer_stream);
+    const int slot = s->pending_peer_slot;
+    const uint64_t step = s->pending_peer_step;
+    const int ps = (int)(step & 1);  // the received buffer alternates like the local pair
+
+    PHX_CK(cudaStreamWaitEvent(st, s->ev_step[slot], 0));
+    if (s->last_pflush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_pflush[s->last_pflush_slot], 0));
+    bool any_torn = false;
+    for (uint32_t j = 0; j < s->n_peers; ++j) any_torn = any_torn || s->torn_peer_chunks[j] >= 0;
+    s->peer[ps].step = step;
+    s->peer[ps].state = any_torn ? SLOT_TORN_INFLIGHT : SLOT_INFLIGHT;
+    for (uint32_t j = 0; j < s->n_peers; ++j) {  // one stream: the source GPU's NVLink egress is the shared limit
+        uint8_t *dst = s->d_peer[j] + (uint64_t)ps * s->info.slot_stride;
+        int rc = enqueue_snapshot_copy(s, st, dst, cudaMemcpyDefault, slot, s->torn_peer_chunks[j]);
+        if (rc != PHX_OK) return rc;
+        s->torn_peer_chunks[j] = -1;
+    }
+    PHX_CK(cudaEventRecord(s->ev_pflush[slot], st));
+    PHX_CK(cudaEventRecord(s->ev_peer[ps], st));
+    s->pflush_valid[slot] = true;
+    s->last_pflush_slot = slot;
+    s->pending_peer_slot = -1;
+    return PHX_OK;
+}
+
+int phx_snapshot_wait_peers(phx_shard_t *s, uint64_t step)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound || s->n_peers == 0) return PHX_ERR_NOT_BOUND;
+    const int ps = (int)(step & 1);
+    if (s->peer[ps].state == SLOT_EMPTY || s->peer[ps].step != step) return PHX_ERR_NO_COMMITTED_SNAPSHOT;
+    int rc = settle_peer_slots(s, true);
+    if (rc != PHX_OK) return rc;
+    return s->peer[ps].state == SLOT_COMMITTED ? PHX_OK : PHX_ERR_CORRUPT_SLOT;
+}
+
+int phx_fault_inject_torn_peer_flush(phx_shard_t *s, uint32_t peer_j, int64_t payload_chunks)
+{
+    if (!s || peer_j == 0 || peer_j > PHX_MAX_PEERS) return PHX_ERR_INVALID_ARG;
+    s->torn_peer_chunks[peer_j - 1] = payload_chunks < 0 ? -1 : payload_chunks;
+    return PHX_OK;
+}
+
+int phx_replica_inspect(const void *replica, uint64_t slot_stride, phx_snapshot_header_t out[2], int valid[2])
+{
+    if (!replica || !out || !valid || slot_stride < kHeaderBytes) return PHX_ERR_INVALID_ARG;
+    for (int i = 0; i < 2; ++i) {
+        const uint8_t *hp = static_cast<const uint8_t *>(replica) + (uint64_t)i * slot_stride;
+        if (cudaMemcpy(&out[i], hp, sizeof(out[i]), cudaMemcpyDefault) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return PHX_ERR_CUDA;
+        }
+        valid[i] = header_valid(&out[i]) ? 1 : 0;
+    }
     return PHX_OK;
 }
 

@@ -1,0 +1,127 @@
+"""Peer replication plumbing: received buffers, CUDA IPC handle exchange around
+the data-parallel ring, binding.  Marshalling only — every byte is moved by libphx's copy-engine
+flush (phx_snapshot_flush_peers_async) or restore (phx_restore_from); ring arithmetic is
+phx_ring_peer.  torch.distributed is used for ONE control-plane exchange of 64-byte IPC handles at
+set-up (the paper's control plane is a TCPStore); the data path has no collective.
+
+One process per GPU (the ring peer is "the rank sharing the same tensor-parallel and
+pipeline-parallel positions but with a different data-parallel index"):
+    ring = PeerRing(shard, k, group=dp_group)      # allocates what this rank holds for its k
+                                                   # predecessors, exchanges handles, opens and
+                                                   # binds its k successors' buffers
+    shard.step_and_snapshot(...); ring.flush_async(peer_stream); ...; ring.wait(step)
+Single process (tests, the 1-GPU bench stand-in): connect_in_process([shard_0, .., shard_{D-1}], k)
+wires D logical ranks living on one device to each other without IPC.
+"""
+from __future__ import annotations
+
+from typing import List, Optional, Sequence
+
+from . import binding as B
+
+
+def successors(dp_size: int, dp_rank: int, k: int) -> List[int]:
+    """Ranks that hold this rank's replicas: ring peers j = 1..k (phx_ring_peer)."""
+    return [B.phx_ring_peer(dp_size, dp_rank, j) for j in range(1, k + 1)]
+
+
+def predecessors(dp_size: int, dp_rank: int, k: int) -> List[int]:
+    """Ranks whose replicas this rank holds: ring peers j = -1..-k."""
+    return [B.phx_ring_peer(dp_size, dp_rank, -j) for j in range(1, k + 1)]
+
+
+def route_handles(table: Sequence[Sequence[bytes]], dp_size: int, dp_rank: int, k: int) -> List[bytes]:
+    """table[h][j-1] = handle of the buffer rank h keeps for ITS j-th predecessor (gathered from all
+    ranks).  Returns the k handles this rank must open: its j-th successor's buffer number j-1."""
+    return [table[h][j] for j, h in enumerate(successors(dp_size, dp_rank, k))]
+
+
+class ReceivedBuffers:
+    """The k received buffers (two snapshot slots each) a rank keeps for its ring predecessors."""
+
+    def __init__(self, slot_stride: int, k: int):
+        self.slot_stride, self.k = slot_stride, k
+        self.ptrs = [B.phx_peer_buffer_alloc(2 * slot_stride) for _ in range(k)]
+
+    def handles(self) -> List[bytes]:
+        return [B.phx_ipc_export(p) for p in self.ptrs]
+
+    def view(self, j: int):
+        """Zero-copy uint8 torch view of the buffer kept for predecessor j (1-based), for inspection."""
+        import torch
+
+        class _Raw:
+            def __init__(self, ptr, nbytes):
+                self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False),
+                                                 "version": 2}
+        return torch.as_tensor(_Raw(self.ptrs[j - 1], 2 * self.slot_stride), device="cuda")
+
+    def inspect(self, j: int):
+        """[(header, valid)] of the buffer kept for predecessor j (1-based)."""
+        return B.phx_replica_inspect(self.ptrs[j - 1], self.slot_stride)
+
+    def free(self):
+        for p in self.ptrs:
+            B.phx_peer_buffer_free(p)
+        self.ptrs = []
+
+
+class PeerRing:
+    """One rank's end of the ring: its received buffers + its successors' buffers opened over IPC."""
+
+    def __init__(self, shard, k: int, group=None):
+        import torch.distributed as dist
+        self.shard, self.k = shard, k
+        D, r = shard.info.dp_size, shard.info.dp_rank
+        assert dist.is_initialized() and dist.get_world_size(group) == D and dist.get_rank(group) == r, \
+            "PeerRing needs the DP group of this shard (one process per GPU)"
+        # every rank reaches both exchanges whatever happens locally, then all ranks agree on the outcome:
+        # a rank whose allocation / IPC open failed must not leave the others waiting
+        self.received, self.opened, err = None, [], None
+        try:
+            self.received = ReceivedBuffers(shard.info.slot_stride, k)
+            mine = self.received.handles()
+        except Exception as e:  # noqa: BLE001
+            mine, err = None, repr(e)
+        table: List[Optional[List[bytes]]] = [None] * D
+        dist.all_gather_object(table, mine, group=group)
+        if err is None and all(t is not None for t in table):
+            try:
+                self.opened = [B.phx_ipc_open(h) for h in route_handles(table, D, r, k)]
+                B.phx_shard_bind_peers(shard.h, self.opened)
+            except Exception as e:  # noqa: BLE001
+                err = repr(e)
+        elif err is None:
+            err = "a peer could not allocate its received buffers"
+        status: List[Optional[str]] = [None] * D
+        dist.all_gather_object(status, err, group=group)
+        if any(x is not None for x in status):
+            self.close()
+            raise RuntimeError("PeerRing set-up failed: " + "; ".join(f"rank {i}: {x}" for i, x in enumerate(status) if x))
+
+    def flush_async(self, peer_stream):
+        B.phx_snapshot_flush_peers_async(self.shard.h, peer_stream)
+
+    def wait(self, step: int):
+        B.phx_snapshot_wait_peers(self.shard.h, step)
+
+    def close(self):
+        if self.opened:
+            B.phx_shard_bind_peers(self.shard.h, [])
+        for p in self.opened:
+            B.phx_ipc_close(p)
+        self.opened = []
+        if self.received is not None:
+            self.received.free()
+            self.received = None
+
+
+def connect_in_process(shards: Sequence, k: int) -> List[ReceivedBuffers]:
+    """D logical ranks in one process on one device: rank r's peer j is rank (r + j) mod D's received
+    buffer number j-1, bound by plain device pointer (no IPC inside one process)."""
+    D = len(shards)
+    assert all(s.info.dp_size == D and s.info.dp_rank == r for r, s in enumerate(shards))
+    recv = [ReceivedBuffers(s.info.slot_stride, k) for s in shards]
+    for r, s in enumerate(shards):
+        B.phx_shard_bind_peers(s.h, [recv[h].ptrs[j] for j, h in enumerate(successors(D, r, k))])
+    return recv

@@ -97,11 +97,12 @@ def test_decay_groups_differ_from_uniform_decay_and_match_wd_zero():
     assert not np.array_equal(out["g"][a:b], out["u"][a:b])
 
 
+@pytest.mark.parametrize("rank", [1, 3])
 @pytest.mark.parametrize("precision", ["bf16", "fp32"])
-def test_c1_with_gpt_parameter_groups_ten_steps(precision):
-    # config c1's real tensor list: biases and LayerNorm weights flagged no-decay (48 small tensors,
-    # 98 toggles, most of them inside a tile)
-    wl = dataclasses.replace(W.CONFIGS["c1"], decay_groups=True, precision=precision)
+def test_c1_with_gpt_parameter_groups_ten_steps(precision, rank):
+    # config c1's real tensor list: biases and LayerNorm weights flagged no-decay (34 small tensors, most
+    # toggles inside a tile); rank 0 holds only the embedding, so the ranks that hold layers are used
+    wl = dataclasses.replace(W.CONFIGS["c1"], decay_groups=True, precision=precision, dp_rank=rank)
     assert sum(wl.flags()) == 4 * 8 + 2
     s, o, gdev, gbits = make_pair(wl, steps=10)
     assert o.no_decay is not None and 0 < int(o.no_decay.sum()) < o.n
