@@ -70,6 +70,10 @@ def parse_args():
                     help="snapshot source: staged = fused kernel also writes the staging slot (40 B/elem, north_star); "
                          "direct = flush DMAs the live planes under the strict sync point (28 B/elem)")
     ap.add_argument("--restore-mode", default="copy", choices=["bulk", "copy"])
+    ap.add_argument("--peers", type=int, default=-1,
+                    help="k ring peers the snapshot is also replicated to over NVLink (SURVEY 8(f1)); -1 = auto: 1 when "
+                         "--gpus > 1 (real P2P ring over CUDA IPC), 0 at one GPU; k > 0 at one GPU measures a loopback "
+                         "stand-in (received buffer on the same device)")
     ap.add_argument("--precision", default="bf16", choices=["bf16", "fp32"],
                     help="bf16 = fp32 state + bf16 grads + bf16 copy (north_star, default); fp32 = the paper's own "
                          "all-FP32 setting (PAPER.md:270; SURVEY 8(f2)): fp32 grads, no bf16 copy, 16 B read + 24 B written")
@@ -338,6 +342,44 @@ class Rig:
         self.off_step = 0
         self._gemm = None
         self.gemm_ms = None
+        self.k_peers = 0
+        self.peers_in_overlap = False
+
+    # -- §8(f1): peer replication ----------------------------------------------------------------------
+    def setup_peers(self, k, rank, world):
+        """Bind k ring peers: a real CUDA-IPC ring over the `world` processes, or, on one GPU, received buffers
+        on the same device (loopback stand-in).  Returns a description; raises on failure (all ranks agree)."""
+        from paper_2607_01646_b200 import ring as PR
+        self.peer_stream = self.torch.cuda.Stream(device=self.device)
+        self.k_peers = k
+        if world > 1:
+            self.ring = PR.PeerRing(self.s, k, ring_size=world, ring_rank=rank)
+            return "NVLink/NVSwitch P2P into the ring successors' HBM, received buffers mapped over CUDA IPC"
+        self.recv = PR.ReceivedBuffers(self.s.info.slot_stride, k)
+        self.B.phx_shard_bind_peers(self.s.h, self.recv.ptrs)
+        return "loopback stand-in: received buffers on the SAME GPU (device-to-device copy engine, not NVLink)"
+
+    def time_peer_flush(self):
+        """One replication of the newest snapshot to all k peers, alone, timed on the peer stream."""
+        torch = self.torch
+        self.do_step()
+        torch.cuda.synchronize()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record(self.peer_stream)
+        self.B.phx_snapshot_flush_peers_async(self.s.h, self.peer_stream)
+        f1.record(self.peer_stream)
+        self.B.phx_snapshot_wait_peers(self.s.h, self.step)
+        torch.cuda.synchronize()
+        return f0.elapsed_time(f1)
+
+    def close_peers(self):
+        if getattr(self, "ring", None) is not None:
+            self.ring.close()
+            self.ring = None
+        if getattr(self, "recv", None) is not None:
+            self.B.phx_shard_bind_peers(self.s.h, [])
+            self.recv.free()
+            self.recv = None
 
     def precision_code(self):
         return self.B.PHX_PRECISION_FP32 if self.fp32 else self.B.PHX_PRECISION_BF16_GRADS
@@ -525,6 +567,8 @@ class Rig:
                     k1.record(self.cur)
                     if arm == "on":
                         self.s.flush_async(self.side)
+                        if getattr(self, "k_peers", 0) and self.peers_in_overlap:
+                            self.B.phx_snapshot_flush_peers_async(self.s.h, self.peer_stream)
                     evs.append(e0)
                     kevs.append((k0, k1))
                 end = torch.cuda.Event(enable_timing=True)
@@ -532,6 +576,8 @@ class Rig:
                 torch.cuda.synchronize()
                 if arm == "on":
                     self.s.wait(self.step)
+                    if getattr(self, "k_peers", 0) and self.peers_in_overlap:
+                        self.B.phx_snapshot_wait_peers(self.s.h, self.step)
                 evs.append(end)
                 it_ms[arm] += [evs[i].elapsed_time(evs[i + 1]) for i in range(warm, warm + iters)]
                 hp_ms[arm] += [x.elapsed_time(y) for x, y in kevs[warm:]]
@@ -550,6 +596,7 @@ class Rig:
         return out
 
     def close(self):
+        self.close_peers()
         if self.s_off is not None:
             self.B.phx_shard_destroy(self.s_off)
             self.s_off = None
@@ -628,6 +675,24 @@ def run_headline(args):
            "steps": args.e2e_steps,
            "note": "H2D grads from pinned host + fused step + chunked D2H of the packed snapshot + commit, per step"}
 
+    # ---- §8(f1): ring peers (real NVLink ring at N > 1; opt-in loopback stand-in at N = 1) -------------
+    k_peers = args.peers if args.peers >= 0 else (1 if world > 1 else 0)
+    k_peers = min(k_peers, max(world - 1, 0)) if world > 1 else k_peers
+    peer = None
+    if k_peers > 0:
+        try:
+            peer = {"k": k_peers, "link": rig.setup_peers(k_peers, rank, world)}
+            rig.peers_in_overlap = world > 1      # the loopback copy is not NVLink traffic: keep it out of the overlap arm
+        except Exception as e:  # noqa: BLE001  (PeerRing makes every rank fail together)
+            peer = {"k": k_peers, "error": str(e)[:300]}
+            rig.k_peers = 0
+    if peer and "error" not in peer:
+        pf_ms = max_over_ranks(rig.time_peer_flush(), world, device)
+        pbytes = k_peers * int(rig.s.info.snapshot_bytes)
+        peer.update(flush_ms=pf_ms, bytes_per_step=pbytes, gbs_per_gpu=pbytes / (pf_ms * 1e-3) / 1e9,
+                    note="replication of one packed snapshot to all k peers, copy engine, alone; max over ranks, "
+                         "all ranks sending at once")
+
     host_link = overlap = restore = cpu = None
     if rank == 0:
         # flush alone (a4+a5) against the measured pinned-copy peak
@@ -647,6 +712,20 @@ def run_headline(args):
         restore = {"restore_ms": rms, "recompute_ms": cms, "mode": rig.restore_mode_name, "restored_step": back,
                    "host_link_gbs": 12 * N / (rms * 1e-3) / 1e9,
                    "frac_of_h2d_peak": 12 * N / (rms * 1e-3) / 1e9 / link["h2d_gbs"]}
+        # restore from the ring successor's received buffer (recovery stage 3 over NVLink)
+        if peer and "error" not in peer:
+            src = rig.ring.opened[0] if world > 1 else rig.recv.ptrs[0]
+            rig.s.drop_live()
+            torch.cuda.synchronize()
+            p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            p0.record(rig.cur)
+            back_p = B.phx_restore_from(rig.s.h, src, rig.cur)
+            p1.record(rig.cur)
+            torch.cuda.synchronize()
+            rig.step = back_p
+            pms = p0.elapsed_time(p1)
+            peer.update(restore_from_peer_ms=pms, restore_from_peer_gbs=12 * N / (pms * 1e-3) / 1e9,
+                        restored_step=back_p)
         # cpu baseline: the oracle on the host cores (rank 0, N == 1 only)
         if world == 1 and not args.no_cpu_baseline:
             cores = len(os.sched_getaffinity(0))
@@ -676,10 +755,11 @@ def run_headline(args):
             "elements_per_s": units / (ms_per_step * 1e-3),
             "exposed_ckpt_ms_per_iter": overlap["exposed_ms"] if overlap else None,
             "roofline": roofline, "host_link": host_link, "e2e": e2e, "overlap": overlap, "restore": restore,
-            "cpu_baseline": cpu, "gpu_launches": int(launches), "clocks": clk,
+            "peer_replication": peer, "cpu_baseline": cpu, "gpu_launches": int(launches), "clocks": clk,
             "step_ms_min_max": [min(per), max(per)],
         }
         print(json.dumps(line), flush=True)
+    barrier(world)      # peers' received buffers stay mapped until rank 0 has finished writing into them
     rig.close()
     if world > 1:
         import torch.distributed as dist

@@ -69,12 +69,17 @@ class ReceivedBuffers:
 class PeerRing:
     """One rank's end of the ring: its received buffers + its successors' buffers opened over IPC."""
 
-    def __init__(self, shard, k: int, group=None):
+    def __init__(self, shard, k: int, group=None, ring_size: Optional[int] = None, ring_rank: Optional[int] = None):
+        """group: the DP group of this shard.  ring_size / ring_rank override the ring the handles are routed
+        on when only some of the D data-parallel ranks are present (e.g. N < D GPUs of one node in a
+        benchmark): the ring then closes among the ranks of `group`."""
         import torch.distributed as dist
         self.shard, self.k = shard, k
-        D, r = shard.info.dp_size, shard.info.dp_rank
+        D = shard.info.dp_size if ring_size is None else ring_size
+        r = shard.info.dp_rank if ring_rank is None else ring_rank
         assert dist.is_initialized() and dist.get_world_size(group) == D and dist.get_rank(group) == r, \
-            "PeerRing needs the DP group of this shard (one process per GPU)"
+            "PeerRing needs one process per ring position"
+        assert 1 <= k <= D - 1
         # every rank reaches both exchanges whatever happens locally, then all ranks agree on the outcome:
         # a rank whose allocation / IPC open failed must not leave the others waiting
         self.received, self.opened, err = None, [], None

@@ -281,3 +281,66 @@ def test_two_process_ipc_replication_and_recovery():
     finally:
         child.join(timeout=120)
     assert child.exitcode == 0
+
+
+def _ring_rank(rank, world, port, q):
+    """One process per ring position (both on the only GPU of the box; control plane on gloo)."""
+    import torch.distributed as dist
+    os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    torch.cuda.set_device(0)
+    dist.init_process_group("gloo")
+    wl = W.tiny_workload([40_000, 77], dp_size=world, dp_rank=rank)
+    s = Shard(wl, device=DEV, chunk_bytes=32 << 10)
+    o = O.OracleShard(wl.layout(), world, rank, chunk_bytes=32 << 10)
+    p0 = W.init_params(s.n, s.n_padded, 50 + rank)
+    s.p.copy_(p0)
+    s.set_state(0)
+    o.set_state(p0.numpy())
+    ring = PR.PeerRing(s, 1)
+    st = torch.cuda.Stream(device=DEV)
+    for t in range(1, 4):
+        g = W.gen_grads(wl, s.segments, s.n_padded, t, 50 + rank)
+        s.step_and_snapshot(g.to(DEV), t)
+        ring.flush_async(st)
+        o.step(grad_record(g), **hp_of(wl), step=t)
+        o.snapshot()
+    ring.wait(3)
+    dist.barrier()
+    # what I hold for my predecessor: its dp_rank, steps 2 and 3, valid
+    (h0, v0), (h1, v1) = ring.received.inspect(1)
+    pred = B.phx_ring_peer(world, rank, -1)
+    held = (v0 and v1, (h0.step, h1.step), (h0.dp_rank, h1.dp_rank))
+    # my own replica, read back from my successor's HBM through the IPC mapping, equals the oracle's snapshot bytes
+    view = torch.as_tensor(type("R", (), {"__cuda_array_interface__": {
+        "shape": (2 * s.info.slot_stride,), "typestr": "|u1", "data": (ring.opened[0], False), "version": 2}})(),
+        device="cuda")
+    same = bool(np.array_equal(view[s.info.slot_stride: s.info.slot_stride + s.info.snapshot_bytes].cpu().numpy(),
+                               o.replica[1]))
+    # every rank loses its live shard and pulls it back from its successor
+    s.drop_live()
+    back = B.phx_restore_from(s.h, ring.opened[0])
+    torch.cuda.synchronize()
+    ok = all(np.array_equal(a.cpu().numpy().view(np.uint32), b.view(np.uint32))
+             for a, b in ((s.p, o.p), (s.m, o.m), (s.v, o.v))) and np.array_equal(bits16(s.p16), o.p16)
+    q.put((rank, held, pred, same, back, bool(ok)))
+    dist.barrier()
+    ring.close()
+    s.close()
+    dist.destroy_process_group()
+
+
+def test_peer_ring_class_two_processes_over_ipc():
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29950 + os.getpid() % 40
+    ps = [ctx.Process(target=_ring_rank, args=(r, world, port, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    res = sorted(q.get(timeout=300) for _ in ps)
+    for p in ps:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    for rank, held, pred, same, back, ok in res:
+        assert held == (True, (2, 3), (pred, pred)), (rank, held)
+        assert same and back == 3 and ok
