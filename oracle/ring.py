@@ -150,6 +150,36 @@ class OracleRing:
         return step
 
 
+# ---- model-parameter publication and reconstruction ---------------------------
+#
+# In a ZeRO-2 distributed optimizer every DP rank of one TP/PP coordinate holds the SAME
+# model parameters for that partition; after the step each rank has updated only its 1/D range of the
+# flat space and the ranges are all-gathered.  Readings:
+#   R29  the model-parameter buffer W of a TP/PP partition is the flat padded space of a0 in the model
+#        dtype: W[r*L : (r+1)*L] = rank r's model-parameter copy (bf16: RNE_bf16(p_r); all-FP32 precision:
+#        p_r itself), L = n_padded.  Publication = concatenation in rank order (an all-gather).
+#   R30  on a permanent failure the replacement "can reconstruct its parameter shard from healthy ranks
+#        at the same TP/PP coordinate via a targeted collective" (171, 248): W is copied
+#        whole from any surviving DP rank of the same partition — they are byte-identical (I2).
+
+
+def publish(shards) -> np.ndarray:
+    """R29: the model-parameter buffer every DP rank holds after the step (uint16 bf16 bits, or float32)."""
+    if shards[0].precision == "fp32":
+        return np.concatenate([o.p for o in shards])
+    return np.concatenate([o.p16 for o in shards])
+
+
+def reconstruct_params(buffers, alive, r: int) -> np.ndarray:
+    """R30: rank r's replacement takes W from the first surviving rank of the partition (ring order)."""
+    D = len(buffers)
+    for j in range(1, D):
+        h = (r + j) % D
+        if alive[h]:
+            return buffers[h].copy()
+    raise O.OracleError("no surviving rank holds the partition's parameters")
+
+
 def p_loss_exact(dp_size: int, k: int, p):
     """Exact probability (any numeric type, e.g. Fraction) that some shard is unrecoverable when every
     rank fails independently with probability p within a step — brute force over all failure subsets."""

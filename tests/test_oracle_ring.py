@@ -179,3 +179,54 @@ def test_holder_refuses_a_foreign_layout():
     ring.shards[0] = O.OracleShard([(1000, 0), (333, 1), (78, 2)], 3, 0)     # a different logical shard
     with pytest.raises(O.OracleError):
         ring.recover(0)
+
+
+# ---------------------------------------------------------------------------- §8(f3) publication
+
+
+def test_publication_is_the_rounded_flat_master_in_rank_order():
+    import torch
+    D = 3
+    ring, rng = _ring(D, 1, numels=(1000, 333, 77), seed=5)
+    for t in range(1, 4):
+        _step_all(ring, _grads(ring, rng), t)
+    W = R.publish(ring.shards)
+    L = ring.shards[0].n_padded
+    assert W.dtype == np.uint16 and W.size == D * L
+    flat = np.concatenate([o.p for o in ring.shards])                      # the flat padded master space of a0
+    want = torch.from_numpy(flat).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+    assert np.array_equal(W, want)                                         # library cast (torch, RNE)
+    # element i of tensor t sits where a0 says: rank = flat // L, offset = flat % L
+    total = ring.shards[0].total_numel
+    assert not W[total:].any()                                             # padding of the flat space stays zero
+    for r, o in enumerate(ring.shards):
+        for tid, off_t, off_s, ln in o.segments:
+            start = sum(n for n, i in o.layout if i < tid) + off_t         # flat index of the segment's first element
+            assert np.array_equal(W[start:start + ln], o.p16[off_s:off_s + ln])
+            assert start == r * L + off_s
+
+
+def test_publication_fp32_precision_is_the_master_itself():
+    ring, rng = _ring(2, 1, numels=(500, 70), precision="fp32")
+    _step_all(ring, _grads(ring, rng, fp32=True), 1)
+    W = R.publish(ring.shards)
+    assert W.dtype == np.float32
+    assert np.array_equal(W.view(np.uint32), np.concatenate([o.p for o in ring.shards]).view(np.uint32))
+
+
+def test_parameter_reconstruction_from_a_surviving_rank():
+    D = 4
+    ring, rng = _ring(D, 2, seed=6)
+    _step_all(ring, _grads(ring, rng), 1)
+    W = R.publish(ring.shards)
+    bufs = [W.copy() for _ in range(D)]                                    # every DP rank holds the same bytes (I2)
+    ring.fail((1, 2))
+    bufs[1][:] = 0
+    bufs[2][:] = 0
+    got = R.reconstruct_params(bufs, ring.alive, 1)                        # successors 2 (dead), 3 (alive)
+    assert np.array_equal(got, W)
+    assert ring.recover(1) == 1
+    L = ring.shards[1].n_padded
+    assert np.array_equal(got[L:2 * L], ring.shards[1].p16)                # consistent with the restored optimizer shard
+    with pytest.raises(O.OracleError):
+        R.reconstruct_params(bufs, [False] * D, 0)
