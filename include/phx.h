@@ -54,7 +54,7 @@ extern "C" {
 enum {
     PHX_OK = 0,
     PHX_ERR_INVALID_ARG = -1,
-    PHX_ERR_ALIGNMENT = -2,           /* a bound pointer is not 256-byte aligned                 */
+    PHX_ERR_ALIGNMENT = -2,           /* a bound pointer is not 256-byte aligned (d_p_bf16: 128) */
     PHX_ERR_NOT_BOUND = -3,           /* phx_shard_bind has not been called                      */
     PHX_ERR_STEP_ORDER = -4,          /* step != last_step + 1 (I4 step atomicity) */
     PHX_ERR_NO_FLUSH_PENDING = -5,    /* flush requested but no un-flushed snapshot exists       */
@@ -167,7 +167,8 @@ PHX_API int phx_shard_segments(const phx_shard_t *s, uint32_t *tensor_id, uint64
  * host memory (may be NULL if snapshots are disabled or only peer replicas are used, see
  * phx_shard_bind_peers; phx_snapshot_flush_async / phx_restore then return PHX_ERR_NOT_BOUND).
  * Requires a CUDA device of compute capability 10.x. */
-/* d_p_bf16 may be NULL iff precision is PHX_PRECISION_FP32. */
+/* d_p_bf16 may be NULL iff precision is PHX_PRECISION_FP32; it needs 128-byte alignment only, so that it can be
+ * the rank's range inside its model-parameter buffer W (W + dp_rank * n_padded elements, §8(f3)). */
 PHX_API int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p_bf16,
                            void *d_staging, void *h_replica);
 /* Declare the bound p, m, v to be the state after optimizer step `step` (0 at initialisation)
@@ -285,6 +286,28 @@ PHX_API int phx_replica_inspect(const void *replica, uint64_t slot_stride, phx_s
  * selection, identity check, restore modes and postconditions as phx_restore; reads the two headers with a
  * blocking copy. */
 PHX_API int phx_restore_from(phx_shard_t *s, const void *replica, void *stream, uint64_t *restored_step);
+
+/* ---- model-parameter publication and reconstruction ---------------------------
+ * In the ZeRO-2 distributed optimizer every DP rank of one TP/PP coordinate holds the same
+ * model parameters W for that partition: the flat padded space of a0 in the model dtype (bf16; float in
+ * PHX_PRECISION_FP32), dp_size * n_padded elements, rank r's range at element offset r * n_padded.  After
+ * the step each rank has updated only its own range and the ranges are all-gathered (R29).
+ * PHX_PUBLISH_FUSED: the step → all-gather pair is ONE kernel: phx_step_and_snapshot's fused kernel stores
+ * every element's model-param copy not only to d_p_bf16 (the caller points it at its own W + r * n_padded)
+ * but also into the same range of each bound peer buffer (peer HBM over NVLink 5 / NVSwitch, mapped with
+ * phx_ipc_open) — no separate all-gather kernel, no extra read of the copy.
+ * PHX_PUBLISH_COPY_ENGINE: the kernel is unchanged and phx_publish_params_async pushes the range to the
+ * peers with `count` copy-engine copies on a side stream (after the step's kernel).
+ * d_param_bufs[i]: base address of another rank's W (device-addressable); count <= PHX_MAX_PARAM_PEERS.
+ * In PHX_PRECISION_FP32 the published values are the fp32 parameters p themselves. */
+#define PHX_MAX_PARAM_PEERS 15
+enum { PHX_PUBLISH_FUSED = 0, PHX_PUBLISH_COPY_ENGINE = 1 };
+PHX_API int phx_shard_bind_param_peers(phx_shard_t *s, void *const *d_param_bufs, uint32_t count, uint32_t mode);
+PHX_API int phx_publish_params_async(phx_shard_t *s, void *stream);
+/* R30: a replacement rank reconstructs its model parameters from a healthy DP rank
+ * of the same TP/PP coordinate: one copy of the whole buffer W (dp_size * n_padded model-dtype elements)
+ * from `d_src_param_buf` (peer HBM) into `d_dst_param_buf`. */
+PHX_API int phx_params_restore_from(phx_shard_t *s, const void *d_src_param_buf, void *d_dst_param_buf, void *stream);
 
 /* ---- introspection ---------------------------------------------------------------------- */
 PHX_API int phx_last_step(const phx_shard_t *s, uint64_t *step);

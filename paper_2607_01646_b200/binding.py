@@ -68,6 +68,8 @@ class phx_snapshot_header_t(C.Structure):
                 ("header_hash", C.c_uint64), ("seq_end", C.c_uint64)]
 
 
+PHX_PUBLISH_FUSED, PHX_PUBLISH_COPY_ENGINE = 0, 1
+PHX_MAX_PARAM_PEERS = 15
 PHX_MAX_PEERS = 4
 PHX_IPC_HANDLE_BYTES = 64
 
@@ -119,6 +121,9 @@ PROTOTYPES = {
     "phx_fault_inject_torn_peer_flush": (C.c_int, [C.c_void_p, C.c_uint32, C.c_int64]),
     "phx_replica_inspect": (C.c_int, [C.c_void_p, C.c_uint64, C.POINTER(phx_snapshot_header_t), C.POINTER(C.c_int)]),
     "phx_restore_from": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_uint64)]),
+    "phx_shard_bind_param_peers": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.c_uint32, C.c_uint32]),
+    "phx_publish_params_async": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "phx_params_restore_from": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
 }
 
 
@@ -345,3 +350,21 @@ def phx_restore_from(h: int, replica, stream=None) -> int:
     st = C.c_uint64()
     _ck(lib().phx_restore_from(h, _ptr(replica), _ptr(stream), C.byref(st)), "phx_restore_from", h)
     return st.value
+
+
+# ---- model-parameter publication and reconstruction ---------------------------
+
+
+def phx_shard_bind_param_peers(h: int, d_param_bufs: Sequence, mode: int = PHX_PUBLISH_FUSED) -> None:
+    k = len(d_param_bufs)
+    arr = (C.c_void_p * max(k, 1))(*[_ptr(x) for x in d_param_bufs])
+    _ck(lib().phx_shard_bind_param_peers(h, arr, k, mode), "phx_shard_bind_param_peers", h)
+
+
+def phx_publish_params_async(h: int, stream=None) -> None:
+    _ck(lib().phx_publish_params_async(h, _ptr(stream)), "phx_publish_params_async", h)
+
+
+def phx_params_restore_from(h: int, d_src_param_buf, d_dst_param_buf, stream=None) -> None:
+    _ck(lib().phx_params_restore_from(h, _ptr(d_src_param_buf), _ptr(d_dst_param_buf), _ptr(stream)),
+        "phx_params_restore_from", h)

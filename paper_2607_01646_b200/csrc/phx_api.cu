@@ -60,6 +60,7 @@ double pow_sqmul(double b, uint64_t t)  // LSB-first square-and-multiply, no lib
 }
 
 inline bool aligned256(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 255u) == 0; }
+inline bool aligned128(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 127u) == 0; }
 
 }  // namespace
 
@@ -111,6 +112,10 @@ struct phx_shard {
     int pending_peer_slot = -1;
     uint64_t pending_peer_step = 0;
     int64_t torn_peer_chunks[PHX_MAX_PEERS] = {-1, -1, -1, -1};
+    // §8(f3) publication of the model-param copy into other DP ranks' parameter buffers
+    uint32_t n_pub = 0, pub_mode = PHX_PUBLISH_FUSED;
+    uint8_t *d_pub[PHX_MAX_PARAM_PEERS] = {nullptr};
+    cudaEvent_t ev_last_step = nullptr;  // recorded after every step's kernel (publication by copy engine waits on it)
     // misc
     int last_cuda_error = 0;
     uint64_t launches = 0;
@@ -177,8 +182,10 @@ bool snapshots_on(const phx_shard *s) { return s->cfg.snapshot_disabled == 0; }
 bool fp32_mode(const phx_shard *s) { return s->cfg.precision == PHX_PRECISION_FP32; }
 uint32_t step_mode(const phx_shard *s)
 {
-    return (fp32_mode(s) ? (uint32_t)phx::kModeF32 : 0u) | (s->has_groups ? (uint32_t)phx::kModeGroups : 0u);
+    return (fp32_mode(s) ? (uint32_t)phx::kModeF32 : 0u) | (s->has_groups ? (uint32_t)phx::kModeGroups : 0u) |
+           ((s->n_pub && s->pub_mode == PHX_PUBLISH_FUSED) ? (uint32_t)phx::kModePublish : 0u);
 }
+uint64_t model_elem_bytes(const phx_shard *s) { return fp32_mode(s) ? 4u : 2u; }
 
 // Decay groups: walk the rank's segments in shard order, record the offsets at which the no-decay flag
 // toggles and classify every 2048-element tile as all-decay (0), all-no-decay (1) or mixed (2).  Pad
@@ -398,6 +405,7 @@ int phx_shard_destroy(phx_shard_t *s)
             if (s->ev_host[k]) cudaEventDestroy(s->ev_host[k]);
             if (s->ev_peer[k]) cudaEventDestroy(s->ev_peer[k]);
         }
+        if (s->ev_last_step) cudaEventSynchronize(s->ev_last_step), cudaEventDestroy(s->ev_last_step);
         if (s->d_scratch) cudaFree(s->d_scratch);
         if (s->d_decay) cudaFree(s->d_decay);
     }
@@ -431,7 +439,8 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
 {
     if (!s || !d_p || !d_m || !d_v || (!d_p_bf16 && !fp32_mode(s))) return PHX_ERR_INVALID_ARG;
     if (snapshots_on(s) && !d_staging && !direct_mode(s)) return PHX_ERR_INVALID_ARG;
-    if (!aligned256(d_p) || !aligned256(d_m) || !aligned256(d_v) || !aligned256(d_p_bf16) || !aligned256(d_staging) ||
+    // d_p_bf16 may be the rank's range inside its model-parameter buffer (§8(f3)): r * n_padded * 2 bytes, a multiple of 128
+    if (!aligned256(d_p) || !aligned256(d_m) || !aligned256(d_v) || !aligned128(d_p_bf16) || !aligned256(d_staging) ||
         !aligned256(h_replica))
         return PHX_ERR_ALIGNMENT;
     if (s->bound) return PHX_ERR_INVALID_ARG;
@@ -462,6 +471,7 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
         PHX_CK(cudaEventCreateWithFlags(&s->ev_flush[k], cudaEventDisableTiming));
         PHX_CK(cudaEventCreateWithFlags(&s->ev_pflush[k], cudaEventDisableTiming));
     }
+    PHX_CK(cudaEventCreateWithFlags(&s->ev_last_step, cudaEventDisableTiming));
     for (int k = 0; k < 2; ++k) {
         PHX_CK(cudaEventCreateWithFlags(&s->ev_host[k], cudaEventDisableTiming));
         PHX_CK(cudaEventCreateWithFlags(&s->ev_peer[k], cudaEventDisableTiming));
@@ -581,10 +591,16 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
         a.n_bnd = (uint32_t)s->decay_bnd.size();
         a.first_nodecay = s->first_nodecay;
     }
+    if (s->n_pub && s->pub_mode == PHX_PUBLISH_FUSED) {
+        a.n_pub = s->n_pub;
+        for (uint32_t q = 0; q < s->n_pub; ++q)
+            a.pub[q] = s->d_pub[q] + (uint64_t)s->info.dp_rank * s->info.n_padded * model_elem_bytes(s);
+    }
 
     // a3: one kernel, one pass
     PHX_CK(phx::launch_step(a, snap && !direct_mode(s), s->variant, step_mode(s), st));
     s->launches += s->info.n_padded ? 1 : 0;
+    PHX_CK(cudaEventRecord(s->ev_last_step, st));
     if (snap) {
         PHX_CK(cudaEventRecord(s->ev_step[slot], st));
         s->pending_slot = slot;
@@ -909,6 +925,45 @@ int phx_replica_inspect(const void *replica, uint64_t slot_stride, phx_snapshot_
     return PHX_OK;
 }
 
+// ---- §8(f3): model-parameter publication and reconstruction ---------------------------------------
+int phx_shard_bind_param_peers(phx_shard_t *s, void *const *d_param_bufs, uint32_t count, uint32_t mode)
+{
+    if (!s || (count && !d_param_bufs) || count > PHX_MAX_PARAM_PEERS || mode > PHX_PUBLISH_COPY_ENGINE)
+        return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (count && mode == PHX_PUBLISH_FUSED && s->variant != 0) return PHX_ERR_INVALID_ARG;
+    for (uint32_t q = 0; q < count; ++q) {
+        if (!d_param_bufs[q]) return PHX_ERR_INVALID_ARG;
+        if (!aligned256(d_param_bufs[q])) return PHX_ERR_ALIGNMENT;
+    }
+    for (uint32_t q = 0; q < PHX_MAX_PARAM_PEERS; ++q) s->d_pub[q] = q < count ? static_cast<uint8_t *>(d_param_bufs[q]) : nullptr;
+    s->n_pub = count;
+    s->pub_mode = mode;
+    return PHX_OK;
+}
+
+int phx_publish_params_async(phx_shard_t *s, void *stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound || s->n_pub == 0) return PHX_ERR_NOT_BOUND;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const uint64_t bytes = s->info.n_padded * model_elem_bytes(s);
+    const uint8_t *src = fp32_mode(s) ? reinterpret_cast<const uint8_t *>(s->d_p) : static_cast<const uint8_t *>(s->d_p16);
+    PHX_CK(cudaStreamWaitEvent(st, s->ev_last_step, 0));  // the newest step's kernel has written the slice
+    for (uint32_t q = 0; q < s->n_pub; ++q)
+        PHX_CK(cudaMemcpyAsync(s->d_pub[q] + (uint64_t)s->info.dp_rank * bytes, src, bytes, cudaMemcpyDefault, st));
+    return PHX_OK;
+}
+
+int phx_params_restore_from(phx_shard_t *s, const void *d_src_param_buf, void *d_dst_param_buf, void *stream)
+{
+    if (!s || !d_src_param_buf || !d_dst_param_buf) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    const uint64_t bytes = (uint64_t)s->info.dp_size * s->info.n_padded * model_elem_bytes(s);
+    PHX_CK(cudaMemcpyAsync(d_dst_param_buf, d_src_param_buf, bytes, cudaMemcpyDefault, static_cast<cudaStream_t>(stream)));
+    return PHX_OK;
+}
+
 // ---- introspection -----------------------------------------------------------------------------
 int phx_last_step(const phx_shard_t *s, uint64_t *step)
 {
@@ -943,7 +998,7 @@ int phx_kernel_launches(const phx_shard_t *s, uint64_t *count)
 int phx_set_kernel_variant(phx_shard_t *s, uint32_t variant)
 {
     if (!s || variant >= phx::kNumStepVariants) return PHX_ERR_INVALID_ARG;
-    if (variant != 0 && step_mode(s) != 0) return PHX_ERR_INVALID_ARG;  // §8(f2) modes: default flavour only
+    if (variant != 0 && step_mode(s) != 0) return PHX_ERR_INVALID_ARG;  // §8(f2)/(f3) modes: default flavour only
     s->variant = variant;
     return PHX_OK;
 }

@@ -231,7 +231,7 @@ __device__ __forceinline__ bool nodecay_at(uint64_t e, const uint64_t *__restric
 template <int HINT, int U, bool SNAP, int MODE>
 __global__ void __launch_bounds__(kStepThreads) k_step8(const __grid_constant__ StepArgs a)
 {
-    constexpr bool GF32 = (MODE & kModeF32) != 0, GROUPS = (MODE & kModeGroups) != 0;
+    constexpr bool GF32 = (MODE & kModeF32) != 0, GROUPS = (MODE & kModeGroups) != 0, PUB = (MODE & kModePublish) != 0;
     const uint64_t ngroups = a.n_padded >> 3;
     const uint64_t base = (uint64_t)blockIdx.x * (kStepThreads * U) + threadIdx.x;
     if (a.shdr != nullptr && blockIdx.x == 0 && threadIdx.x < 16)
@@ -293,6 +293,10 @@ __global__ void __launch_bounds__(kStepThreads) k_step8(const __grid_constant__ 
                 h.z = pack_bf16x2(P[u].x[4], P[u].x[5]);
                 h.w = pack_bf16x2(P[u].x[6], P[u].x[7]);
                 st128u<HINT>(reinterpret_cast<uint16_t *>(a.p16) + e, h);
+                if (PUB)  // all-gather fused into the step: the same 16 bytes go to every peer's buffer (P2P stores)
+                    for (uint32_t q = 0; q < a.n_pub; ++q) st128u<HINT>(reinterpret_cast<uint16_t *>(a.pub[q]) + e, h);
+            } else if (PUB) {
+                for (uint32_t q = 0; q < a.n_pub; ++q) st256<HINT>(reinterpret_cast<float *>(a.pub[q]) + e, P[u]);
             }
             if (SNAP) {
                 st256<HINT>(a.sp + e, P[u]);
@@ -516,12 +520,16 @@ static cudaError_t launch_tma(const StepArgs &a, bool snapshot, cudaStream_t st)
 
 cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, uint32_t mode, cudaStream_t st)
 {
-    if (mode != 0) {  // §8(f2) modes exist for the default flavour only
+    if (mode != 0) {  // §8(f2)/(f3) modes (bit set of kMode*) exist for the default flavour only
         if (variant != 0) return cudaErrorInvalidValue;
         switch (mode) {
-        case kModeF32: return launch8<1, 1, kModeF32>(a, snapshot, st);
-        case kModeGroups: return launch8<1, 1, kModeGroups>(a, snapshot, st);
-        case kModeF32 | kModeGroups: return launch8<1, 1, kModeF32 | kModeGroups>(a, snapshot, st);
+        case 1: return launch8<1, 1, 1>(a, snapshot, st);
+        case 2: return launch8<1, 1, 2>(a, snapshot, st);
+        case 3: return launch8<1, 1, 3>(a, snapshot, st);
+        case 4: return launch8<1, 1, 4>(a, snapshot, st);
+        case 5: return launch8<1, 1, 5>(a, snapshot, st);
+        case 6: return launch8<1, 1, 6>(a, snapshot, st);
+        case 7: return launch8<1, 1, 7>(a, snapshot, st);
         default: return cudaErrorInvalidValue;
         }
     }

@@ -17,6 +17,8 @@ struct alignas(16) HeaderBlob {
     uint4 q[16];
 };
 
+enum { kMaxPublish = 15 };
+
 struct StepArgs {
     float *p, *m, *v;            // live planes, n_padded each
     const void *g;               // bf16 grads (float grads under kModeF32)
@@ -29,6 +31,10 @@ struct StepArgs {
     const uint8_t *decay_cls;
     const uint64_t *decay_bnd;
     uint32_t n_bnd, first_nodecay;
+    // publication (kModePublish): the model-param copy of every element also goes to pub[0..n_pub), the
+    // rank's slice inside other DP ranks' parameter buffers (peer HBM over NVLink), already offset
+    void *pub[kMaxPublish];
+    uint32_t n_pub;
     AdamScalars sc;
     HeaderBlob hdr;
 };
@@ -36,7 +42,8 @@ struct StepArgs {
 enum { kNumStepVariants = 12 };
 // SURVEY §8(f2) modes of the fused step (default flavour only): binary32 gradients without a bf16
 // copy (the paper's precision) and per-tensor decay groups.
-enum { kModeF32 = 1, kModeGroups = 2 };
+// §8(f3): kModePublish fuses the parameter all-gather into the step (P2P stores into the peers' buffers).
+enum { kModeF32 = 1, kModeGroups = 2, kModePublish = 4 };
 enum { kDecayTileShift = 11 };  // decay_cls granularity: 2048 elements
 
 // a3.  variant selects the kernel flavour (see phx_kernels.cu); snapshot=false drops the staging stores.

@@ -18,7 +18,7 @@ class Shard:
     def __init__(self, wl: Workload, *, device="cuda:0", staging_depth=2, sync_mode=B.PHX_SYNC_STRICT,
                  chunk_bytes=0, snapshot=True, restore_mode=B.PHX_RESTORE_COPY_ENGINE,
                  max_grad_norm: Optional[float] = None, replica: Optional[torch.Tensor] = None,
-                 snapshot_source=B.PHX_SNAPSHOT_STAGED):
+                 snapshot_source=B.PHX_SNAPSHOT_STAGED, p16: Optional[torch.Tensor] = None):
         self.wl = wl
         self.device = torch.device(device)
         self.hyper: Hyper = wl.hyper
@@ -39,7 +39,12 @@ class Shard:
             self.m = torch.zeros(N, dtype=torch.float32, device=self.device)
             self.v = torch.zeros(N, dtype=torch.float32, device=self.device)
             # no bf16 model-param copy in the all-FP32 precision
-            self.p16 = None if self.fp32 else torch.zeros(N, dtype=torch.bfloat16, device=self.device)
+            # (p16 may be handed in: the rank's range inside its model-parameter buffer W)
+            if p16 is not None:
+                assert not self.fp32 and p16.dtype == torch.bfloat16 and p16.numel() == N and p16.is_contiguous()
+                self.p16 = p16
+            else:
+                self.p16 = None if self.fp32 else torch.zeros(N, dtype=torch.bfloat16, device=self.device)
             self.staging = None
             self.replica = None
             if snapshot:

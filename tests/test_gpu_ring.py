@@ -344,3 +344,78 @@ def test_peer_ring_class_two_processes_over_ipc():
     for rank, held, pred, same, back, ok in res:
         assert held == (True, (2, 3), (pred, pred)), (rank, held)
         assert same and back == 3 and ok
+
+
+# ------------------------------------------------------------------------------------------------
+# §8(f3): model-parameter publication (the all-gather fused into the step, or by copy engine) and
+# reconstruction from a surviving DP rank
+# ------------------------------------------------------------------------------------------------
+
+
+@pytest.mark.parametrize("precision", ["bf16", "fp32"])
+@pytest.mark.parametrize("mode", [B.PHX_PUBLISH_FUSED, B.PHX_PUBLISH_COPY_ENGINE])
+@pytest.mark.parametrize("D,numels", [(2, [64]), (3, [5000, 77, 2048 * 3]), (4, [100_000, 12_345])])
+def test_parameter_publication_equals_the_oracle_all_gather(D, numels, mode, precision):
+    wls = [W.tiny_workload(numels, dp_size=D, dp_rank=r, precision=precision) for r in range(D)]
+    probe = B.phx_shard_create(wls[0].layout(), D, 0)
+    L = B.phx_shard_info(probe).n_padded
+    B.phx_shard_destroy(probe)
+    mdt = torch.float32 if precision == "fp32" else torch.bfloat16
+    Wbuf = [torch.zeros(D * L, dtype=mdt, device=DEV) for _ in range(D)]          # every rank's model-parameter buffer
+    shards, oshards = [], []
+    for r, wl in enumerate(wls):
+        kw = {} if precision == "fp32" else dict(p16=Wbuf[r][r * L:(r + 1) * L])
+        s = Shard(wl, device=DEV, chunk_bytes=8192, **kw)
+        o = O.OracleShard(wl.layout(), D, r, chunk_bytes=8192, precision=precision)
+        p0 = W.init_params(s.n, s.n_padded, 30 + r)
+        s.p.copy_(p0)
+        s.set_state(0)
+        o.set_state(p0.numpy())
+        others = [Wbuf[j] for j in range(D) if j != r] + ([Wbuf[r]] if precision == "fp32" else [])
+        B.phx_shard_bind_param_peers(s.h, others, mode)
+        shards.append(s)
+        oshards.append(o)
+    st = torch.cuda.Stream(device=DEV)
+    gdt = torch.float32 if precision == "fp32" else torch.bfloat16
+    for t in range(1, 4):
+        for r, (s, o) in enumerate(zip(shards, oshards)):
+            g = W.gen_grads(wls[r], s.segments, s.n_padded, t, 30 + r, dtype=gdt)
+            s.step_and_snapshot(g.to(DEV), t)
+            if mode == B.PHX_PUBLISH_COPY_ENGINE:
+                B.phx_publish_params_async(s.h, st)
+            o.step(grad_record(g), **hp_of(wls[r]), step=t)
+        torch.cuda.synchronize()
+        want = R.publish(oshards)
+        for j in range(D):                                                        # every rank holds the same W
+            got = Wbuf[j].cpu().numpy() if precision == "fp32" else bits16(Wbuf[j])
+            assert np.array_equal(got.view(np.uint8), want.view(np.uint8)), (t, j)
+    for r, (s, o) in enumerate(zip(shards, oshards)):
+        assert_state_equal(s, o, f"rank {r}")
+    # R30: a replacement of rank 1 (or 0) reconstructs W from a surviving rank, then its optimizer shard
+    lost = min(1, D - 1)
+    fresh_W = torch.zeros_like(Wbuf[lost])
+    src = Wbuf[(lost + 1) % D]
+    B.phx_params_restore_from(shards[lost].h, src, fresh_W)
+    torch.cuda.synchronize()
+    assert torch.equal(fresh_W.view(torch.uint8), src.view(torch.uint8))
+    for s in shards:
+        B.phx_shard_bind_param_peers(s.h, [])
+        s.close()
+
+
+def test_publication_argument_errors():
+    wl = W.tiny_workload([4096], dp_size=2, dp_rank=0)
+    s = Shard(wl, device=DEV)
+    buf = torch.zeros(2 * s.n_padded, dtype=torch.bfloat16, device=DEV)
+    L = B.lib()
+    import ctypes as C
+    arr = (C.c_void_p * 16)(*[buf.data_ptr()] * 16)
+    assert L.phx_shard_bind_param_peers(s.h, arr, 16, 0) == B.PHX_ERR_INVALID_ARG
+    assert L.phx_shard_bind_param_peers(s.h, arr, 1, 2) == B.PHX_ERR_INVALID_ARG
+    assert L.phx_publish_params_async(s.h, None) == B.PHX_ERR_NOT_BOUND
+    arr2 = (C.c_void_p * 1)(buf.data_ptr() + 2)
+    assert L.phx_shard_bind_param_peers(s.h, arr2, 1, 0) == B.PHX_ERR_ALIGNMENT
+    B.phx_shard_bind_param_peers(s.h, [buf])
+    with pytest.raises(B.PhxError):
+        B.phx_set_kernel_variant(s.h, 3)            # fused publication exists for the default flavour only
+    s.close()
