@@ -74,6 +74,10 @@ def parse_args():
                     help="k ring peers the snapshot is also replicated to over NVLink (SURVEY 8(f1)); -1 = auto: 1 when "
                          "--gpus > 1 (real P2P ring over CUDA IPC), 0 at one GPU; k > 0 at one GPU measures a loopback "
                          "stand-in (received buffer on the same device)")
+    ap.add_argument("--publish", default="none", choices=["none", "fused", "copy"],
+                    help="SURVEY 8(f3): also publish the model-param copy into the other DP ranks' parameter buffers — "
+                         "fused = P2P stores from the step kernel, copy = copy engine after it.  N > 1: real buffers over "
+                         "CUDA IPC; N = 1: loopback stand-in with dp_size-1 buffers on the same GPU")
     ap.add_argument("--precision", default="bf16", choices=["bf16", "fp32"],
                     help="bf16 = fp32 state + bf16 grads + bf16 copy (north_star, default); fp32 = the paper's own "
                          "all-FP32 setting (PAPER.md:270; SURVEY 8(f2)): fp32 grads, no bf16 copy, 16 B read + 24 B written")
@@ -693,6 +697,46 @@ def run_headline(args):
                     note="replication of one packed snapshot to all k peers, copy engine, alone; max over ranks, "
                          "all ranks sending at once")
 
+    # ---- §8(f3): parameter publication (opt-in) --------------------------------------------------------
+    publication = None
+    if args.publish != "none":
+        from paper_2607_01646_b200 import ring as PR
+        pmode = B.PHX_PUBLISH_FUSED if args.publish == "fused" else B.PHX_PUBLISH_COPY_ENGINE
+        pub_stream = torch.cuda.Stream(device=device)
+        try:
+            if world > 1:
+                pg, npeers = PR.ParamGroup(rig.s, pmode, ring_size=world, ring_rank=rank), world
+                plink = "NVLink/NVSwitch P2P into every rank's parameter buffer (CUDA IPC), own buffer included"
+            else:
+                npeers = min(wl.dp_size - 1, B.PHX_MAX_PARAM_PEERS)
+                lbufs = [torch.zeros(wl.dp_size * N, dtype=torch.float32 if rig.fp32 else torch.bfloat16, device=device)
+                         for _ in range(npeers)]
+                B.phx_shard_bind_param_peers(rig.s.h, lbufs, pmode)
+                pg = None
+                plink = "loopback stand-in: dp_size-1 parameter buffers on the SAME GPU (HBM writes, not NVLink)"
+            for _ in range(3):
+                rig.do_step()
+            torch.cuda.synchronize()
+            barrier(world)
+            q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            q0.record(rig.cur)
+            for _ in range(20):
+                rig.do_step()
+                if pmode == B.PHX_PUBLISH_COPY_ENGINE:
+                    B.phx_publish_params_async(rig.s.h, pub_stream)
+                    rig.cur.wait_stream(pub_stream)      # the next forward pass needs the published parameters
+            q1.record(rig.cur)
+            torch.cuda.synchronize()
+            barrier(world)
+            pms = max_over_ranks(q0.elapsed_time(q1) / 20, world, device)
+            publication = {"mode": args.publish, "buffers_written": npeers, "link": plink, "step_plus_publish_ms": pms,
+                           "bytes_published_per_step": int(npeers * N * (4 if rig.fp32 else 2))}
+            B.phx_shard_bind_param_peers(rig.s.h, [])
+            if pg is not None:
+                pg.close()
+        except Exception as e:  # noqa: BLE001
+            publication = {"mode": args.publish, "error": str(e)[:300]}
+
     host_link = overlap = restore = cpu = None
     if rank == 0:
         # flush alone (a4+a5) against the measured pinned-copy peak
@@ -755,7 +799,7 @@ def run_headline(args):
             "elements_per_s": units / (ms_per_step * 1e-3),
             "exposed_ckpt_ms_per_iter": overlap["exposed_ms"] if overlap else None,
             "roofline": roofline, "host_link": host_link, "e2e": e2e, "overlap": overlap, "restore": restore,
-            "peer_replication": peer, "cpu_baseline": cpu, "gpu_launches": int(launches), "clocks": clk,
+            "peer_replication": peer, "publication": publication, "cpu_baseline": cpu, "gpu_launches": int(launches), "clocks": clk,
             "step_ms_min_max": [min(per), max(per)],
         }
         print(json.dumps(line), flush=True)

@@ -36,6 +36,17 @@ def route_handles(table: Sequence[Sequence[bytes]], dp_size: int, dp_rank: int, 
     return [table[h][j] for j, h in enumerate(successors(dp_size, dp_rank, k))]
 
 
+class _Raw:
+    def __init__(self, ptr: int, nbytes: int):
+        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False), "version": 2}
+
+
+def device_view(ptr: int, nbytes: int):
+    """Zero-copy uint8 torch view of a raw device address (memory owned by libphx allocations)."""
+    import torch
+    return torch.as_tensor(_Raw(ptr, nbytes), device="cuda")
+
+
 class ReceivedBuffers:
     """The k received buffers (two snapshot slots each) a rank keeps for its ring predecessors."""
 
@@ -48,13 +59,7 @@ class ReceivedBuffers:
 
     def view(self, j: int):
         """Zero-copy uint8 torch view of the buffer kept for predecessor j (1-based), for inspection."""
-        import torch
-
-        class _Raw:
-            def __init__(self, ptr, nbytes):
-                self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False),
-                                                 "version": 2}
-        return torch.as_tensor(_Raw(self.ptrs[j - 1], 2 * self.slot_stride), device="cuda")
+        return device_view(self.ptrs[j - 1], 2 * self.slot_stride)
 
     def inspect(self, j: int):
         """[(header, valid)] of the buffer kept for predecessor j (1-based)."""
@@ -119,6 +124,66 @@ class PeerRing:
         if self.received is not None:
             self.received.free()
             self.received = None
+
+
+class ParamGroup:
+    """one rank's end of the model-parameter publication.  Every rank of the DP group owns
+    a model-parameter buffer W (dp_size * n_padded model-dtype elements, IPC-exportable); the others' buffers
+    are opened over CUDA IPC and bound, so that the fused step kernel (PHX_PUBLISH_FUSED) or the copy engine
+    (PHX_PUBLISH_COPY_ENGINE) writes this rank's range into all of them — the all-gather."""
+
+    def __init__(self, shard, mode=B.PHX_PUBLISH_FUSED, group=None, ring_size: Optional[int] = None,
+                 ring_rank: Optional[int] = None):
+        import torch.distributed as dist
+        self.shard = shard
+        D = shard.info.dp_size if ring_size is None else ring_size
+        r = shard.info.dp_rank if ring_rank is None else ring_rank
+        assert dist.is_initialized() and dist.get_world_size(group) == D and dist.get_rank(group) == r
+        assert D <= B.PHX_MAX_PARAM_PEERS
+        elem = 4 if shard.fp32 else 2
+        self.nbytes = shard.info.dp_size * shard.info.n_padded * elem
+        self.own, self.opened, err = None, [], None
+        try:
+            self.own = B.phx_peer_buffer_alloc(self.nbytes)
+            mine = B.phx_ipc_export(self.own)
+        except Exception as e:  # noqa: BLE001
+            mine, err = None, repr(e)
+        table: List[Optional[bytes]] = [None] * D
+        dist.all_gather_object(table, mine, group=group)
+        if err is None and all(t is not None for t in table):
+            try:
+                self.opened = [B.phx_ipc_open(table[j]) for j in range(D) if j != r]
+                # the rank's own W is bound like a peer: its range is written there too (the shard keeps a
+                # separate d_p_bf16; 2 B/element of local writes buys independence from allocation order)
+                B.phx_shard_bind_param_peers(shard.h, [self.own] + self.opened, mode)
+            except Exception as e:  # noqa: BLE001
+                err = repr(e)
+        elif err is None:
+            err = "a peer could not allocate its parameter buffer"
+        status: List[Optional[str]] = [None] * D
+        dist.all_gather_object(status, err, group=group)
+        if any(x is not None for x in status):
+            self.close()
+            raise RuntimeError("ParamGroup set-up failed: " + "; ".join(f"rank {i}: {x}" for i, x in enumerate(status) if x))
+
+    def publish_async(self, stream):
+        B.phx_publish_params_async(self.shard.h, stream)
+
+    def view(self):
+        """Zero-copy torch view (model dtype) of this rank's parameter buffer W."""
+        import torch
+        t = device_view(self.own, self.nbytes)
+        return t.view(torch.float32 if self.shard.fp32 else torch.bfloat16)
+
+    def close(self):
+        if self.opened:
+            B.phx_shard_bind_param_peers(self.shard.h, [])
+        for p in self.opened:
+            B.phx_ipc_close(p)
+        self.opened = []
+        if self.own is not None:
+            B.phx_peer_buffer_free(self.own)
+            self.own = None
 
 
 def connect_in_process(shards: Sequence, k: int) -> List[ReceivedBuffers]:

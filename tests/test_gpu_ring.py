@@ -419,3 +419,52 @@ def test_publication_argument_errors():
     with pytest.raises(B.PhxError):
         B.phx_set_kernel_variant(s.h, 3)            # fused publication exists for the default flavour only
     s.close()
+
+
+def _param_rank(rank, world, port, mode, q):
+    import torch.distributed as dist
+    os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    torch.cuda.set_device(0)
+    dist.init_process_group("gloo")
+    wl = W.tiny_workload([40_000, 77], dp_size=world, dp_rank=rank)
+    s = Shard(wl, device=DEV)
+    o = O.OracleShard(wl.layout(), world, rank)
+    p0 = W.init_params(s.n, s.n_padded, 70 + rank)
+    s.p.copy_(p0)
+    s.set_state(0)
+    o.set_state(p0.numpy())
+    pg = PR.ParamGroup(s, mode)
+    st = torch.cuda.Stream(device=DEV)
+    for t in range(1, 3):
+        g = W.gen_grads(wl, s.segments, s.n_padded, t, 70 + rank)
+        s.step_and_snapshot(g.to(DEV), t)
+        if mode == B.PHX_PUBLISH_COPY_ENGINE:
+            pg.publish_async(st)
+        o.step(grad_record(g), **hp_of(wl), step=t)
+    torch.cuda.synchronize()
+    dist.barrier()                      # every rank's stores into my W have completed
+    mine = bits16(pg.view())
+    gathered = [None] * world
+    dist.all_gather_object(gathered, o.p16.tobytes())           # the oracle's all-gather (control plane, gloo)
+    want = np.frombuffer(b"".join(gathered), np.uint16)
+    q.put((rank, bool(np.array_equal(mine, want)), bool(np.array_equal(bits16(s.p16), o.p16))))
+    dist.barrier()
+    pg.close()
+    s.close()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("mode", [B.PHX_PUBLISH_FUSED, B.PHX_PUBLISH_COPY_ENGINE])
+def test_param_group_two_processes_over_ipc(mode):
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29900 + (os.getpid() + mode) % 40
+    ps = [ctx.Process(target=_param_rank, args=(r, world, port, mode, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    res = sorted(q.get(timeout=300) for _ in ps)
+    for p in ps:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    assert res == [(0, True, True), (1, True, True)]
