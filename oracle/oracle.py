@@ -187,11 +187,14 @@ assert struct.calcsize(_HDR_FMT) == 240
 
 
 def pack_header(*, step, n, n_padded, total_numel, shard_begin, layout_hash, dp, tp, pp,
-                chunk_bytes, user=b"", committed=True) -> bytes:
+                chunk_bytes, user=b"", committed=True, payload=0) -> bytes:
+    """`payload` (the u32 after user_len): 0 = optimizer-only payload (the H2H payload, PAPER.md:146);
+    1 | elem_bytes << 8 = full rank state, the model-parameter buffer follows p ‖ m ‖ v
+    (the D2H payload, reading R31 — see oracle/rank_state.py)."""
     assert len(user) <= 128
     body = struct.pack(_HDR_FMT, MAGIC, VERSION, HEADER_BYTES, step, step, n, n_padded,
                        total_numel, shard_begin, layout_hash, dp[0], dp[1], tp[0], tp[1],
-                       pp[0], pp[1], chunk_bytes, len(user), 0, user.ljust(128, b"\0"))
+                       pp[0], pp[1], chunk_bytes, len(user), payload, user.ljust(128, b"\0"))
     return body + struct.pack("<QQ", fnv1a64(body), step if committed else 0)
 
 
@@ -208,7 +211,7 @@ def parse_header(raw: bytes) -> Optional[dict]:
         return None
     return dict(seq=f[3], step=f[4], n=f[5], n_padded=f[6], total_numel=f[7], shard_begin=f[8],
                 layout_hash=f[9], dp=(f[10], f[11]), tp=(f[12], f[13]), pp=(f[14], f[15]),
-                chunk_bytes=f[16], user=f[19][:f[17]])
+                chunk_bytes=f[16], user=f[19][:f[17]], payload=f[18])
 
 
 # ----------------------------------------------------------------------------
