@@ -64,7 +64,8 @@ enum {
     PHX_ERR_CUDA = -9,                /* see phx_last_cuda_error                                  */
     PHX_ERR_UNSUPPORTED_DEVICE = -10, /* not compute capability 10.x; there is no fallback       */
     PHX_ERR_SNAPSHOT_DISABLED = -11,  /* flush/restore asked of a shard created with snapshots off */
-    PHX_ERR_NOMEM = -12
+    PHX_ERR_NOMEM = -12,
+    PHX_ERR_PARAMS_NOT_READY = -13    /* full-rank-state flush before phx_params_ready for that step  */
 };
 
 /* ---- types ----------------------------------------------------------------------------- */
@@ -90,6 +91,14 @@ enum { PHX_SNAPSHOT_STAGED = 0, PHX_SNAPSHOT_DIRECT = 1 };
  * gradients are float[n_padded], there is no bf16 copy (d_p_bf16 may be NULL) and the fused kernel moves
  * 16 B read + 24 B written per element (12 written with snapshots off). */
 enum { PHX_PRECISION_BF16_GRADS = 0, PHX_PRECISION_FP32 = 1 };
+/* What the LOCAL host slots hold (the payloads are asymmetric by design).
+ * PHX_PAYLOAD_OPTIMIZER (default): envelope ‖ p ‖ m ‖ v — the H2H payload, which is what the
+ * host replica holds when it stands in for the peer (BASELINE.json:north_star).
+ * PHX_PAYLOAD_FULL_RANK_STATE: the D2H payload of PAPER.md:145 — "the optimizer-state shard, the local
+ * model-parameter shard, and a metadata envelope" — envelope ‖ p ‖ m ‖ v ‖ W, where W is the rank's
+ * model-parameter buffer (see phx_shard_bind_params), so that a transient GPU fault is recovered in place
+ * "without any network transfer".  Ring peers still receive the optimizer-only snapshot. */
+enum { PHX_PAYLOAD_OPTIMIZER = 0, PHX_PAYLOAD_FULL_RANK_STATE = 1 };
 
 /* Any field left 0 takes its default; cfg == NULL means all defaults. */
 typedef struct {
@@ -115,7 +124,8 @@ typedef struct {
                                  (exactly the paper's sync point); requires PHX_SYNC_STRICT.
                                  The kernel then moves 28 B/element instead of 40.                           */
     uint32_t precision;       /* PHX_PRECISION_BF16_GRADS (default) | PHX_PRECISION_FP32                   */
-    uint32_t reserved[3];
+    uint32_t payload;         /* PHX_PAYLOAD_OPTIMIZER (default) | PHX_PAYLOAD_FULL_RANK_STATE (local slots) */
+    uint32_t reserved[2];
 } phx_config_t;
 
 typedef struct {
@@ -128,6 +138,10 @@ typedef struct {
     uint64_t slot_stride;    /* snapshot_bytes rounded up to 256                                  */
     uint32_t n_segments, staging_depth;
     uint32_t dp_size, dp_rank;
+    /* local host slots (h_replica): equal to snapshot_bytes / slot_stride under PHX_PAYLOAD_OPTIMIZER;
+     * under PHX_PAYLOAD_FULL_RANK_STATE host_snapshot_bytes = snapshot_bytes + param_bytes */
+    uint64_t host_snapshot_bytes, host_slot_stride;
+    uint64_t param_bytes;    /* dp_size * n_padded * (2 | 4): size of the model-parameter buffer W   */
 } phx_shard_info_t;
 
 /* The 256-byte metadata envelope at the front of every snapshot slot. */
@@ -141,7 +155,7 @@ typedef struct {
     uint32_t dp_size, dp_rank, tp_size, tp_rank, pp_size, pp_rank;
     uint64_t chunk_bytes;
     uint32_t user_len;      /* bytes used of user[]                                               */
-    uint32_t reserved;
+    uint32_t payload;       /* 0: p ‖ m ‖ v follow; 1 | elem_bytes << 8: p ‖ m ‖ v ‖ W follow (full rank state) */
     uint8_t user[128];      /* opaque caller blob (RNG states...), restored bit-exactly           */
     uint64_t header_hash;   /* FNV-1a 64 of bytes [0, 240)                                        */
     uint64_t seq_end;       /* == seq_begin once the slot is committed; written last              */
@@ -308,6 +322,35 @@ PHX_API int phx_publish_params_async(phx_shard_t *s, void *stream);
  * of the same TP/PP coordinate: one copy of the whole buffer W (dp_size * n_padded model-dtype elements)
  * from `d_src_param_buf` (peer HBM) into `d_dst_param_buf`. */
 PHX_API int phx_params_restore_from(phx_shard_t *s, const void *d_src_param_buf, void *d_dst_param_buf, void *stream);
+
+/* ---- full rank-state local snapshot and in-place recovery ---------------------
+ * With cfg.payload = PHX_PAYLOAD_FULL_RANK_STATE the local host slots hold the D2H payload of
+ * envelope(payload = 1 | elem_bytes << 8) ‖ p ‖ m ‖ v ‖ W, host_snapshot_bytes long at
+ * host_slot_stride (h_replica of phx_shard_bind must then hold 2 * host_slot_stride bytes).  W is the
+ * model-parameter buffer the rank holds for its TP/PP partition (the buffer of §8(f3): dp_size * n_padded
+ * elements of the model dtype, rank r's range at element r * n_padded); in PHX_PRECISION_BF16_GRADS
+ * d_p_bf16 of phx_shard_bind must be the rank's own range inside it (d_W + dp_rank * n_padded elements).
+ * Staging slots and ring-peer slots keep the optimizer-only layout.
+ *
+ * Protocol per step k:  phx_step_and_snapshot(k)  →  [the partition's all-gather of step k lands in W]  →
+ * phx_params_ready(stream): the caller declares, in `stream` order, that W now holds every rank's
+ * parameters after step k  →  phx_snapshot_flush_async: waits for the step's kernel AND for that
+ * declaration (PHX_ERR_PARAMS_NOT_READY if it was not made for step k), then header invalidated, W in
+ * chunk_bytes pieces, p ‖ m ‖ v in chunk_bytes pieces, valid header last (W first: it is the part other
+ * ranks overwrite at their next publication).  phx_fault_inject_torn_flush counts chunks in that order.
+ * phx_params_guard(stream): `stream` waits until the newest flush has finished READING W — to be enqueued
+ * ahead of whatever lets other ranks publish step k+1 into this rank's W (handing this rank's gradients to
+ * the reduce-scatter of iteration k+1; a local copy-engine publication).  The rank's own step k+1 is
+ * covered by the sync point of phx_step_and_snapshot as before.
+ *
+ * phx_restore on such a shard is the in-place recovery: p, m, v AND W come back from
+ * the rank's own host slot (newest valid slot whose payload word and identity match), nothing is read from
+ * any other rank; the rank's own range of W equals RNE_bf16(p) again by construction.  Copy engine only
+ * (cfg.restore_mode is ignored for the W part).  phx_restore_from (a peer's optimizer-only replica) and
+ * phx_params_restore_from remain the permanent-failure path. */
+PHX_API int phx_shard_bind_params(phx_shard_t *s, void *d_W);
+PHX_API int phx_params_ready(phx_shard_t *s, void *stream);
+PHX_API int phx_params_guard(phx_shard_t *s, void *stream);
 
 /* ---- introspection ---------------------------------------------------------------------- */
 PHX_API int phx_last_step(const phx_shard_t *s, uint64_t *step);

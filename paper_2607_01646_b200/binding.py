@@ -30,11 +30,13 @@ PHX_ERR_CUDA = -9
 PHX_ERR_UNSUPPORTED_DEVICE = -10
 PHX_ERR_SNAPSHOT_DISABLED = -11
 PHX_ERR_NOMEM = -12
+PHX_ERR_PARAMS_NOT_READY = -13
 
 PHX_SYNC_STRICT, PHX_SYNC_RELAXED = 0, 1
 PHX_RESTORE_COPY_ENGINE, PHX_RESTORE_BULK_KERNEL = 0, 1
 PHX_SNAPSHOT_STAGED, PHX_SNAPSHOT_DIRECT = 0, 1
 PHX_PRECISION_BF16_GRADS, PHX_PRECISION_FP32 = 0, 1
+PHX_PAYLOAD_OPTIMIZER, PHX_PAYLOAD_FULL_RANK_STATE = 0, 1
 PHX_TENSOR_NO_DECAY = 1
 
 
@@ -47,7 +49,8 @@ class phx_config_t(C.Structure):
                 ("pp_rank", C.c_uint32), ("staging_depth", C.c_uint32), ("sync_mode", C.c_uint32),
                 ("chunk_bytes", C.c_uint64), ("snapshot_disabled", C.c_uint32),
                 ("restore_mode", C.c_uint32), ("max_grad_norm", C.c_float),
-                ("snapshot_source", C.c_uint32), ("precision", C.c_uint32), ("reserved", C.c_uint32 * 3)]
+                ("snapshot_source", C.c_uint32), ("precision", C.c_uint32), ("payload", C.c_uint32),
+                ("reserved", C.c_uint32 * 2)]
 
 
 class phx_shard_info_t(C.Structure):
@@ -55,7 +58,8 @@ class phx_shard_info_t(C.Structure):
                 ("shard_begin", C.c_uint64), ("layout_hash", C.c_uint64),
                 ("snapshot_bytes", C.c_uint64), ("slot_stride", C.c_uint64),
                 ("n_segments", C.c_uint32), ("staging_depth", C.c_uint32),
-                ("dp_size", C.c_uint32), ("dp_rank", C.c_uint32)]
+                ("dp_size", C.c_uint32), ("dp_rank", C.c_uint32),
+                ("host_snapshot_bytes", C.c_uint64), ("host_slot_stride", C.c_uint64), ("param_bytes", C.c_uint64)]
 
 
 class phx_snapshot_header_t(C.Structure):
@@ -64,7 +68,7 @@ class phx_snapshot_header_t(C.Structure):
                 ("total_numel", C.c_uint64), ("shard_begin", C.c_uint64), ("layout_hash", C.c_uint64),
                 ("dp_size", C.c_uint32), ("dp_rank", C.c_uint32), ("tp_size", C.c_uint32), ("tp_rank", C.c_uint32),
                 ("pp_size", C.c_uint32), ("pp_rank", C.c_uint32), ("chunk_bytes", C.c_uint64),
-                ("user_len", C.c_uint32), ("reserved", C.c_uint32), ("user", C.c_uint8 * 128),
+                ("user_len", C.c_uint32), ("payload", C.c_uint32), ("user", C.c_uint8 * 128),
                 ("header_hash", C.c_uint64), ("seq_end", C.c_uint64)]
 
 
@@ -124,6 +128,9 @@ PROTOTYPES = {
     "phx_shard_bind_param_peers": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.c_uint32, C.c_uint32]),
     "phx_publish_params_async": (C.c_int, [C.c_void_p, C.c_void_p]),
     "phx_params_restore_from": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "phx_shard_bind_params": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "phx_params_ready": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "phx_params_guard": (C.c_int, [C.c_void_p, C.c_void_p]),
 }
 
 
@@ -169,7 +176,8 @@ def phx_shard_create(layout: Sequence[Tuple[int, int]], dp_size: int, dp_rank: i
                      pp=(1, 0), staging_depth=0, sync_mode=PHX_SYNC_STRICT, chunk_bytes=0,
                      snapshot_disabled=False, restore_mode=PHX_RESTORE_COPY_ENGINE,
                      max_grad_norm=0.0, snapshot_source=PHX_SNAPSHOT_STAGED,
-                     flags: Optional[Sequence[int]] = None, precision=PHX_PRECISION_BF16_GRADS) -> int:
+                     flags: Optional[Sequence[int]] = None, precision=PHX_PRECISION_BF16_GRADS,
+                     payload=PHX_PAYLOAD_OPTIMIZER) -> int:
     """layout = [(numel, tensor_id)] in flattening order.  Returns the opaque handle."""
     n = len(layout)
     arr = (phx_tensor_desc_t * max(n, 1))()
@@ -179,7 +187,8 @@ def phx_shard_create(layout: Sequence[Tuple[int, int]], dp_size: int, dp_rank: i
     cfg = phx_config_t(tp_size=tp[0], tp_rank=tp[1], pp_size=pp[0], pp_rank=pp[1],
                        staging_depth=staging_depth, sync_mode=sync_mode, chunk_bytes=chunk_bytes,
                        snapshot_disabled=1 if snapshot_disabled else 0, restore_mode=restore_mode,
-                       max_grad_norm=max_grad_norm, snapshot_source=snapshot_source, precision=precision)
+                       max_grad_norm=max_grad_norm, snapshot_source=snapshot_source, precision=precision,
+                       payload=payload)
     h = C.c_void_p()
     _ck(lib().phx_shard_create(arr, n, dp_size, dp_rank, C.byref(cfg), C.byref(h)), "phx_shard_create")
     return h.value
@@ -368,3 +377,18 @@ def phx_publish_params_async(h: int, stream=None) -> None:
 def phx_params_restore_from(h: int, d_src_param_buf, d_dst_param_buf, stream=None) -> None:
     _ck(lib().phx_params_restore_from(h, _ptr(d_src_param_buf), _ptr(d_dst_param_buf), _ptr(stream)),
         "phx_params_restore_from", h)
+
+
+# ---- full rank-state local snapshot ---------------------------------------------
+
+
+def phx_shard_bind_params(h: int, d_W) -> None:
+    _ck(lib().phx_shard_bind_params(h, _ptr(d_W)), "phx_shard_bind_params", h)
+
+
+def phx_params_ready(h: int, stream=None) -> None:
+    _ck(lib().phx_params_ready(h, _ptr(stream)), "phx_params_ready", h)
+
+
+def phx_params_guard(h: int, stream=None) -> None:
+    _ck(lib().phx_params_guard(h, _ptr(stream)), "phx_params_guard", h)

@@ -36,7 +36,8 @@ constexpr size_t kScrCoef = 260;       // float: clip coefficient of the current
 constexpr size_t kScrSumsq = 264;      // double
 constexpr size_t kScrPartials = 512;   // kSumsqMaxBlocks doubles
 constexpr size_t kScrHdr = kScrPartials + phx::kSumsqMaxBlocks * sizeof(double);  // 2 x 256 B headers (direct mode)
-constexpr size_t kScrBytes = kScrHdr + 2 * 256;
+constexpr size_t kScrHdrFull = kScrHdr + 2 * 256;  // kMaxDepth x 256 B full-rank-state headers (§8(f4))
+constexpr size_t kScrBytes = kScrHdrFull + 4 * 256;
 
 uint64_t fnv1a64(const void *data, size_t len, uint64_t h = 0xCBF29CE484222325ull)
 {
@@ -116,6 +117,12 @@ struct phx_shard {
     uint32_t n_pub = 0, pub_mode = PHX_PUBLISH_FUSED;
     uint8_t *d_pub[PHX_MAX_PARAM_PEERS] = {nullptr};
     cudaEvent_t ev_last_step = nullptr;  // recorded after every step's kernel (publication by copy engine waits on it)
+    // §8(f4) full rank-state local snapshot: the model-parameter buffer W and its readiness / guard events
+    uint8_t *d_W = nullptr;
+    cudaEvent_t ev_params = nullptr;   // W holds every rank's parameters after step params_ready_step
+    cudaEvent_t ev_wflush = nullptr;   // the newest local flush has finished reading W
+    uint64_t params_ready_step = 0;
+    bool params_ready = false, wflush_valid = false;
     // misc
     int last_cuda_error = 0;
     uint64_t launches = 0;
@@ -134,7 +141,7 @@ struct phx_shard {
 
 namespace {
 
-void build_header(const phx_shard *s, uint64_t step, bool committed, phx_snapshot_header_t *h)
+void build_header(const phx_shard *s, uint64_t step, bool committed, phx_snapshot_header_t *h, uint32_t payload = 0)
 {
     static_assert(sizeof(phx_snapshot_header_t) == 256, "envelope must be 256 bytes");
     std::memset(h, 0, sizeof(*h));
@@ -156,6 +163,7 @@ void build_header(const phx_shard *s, uint64_t step, bool committed, phx_snapsho
     h->pp_rank = s->cfg.pp_rank;
     h->chunk_bytes = s->cfg.chunk_bytes;
     h->user_len = s->user_len;
+    h->payload = payload;
     std::memcpy(h->user, s->user, s->user_len);
     h->header_hash = fnv1a64(h, 240);
     h->seq_end = committed ? step : 0;
@@ -186,6 +194,8 @@ uint32_t step_mode(const phx_shard *s)
            ((s->n_pub && s->pub_mode == PHX_PUBLISH_FUSED) ? (uint32_t)phx::kModePublish : 0u);
 }
 uint64_t model_elem_bytes(const phx_shard *s) { return fp32_mode(s) ? 4u : 2u; }
+bool full_payload(const phx_shard *s) { return s->cfg.payload == PHX_PAYLOAD_FULL_RANK_STATE; }
+uint32_t full_payload_word(const phx_shard *s) { return 1u | ((uint32_t)model_elem_bytes(s) << 8); }
 
 // Decay groups: walk the rank's segments in shard order, record the offsets at which the no-decay flag
 // toggles and classify every 2048-element tile as all-decay (0), all-no-decay (1) or mixed (2).  Pad
@@ -254,11 +264,15 @@ int settle_peer_slots(phx_shard *s, bool block) { return settle_slots(s, s->peer
 // destination header, copy the payload in chunk_bytes pieces (from the staging slot, or from the live
 // planes in direct mode), copy the valid header last.  torn_chunks >= 0: stop after that many payload
 // chunks and never commit (fault injection).
-int enqueue_snapshot_copy(phx_shard *s, cudaStream_t st, uint8_t *dst, cudaMemcpyKind kind, int slot, int64_t torn_chunks)
+// full = true (§8(f4), local slot only): the model-parameter buffer W goes first, behind the optimizer part,
+// and the committed header is the full-rank-state one; ev_wflush marks the end of the reads of W.
+int enqueue_snapshot_copy(phx_shard *s, cudaStream_t st, uint8_t *dst, cudaMemcpyKind kind, int slot, int64_t torn_chunks,
+                          bool full = false)
 {
     const bool direct = direct_mode(s);
     const uint8_t *src = direct ? nullptr : s->d_staging + (uint64_t)slot * s->info.slot_stride;
     const uint8_t *src_hdr = direct ? s->d_scratch + kScrHdr + (size_t)slot * kHeaderBytes : src;
+    if (full) src_hdr = s->d_scratch + kScrHdrFull + (size_t)slot * kHeaderBytes;
     const bool torn = torn_chunks >= 0;
     // 1. invalidate the target slot's header; the OTHER slot keeps the previous committed snapshot
     PHX_CK(cudaMemcpyAsync(dst, s->d_scratch + kScrZeroHdr, kHeaderBytes, kind, st));
@@ -266,7 +280,21 @@ int enqueue_snapshot_copy(phx_shard *s, cudaStream_t st, uint8_t *dst, cudaMemcp
     const uint64_t payload = s->info.snapshot_bytes - kHeaderBytes;
     const uint64_t chunk = s->cfg.chunk_bytes;
     uint64_t done_chunks = 0;
-    for (uint64_t off = 0; off < payload; off += chunk, ++done_chunks) {
+    bool stopped = false;
+    if (full) {  // 2a. W, read from the live model-parameter buffer
+        uint8_t *wdst = dst + s->info.snapshot_bytes;
+        for (uint64_t off = 0; off < s->info.param_bytes; off += chunk, ++done_chunks) {
+            if (torn && (int64_t)done_chunks >= torn_chunks) {
+                stopped = true;
+                break;
+            }
+            const uint64_t len = s->info.param_bytes - off < chunk ? s->info.param_bytes - off : chunk;
+            PHX_CK(cudaMemcpyAsync(wdst + off, s->d_W + off, len, kind, st));
+        }
+        PHX_CK(cudaEventRecord(s->ev_wflush, st));
+        s->wflush_valid = true;
+    }
+    for (uint64_t off = 0; off < payload && !stopped; off += chunk, ++done_chunks) {
         if (torn && (int64_t)done_chunks >= torn_chunks) break;
         const uint64_t len = payload - off < chunk ? payload - off : chunk;
         if (!direct) {
@@ -314,6 +342,7 @@ const char *phx_strerror(int err)
     case PHX_ERR_UNSUPPORTED_DEVICE: return "device is not compute capability 10.x";
     case PHX_ERR_SNAPSHOT_DISABLED: return "snapshots are disabled on this shard";
     case PHX_ERR_NOMEM: return "out of memory";
+    case PHX_ERR_PARAMS_NOT_READY: return "model-parameter buffer not declared ready for this step";
     default: return "unknown error";
     }
 }
@@ -339,6 +368,7 @@ int phx_shard_create(const phx_tensor_desc_t *layout, size_t n_tensors, uint32_t
     if (c.tp_rank >= c.tp_size || c.pp_rank >= c.pp_size || c.staging_depth > kMaxDepth ||
         c.sync_mode > PHX_SYNC_RELAXED || c.restore_mode > PHX_RESTORE_BULK_KERNEL || !(c.max_grad_norm == c.max_grad_norm) ||
         c.snapshot_source > PHX_SNAPSHOT_DIRECT || c.precision > PHX_PRECISION_FP32 ||
+        c.payload > PHX_PAYLOAD_FULL_RANK_STATE || (c.payload == PHX_PAYLOAD_FULL_RANK_STATE && c.snapshot_disabled) ||
         (c.snapshot_source == PHX_SNAPSHOT_DIRECT && c.sync_mode != PHX_SYNC_STRICT)) {
         delete s;
         return PHX_ERR_INVALID_ARG;
@@ -384,6 +414,9 @@ int phx_shard_create(const phx_tensor_desc_t *layout, size_t n_tensors, uint32_t
     i.staging_depth = c.snapshot_source == PHX_SNAPSHOT_DIRECT ? 0 : c.staging_depth;
     i.dp_size = dp_size;
     i.dp_rank = dp_rank;
+    i.param_bytes = (uint64_t)dp_size * L * model_elem_bytes(s);
+    i.host_snapshot_bytes = i.snapshot_bytes + (full_payload(s) ? i.param_bytes : 0);
+    i.host_slot_stride = (i.host_snapshot_bytes + 255) & ~255ull;
     build_decay_groups(s);
     *out = s;
     return PHX_OK;
@@ -406,6 +439,8 @@ int phx_shard_destroy(phx_shard_t *s)
             if (s->ev_peer[k]) cudaEventDestroy(s->ev_peer[k]);
         }
         if (s->ev_last_step) cudaEventSynchronize(s->ev_last_step), cudaEventDestroy(s->ev_last_step);
+        if (s->ev_params) cudaEventDestroy(s->ev_params);
+        if (s->ev_wflush) cudaEventDestroy(s->ev_wflush);
         if (s->d_scratch) cudaFree(s->d_scratch);
         if (s->d_decay) cudaFree(s->d_decay);
     }
@@ -472,6 +507,8 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
         PHX_CK(cudaEventCreateWithFlags(&s->ev_pflush[k], cudaEventDisableTiming));
     }
     PHX_CK(cudaEventCreateWithFlags(&s->ev_last_step, cudaEventDisableTiming));
+    PHX_CK(cudaEventCreateWithFlags(&s->ev_params, cudaEventDisableTiming));
+    PHX_CK(cudaEventCreateWithFlags(&s->ev_wflush, cudaEventDisableTiming));
     for (int k = 0; k < 2; ++k) {
         PHX_CK(cudaEventCreateWithFlags(&s->ev_host[k], cudaEventDisableTiming));
         PHX_CK(cudaEventCreateWithFlags(&s->ev_peer[k], cudaEventDisableTiming));
@@ -578,6 +615,13 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
         phx_snapshot_header_t hdr;
         build_header(s, step, true, &hdr);
         std::memcpy(&a.hdr, &hdr, sizeof(hdr));
+        if (full_payload(s)) {  // §8(f4): the local slot's envelope differs in the payload word and the hash
+            phx_snapshot_header_t hf;
+            build_header(s, step, true, &hf, full_payload_word(s));
+            a.shdr_full = s->d_scratch + kScrHdrFull + (size_t)slot * kHeaderBytes;
+            a.full_payload = hf.payload;
+            a.full_hash = hf.header_hash;
+        }
     }
     a.p = s->d_p;
     a.m = s->d_m;
@@ -609,6 +653,7 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
         s->pending_peer_step = step;
     }
     s->last_step = step;
+    s->params_ready = false;
     return PHX_OK;
 }
 
@@ -623,7 +668,13 @@ int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream)
     const int slot = s->pending_slot;
     const uint64_t step = s->pending_step;
     const int hs = (int)(step & 1);  // ping-pong
-    uint8_t *dst = s->h_replica + (uint64_t)hs * s->info.slot_stride;
+    uint8_t *dst = s->h_replica + (uint64_t)hs * s->info.host_slot_stride;
+    const bool full = full_payload(s);
+    if (full) {
+        if (!s->d_W) return PHX_ERR_NOT_BOUND;
+        if (!s->params_ready || s->params_ready_step != step) return PHX_ERR_PARAMS_NOT_READY;
+        PHX_CK(cudaStreamWaitEvent(st, s->ev_params, 0));  // the all-gather of this step has landed in W
+    }
 
     PHX_CK(cudaStreamWaitEvent(st, s->ev_step[slot], 0));  // the step's kernel has written the slot
     if (s->last_flush_slot >= 0)                            // flushes are serialised whatever stream they use
@@ -632,7 +683,7 @@ int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream)
     const bool torn = s->torn_chunks >= 0;
     s->host[hs].step = step;
     s->host[hs].state = torn ? SLOT_TORN_INFLIGHT : SLOT_INFLIGHT;
-    int rc = enqueue_snapshot_copy(s, st, dst, cudaMemcpyDeviceToHost, slot, s->torn_chunks);
+    int rc = enqueue_snapshot_copy(s, st, dst, cudaMemcpyDeviceToHost, slot, s->torn_chunks, full);
     if (rc != PHX_OK) return rc;
     PHX_CK(cudaEventRecord(s->ev_flush[slot], st));
     PHX_CK(cudaEventRecord(s->ev_host[hs], st));
@@ -682,25 +733,28 @@ namespace {
 // Rebuild the live shard from `replica` (two slots at slot_stride).  hdr_src: where the host can read the
 // two headers with a blocking copy; copy_src: address for copy-engine copies; kern_src: device-visible
 // address for the bulk kernel.  Selection depends only on what is IN the replica.
+// stride: distance of the two slots; want_payload: the envelope's payload word the slot must carry (0 =
+// optimizer-only; the full-rank-state word: the model-parameter buffer W behind p ‖ m ‖ v is restored too).
 int restore_impl(phx_shard *s, const uint8_t *hdr_src, const uint8_t *copy_src, const uint8_t *kern_src,
-                 bool hdr_on_host, cudaStream_t st, uint64_t *restored_step, bool *valid_out)
+                 bool hdr_on_host, cudaStream_t st, uint64_t *restored_step, bool *valid_out, uint64_t stride,
+                 uint32_t want_payload)
 {
     int best = -1;
     bool any_valid = false;
     phx_snapshot_header_t hdr[2];
     for (int i = 0; i < 2; ++i) {
-        const uint8_t *hp = hdr_src + (uint64_t)i * s->info.slot_stride;
+        const uint8_t *hp = hdr_src + (uint64_t)i * stride;
         if (hdr_on_host) std::memcpy(&hdr[i], hp, sizeof(hdr[i]));
         else PHX_CK(cudaMemcpy(&hdr[i], hp, sizeof(hdr[i]), cudaMemcpyDefault));
         if (!header_valid(&hdr[i])) continue;
         any_valid = true;
-        if (!header_matches(s, &hdr[i])) continue;
+        if (!header_matches(s, &hdr[i]) || hdr[i].payload != want_payload) continue;
         if (best < 0 || hdr[i].step > hdr[best].step) best = i;
     }
     if (best < 0) return any_valid ? PHX_ERR_LAYOUT_MISMATCH : PHX_ERR_NO_COMMITTED_SNAPSHOT;
 
     const uint64_t N = s->info.n_padded;
-    const uint64_t off = (uint64_t)best * s->info.slot_stride + kHeaderBytes;
+    const uint64_t off = (uint64_t)best * stride + kHeaderBytes;
     if (s->cfg.restore_mode == PHX_RESTORE_BULK_KERNEL) {
         PHX_CK(phx::launch_restore_bulk(kern_src + off, s->d_p, s->d_m, s->d_v, fp32_mode(s) ? nullptr : s->d_p16, N,
                                         s->sm_count, st));
@@ -715,12 +769,16 @@ int restore_impl(phx_shard *s, const uint8_t *hdr_src, const uint8_t *copy_src, 
             s->launches += N ? 1 : 0;
         }
     }
+    if (want_payload != 0)  // §8(f4) in-place recovery: W comes back from the same slot, no other rank is read
+        PHX_CK(cudaMemcpyAsync(s->d_W, copy_src + off + 12 * N, s->info.param_bytes, cudaMemcpyDefault, st));
     s->last_step = hdr[best].step;
     s->pending_slot = -1;
     s->pending_peer_slot = -1;
+    s->params_ready = false;
     s->restored_user_len = hdr[best].user_len <= 128 ? hdr[best].user_len : 128;
     std::memcpy(s->restored_user, hdr[best].user, 128);
-    for (int i = 0; i < 2; ++i) valid_out[i] = header_valid(&hdr[i]) && header_matches(s, &hdr[i]);
+    for (int i = 0; i < 2; ++i)
+        valid_out[i] = header_valid(&hdr[i]) && header_matches(s, &hdr[i]) && hdr[i].payload == want_payload;
     if (restored_step) *restored_step = s->last_step;
     // the slots' steps, for the caller's own slot bookkeeping
     s->restore_hdr_step[0] = hdr[0].step;
@@ -739,7 +797,9 @@ int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
     int rc = settle_host_slots(s, true);
     if (rc != PHX_OK) return rc;
     bool ok[2] = {false, false};
-    rc = restore_impl(s, s->h_replica, s->h_replica, s->d_replica, true, static_cast<cudaStream_t>(stream), restored_step, ok);
+    if (full_payload(s) && !s->d_W) return PHX_ERR_NOT_BOUND;
+    rc = restore_impl(s, s->h_replica, s->h_replica, s->d_replica, true, static_cast<cudaStream_t>(stream), restored_step, ok,
+                      s->info.host_slot_stride, full_payload(s) ? full_payload_word(s) : 0u);
     if (rc != PHX_OK) return rc;
     for (int i = 0; i < 2; ++i) {
         s->host[i].state = ok[i] ? SLOT_COMMITTED : (s->host[i].state == SLOT_EMPTY ? SLOT_EMPTY : SLOT_TORN);
@@ -764,7 +824,7 @@ int phx_restore_from(phx_shard_t *s, const void *replica, void *stream, uint64_t
     const uint8_t *r = static_cast<const uint8_t *>(replica);
     bool ok[2];
     return restore_impl(s, r, r, static_cast<const uint8_t *>(at.devicePointer), false, static_cast<cudaStream_t>(stream),
-                        restored_step, ok);
+                        restored_step, ok, s->info.slot_stride, 0u);
 }
 
 int phx_restored_user_metadata(const phx_shard_t *s, void *blob, uint32_t cap, uint32_t *len)
@@ -961,6 +1021,38 @@ int phx_params_restore_from(phx_shard_t *s, const void *d_src_param_buf, void *d
     if (!s->bound) return PHX_ERR_NOT_BOUND;
     const uint64_t bytes = (uint64_t)s->info.dp_size * s->info.n_padded * model_elem_bytes(s);
     PHX_CK(cudaMemcpyAsync(d_dst_param_buf, d_src_param_buf, bytes, cudaMemcpyDefault, static_cast<cudaStream_t>(stream)));
+    return PHX_OK;
+}
+
+// ---- §8(f4): full rank-state local snapshot --------------------------------------------------------
+int phx_shard_bind_params(phx_shard_t *s, void *d_W)
+{
+    if (!s || !d_W) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!aligned256(d_W)) return PHX_ERR_ALIGNMENT;
+    // bf16 precision: the fused kernel keeps the rank's own range of W current through d_p_bf16
+    if (!fp32_mode(s) &&
+        static_cast<uint8_t *>(s->d_p16) != static_cast<uint8_t *>(d_W) + (uint64_t)s->info.dp_rank * s->info.n_padded * 2)
+        return PHX_ERR_INVALID_ARG;
+    s->d_W = static_cast<uint8_t *>(d_W);
+    return PHX_OK;
+}
+
+int phx_params_ready(phx_shard_t *s, void *stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound || !s->d_W) return PHX_ERR_NOT_BOUND;
+    PHX_CK(cudaEventRecord(s->ev_params, static_cast<cudaStream_t>(stream)));
+    s->params_ready = true;
+    s->params_ready_step = s->last_step;
+    return PHX_OK;
+}
+
+int phx_params_guard(phx_shard_t *s, void *stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound || !s->d_W) return PHX_ERR_NOT_BOUND;
+    if (s->wflush_valid) PHX_CK(cudaStreamWaitEvent(static_cast<cudaStream_t>(stream), s->ev_wflush, 0));
     return PHX_OK;
 }
 

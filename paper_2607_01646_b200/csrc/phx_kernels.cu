@@ -228,14 +228,30 @@ __device__ __forceinline__ bool nodecay_at(uint64_t e, const uint64_t *__restric
     return ((first ^ lo) & 1u) != 0;
 }
 
+// Block 0 stores the 256-byte envelope in front of the staging slot (and, §8(f4), a second copy whose
+// payload word and hash describe the full rank state) so that the packed snapshot is produced by ONE kernel.
+__device__ __forceinline__ void store_headers(const StepArgs &a)
+{
+    if (blockIdx.x != 0 || threadIdx.x >= 16) return;
+    uint4 q = a.hdr.q[threadIdx.x];
+    if (a.shdr != nullptr) reinterpret_cast<uint4 *>(a.shdr)[threadIdx.x] = q;
+    if (a.shdr_full != nullptr) {
+        if (threadIdx.x == 6) q.w = a.full_payload;                 // bytes 108..111
+        if (threadIdx.x == 15) {                                    // bytes 240..247
+            q.x = (uint32_t)a.full_hash;
+            q.y = (uint32_t)(a.full_hash >> 32);
+        }
+        reinterpret_cast<uint4 *>(a.shdr_full)[threadIdx.x] = q;
+    }
+}
+
 template <int HINT, int U, bool SNAP, int MODE>
 __global__ void __launch_bounds__(kStepThreads) k_step8(const __grid_constant__ StepArgs a)
 {
     constexpr bool GF32 = (MODE & kModeF32) != 0, GROUPS = (MODE & kModeGroups) != 0, PUB = (MODE & kModePublish) != 0;
     const uint64_t ngroups = a.n_padded >> 3;
     const uint64_t base = (uint64_t)blockIdx.x * (kStepThreads * U) + threadIdx.x;
-    if (a.shdr != nullptr && blockIdx.x == 0 && threadIdx.x < 16)
-        reinterpret_cast<uint4 *>(a.shdr)[threadIdx.x] = a.hdr.q[threadIdx.x];
+    store_headers(a);
     const float coef = __ldg(a.coef);
 
     F8 P[U], M[U], V[U];
@@ -313,8 +329,7 @@ __global__ void __launch_bounds__(kStepThreads) k_step4(const __grid_constant__ 
 {
     const uint64_t ngroups = a.n_padded >> 2;
     const uint64_t base = (uint64_t)blockIdx.x * (kStepThreads * U) + threadIdx.x;
-    if (a.shdr != nullptr && blockIdx.x == 0 && threadIdx.x < 16)
-        reinterpret_cast<uint4 *>(a.shdr)[threadIdx.x] = a.hdr.q[threadIdx.x];
+    store_headers(a);
     const float coef = __ldg(a.coef);
 
     F4 P[U], M[U], V[U];
@@ -408,8 +423,7 @@ __global__ void __launch_bounds__(kStepThreads) k_step_tma(const __grid_constant
     const uint64_t first = blockIdx.x, stride = gridDim.x;
     const uint64_t my_count = first < ntiles ? (ntiles - first + stride - 1) / stride : 0;
 
-    if (a.shdr != nullptr && blockIdx.x == 0 && threadIdx.x < 16)
-        reinterpret_cast<uint4 *>(a.shdr)[threadIdx.x] = a.hdr.q[threadIdx.x];
+    store_headers(a);
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");

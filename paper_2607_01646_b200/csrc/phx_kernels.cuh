@@ -25,6 +25,11 @@ struct StepArgs {
     void *p16;                   // bf16 param copy (unused under kModeF32)
     float *sp, *sm, *sv;         // staging planes of the slot being written (null if !snapshot)
     void *shdr;                  // where block 0 stores the 256-B header (null: no header)
+    // §8(f4): second copy of the header for the full-rank-state local slot — same bytes except the
+    // payload word (byte 108) and the header hash (byte 240); null: not written
+    void *shdr_full;
+    uint32_t full_payload;
+    uint64_t full_hash;
     const float *coef;           // device scalar: clip coefficient (1.0f when clipping is off)
     uint64_t n_padded;           // multiple of 64
     // decay groups (kModeGroups): class per 2048-element tile, toggle offsets, flag before the first toggle

@@ -18,7 +18,8 @@ class Shard:
     def __init__(self, wl: Workload, *, device="cuda:0", staging_depth=2, sync_mode=B.PHX_SYNC_STRICT,
                  chunk_bytes=0, snapshot=True, restore_mode=B.PHX_RESTORE_COPY_ENGINE,
                  max_grad_norm: Optional[float] = None, replica: Optional[torch.Tensor] = None,
-                 snapshot_source=B.PHX_SNAPSHOT_STAGED, p16: Optional[torch.Tensor] = None):
+                 snapshot_source=B.PHX_SNAPSHOT_STAGED, p16: Optional[torch.Tensor] = None,
+                 payload=B.PHX_PAYLOAD_OPTIMIZER, W: Optional[torch.Tensor] = None):
         self.wl = wl
         self.device = torch.device(device)
         self.hyper: Hyper = wl.hyper
@@ -28,7 +29,9 @@ class Shard:
             staging_depth=staging_depth, sync_mode=sync_mode, chunk_bytes=chunk_bytes,
             snapshot_disabled=not snapshot, restore_mode=restore_mode, max_grad_norm=mgn,
             snapshot_source=snapshot_source, flags=wl.flags(),
-            precision=B.PHX_PRECISION_FP32 if wl.precision == "fp32" else B.PHX_PRECISION_BF16_GRADS)
+            precision=B.PHX_PRECISION_FP32 if wl.precision == "fp32" else B.PHX_PRECISION_BF16_GRADS,
+            payload=payload)
+        self.full = payload == B.PHX_PAYLOAD_FULL_RANK_STATE
         self.fp32 = wl.precision == "fp32"
         self.info = B.phx_shard_info(self.h)
         self.n, self.n_padded = self.info.n, self.info.n_padded
@@ -40,6 +43,14 @@ class Shard:
             self.v = torch.zeros(N, dtype=torch.float32, device=self.device)
             # no bf16 model-param copy in the all-FP32 precision
             # (p16 may be handed in: the rank's range inside its model-parameter buffer W)
+            # §8(f4): W is the rank's model-parameter buffer (dp_size * N model-dtype elements); in the bf16
+            # precision the bf16 copy is the rank's own range inside it
+            self.W = W
+            if self.full and W is None:
+                self.W = torch.zeros(wl.dp_size * N, dtype=torch.float32 if self.fp32 else torch.bfloat16,
+                                     device=self.device)
+            if self.W is not None and not self.fp32 and p16 is None:
+                p16 = self.W[wl.dp_rank * N:(wl.dp_rank + 1) * N]
             if p16 is not None:
                 assert not self.fp32 and p16.dtype == torch.bfloat16 and p16.numel() == N and p16.is_contiguous()
                 self.p16 = p16
@@ -52,10 +63,12 @@ class Shard:
                     self.staging = torch.zeros(self.info.staging_depth * self.info.slot_stride,
                                                dtype=torch.uint8, device=self.device)
                 if replica is None:
-                    replica = torch.zeros(2 * self.info.slot_stride, dtype=torch.uint8).pin_memory()
-                assert replica.is_pinned() and replica.numel() >= 2 * self.info.slot_stride
+                    replica = torch.zeros(2 * self.info.host_slot_stride, dtype=torch.uint8).pin_memory()
+                assert replica.is_pinned() and replica.numel() >= 2 * self.info.host_slot_stride
                 self.replica = replica
             B.phx_shard_bind(self.h, self.p, self.m, self.v, self.p16, self.staging, self.replica)
+            if self.W is not None:
+                B.phx_shard_bind_params(self.h, self.W)
 
     # -- thin forwards -----------------------------------------------------------------
     def set_state(self, step: int = 0, stream=None):
@@ -83,12 +96,18 @@ class Shard:
 
     def replica_slot(self, step: int) -> torch.Tensor:
         k = step % 2
-        return self.replica[k * self.info.slot_stride: k * self.info.slot_stride + self.info.snapshot_bytes]
+        return self.replica[k * self.info.host_slot_stride: k * self.info.host_slot_stride + self.info.host_snapshot_bytes]
+
+    def params_ready(self, stream=None):
+        B.phx_params_ready(self.h, stream or torch.cuda.current_stream(self.device))
+
+    def params_guard(self, stream=None):
+        B.phx_params_guard(self.h, stream or torch.cuda.current_stream(self.device))
 
     def drop_live(self):
         """'Drop the live shard' (BASELINE.json:configs[3]): zero p, m, v, bf16 copy and scribble
         over the device staging ring — restore must not depend on anything device-resident."""
-        for t in (self.p, self.m, self.v, self.p16):
+        for t in (self.p, self.m, self.v, self.p16, self.W):
             if t is not None:
                 t.zero_()
         if self.staging is not None:

@@ -42,7 +42,8 @@ def test_library_exports_every_declared_symbol():
 def test_struct_sizes_match_the_header():
     assert C.sizeof(B.phx_tensor_desc_t) == 16
     assert C.sizeof(B.phx_config_t) == 64
-    assert C.sizeof(B.phx_shard_info_t) == 72
+    assert C.sizeof(B.phx_shard_info_t) == 96
+    assert C.sizeof(B.phx_snapshot_header_t) == 256
 
 
 @pytest.mark.parametrize("numels,dp", [([5], 1), ([100, 3, 64, 1], 3), ([63, 1, 64, 129], 2),
@@ -84,7 +85,8 @@ def test_argument_and_state_errors_without_a_gpu():
     assert e.value.code == B.PHX_ERR_INVALID_ARG
     for kw in (dict(dp_rank=2), dict(staging_depth=5), dict(tp=(2, 2)), dict(pp=(1, 1)), dict(sync_mode=2),
                dict(restore_mode=2), dict(max_grad_norm=float("nan")), dict(snapshot_source=2),
-               dict(snapshot_source=B.PHX_SNAPSHOT_DIRECT, sync_mode=B.PHX_SYNC_RELAXED)):
+               dict(snapshot_source=B.PHX_SNAPSHOT_DIRECT, sync_mode=B.PHX_SYNC_RELAXED),
+               dict(payload=2), dict(payload=B.PHX_PAYLOAD_FULL_RANK_STATE, snapshot_disabled=True)):
         args = dict(dp_size=2, dp_rank=0)
         args.update(kw)
         with pytest.raises(B.PhxError) as e:
@@ -118,3 +120,27 @@ def test_bind_without_a_gpu_fails_loudly():
     rc = B.lib().phx_shard_bind(h, 256, 256, 256, 256, 256, 256)
     assert rc in (B.PHX_ERR_CUDA, B.PHX_ERR_UNSUPPORTED_DEVICE)   # never a silent CPU path
     B.phx_shard_destroy(h)
+
+
+@pytest.mark.parametrize("precision,eb", [(B.PHX_PRECISION_BF16_GRADS, 2), (B.PHX_PRECISION_FP32, 4)])
+def test_full_rank_state_slot_sizes(precision, eb):
+    # the local slot = optimizer-only snapshot + the model-parameter buffer W (oracle/rank_state.py)
+    from oracle import rank_state as RS
+    layout, D = [(1000, 0), (333, 1), (77, 2)], 3
+    for r in range(D):
+        h = B.phx_shard_create(layout, D, r, precision=precision, payload=B.PHX_PAYLOAD_FULL_RANK_STATE)
+        h0 = B.phx_shard_create(layout, D, r, precision=precision)
+        i, i0 = B.phx_shard_info(h), B.phx_shard_info(h0)
+        fr = RS.FullRankState(O.OracleShard(layout, D, r, precision="fp32" if eb == 4 else "bf16"))
+        assert i.param_bytes == D * i.n_padded * eb == fr.w_bytes == i0.param_bytes
+        assert i.host_snapshot_bytes == fr.snapshot_bytes == i.snapshot_bytes + i.param_bytes
+        assert i.host_slot_stride % 256 == 0 and 0 <= i.host_slot_stride - i.host_snapshot_bytes < 256
+        assert (i0.host_snapshot_bytes, i0.host_slot_stride) == (i0.snapshot_bytes, i0.slot_stride)
+        assert (i.snapshot_bytes, i.slot_stride, i.layout_hash) == (i0.snapshot_bytes, i0.slot_stride, i0.layout_hash)
+        L = B.lib()
+        assert L.phx_shard_bind_params(h, 256) == B.PHX_ERR_NOT_BOUND
+        assert L.phx_params_ready(h, None) == B.PHX_ERR_NOT_BOUND
+        assert L.phx_params_guard(h, None) == B.PHX_ERR_NOT_BOUND
+        assert L.phx_shard_bind_params(h, None) == B.PHX_ERR_INVALID_ARG
+        B.phx_shard_destroy(h)
+        B.phx_shard_destroy(h0)
