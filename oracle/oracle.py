@@ -268,15 +268,20 @@ class OracleShard:
         self.last_step = int(step)
 
     # -- a1 + a3 ---------------------------------------------------------------
-    def step(self, g_bits: np.ndarray, lr, beta1, beta2, eps, wd, step, nthreads=1):
+    def step(self, g_bits: np.ndarray, lr, beta1, beta2, eps, wd, step, nthreads=1, coef=None):
         """One optimizer step; `step` is 1-based and must be last_step+1 (I4 step
-        atomicity; reading R3)."""
+        atomicity; reading R3).  `coef`: a clip coefficient decided outside
+        the shard (the DP-global norm of oracle/global_clip.py); None = the
+        shard-local rule of reading R7."""
         if int(step) != self.last_step + 1:
             raise OracleError("step order")
         g_bits = np.ascontiguousarray(g_bits, dtype=np.uint16 if self.precision == "bf16" else np.float32)
-        coef = np.float32(1.0)
-        if self.max_grad_norm > 0.0:
+        if coef is not None:
+            coef = np.float32(coef)
+        elif self.max_grad_norm > 0.0:
             coef = clip_coef(sumsq(g_bits), self.max_grad_norm)
+        else:
+            coef = np.float32(1.0)
         self.last_coef = coef
         if self.precision == "bf16" and self.no_decay is None:
             adamw_step(self.p, self.m, self.v, g_bits, self.p16, lr, beta1, beta2, eps, wd,
