@@ -83,6 +83,10 @@ def parse_args():
                          "all-FP32 setting (PAPER.md:270; SURVEY 8(f2)): fp32 grads, no bf16 copy, 16 B read + 24 B written")
     ap.add_argument("--decay-groups", action="store_true",
                     help="flag biases and norm weights no-decay (per-tensor AdamW parameter groups, SURVEY 8(f2))")
+    ap.add_argument("--clip-scope", default="local", choices=["local", "global"],
+                    help="configs with a clip (c3): local = the shard's own norm (a1 inside the step); global = "
+                         "SURVEY 8(e): per-rank sum of squares, all-gather of one double per rank (NCCL when "
+                         "--gpus > 1), coefficient from the D sums inside the step")
     ap.add_argument("--chunks", default="4,8,16,32,64,128,256", help="chunk sizes (MiB) of --mode sweep")
     ap.add_argument("--depths", default="1,2,3,4", help="staging depths of --mode sweep")
     ap.add_argument("--syncs", default="strict,relaxed", help="sync modes of --mode sweep")
@@ -348,6 +352,10 @@ class Rig:
         self.gemm_ms = None
         self.k_peers = 0
         self.peers_in_overlap = False
+        self.gclip = None
+        if getattr(args, "clip_scope", "local") == "global" and self.wl.hyper.max_grad_norm > 0:
+            from paper_2607_01646_b200.clip import GlobalClip
+            self.gclip = GlobalClip(self.s)     # default process group = the DP group of this bench
 
     # -- §8(f1): peer replication ----------------------------------------------------------------------
     def setup_peers(self, k, rank, world):
@@ -395,7 +403,10 @@ class Rig:
     # -- the hot path -------------------------------------------------------------------------------
     def do_step(self):
         self.step += 1
-        self.s.step_and_snapshot(self.grads[self.step & 1], self.step)
+        if self.gclip is not None:
+            self.gclip.step_and_snapshot(self.grads[self.step & 1], self.step, stream=self.cur)
+        else:
+            self.s.step_and_snapshot(self.grads[self.step & 1], self.step)
 
     def time_steps(self, K, Wm):
         """K back-to-back a1..a3 passes after Wm warm-ups; CUDA events on the launching stream."""
@@ -795,7 +806,11 @@ def run_headline(args):
                        "l2": "inputs larger than L2 (working set %.2f GB per step >> 126 MB)" % (BYTES_PER_ELEM * N / 1e9),
                        "timed_region": "K x phx_step_and_snapshot (a1 clip if configured, a2 sync-point wait, a3 fused "
                                        "AdamW+bf16 copy+packed snapshot); a4/a5 host flush is in e2e and overlap",
-                       "parallelism": f"dp{world} independent shards, no data-path collective"},
+                       "clip_scope": ("global: all-gather of one fp64 sum per rank (SURVEY 8(e))" if rig.gclip is not None
+                                      else ("local" if wl.hyper.max_grad_norm > 0 else "none")),
+                       "parallelism": (f"dp{world} shards, one 8-byte-per-rank all-gather per step (global clip)"
+                                       if rig.gclip is not None else
+                                       f"dp{world} independent shards, no data-path collective")},
             "elements_per_s": units / (ms_per_step * 1e-3),
             "exposed_ckpt_ms_per_iter": overlap["exposed_ms"] if overlap else None,
             "roofline": roofline, "host_link": host_link, "e2e": e2e, "overlap": overlap, "restore": restore,

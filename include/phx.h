@@ -352,6 +352,28 @@ PHX_API int phx_shard_bind_params(phx_shard_t *s, void *d_W);
 PHX_API int phx_params_ready(phx_shard_t *s, void *stream);
 PHX_API int phx_params_guard(phx_shard_t *s, void *stream);
 
+/* ---- the DP-global gradient-norm clip (the one scalar exchange of the path) -------
+ * "Global grad-norm clip 1.0" (BASELINE.json:configs[2]); "all-reduce of sum g^2 for
+ * the global clip".  With dp_size > 1 the norm that decides the clip is the norm of the WHOLE gradient:
+ *     S = sum over ranks r of S_r,  S_r = sum_i g_{r,i}^2,  c = fp32(min(1, max_grad_norm/(sqrt(S)+1e-6)))
+ * and every rank applies the same c (oracle/global_clip.py).  a1 is therefore split in two around the
+ * caller's exchange of D doubles (NCCL all-gather on the same stream; 8*D bytes):
+ *
+ *   phx_grad_sumsq_async(s, d_grads, d_out, stream)   S_r of this rank's gradient shard (same kernels, same
+ *        fixed two-stage fp64 tree as the local a1) written to the caller-owned device double *d_out
+ *        (8-byte aligned).  Needs a bound shard; does not touch the optimizer state or the step counter.
+ *   [caller: all-gather the D values into a device array ordered by dp_rank]
+ *   phx_set_clip_partials(s, d_partials, count)       ONE-SHOT: the next phx_step_and_snapshot skips its own
+ *        sum-of-squares pass and takes S = d_partials[0] + ... + d_partials[count-1] (fixed tree, so every
+ *        rank that was handed the same array gets the same bits; count in 1..1024; the array is read on the
+ *        step's stream, in stream order, and must stay valid until that kernel has run).  count = 1 with an
+ *        already all-reduced scalar is equally valid.  Requires cfg.max_grad_norm > 0, else
+ *        PHX_ERR_INVALID_ARG.  Cleared by the step that consumes it and by phx_restore* (the recompute of
+ *        the in-flight step supplies its partials again).  d_partials = NULL clears it.
+ * With count = 1 and d_partials = the rank's own S_r the coefficient is bit-identical to the local a1. */
+PHX_API int phx_grad_sumsq_async(phx_shard_t *s, const void *d_grads, double *d_out, void *stream);
+PHX_API int phx_set_clip_partials(phx_shard_t *s, const double *d_partials, uint32_t count);
+
 /* ---- introspection ---------------------------------------------------------------------- */
 PHX_API int phx_last_step(const phx_shard_t *s, uint64_t *step);
 /* Host-blocking: clip coefficient and sum of squares of the last step (1.0 / 0 if clip is off). */

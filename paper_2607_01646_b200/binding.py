@@ -111,6 +111,8 @@ PROTOTYPES = {
     "phx_restored_user_metadata": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(C.c_uint32)]),
     "phx_last_step": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_last_clip": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)]),
+    "phx_grad_sumsq_async": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "phx_set_clip_partials": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32]),
     "phx_kernel_launches": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_set_kernel_variant": (C.c_int, [C.c_void_p, C.c_uint32]),
     "phx_ring_peer": (C.c_int, [C.c_uint32, C.c_uint32, C.c_int32, C.POINTER(C.c_uint32)]),
@@ -277,6 +279,16 @@ def phx_last_clip(h: int) -> Tuple[float, float]:
     c, q = C.c_float(), C.c_double()
     _ck(lib().phx_last_clip(h, C.byref(c), C.byref(q)), "phx_last_clip", h)
     return c.value, q.value
+
+
+def phx_grad_sumsq_async(h: int, d_grads, d_out, stream=None) -> None:
+    """this rank's sum of squared gradients into a caller-owned device double."""
+    _ck(lib().phx_grad_sumsq_async(h, _ptr(d_grads), _ptr(d_out), _ptr(stream)), "phx_grad_sumsq_async", h)
+
+
+def phx_set_clip_partials(h: int, d_partials, count: int) -> None:
+    """one-shot per-rank sums (device doubles, rank order) the next step clips by."""
+    _ck(lib().phx_set_clip_partials(h, _ptr(d_partials) or None, count), "phx_set_clip_partials", h)
 
 
 def phx_kernel_launches(h: int) -> int:

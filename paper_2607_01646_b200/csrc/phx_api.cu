@@ -128,6 +128,8 @@ struct phx_shard {
     uint64_t launches = 0;
     uint32_t variant = 0;
     bool clip_valid = false;
+    const double *clip_partials = nullptr;  // §8(e) global clip: one-shot per-rank sums for the next step
+    uint32_t clip_count = 0;
 };
 
 #define PHX_CK(call)                                  \
@@ -580,7 +582,17 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
     // a1: optional clip by the shard-local gradient norm
     a.coef = reinterpret_cast<const float *>(s->d_scratch + kScrOne);
     s->clip_valid = false;
-    if (s->cfg.max_grad_norm > 0.0f) {
+    if (s->cfg.max_grad_norm > 0.0f && s->clip_partials != nullptr) {
+        // §8(e): S = sum of the per-rank sums the caller exchanged; this rank's own pass already ran
+        PHX_CK(phx::launch_clip_from_partials(s->clip_partials, s->clip_count, s->cfg.max_grad_norm,
+                                              reinterpret_cast<double *>(s->d_scratch + kScrSumsq),
+                                              reinterpret_cast<float *>(s->d_scratch + kScrCoef), st));
+        s->launches += 1;
+        a.coef = reinterpret_cast<const float *>(s->d_scratch + kScrCoef);
+        s->clip_valid = true;
+        s->clip_partials = nullptr;
+        s->clip_count = 0;
+    } else if (s->cfg.max_grad_norm > 0.0f) {
         int nl = 0;
         PHX_CK(phx::launch_sumsq_clip(d_grads, fp32_mode(s), s->info.n_padded, s->cfg.max_grad_norm,
                                       reinterpret_cast<double *>(s->d_scratch + kScrPartials),
@@ -775,6 +787,8 @@ int restore_impl(phx_shard *s, const uint8_t *hdr_src, const uint8_t *copy_src, 
     s->pending_slot = -1;
     s->pending_peer_slot = -1;
     s->params_ready = false;
+    s->clip_partials = nullptr;  // the recompute of the in-flight step exchanges its sums again
+    s->clip_count = 0;
     s->restored_user_len = hdr[best].user_len <= 128 ? hdr[best].user_len : 128;
     std::memcpy(s->restored_user, hdr[best].user, 128);
     for (int i = 0; i < 2; ++i)
@@ -1061,6 +1075,35 @@ int phx_last_step(const phx_shard_t *s, uint64_t *step)
 {
     if (!s || !step) return PHX_ERR_INVALID_ARG;
     *step = s->last_step;
+    return PHX_OK;
+}
+
+// ---- §8(e): global clip, a1 split around the caller's exchange ------------------------------------
+int phx_grad_sumsq_async(phx_shard_t *s, const void *d_grads, double *d_out, void *stream)
+{
+    if (!s || !d_grads || !d_out) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!aligned256(d_grads) || (reinterpret_cast<uintptr_t>(d_out) & 7u)) return PHX_ERR_ALIGNMENT;
+    int nl = 0;
+    PHX_CK(phx::launch_sumsq(d_grads, fp32_mode(s), s->info.n_padded,
+                             reinterpret_cast<double *>(s->d_scratch + kScrPartials), d_out,
+                             static_cast<cudaStream_t>(stream), &nl));
+    s->launches += nl;
+    return PHX_OK;
+}
+
+int phx_set_clip_partials(phx_shard_t *s, const double *d_partials, uint32_t count)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (d_partials == nullptr) {
+        s->clip_partials = nullptr;
+        s->clip_count = 0;
+        return PHX_OK;
+    }
+    if (!(s->cfg.max_grad_norm > 0.0f) || count < 1 || count > (uint32_t)phx::kSumsqMaxBlocks) return PHX_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(d_partials) & 7u) return PHX_ERR_ALIGNMENT;
+    s->clip_partials = d_partials;
+    s->clip_count = count;
     return PHX_OK;
 }
 

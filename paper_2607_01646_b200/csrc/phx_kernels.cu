@@ -670,7 +670,7 @@ __global__ void __launch_bounds__(kSumsqMaxBlocks) k_sumsq_final(const double *_
         double c = (double)max_norm / (sqrt(S) + 1e-6);  // IEEE double sqrt and divide
         if (c > 1.0) c = 1.0;
         *out_sumsq = S;
-        *out_coef = (float)c;  // cvt.rn.f32.f64
+        if (out_coef != nullptr) *out_coef = (float)c;  // cvt.rn.f32.f64
     }
 }
 
@@ -685,6 +685,22 @@ cudaError_t launch_sumsq_clip(const void *g, bool grads_f32, uint64_t n_padded, 
     else k_sumsq_partial<<<nblocks, 256, 0, st>>>(reinterpret_cast<const uint4 *>(g), ngroups, partials);
     k_sumsq_final<<<1, kSumsqMaxBlocks, 0, st>>>(partials, nblocks, max_norm, out_sumsq, out_coef);
     if (n_launches) *n_launches = 2;
+    return cudaGetLastError();
+}
+
+// §8(e) global clip, first half: S_r of this rank's gradient shard -> *out_sumsq (no coefficient)
+cudaError_t launch_sumsq(const void *g, bool grads_f32, uint64_t n_padded, double *partials, double *out_sumsq,
+                         cudaStream_t st, int *n_launches)
+{
+    return launch_sumsq_clip(g, grads_f32, n_padded, 0.0f, partials, out_sumsq, nullptr, st, n_launches);
+}
+
+// §8(e) global clip, second half: S = sum of `count` per-rank values (same fixed tree) -> coefficient
+cudaError_t launch_clip_from_partials(const double *partials, uint32_t count, float max_norm, double *out_sumsq,
+                                      float *out_coef, cudaStream_t st)
+{
+    if (count < 1 || count > (uint32_t)kSumsqMaxBlocks) return cudaErrorInvalidValue;
+    k_sumsq_final<<<1, kSumsqMaxBlocks, 0, st>>>(partials, (int)count, max_norm, out_sumsq, out_coef);
     return cudaGetLastError();
 }
 

@@ -59,6 +59,12 @@ enum { kSumsqMaxBlocks = 1024 };
 cudaError_t launch_sumsq_clip(const void *g, bool grads_f32, uint64_t n_padded, float max_norm, double *partials,
                               double *out_sumsq, float *out_coef, cudaStream_t st, int *n_launches);
 
+// §8(e) global clip: a1 split around the caller's exchange of per-rank sums (include/phx.h).
+cudaError_t launch_sumsq(const void *g, bool grads_f32, uint64_t n_padded, double *partials, double *out_sumsq,
+                         cudaStream_t st, int *n_launches);
+cudaError_t launch_clip_from_partials(const double *partials, uint32_t count, float max_norm, double *out_sumsq,
+                                      float *out_coef, cudaStream_t st);
+
 // p16 = RNE_bf16(p)
 cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cudaStream_t st);
 
