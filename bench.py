@@ -59,6 +59,7 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-overlap", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-mix-ceiling", action="store_true", help="skip the no-arithmetic HBM mix-ceiling probe")
     ap.add_argument("--cpu-sample", type=int, default=0, help="elements of the shard the oracle is timed on (0 = auto)")
     ap.add_argument("--mode", default="headline",
                     choices=["headline", "configs", "overlap-curve", "sweep", "hotswap"],
@@ -637,6 +638,30 @@ def measure_host_link(torch, device, nbytes=1 << 30, reps=5):
     return out
 
 
+def measure_hbm_mix_ceiling(torch, B, device, plane_elems, reps=20):
+    """No-arithmetic streaming passes with the fused kernel's access pattern (phx_hbm_probe_async): the HBM
+    ceiling for a read:write mix.  Returns GB/s per mix; planes of `plane_elems` fp32 each (larger than L2)."""
+    mixes = {"read_only_4r": (4, 0), "write_only_4w": (0, 4), "copy_1r1w": (1, 1), "step_mix_3r6w": (3, 6),
+             "off_mix_3r3w": (3, 3)}
+    plane_bytes = int(plane_elems) * 4
+    buf = torch.empty(9 * plane_bytes, dtype=torch.uint8, device=device)
+    buf.zero_()
+    st = torch.cuda.current_stream(device)
+    out = {}
+    for name, (r, w) in mixes.items():
+        for _ in range(3):
+            B.phx_hbm_probe_async(buf, plane_bytes, r, w, st)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        for _ in range(reps):
+            B.phx_hbm_probe_async(buf, plane_bytes, r, w, st)
+        e1.record(st)
+        torch.cuda.synchronize()
+        out[name] = (r + w) * plane_bytes / (e0.elapsed_time(e1) / reps * 1e-3) / 1e9
+    del buf
+    return out
+
+
 def gpu_setup():
     import torch
     rank, world, local_rank = rank_env()
@@ -681,6 +706,11 @@ def run_headline(args):
                 "kernel_ms": kern_ms, "algorithmic_bytes_per_launch": BPE * N, "bytes_per_element": BPE,
                 "snapshot_off_step_ms": off_ms,
                 "snapshot_off_gbs": BYTES_PER_ELEM_OFF * N / (off_ms * 1e-3) / 1e9}
+    if rank == 0 and not args.no_mix_ceiling:
+        # context, not the denominator: what a kernel with NO arithmetic reaches with this read:write mix
+        ceil = measure_hbm_mix_ceiling(torch, rig.B, device, N)
+        roofline["mix_ceiling_gbs"] = ceil
+        roofline["frac_of_mix_ceiling"] = achieved / ceil["off_mix_3r3w" if rig.source_name == "direct" else "step_mix_3r6w"]
 
     # ---- e2e -----------------------------------------------------------------------------------------
     e2e_ms = max_over_ranks(rig.e2e(args.e2e_steps, world), world, device)

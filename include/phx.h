@@ -383,6 +383,12 @@ PHX_API int phx_kernel_launches(const phx_shard_t *s, uint64_t *count);
 /* Selects a kernel variant of the fused step (0 = default); for tuning/benchmarks only.  Shards with
  * PHX_PRECISION_FP32 or decay groups accept variant 0 only. */
 PHX_API int phx_set_kernel_variant(phx_shard_t *s, uint32_t variant);
+/* Diagnostic for bench.py's roofline context (no handle, no state): enqueue ONE streaming pass over
+ * n_read planes that are read and n_write planes that are written (plane i at d_buf + i*plane_bytes,
+ * reads first; d_buf: device memory of (n_read+n_write)*plane_bytes bytes, 256-byte aligned; plane_bytes
+ * a multiple of 256; each count <= 8) with the fused step's access pattern and no arithmetic — the HBM
+ * ceiling for that read:write mix.  The written planes are overwritten with junk. */
+PHX_API int phx_hbm_probe_async(void *d_buf, uint64_t plane_bytes, uint32_t n_read, uint32_t n_write, void *stream);
 PHX_API const char *phx_strerror(int err);
 PHX_API int phx_last_cuda_error(const phx_shard_t *s);
 PHX_API uint32_t phx_version(void);

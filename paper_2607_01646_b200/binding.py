@@ -111,6 +111,7 @@ PROTOTYPES = {
     "phx_restored_user_metadata": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(C.c_uint32)]),
     "phx_last_step": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_last_clip": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)]),
+    "phx_hbm_probe_async": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]),
     "phx_grad_sumsq_async": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "phx_set_clip_partials": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32]),
     "phx_kernel_launches": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
@@ -289,6 +290,11 @@ def phx_grad_sumsq_async(h: int, d_grads, d_out, stream=None) -> None:
 def phx_set_clip_partials(h: int, d_partials, count: int) -> None:
     """one-shot per-rank sums (device doubles, rank order) the next step clips by."""
     _ck(lib().phx_set_clip_partials(h, _ptr(d_partials) or None, count), "phx_set_clip_partials", h)
+
+
+def phx_hbm_probe_async(d_buf, plane_bytes: int, n_read: int, n_write: int, stream=None) -> None:
+    """Diagnostic: one no-arithmetic streaming pass (n_read planes read, n_write written)."""
+    _ck(lib().phx_hbm_probe_async(_ptr(d_buf), plane_bytes, n_read, n_write, _ptr(stream)), "phx_hbm_probe_async")
 
 
 def phx_kernel_launches(h: int) -> int:

@@ -1123,6 +1123,20 @@ int phx_last_clip(phx_shard_t *s, float *coef, double *sumsq)
     return PHX_OK;
 }
 
+int phx_hbm_probe_async(void *d_buf, uint64_t plane_bytes, uint32_t n_read, uint32_t n_write, void *stream)
+{
+    if (!d_buf || plane_bytes == 0 || (plane_bytes & 255u) || n_read > (uint32_t)phx::kProbeMaxPlanes ||
+        n_write > (uint32_t)phx::kProbeMaxPlanes || n_read + n_write == 0)
+        return PHX_ERR_INVALID_ARG;
+    if (!aligned256(d_buf)) return PHX_ERR_ALIGNMENT;
+    cudaError_t e = phx::launch_hbm_probe(d_buf, plane_bytes, n_read, n_write, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        return PHX_ERR_CUDA;
+    }
+    return PHX_OK;
+}
+
 int phx_kernel_launches(const phx_shard_t *s, uint64_t *count)
 {
     if (!s || !count) return PHX_ERR_INVALID_ARG;

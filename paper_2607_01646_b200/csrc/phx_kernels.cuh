@@ -73,4 +73,8 @@ cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cuda
 cudaError_t launch_restore_bulk(const void *src_payload, float *p, float *m, float *v, void *p16,
                                 uint64_t n_padded, int sm_count, cudaStream_t st);
 
+// Diagnostic: streaming pass over n_read + n_write planes of plane_bytes each inside d_buf, no arithmetic.
+enum { kProbeMaxPlanes = 8 };
+cudaError_t launch_hbm_probe(void *d_buf, uint64_t plane_bytes, uint32_t n_read, uint32_t n_write, cudaStream_t st);
+
 }  // namespace phx
