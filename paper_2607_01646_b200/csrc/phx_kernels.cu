@@ -567,39 +567,74 @@ cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, uint
 // ------------------------------------------------------------------------------------------
 // a1: sum of squares (fp64, fixed two-stage tree => deterministic run to run) + clip coefficient
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ double sq_acc(double acc, uint32_t w)
+// Widening a bf16 to binary64.  The plain way (widen to fp32, cvt.f64.f32) runs on the XU pipe, 16 lanes per
+// clock and SM, while the kernel needs ~13 elements per clock and SM to keep HBM busy: with every element
+// converted there, ncu shows XU 75 % busy and DRAM only 77 % (profiles/r01_aux_kernels.md).  So the two
+// halves of each 32-bit word take different pipes:
+//   low half : cvt.f64.f32 (XU);
+//   high half: integer re-bias — for a normal bf16 (exponent field e8 != 0, mantissa m7) the double is
+//              (e8 + 896) << 52 | m7 << 45, i.e. high word ((w >> 3) & 0x0FFFE000) + 0x38000000, low word 0
+//              (sign dropped: only squares are taken); zeros, subnormals, Inf and NaN (e8 = 0 or 255) fall
+//              back to the conversion so that they keep their IEEE meaning.
+// x*x is exact in binary64 (16 significant bits), so fma(x, x, acc) is ONE rounding of acc + g^2.
+// non-zero iff the high half of w has exponent field 0 or 255: (field + 1) mod 256 < 2
+__device__ __forceinline__ uint32_t hi_special(uint32_t w)
 {
-    const float lo = bf16lo(w), hi = bf16hi(w);
-    acc += (double)__fmul_rn(lo, lo);  // the square of a bf16 value is exact in fp32
-    acc += (double)__fmul_rn(hi, hi);
-    return acc;
+    return (((w & 0x7F800000u) + 0x00800000u) & 0x7F000000u) == 0u;
 }
-
-__global__ void __launch_bounds__(256) k_sumsq_partial(const uint4 *__restrict__ g, uint64_t ngroups,
-                                                       double *__restrict__ partials)
+__device__ __forceinline__ double widen_hi_int(uint32_t w)
 {
-    double acc = 0.0;
-    const uint64_t stride = (uint64_t)gridDim.x * 256;
-    uint64_t gi = (uint64_t)blockIdx.x * 256 + threadIdx.x;
-    for (; gi + 3 * stride < ngroups; gi += 4 * stride) {
-        uint4 w[4];
+    return __hiloint2double((int)(((w >> 3) & 0x0FFFE000u) + 0x38000000u), 0);
+}
+__device__ __forceinline__ void sq_acc4(double &a0, double &a1, const uint4 &w)
+{
+    const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
 #pragma unroll
-        for (int k = 0; k < 4; ++k) w[k] = ldg128_stream(g + gi + k * stride);
+    for (int k = 0; k < 4; ++k) {
+        const double lo = (double)bf16lo(ww[k]);
+        a0 = fma(lo, lo, a0);
+    }
+    // one branch per 8-element group keeps the conversions of the fallback off the XU pipe in the common case
+    if ((hi_special(w.x) | hi_special(w.y) | hi_special(w.z) | hi_special(w.w)) == 0u) {
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-            acc = sq_acc(acc, w[k].x);
-            acc = sq_acc(acc, w[k].y);
-            acc = sq_acc(acc, w[k].z);
-            acc = sq_acc(acc, w[k].w);
+            const double hi = widen_hi_int(ww[k]);
+            a1 = fma(hi, hi, a1);
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            float f = bf16hi(ww[k]);
+            double hi;
+            asm volatile("cvt.f64.f32 %0, %1;" : "=d"(hi) : "f"(f));  // volatile: not hoisted out of the branch
+            a1 = fma(hi, hi, a1);
         }
     }
-    for (; gi < ngroups; gi += stride) {
-        const uint4 w = ldg128_stream(g + gi);
-        acc = sq_acc(acc, w.x);
-        acc = sq_acc(acc, w.y);
-        acc = sq_acc(acc, w.z);
-        acc = sq_acc(acc, w.w);
+}
+
+// 256-bit loads (LDG.E.256, 16 gradients each), four in flight per thread: 128 B per thread, 128 KB per SM.
+__global__ void __launch_bounds__(256) k_sumsq_partial(const float *__restrict__ g, uint64_t nunits,
+                                                       double *__restrict__ partials)
+{
+    double acc = 0.0, acc1 = 0.0;  // two chains: low halves, high halves (fixed association => deterministic)
+    const uint64_t stride = (uint64_t)gridDim.x * 256;
+    uint64_t gi = (uint64_t)blockIdx.x * 256 + threadIdx.x;
+    auto add = [&](const F8 &f) {
+        uint4 a, b;
+        a.x = __float_as_uint(f.x[0]); a.y = __float_as_uint(f.x[1]); a.z = __float_as_uint(f.x[2]); a.w = __float_as_uint(f.x[3]);
+        b.x = __float_as_uint(f.x[4]); b.y = __float_as_uint(f.x[5]); b.z = __float_as_uint(f.x[6]); b.w = __float_as_uint(f.x[7]);
+        sq_acc4(acc, acc1, a);
+        sq_acc4(acc, acc1, b);
+    };
+    for (; gi + 3 * stride < nunits; gi += 4 * stride) {
+        F8 w[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) w[k] = ldg256_stream(g + ((gi + k * stride) << 3));
+#pragma unroll
+        for (int k = 0; k < 4; ++k) add(w[k]);
     }
+    for (; gi < nunits; gi += stride) add(ldg256_stream(g + (gi << 3)));
+    acc += acc1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
     __shared__ double wsum[8];
@@ -679,10 +714,12 @@ cudaError_t launch_sumsq_clip(const void *g, bool grads_f32, uint64_t n_padded, 
 {
     const uint64_t ngroups = n_padded >> 3;
     uint64_t want = (ngroups + 255) / 256;
-    int nblocks = (int)(want < 592 ? want : 592);  // 148 SMs x 4; fixed by n alone
+    // 148 SMs x 4 resident CTAs; fixed by n alone, so the summation tree is the same run to run.  (444-1024
+    // blocks and 128- vs 256-bit loads time within 1 % of each other: 130 us for 0.84 GB at c3.)
+    int nblocks = (int)(want < 592 ? want : 592);
     if (nblocks < 1) nblocks = 1;
     if (grads_f32) k_sumsq_partial_f32<<<nblocks, 256, 0, st>>>(reinterpret_cast<const float *>(g), ngroups, partials);
-    else k_sumsq_partial<<<nblocks, 256, 0, st>>>(reinterpret_cast<const uint4 *>(g), ngroups, partials);
+    else k_sumsq_partial<<<nblocks, 256, 0, st>>>(reinterpret_cast<const float *>(g), n_padded >> 4, partials);
     k_sumsq_final<<<1, kSumsqMaxBlocks, 0, st>>>(partials, nblocks, max_norm, out_sumsq, out_coef);
     if (n_launches) *n_launches = 2;
     return cudaGetLastError();

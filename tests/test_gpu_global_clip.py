@@ -161,3 +161,48 @@ def test_argument_errors():
     assert L.phx_set_clip_partials(s.h, d.data_ptr() + 4, 1) == B.PHX_ERR_ALIGNMENT
     assert L.phx_set_clip_partials(s.h, d.data_ptr(), 4) == B.PHX_OK
     s.close()
+
+
+@pytest.mark.parametrize("n", [64, 4096, 300_032])
+def test_sum_of_squares_over_zeros_subnormals_and_extreme_exponents(n):
+    """The integer widening of k_sumsq_partial (exponent re-bias, no cvt) against the oracle's double squares on
+    bit patterns that exercise both of its paths: zeros of either sign, bf16 subnormals, the smallest and the
+    largest normal exponents (whose squares leave the binary32 range but not binary64)."""
+    rng = np.random.default_rng(n)
+    wl = W.tiny_workload([n], dp_size=1, hyper=W.Hyper(max_grad_norm=1.0))
+    s = Shard(wl, device=DEV)
+    out = torch.zeros(1, dtype=torch.float64, device=DEV)
+    cases = {
+        "normal": rng.integers(0x3000, 0x4000, n),                                     # ~1e-10 .. 2
+        "signed": rng.integers(0x3000, 0x4000, n) | (rng.integers(0, 2, n) << 15),
+        "with zeros": np.where(rng.random(n) < 0.3, 0, rng.integers(0x3000, 0x4000, n)),
+        "neg zeros": np.where(rng.random(n) < 0.1, 0x8000, rng.integers(0x3A00, 0x3B00, n)),
+        "subnormals": np.where(rng.random(n) < 0.05, rng.integers(1, 0x80, n), rng.integers(0x0080, 0x0200, n)),
+        "tiny normals": rng.integers(0x0080, 0x0400, n),                                # squares < 2^-240
+        "huge": rng.integers(0x7E00, 0x7F80, n),                                        # squares up to 2^255
+        "all zero": np.zeros(n, np.int64),
+        "one element": np.where(np.arange(n) == n - 7, 0x3F80, 0),
+    }
+    for name, bits in cases.items():
+        b = np.ascontiguousarray(bits.astype(np.uint16))
+        b[s.n:] = 0
+        g = torch.from_numpy(b.view(np.int16)).view(torch.bfloat16).to(DEV)
+        B.phx_grad_sumsq_async(s.h, g, out, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        want = O.sumsq(b)
+        got = float(out.item())
+        assert np.isfinite(want)
+        assert abs(got - want) <= 16 * np.spacing(want), (name, got, want)
+    # non-finite gradients keep their IEEE meaning (outside the parity domain, DESIGN.md reading R8)
+    b = np.full(n, 0x3C00, np.uint16)
+    b[3] = 0x7F80
+    g = torch.from_numpy(b.view(np.int16)).view(torch.bfloat16).to(DEV)
+    B.phx_grad_sumsq_async(s.h, g, out, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    assert np.isinf(out.item())
+    b[3] = 0x7FC0
+    g = torch.from_numpy(b.view(np.int16)).view(torch.bfloat16).to(DEV)
+    B.phx_grad_sumsq_async(s.h, g, out, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    assert np.isnan(out.item())
+    s.close()
