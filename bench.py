@@ -84,6 +84,10 @@ def parse_args():
                          "all-FP32 setting (PAPER.md:270; SURVEY 8(f2)): fp32 grads, no bf16 copy, 16 B read + 24 B written")
     ap.add_argument("--decay-groups", action="store_true",
                     help="flag biases and norm weights no-decay (per-tensor AdamW parameter groups, SURVEY 8(f2))")
+    ap.add_argument("--payload", default="optimizer", choices=["optimizer", "full"],
+                    help="what the local host slots hold: optimizer = p,m,v + envelope (the H2H payload, default); "
+                         "full = SURVEY 8(f4), the paper's D2H payload (PAPER.md:145): p,m,v + the rank's whole "
+                         "model-parameter buffer W + envelope, for in-place recovery")
     ap.add_argument("--clip-scope", default="local", choices=["local", "global"],
                     help="configs with a clip (c3): local = the shard's own norm (a1 inside the step); global = "
                          "SURVEY 8(e): per-rank sum of squares, all-gather of one double per rank (NCCL when "
@@ -330,9 +334,11 @@ class Rig:
         if restore_mode is None:
             restore_mode = B.PHX_RESTORE_COPY_ENGINE if args.restore_mode == "copy" else B.PHX_RESTORE_BULK_KERNEL
         self.restore_mode_name = "copy_engine" if restore_mode == B.PHX_RESTORE_COPY_ENGINE else "bulk_kernel"
+        self.full = getattr(args, "payload", "optimizer") == "full"
         self.s = Shard(self.wl, device=self.device, staging_depth=self.depth, sync_mode=sync_mode,
                        chunk_bytes=self.chunk_mib << 20, replica=replica, restore_mode=restore_mode,
-                       snapshot_source=self.source)
+                       snapshot_source=self.source,
+                       payload=B.PHX_PAYLOAD_FULL_RANK_STATE if self.full else B.PHX_PAYLOAD_OPTIMIZER)
         B.phx_set_kernel_variant(self.s.h, args.variant)
         self.N = self.s.n_padded
         self.s.p.copy_(W.init_params(self.s.n, self.N, self.wl.seed, device=self.device))
@@ -477,6 +483,13 @@ class Rig:
         torch.cuda.synchronize()
         return e0.elapsed_time(e1) / K
 
+    def flush(self):
+        """a4+a5 of the newest snapshot on the side stream.  Full rank state (8(f4)): the caller first declares, in
+        compute-stream order, that W holds every rank's parameters of this step (here only the own range changes)."""
+        if self.full:
+            self.s.params_ready(self.cur)
+        self.s.flush_async(self.side)
+
     def time_flush(self):
         """One a4+a5 flush alone, timed on the side stream."""
         torch = self.torch
@@ -484,7 +497,7 @@ class Rig:
         torch.cuda.synchronize()
         f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         f0.record(self.side)
-        self.s.flush_async(self.side)
+        self.flush()
         f1.record(self.side)
         self.s.wait(self.step)
         torch.cuda.synchronize()
@@ -500,7 +513,7 @@ class Rig:
                 g = self.grads[self.step & 1]
                 g.copy_(self.hgrads[self.step & 1], non_blocking=True)   # H2D of this step's inputs
                 self.s.step_and_snapshot(g, self.step)
-                self.s.flush_async(self.side)                            # D2H of this step's result (a4 + a5)
+                self.flush()                                             # D2H of this step's result (a4 + a5)
             self.s.wait(self.step)
         loop(2)
         torch.cuda.synchronize()
@@ -582,7 +595,7 @@ class Rig:
                         self.do_step()
                     k1.record(self.cur)
                     if arm == "on":
-                        self.s.flush_async(self.side)
+                        self.flush()
                         if getattr(self, "k_peers", 0) and self.peers_in_overlap:
                             self.B.phx_snapshot_flush_peers_async(self.s.h, self.peer_stream)
                     evs.append(e0)
@@ -714,7 +727,7 @@ def run_headline(args):
 
     # ---- e2e -----------------------------------------------------------------------------------------
     e2e_ms = max_over_ranks(rig.e2e(args.e2e_steps, world), world, device)
-    d2h_bytes = int(rig.s.info.snapshot_bytes)
+    d2h_bytes = int(rig.s.info.host_snapshot_bytes)          # = snapshot_bytes unless --payload full
     e2e = {"value": BPE * units / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
            "h2d_bytes_per_step": int(rig.grad_bytes * N), "d2h_bytes_per_step": d2h_bytes, "ms_per_step": e2e_ms,
            "steps": args.e2e_steps,
@@ -795,8 +808,8 @@ def run_headline(args):
         # restore + recompute (a6, a7)
         back, rms, cms = rig.restore_timing()
         restore = {"restore_ms": rms, "recompute_ms": cms, "mode": rig.restore_mode_name, "restored_step": back,
-                   "host_link_gbs": 12 * N / (rms * 1e-3) / 1e9,
-                   "frac_of_h2d_peak": 12 * N / (rms * 1e-3) / 1e9 / link["h2d_gbs"]}
+                   "host_link_gbs": (d2h_bytes - 256) / (rms * 1e-3) / 1e9,
+                   "frac_of_h2d_peak": (d2h_bytes - 256) / (rms * 1e-3) / 1e9 / link["h2d_gbs"]}
         # restore from the ring successor's received buffer (recovery stage 3 over NVLink)
         if peer and "error" not in peer:
             src = rig.ring.opened[0] if world > 1 else rig.recv.ptrs[0]
@@ -836,6 +849,8 @@ def run_headline(args):
                        "l2": "inputs larger than L2 (working set %.2f GB per step >> 126 MB)" % (BYTES_PER_ELEM * N / 1e9),
                        "timed_region": "K x phx_step_and_snapshot (a1 clip if configured, a2 sync-point wait, a3 fused "
                                        "AdamW+bf16 copy+packed snapshot); a4/a5 host flush is in e2e and overlap",
+                       "host_payload": ("full rank state: envelope + p,m,v + model-parameter buffer W (SURVEY 8(f4))"
+                                        if rig.full else "optimizer shard: envelope + p,m,v"),
                        "clip_scope": ("global: all-gather of one fp64 sum per rank (SURVEY 8(e))" if rig.gclip is not None
                                       else ("local" if wl.hyper.max_grad_norm > 0 else "none")),
                        "parallelism": (f"dp{world} shards, one 8-byte-per-rank all-gather per step (global clip)"
