@@ -62,7 +62,7 @@ def parse_args():
     ap.add_argument("--no-mix-ceiling", action="store_true", help="skip the no-arithmetic HBM mix-ceiling probe")
     ap.add_argument("--cpu-sample", type=int, default=0, help="elements of the shard the oracle is timed on (0 = auto)")
     ap.add_argument("--mode", default="headline",
-                    choices=["headline", "configs", "overlap-curve", "sweep", "hotswap"],
+                    choices=["headline", "configs", "overlap-curve", "sweep", "hotswap", "timeline"],
                     help="headline: the ONE contract line (default).  The others print one JSON line per "
                          "measurement: configs = every config's kernel/flush/restore; overlap-curve = exposed ms vs G; "
                          "sweep = chunk x depth x sync-mode grid (BASELINE.json:configs[4]); hotswap = configs[3]")
@@ -945,6 +945,67 @@ def run_overlap_curve(args):
     return 0
 
 
+def run_timeline(args):
+    """Copy/compute overlap as a timeline from CUDA events (nsys is not on the image): per iteration, when the
+    GEMM window, the hot path (a1-a3) and the side-stream flush (a4+a5) of that iteration's snapshot start and end,
+    all in ms since the first iteration's start.  One JSON line per iteration plus a summary."""
+    torch, rank, world, local_rank = gpu_setup()
+    rig = Rig(args, args.config, host_grads=False)
+    flush_ms = rig.time_flush()
+    rig.gemm_setup()
+    a, b, c = rig._gemm
+    G = args.gemms if args.gemms > 0 else rig.headline_gemms(flush_ms)
+    iters, marks = 6, 8
+    E = lambda: torch.cuda.Event(enable_timing=True)
+    rows = []
+    for _ in range(2):                       # warm-up iterations (not recorded)
+        for _ in range(G):
+            torch.matmul(a, b, out=c)
+        rig.do_step()
+        rig.flush()
+    torch.cuda.synchronize()
+    base = E()
+    base.record(rig.cur)
+    for it in range(iters):
+        ev = {"gemm": [E()], "k0": E(), "k1": E(), "f0": E(), "f1": E()}
+        ev["gemm"][0].record(rig.cur)
+        for part in range(marks):
+            for _ in range(G // marks):
+                torch.matmul(a, b, out=c)
+            e = E()
+            e.record(rig.cur)
+            ev["gemm"].append(e)
+        ev["k0"].record(rig.cur)
+        rig.do_step()                         # a2: waits (stream-side) for the commit of the previous flush
+        ev["k1"].record(rig.cur)
+        ev["f0"].record(rig.side)             # side stream: flush of THIS step's snapshot, runs under the next window
+        rig.flush()
+        ev["f1"].record(rig.side)
+        rows.append(ev)
+    torch.cuda.synchronize()
+    rig.s.wait(rig.step)
+    t = lambda e: base.elapsed_time(e)
+    for it, ev in enumerate(rows):
+        # the flush is enqueued behind an event of the step kernel: its real start is max(f0, k1)
+        emit(mode="timeline", config=args.config, iteration=it, gemms=G,
+             gemm_window_ms=[t(ev["gemm"][0]), t(ev["gemm"][-1])],
+             gemm_marks_ms=[t(e) for e in ev["gemm"]],
+             hot_path_ms=[t(ev["k0"]), t(ev["k1"])],
+             flush_ms=[max(t(ev["f0"]), t(ev["k1"])), t(ev["f1"])])
+    # summary: how much of each flush lies under the NEXT iteration's GEMM window, and the wait at the sync point
+    under, waits = [], []
+    for it in range(iters - 1):
+        f0, f1 = max(t(rows[it]["f0"]), t(rows[it]["k1"])), t(rows[it]["f1"])
+        g0, g1 = t(rows[it + 1]["gemm"][0]), t(rows[it + 1]["gemm"][-1])
+        under.append(max(0.0, min(f1, g1) - max(f0, g0)) / (f1 - f0))
+        waits.append(max(0.0, f1 - t(rows[it + 1]["k0"])))
+    emit(mode="timeline-summary", config=args.config, gemms=G, flush_alone_ms=flush_ms,
+         flush_fraction_under_next_gemm_window=under, commit_after_next_step_enqueued_ms=waits,
+         note="commit_after_next_step_enqueued_ms > 0 would be a stall at the single sync point (PAPER.md:226)")
+    rig.close()
+    return 0
+
+
 def run_sweep(args):
     """BASELINE.json:configs[4]: D2H chunk size 4..256 MiB x staging depth 1..4 (x sync mode), reporting exposed
     checkpoint ms/iteration and host-link GB/s.  Run at a TIGHT compute window (T_c = 1.25 x T_D2H, where depth and
@@ -1062,7 +1123,7 @@ def main():
     if args.impl == "reference":
         return run_reference(args)
     return {"headline": run_headline, "configs": run_configs, "overlap-curve": run_overlap_curve,
-            "sweep": run_sweep, "hotswap": run_hotswap}[args.mode](args)
+            "sweep": run_sweep, "hotswap": run_hotswap, "timeline": run_timeline}[args.mode](args)
 
 
 if __name__ == "__main__":
