@@ -84,6 +84,10 @@ def parse_args():
                          "all-FP32 setting (PAPER.md:270; SURVEY 8(f2)): fp32 grads, no bf16 copy, 16 B read + 24 B written")
     ap.add_argument("--decay-groups", action="store_true",
                     help="flag biases and norm weights no-decay (per-tensor AdamW parameter groups, SURVEY 8(f2))")
+    ap.add_argument("--window", default="eager", choices=["eager", "graph"],
+                    help="how the stand-in GEMM window of the overlap runs is launched: eager torch.matmul calls "
+                         "(default) or replays of a CUDA graph of 64 GEMMs")
+    ap.add_argument("--no-graph-arm", action="store_true", help="skip the CUDA-graph repeat of the overlap run")
     ap.add_argument("--payload", default="optimizer", choices=["optimizer", "full"],
                     help="what the local host slots hold: optimizer = p,m,v + envelope (the H2H payload, default); "
                          "full = SURVEY 8(f4), the paper's D2H payload (PAPER.md:145): p,m,v + the rank's whole "
@@ -559,6 +563,33 @@ class Rig:
             self.gemm_ms = g0.elapsed_time(g1) / 200
         return self.gemm_ms
 
+    def gemm_window(self, G, mode=None):
+        """The stand-in compute window: G GEMMs, launched eagerly (default) or — `--window graph` — as replays of
+        one CUDA graph of 64 GEMMs (plus an eager remainder), the launch form a B200 training step would use."""
+        torch = self.torch
+        a, b, c = self._gemm
+        if (mode or getattr(self.args, "window", "eager")) != "graph":
+            for _ in range(G):
+                torch.matmul(a, b, out=c)
+            return
+        if getattr(self, "_graph", None) is None:
+            s = torch.cuda.Stream(device=self.device)
+            s.wait_stream(self.cur)
+            with torch.cuda.stream(s):
+                for _ in range(3):
+                    torch.matmul(a, b, out=c)
+            self.cur.wait_stream(s)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                for _ in range(64):
+                    torch.matmul(a, b, out=c)
+            self._graph = g
+        for _ in range(G // 64):
+            self._graph.replay()
+        for _ in range(G % 64):
+            torch.matmul(a, b, out=c)
+
     def headline_gemms(self, flush_ms, factor=4.0):
         """R21: smallest power of two G with T_c >= factor x T_D2H."""
         gm = self.gemm_setup()
@@ -567,7 +598,7 @@ class Rig:
             G *= 2
         return G
 
-    def overlap(self, G, iters, reps, arms=("off", "staged", "on"), warm=2):
+    def overlap(self, G, iters, reps, arms=("off", "staged", "on"), warm=2, window=None):
         """Iterations of G GEMMs + the hot path, three arms alternated `reps` times (ABCABC) to average
         out clock drift:
           off    — snapshot-disabled kernel, no flush (the paper's baseline run);
@@ -585,8 +616,7 @@ class Rig:
                 for it in range(warm + iters):
                     e0 = torch.cuda.Event(enable_timing=True)
                     e0.record(self.cur)
-                    for _ in range(G):
-                        torch.matmul(a, b, out=c)
+                    self.gemm_window(G, window)
                     k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                     k0.record(self.cur)
                     if arm == "off":
@@ -612,6 +642,7 @@ class Rig:
                 hp_ms[arm] += [x.elapsed_time(y) for x, y in kevs[warm:]]
         t = {k: trimmed_mean(v) for k, v in it_ms.items()}
         out = {"gemms_per_iter": G, "gemm_ms": self.gemm_ms, "compute_window_ms": G * self.gemm_ms,
+               "window_launch": window or getattr(self.args, "window", "eager"),
                "iters_per_arm": iters * reps, "reps": reps,
                "protocol": "PAPER.md:283: warm-up dropped, slowest 5% dropped, mean of the rest; arms alternated"}
         for k in arms:
@@ -803,6 +834,12 @@ def run_headline(args):
         if not args.no_overlap:
             G = args.gemms if args.gemms > 0 else rig.headline_gemms(flush_ms)
             overlap = rig.overlap(G, args.overlap_iters, args.overlap_reps)
+            if args.window == "eager" and not args.no_graph_arm:
+                # the same experiment with the GEMM window replayed from a CUDA graph: separates the part of the
+                # exposed time that is kernel-LAUNCH interference (PCIe busy with the D2H) from real contention
+                og = rig.overlap(G, args.overlap_iters, args.overlap_reps, arms=("off", "on"), window="graph")
+                overlap["graph_window"] = {k: og[k] for k in ("iter_ms_off", "iter_ms_on", "exposed_ms",
+                                                              "exposed_frac_of_compute_step", "window_launch")}
             overlap["flush_ms"] = flush_ms
             overlap["rule"] = "G = smallest power of two with T_c >= 4 x T_D2H" if args.gemms <= 0 else "G given"
         # restore + recompute (a6, a7)
