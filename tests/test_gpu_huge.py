@@ -1,0 +1,93 @@
+"""Maximum-size edge case: a shard with MORE THAN 2^32 elements (64-bit element indexing everywhere: the fused
+kernel, the staging planes, the sum of squares) — sampled element-by-element parity with the oracle around the
+2^31 and 2^32 boundaries and the ragged tail, plus whole-array properties.  ~122 GB of the 180 GB HBM; no host
+replica (2 x 52 GB of pinned memory is not a test-box assumption), so the snapshot is checked in the staging slot."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2607_01646_b200 import binding as B
+from paper_2607_01646_b200 import workloads as W
+
+from gpu_util import DEV, bits16
+
+pytestmark = pytest.mark.gpu
+
+N_HUGE = (1 << 32) + (1 << 20) + 64 * 37          # one tensor, dp_size 1, already a multiple of 64
+
+
+def _fill_normal(t, std, seed, chunk=1 << 28):
+    g = torch.Generator(device=DEV).manual_seed(seed)
+    for o in range(0, t.numel(), chunk):
+        v = t[o:o + chunk]
+        if t.dtype == torch.float32:
+            v.normal_(0.0, std, generator=g)
+        else:
+            v.copy_((torch.randn(v.numel(), generator=g, device=DEV, dtype=torch.float32) * std).to(t.dtype))
+
+
+def test_more_than_2_pow_32_elements_sampled_parity():
+    torch.cuda.empty_cache()
+    free, total = torch.cuda.mem_get_info()
+    need = N_HUGE * (12 + 12 + 2 + 2) + (2 << 30)
+    if free < need:
+        pytest.skip(f"needs {need >> 30} GiB of free HBM, {free >> 30} GiB free")
+    max_norm = 1.0
+    h = B.phx_shard_create([(N_HUGE, 0)], 1, 0, staging_depth=1, max_grad_norm=max_norm)
+    info = B.phx_shard_info(h)
+    N = info.n_padded
+    assert (info.n, N) == (N_HUGE, N_HUGE) and N > 1 << 32
+    p = torch.empty(N, dtype=torch.float32, device=DEV)
+    m = torch.zeros(N, dtype=torch.float32, device=DEV)
+    v = torch.zeros(N, dtype=torch.float32, device=DEV)
+    p16 = torch.empty(N, dtype=torch.bfloat16, device=DEV)
+    g = torch.empty(N, dtype=torch.bfloat16, device=DEV)
+    staging = torch.empty(info.slot_stride, dtype=torch.uint8, device=DEV)
+    _fill_normal(p, 0.02, 1)
+    B.phx_shard_bind(h, p, m, v, p16, staging, None)
+    B.phx_shard_set_state(h, 0, torch.cuda.current_stream())
+
+    w = 2048
+    centres = [w, 1 << 31, (1 << 32) - 64 * 5, 1 << 32, (1 << 32) + (1 << 19), N - w]
+    wins = [(max(0, c - w), min(N, c + w)) for c in centres]
+    idx = torch.cat([torch.arange(a, b, device=DEV) for a, b in wins])
+    ref = dict(p=p[idx].cpu().numpy().copy(), m=np.zeros(idx.numel(), np.float32),
+               v=np.zeros(idx.numel(), np.float32), h=np.zeros(idx.numel(), np.uint16))
+    hp = dict(lr=3e-4, beta1=0.9, beta2=0.95, eps=1e-8, wd=0.1)
+    for t in (1, 2):
+        _fill_normal(g, 1e-3, 100 + t)
+        B.phx_step_and_snapshot(h, g, hp["lr"], hp["beta1"], hp["beta2"], hp["eps"], hp["wd"], t,
+                                torch.cuda.current_stream())
+        coef, S = B.phx_last_clip(h)
+        # sum of squares over 4.3e9 elements against an independent chunked fp64 reduction
+        So = 0.0
+        for o in range(0, N, 1 << 28):
+            So += float(g[o:o + (1 << 28)].double().square().sum().item())
+        assert abs(S - So) <= 1e-12 * So
+        assert np.float32(coef) == O.clip_coef(S, max_norm) and coef < 0.05    # norm ~ 65
+        O.adamw_step(ref["p"], ref["m"], ref["v"], bits16(g[idx]).copy(), ref["h"], **hp, step=t, coef=float(coef),
+                     nthreads=2)
+        torch.cuda.synchronize()
+        assert np.array_equal(p[idx].cpu().numpy().view(np.uint32), ref["p"].view(np.uint32)), t
+        assert np.array_equal(m[idx].cpu().numpy().view(np.uint32), ref["m"].view(np.uint32)), t
+        assert np.array_equal(v[idx].cpu().numpy().view(np.uint32), ref["v"].view(np.uint32)), t
+        assert np.array_equal(bits16(p16[idx]), ref["h"]), t
+        # whole-array properties: staging planes == live planes, bf16 copy == RNE(p), header describes the shard
+        CH = 1 << 28
+        for o in range(0, N, CH):
+            e = min(N, o + CH)
+            assert torch.equal(staging[256 + 4 * o:256 + 4 * e].view(torch.float32), p[o:e])
+            assert torch.equal(staging[256 + 4 * N + 4 * o:256 + 4 * N + 4 * e].view(torch.float32), m[o:e])
+            assert torch.equal(staging[256 + 8 * N + 4 * o:256 + 8 * N + 4 * e].view(torch.float32), v[o:e])
+            assert torch.equal(p[o:e].to(torch.bfloat16), p16[o:e])
+        hdr = O.parse_header(staging[:256].cpu().numpy().tobytes())
+        assert hdr is not None and hdr["step"] == t and hdr["n"] == N_HUGE and hdr["n_padded"] == N
+    # every element moved (no range skipped by a 32-bit wrap): m is non-zero almost everywhere after two steps
+    zeros = 0
+    for o in range(0, N, 1 << 28):
+        zeros += int((m[o:o + (1 << 28)] == 0).sum().item())
+    assert zeros < N // 100          # bf16 gradients are exactly 0 only rarely
+    B.phx_shard_destroy(h)
+    del p, m, v, p16, g, staging
+    torch.cuda.empty_cache()
