@@ -362,6 +362,7 @@ PHX_API int phx_params_guard(phx_shard_t *s, void *stream);
  *   phx_grad_sumsq_async(s, d_grads, d_out, stream)   S_r of this rank's gradient shard (same kernels, same
  *        fixed two-stage fp64 tree as the local a1) written to the caller-owned device double *d_out
  *        (8-byte aligned).  Needs a bound shard; does not touch the optimizer state or the step counter.
+ *        It uses the handle's reduction scratch: enqueue it on the SAME stream as the step that follows.
  *   [caller: all-gather the D values into a device array ordered by dp_rank]
  *   phx_set_clip_partials(s, d_partials, count)       ONE-SHOT: the next phx_step_and_snapshot skips its own
  *        sum-of-squares pass and takes S = d_partials[0] + ... + d_partials[count-1] (fixed tree, so every
