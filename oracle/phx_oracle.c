@@ -213,3 +213,30 @@ double phx_oracle_sumsq_f32(const float *g, size_t n)
     }
     return (double)s;
 }
+
+/* ==== SURVEY.md §8(f4), second half: the gradient producer's epilogue ======================
+ *
+ * "single-pass fusion of the sum-of-squares with the previous step's epilogue" (SURVEY.md §8(f),
+ * row f4).  What precedes a1 in the ZeRO-2 distributed optimizer is the
+ * reduce-scatter of the binary32 main gradients ("main gradients ... torch.float32")
+ * and their averaging / cast to the optimizer's gradient dtype.  DESIGN.md reading R34:
+ *
+ *   h_i   = g32_i * scale          one binary32 multiply (scale = 1/(dp_size*microbatches); 1.0f is exact)
+ *   g16_i = RNE_bf16(h_i)          the same integer rounding as the last line of reading R1
+ *   S     = sum_i widen(g16_i)^2   of the ROUNDED values — it must equal what a1 (phx_oracle_sumsq)
+ *                                  computes from the bf16 gradients the optimizer then reads
+ *
+ * Plain statement: one loop, the rounding first, the square of the rounded value second, the
+ * running sum in long double rounded to double once (exactly as phx_oracle_sumsq). */
+double phx_oracle_grads_finalize(const float *g32, float scale, uint16_t *g_bf16, size_t n)
+{
+    long double s = 0.0L;
+    for (size_t i = 0; i < n; ++i) {
+        float h = g32[i] * scale;
+        uint16_t b = phx_oracle_rne_bf16(h);
+        g_bf16[i] = b;
+        double w = (double)widen_bf16(b);
+        s += (long double)(w * w);
+    }
+    return (double)s;
+}
