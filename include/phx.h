@@ -18,8 +18,11 @@
  *     them with any CUDA allocator, e.g. torch); the library never frees them and only owns
  *     small internals (events, a few hundred bytes of device scratch).
  *   - Streams are cudaStream_t passed as void*.  Calls that take a stream only ENQUEUE work;
- *     they never block the host on the device unless stated (phx_snapshot_wait, phx_restore's
- *     host-side slot validation).  Ordering between the compute stream and the flush stream
+ *     they never block the host on the device unless stated.  The three hot calls
+ *     (phx_step_and_snapshot, phx_snapshot_flush_async, phx_restore) never do.  Host-blocking by
+ *     contract: phx_snapshot_wait*, phx_restore_from / phx_replica_inspect (a blocking 512-byte read
+ *     of a FOREIGN replica's envelopes), phx_last_clip, phx_graph_begin / phx_graph_end (mode
+ *     switches), phx_shard_destroy.  Ordering between the compute stream and the flush stream
  *     is by library-owned events.  One host thread uses a handle at a time.
  *   - There is deliberately no fallback: a device that is not compute capability 10.x gives
  *     PHX_ERR_UNSUPPORTED_DEVICE at phx_shard_bind.
@@ -65,7 +68,8 @@ enum {
     PHX_ERR_UNSUPPORTED_DEVICE = -10, /* not compute capability 10.x; there is no fallback       */
     PHX_ERR_SNAPSHOT_DISABLED = -11,  /* flush/restore asked of a shard created with snapshots off */
     PHX_ERR_NOMEM = -12,
-    PHX_ERR_PARAMS_NOT_READY = -13    /* full-rank-state flush before phx_params_ready for that step  */
+    PHX_ERR_PARAMS_NOT_READY = -13,   /* full-rank-state flush before phx_params_ready for that step  */
+    PHX_ERR_GRAPH_MODE = -14          /* eager call between phx_graph_begin/end, or a phx_graph_* call outside them */
 };
 
 /* ---- types ----------------------------------------------------------------------------- */
@@ -207,6 +211,10 @@ PHX_API int phx_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len
  *      v' bits plus the header into staging slot `step mod depth` ("packed into a contiguous
  *      buffer") — the snapshot costs no extra read pass and no extra kernel.
  * `step` is the 1-based index of the update and must equal last_step + 1.
+ * Caller's contract (strict mode, "replay <= 1 step"): flush snapshot k (phx_snapshot_flush_async
+ * and/or phx_snapshot_flush_peers_async) BEFORE enqueuing step k+1 — the sync point can only wait for a flush
+ * that has been enqueued.  A step that finds its predecessor's snapshot never flushed goes ahead (that snapshot
+ * is superseded, replay grows by one step) and counts it: phx_dropped_snapshots.
  * d_grads: bf16[n_padded] (PHX_PRECISION_BF16_GRADS) or float[n_padded] (PHX_PRECISION_FP32: first line
  * g = g_f32 * c, no bf16 copy is written, the sum of squares uses exact fp64 squares of the fp32 values).
  * Elements of tensors flagged PHX_TENSOR_NO_DECAY use decay = 1.0f.
@@ -230,11 +238,16 @@ PHX_API int phx_snapshot_query(phx_shard_t *s, uint64_t *newest_committed_step, 
 PHX_API int phx_fault_inject_torn_flush(phx_shard_t *s, int64_t payload_chunks);
 
 /* ---- a6: restore ---------------------------------------------------------------------------
- * Waits (host side) for in-flight flushes, then chooses between the two host slots the valid
+ * ENQUEUE-ONLY: the host never waits for the device.  Chooses between the two host slots the valid
  * one (magic, version, header hash, seq_begin == seq_end) with the largest step, refuses it if
  * its logical identity (layout hash, dp/tp/pp coordinates, n) differs from this shard's, and
  * enqueues on `stream` the rebuild of the live shard: p, m, v from the slot and d_p_bf16 =
- * RNE_bf16(p).  PHX_RESTORE_COPY_ENGINE: three H2D copies straight into the live planes (the packed
+ * RNE_bf16(p).  The envelope that decides is the one IN the pinned slot (plain host read) for every slot
+ * this handle is not writing at that moment; for a slot whose flush by THIS handle is still in flight the
+ * handle's own record of the envelope it sent decides (a flush cannot tear unless told to, and a torn one is
+ * skipped), and `stream` waits for that flush's event before the copies.  `stream` also waits for whatever of
+ * this handle may still touch the live planes (the newest step's kernel, a direct-source flush, a
+ * publication), so a restore issued while step k+1's kernel and flush(k) are in flight is well ordered.  PHX_RESTORE_COPY_ENGINE: three H2D copies straight into the live planes (the packed
  * layout is planar, so no unpack pass is needed) plus a bf16 regeneration kernel;
  * PHX_RESTORE_BULK_KERNEL: one kernel pulls the replica straight from mapped host memory with 1-D
  * bulk async (TMA) loads into shared memory and writes all four arrays.  Both are bit-exact; the
@@ -281,8 +294,9 @@ PHX_API int phx_ipc_close(void *d_buf);
  * peer j keeps for this rank; k <= min(PHX_MAX_PEERS, dp_size - 1) distinct buffers; k = 0 unbinds.
  * h_replica of phx_shard_bind may be NULL when only peers are used. */
 PHX_API int phx_shard_bind_peers(phx_shard_t *s, void *const *d_peer_replicas, uint32_t k);
-/* Enqueues on `peer_stream` the replication of the newest snapshot to all k peers (one after the other: the
- * source GPU's NVLink egress is the shared limit).  Independent of phx_snapshot_flush_async: either or both
+/* Enqueues the replication of the newest snapshot to all k peers.  k = 1: on `peer_stream`.  k > 1: on k
+ * library-owned copy streams forked from and joined back into `peer_stream` (one copy engine / NVSwitch path
+ * per peer; `peer_stream` observes the completion of all of them).  Independent of phx_snapshot_flush_async: either or both
  * may be called after a step, on different streams, and overlap (PCIe and NVLink are separate links). */
 PHX_API int phx_snapshot_flush_peers_async(phx_shard_t *s, void *peer_stream);
 /* Host-blocking wait until the peer replication of `step` is committed on every peer. */
@@ -297,8 +311,9 @@ PHX_API int phx_replica_inspect(const void *replica, uint64_t slot_stride, phx_s
 /* a6 from a replica held elsewhere (recovery stage 3: "optimizer state is restored from
  * in-memory replicas"): `replica` is any device-accessible address of two snapshot slots — the surviving
  * holder's received buffer opened over IPC, a device buffer, or pinned mapped host memory.  Same slot
- * selection, identity check, restore modes and postconditions as phx_restore; reads the two headers with a
- * blocking copy. */
+ * selection, identity check, restore modes and postconditions as phx_restore.  The replica is foreign (this
+ * handle has no commit record of it), so the two envelopes are read with a BLOCKING 512-byte copy — the one
+ * documented exception to "restore only enqueues". */
 PHX_API int phx_restore_from(phx_shard_t *s, const void *replica, void *stream, uint64_t *restored_step);
 
 /* ---- model-parameter publication and reconstruction ---------------------------
@@ -341,7 +356,9 @@ PHX_API int phx_params_restore_from(phx_shard_t *s, const void *d_src_param_buf,
  * phx_params_guard(stream): `stream` waits until the newest flush has finished READING W — to be enqueued
  * ahead of whatever lets other ranks publish step k+1 into this rank's W (handing this rank's gradients to
  * the reduce-scatter of iteration k+1; a local copy-engine publication).  The rank's own step k+1 is
- * covered by the sync point of phx_step_and_snapshot as before.
+ * covered by phx_step_and_snapshot: the strict sync point waits for the whole flush, and under
+ * PHX_SYNC_RELAXED the step additionally waits until the newest flush has finished reading W (its own range
+ * of W is d_p_bf16, which the kernel rewrites).
  *
  * phx_restore on such a shard is the in-place recovery: p, m, v AND W come back from
  * the rank's own host slot (newest valid slot whose payload word and identity match), nothing is read from
@@ -375,21 +392,76 @@ PHX_API int phx_params_guard(phx_shard_t *s, void *stream);
 PHX_API int phx_grad_sumsq_async(phx_shard_t *s, const void *d_grads, double *d_out, void *stream);
 PHX_API int phx_set_clip_partials(phx_shard_t *s, const double *d_partials, uint32_t count);
 
+/* ---- SURVEY.md §8(f4), second half: the gradient producer's epilogue -------------------------------
+ * "single-pass fusion of the sum-of-squares with the previous step's epilogue".  The
+ * gradients of step k+1 do not exist while step k's kernel runs and the clip coefficient must be known before
+ * the first element of step k+1 moves, so the one place where the norm costs no pass of its own is the
+ * PRODUCER of the optimizer's gradients: the epilogue of the reduce-scatter of the binary32 main gradients
+ * (ZeRO-2 distributed optimizer; "main gradients ... torch.float32").  One kernel,
+ * one pass (4 B read + 2 B written per element; reading R34):
+ *     g16_i = RNE_bf16(g32_i * scale)      one binary32 multiply (scale: gradient averaging; 1.0f exact), then
+ *                                          the same rounding as the bf16 model-param copy
+ *     *d_sumsq_out = sum_i widen(g16_i)^2  fp64, fixed two-stage tree, of the ROUNDED values — the very number
+ *                                          a1 would compute from g16
+ * d_main_grads_fp32: float[n_padded] (pad lanes zero), d_grads_bf16_out: bf16[n_padded], both 256-byte
+ * aligned, not overlapping; d_sumsq_out: device double, 8-byte aligned.  Then
+ *     phx_set_clip_partials(s, d_sumsq_out, 1);  phx_step_and_snapshot(s, d_grads_bf16_out, ...)
+ * runs the step with NO sum-of-squares pass (40 instead of 42 B/element on the critical path).  Uses the
+ * handle's reduction scratch: same stream as the step.  PHX_PRECISION_BF16_GRADS only. */
+PHX_API int phx_grads_finalize_async(phx_shard_t *s, const float *d_main_grads_fp32, float scale,
+                                     void *d_grads_bf16_out, double *d_sumsq_out, void *stream);
+
+/* ---- the graph-capturable form of a1..a5 -----------------------------------------------------------
+ * phx_step_and_snapshot carries per-step values (ss, sbc2, the envelope) as kernel parameters, so a captured
+ * launch would replay a stale step.  Between phx_graph_begin and phx_graph_end the step index, the
+ * hyperparameters, the derived scalars and the envelope live in a DEVICE-RESIDENT step block: a one-thread
+ * prologue kernel advances the counter, derives the scalars in binary64 with individually rounded operations
+ * (the same bits as the host path) and writes the envelope; the fused kernel reads the scalars from there.
+ * Nothing per-step crosses the host, so  [compute window ‖ flush(k-1)] -> step k  can be captured once with
+ * cudaStreamBeginCapture / torch.cuda.graph and replayed (the sync point is then an edge of the
+ * graph).  The calls also work eagerly (same kernels), which is how a run enters and leaves.
+ *
+ *   phx_graph_begin(s, lr, beta1, beta2, eps, wd, stream)   mode switch (host-blocking: lands this handle's eager
+ *        flushes), initialises the step block at last_step on `stream`.  An un-flushed eager snapshot becomes
+ *        the first phx_graph_flush_async's work.  Not available with PHX_PAYLOAD_FULL_RANK_STATE.
+ *   phx_graph_set_hyper(...)                                 stream-ordered update of the hyperparameters (learning-
+ *        rate schedules) between replays; not captured itself.
+ *   phx_graph_step_and_snapshot(s, d_grads, stream)          a1 (if configured) + a2 + prologue + a3, capturable.  The
+ *        staging slot (issue index mod depth) and the host slot parity are fixed when the call is CAPTURED:
+ *        a captured sequence must span a multiple of lcm(depth, 2) steps and be replayed from the step
+ *        parity it was captured at; the prologue checks it on the device and phx_graph_end reports
+ *        PHX_ERR_STEP_ORDER if a replay ever ran misaligned.
+ *   phx_graph_flush_async(s, side_stream)                    a4 + a5 of the snapshot of the last ISSUED step,
+ *        capturable.  Inside a capture `side_stream` must already belong to the capture (fork it from the
+ *        capturing stream: record an event there, wait for it on side_stream); the next
+ *        phx_graph_step_and_snapshot's sync point joins it back.
+ *   phx_graph_end(s, &last_step)                             mode switch (cudaDeviceSynchronize): reads the device step
+ *        counter, rebuilds the commit bookkeeping from the self-describing host slots; afterwards the eager
+ *        calls continue at last_step + 1 and a still-staged newest snapshot can be flushed eagerly.
+ * Eager calls (step, flush, restore) return PHX_ERR_GRAPH_MODE in between, phx_graph_* outside. */
+PHX_API int phx_graph_begin(phx_shard_t *s, float lr, float beta1, float beta2, float eps, float wd, void *stream);
+PHX_API int phx_graph_set_hyper(phx_shard_t *s, float lr, float beta1, float beta2, float eps, float wd, void *stream);
+PHX_API int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *stream);
+PHX_API int phx_graph_flush_async(phx_shard_t *s, void *side_stream);
+PHX_API int phx_graph_end(phx_shard_t *s, uint64_t *last_step);
+
 /* ---- introspection ---------------------------------------------------------------------- */
 PHX_API int phx_last_step(const phx_shard_t *s, uint64_t *step);
-/* Host-blocking: clip coefficient and sum of squares of the last step (1.0 / 0 if clip is off). */
+/* Host-blocking (waits for the last step's kernel, not for the device): clip coefficient and sum of squares
+ * of the last step (1.0 / 0 if clip is off). */
 PHX_API int phx_last_clip(phx_shard_t *s, float *coef, double *sumsq);
 /* Number of kernels the library has launched on this handle (bench.py's gpu_launches). */
 PHX_API int phx_kernel_launches(const phx_shard_t *s, uint64_t *count);
-/* Selects a kernel variant of the fused step (0 = default); for tuning/benchmarks only.  Shards with
- * PHX_PRECISION_FP32 or decay groups accept variant 0 only. */
-PHX_API int phx_set_kernel_variant(phx_shard_t *s, uint32_t variant);
-/* Diagnostic for bench.py's roofline context (no handle, no state): enqueue ONE streaming pass over
- * n_read planes that are read and n_write planes that are written (plane i at d_buf + i*plane_bytes,
- * reads first; d_buf: device memory of (n_read+n_write)*plane_bytes bytes, 256-byte aligned; plane_bytes
- * a multiple of 256; each count <= 8) with the fused step's access pattern and no arithmetic — the HBM
- * ceiling for that read:write mix.  The written planes are overwritten with junk. */
-PHX_API int phx_hbm_probe_async(void *d_buf, uint64_t plane_bytes, uint32_t n_read, uint32_t n_write, void *stream);
+/* Snapshots that a later step superseded before the caller flushed them (see phx_step_and_snapshot's
+ * contract), to the host replica and to the ring peers. */
+PHX_API int phx_dropped_snapshots(const phx_shard_t *s, uint64_t *host, uint64_t *peers);
+/* The derived AdamW scalars {decay, omb1, omb2, ss, sbc2} exactly as the library computes them: on the host
+ * (binary64, individually rounded, works without a GPU) and by the device-side derivation of the
+ * graph-capturable form for n step indices (host arrays in and out: out[5*i..]; host-blocking; needs a GPU).
+ * Both must equal the oracle's bits; the tests pin them. */
+PHX_API int phx_derived_scalars_host(float lr, float beta1, float beta2, float wd, uint64_t step, float out[5]);
+PHX_API int phx_derived_scalars_device(float lr, float beta1, float beta2, float wd, const uint64_t *steps,
+                                       uint32_t n, float *out);
 PHX_API const char *phx_strerror(int err);
 PHX_API int phx_last_cuda_error(const phx_shard_t *s);
 PHX_API uint32_t phx_version(void);

@@ -31,6 +31,7 @@ PHX_ERR_UNSUPPORTED_DEVICE = -10
 PHX_ERR_SNAPSHOT_DISABLED = -11
 PHX_ERR_NOMEM = -12
 PHX_ERR_PARAMS_NOT_READY = -13
+PHX_ERR_GRAPH_MODE = -14
 
 PHX_SYNC_STRICT, PHX_SYNC_RELAXED = 0, 1
 PHX_RESTORE_COPY_ENGINE, PHX_RESTORE_BULK_KERNEL = 0, 1
@@ -111,11 +112,20 @@ PROTOTYPES = {
     "phx_restored_user_metadata": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(C.c_uint32)]),
     "phx_last_step": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_last_clip": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)]),
-    "phx_hbm_probe_async": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]),
     "phx_grad_sumsq_async": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "phx_set_clip_partials": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32]),
     "phx_kernel_launches": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
-    "phx_set_kernel_variant": (C.c_int, [C.c_void_p, C.c_uint32]),
+    "phx_dropped_snapshots": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]),
+    "phx_derived_scalars_host": (C.c_int, [C.c_float, C.c_float, C.c_float, C.c_float, C.c_uint64,
+                                           C.POINTER(C.c_float)]),
+    "phx_derived_scalars_device": (C.c_int, [C.c_float, C.c_float, C.c_float, C.c_float, C.POINTER(C.c_uint64),
+                                             C.c_uint32, C.POINTER(C.c_float)]),
+    "phx_grads_finalize_async": (C.c_int, [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "phx_graph_begin": (C.c_int, [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float, C.c_void_p]),
+    "phx_graph_set_hyper": (C.c_int, [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float, C.c_void_p]),
+    "phx_graph_step_and_snapshot": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "phx_graph_flush_async": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "phx_graph_end": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_ring_peer": (C.c_int, [C.c_uint32, C.c_uint32, C.c_int32, C.POINTER(C.c_uint32)]),
     "phx_peer_buffer_alloc": (C.c_int, [C.c_uint64, C.POINTER(C.c_void_p)]),
     "phx_peer_buffer_free": (C.c_int, [C.c_void_p]),
@@ -292,19 +302,65 @@ def phx_set_clip_partials(h: int, d_partials, count: int) -> None:
     _ck(lib().phx_set_clip_partials(h, _ptr(d_partials) or None, count), "phx_set_clip_partials", h)
 
 
-def phx_hbm_probe_async(d_buf, plane_bytes: int, n_read: int, n_write: int, stream=None) -> None:
-    """Diagnostic: one no-arithmetic streaming pass (n_read planes read, n_write written)."""
-    _ck(lib().phx_hbm_probe_async(_ptr(d_buf), plane_bytes, n_read, n_write, _ptr(stream)), "phx_hbm_probe_async")
-
-
 def phx_kernel_launches(h: int) -> int:
     n = C.c_uint64()
     _ck(lib().phx_kernel_launches(h, C.byref(n)), "phx_kernel_launches", h)
     return n.value
 
 
-def phx_set_kernel_variant(h: int, variant: int) -> None:
-    _ck(lib().phx_set_kernel_variant(h, variant), "phx_set_kernel_variant", h)
+def phx_dropped_snapshots(h: int) -> Tuple[int, int]:
+    """(snapshots superseded before a host flush, before a peer flush)."""
+    a, b = C.c_uint64(), C.c_uint64()
+    _ck(lib().phx_dropped_snapshots(h, C.byref(a), C.byref(b)), "phx_dropped_snapshots", h)
+    return a.value, b.value
+
+
+def phx_derived_scalars_host(lr: float, beta1: float, beta2: float, wd: float, step: int) -> List[float]:
+    """[decay, omb1, omb2, ss, sbc2] as the library's HOST code derives them (no GPU needed)."""
+    out = (C.c_float * 5)()
+    _ck(lib().phx_derived_scalars_host(lr, beta1, beta2, wd, step, out), "phx_derived_scalars_host")
+    return list(out)
+
+
+def phx_derived_scalars_device(lr: float, beta1: float, beta2: float, wd: float, steps: Sequence[int]) -> List[List[float]]:
+    """Per step index, [decay, omb1, omb2, ss, sbc2] as the graph form's DEVICE prologue derives them."""
+    n = len(steps)
+    arr = (C.c_uint64 * max(n, 1))(*[int(t) for t in steps])
+    out = (C.c_float * (5 * max(n, 1)))()
+    _ck(lib().phx_derived_scalars_device(lr, beta1, beta2, wd, arr, n, out), "phx_derived_scalars_device")
+    return [list(out[5 * i:5 * i + 5]) for i in range(n)]
+
+
+def phx_grads_finalize_async(h: int, d_main_grads_fp32, scale: float, d_grads_bf16_out, d_sumsq_out, stream=None) -> None:
+    """SURVEY 8(f4) second half: g16 = RNE_bf16(g32 * scale) and the fp64 sum of squares of the rounded values."""
+    _ck(lib().phx_grads_finalize_async(h, _ptr(d_main_grads_fp32), scale, _ptr(d_grads_bf16_out), _ptr(d_sumsq_out),
+                                       _ptr(stream)), "phx_grads_finalize_async", h)
+
+
+# ---- the graph-capturable form -------------------------------------------------------------------
+
+
+def phx_graph_begin(h: int, lr: float, beta1: float, beta2: float, eps: float, wd: float, stream=None) -> None:
+    _ck(lib().phx_graph_begin(h, lr, beta1, beta2, eps, wd, _ptr(stream)), "phx_graph_begin", h)
+
+
+def phx_graph_set_hyper(h: int, lr: float, beta1: float, beta2: float, eps: float, wd: float, stream=None) -> None:
+    _ck(lib().phx_graph_set_hyper(h, lr, beta1, beta2, eps, wd, _ptr(stream)), "phx_graph_set_hyper", h)
+
+
+def phx_graph_step_and_snapshot(h: int, d_grads, stream=None) -> None:
+    _ck(lib().phx_graph_step_and_snapshot(h, _ptr(d_grads), _ptr(stream)), "phx_graph_step_and_snapshot", h)
+
+
+def phx_graph_flush_async(h: int, side_stream=None) -> None:
+    _ck(lib().phx_graph_flush_async(h, _ptr(side_stream)), "phx_graph_flush_async", h)
+
+
+def phx_graph_end(h: int) -> int:
+    """Leaves the graph form; returns the device step counter (raises PHX_ERR_STEP_ORDER on a misaligned replay)."""
+    st = C.c_uint64()
+    _ck(lib().phx_graph_end(h, C.byref(st)), "phx_graph_end", h)
+    return st.value
 
 
 def phx_version() -> int:

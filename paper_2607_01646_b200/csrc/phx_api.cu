@@ -27,6 +27,17 @@ enum SlotState { SLOT_EMPTY = 0, SLOT_INFLIGHT, SLOT_COMMITTED, SLOT_TORN_INFLIG
 struct HostSlot {
     uint64_t step = 0;
     SlotState state = SLOT_EMPTY;
+    phx_snapshot_header_t hdr{};  // the committed envelope this handle sent to the slot (valid while state != EMPTY)
+};
+
+// an event plus the capture sequence it was last recorded in (0 = recorded eagerly).  A wait is enqueued only
+// when the waiting stream is in the same capture state: inside a capture the dependency on earlier eager work
+// (or on an earlier replay) is already given by the launch stream's order, and an event recorded in a capture
+// must not be waited on eagerly.
+struct GraphEvent {
+    cudaEvent_t ev = nullptr;
+    unsigned long long cap = 0;
+    bool valid = false;
 };
 
 // device scratch layout (bytes)
@@ -37,7 +48,9 @@ constexpr size_t kScrSumsq = 264;      // double
 constexpr size_t kScrPartials = 512;   // kSumsqMaxBlocks doubles
 constexpr size_t kScrHdr = kScrPartials + phx::kSumsqMaxBlocks * sizeof(double);  // 2 x 256 B headers (direct mode)
 constexpr size_t kScrHdrFull = kScrHdr + 2 * 256;  // kMaxDepth x 256 B full-rank-state headers (§8(f4))
-constexpr size_t kScrBytes = kScrHdrFull + 4 * 256;
+constexpr size_t kScrBlock = kScrHdrFull + 4 * 256;  // phx::StepBlock of the graph-capturable form
+constexpr size_t kScrBytes = kScrBlock + 1024;
+static_assert(sizeof(phx::StepBlock) <= 1024, "step block must fit its scratch region");
 
 uint64_t fnv1a64(const void *data, size_t len, uint64_t h = 0xCBF29CE484222325ull)
 {
@@ -91,7 +104,6 @@ struct phx_shard {
     uint32_t user_len = 0;
     uint8_t restored_user[128] = {0};
     uint32_t restored_user_len = 0;
-    uint64_t restore_hdr_step[2] = {0, 0};
     // staging ring / flush bookkeeping
     cudaEvent_t ev_step[kMaxDepth] = {nullptr, nullptr, nullptr, nullptr};
     cudaEvent_t ev_flush[kMaxDepth] = {nullptr, nullptr, nullptr, nullptr};
@@ -113,10 +125,16 @@ struct phx_shard {
     int pending_peer_slot = -1;
     uint64_t pending_peer_step = 0;
     int64_t torn_peer_chunks[PHX_MAX_PEERS] = {-1, -1, -1, -1};
+    // k > 1: one library-owned copy stream per peer, forked from / joined into the caller's peer stream
+    cudaStream_t peer_st[PHX_MAX_PEERS] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev_peer_fork = nullptr;
+    cudaEvent_t ev_peer_join[PHX_MAX_PEERS] = {nullptr, nullptr, nullptr, nullptr};
     // §8(f3) publication of the model-param copy into other DP ranks' parameter buffers
     uint32_t n_pub = 0, pub_mode = PHX_PUBLISH_FUSED;
     uint8_t *d_pub[PHX_MAX_PARAM_PEERS] = {nullptr};
     cudaEvent_t ev_last_step = nullptr;  // recorded after every step's kernel (publication by copy engine waits on it)
+    cudaEvent_t ev_pub = nullptr;        // the newest copy-engine publication has finished reading the model-param copy
+    bool pub_valid = false;
     // §8(f4) full rank-state local snapshot: the model-parameter buffer W and its readiness / guard events
     uint8_t *d_W = nullptr;
     cudaEvent_t ev_params = nullptr;   // W holds every rank's parameters after step params_ready_step
@@ -126,10 +144,17 @@ struct phx_shard {
     // misc
     int last_cuda_error = 0;
     uint64_t launches = 0;
-    uint32_t variant = 0;
+    uint64_t dropped_host = 0, dropped_peers = 0;  // snapshots overwritten before they were flushed
     bool clip_valid = false;
     const double *clip_partials = nullptr;  // §8(e) global clip: one-shot per-rank sums for the next step
     uint32_t clip_count = 0;
+    // graph-capturable form (include/phx.h "graph"): host mirror of the issue order; the device step block is the truth
+    bool graph = false;
+    uint64_t g_issue = 0;          // steps issued (captured or eager) since phx_graph_begin, on top of last_step at begin
+    int g_pending_slot = -1;
+    uint64_t g_pending_step = 0;
+    int g_last_flush_slot = -1;
+    GraphEvent gev_step[kMaxDepth], gev_flush[kMaxDepth];
 };
 
 #define PHX_CK(call)                                  \
@@ -345,6 +370,7 @@ const char *phx_strerror(int err)
     case PHX_ERR_SNAPSHOT_DISABLED: return "snapshots are disabled on this shard";
     case PHX_ERR_NOMEM: return "out of memory";
     case PHX_ERR_PARAMS_NOT_READY: return "model-parameter buffer not declared ready for this step";
+    case PHX_ERR_GRAPH_MODE: return "call not available between phx_graph_begin and phx_graph_end (or outside them)";
     default: return "unknown error";
     }
 }
@@ -441,6 +467,16 @@ int phx_shard_destroy(phx_shard_t *s)
             if (s->ev_peer[k]) cudaEventDestroy(s->ev_peer[k]);
         }
         if (s->ev_last_step) cudaEventSynchronize(s->ev_last_step), cudaEventDestroy(s->ev_last_step);
+        if (s->ev_pub) cudaEventSynchronize(s->ev_pub), cudaEventDestroy(s->ev_pub);
+        if (s->ev_peer_fork) cudaEventDestroy(s->ev_peer_fork);
+        for (int k = 0; k < PHX_MAX_PEERS; ++k) {
+            if (s->ev_peer_join[k]) cudaEventDestroy(s->ev_peer_join[k]);
+            if (s->peer_st[k]) cudaStreamSynchronize(s->peer_st[k]), cudaStreamDestroy(s->peer_st[k]);
+        }
+        for (int k = 0; k < kMaxDepth; ++k) {
+            if (s->gev_step[k].ev) cudaEventDestroy(s->gev_step[k].ev);
+            if (s->gev_flush[k].ev) cudaEventDestroy(s->gev_flush[k].ev);
+        }
         if (s->ev_params) cudaEventDestroy(s->ev_params);
         if (s->ev_wflush) cudaEventDestroy(s->ev_wflush);
         if (s->d_scratch) cudaFree(s->d_scratch);
@@ -509,6 +545,11 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
         PHX_CK(cudaEventCreateWithFlags(&s->ev_pflush[k], cudaEventDisableTiming));
     }
     PHX_CK(cudaEventCreateWithFlags(&s->ev_last_step, cudaEventDisableTiming));
+    PHX_CK(cudaEventCreateWithFlags(&s->ev_pub, cudaEventDisableTiming));
+    for (int k = 0; k < kMaxDepth; ++k) {
+        PHX_CK(cudaEventCreateWithFlags(&s->gev_step[k].ev, cudaEventDisableTiming));
+        PHX_CK(cudaEventCreateWithFlags(&s->gev_flush[k].ev, cudaEventDisableTiming));
+    }
     PHX_CK(cudaEventCreateWithFlags(&s->ev_params, cudaEventDisableTiming));
     PHX_CK(cudaEventCreateWithFlags(&s->ev_wflush, cudaEventDisableTiming));
     for (int k = 0; k < 2; ++k) {
@@ -556,65 +597,77 @@ int phx_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len)
 }
 
 // ---- a1 + a2 + a3 --------------------------------------------------------------------------------
-int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float beta1, float beta2, float eps,
-                          float wd, uint64_t step, void *stream)
+namespace {
+
+// derived scalars: double on the host, every operation individually rounded (the file is compiled with
+// -ffp-contract=off), rounded once to fp32 (include/phx.h a3, reading R6)
+void derive_scalars_host(float lr, float beta1, float beta2, float eps, float wd, uint64_t step, phx::AdamScalars *sc)
 {
-    if (!s || !d_grads) return PHX_ERR_INVALID_ARG;
-    if (!s->bound) return PHX_ERR_NOT_BOUND;
-    if (!aligned256(d_grads)) return PHX_ERR_ALIGNMENT;
-    if (step != s->last_step + 1) return PHX_ERR_STEP_ORDER;  // I4 step atomicity (PAPER.md:169)
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const bool snap = snapshots_on(s);
-
-    phx::StepArgs a;
-    std::memset(&a, 0, sizeof(a));
-    // derived scalars: double on the host, rounded once to fp32 (include/phx.h a3)
     const double dlr = lr, db1 = beta1, db2 = beta2, dwd = wd;
-    a.sc.beta1 = beta1;
-    a.sc.beta2 = beta2;
-    a.sc.eps = eps;
-    a.sc.decay = (float)(1.0 - dlr * dwd);
-    a.sc.omb1 = (float)(1.0 - db1);
-    a.sc.omb2 = (float)(1.0 - db2);
-    a.sc.ss = (float)(dlr / (1.0 - pow_sqmul(db1, step)));
-    a.sc.sbc2 = (float)std::sqrt(1.0 - pow_sqmul(db2, step));
+    sc->beta1 = beta1;
+    sc->beta2 = beta2;
+    sc->eps = eps;
+    const double lw = dlr * dwd;
+    sc->decay = (float)(1.0 - lw);
+    sc->omb1 = (float)(1.0 - db1);
+    sc->omb2 = (float)(1.0 - db2);
+    const double b1t = pow_sqmul(db1, step), b2t = pow_sqmul(db2, step);
+    sc->ss = (float)(dlr / (1.0 - b1t));
+    sc->sbc2 = (float)std::sqrt(1.0 - b2t);
+}
 
-    // a1: optional clip by the shard-local gradient norm
+unsigned long long capture_id(cudaStream_t st)
+{
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    unsigned long long id = 0;
+    if (cudaStreamGetCaptureInfo(st, &cs, &id) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 0;
+    }
+    return cs == cudaStreamCaptureStatusActive ? id : 0;
+}
+int gev_record(phx_shard *s, GraphEvent &g, cudaStream_t st)
+{
+    PHX_CK(cudaEventRecord(g.ev, st));
+    g.cap = capture_id(st);
+    g.valid = true;
+    return PHX_OK;
+}
+int gev_wait(phx_shard *s, const GraphEvent &g, cudaStream_t st)
+{
+    if (g.valid && g.cap == capture_id(st)) PHX_CK(cudaStreamWaitEvent(st, g.ev, 0));
+    return PHX_OK;
+}
+
+// a1: optional clip — from the one-shot partials the caller exchanged (§8(e), §8(f4b)) or by the shard's own pass
+int enqueue_clip(phx_shard *s, const void *d_grads, phx::StepArgs &a, cudaStream_t st)
+{
     a.coef = reinterpret_cast<const float *>(s->d_scratch + kScrOne);
     s->clip_valid = false;
-    if (s->cfg.max_grad_norm > 0.0f && s->clip_partials != nullptr) {
-        // §8(e): S = sum of the per-rank sums the caller exchanged; this rank's own pass already ran
+    if (!(s->cfg.max_grad_norm > 0.0f)) return PHX_OK;
+    if (s->clip_partials != nullptr) {
         PHX_CK(phx::launch_clip_from_partials(s->clip_partials, s->clip_count, s->cfg.max_grad_norm,
                                               reinterpret_cast<double *>(s->d_scratch + kScrSumsq),
                                               reinterpret_cast<float *>(s->d_scratch + kScrCoef), st));
         s->launches += 1;
-        a.coef = reinterpret_cast<const float *>(s->d_scratch + kScrCoef);
-        s->clip_valid = true;
         s->clip_partials = nullptr;
         s->clip_count = 0;
-    } else if (s->cfg.max_grad_norm > 0.0f) {
+    } else {
         int nl = 0;
         PHX_CK(phx::launch_sumsq_clip(d_grads, fp32_mode(s), s->info.n_padded, s->cfg.max_grad_norm,
                                       reinterpret_cast<double *>(s->d_scratch + kScrPartials),
                                       reinterpret_cast<double *>(s->d_scratch + kScrSumsq),
                                       reinterpret_cast<float *>(s->d_scratch + kScrCoef), st, &nl));
         s->launches += nl;
-        a.coef = reinterpret_cast<const float *>(s->d_scratch + kScrCoef);
-        s->clip_valid = true;
     }
+    a.coef = reinterpret_cast<const float *>(s->d_scratch + kScrCoef);
+    s->clip_valid = true;
+    return PHX_OK;
+}
 
-    int slot = -1;
-    if (snap) {
-        slot = (int)(step % ring_depth(s));
-        // a2: the single sync point (PAPER.md:226) — stream-side wait, the host never blocks
-        // ("guarantees the peer-resident replica is fully committed before the optimizer mutates the protected state")
-        if (s->cfg.sync_mode == PHX_SYNC_STRICT) {
-            if (s->last_flush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[s->last_flush_slot], 0));
-            if (s->last_pflush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_pflush[s->last_pflush_slot], 0));
-        } else {
-            if (s->flush_valid[slot]) PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[slot], 0));
-            if (s->pflush_valid[slot]) PHX_CK(cudaStreamWaitEvent(st, s->ev_pflush[slot], 0));
-        }
+void fill_common_args(const phx_shard *s, const void *d_grads, int slot, phx::StepArgs &a)
+{
+    if (slot >= 0) {
         if (direct_mode(s)) {
             a.shdr = s->d_scratch + kScrHdr + (size_t)slot * kHeaderBytes;  // header only; planes stay live
         } else {
@@ -623,16 +676,6 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
             a.sp = reinterpret_cast<float *>(base + kHeaderBytes);
             a.sm = a.sp + s->info.n_padded;
             a.sv = a.sm + s->info.n_padded;
-        }
-        phx_snapshot_header_t hdr;
-        build_header(s, step, true, &hdr);
-        std::memcpy(&a.hdr, &hdr, sizeof(hdr));
-        if (full_payload(s)) {  // §8(f4): the local slot's envelope differs in the payload word and the hash
-            phx_snapshot_header_t hf;
-            build_header(s, step, true, &hf, full_payload_word(s));
-            a.shdr_full = s->d_scratch + kScrHdrFull + (size_t)slot * kHeaderBytes;
-            a.full_payload = hf.payload;
-            a.full_hash = hf.header_hash;
         }
     }
     a.p = s->d_p;
@@ -652,9 +695,63 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
         for (uint32_t q = 0; q < s->n_pub; ++q)
             a.pub[q] = s->d_pub[q] + (uint64_t)s->info.dp_rank * s->info.n_padded * model_elem_bytes(s);
     }
+}
+
+}  // namespace
+
+int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float beta1, float beta2, float eps,
+                          float wd, uint64_t step, void *stream)
+{
+    if (!s || !d_grads) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (s->graph) return PHX_ERR_GRAPH_MODE;
+    if (!aligned256(d_grads)) return PHX_ERR_ALIGNMENT;
+    if (step != s->last_step + 1) return PHX_ERR_STEP_ORDER;  // I4 step atomicity (PAPER.md:169)
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const bool snap = snapshots_on(s);
+
+    phx::StepArgs a;
+    std::memset(&a, 0, sizeof(a));
+    derive_scalars_host(lr, beta1, beta2, eps, wd, step, &a.sc);
+    int rc = enqueue_clip(s, d_grads, a, st);
+    if (rc != PHX_OK) return rc;
+
+    int slot = -1;
+    if (snap) {
+        slot = (int)(step % ring_depth(s));
+        // a2: the single sync point (PAPER.md:226) — stream-side wait, the host never blocks
+        // ("guarantees the peer-resident replica is fully committed before the optimizer mutates the protected state")
+        if (s->cfg.sync_mode == PHX_SYNC_STRICT) {
+            if (s->last_flush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[s->last_flush_slot], 0));
+            if (s->last_pflush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_pflush[s->last_pflush_slot], 0));
+        } else {
+            if (s->flush_valid[slot]) PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[slot], 0));
+            if (s->pflush_valid[slot]) PHX_CK(cudaStreamWaitEvent(st, s->ev_pflush[slot], 0));
+            // §8(f4): the full-rank-state flush reads the live W (this rank's range of it is d_p_bf16) whatever the
+            // staging depth, so even a relaxed step must not start before the newest flush has finished READING W
+            if (full_payload(s) && s->wflush_valid) PHX_CK(cudaStreamWaitEvent(st, s->ev_wflush, 0));
+        }
+        // contract: a snapshot the caller never flushed is overwritten by its successor's slot reuse / superseded;
+        // it is counted, not an error (phx_dropped_snapshots)
+        if (s->pending_slot >= 0 && s->h_replica) s->dropped_host += 1;
+        if (s->pending_peer_slot >= 0 && s->n_peers) s->dropped_peers += 1;
+        phx_snapshot_header_t hdr;
+        build_header(s, step, true, &hdr);
+        std::memcpy(&a.hdr, &hdr, sizeof(hdr));
+        if (full_payload(s)) {  // §8(f4): the local slot's envelope differs in the payload word and the hash
+            phx_snapshot_header_t hf;
+            build_header(s, step, true, &hf, full_payload_word(s));
+            a.shdr_full = s->d_scratch + kScrHdrFull + (size_t)slot * kHeaderBytes;
+            a.full_payload = hf.payload;
+            a.full_hash = hf.header_hash;
+        }
+    }
+    // a copy-engine publication of the previous step may still be reading the model-param copy this kernel rewrites
+    if (s->pub_valid) PHX_CK(cudaStreamWaitEvent(st, s->ev_pub, 0));
+    fill_common_args(s, d_grads, slot, a);
 
     // a3: one kernel, one pass
-    PHX_CK(phx::launch_step(a, snap && !direct_mode(s), s->variant, step_mode(s), st));
+    PHX_CK(phx::launch_step(a, snap && !direct_mode(s), step_mode(s), false, st));
     s->launches += s->info.n_padded ? 1 : 0;
     PHX_CK(cudaEventRecord(s->ev_last_step, st));
     if (snap) {
@@ -675,6 +772,7 @@ int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream)
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound || (snapshots_on(s) && !s->h_replica)) return PHX_ERR_NOT_BOUND;
     if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
+    if (s->graph) return PHX_ERR_GRAPH_MODE;
     if (s->pending_slot < 0) return PHX_ERR_NO_FLUSH_PENDING;
     cudaStream_t st = static_cast<cudaStream_t>(side_stream);
     const int slot = s->pending_slot;
@@ -695,6 +793,7 @@ int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream)
     const bool torn = s->torn_chunks >= 0;
     s->host[hs].step = step;
     s->host[hs].state = torn ? SLOT_TORN_INFLIGHT : SLOT_INFLIGHT;
+    build_header(s, step, true, &s->host[hs].hdr, full ? full_payload_word(s) : 0u);  // what lands last, if it lands
     int rc = enqueue_snapshot_copy(s, st, dst, cudaMemcpyDeviceToHost, slot, s->torn_chunks, full);
     if (rc != PHX_OK) return rc;
     PHX_CK(cudaEventRecord(s->ev_flush[slot], st));
@@ -742,28 +841,37 @@ int phx_fault_inject_torn_flush(phx_shard_t *s, int64_t payload_chunks)
 // ---- a6 ------------------------------------------------------------------------------------------
 namespace {
 
-// Rebuild the live shard from `replica` (two slots at slot_stride).  hdr_src: where the host can read the
-// two headers with a blocking copy; copy_src: address for copy-engine copies; kern_src: device-visible
-// address for the bulk kernel.  Selection depends only on what is IN the replica.
-// stride: distance of the two slots; want_payload: the envelope's payload word the slot must carry (0 =
-// optimizer-only; the full-rank-state word: the model-parameter buffer W behind p ‖ m ‖ v is restored too).
-int restore_impl(phx_shard *s, const uint8_t *hdr_src, const uint8_t *copy_src, const uint8_t *kern_src,
-                 bool hdr_on_host, cudaStream_t st, uint64_t *restored_step, bool *valid_out, uint64_t stride,
-                 uint32_t want_payload)
+// Choose between two envelopes the valid, identity-matching one with the largest step.
+int choose_slot(const phx_shard *s, const phx_snapshot_header_t hdr[2], const bool usable[2], uint32_t want_payload,
+                bool ok[2])
 {
     int best = -1;
     bool any_valid = false;
-    phx_snapshot_header_t hdr[2];
     for (int i = 0; i < 2; ++i) {
-        const uint8_t *hp = hdr_src + (uint64_t)i * stride;
-        if (hdr_on_host) std::memcpy(&hdr[i], hp, sizeof(hdr[i]));
-        else PHX_CK(cudaMemcpy(&hdr[i], hp, sizeof(hdr[i]), cudaMemcpyDefault));
-        if (!header_valid(&hdr[i])) continue;
+        ok[i] = false;
+        if (!usable[i] || !header_valid(&hdr[i])) continue;
         any_valid = true;
         if (!header_matches(s, &hdr[i]) || hdr[i].payload != want_payload) continue;
+        ok[i] = true;
         if (best < 0 || hdr[i].step > hdr[best].step) best = i;
     }
     if (best < 0) return any_valid ? PHX_ERR_LAYOUT_MISMATCH : PHX_ERR_NO_COMMITTED_SNAPSHOT;
+    return best;
+}
+
+// Enqueue the rebuild of the live shard from slot `best` of a replica (two slots `stride` apart).
+// copy_src: address for copy-engine copies; kern_src: device-visible address for the bulk kernel.
+int enqueue_restore(phx_shard *s, int best, const phx_snapshot_header_t &hdr, const uint8_t *copy_src,
+                    const uint8_t *kern_src, cudaStream_t st, uint64_t stride, uint32_t want_payload)
+{
+    // The copies overwrite the live planes (and W): order them behind everything of THIS handle that may still be
+    // reading or writing them — the newest step's kernel, a direct-source flush to the host or to the peers, a
+    // full-rank-state flush reading W, a copy-engine publication.
+    if (s->last_step > 0 || s->ev_last_step) PHX_CK(cudaStreamWaitEvent(st, s->ev_last_step, 0));
+    if (s->last_flush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[s->last_flush_slot], 0));
+    if (s->last_pflush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_pflush[s->last_pflush_slot], 0));
+    if (s->wflush_valid) PHX_CK(cudaStreamWaitEvent(st, s->ev_wflush, 0));
+    if (s->pub_valid) PHX_CK(cudaStreamWaitEvent(st, s->ev_pub, 0));
 
     const uint64_t N = s->info.n_padded;
     const uint64_t off = (uint64_t)best * stride + kHeaderBytes;
@@ -783,51 +891,71 @@ int restore_impl(phx_shard *s, const uint8_t *hdr_src, const uint8_t *copy_src, 
     }
     if (want_payload != 0)  // §8(f4) in-place recovery: W comes back from the same slot, no other rank is read
         PHX_CK(cudaMemcpyAsync(s->d_W, copy_src + off + 12 * N, s->info.param_bytes, cudaMemcpyDefault, st));
-    s->last_step = hdr[best].step;
+    PHX_CK(cudaEventRecord(s->ev_last_step, st));  // later flushes / publications order behind the restore
+    s->last_step = hdr.step;
     s->pending_slot = -1;
     s->pending_peer_slot = -1;
     s->params_ready = false;
     s->clip_partials = nullptr;  // the recompute of the in-flight step exchanges its sums again
     s->clip_count = 0;
-    s->restored_user_len = hdr[best].user_len <= 128 ? hdr[best].user_len : 128;
-    std::memcpy(s->restored_user, hdr[best].user, 128);
-    for (int i = 0; i < 2; ++i)
-        valid_out[i] = header_valid(&hdr[i]) && header_matches(s, &hdr[i]) && hdr[i].payload == want_payload;
-    if (restored_step) *restored_step = s->last_step;
-    // the slots' steps, for the caller's own slot bookkeeping
-    s->restore_hdr_step[0] = hdr[0].step;
-    s->restore_hdr_step[1] = hdr[1].step;
+    s->restored_user_len = hdr.user_len <= 128 ? hdr.user_len : 128;
+    std::memcpy(s->restored_user, hdr.user, 128);
     return PHX_OK;
 }
 
 }  // namespace
 
+// Enqueue-only: the host never waits for the device here.  Which slot to take is decided from
+//   - the envelope IN the pinned host slot, read with a plain memcpy, for a slot this handle is not writing
+//     (never used by this handle, or its flush event has completed — cudaEventQuery, non-blocking);
+//   - the handle's own commit bookkeeping for a slot whose flush is still in flight: the envelope it sent is
+//     known, the flush cannot tear (a torn flush is known as such and skipped), and `stream` is made to wait
+//     for the flush event before the copies, so the payload has landed when it is read.
 int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
 {
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound || (snapshots_on(s) && !s->h_replica)) return PHX_ERR_NOT_BOUND;
     if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
-    // in-flight flushes must land (or be known torn) before the host reads the headers
-    int rc = settle_host_slots(s, true);
-    if (rc != PHX_OK) return rc;
-    bool ok[2] = {false, false};
+    if (s->graph) return PHX_ERR_GRAPH_MODE;
     if (full_payload(s) && !s->d_W) return PHX_ERR_NOT_BOUND;
-    rc = restore_impl(s, s->h_replica, s->h_replica, s->d_replica, true, static_cast<cudaStream_t>(stream), restored_step, ok,
-                      s->info.host_slot_stride, full_payload(s) ? full_payload_word(s) : 0u);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int rc = settle_host_slots(s, false);
     if (rc != PHX_OK) return rc;
+    phx_snapshot_header_t hdr[2];
+    bool usable[2], inflight[2], ok[2];
     for (int i = 0; i < 2; ++i) {
-        s->host[i].state = ok[i] ? SLOT_COMMITTED : (s->host[i].state == SLOT_EMPTY ? SLOT_EMPTY : SLOT_TORN);
-        if (ok[i]) s->host[i].step = s->restore_hdr_step[i];
+        inflight[i] = s->host[i].state == SLOT_INFLIGHT;
+        usable[i] = s->host[i].state != SLOT_TORN_INFLIGHT;  // being torn right now: whatever it shows is going away
+        if (inflight[i]) hdr[i] = s->host[i].hdr;
+        else std::memcpy(&hdr[i], s->h_replica + (uint64_t)i * s->info.host_slot_stride, sizeof(hdr[i]));
     }
+    const uint32_t want = full_payload(s) ? full_payload_word(s) : 0u;
+    const int best = choose_slot(s, hdr, usable, want, ok);
+    if (best < 0) return best;
+    if (inflight[best]) PHX_CK(cudaStreamWaitEvent(st, s->ev_host[best], 0));
+    rc = enqueue_restore(s, best, hdr[best], s->h_replica, s->d_replica, st, s->info.host_slot_stride, want);
+    if (rc != PHX_OK) return rc;
+    for (int i = 0; i < 2; ++i) {  // adopt what the replica shows (a replacement handle starts with EMPTY slots)
+        if (inflight[i] || s->host[i].state == SLOT_TORN_INFLIGHT) continue;
+        s->host[i].state = ok[i] ? SLOT_COMMITTED : (s->host[i].state == SLOT_EMPTY ? SLOT_EMPTY : SLOT_TORN);
+        if (ok[i]) {
+            s->host[i].step = hdr[i].step;
+            s->host[i].hdr = hdr[i];
+        }
+    }
+    if (restored_step) *restored_step = s->last_step;
     return PHX_OK;
 }
 
 // §8(f1): restore from a replica held elsewhere — a peer's received buffer mapped into this process
-// (PAPER.md:171 stage 3, 248-250), a device buffer, or pinned host memory.
+// (PAPER.md:171 stage 3, 248-250), a device buffer, or pinned host memory.  The replica is FOREIGN: this
+// handle has no bookkeeping for it, so the two envelopes are read with a blocking copy (the documented
+// exception to "only enqueue"; 512 bytes).
 int phx_restore_from(phx_shard_t *s, const void *replica, void *stream, uint64_t *restored_step)
 {
     if (!s || !replica) return PHX_ERR_INVALID_ARG;
     if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (s->graph) return PHX_ERR_GRAPH_MODE;
     if (!aligned256(replica)) return PHX_ERR_ALIGNMENT;
     cudaPointerAttributes at;
     cudaError_t e = cudaPointerGetAttributes(&at, replica);
@@ -836,9 +964,17 @@ int phx_restore_from(phx_shard_t *s, const void *replica, void *stream, uint64_t
         return PHX_ERR_INVALID_ARG;  // pageable host memory or an unknown address
     }
     const uint8_t *r = static_cast<const uint8_t *>(replica);
+    phx_snapshot_header_t hdr[2];
+    const bool usable[2] = {true, true};
     bool ok[2];
-    return restore_impl(s, r, r, static_cast<const uint8_t *>(at.devicePointer), false, static_cast<cudaStream_t>(stream),
-                        restored_step, ok, s->info.slot_stride, 0u);
+    for (int i = 0; i < 2; ++i)
+        PHX_CK(cudaMemcpy(&hdr[i], r + (uint64_t)i * s->info.slot_stride, sizeof(hdr[i]), cudaMemcpyDefault));
+    const int best = choose_slot(s, hdr, usable, 0u, ok);
+    if (best < 0) return best;
+    int rc = enqueue_restore(s, best, hdr[best], r, static_cast<const uint8_t *>(at.devicePointer),
+                             static_cast<cudaStream_t>(stream), s->info.slot_stride, 0u);
+    if (rc == PHX_OK && restored_step) *restored_step = s->last_step;
+    return rc;
 }
 
 int phx_restored_user_metadata(const phx_shard_t *s, void *blob, uint32_t cap, uint32_t *len)
@@ -931,6 +1067,11 @@ int phx_shard_bind_peers(phx_shard_t *s, void *const *d_peer_replicas, uint32_t 
     }
     int rc = settle_peer_slots(s, true);
     if (rc != PHX_OK) return rc;
+    if (k > 1 && !s->ev_peer_fork) PHX_CK(cudaEventCreateWithFlags(&s->ev_peer_fork, cudaEventDisableTiming));
+    for (uint32_t j = 0; k > 1 && j < k; ++j) {
+        if (!s->peer_st[j]) PHX_CK(cudaStreamCreateWithFlags(&s->peer_st[j], cudaStreamNonBlocking));
+        if (!s->ev_peer_join[j]) PHX_CK(cudaEventCreateWithFlags(&s->ev_peer_join[j], cudaEventDisableTiming));
+    }
     for (uint32_t j = 0; j < PHX_MAX_PEERS; ++j) s->d_peer[j] = j < k ? static_cast<uint8_t *>(d_peer_replicas[j]) : nullptr;
     s->n_peers = k;
     return PHX_OK;
@@ -941,6 +1082,7 @@ int phx_snapshot_flush_peers_async(phx_shard_t *s, void *peer_stream)
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound || s->n_peers == 0) return PHX_ERR_NOT_BOUND;
     if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
+    if (s->graph) return PHX_ERR_GRAPH_MODE;
     if (s->pending_peer_slot < 0) return PHX_ERR_NO_FLUSH_PENDING;
     cudaStream_t st = static_cast<cudaStream_t>(peer_stream);
     const int slot = s->pending_peer_slot;
@@ -953,11 +1095,22 @@ int phx_snapshot_flush_peers_async(phx_shard_t *s, void *peer_stream)
     for (uint32_t j = 0; j < s->n_peers; ++j) any_torn = any_torn || s->torn_peer_chunks[j] >= 0;
     s->peer[ps].step = step;
     s->peer[ps].state = any_torn ? SLOT_TORN_INFLIGHT : SLOT_INFLIGHT;
-    for (uint32_t j = 0; j < s->n_peers; ++j) {  // one stream: the source GPU's NVLink egress is the shared limit
+    // k = 1: the caller's stream.  k > 1: one library-owned copy stream per peer, forked from and joined back
+    // into the caller's stream, so that the k transfers use k copy engines / NVLink ports at once (NVSwitch
+    // gives every peer its own path; whether the source's egress then is the limit is for hardware to say).
+    const bool fan = s->n_peers > 1;
+    if (fan) PHX_CK(cudaEventRecord(s->ev_peer_fork, st));
+    for (uint32_t j = 0; j < s->n_peers; ++j) {
+        cudaStream_t pst = fan ? s->peer_st[j] : st;
+        if (fan) PHX_CK(cudaStreamWaitEvent(pst, s->ev_peer_fork, 0));
         uint8_t *dst = s->d_peer[j] + (uint64_t)ps * s->info.slot_stride;
-        int rc = enqueue_snapshot_copy(s, st, dst, cudaMemcpyDefault, slot, s->torn_peer_chunks[j]);
+        int rc = enqueue_snapshot_copy(s, pst, dst, cudaMemcpyDefault, slot, s->torn_peer_chunks[j]);
         if (rc != PHX_OK) return rc;
         s->torn_peer_chunks[j] = -1;
+        if (fan) {
+            PHX_CK(cudaEventRecord(s->ev_peer_join[j], pst));
+            PHX_CK(cudaStreamWaitEvent(st, s->ev_peer_join[j], 0));
+        }
     }
     PHX_CK(cudaEventRecord(s->ev_pflush[slot], st));
     PHX_CK(cudaEventRecord(s->ev_peer[ps], st));
@@ -1005,7 +1158,6 @@ int phx_shard_bind_param_peers(phx_shard_t *s, void *const *d_param_bufs, uint32
     if (!s || (count && !d_param_bufs) || count > PHX_MAX_PARAM_PEERS || mode > PHX_PUBLISH_COPY_ENGINE)
         return PHX_ERR_INVALID_ARG;
     if (!s->bound) return PHX_ERR_NOT_BOUND;
-    if (count && mode == PHX_PUBLISH_FUSED && s->variant != 0) return PHX_ERR_INVALID_ARG;
     for (uint32_t q = 0; q < count; ++q) {
         if (!d_param_bufs[q]) return PHX_ERR_INVALID_ARG;
         if (!aligned256(d_param_bufs[q])) return PHX_ERR_ALIGNMENT;
@@ -1026,6 +1178,8 @@ int phx_publish_params_async(phx_shard_t *s, void *stream)
     PHX_CK(cudaStreamWaitEvent(st, s->ev_last_step, 0));  // the newest step's kernel has written the slice
     for (uint32_t q = 0; q < s->n_pub; ++q)
         PHX_CK(cudaMemcpyAsync(s->d_pub[q] + (uint64_t)s->info.dp_rank * bytes, src, bytes, cudaMemcpyDefault, st));
+    PHX_CK(cudaEventRecord(s->ev_pub, st));  // the next step (a2) and a restore wait for these reads
+    s->pub_valid = true;
     return PHX_OK;
 }
 
@@ -1114,26 +1268,12 @@ int phx_last_clip(phx_shard_t *s, float *coef, double *sumsq)
     float c = 1.0f;
     double q = 0.0;
     if (s->clip_valid) {
-        PHX_CK(cudaDeviceSynchronize());
+        PHX_CK(cudaEventSynchronize(s->ev_last_step));  // the step that used it has run
         PHX_CK(cudaMemcpy(&c, s->d_scratch + kScrCoef, 4, cudaMemcpyDeviceToHost));
         PHX_CK(cudaMemcpy(&q, s->d_scratch + kScrSumsq, 8, cudaMemcpyDeviceToHost));
     }
     if (coef) *coef = c;
     if (sumsq) *sumsq = q;
-    return PHX_OK;
-}
-
-int phx_hbm_probe_async(void *d_buf, uint64_t plane_bytes, uint32_t n_read, uint32_t n_write, void *stream)
-{
-    if (!d_buf || plane_bytes == 0 || (plane_bytes & 255u) || n_read > (uint32_t)phx::kProbeMaxPlanes ||
-        n_write > (uint32_t)phx::kProbeMaxPlanes || n_read + n_write == 0)
-        return PHX_ERR_INVALID_ARG;
-    if (!aligned256(d_buf)) return PHX_ERR_ALIGNMENT;
-    cudaError_t e = phx::launch_hbm_probe(d_buf, plane_bytes, n_read, n_write, static_cast<cudaStream_t>(stream));
-    if (e != cudaSuccess) {
-        (void)cudaGetLastError();
-        return PHX_ERR_CUDA;
-    }
     return PHX_OK;
 }
 
@@ -1144,12 +1284,204 @@ int phx_kernel_launches(const phx_shard_t *s, uint64_t *count)
     return PHX_OK;
 }
 
-int phx_set_kernel_variant(phx_shard_t *s, uint32_t variant)
+int phx_dropped_snapshots(const phx_shard_t *s, uint64_t *host, uint64_t *peers)
 {
-    if (!s || variant >= phx::kNumStepVariants) return PHX_ERR_INVALID_ARG;
-    if (variant != 0 && step_mode(s) != 0) return PHX_ERR_INVALID_ARG;  // §8(f2)/(f3) modes: default flavour only
-    s->variant = variant;
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (host) *host = s->dropped_host;
+    if (peers) *peers = s->dropped_peers;
     return PHX_OK;
+}
+
+// ---- §8(f4), second half: the gradient producer's epilogue ------------------------------------------
+int phx_grads_finalize_async(phx_shard_t *s, const float *d_main_grads_fp32, float scale, void *d_grads_bf16_out,
+                             double *d_sumsq_out, void *stream)
+{
+    if (!s || !d_main_grads_fp32 || !d_grads_bf16_out || !d_sumsq_out || !(scale == scale)) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (fp32_mode(s)) return PHX_ERR_INVALID_ARG;  // the all-FP32 precision has no bf16 gradients to produce
+    if (!aligned256(d_main_grads_fp32) || !aligned256(d_grads_bf16_out) || (reinterpret_cast<uintptr_t>(d_sumsq_out) & 7u))
+        return PHX_ERR_ALIGNMENT;
+    const uint64_t N = s->info.n_padded;
+    const uint8_t *in0 = reinterpret_cast<const uint8_t *>(d_main_grads_fp32), *out0 = static_cast<const uint8_t *>(d_grads_bf16_out);
+    if (in0 < out0 + 2 * N && out0 < in0 + 4 * N) return PHX_ERR_INVALID_ARG;  // the two arrays must not overlap
+    int nl = 0;
+    PHX_CK(phx::launch_grads_finalize(d_main_grads_fp32, scale, d_grads_bf16_out, N,
+                                      reinterpret_cast<double *>(s->d_scratch + kScrPartials), d_sumsq_out,
+                                      static_cast<cudaStream_t>(stream), &nl));
+    s->launches += nl;
+    return PHX_OK;
+}
+
+// ---- derived scalars, exposed for the tests that pin them to the oracle ------------------------------
+int phx_derived_scalars_host(float lr, float beta1, float beta2, float wd, uint64_t step, float out[5])
+{
+    if (!out || step == 0) return PHX_ERR_INVALID_ARG;
+    phx::AdamScalars sc;
+    derive_scalars_host(lr, beta1, beta2, 0.0f, wd, step, &sc);
+    out[0] = sc.decay, out[1] = sc.omb1, out[2] = sc.omb2, out[3] = sc.ss, out[4] = sc.sbc2;
+    return PHX_OK;
+}
+
+int phx_derived_scalars_device(float lr, float beta1, float beta2, float wd, const uint64_t *steps, uint32_t n, float *out)
+{
+    if ((!steps || !out) && n) return PHX_ERR_INVALID_ARG;
+    if (n == 0) return PHX_OK;
+    uint64_t *d_steps = nullptr;
+    float *d_out = nullptr;
+    int rc = PHX_OK;
+    if (cudaMalloc(reinterpret_cast<void **>(&d_steps), (size_t)n * 8) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void **>(&d_out), (size_t)n * 20) != cudaSuccess)
+        rc = PHX_ERR_NOMEM;
+    if (rc == PHX_OK &&
+        (cudaMemcpy(d_steps, steps, (size_t)n * 8, cudaMemcpyHostToDevice) != cudaSuccess ||
+         phx::launch_derive_scalars(lr, beta1, beta2, wd, d_steps, n, d_out, nullptr) != cudaSuccess ||
+         cudaMemcpy(out, d_out, (size_t)n * 20, cudaMemcpyDeviceToHost) != cudaSuccess))
+        rc = PHX_ERR_CUDA;
+    if (rc != PHX_OK) (void)cudaGetLastError();
+    cudaFree(d_steps);
+    cudaFree(d_out);
+    return rc;
+}
+
+// ---- the graph-capturable form (include/phx.h "graph") -----------------------------------------------
+namespace {
+phx::StepBlock *step_block(phx_shard *s) { return reinterpret_cast<phx::StepBlock *>(s->d_scratch + kScrBlock); }
+}  // namespace
+
+int phx_graph_begin(phx_shard_t *s, float lr, float beta1, float beta2, float eps, float wd, void *stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (s->graph) return PHX_ERR_GRAPH_MODE;
+    if (full_payload(s)) return PHX_ERR_INVALID_ARG;  // the params_ready protocol of §8(f4) is eager-only
+    // a mode switch, not a hot call: every eager flush of this handle lands before the first captured / replayed
+    // step may touch what it reads
+    int rc = settle_host_slots(s, true);
+    if (rc != PHX_OK) return rc;
+    rc = settle_peer_slots(s, true);
+    if (rc != PHX_OK) return rc;
+    phx_snapshot_header_t tmpl;
+    build_header(s, 0, true, &tmpl);
+    phx::HeaderBlob blob;
+    std::memcpy(&blob, &tmpl, sizeof(blob));
+    PHX_CK(phx::launch_step_block_init(step_block(s), lr, beta1, beta2, eps, wd, s->last_step, blob,
+                                       static_cast<cudaStream_t>(stream)));
+    s->launches += 1;
+    s->graph = true;
+    s->g_issue = s->last_step;
+    s->g_pending_slot = s->pending_slot;   // an eager step's un-flushed snapshot becomes the graph's first flush
+    s->g_pending_step = s->pending_step;
+    s->g_last_flush_slot = -1;
+    for (int k = 0; k < kMaxDepth; ++k) s->gev_step[k].valid = s->gev_flush[k].valid = false;
+    return PHX_OK;
+}
+
+int phx_graph_set_hyper(phx_shard_t *s, float lr, float beta1, float beta2, float eps, float wd, void *stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!s->graph) return PHX_ERR_GRAPH_MODE;
+    // five floats at the front of the block's hyperparameter area, stream-ordered; the step counter stays
+    const float h[5] = {lr, beta1, beta2, eps, wd};
+    PHX_CK(cudaMemcpyAsync(reinterpret_cast<uint8_t *>(step_block(s)) + offsetof(phx::StepBlock, lr), h, sizeof(h),
+                           cudaMemcpyHostToDevice, static_cast<cudaStream_t>(stream)));
+    return PHX_OK;
+}
+
+int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *stream)
+{
+    if (!s || !d_grads) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!s->graph) return PHX_ERR_GRAPH_MODE;
+    if (!aligned256(d_grads)) return PHX_ERR_ALIGNMENT;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const bool snap = snapshots_on(s);
+    const uint64_t step = s->g_issue + 1;  // issue order; on a replay the device counter is the truth
+
+    phx::StepArgs a;
+    std::memset(&a, 0, sizeof(a));
+    int rc = enqueue_clip(s, d_grads, a, st);
+    if (rc != PHX_OK) return rc;
+    int slot = -1;
+    const uint32_t depth = ring_depth(s);
+    if (snap) {
+        slot = (int)(step % depth);
+        // a2, the single sync point: a dependency edge inside a captured graph, a stream wait outside
+        if (s->cfg.sync_mode == PHX_SYNC_STRICT) {
+            if (s->g_last_flush_slot >= 0 && (rc = gev_wait(s, s->gev_flush[s->g_last_flush_slot], st)) != PHX_OK) return rc;
+        } else if ((rc = gev_wait(s, s->gev_flush[slot], st)) != PHX_OK) {
+            return rc;
+        }
+        if (s->g_pending_slot >= 0 && s->h_replica) s->dropped_host += 1;
+    }
+    fill_common_args(s, d_grads, slot, a);
+    void *shdr = a.shdr;
+    a.shdr = nullptr;  // the prologue writes the envelope; the fused kernel only moves elements
+    a.dsc = &step_block(s)->sc;
+    PHX_CK(phx::launch_step_prologue(step_block(s), shdr, nullptr, 0u, snap ? (uint32_t)slot : 0u, snap ? depth : 0u, st));
+    PHX_CK(phx::launch_step(a, snap && !direct_mode(s), step_mode(s), true, st));
+    s->launches += 1 + (s->info.n_padded ? 1 : 0);
+    if (snap) {
+        if ((rc = gev_record(s, s->gev_step[slot], st)) != PHX_OK) return rc;
+        s->g_pending_slot = slot;
+        s->g_pending_step = step;
+    }
+    s->g_issue = step;
+    return PHX_OK;
+}
+
+int phx_graph_flush_async(phx_shard_t *s, void *side_stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound || (snapshots_on(s) && !s->h_replica)) return PHX_ERR_NOT_BOUND;
+    if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
+    if (!s->graph) return PHX_ERR_GRAPH_MODE;
+    if (s->g_pending_slot < 0) return PHX_ERR_NO_FLUSH_PENDING;
+    cudaStream_t st = static_cast<cudaStream_t>(side_stream);
+    const int slot = s->g_pending_slot;
+    const int hs = (int)(s->g_pending_step & 1);  // ping-pong; kept on a replay by the alignment rule
+    uint8_t *dst = s->h_replica + (uint64_t)hs * s->info.host_slot_stride;
+    int rc;
+    if ((rc = gev_wait(s, s->gev_step[slot], st)) != PHX_OK) return rc;  // the step's kernel has written the slot
+    if (s->g_last_flush_slot >= 0 && (rc = gev_wait(s, s->gev_flush[s->g_last_flush_slot], st)) != PHX_OK) return rc;
+    rc = enqueue_snapshot_copy(s, st, dst, cudaMemcpyDeviceToHost, slot, -1, false);
+    if (rc != PHX_OK) return rc;
+    if ((rc = gev_record(s, s->gev_flush[slot], st)) != PHX_OK) return rc;
+    s->g_last_flush_slot = slot;
+    s->g_pending_slot = -1;
+    return PHX_OK;
+}
+
+int phx_graph_end(phx_shard_t *s, uint64_t *last_step)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!s->graph) return PHX_ERR_GRAPH_MODE;
+    PHX_CK(cudaDeviceSynchronize());  // mode switch: every replay and every flush has finished
+    phx::StepBlock blk;
+    PHX_CK(cudaMemcpy(&blk, step_block(s), sizeof(blk), cudaMemcpyDeviceToHost));
+    s->graph = false;
+    s->last_step = blk.step;
+    // the eager bookkeeping restarts from what is self-describing: the envelopes in the host slots
+    for (int k = 0; k < kMaxDepth; ++k) s->flush_valid[k] = s->pflush_valid[k] = false;
+    s->last_flush_slot = s->last_pflush_slot = -1;
+    s->pending_slot = s->pending_peer_slot = -1;
+    uint64_t newest = 0;
+    for (int i = 0; i < 2 && s->h_replica; ++i) {
+        phx_snapshot_header_t h;
+        std::memcpy(&h, s->h_replica + (uint64_t)i * s->info.host_slot_stride, sizeof(h));
+        const bool ok = header_valid(&h) && header_matches(s, &h) && h.payload == 0u;
+        s->host[i].state = ok ? SLOT_COMMITTED : SLOT_EMPTY;
+        s->host[i].step = ok ? h.step : 0;
+        if (ok) s->host[i].hdr = h;
+        if (ok && h.step > newest) newest = h.step;
+    }
+    if (snapshots_on(s) && s->last_step > 0 && newest != s->last_step) {  // the newest step's snapshot is still staged
+        s->pending_slot = s->pending_peer_slot = (int)(s->last_step % ring_depth(s));
+        s->pending_step = s->pending_peer_step = s->last_step;
+    }
+    if (last_step) *last_step = s->last_step;
+    return blk.misaligned ? PHX_ERR_STEP_ORDER : PHX_OK;
 }
 
 }  // extern "C"

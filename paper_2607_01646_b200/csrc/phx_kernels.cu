@@ -1,17 +1,26 @@
 // phx_kernels.cu — hand-written sm_100a kernels of the phx hot path.
 //
-//   k_step8 / k_step4 : a3, fused AdamW step + bf16 copy + packed snapshot (include/phx.h).
+//   k_step8           : a3, fused AdamW step + bf16 copy + packed snapshot (include/phx.h).
 //                       Pure HBM streaming: 14 B/element read, 26 B/element written, one pass,
-//                       256-bit (LDG.E.256 / STG.E.256, new on sm_100) or 128-bit vectors,
-//                       streaming cache hints, no shared memory, no tensor cores (no contraction).
-//                       k_step8 MODE bits: kModeF32 = binary32 gradients and no bf16
+//                       256-bit vectors (LDG.E.256 / STG.E.256, new on sm_100), streaming cache
+//                       hints, no shared memory, no tensor cores (no contraction).
+//                       MODE bits: kModeF32 = binary32 gradients and no bf16
 //                       copy (the paper's precision; 16 B read + 24 B written);
-//                       kModeGroups = per-tensor decay groups (no-decay tensors take decay 1.0f).
+//                       kModeGroups = per-tensor decay groups; kModePublish = the model-param copy also
+//                       goes to the peers' parameter buffers (P2P stores, the fused all-gather).
+//                       DEV: the derived scalars come from the device-resident step block (graph-capturable form).
+//   k_step_prologue   : graph-capturable form: advances the device step counter, derives the AdamW scalars in
+//                       binary64 with individually rounded operations and writes the envelope(s).
 //   k_sumsq_*         : a1, deterministic fp64 sum of squares + clip coefficient.
+//   k_grads_finalize  : SURVEY §8(f4) second half: the gradient producer's epilogue — fp32 main gradients
+//                       x scale -> RNE bf16 gradients AND the fp64 sum of squares of the rounded values, one pass.
 //   k_regen_bf16      : p16 = RNE_bf16(p).
 //   k_restore_bulk    : a6, pulls the replica from mapped pinned host memory with 1-D bulk
 //                       async copies (TMA, cp.async.bulk + mbarrier) into shared memory, writes
 //                       p, m, v back with bulk stores and regenerates the bf16 copy.
+//
+// The other flavours tried in round 1 (128-bit vectors, two/four groups per thread, .cs hints, a TMA tile
+// pipeline: 5.8-6.4 TB/s against 6.65 for this one) are recorded in profiles/r01_step8_c2_full.md.
 //
 // Arithmetic contract (include/phx.h a3): every fp32 operation individually rounded —
 // __fmul_rn/__fadd_rn/__fsub_rn never fuse into FMA, __fdiv_rn/__fsqrt_rn are IEEE — and the
@@ -23,16 +32,13 @@
 namespace phx {
 
 // ------------------------------------------------------------------------------------------
-// vector memory helpers.  HINT: 0 plain, 1 L1::no_allocate (+L2::evict_first on loads),
-// 2 .cs (cache-streaming) both ways, 3 like 1 with L2::evict_first on stores as well.
+// vector memory helpers.  Streaming hints: loads never allocate in L1 and are marked evict-first in
+// L2, stores never allocate in L1 (measured best of the hint combinations, profiles/r01_step8_c2_full.md).
 // p/m/v are read then overwritten by the same thread, so the non-coherent (.nc) path is used
 // only for the gradients.
 // ------------------------------------------------------------------------------------------
 struct F8 {
     float x[8];
-};
-struct F4 {
-    float x[4];
 };
 
 #define PHX_LD256(QUAL)                                                                              \
@@ -40,53 +46,18 @@ struct F4 {
                  : "=f"(r.x[0]), "=f"(r.x[1]), "=f"(r.x[2]), "=f"(r.x[3]), "=f"(r.x[4]), "=f"(r.x[5]), \
                    "=f"(r.x[6]), "=f"(r.x[7])                                                         \
                  : "l"(ptr))
-#define PHX_ST256(QUAL)                                                                              \
-    asm volatile("st.global" QUAL ".v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(ptr), "f"(r.x[0]), \
-                 "f"(r.x[1]), "f"(r.x[2]), "f"(r.x[3]), "f"(r.x[4]), "f"(r.x[5]), "f"(r.x[6]),        \
-                 "f"(r.x[7])                                                                          \
-                 : "memory")
-#define PHX_LD128F(QUAL)                                                   \
-    asm volatile("ld.global" QUAL ".v4.f32 {%0,%1,%2,%3}, [%4];"            \
-                 : "=f"(r.x[0]), "=f"(r.x[1]), "=f"(r.x[2]), "=f"(r.x[3])   \
-                 : "l"(ptr))
-#define PHX_ST128F(QUAL)                                                                          \
-    asm volatile("st.global" QUAL ".v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(ptr), "f"(r.x[0]), "f"(r.x[1]), \
-                 "f"(r.x[2]), "f"(r.x[3])                                                          \
-                 : "memory")
 
-template <int HINT>
 __device__ __forceinline__ F8 ld256(const float *ptr)
 {
     F8 r;
-    if (HINT == 0) PHX_LD256("");
-    else if (HINT == 2) PHX_LD256(".cs");
-    else PHX_LD256(".L1::no_allocate.L2::evict_first");
+    PHX_LD256(".L1::no_allocate.L2::evict_first");
     return r;
 }
-template <int HINT>
 __device__ __forceinline__ void st256(float *ptr, const F8 &r)
 {
-    if (HINT == 0) PHX_ST256("");
-    else if (HINT == 2) PHX_ST256(".cs");
-    else if (HINT == 3) PHX_ST256(".L1::no_allocate.L2::evict_first");
-    else PHX_ST256(".L1::no_allocate");
-}
-template <int HINT>
-__device__ __forceinline__ F4 ld128f(const float *ptr)
-{
-    F4 r;
-    if (HINT == 0) PHX_LD128F("");
-    else if (HINT == 2) PHX_LD128F(".cs");
-    else PHX_LD128F(".L1::no_allocate");  // ptxas: L2::evict_first needs a 256-bit type
-    return r;
-}
-template <int HINT>
-__device__ __forceinline__ void st128f(float *ptr, const F4 &r)
-{
-    if (HINT == 0) PHX_ST128F("");
-    else if (HINT == 2) PHX_ST128F(".cs");
-    else if (HINT == 3) PHX_ST128F(".L1::no_allocate.L2::evict_first");
-    else PHX_ST128F(".L1::no_allocate");
+    asm volatile("st.global.L1::no_allocate.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(ptr), "f"(r.x[0]),
+                 "f"(r.x[1]), "f"(r.x[2]), "f"(r.x[3]), "f"(r.x[4]), "f"(r.x[5]), "f"(r.x[6]), "f"(r.x[7])
+                 : "memory");
 }
 // gradients: read-only for the whole kernel -> non-coherent path, never allocate in L1
 __device__ __forceinline__ uint4 ldg128_stream(const void *ptr)
@@ -103,33 +74,9 @@ __device__ __forceinline__ F8 ldg256_stream(const float *ptr)
     PHX_LD256(".nc.L1::no_allocate.L2::evict_first");
     return r;
 }
-__device__ __forceinline__ uint2 ldg64_stream(const void *ptr)
-{
-    uint2 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];"
-                 : "=r"(r.x), "=r"(r.y)
-                 : "l"(ptr));
-    return r;
-}
-template <int HINT>
 __device__ __forceinline__ void st128u(void *ptr, const uint4 &r)
 {
-    if (HINT == 0)
-        asm volatile("st.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(ptr), "r"(r.x), "r"(r.y), "r"(r.z), "r"(r.w) : "memory");
-    else if (HINT == 2)
-        asm volatile("st.global.cs.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(ptr), "r"(r.x), "r"(r.y), "r"(r.z), "r"(r.w) : "memory");
-    else
-        asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(ptr), "r"(r.x), "r"(r.y), "r"(r.z), "r"(r.w) : "memory");
-}
-template <int HINT>
-__device__ __forceinline__ void st64u(void *ptr, const uint2 &r)
-{
-    if (HINT == 0)
-        asm volatile("st.global.v2.u32 [%0], {%1,%2};" ::"l"(ptr), "r"(r.x), "r"(r.y) : "memory");
-    else if (HINT == 2)
-        asm volatile("st.global.cs.v2.u32 [%0], {%1,%2};" ::"l"(ptr), "r"(r.x), "r"(r.y) : "memory");
-    else
-        asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};" ::"l"(ptr), "r"(r.x), "r"(r.y) : "memory");
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(ptr), "r"(r.x), "r"(r.y), "r"(r.z), "r"(r.w) : "memory");
 }
 
 // ------------------------------------------------------------------------------------------
@@ -161,7 +108,7 @@ __device__ __forceinline__ void adamw_element(float &p, float &m, float &v, floa
 }
 
 // ------------------------------------------------------------------------------------------
-// 1-D bulk async copy (TMA) + mbarrier helpers (shared by the TMA step kernel and the restore kernel)
+// 1-D bulk async copy (TMA) + mbarrier helpers (the restore kernel)
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
@@ -204,10 +151,6 @@ __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.comm
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-__device__ __forceinline__ void bulk_wait_read1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
-// make this thread's generic-proxy shared-memory writes visible to the async proxy (bulk stores)
-__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
 // ------------------------------------------------------------------------------------------
 // a3: fused step + snapshot, 8 elements per thread-group, 256-bit vectors
 // ------------------------------------------------------------------------------------------
@@ -245,323 +188,230 @@ __device__ __forceinline__ void store_headers(const StepArgs &a)
     }
 }
 
-template <int HINT, int U, bool SNAP, int MODE>
+template <bool SNAP, int MODE, bool DEV>
 __global__ void __launch_bounds__(kStepThreads) k_step8(const __grid_constant__ StepArgs a)
 {
     constexpr bool GF32 = (MODE & kModeF32) != 0, GROUPS = (MODE & kModeGroups) != 0, PUB = (MODE & kModePublish) != 0;
-    const uint64_t ngroups = a.n_padded >> 3;
-    const uint64_t base = (uint64_t)blockIdx.x * (kStepThreads * U) + threadIdx.x;
-    store_headers(a);
+    const uint64_t gi = (uint64_t)blockIdx.x * kStepThreads + threadIdx.x;
+    AdamScalars sc;
+    if (DEV) {  // graph-capturable form: k_step_prologue left the scalars (and the envelopes) in device memory
+        const float4 s0 = __ldg(reinterpret_cast<const float4 *>(a.dsc));
+        const float4 s1 = __ldg(reinterpret_cast<const float4 *>(a.dsc) + 1);
+        sc.beta1 = s0.x, sc.beta2 = s0.y, sc.eps = s0.z, sc.decay = s0.w;
+        sc.omb1 = s1.x, sc.omb2 = s1.y, sc.ss = s1.z, sc.sbc2 = s1.w;
+    } else {
+        sc = a.sc;
+        store_headers(a);
+    }
+    if (gi >= (a.n_padded >> 3)) return;
     const float coef = __ldg(a.coef);
+    const uint64_t e = gi << 3;
 
-    F8 P[U], M[U], V[U];
-    uint4 G[U];
-    F8 GF[GF32 ? U : 1];
+    uint4 G;
+    F8 GF;
+    if (GF32) GF = ldg256_stream(reinterpret_cast<const float *>(a.g) + e);
+    else G = ldg128_stream(reinterpret_cast<const uint16_t *>(a.g) + e);
+    F8 P = ld256(a.p + e);
+    F8 M = ld256(a.m + e);
+    F8 V = ld256(a.v + e);
+
+    float gv[8];
+    if (GF32) {
 #pragma unroll
-    for (int u = 0; u < U; ++u) {
-        const uint64_t gi = base + (uint64_t)u * kStepThreads;
-        if (gi < ngroups) {
-            const uint64_t e = gi << 3;
-            if (GF32) GF[GF32 ? u : 0] = ldg256_stream(reinterpret_cast<const float *>(a.g) + e);
-            else G[u] = ldg128_stream(reinterpret_cast<const uint16_t *>(a.g) + e);
-            P[u] = ld256<HINT>(a.p + e);
-            M[u] = ld256<HINT>(a.m + e);
-            V[u] = ld256<HINT>(a.v + e);
+        for (int j = 0; j < 8; ++j) gv[j] = GF.x[j];
+    } else {
+        const uint32_t gw[4] = {G.x, G.y, G.z, G.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            gv[2 * j] = bf16lo(gw[j]);
+            gv[2 * j + 1] = bf16hi(gw[j]);
         }
     }
+    uint32_t cls = 0;
+    if (GROUPS) cls = __ldg(a.decay_cls + (e >> kDecayTileShift));
+    if (!GROUPS || cls != 2) {
+        const float decay = (GROUPS && cls == 1) ? 1.0f : sc.decay;
 #pragma unroll
-    for (int u = 0; u < U; ++u) {
-        const uint64_t gi = base + (uint64_t)u * kStepThreads;
-        if (gi < ngroups) {
-            const uint64_t e = gi << 3;
-            float gv[8];
-            if (GF32) {
+        for (int j = 0; j < 8; ++j) adamw_element(P.x[j], M.x[j], V.x[j], gv[j], coef, sc, decay);
+    } else {
 #pragma unroll
-                for (int j = 0; j < 8; ++j) gv[j] = GF[GF32 ? u : 0].x[j];
-            } else {
-                const uint32_t gw[4] = {G[u].x, G[u].y, G[u].z, G[u].w};
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    gv[2 * j] = bf16lo(gw[j]);
-                    gv[2 * j + 1] = bf16hi(gw[j]);
-                }
-            }
-            uint32_t cls = 0;
-            if (GROUPS) cls = __ldg(a.decay_cls + (e >> kDecayTileShift));
-            if (!GROUPS || cls != 2) {
-                const float decay = (GROUPS && cls == 1) ? 1.0f : a.sc.decay;
-#pragma unroll
-                for (int j = 0; j < 8; ++j) adamw_element(P[u].x[j], M[u].x[j], V[u].x[j], gv[j], coef, a.sc, decay);
-            } else {
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const float decay = nodecay_at(e + j, a.decay_bnd, a.n_bnd, a.first_nodecay) ? 1.0f : a.sc.decay;
-                    adamw_element(P[u].x[j], M[u].x[j], V[u].x[j], gv[j], coef, a.sc, decay);
-                }
-            }
-            st256<HINT>(a.p + e, P[u]);
-            st256<HINT>(a.m + e, M[u]);
-            st256<HINT>(a.v + e, V[u]);
-            if (!GF32) {
-                uint4 h;
-                h.x = pack_bf16x2(P[u].x[0], P[u].x[1]);
-                h.y = pack_bf16x2(P[u].x[2], P[u].x[3]);
-                h.z = pack_bf16x2(P[u].x[4], P[u].x[5]);
-                h.w = pack_bf16x2(P[u].x[6], P[u].x[7]);
-                st128u<HINT>(reinterpret_cast<uint16_t *>(a.p16) + e, h);
-                if (PUB)  // all-gather fused into the step: the same 16 bytes go to every peer's buffer (P2P stores)
-                    for (uint32_t q = 0; q < a.n_pub; ++q) st128u<HINT>(reinterpret_cast<uint16_t *>(a.pub[q]) + e, h);
-            } else if (PUB) {
-                for (uint32_t q = 0; q < a.n_pub; ++q) st256<HINT>(reinterpret_cast<float *>(a.pub[q]) + e, P[u]);
-            }
-            if (SNAP) {
-                st256<HINT>(a.sp + e, P[u]);
-                st256<HINT>(a.sm + e, M[u]);
-                st256<HINT>(a.sv + e, V[u]);
-            }
+        for (int j = 0; j < 8; ++j) {
+            const float decay = nodecay_at(e + j, a.decay_bnd, a.n_bnd, a.first_nodecay) ? 1.0f : sc.decay;
+            adamw_element(P.x[j], M.x[j], V.x[j], gv[j], coef, sc, decay);
         }
+    }
+    st256(a.p + e, P);
+    st256(a.m + e, M);
+    st256(a.v + e, V);
+    if (!GF32) {
+        uint4 h;
+        h.x = pack_bf16x2(P.x[0], P.x[1]);
+        h.y = pack_bf16x2(P.x[2], P.x[3]);
+        h.z = pack_bf16x2(P.x[4], P.x[5]);
+        h.w = pack_bf16x2(P.x[6], P.x[7]);
+        st128u(reinterpret_cast<uint16_t *>(a.p16) + e, h);
+        if (PUB)  // all-gather fused into the step: the same 16 bytes go to every peer's buffer (P2P stores)
+            for (uint32_t q = 0; q < a.n_pub; ++q) st128u(reinterpret_cast<uint16_t *>(a.pub[q]) + e, h);
+    } else if (PUB) {
+        for (uint32_t q = 0; q < a.n_pub; ++q) st256(reinterpret_cast<float *>(a.pub[q]) + e, P);
+    }
+    if (SNAP) {
+        st256(a.sp + e, P);
+        st256(a.sm + e, M);
+        st256(a.sv + e, V);
     }
 }
 
-// 128-bit flavour: 4 elements per thread-group (classic float4 streaming)
-template <int HINT, int U, bool SNAP>
-__global__ void __launch_bounds__(kStepThreads) k_step4(const __grid_constant__ StepArgs a)
-{
-    const uint64_t ngroups = a.n_padded >> 2;
-    const uint64_t base = (uint64_t)blockIdx.x * (kStepThreads * U) + threadIdx.x;
-    store_headers(a);
-    const float coef = __ldg(a.coef);
-
-    F4 P[U], M[U], V[U];
-    uint2 G[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-        const uint64_t gi = base + (uint64_t)u * kStepThreads;
-        if (gi < ngroups) {
-            const uint64_t e = gi << 2;
-            G[u] = ldg64_stream(reinterpret_cast<const uint16_t *>(a.g) + e);
-            P[u] = ld128f<HINT>(a.p + e);
-            M[u] = ld128f<HINT>(a.m + e);
-            V[u] = ld128f<HINT>(a.v + e);
-        }
-    }
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-        const uint64_t gi = base + (uint64_t)u * kStepThreads;
-        if (gi < ngroups) {
-            const uint64_t e = gi << 2;
-            const uint32_t gw[2] = {G[u].x, G[u].y};
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                adamw_element(P[u].x[2 * j], M[u].x[2 * j], V[u].x[2 * j], bf16lo(gw[j]), coef, a.sc, a.sc.decay);
-                adamw_element(P[u].x[2 * j + 1], M[u].x[2 * j + 1], V[u].x[2 * j + 1], bf16hi(gw[j]), coef, a.sc, a.sc.decay);
-            }
-            uint2 h;
-            h.x = pack_bf16x2(P[u].x[0], P[u].x[1]);
-            h.y = pack_bf16x2(P[u].x[2], P[u].x[3]);
-            st128f<HINT>(a.p + e, P[u]);
-            st128f<HINT>(a.m + e, M[u]);
-            st128f<HINT>(a.v + e, V[u]);
-            st64u<HINT>(reinterpret_cast<uint16_t *>(a.p16) + e, h);
-            if (SNAP) {
-                st128f<HINT>(a.sp + e, P[u]);
-                st128f<HINT>(a.sm + e, M[u]);
-                st128f<HINT>(a.sv + e, V[u]);
-            }
-        }
-    }
-}
-
-template <int HINT, int U, int MODE = 0>
+template <int MODE, bool DEV>
 static cudaError_t launch8(const StepArgs &a, bool snapshot, cudaStream_t st)
 {
     const uint64_t ngroups = a.n_padded >> 3;
-    const uint64_t per_block = (uint64_t)kStepThreads * U;
-    const unsigned grid = (unsigned)((ngroups + per_block - 1) / per_block);
+    const unsigned grid = (unsigned)((ngroups + kStepThreads - 1) / kStepThreads);
     if (grid == 0) return cudaSuccess;
-    if (snapshot) k_step8<HINT, U, true, MODE><<<grid, kStepThreads, 0, st>>>(a);
-    else k_step8<HINT, U, false, MODE><<<grid, kStepThreads, 0, st>>>(a);
-    return cudaGetLastError();
-}
-template <int HINT, int U>
-static cudaError_t launch4(const StepArgs &a, bool snapshot, cudaStream_t st)
-{
-    const uint64_t ngroups = a.n_padded >> 2;
-    const uint64_t per_block = (uint64_t)kStepThreads * U;
-    const unsigned grid = (unsigned)((ngroups + per_block - 1) / per_block);
-    if (grid == 0) return cudaSuccess;
-    if (snapshot) k_step4<HINT, U, true><<<grid, kStepThreads, 0, st>>>(a);
-    else k_step4<HINT, U, false><<<grid, kStepThreads, 0, st>>>(a);
+    if (snapshot) k_step8<true, MODE, DEV><<<grid, kStepThreads, 0, st>>>(a);
+    else k_step8<false, MODE, DEV><<<grid, kStepThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 
-
-// ------------------------------------------------------------------------------------------
-// a3, TMA flavour: persistent CTAs, STAGES shared-memory stages of one TT-element tile each.
-//   producer (thread 0): cp.async.bulk loads of the p, m, v, g tiles, completion on an mbarrier;
-//   all threads: canonical AdamW in place in shared memory (conflict-free 128-bit accesses),
-//                bf16 copy into the stage's h tile;
-//   thread 0: cp.async.bulk stores of the SAME shared tiles to the live planes AND to the staging
-//             planes — the snapshot costs no extra SM instruction at all, only the extra bulk store.
-// ------------------------------------------------------------------------------------------
-template <int TT>
-struct alignas(128) StepTile {
-    float p[TT], m[TT], v[TT];
-    uint16_t g[TT], h[TT];
-};
-
-template <int TT, int STAGES, bool SNAP>
-__global__ void __launch_bounds__(kStepThreads) k_step_tma(const __grid_constant__ StepArgs a)
+// mode: bit set of kMode* (SURVEY §8(f2)/(f3)); dev: the derived scalars come from the device-resident step
+// block (a.dsc) instead of the kernel parameters (the graph-capturable form).
+cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t mode, bool dev, cudaStream_t st)
 {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    StepTile<TT> *tiles = reinterpret_cast<StepTile<TT> *>(smem_raw);
-    __shared__ __align__(8) uint64_t full[STAGES];
-    constexpr int kHalves = TT / (kStepThreads * 4);
-
-    const uint64_t N = a.n_padded;
-    const uint64_t ntiles = (N + TT - 1) / TT;
-    const uint64_t first = blockIdx.x, stride = gridDim.x;
-    const uint64_t my_count = first < ntiles ? (ntiles - first + stride - 1) / stride : 0;
-
-    store_headers(a);
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-    const float coef = __ldg(a.coef);
-    const uint16_t *g16 = reinterpret_cast<const uint16_t *>(a.g);
-    uint16_t *p16 = reinterpret_cast<uint16_t *>(a.p16);
-
-    auto tile_cnt = [&](uint64_t it) -> uint32_t {
-        const uint64_t e0 = (first + it * stride) * TT;
-        return (uint32_t)((N - e0) < (uint64_t)TT ? (N - e0) : TT);
-    };
-    auto issue_loads = [&](uint64_t it) {  // thread 0
-        const int s = (int)(it % STAGES);
-        const uint64_t e0 = (first + it * stride) * TT;
-        const uint32_t cnt = tile_cnt(it);
-        StepTile<TT> &t = tiles[s];
-        mbar_expect_tx(&full[s], cnt * 14u);
-        bulk_g2s(t.p, a.p + e0, cnt * 4u, &full[s]);
-        bulk_g2s(t.m, a.m + e0, cnt * 4u, &full[s]);
-        bulk_g2s(t.v, a.v + e0, cnt * 4u, &full[s]);
-        bulk_g2s(t.g, g16 + e0, cnt * 2u, &full[s]);
-    };
-
-    if (threadIdx.x == 0)
-        for (uint64_t it = 0; it < my_count && it < (uint64_t)STAGES; ++it) issue_loads(it);
-
-    for (uint64_t it = 0; it < my_count; ++it) {
-        const int s = (int)(it % STAGES);
-        const uint32_t parity = (uint32_t)((it / STAGES) & 1);
-        const uint64_t e0 = (first + it * stride) * TT;
-        const uint32_t cnt = tile_cnt(it);
-        StepTile<TT> &t = tiles[s];
-        mbar_wait(&full[s], parity);
-#pragma unroll
-        for (int hf = 0; hf < kHalves; ++hf) {
-            const uint32_t e = hf * (kStepThreads * 4) + threadIdx.x * 4;
-            if (e < cnt) {
-                float4 P = *reinterpret_cast<float4 *>(t.p + e);
-                float4 M = *reinterpret_cast<float4 *>(t.m + e);
-                float4 V = *reinterpret_cast<float4 *>(t.v + e);
-                const uint2 G = *reinterpret_cast<const uint2 *>(t.g + e);
-                adamw_element(P.x, M.x, V.x, bf16lo(G.x), coef, a.sc, a.sc.decay);
-                adamw_element(P.y, M.y, V.y, bf16hi(G.x), coef, a.sc, a.sc.decay);
-                adamw_element(P.z, M.z, V.z, bf16lo(G.y), coef, a.sc, a.sc.decay);
-                adamw_element(P.w, M.w, V.w, bf16hi(G.y), coef, a.sc, a.sc.decay);
-                *reinterpret_cast<float4 *>(t.p + e) = P;
-                *reinterpret_cast<float4 *>(t.m + e) = M;
-                *reinterpret_cast<float4 *>(t.v + e) = V;
-                uint2 H;
-                H.x = pack_bf16x2(P.x, P.y);
-                H.y = pack_bf16x2(P.z, P.w);
-                *reinterpret_cast<uint2 *>(t.h + e) = H;
-            }
-        }
-        fence_proxy_async_smem();
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            bulk_s2g(a.p + e0, t.p, cnt * 4u);
-            bulk_s2g(a.m + e0, t.m, cnt * 4u);
-            bulk_s2g(a.v + e0, t.v, cnt * 4u);
-            bulk_s2g(p16 + e0, t.h, cnt * 2u);
-            if (SNAP) {
-                bulk_s2g(a.sp + e0, t.p, cnt * 4u);
-                bulk_s2g(a.sm + e0, t.m, cnt * 4u);
-                bulk_s2g(a.sv + e0, t.v, cnt * 4u);
-            }
-            bulk_commit();
-            // refill the stage used one iteration ago: its stores must have finished READING smem
-            if (it >= 1 && it - 1 + STAGES < my_count) {
-                bulk_wait_read1();
-                issue_loads(it - 1 + STAGES);
-            }
-        }
-    }
-    if (threadIdx.x == 0) bulk_wait_all0();
-}
-
-template <int TT, int STAGES>
-static cudaError_t launch_tma(const StepArgs &a, bool snapshot, cudaStream_t st)
-{
-    if (a.n_padded == 0) return cudaSuccess;
-    const size_t smem = sizeof(StepTile<TT>) * STAGES;
-    static int sm_count = 0;
-    static int ctas_per_sm = 0;
-    if (sm_count == 0) {
-        int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e != cudaSuccess) return e;
-        e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(k_step_tma<TT, STAGES, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(k_step_tma<TT, STAGES, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        ctas_per_sm = (int)((227u * 1024u) / (smem + 1024));
-        if (ctas_per_sm < 1) ctas_per_sm = 1;
-        if (ctas_per_sm > 8) ctas_per_sm = 8;
-    }
-    const uint64_t ntiles = (a.n_padded + TT - 1) / TT;
-    uint64_t grid = (uint64_t)sm_count * ctas_per_sm;
-    if (grid > ntiles) grid = ntiles;
-    if (snapshot) k_step_tma<TT, STAGES, true><<<(unsigned)grid, kStepThreads, smem, st>>>(a);
-    else k_step_tma<TT, STAGES, false><<<(unsigned)grid, kStepThreads, smem, st>>>(a);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, uint32_t mode, cudaStream_t st)
-{
-    if (mode != 0) {  // §8(f2)/(f3) modes (bit set of kMode*) exist for the default flavour only
-        if (variant != 0) return cudaErrorInvalidValue;
-        switch (mode) {
-        case 1: return launch8<1, 1, 1>(a, snapshot, st);
-        case 2: return launch8<1, 1, 2>(a, snapshot, st);
-        case 3: return launch8<1, 1, 3>(a, snapshot, st);
-        case 4: return launch8<1, 1, 4>(a, snapshot, st);
-        case 5: return launch8<1, 1, 5>(a, snapshot, st);
-        case 6: return launch8<1, 1, 6>(a, snapshot, st);
-        case 7: return launch8<1, 1, 7>(a, snapshot, st);
-        default: return cudaErrorInvalidValue;
-        }
-    }
-    switch (variant) {
-    case 0: return launch8<1, 1>(a, snapshot, st);  // 256-bit, streaming hints (default)
-    case 1: return launch8<0, 1>(a, snapshot, st);  // 256-bit, no hints
-    case 2: return launch8<1, 2>(a, snapshot, st);  // 256-bit, two groups in flight per thread
-    case 3: return launch4<1, 2>(a, snapshot, st);  // 128-bit, two groups per thread
-    case 4: return launch8<2, 1>(a, snapshot, st);  // 256-bit, .cs both ways
-    case 5: return launch8<3, 1>(a, snapshot, st);  // 256-bit, evict_first on stores too
-    case 6: return launch4<1, 4>(a, snapshot, st);  // 128-bit, four groups per thread
-    case 7: return launch4<0, 2>(a, snapshot, st);  // 128-bit, no hints
-    case 8: return launch_tma<2048, 3>(a, snapshot, st);   // TMA pipeline, 32 KB stages x3, 2 CTAs/SM
-    case 9: return launch_tma<4096, 3>(a, snapshot, st);   // TMA pipeline, 64 KB stages x3, 1 CTA/SM
-    case 10: return launch_tma<1024, 4>(a, snapshot, st);  // TMA pipeline, 16 KB stages x4, 3 CTAs/SM
-    case 11: return launch_tma<2048, 2>(a, snapshot, st);  // TMA pipeline, 32 KB stages x2, 3 CTAs/SM
+#define PHX_MODE_CASE(M) \
+    case M: return dev ? launch8<M, true>(a, snapshot, st) : launch8<M, false>(a, snapshot, st)
+    switch (mode) {
+        PHX_MODE_CASE(0);
+        PHX_MODE_CASE(1);
+        PHX_MODE_CASE(2);
+        PHX_MODE_CASE(3);
+        PHX_MODE_CASE(4);
+        PHX_MODE_CASE(5);
+        PHX_MODE_CASE(6);
+        PHX_MODE_CASE(7);
     default: return cudaErrorInvalidValue;
     }
+#undef PHX_MODE_CASE
+}
+
+// ------------------------------------------------------------------------------------------
+// Graph-capturable form (include/phx.h "graph"): the per-step scalars and the envelope are DERIVED ON THE
+// DEVICE from a device-resident step counter, so that a captured step carries no per-step kernel parameter.
+// One thread.  Every binary64 operation is an individually rounded intrinsic (__dmul_rn, __dsub_rn,
+// __ddiv_rn, __dsqrt_rn) in the same order as the host code of phx_api.cu, so the fp32 results are the same
+// bits (tests/test_gpu_graph.py compares them with the oracle for t up to 10^6).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double pow_sqmul_dev(double b, uint64_t t)  // LSB-first square-and-multiply
+{
+    double r = 1.0;
+    while (t) {
+        if (t & 1) r = __dmul_rn(r, b);
+        b = __dmul_rn(b, b);
+        t >>= 1;
+    }
+    return r;
+}
+__device__ __forceinline__ void derive_scalars_dev(float lr, float beta1, float beta2, float eps, float wd, uint64_t t,
+                                                   AdamScalars *out)
+{
+    const double dlr = (double)lr, db1 = (double)beta1, db2 = (double)beta2, dwd = (double)wd;
+    out->beta1 = beta1;
+    out->beta2 = beta2;
+    out->eps = eps;
+    out->decay = __double2float_rn(__dsub_rn(1.0, __dmul_rn(dlr, dwd)));
+    out->omb1 = __double2float_rn(__dsub_rn(1.0, db1));
+    out->omb2 = __double2float_rn(__dsub_rn(1.0, db2));
+    out->ss = __double2float_rn(__ddiv_rn(dlr, __dsub_rn(1.0, pow_sqmul_dev(db1, t))));
+    out->sbc2 = __double2float_rn(__dsqrt_rn(__dsub_rn(1.0, pow_sqmul_dev(db2, t))));
+}
+__device__ __forceinline__ uint64_t fnv1a64_dev(const uint8_t *b, int len)
+{
+    uint64_t h = 0xCBF29CE484222325ull;
+    for (int i = 0; i < len; ++i) {
+        h ^= b[i];
+        h *= 0x100000001B3ull;
+    }
+    return h;
+}
+
+// blk->step += 1; scalars of that step -> blk->sc; envelope of that step (template + step + hash) -> shdr
+// and, §8(f4), the full-rank-state flavour -> shdr_full.  expect_slot/expect_depth: the staging slot the
+// host baked into the captured kernel node; a replay whose device step does not land on it is counted in
+// blk->misaligned (phx_graph_end reports it) instead of silently writing the wrong slot.
+__global__ void __launch_bounds__(32) k_step_prologue(StepBlock *blk, uint8_t *shdr, uint8_t *shdr_full,
+                                                      uint32_t full_payload, uint32_t expect_slot, uint32_t expect_depth)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const uint64_t t = blk->step + 1;
+    blk->step = t;
+    if (expect_depth != 0 && (uint32_t)(t % expect_depth) != expect_slot) blk->misaligned += 1;
+    derive_scalars_dev(blk->lr, blk->beta1, blk->beta2, blk->eps, blk->wd, t, &blk->sc);
+    if (shdr == nullptr && shdr_full == nullptr) return;
+    // envelope: the template's constant fields + seq_begin = step = seq_end = t + FNV-1a of bytes [0, 240)
+    uint8_t *h = blk->hdr_work;
+    for (int i = 0; i < 256; ++i) h[i] = blk->hdr_tmpl[i];
+    auto put64 = [&](int off, uint64_t v) {
+        for (int i = 0; i < 8; ++i) h[off + i] = (uint8_t)(v >> (8 * i));
+    };
+    auto put32 = [&](int off, uint32_t v) {
+        for (int i = 0; i < 4; ++i) h[off + i] = (uint8_t)(v >> (8 * i));
+    };
+    put64(16, t);   // seq_begin
+    put64(24, t);   // step
+    put64(248, t);  // seq_end: the slot commits when this header lands
+    if (shdr != nullptr) {
+        put32(108, 0u);
+        put64(240, fnv1a64_dev(h, 240));
+        for (int i = 0; i < 16; ++i) reinterpret_cast<uint4 *>(shdr)[i] = reinterpret_cast<const uint4 *>(h)[i];
+    }
+    if (shdr_full != nullptr) {
+        put32(108, full_payload);
+        put64(240, fnv1a64_dev(h, 240));
+        for (int i = 0; i < 16; ++i) reinterpret_cast<uint4 *>(shdr_full)[i] = reinterpret_cast<const uint4 *>(h)[i];
+    }
+}
+
+cudaError_t launch_step_prologue(StepBlock *blk, void *shdr, void *shdr_full, uint32_t full_payload, uint32_t expect_slot,
+                                 uint32_t expect_depth, cudaStream_t st)
+{
+    k_step_prologue<<<1, 32, 0, st>>>(blk, static_cast<uint8_t *>(shdr), static_cast<uint8_t *>(shdr_full), full_payload,
+                                      expect_slot, expect_depth);
+    return cudaGetLastError();
+}
+
+// (re)initialise the step block: hyperparameters, the step the live state stands at, the envelope template
+__global__ void __launch_bounds__(32) k_step_block_init(StepBlock *blk, float lr, float beta1, float beta2, float eps,
+                                                        float wd, uint64_t step, HeaderBlob tmpl)
+{
+    if (threadIdx.x < 16) reinterpret_cast<uint4 *>(blk->hdr_tmpl)[threadIdx.x] = tmpl.q[threadIdx.x];
+    if (threadIdx.x == 0) {
+        blk->lr = lr, blk->beta1 = beta1, blk->beta2 = beta2, blk->eps = eps, blk->wd = wd;
+        blk->step = step;
+        blk->misaligned = 0;
+    }
+}
+cudaError_t launch_step_block_init(StepBlock *blk, float lr, float beta1, float beta2, float eps, float wd, uint64_t step,
+                                   const HeaderBlob &tmpl, cudaStream_t st)
+{
+    k_step_block_init<<<1, 32, 0, st>>>(blk, lr, beta1, beta2, eps, wd, step, tmpl);
+    return cudaGetLastError();
+}
+
+// test hook (phx_derived_scalars_device): the device derivation for n step indices -> out[5*i] = {decay, omb1, omb2, ss, sbc2}
+__global__ void __launch_bounds__(128) k_derive_scalars(float lr, float beta1, float beta2, float wd,
+                                                        const uint64_t *__restrict__ steps, uint32_t n, float *__restrict__ out)
+{
+    const uint32_t i = blockIdx.x * 128 + threadIdx.x;
+    if (i >= n) return;
+    AdamScalars sc;
+    derive_scalars_dev(lr, beta1, beta2, 0.0f, wd, steps[i], &sc);
+    out[5 * i + 0] = sc.decay, out[5 * i + 1] = sc.omb1, out[5 * i + 2] = sc.omb2, out[5 * i + 3] = sc.ss, out[5 * i + 4] = sc.sbc2;
+}
+cudaError_t launch_derive_scalars(float lr, float beta1, float beta2, float wd, const uint64_t *d_steps, uint32_t n,
+                                  float *d_out, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    k_derive_scalars<<<(n + 127) / 128, 128, 0, st>>>(lr, beta1, beta2, wd, d_steps, n, d_out);
+    return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------------------------------
@@ -742,19 +592,77 @@ cudaError_t launch_clip_from_partials(const double *partials, uint32_t count, fl
 }
 
 // ------------------------------------------------------------------------------------------
+// SURVEY §8(f4), second half — the gradient producer's epilogue (reading R34): ONE pass that
+// reads the binary32 main gradients (the reduce-scatter output of the ZeRO-2 optimizer),
+// writes the optimizer's bf16 gradients  g16 = RNE_bf16(g32 * scale)  and leaves the fp64 per-block sums
+// of widen(g16)^2 — the squares of the ROUNDED values, i.e. exactly what a1 would compute from g16 — so
+// that the step needs no pass of its own over the gradients (phx_set_clip_partials, count = 1).
+// 4 B read + 2 B written per element; same fixed two-stage tree as a1 (deterministic run to run).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_grads_finalize(const float *__restrict__ g32, float scale, void *__restrict__ g16,
+                                                        uint64_t ngroups, double *__restrict__ partials)
+{
+    double acc = 0.0, acc1 = 0.0;
+    const uint64_t stride = (uint64_t)gridDim.x * 256;
+    uint64_t gi = (uint64_t)blockIdx.x * 256 + threadIdx.x;
+    auto one = [&](const F8 &f, uint64_t g) {
+        uint4 h;  // cvt.rn.bf16x2.f32 of the individually rounded products
+        h.x = pack_bf16x2(__fmul_rn(f.x[0], scale), __fmul_rn(f.x[1], scale));
+        h.y = pack_bf16x2(__fmul_rn(f.x[2], scale), __fmul_rn(f.x[3], scale));
+        h.z = pack_bf16x2(__fmul_rn(f.x[4], scale), __fmul_rn(f.x[5], scale));
+        h.w = pack_bf16x2(__fmul_rn(f.x[6], scale), __fmul_rn(f.x[7], scale));
+        st128u(reinterpret_cast<uint16_t *>(g16) + (g << 3), h);
+        sq_acc4(acc, acc1, h);
+    };
+    for (; gi + 3 * stride < ngroups; gi += 4 * stride) {
+        F8 w[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) w[k] = ldg256_stream(g32 + ((gi + k * stride) << 3));
+#pragma unroll
+        for (int k = 0; k < 4; ++k) one(w[k], gi + k * stride);
+    }
+    for (; gi < ngroups; gi += stride) one(ldg256_stream(g32 + (gi << 3)), gi);
+    acc += acc1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+    __shared__ double wsum[8];
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = wsum[0];
+#pragma unroll
+        for (int k = 1; k < 8; ++k) s += wsum[k];
+        partials[blockIdx.x] = s;
+    }
+}
+
+cudaError_t launch_grads_finalize(const float *g32, float scale, void *g16, uint64_t n_padded, double *partials,
+                                  double *out_sumsq, cudaStream_t st, int *n_launches)
+{
+    const uint64_t ngroups = n_padded >> 3;
+    uint64_t want = (ngroups + 255) / 256;
+    int nblocks = (int)(want < 592 ? want : 592);  // 148 SMs x 4 resident CTAs; fixed by n alone
+    if (nblocks < 1) nblocks = 1;
+    k_grads_finalize<<<nblocks, 256, 0, st>>>(g32, scale, g16, ngroups, partials);
+    k_sumsq_final<<<1, kSumsqMaxBlocks, 0, st>>>(partials, nblocks, 0.0f, out_sumsq, nullptr);
+    if (n_launches) *n_launches = 2;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
 // p16 = RNE_bf16(p)
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_regen_bf16(const float *__restrict__ p, void *__restrict__ p16, uint64_t ngroups)
 {
     const uint64_t gi = (uint64_t)blockIdx.x * 256 + threadIdx.x;
     if (gi >= ngroups) return;
-    const F8 P = ld256<1>(p + (gi << 3));
+    const F8 P = ld256(p + (gi << 3));
     uint4 h;
     h.x = pack_bf16x2(P.x[0], P.x[1]);
     h.y = pack_bf16x2(P.x[2], P.x[3]);
     h.z = pack_bf16x2(P.x[4], P.x[5]);
     h.w = pack_bf16x2(P.x[6], P.x[7]);
-    st128u<1>(reinterpret_cast<uint16_t *>(p16) + (gi << 3), h);
+    st128u(reinterpret_cast<uint16_t *>(p16) + (gi << 3), h);
 }
 
 cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cudaStream_t st)
@@ -837,7 +745,7 @@ __global__ void __launch_bounds__(kRestoreThreads) k_restore_bulk(const float *_
             h.y = pack_bf16x2(a.z, a.w);
             h.z = pack_bf16x2(b.x, b.y);
             h.w = pack_bf16x2(b.z, b.w);
-            st128u<1>(reinterpret_cast<uint16_t *>(p16) + e0 + e, h);
+            st128u(reinterpret_cast<uint16_t *>(p16) + e0 + e, h);
         }
         __syncthreads();  // everyone is done reading stage s
         if (threadIdx.x == 0) {
@@ -864,69 +772,6 @@ cudaError_t launch_restore_bulk(const void *src_payload, float *p, float *m, flo
     if (grid > ntiles) grid = ntiles;
     k_restore_bulk<<<(unsigned)grid, kRestoreThreads, smem, st>>>(reinterpret_cast<const float *>(src_payload), p, m, v,
                                                                    p16, n_padded);
-    return cudaGetLastError();
-}
-
-// ------------------------------------------------------------------------------------------
-// Diagnostic: the HBM ceiling of a read:write mix.  One pass over n_read + n_write disjoint planes
-// with the fused step's access pattern (one 256-bit vector per thread and plane, the same cache
-// hints, 256-thread CTAs) and NO arithmetic beyond what keeps the loads alive.  bench.py reports the
-// fused kernel against the ceiling of its own mix (3 fp32 planes read, 6 written) next to the
-// driver-measured copy peak.  RT/WT >= 0: compile-time plane counts (few registers, full occupancy,
-// used for the mixes bench.py reports); -1: run-time counts (any mix up to 8 + 8 planes).
-// ------------------------------------------------------------------------------------------
-template <int RT, int WT>
-__global__ void __launch_bounds__(kStepThreads) k_hbm_probe(float *__restrict__ base, uint64_t plane_elems, uint64_t ngroups,
-                                                            uint32_t n_read_rt, uint32_t n_write_rt)
-{
-    constexpr int RMAX = RT >= 0 ? (RT > 0 ? RT : 1) : kProbeMaxPlanes;
-    constexpr int WMAX = WT >= 0 ? (WT > 0 ? WT : 1) : kProbeMaxPlanes;
-    const int n_read = RT >= 0 ? RT : (int)n_read_rt, n_write = WT >= 0 ? WT : (int)n_write_rt;
-    const uint64_t gi = (uint64_t)blockIdx.x * kStepThreads + threadIdx.x;
-    if (gi >= ngroups) return;
-    const uint64_t e = gi << 3;
-    F8 acc;
-#pragma unroll
-    for (int j = 0; j < 8; ++j) acc.x[j] = (float)(uint32_t)gi;
-    F8 r[RMAX];
-#pragma unroll
-    for (int i = 0; i < RMAX; ++i)
-        if (i < n_read) r[i] = ld256<1>(base + (uint64_t)i * plane_elems + e);
-#pragma unroll
-    for (int i = 0; i < RMAX; ++i)
-        if (i < n_read) {
-#pragma unroll
-            for (int j = 0; j < 8; ++j) acc.x[j] = __fadd_rn(acc.x[j], r[i].x[j]);
-        }
-#pragma unroll
-    for (int i = 0; i < WMAX; ++i)
-        if (i < n_write) st256<1>(base + (uint64_t)(n_read + i) * plane_elems + e, acc);
-    if (n_write == 0) {  // keep the loads alive: a store that never happens
-        float t = 0.f;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) t += acc.x[j];
-        if (t == -123.456f) base[e] = t;
-    }
-}
-
-cudaError_t launch_hbm_probe(void *d_buf, uint64_t plane_bytes, uint32_t n_read, uint32_t n_write, cudaStream_t st)
-{
-    if (n_read > (uint32_t)kProbeMaxPlanes || n_write > (uint32_t)kProbeMaxPlanes || n_read + n_write == 0)
-        return cudaErrorInvalidValue;
-    const uint64_t plane_elems = plane_bytes / 4, ngroups = plane_elems >> 3;
-    if (ngroups == 0) return cudaSuccess;
-    const unsigned grid = (unsigned)((ngroups + kStepThreads - 1) / kStepThreads);
-    float *b = static_cast<float *>(d_buf);
-#define PHX_PROBE(R, W) k_hbm_probe<R, W><<<grid, kStepThreads, 0, st>>>(b, plane_elems, ngroups, n_read, n_write)
-    switch (n_read * 16 + n_write) {
-    case 4 * 16 + 0: PHX_PROBE(4, 0); break;
-    case 0 * 16 + 4: PHX_PROBE(0, 4); break;
-    case 1 * 16 + 1: PHX_PROBE(1, 1); break;
-    case 3 * 16 + 6: PHX_PROBE(3, 6); break;
-    case 3 * 16 + 3: PHX_PROBE(3, 3); break;
-    default: PHX_PROBE(-1, -1); break;
-    }
-#undef PHX_PROBE
     return cudaGetLastError();
 }
 

@@ -41,18 +41,38 @@ struct StepArgs {
     void *pub[kMaxPublish];
     uint32_t n_pub;
     AdamScalars sc;
+    // graph-capturable form: where k_step_prologue left the scalars of the step (null: use sc and hdr above)
+    const AdamScalars *dsc;
     HeaderBlob hdr;
 };
 
-enum { kNumStepVariants = 12 };
+// Device-resident step block of the graph-capturable form (include/phx.h "graph"): the hyperparameters, the
+// step counter the live state stands at, the scalars k_step_prologue derived for the step in flight, the
+// envelope template.  Lives in the handle's device scratch.
+struct alignas(16) StepBlock {
+    AdamScalars sc;            // must stay first (16-byte aligned vector loads in k_step8<.., DEV>)
+    float lr, beta1, beta2, eps, wd;
+    uint32_t misaligned;       // replays whose device step did not land on the staging slot baked at capture
+    uint64_t step;
+    alignas(16) uint8_t hdr_tmpl[256];
+    alignas(16) uint8_t hdr_work[256];
+};
+
 // SURVEY §8(f2) modes of the fused step (default flavour only): binary32 gradients without a bf16
 // copy (the paper's precision) and per-tensor decay groups.
 // §8(f3): kModePublish fuses the parameter all-gather into the step (P2P stores into the peers' buffers).
 enum { kModeF32 = 1, kModeGroups = 2, kModePublish = 4 };
 enum { kDecayTileShift = 11 };  // decay_cls granularity: 2048 elements
 
-// a3.  variant selects the kernel flavour (see phx_kernels.cu); snapshot=false drops the staging stores.
-cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t variant, uint32_t mode, cudaStream_t st);
+// a3.  snapshot=false drops the staging stores; mode = kMode* bits; dev = scalars from a.dsc.
+cudaError_t launch_step(const StepArgs &a, bool snapshot, uint32_t mode, bool dev, cudaStream_t st);
+// graph-capturable form: ++blk->step, scalars -> blk->sc, envelopes -> shdr / shdr_full (either may be null)
+cudaError_t launch_step_prologue(StepBlock *blk, void *shdr, void *shdr_full, uint32_t full_payload, uint32_t expect_slot,
+                                 uint32_t expect_depth, cudaStream_t st);
+cudaError_t launch_step_block_init(StepBlock *blk, float lr, float beta1, float beta2, float eps, float wd, uint64_t step,
+                                   const HeaderBlob &tmpl, cudaStream_t st);
+cudaError_t launch_derive_scalars(float lr, float beta1, float beta2, float wd, const uint64_t *d_steps, uint32_t n,
+                                  float *d_out, cudaStream_t st);
 
 // a1.  partials: >= kSumsqMaxBlocks doubles of device scratch; out_sumsq/out_coef device scalars.
 enum { kSumsqMaxBlocks = 1024 };
@@ -65,6 +85,10 @@ cudaError_t launch_sumsq(const void *g, bool grads_f32, uint64_t n_padded, doubl
 cudaError_t launch_clip_from_partials(const double *partials, uint32_t count, float max_norm, double *out_sumsq,
                                       float *out_coef, cudaStream_t st);
 
+// §8(f4) second half: g16 = RNE_bf16(g32 * scale) and the sum of squares of the rounded values, one pass
+cudaError_t launch_grads_finalize(const float *g32, float scale, void *g16, uint64_t n_padded, double *partials,
+                                  double *out_sumsq, cudaStream_t st, int *n_launches);
+
 // p16 = RNE_bf16(p)
 cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cudaStream_t st);
 
@@ -72,9 +96,5 @@ cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cuda
 // p16 == nullptr skips the bf16 regeneration (kModeF32 shards have no bf16 copy).
 cudaError_t launch_restore_bulk(const void *src_payload, float *p, float *m, float *v, void *p16,
                                 uint64_t n_padded, int sm_count, cudaStream_t st);
-
-// Diagnostic: streaming pass over n_read + n_write planes of plane_bytes each inside d_buf, no arithmetic.
-enum { kProbeMaxPlanes = 8 };
-cudaError_t launch_hbm_probe(void *d_buf, uint64_t plane_bytes, uint32_t n_read, uint32_t n_write, cudaStream_t st);
 
 }  // namespace phx

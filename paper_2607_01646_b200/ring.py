@@ -126,36 +126,79 @@ class PeerRing:
             self.received = None
 
 
+class ParamBuffer:
+    """A rank's model-parameter buffer W (dp_size * n_padded model-dtype elements), allocated so that it can be
+    exported over CUDA IPC.  Allocate it BEFORE the Shard and hand `own_range()` to the Shard as its bf16 copy
+    (`Shard(wl, p16=buf.own_range())`): the fused kernel then keeps the rank's own range of W current through
+    d_p_bf16 and the rank's own buffer need not be bound as a publication target."""
+
+    def __init__(self, wl):
+        h = B.phx_shard_create(wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank),
+                               pp=(wl.pp_size, wl.pp_rank), flags=wl.flags(),
+                               precision=B.PHX_PRECISION_FP32 if wl.precision == "fp32" else B.PHX_PRECISION_BF16_GRADS)
+        info = B.phx_shard_info(h)
+        B.phx_shard_destroy(h)
+        self.fp32 = wl.precision == "fp32"
+        self.n_padded, self.dp_size, self.dp_rank = info.n_padded, info.dp_size, info.dp_rank
+        self.nbytes = info.param_bytes
+        self.ptr = B.phx_peer_buffer_alloc(self.nbytes)
+
+    def view(self):
+        """Zero-copy torch view (model dtype) of W."""
+        import torch
+        return device_view(self.ptr, self.nbytes).view(torch.float32 if self.fp32 else torch.bfloat16)
+
+    def own_range(self):
+        """The rank's own range of W (for Shard(p16=...) in the bf16 precision)."""
+        return self.view()[self.dp_rank * self.n_padded:(self.dp_rank + 1) * self.n_padded]
+
+    def free(self):
+        if self.ptr is not None:
+            B.phx_peer_buffer_free(self.ptr)
+            self.ptr = None
+
+
 class ParamGroup:
     """one rank's end of the model-parameter publication.  Every rank of the DP group owns
     a model-parameter buffer W (dp_size * n_padded model-dtype elements, IPC-exportable); the others' buffers
     are opened over CUDA IPC and bound, so that the fused step kernel (PHX_PUBLISH_FUSED) or the copy engine
-    (PHX_PUBLISH_COPY_ENGINE) writes this rank's range into all of them — the all-gather."""
+    (PHX_PUBLISH_COPY_ENGINE) writes this rank's range into all of them — the all-gather.
+
+    `own`: a ParamBuffer the shard was built on (Shard(p16=own.own_range())): only the D-1 OTHER buffers are
+    bound (D <= PHX_MAX_PARAM_PEERS + 1 = 16, no redundant local stores).  Without it (or in the all-FP32
+    precision, where the kernel has no model-param copy of its own) the rank's W is allocated here and bound
+    like a peer: D targets, D <= PHX_MAX_PARAM_PEERS."""
 
     def __init__(self, shard, mode=B.PHX_PUBLISH_FUSED, group=None, ring_size: Optional[int] = None,
-                 ring_rank: Optional[int] = None):
+                 ring_rank: Optional[int] = None, own: Optional[ParamBuffer] = None):
         import torch.distributed as dist
         self.shard = shard
         D = shard.info.dp_size if ring_size is None else ring_size
         r = shard.info.dp_rank if ring_rank is None else ring_rank
         assert dist.is_initialized() and dist.get_world_size(group) == D and dist.get_rank(group) == r
-        assert D <= B.PHX_MAX_PARAM_PEERS
         elem = 4 if shard.fp32 else 2
         self.nbytes = shard.info.dp_size * shard.info.n_padded * elem
         self.own, self.opened, err = None, [], None
-        try:
-            self.own = B.phx_peer_buffer_alloc(self.nbytes)
-            mine = B.phx_ipc_export(self.own)
-        except Exception as e:  # noqa: BLE001
-            mine, err = None, repr(e)
+        self.owns_buffer = own is None
+        in_place = (own is not None and not shard.fp32 and shard.p16 is not None
+                    and shard.p16.data_ptr() == own.ptr + shard.info.dp_rank * shard.info.n_padded * 2)
+        n_targets = (D - 1) if in_place else D
+        if n_targets > B.PHX_MAX_PARAM_PEERS:
+            err = (f"publication to {n_targets} buffers exceeds PHX_MAX_PARAM_PEERS = {B.PHX_MAX_PARAM_PEERS}"
+                   + ("" if in_place else "; build the Shard on a ParamBuffer (own=) to need only dp_size - 1"))
+        mine = None
+        if err is None:
+            try:
+                self.own = own.ptr if own is not None else B.phx_peer_buffer_alloc(self.nbytes)
+                mine = B.phx_ipc_export(self.own)
+            except Exception as e:  # noqa: BLE001
+                mine, err = None, repr(e)
         table: List[Optional[bytes]] = [None] * D
         dist.all_gather_object(table, mine, group=group)
         if err is None and all(t is not None for t in table):
             try:
                 self.opened = [B.phx_ipc_open(table[j]) for j in range(D) if j != r]
-                # the rank's own W is bound like a peer: its range is written there too (the shard keeps a
-                # separate d_p_bf16; 2 B/element of local writes buys independence from allocation order)
-                B.phx_shard_bind_param_peers(shard.h, [self.own] + self.opened, mode)
+                B.phx_shard_bind_param_peers(shard.h, ([] if in_place else [self.own]) + self.opened, mode)
             except Exception as e:  # noqa: BLE001
                 err = repr(e)
         elif err is None:
@@ -181,9 +224,9 @@ class ParamGroup:
         for p in self.opened:
             B.phx_ipc_close(p)
         self.opened = []
-        if self.own is not None:
+        if self.own is not None and self.owns_buffer:
             B.phx_peer_buffer_free(self.own)
-            self.own = None
+        self.own = None
 
 
 def connect_in_process(shards: Sequence, k: int) -> List[ReceivedBuffers]:

@@ -39,6 +39,41 @@ def test_library_exports_every_declared_symbol():
     assert B.lib().phx_strerror(B.PHX_ERR_STEP_ORDER) == b"step is not last_step + 1"
 
 
+def dynamic_symbols(path):
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", path], capture_output=True, text=True, check=True).stdout
+    return [ln.split()[-1] for ln in out.splitlines() if ln.strip()]
+
+
+def test_library_exports_product_symbols_only():
+    """nothing but the C ABI of include/phx.h is visible — no tuning knob, no diagnostic,
+    no leaked C++ runtime template instantiation (linker version script csrc/phx.map)."""
+    syms = dynamic_symbols(B.LIB_PATH)
+    assert sorted(syms) == sorted(declared_functions()), set(syms) ^ set(declared_functions())
+    assert "phx_set_kernel_variant" not in syms and "phx_hbm_probe_async" not in syms
+    # the bench-only diagnostic lives in a library of its own
+    from paper_2607_01646_b200 import probe
+    assert dynamic_symbols(probe.LIB_PATH) == ["phx_hbm_probe_async"]
+
+
+def test_host_derived_scalars_equal_the_oracle_bitwise():
+    """the host code of libphx.so must round every binary64 operation like the oracle
+    (-ffp-contract=off in build.py); compared for several (lr, wd, beta, t) incl. the Appendix A values."""
+    import numpy as np
+    cases = [(3e-4, 0.9, 0.95, 0.1), (1e-3, 0.9, 0.999, 0.01), (6e-4, 0.8, 0.98, 0.0), (1.0, 0.5, 0.25, 0.3),
+             (2.5e-5, 0.95, 0.9999, 1e-4)]
+    steps = [1, 2, 3, 10, 17, 100, 1000, 4097, 65535, 10**6, 2**33 + 5]
+    for lr, b1, b2, wd in cases:
+        for t in steps:
+            got = np.array(B.phx_derived_scalars_host(lr, b1, b2, wd, t), np.float32).view(np.uint32)
+            exp = O.scalars(lr, b1, b2, 1e-8, wd, t).view(np.uint32)
+            assert np.array_equal(got, exp), (lr, b1, b2, wd, t)
+    # SURVEY.md Appendix A bit patterns (lr 3e-4, betas (0.9, 0.95), wd 0.1)
+    got = np.array(B.phx_derived_scalars_host(3e-4, 0.9, 0.95, 0.1, 1), np.float32).view(np.uint32)
+    assert [hex(x) for x in got] == ["0x3f7ffe09", "0x3dccccd0", "0x3d4cccd0", "0x3b449ba3", "0x3e64f930"]
+    assert B.lib().phx_derived_scalars_host(3e-4, 0.9, 0.95, 0.1, 0, (C.c_float * 5)()) == B.PHX_ERR_INVALID_ARG
+
+
 def test_struct_sizes_match_the_header():
     assert C.sizeof(B.phx_tensor_desc_t) == 16
     assert C.sizeof(B.phx_config_t) == 64
@@ -106,7 +141,13 @@ def test_argument_and_state_errors_without_a_gpu():
     assert L.phx_shard_bind(h, 256, 256, 264, 256, 256, 256) == B.PHX_ERR_ALIGNMENT
     assert L.phx_set_user_metadata(h, b"x" * 129, 129) == B.PHX_ERR_INVALID_ARG
     assert L.phx_set_user_metadata(h, b"x" * 128, 128) == B.PHX_OK
-    assert L.phx_set_kernel_variant(h, 99) == B.PHX_ERR_INVALID_ARG
+    # the graph-capturable form and the producer epilogue need bound memory too
+    assert L.phx_graph_begin(h, 1e-3, 0.9, 0.95, 1e-8, 0.0, None) == B.PHX_ERR_NOT_BOUND
+    assert L.phx_graph_step_and_snapshot(h, 256, None) == B.PHX_ERR_NOT_BOUND
+    assert L.phx_graph_end(h, None) == B.PHX_ERR_NOT_BOUND
+    assert L.phx_grads_finalize_async(h, 256, 1.0, 512, 1024, None) == B.PHX_ERR_NOT_BOUND
+    assert L.phx_grads_finalize_async(h, None, 1.0, 512, 1024, None) == B.PHX_ERR_INVALID_ARG
+    assert B.phx_dropped_snapshots(h) == (0, 0)
     assert B.phx_last_step(h) == 0 and B.phx_kernel_launches(h) == 0
     B.phx_shard_destroy(h)
     assert L.phx_shard_destroy(None) == B.PHX_ERR_INVALID_ARG

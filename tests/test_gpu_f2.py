@@ -152,13 +152,10 @@ def test_fp32_hand_computable_clip():
     s.close()
 
 
-def test_f2_modes_accept_only_the_default_variant_and_need_no_bf16_buffer():
+def test_f2_fp32_shard_needs_no_bf16_buffer_but_bf16_precision_does():
     wl = W.tiny_workload([4096], dp_size=1, precision="fp32")
     s = Shard(wl, device=DEV)
-    with pytest.raises(B.PhxError) as e:
-        B.phx_set_kernel_variant(s.h, 3)
-    assert e.value.code == B.PHX_ERR_INVALID_ARG
-    B.phx_set_kernel_variant(s.h, 0)
+    assert s.p16 is None
     s.close()
     # a bf16-precision shard still requires the bf16 buffer
     h = B.phx_shard_create([(4096, 0)], 1, 0)

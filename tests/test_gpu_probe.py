@@ -1,9 +1,10 @@
-"""phx_hbm_probe_async (diagnostic of bench.py's roofline context): touches exactly the planes it is told
-to, leaves the read planes and everything behind the last plane alone, rejects bad arguments."""
+"""phx_hbm_probe_async (BENCH-ONLY diagnostic of bench.py's roofline context, libphx_probe.so — not part of the
+product library): touches exactly the planes it is told to, leaves the read planes and everything behind the
+last plane alone, rejects bad arguments."""
 import pytest
 import torch
 
-from paper_2607_01646_b200 import binding as B
+from paper_2607_01646_b200 import probe as PB
 
 from gpu_util import DEV
 
@@ -15,7 +16,7 @@ def test_probe_reads_and_writes_only_its_planes(r, w):
     plane = 256 * 37
     buf = torch.full(((r + w + 1) * plane,), 0x5A, dtype=torch.uint8, device=DEV)
     buf[:r * plane].view(torch.float32).fill_(0.25)                   # small values: group index + sum stays exact
-    B.phx_hbm_probe_async(buf, plane, r, w, torch.cuda.current_stream())
+    assert PB.phx_hbm_probe_async(buf, plane, r, w, torch.cuda.current_stream()) == 0
     torch.cuda.synchronize()
     assert bool((buf[:r * plane].view(torch.float32) == 0.25).all())  # read planes untouched
     assert bool((buf[(r + w) * plane:] == 0x5A).all())                # nothing behind the last plane
@@ -28,11 +29,11 @@ def test_probe_reads_and_writes_only_its_planes(r, w):
 
 
 def test_probe_argument_errors():
-    L = B.lib()
+    L = PB.lib()
     buf = torch.zeros(4096, dtype=torch.uint8, device=DEV)
-    assert L.phx_hbm_probe_async(None, 256, 1, 1, None) == B.PHX_ERR_INVALID_ARG
-    assert L.phx_hbm_probe_async(buf.data_ptr(), 0, 1, 1, None) == B.PHX_ERR_INVALID_ARG
-    assert L.phx_hbm_probe_async(buf.data_ptr(), 100, 1, 1, None) == B.PHX_ERR_INVALID_ARG
-    assert L.phx_hbm_probe_async(buf.data_ptr(), 256, 9, 0, None) == B.PHX_ERR_INVALID_ARG
-    assert L.phx_hbm_probe_async(buf.data_ptr(), 256, 0, 0, None) == B.PHX_ERR_INVALID_ARG
-    assert L.phx_hbm_probe_async(buf.data_ptr() + 16, 256, 1, 1, None) == B.PHX_ERR_ALIGNMENT
+    assert L.phx_hbm_probe_async(None, 256, 1, 1, None) == -1
+    assert L.phx_hbm_probe_async(buf.data_ptr(), 0, 1, 1, None) == -1
+    assert L.phx_hbm_probe_async(buf.data_ptr(), 100, 1, 1, None) == -1
+    assert L.phx_hbm_probe_async(buf.data_ptr(), 256, 9, 0, None) == -1
+    assert L.phx_hbm_probe_async(buf.data_ptr(), 256, 0, 0, None) == -1
+    assert L.phx_hbm_probe_async(buf.data_ptr() + 16, 256, 1, 1, None) == -2

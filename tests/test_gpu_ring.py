@@ -416,24 +416,24 @@ def test_publication_argument_errors():
     arr2 = (C.c_void_p * 1)(buf.data_ptr() + 2)
     assert L.phx_shard_bind_param_peers(s.h, arr2, 1, 0) == B.PHX_ERR_ALIGNMENT
     B.phx_shard_bind_param_peers(s.h, [buf])
-    with pytest.raises(B.PhxError):
-        B.phx_set_kernel_variant(s.h, 3)            # fused publication exists for the default flavour only
     s.close()
 
 
-def _param_rank(rank, world, port, mode, q):
+def _param_rank(rank, world, port, mode, q, in_place=False):
     import torch.distributed as dist
     os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     torch.cuda.set_device(0)
     dist.init_process_group("gloo")
     wl = W.tiny_workload([40_000, 77], dp_size=world, dp_rank=rank)
-    s = Shard(wl, device=DEV)
+    # in_place: the shard's bf16 copy IS the rank's own range of W, only the other D-1 buffers are bound
+    own = PR.ParamBuffer(wl) if in_place else None
+    s = Shard(wl, device=DEV, p16=own.own_range() if in_place else None)
     o = O.OracleShard(wl.layout(), world, rank)
     p0 = W.init_params(s.n, s.n_padded, 70 + rank)
     s.p.copy_(p0)
     s.set_state(0)
     o.set_state(p0.numpy())
-    pg = PR.ParamGroup(s, mode)
+    pg = PR.ParamGroup(s, mode, own=own)
     st = torch.cuda.Stream(device=DEV)
     for t in range(1, 3):
         g = W.gen_grads(wl, s.segments, s.n_padded, t, 70 + rank)
@@ -451,16 +451,19 @@ def _param_rank(rank, world, port, mode, q):
     dist.barrier()
     pg.close()
     s.close()
+    if own is not None:
+        own.free()
     dist.destroy_process_group()
 
 
+@pytest.mark.parametrize("in_place", [False, True])
 @pytest.mark.parametrize("mode", [B.PHX_PUBLISH_FUSED, B.PHX_PUBLISH_COPY_ENGINE])
-def test_param_group_two_processes_over_ipc(mode):
+def test_param_group_two_processes_over_ipc(mode, in_place):
     world = 2
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    port = 29900 + (os.getpid() + mode) % 40
-    ps = [ctx.Process(target=_param_rank, args=(r, world, port, mode, q)) for r in range(world)]
+    port = 29900 + (os.getpid() + mode + 2 * int(in_place)) % 40
+    ps = [ctx.Process(target=_param_rank, args=(r, world, port, mode, q, in_place)) for r in range(world)]
     for p in ps:
         p.start()
     res = sorted(q.get(timeout=300) for _ in ps)
