@@ -1,30 +1,37 @@
 #!/usr/bin/env python
-"""bench.py — measures the phx hot path on B200 and prints ONE JSON line (see DESIGN.md §Measurement).
+"""bench.py — measures the phx hot path on B200 and prints ONE JSON line (DESIGN.md §9).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c2] [--impl phx|reference]
-    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--configs c2,c3,c4a,c4b,c5] [--impl phx|reference]
 
-What is timed (config c2 = BASELINE.json:configs[1], the 1.3B-style shard, by default):
-  value     fused AdamW+snapshot HBM GB/s: K back-to-back passes of a1..a3 (phx_step_and_snapshot:
-            [clip,] sync-point wait, ONE fused kernel writing live state + bf16 copy + packed snapshot
-            into the staging ring) with gradients already resident in HBM; 40 algorithmic bytes per
-            element / device time (CUDA events on the launching stream).  Working set >> L2.
-  e2e       the same metric through the same C-ABI calls with HOST buffers: every step copies the
-            step's bf16 gradients from pinned host memory (H2D) and brings the step's result — the
-            packed snapshot — back to the pinned host replica (a4 chunked D2H + a5 commit).
-  overlap   the paper's experiment: iterations of G bf16 4096^3 GEMMs (stand-in for
-            forward/backward) + the hot path, with the flush on a side stream, against the same loop
-            with snapshots disabled; exposed checkpoint ms/iteration = difference of trimmed means.
-  roofline  HBM roofline of the dominant (fused) kernel; host_link: the flush against the measured
-            pinned-copy peak.
-  cpu_baseline  the oracle as it stands on the box's host cores (rank 0, N=1), bounded sample.
+`--gpus N` with N > 1 starts N ranks BY ITSELF (re-exec through torch.distributed.run on 127.0.0.1) when it
+was not launched under torchrun already; it fails loudly when the box has fewer than N GPUs.
+
+The one line covers EVERY bandwidth-sized config of BASELINE.json (c2, c3, c4a, c4b, c5) in one process:
+  value      fused AdamW+snapshot HBM GB/s of the HEADLINE config — c3, the largest single-GPU configuration —
+             K back-to-back passes of the whole device-side hot path (a1 clip pass where the config has one, a2
+             sync-point wait, a3 ONE fused kernel writing live state + bf16 copy + packed snapshot) with the
+             gradients resident in HBM; the step's TRUE algorithmic bytes (42 B/element with the a1 pass, 40
+             without) / device time (CUDA events on the launching stream).  Working set >> L2.
+  roofline   the dominant kernel (the fused step) alone, 40 B/element, against the measured HBM peak.
+  configs    per config: step / kernel / snapshot-off ms and GB/s, flush GB/s against the pinned-copy peak measured
+             in the same run, exposed checkpoint ms/iteration at T_c >= 4 T_D2H and at the tight 1.25 T_D2H window,
+             with eagerly launched iterations and with the whole iteration captured in a CUDA graph (the
+             graph-capturable form of the step), e2e through host buffers, restore + recompute, the c4 hot-swap
+             scenario (bit-exact trajectory flag), the c5 chunk x depth grid, the c3 producer-side clip.
+  e2e        the headline config through the same C-ABI calls with HOST buffers (H2D grads, D2H snapshot + commit).
+  cpu_baseline  the oracle as it stands on the box's host cores, on the SAME bounded sample `--impl reference` times.
+  clocks     nvidia-smi sampled over the whole run (50 ms), reported per timed leg.
 `--impl reference` times the oracle instead (the reference arm of this tier).
 """
 from __future__ import annotations
 
 import argparse
+import contextlib
+import datetime
 import json
+import math
 import os
+import socket
 import statistics
 import subprocess
 import sys
@@ -37,69 +44,68 @@ if ROOT not in sys.path:
 
 METRIC = "fused_adamw_snapshot_hbm_gbs"
 UNIT = "GB/s"
-BYTES_PER_ELEM = 40          # 14 read + 26 written
-BYTES_PER_ELEM_OFF = 28
+BYTES_PER_ELEM = 40          # a3: 14 read + 26 written
+BYTES_PER_ELEM_OFF = 28      # a3 with snapshots off / direct source
+BYTES_A1 = 2                 # a1: one read of the bf16 gradients (4 in the all-FP32 precision)
 NOMINAL_HBM_GBS = 8000.0     # north_star "~8 TB/s"
 FALLBACK_HBM_GBS = 6650.0    # /opt/skills/guides/B200_PROFILING.md, only if MEASURED_PEAKS.json is absent
+ALL_CONFIGS = ["c2", "c3", "c4a", "c4b", "c5"]
+HEADLINE = "c3"              # the largest single-GPU configuration of BASELINE.json:configs
+ORACLE_SAMPLE = 1 << 26      # elements of the shard the oracle is timed on (both arms): ~10-30 s of CPU work
 
 
-def parse_args():
+def parse_args(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=500)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="phx", choices=["phx", "reference"])
-    ap.add_argument("--config", default="c2", help="workload key (c1, c2, c3, c4a, c4b, c5)")
-    ap.add_argument("--variant", type=int, default=0, help="fused-kernel variant (tuning)")
+    ap.add_argument("--configs", default="", help="comma list of workload keys (default: c2,c3,c4a,c4b,c5 at one GPU, "
+                                                  "the headline config at N > 1)")
+    ap.add_argument("--config", default="", help="shorthand for --configs X --headline X")
+    ap.add_argument("--headline", default=HEADLINE, help="config `value` / `roofline` / `e2e` are quoted on")
     ap.add_argument("--depth", type=int, default=2)
     ap.add_argument("--chunk-mib", type=int, default=8)
     ap.add_argument("--sync", default="strict", choices=["strict", "relaxed"])
     ap.add_argument("--gemms", type=int, default=0, help="GEMMs per overlapped iteration (0 = auto: T_c >= 4 T_D2H)")
-    ap.add_argument("--overlap-iters", type=int, default=20)
-    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--overlap-secs", type=float, default=3.5, help="time budget per overlap arm (sets the iteration count)")
+    ap.add_argument("--overlap-iters", type=int, default=0, help="iterations per overlap arm (0 = from --overlap-secs, 8..30)")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="0 = auto (>= 1.5 s)")
     ap.add_argument("--no-overlap", action="store_true")
+    ap.add_argument("--no-graph-step", action="store_true", help="skip the CUDA-graph-captured iteration arms")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-mix-ceiling", action="store_true", help="skip the no-arithmetic HBM mix-ceiling probe")
-    ap.add_argument("--cpu-sample", type=int, default=0, help="elements of the shard the oracle is timed on (0 = auto)")
-    ap.add_argument("--mode", default="headline",
-                    choices=["headline", "configs", "overlap-curve", "sweep", "hotswap", "timeline"],
-                    help="headline: the ONE contract line (default).  The others print one JSON line per "
-                         "measurement: configs = every config's kernel/flush/restore; overlap-curve = exposed ms vs G; "
-                         "sweep = chunk x depth x sync-mode grid (BASELINE.json:configs[4]); hotswap = configs[3]")
-    ap.add_argument("--overlap-reps", type=int, default=2, help="ABAB alternations of the overlap arms")
+    ap.add_argument("--no-grid", action="store_true", help="skip the c5 chunk x depth grid")
+    ap.add_argument("--cpu-sample", type=int, default=0, help="elements the oracle is timed on (0 = %d)" % ORACLE_SAMPLE)
+    ap.add_argument("--mode", default="headline", choices=["headline", "overlap-curve", "sweep", "timeline"],
+                    help="headline: the ONE contract line (default).  The others print one JSON line per measurement: "
+                         "overlap-curve = exposed ms vs G; sweep = the full chunk x depth x sync-mode grid "
+                         "(BASELINE.json:configs[4]); timeline = copy/compute overlap from CUDA events")
     ap.add_argument("--source", default="staged", choices=["staged", "direct"],
                     help="snapshot source: staged = fused kernel also writes the staging slot (40 B/elem, north_star); "
                          "direct = flush DMAs the live planes under the strict sync point (28 B/elem)")
     ap.add_argument("--restore-mode", default="copy", choices=["bulk", "copy"])
     ap.add_argument("--peers", type=int, default=-1,
-                    help="k ring peers the snapshot is also replicated to over NVLink (SURVEY 8(f1)); -1 = auto: 1 when "
-                         "--gpus > 1 (real P2P ring over CUDA IPC), 0 at one GPU; k > 0 at one GPU measures a loopback "
-                         "stand-in (received buffer on the same device)")
-    ap.add_argument("--publish", default="none", choices=["none", "fused", "copy"],
-                    help="SURVEY 8(f3): also publish the model-param copy into the other DP ranks' parameter buffers — "
-                         "fused = P2P stores from the step kernel, copy = copy engine after it.  N > 1: real buffers over "
-                         "CUDA IPC; N = 1: loopback stand-in with dp_size-1 buffers on the same GPU")
-    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp32"],
-                    help="bf16 = fp32 state + bf16 grads + bf16 copy (north_star, default); fp32 = the paper's own "
-                         "all-FP32 setting (PAPER.md:270; SURVEY 8(f2)): fp32 grads, no bf16 copy, 16 B read + 24 B written")
-    ap.add_argument("--decay-groups", action="store_true",
-                    help="flag biases and norm weights no-decay (per-tensor AdamW parameter groups, SURVEY 8(f2))")
-    ap.add_argument("--window", default="eager", choices=["eager", "graph"],
-                    help="how the stand-in GEMM window of the overlap runs is launched: eager torch.matmul calls "
-                         "(default) or replays of a CUDA graph of 64 GEMMs")
-    ap.add_argument("--no-graph-arm", action="store_true", help="skip the CUDA-graph repeat of the overlap run")
-    ap.add_argument("--payload", default="optimizer", choices=["optimizer", "full"],
-                    help="what the local host slots hold: optimizer = p,m,v + envelope (the H2H payload, default); "
-                         "full = SURVEY 8(f4), the paper's D2H payload (PAPER.md:145): p,m,v + the rank's whole "
-                         "model-parameter buffer W + envelope, for in-place recovery")
-    ap.add_argument("--clip-scope", default="local", choices=["local", "global"],
-                    help="configs with a clip (c3): local = the shard's own norm (a1 inside the step); global = "
-                         "SURVEY 8(e): per-rank sum of squares, all-gather of one double per rank (NCCL when "
-                         "--gpus > 1), coefficient from the D sums inside the step")
+                    help="k ring peers (SURVEY 8(f1)); -1 = auto: k = 1 and 2 over the real CUDA-IPC ring when --gpus > 1, "
+                         "none at one GPU; k > 0 at one GPU measures a loopback stand-in (same device)")
+    ap.add_argument("--publish", default="auto", choices=["auto", "none", "fused", "copy", "both"],
+                    help="SURVEY 8(f3) model-parameter publication: auto = both at N > 1, none at one GPU")
+    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp32"])
+    ap.add_argument("--decay-groups", action="store_true")
+    ap.add_argument("--payload", default="optimizer", choices=["optimizer", "full"])
+    ap.add_argument("--clip-scope", default="auto", choices=["auto", "local", "global"],
+                    help="configs with a clip (c3): local = the shard's own norm; global = SURVEY 8(e) all-gather of one "
+                         "double per rank; auto = local at one GPU, both at N > 1")
     ap.add_argument("--chunks", default="4,8,16,32,64,128,256", help="chunk sizes (MiB) of --mode sweep")
     ap.add_argument("--depths", default="1,2,3,4", help="staging depths of --mode sweep")
     ap.add_argument("--syncs", default="strict,relaxed", help="sync modes of --mode sweep")
-    return ap.parse_args()
+    ap.add_argument("--debug-shared-gpu", action="store_true",
+                    help="N > 1 ranks all on cuda:0 with a gloo control plane — a functional check of the N-rank code "
+                         "path on a one-GPU box; the numbers it prints are NOT multi-GPU numbers and say so")
+    a = ap.parse_args(argv)
+    if a.config:
+        a.configs, a.headline = a.config, a.config
+    return a
 
 
 # ----------------------------------------------------------------------------------------------
@@ -131,48 +137,75 @@ def committed_traffic(config):
     return None
 
 
-class ClockSampler:
-    """nvidia-smi clocks/throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+class ClockLog:
+    """nvidia-smi clocks / throttle reasons sampled over the WHOLE run with timestamps (one process, 50 ms), cut
+    into the timed legs afterwards — every leg gets its own record (B200_PROFILING.md clocks line)."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
-    def __init__(self, index=0):
+    def __init__(self, index=0, period_ms=50):
+        self.legs = []
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", str(period_ms)],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 
+    @contextlib.contextmanager
+    def leg(self, name):
+        t0 = time.time()
+        try:
+            yield
+        finally:
+            self.legs.append((name, t0, time.time()))
+
+    @staticmethod
+    def _parse(path):
+        rows = []
+        for r in open(path):
+            w = [x.strip() for x in r.strip().split(",")]
+            if len(w) < 8:
+                continue
+            try:
+                ts = datetime.datetime.strptime(w[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                rows.append((ts, float(w[1]), float(w[2]), float(w[3]), [x.lower().startswith("active") for x in w[4:8]]))
+            except Exception:
+                continue
+        return rows
+
+    @classmethod
+    def _summary(cls, rows):
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        reasons = sorted({cls.NAMES[k] for r in rows for k in range(4) if r[4][k]})
+        return {"sm_mhz": statistics.median(r[1] for r in rows), "sm_min_mhz": min(r[1] for r in rows),
+                "sm_max_mhz": max(r[2] for r in rows), "power_w_max": max(r[3] for r in rows),
+                "reasons": reasons, "samples": len(rows)}
+
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        """-> (summary over all legs, {leg name: summary})"""
         if self.p is None:
-            return out
-        time.sleep(0.15)
+            return self._summary([]), {}
+        time.sleep(0.12)
         self.p.terminate()
         try:
             self.p.wait(timeout=5)
         except Exception:
             self.p.kill()
         self.f.flush()
-        rows = [r.strip().split(",") for r in open(self.f.name) if r.strip()]
+        rows = self._parse(self.f.name)
         os.unlink(self.f.name)
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in rows:
-            try:
-                sm.append(float(r[0])); mx.append(float(r[1]))
-                for k, nme in enumerate(names):
-                    if r[3 + k].strip().lower().startswith("active"):
-                        reasons.add(nme)
-            except Exception:
-                continue
-        if sm:
-            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
-        return out
+        per = {}
+        for name, t0, t1 in self.legs:
+            per[name] = self._summary([r for r in rows if t0 <= r[0] <= t1])
+            per[name]["seconds"] = round(t1 - t0, 3)
+        inside = [r for r in rows if any(t0 <= r[0] <= t1 for _, t0, t1 in self.legs)]
+        return self._summary(inside), per
 
 
 def trimmed_mean(xs, drop_first=0, drop_slowest_frac=0.05):
@@ -197,25 +230,30 @@ def dist_init(world, use_cuda):
     return dist
 
 
-def max_over_ranks(x: float, world, device) -> float:
-    """The slowest rank defines the step time (max over ranks)."""
+def _reduce(x: float, world, device, op):
     if world == 1:
         return x
     import torch
     import torch.distributed as dist
-    t = torch.tensor([x], dtype=torch.float64, device=device)
-    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dev = device if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([x], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=op)
     return float(t.item())
+
+
+def max_over_ranks(x: float, world, device) -> float:
+    """The slowest rank defines the step time (max over ranks)."""
+    if world == 1:
+        return x
+    import torch.distributed as dist
+    return _reduce(x, world, device, dist.ReduceOp.MAX)
 
 
 def sum_over_ranks(x: float, world, device) -> float:
     if world == 1:
         return x
-    import torch
     import torch.distributed as dist
-    t = torch.tensor([x], dtype=torch.float64, device=device)
-    dist.all_reduce(t, op=dist.ReduceOp.SUM)
-    return float(t.item())
+    return _reduce(x, world, device, dist.ReduceOp.SUM)
 
 
 def barrier(world):
@@ -224,8 +262,33 @@ def barrier(world):
         dist.barrier()
 
 
+def free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def self_spawn(args):
+    """`python bench.py --gpus N` launched plainly: start N ranks (one per GPU) through torch.distributed.run."""
+    if args.impl == "phx" and not args.debug_shared_gpu:
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            raise SystemExit(f"bench.py --gpus {args.gpus}: this box has {have} CUDA device(s); refusing to time fewer "
+                             f"ranks than asked for (there is no CPU fallback)")
+    env = dict(os.environ)
+    if args.impl == "phx":
+        # leave NCCL's own init lines visible, on stderr so that stdout stays ONE JSON line
+        env.setdefault("NCCL_DEBUG", "INFO")
+        env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        env.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
+
+
 # ----------------------------------------------------------------------------------------------
-# reference arm / cpu baseline: the oracle on the host cores
+# reference arm / cpu baseline: the oracle on the host cores — ONE sample definition for both
 # ----------------------------------------------------------------------------------------------
 
 
@@ -236,8 +299,18 @@ def workload_of(args, key):
     return dataclasses.replace(W.CONFIGS[key], precision=args.precision, decay_groups=bool(args.decay_groups))
 
 
+def step_bytes_per_elem(wl, source="staged", clip_pass=True):
+    """Algorithmic bytes per element of one pass of the device-side hot path."""
+    fp32 = wl.precision == "fp32"
+    b = BYTES_PER_ELEM_OFF if source == "direct" else BYTES_PER_ELEM
+    if clip_pass and wl.hyper.max_grad_norm > 0:
+        b += 4 if fp32 else BYTES_A1
+    return b
+
+
 def time_oracle(wl, sample, steps, warmup, nthreads):
-    """Oracle AdamW step (phx_oracle.c, as it stands) on the first `sample` elements of the shard."""
+    """Oracle hot path (phx_oracle.c as it stands: a1 sum of squares + clip where the config has one, a3 AdamW
+    step) on the first `sample` elements of the shard.  Inputs generated on the CPU from the workload's seed."""
     import numpy as np
     import torch
     from oracle import oracle as O
@@ -281,26 +354,39 @@ def time_oracle(wl, sample, steps, warmup, nthreads):
     return n, times
 
 
+def oracle_sample_desc(n, wl, steps, warmup):
+    return (f"first {n} of {wl.n_expected} elements of the {wl.key} shard, {steps} steps after {warmup} warm-up; "
+            f"a1 sum of squares (single thread) + a3 AdamW step (all cores)" if wl.hyper.max_grad_norm > 0 else
+            f"first {n} of {wl.n_expected} elements of the {wl.key} shard, {steps} steps after {warmup} warm-up; a3 AdamW step")
+
+
+def cpu_baseline(wl, sample, steps, warmup):
+    """The record both arms print for the oracle on the host cores: same workload, same sample, same byte count."""
+    cores = len(os.sched_getaffinity(0))
+    n, times = time_oracle(wl, sample, steps, warmup, cores)
+    t = sum(times) / len(times)
+    bpe = step_bytes_per_elem(wl)
+    return {"value": bpe * n / t / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": oracle_sample_desc(n, wl, steps, warmup), "sample_elements": n, "ms_per_step": t * 1e3,
+            "elements_per_s": n / t, "bytes_per_element": bpe}
+
+
 def run_reference(args):
     rank, world, _ = rank_env()
     if rank != 0:
         return 0
-    wl = workload_of(args, args.config)
-    cores = len(os.sched_getaffinity(0))
-    sample = args.cpu_sample or (1 << 24)
-    n, times = time_oracle(wl, sample, args.steps, args.warmup, cores)
-    ms = 1e3 * sum(times) / len(times)
-    value = BYTES_PER_ELEM * n / (ms * 1e-3) / 1e9
+    wl = workload_of(args, args.headline)
+    cb = cpu_baseline(wl, args.cpu_sample or ORACLE_SAMPLE, args.steps, args.warmup)
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": cb["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{wl.key}: {wl.title}", "sample_elements": n,
-                   "note": "oracle/phx_oracle.c AdamW step (+clip) on the first sample_elements of the shard, OpenMP over all host cores"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
-                         "sample": f"first {n} of {wl.n_expected} elements, {args.steps} steps",
-                         "elements_per_s": n / (ms * 1e-3)},
-        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "config": {"workload": f"{wl.key}: {wl.title}", "sample_elements": cb["sample_elements"],
+                   "bytes_per_element": cb["bytes_per_element"],
+                   "note": "oracle/phx_oracle.c as it stands on the host cores; the same bounded sample the phx arm's "
+                           "cpu_baseline times"},
+        "cpu_baseline": cb,
+        "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
@@ -317,7 +403,7 @@ class Rig:
     and in pinned host memory, a flush stream, the GEMM operands of the stand-in compute window."""
 
     def __init__(self, args, key, rank=0, world=1, local_rank=0, depth=None, chunk_mib=None, sync=None,
-                 replica=None, host_grads=True, restore_mode=None, source=None):
+                 replica=None, host_grads=True, restore_mode=None, source=None, clip_scope="local"):
         import dataclasses
         import torch
         from paper_2607_01646_b200 import binding as B
@@ -331,7 +417,7 @@ class Rig:
         self.depth = depth or args.depth
         self.chunk_mib = chunk_mib or args.chunk_mib
         self.sync_name = sync or args.sync
-        sync_mode = B.PHX_SYNC_STRICT if self.sync_name == "strict" else B.PHX_SYNC_RELAXED
+        self.sync_mode = B.PHX_SYNC_STRICT if self.sync_name == "strict" else B.PHX_SYNC_RELAXED
         self.source_name = source or args.source
         self.source = B.PHX_SNAPSHOT_DIRECT if self.source_name == "direct" else B.PHX_SNAPSHOT_STAGED
         self.bytes_per_elem = BYTES_PER_ELEM_OFF if self.source_name == "direct" else BYTES_PER_ELEM
@@ -339,11 +425,10 @@ class Rig:
             restore_mode = B.PHX_RESTORE_COPY_ENGINE if args.restore_mode == "copy" else B.PHX_RESTORE_BULK_KERNEL
         self.restore_mode_name = "copy_engine" if restore_mode == B.PHX_RESTORE_COPY_ENGINE else "bulk_kernel"
         self.full = getattr(args, "payload", "optimizer") == "full"
-        self.s = Shard(self.wl, device=self.device, staging_depth=self.depth, sync_mode=sync_mode,
+        self.s = Shard(self.wl, device=self.device, staging_depth=self.depth, sync_mode=self.sync_mode,
                        chunk_bytes=self.chunk_mib << 20, replica=replica, restore_mode=restore_mode,
                        snapshot_source=self.source,
                        payload=B.PHX_PAYLOAD_FULL_RANK_STATE if self.full else B.PHX_PAYLOAD_OPTIMIZER)
-        B.phx_set_kernel_variant(self.s.h, args.variant)
         self.N = self.s.n_padded
         self.s.p.copy_(W.init_params(self.s.n, self.N, self.wl.seed, device=self.device))
         self.s.set_state(0)
@@ -364,7 +449,8 @@ class Rig:
         self.k_peers = 0
         self.peers_in_overlap = False
         self.gclip = None
-        if getattr(args, "clip_scope", "local") == "global" and self.wl.hyper.max_grad_norm > 0:
+        self.clip = self.wl.hyper.max_grad_norm > 0
+        if clip_scope == "global" and self.clip:
             from paper_2607_01646_b200.clip import GlobalClip
             self.gclip = GlobalClip(self.s)     # default process group = the DP group of this bench
 
@@ -377,7 +463,7 @@ class Rig:
         self.k_peers = k
         if world > 1:
             self.ring = PR.PeerRing(self.s, k, ring_size=world, ring_rank=rank)
-            return "NVLink/NVSwitch P2P into the ring successors' HBM, received buffers mapped over CUDA IPC"
+            return "P2P into the ring successors' HBM, received buffers mapped over CUDA IPC"
         self.recv = PR.ReceivedBuffers(self.s.info.slot_stride, k)
         self.B.phx_shard_bind_peers(self.s.h, self.recv.ptrs)
         return "loopback stand-in: received buffers on the SAME GPU (device-to-device copy engine, not NVLink)"
@@ -403,13 +489,14 @@ class Rig:
             self.B.phx_shard_bind_peers(self.s.h, [])
             self.recv.free()
             self.recv = None
+        self.k_peers = 0
 
     def precision_code(self):
         return self.B.PHX_PRECISION_FP32 if self.fp32 else self.B.PHX_PRECISION_BF16_GRADS
 
     def kernel_name(self):
         mode = (1 if self.fp32 else 0) | (2 if any(self.wl.flags()) else 0)
-        return "phx::k_step8<1,1,%s,%d>" % ("true" if self.source_name == "staged" else "false", mode)
+        return "phx::k_step8<%s,%d,false>" % ("true" if self.source_name == "staged" else "false", mode)
 
     # -- the hot path -------------------------------------------------------------------------------
     def do_step(self):
@@ -435,16 +522,19 @@ class Rig:
         per = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
         return ev[0].elapsed_time(ev[K]), per, B.phx_kernel_launches(self.s.h) - l0
 
+    def _aux_handle(self, **kw):
+        B, wl = self.B, self.wl
+        h = B.phx_shard_create(wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank),
+                               pp=(wl.pp_size, wl.pp_rank), flags=wl.flags(), precision=self.precision_code(), **kw)
+        return h
+
     def time_fused_kernel_alone(self, K):
         """The dominant kernel without the clip kernels: a second handle with clipping off bound to the same memory."""
-        torch, B, wl = self.torch, self.B, self.wl
-        h0 = B.phx_shard_create(wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank),
-                                pp=(wl.pp_size, wl.pp_rank), staging_depth=self.depth, max_grad_norm=0.0,
-                                snapshot_source=self.source, flags=wl.flags(), precision=self.precision_code())
+        torch, B = self.torch, self.B
+        h0 = self._aux_handle(staging_depth=self.depth, max_grad_norm=0.0, snapshot_source=self.source)
         B.phx_shard_bind(h0, self.s.p, self.s.m, self.s.v, self.s.p16, self.s.staging, self.s.replica)
         B.phx_shard_set_state(h0, 0, self.cur)
-        B.phx_set_kernel_variant(h0, self.args.variant)
-        hp = wl.hyper
+        hp = self.wl.hyper
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         for k in range(3 + K):
             if k == 3:
@@ -455,17 +545,45 @@ class Rig:
         B.phx_shard_destroy(h0)
         return e0.elapsed_time(e1) / K
 
+    def time_producer_clip(self, K):
+        """the gradients come out of the producer's epilogue (fp32 main gradients -> bf16 + sum of
+        squares, one pass) and the step takes the sum: no a1 pass.  Returns (finalize ms, step ms)."""
+        torch, B = self.torch, self.B
+        g32 = self.W.gen_grads(self.wl, self.s.segments, self.N, 3, self.wl.seed, device=self.device, dtype=torch.float32)
+        g16 = torch.empty(self.N, dtype=torch.bfloat16, device=self.device)
+        S = torch.zeros(1, dtype=torch.float64, device=self.device)
+        for _ in range(2):
+            self.s.grads_finalize(g32, 1.0, g16, S)
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nf = max(5, K // 10)
+        f0.record(self.cur)
+        for _ in range(nf):
+            self.s.grads_finalize(g32, 1.0, g16, S)
+        f1.record(self.cur)
+        for _ in range(3):
+            self.step += 1
+            B.phx_set_clip_partials(self.s.h, S, 1)
+            self.s.step_and_snapshot(g16, self.step)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = B.phx_kernel_launches(self.s.h)
+        e0.record(self.cur)
+        for _ in range(K):
+            self.step += 1
+            B.phx_set_clip_partials(self.s.h, S, 1)
+            self.s.step_and_snapshot(g16, self.step)
+        e1.record(self.cur)
+        torch.cuda.synchronize()
+        launches = B.phx_kernel_launches(self.s.h) - l0
+        del g32, g16
+        return f0.elapsed_time(f1) / nf, e0.elapsed_time(e1) / K, launches / K
+
     def off_shard(self):
         """Snapshot-disabled handle (the paper's 'mechanism disabled' baseline) bound to the same live arrays."""
         if self.s_off is None:
-            B, wl = self.B, self.wl
-            h = B.phx_shard_create(wl.layout(), wl.dp_size, wl.dp_rank, tp=(wl.tp_size, wl.tp_rank),
-                                   pp=(wl.pp_size, wl.pp_rank), snapshot_disabled=True,
-                                   max_grad_norm=wl.hyper.max_grad_norm, flags=wl.flags(),
-                                   precision=self.precision_code())
+            B = self.B
+            h = self._aux_handle(snapshot_disabled=True, max_grad_norm=self.wl.hyper.max_grad_norm)
             B.phx_shard_bind(h, self.s.p, self.s.m, self.s.v, self.s.p16, None, None)
             B.phx_shard_set_state(h, 0, self.cur)
-            B.phx_set_kernel_variant(h, self.args.variant)
             self.s_off = h
         return self.s_off
 
@@ -544,6 +662,56 @@ class Rig:
         torch.cuda.synchronize()
         return back, r0.elapsed_time(r1), r1.elapsed_time(r2)
 
+    def hotswap(self, G):
+        """BASELINE.json:configs[3]: 20 steps with snapshots (overlapped with G GEMMs each), the live shard is dropped
+        while step 21 is in flight, restore from the pinned host replica, recompute 21, run 22..25; timed, and the
+        trajectory compared bit for bit with an uninterrupted run (GPU vs GPU; GPU vs oracle is in tests/)."""
+        torch, W, wl, N = self.torch, self.W, self.wl, self.N
+        torch.cuda.synchronize()
+        self.s.wait(self.step) if self.step and self.B.phx_snapshot_query(self.s.h) else None
+        self.s.p.copy_(W.init_params(self.s.n, N, wl.seed, device=self.device))
+        self.s.m.zero_(); self.s.v.zero_()
+        self.s.set_state(0)
+        self.step = 0
+        ref = self.Shard(wl, device=self.device, snapshot=False)
+        ref.p.copy_(self.s.p); ref.set_state(0)
+        for t in range(1, 26):
+            ref.step_and_snapshot(self.grads[t & 1], t)
+        torch.cuda.synchronize()
+        self.gemm_setup()
+        for t in range(1, 21):
+            self.gemm_window(G)
+            self.do_step()
+            self.s.flush_async(self.side)
+        self.do_step()                                # step 21 launched: in flight when the fault hits
+        torch.cuda.synchronize()
+        self.s.drop_live()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r0, r1, r2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        r0.record(self.cur)
+        back = self.s.restore()
+        r1.record(self.cur)
+        self.step = back
+        self.do_step()                                # recompute of the in-flight step (a7)
+        r2.record(self.cur)
+        torch.cuda.synchronize()
+        wall_ms = (time.perf_counter() - t0) * 1e3
+        for t in range(22, 26):
+            self.do_step()
+            self.s.flush_async(self.side)
+        self.s.wait(25)
+        torch.cuda.synchronize()
+        same = all(torch.equal(x, y) for x, y in ((self.s.p, ref.p), (self.s.m, ref.m), (self.s.v, ref.v),
+                                                  (self.s.p16, ref.p16)))
+        ref.close()
+        del ref
+        rms = r0.elapsed_time(r1)
+        return {"restored_step": int(back), "restore_ms": rms, "recompute_ms": r1.elapsed_time(r2),
+                "restore_plus_recompute_ms": r0.elapsed_time(r2), "restore_plus_recompute_wall_ms": wall_ms,
+                "host_link_gbs": 12 * N / (rms * 1e-3) / 1e9, "trajectory_bit_exact_vs_uninterrupted": bool(same),
+                "steps_before_fault": 20, "steps_after": 5, "gemms_per_iter": G, "mode": self.restore_mode_name}
+
     # -- the stand-in compute window ----------------------------------------------------------------
     def gemm_setup(self):
         torch = self.torch
@@ -563,51 +731,37 @@ class Rig:
             self.gemm_ms = g0.elapsed_time(g1) / 200
         return self.gemm_ms
 
-    def gemm_window(self, G, mode=None):
-        """The stand-in compute window: G GEMMs, launched eagerly (default) or — `--window graph` — as replays of
-        one CUDA graph of 64 GEMMs (plus an eager remainder), the launch form a B200 training step would use."""
-        torch = self.torch
+    def gemm_window(self, G):
+        """The stand-in compute window: G bf16 4096^3 GEMMs (BASELINE.json:configs[1])."""
         a, b, c = self._gemm
-        if (mode or getattr(self.args, "window", "eager")) != "graph":
-            for _ in range(G):
-                torch.matmul(a, b, out=c)
-            return
-        if getattr(self, "_graph", None) is None:
-            s = torch.cuda.Stream(device=self.device)
-            s.wait_stream(self.cur)
-            with torch.cuda.stream(s):
-                for _ in range(3):
-                    torch.matmul(a, b, out=c)
-            self.cur.wait_stream(s)
-            torch.cuda.synchronize()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g):
-                for _ in range(64):
-                    torch.matmul(a, b, out=c)
-            self._graph = g
-        for _ in range(G // 64):
-            self._graph.replay()
-        for _ in range(G % 64):
-            torch.matmul(a, b, out=c)
+        mm = self.torch.matmul
+        for _ in range(G):
+            mm(a, b, out=c)
 
-    def headline_gemms(self, flush_ms, factor=4.0):
-        """R21: smallest power of two G with T_c >= factor x T_D2H."""
+    def gemms_for(self, flush_ms, factor=4.0, pow2=True):
+        """R21: smallest power of two G with T_c >= factor x T_D2H (or the plain quotient for the tight window)."""
         gm = self.gemm_setup()
+        if not pow2:
+            return max(1, int(round(factor * flush_ms / gm)))
         G = 64
         while G * gm < factor * flush_ms:
             G *= 2
         return G
 
-    def overlap(self, G, iters, reps, arms=("off", "staged", "on"), warm=2, window=None):
-        """Iterations of G GEMMs + the hot path, three arms alternated `reps` times (ABCABC) to average
-        out clock drift:
+    def iters_for(self, G):
+        if self.args.overlap_iters > 0:
+            return self.args.overlap_iters
+        t_iter = (G * self.gemm_ms * 1.1 + 1.0) * 1e-3
+        return max(8, min(30, int(self.args.overlap_secs / t_iter)))
+
+    def overlap(self, G, iters, arms=("off", "on"), warm=2, reps=1):
+        """Iterations of G GEMMs + the hot path, EAGERLY launched, arms alternated `reps` times:
           off    — snapshot-disabled kernel, no flush (the paper's baseline run);
           staged — snapshot-on kernel (writes the staging slot), no flush;
           on     — snapshot-on kernel + flush on the side stream (PHOENIX enabled).
         Per-iteration times from CUDA events on the compute stream; PAPER.md:283 trimming."""
         torch = self.torch
         self.gemm_setup()
-        a, b, c = self._gemm
         it_ms = {k: [] for k in arms}
         hp_ms = {k: [] for k in arms}
         for _ in range(reps):
@@ -616,7 +770,7 @@ class Rig:
                 for it in range(warm + iters):
                     e0 = torch.cuda.Event(enable_timing=True)
                     e0.record(self.cur)
-                    self.gemm_window(G, window)
+                    self.gemm_window(G)
                     k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                     k0.record(self.cur)
                     if arm == "off":
@@ -626,7 +780,7 @@ class Rig:
                     k1.record(self.cur)
                     if arm == "on":
                         self.flush()
-                        if getattr(self, "k_peers", 0) and self.peers_in_overlap:
+                        if self.k_peers and self.peers_in_overlap:
                             self.B.phx_snapshot_flush_peers_async(self.s.h, self.peer_stream)
                     evs.append(e0)
                     kevs.append((k0, k1))
@@ -635,16 +789,15 @@ class Rig:
                 torch.cuda.synchronize()
                 if arm == "on":
                     self.s.wait(self.step)
-                    if getattr(self, "k_peers", 0) and self.peers_in_overlap:
+                    if self.k_peers and self.peers_in_overlap:
                         self.B.phx_snapshot_wait_peers(self.s.h, self.step)
                 evs.append(end)
                 it_ms[arm] += [evs[i].elapsed_time(evs[i + 1]) for i in range(warm, warm + iters)]
                 hp_ms[arm] += [x.elapsed_time(y) for x, y in kevs[warm:]]
         t = {k: trimmed_mean(v) for k, v in it_ms.items()}
         out = {"gemms_per_iter": G, "gemm_ms": self.gemm_ms, "compute_window_ms": G * self.gemm_ms,
-               "window_launch": window or getattr(self.args, "window", "eager"),
-               "iters_per_arm": iters * reps, "reps": reps,
-               "protocol": "PAPER.md:283: warm-up dropped, slowest 5% dropped, mean of the rest; arms alternated"}
+               "launch": "eager", "iters_per_arm": iters * reps,
+               "protocol": "PAPER.md:283: warm-up dropped, slowest 5% dropped, mean of the rest"}
         for k in arms:
             out[f"iter_ms_{k}"] = t[k]
             out[f"hot_path_ms_in_loop_{k}"] = trimmed_mean(hp_ms[k])
@@ -654,6 +807,55 @@ class Rig:
         if "staged" in t and "off" in t:
             out["exposed_ms_kernel_only"] = t["staged"] - t["off"]
         return out
+
+    def overlap_graph_step(self, G, iters, warm=1):
+        """The same experiment with the WHOLE iteration captured in a CUDA graph — the B200-native launch form
+        (DESIGN.md §12): [flush of snapshot k-1 on the side stream ‖ G GEMMs] -> step k, two iterations per graph
+        (staging / host slot ping-pong), through the graph-capturable form of the step (phx_graph_*).  Arms:
+        off = snapshot-disabled handle, no flush; on = snapshots + flush.  One eager event pair per replay:
+        iteration time = replay time / 2."""
+        torch, B = self.torch, self.B
+        self.gemm_setup()
+        hp = self.wl.hyper
+        cap = torch.cuda.Stream(device=self.device)
+        res = {}
+        nrep = max(4, (iters + 1) // 2)
+        for arm in ("off", "on"):
+            h = self.off_shard() if arm == "off" else self.s.h
+            torch.cuda.synchronize()
+            B.phx_graph_begin(h, hp.lr, hp.beta1, hp.beta2, hp.eps, hp.wd, cap)
+            B.phx_graph_step_and_snapshot(h, self.grads[1], cap)         # a snapshot for the first captured flush
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=cap):
+                for i in range(2):
+                    if arm == "on":
+                        self.side.wait_stream(cap)                       # fork: the flush runs beside the window
+                        B.phx_graph_flush_async(h, self.side)
+                    self.gemm_window(G)
+                    B.phx_graph_step_and_snapshot(h, self.grads[i & 1], cap)   # a2 joins the flush back
+                cap.wait_stream(self.side)
+            times = []
+            for r in range(warm + nrep):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(cap)
+                graph.replay()
+                e1.record(cap)
+                times.append((e0, e1))
+            torch.cuda.synchronize()
+            ms = [a.elapsed_time(b) / 2 for a, b in times[warm:]]
+            res[arm] = trimmed_mean(ms)
+            last = B.phx_graph_end(h)
+            if arm == "on":
+                self.step = last
+                self.s.flush_async(self.side)                            # the newest snapshot is still staged
+                self.s.wait(self.step)
+            else:
+                self.off_step = last
+            del graph
+        return {"gemms_per_iter": G, "compute_window_ms": G * self.gemm_ms, "launch": "cuda graph (2 iterations per graph)",
+                "iters_per_arm": 2 * nrep, "iter_ms_off": res["off"], "iter_ms_on": res["on"],
+                "exposed_ms": res["on"] - res["off"], "exposed_frac_of_compute_step": (res["on"] - res["off"]) / res["off"]}
 
     def close(self):
         self.close_peers()
@@ -682,9 +884,10 @@ def measure_host_link(torch, device, nbytes=1 << 30, reps=5):
     return out
 
 
-def measure_hbm_mix_ceiling(torch, B, device, plane_elems, reps=20):
-    """No-arithmetic streaming passes with the fused kernel's access pattern (phx_hbm_probe_async): the HBM
+def measure_hbm_mix_ceiling(torch, device, plane_elems, reps=20):
+    """No-arithmetic streaming passes with the fused kernel's access pattern (libphx_probe.so, bench-only): the HBM
     ceiling for a read:write mix.  Returns GB/s per mix; planes of `plane_elems` fp32 each (larger than L2)."""
+    from paper_2607_01646_b200 import probe as PB
     mixes = {"read_only_4r": (4, 0), "write_only_4w": (0, 4), "copy_1r1w": (1, 1), "step_mix_3r6w": (3, 6),
              "off_mix_3r3w": (3, 3)}
     plane_bytes = int(plane_elems) * 4
@@ -694,11 +897,11 @@ def measure_hbm_mix_ceiling(torch, B, device, plane_elems, reps=20):
     out = {}
     for name, (r, w) in mixes.items():
         for _ in range(3):
-            B.phx_hbm_probe_async(buf, plane_bytes, r, w, st)
+            assert PB.phx_hbm_probe_async(buf, plane_bytes, r, w, st) == 0
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(st)
         for _ in range(reps):
-            B.phx_hbm_probe_async(buf, plane_bytes, r, w, st)
+            PB.phx_hbm_probe_async(buf, plane_bytes, r, w, st)
         e1.record(st)
         torch.cuda.synchronize()
         out[name] = (r + w) * plane_bytes / (e0.elapsed_time(e1) / reps * 1e-3) / 1e9
@@ -706,202 +909,409 @@ def measure_hbm_mix_ceiling(torch, B, device, plane_elems, reps=20):
     return out
 
 
-def gpu_setup():
+def gpu_setup(args):
     import torch
     rank, world, local_rank = rank_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --impl phx needs a B200: there is no CPU fallback")
+    if args.debug_shared_gpu:
+        local_rank = 0
+    elif world > 1 and torch.cuda.device_count() < world:
+        raise SystemExit(f"bench.py: {world} ranks but {torch.cuda.device_count()} CUDA device(s)")
     torch.cuda.set_device(local_rank)
-    dist_init(world, True)
+    dist_init(world, not args.debug_shared_gpu)
     return torch, rank, world, local_rank
 
 
-def run_headline(args):
-    torch, rank, world, local_rank = gpu_setup()
-    rig = Rig(args, args.config, rank, world, local_rank)
-    device, N, wl, B = rig.device, rig.N, rig.wl, rig.B
-    K, Wm = args.steps, max(args.warmup, 3)
-    link = measure_host_link(torch, device) if rank == 0 else {}
+# ----------------------------------------------------------------------------------------------
+# one config: every number of SURVEY.md §8(d) for it
+# ----------------------------------------------------------------------------------------------
 
-    # ---- value: K back-to-back a1..a3 passes, inputs resident in HBM ---------------------------------
+
+def measure_config(args, key, link, clk, rank, world, local_rank, K, Wm, peak, headline):
+    """Returns (record, extras): `record` goes into the line's `configs` array; `extras` carries what only the
+    headline config reports at top level (launch count, per-step times, the Rig itself for the N > 1 legs)."""
+    import torch
+    rig = Rig(args, key, rank, world, local_rank)
+    device, N, wl, B = rig.device, rig.N, rig.wl, rig.B
+    tag = key
+    BPE = rig.bytes_per_elem
+    step_bpe = step_bytes_per_elem(wl, rig.source_name)
+    rec = {"config": key, "workload": wl.title, "elements": int(N), "state_bytes": int(12 * N),
+           "clip": "local a1 pass over the bf16 gradients" if rig.clip else "none"}
+
+    # ---- the step: K back-to-back a1..a3 passes, inputs resident in HBM --------------------------------
     for _ in range(Wm):
         rig.do_step()
     torch.cuda.synchronize()
     barrier(world)
-    clocks = ClockSampler(local_rank) if rank == 0 else None
-    total_ms, per, launches = rig.time_steps(K, 0)
+    with clk.leg(f"{tag}.step"):
+        total_ms, per, launches = rig.time_steps(K, 0)
     barrier(world)
-    clk = clocks.stop() if clocks else None
-    total_ms = max_over_ranks(total_ms, world, device)
-    ms_per_step = total_ms / K
-    units = sum_over_ranks(float(N), world, device)            # elements all ranks processed per step
-    BPE = rig.bytes_per_elem                                   # 40 staged (north_star), 28 direct
-    value = BPE * units / (ms_per_step * 1e-3) / 1e9
+    step_ms = max_over_ranks(total_ms, world, device) / K
+    with clk.leg(f"{tag}.kernel"):
+        kern_ms = rig.time_fused_kernel_alone(K) if rig.clip else step_ms
+        off_ms = rig.time_steps_off(min(K, max(50, K // 4)))
+    step_gbs = step_bpe * N / (step_ms * 1e-3) / 1e9
+    kern_gbs = BPE * N / (kern_ms * 1e-3) / 1e9
+    rec.update(step_ms=step_ms, step_bytes_per_element=step_bpe, step_gbs=step_gbs,
+               step_frac_of_measured_peak=step_gbs / peak,
+               kernel_ms=kern_ms, kernel_bytes_per_element=BPE, kernel_gbs=kern_gbs,
+               kernel_frac_of_measured_peak=kern_gbs / peak, kernel_frac_of_nominal_8TBps=kern_gbs / NOMINAL_HBM_GBS,
+               elements_per_s=N / (step_ms * 1e-3), snapshot_off_step_ms=off_ms,
+               snapshot_off_gbs=(step_bpe - 12) * N / (off_ms * 1e-3) / 1e9, steps_timed=K)
+    if rig.clip and not rig.fp32 and rank == 0:
+        with clk.leg(f"{tag}.producer_clip"):
+            fin_ms, pstep_ms, pl = rig.time_producer_clip(max(50, K // 4))
+        rec["clip_source_producer"] = {
+            "clip_source": "producer", "step_ms": pstep_ms, "step_bytes_per_element": BPE,
+            "step_gbs": BPE * N / (pstep_ms * 1e-3) / 1e9, "kernels_per_step": pl,
+            "finalize_ms": fin_ms, "finalize_bytes_per_element": 6,
+            "finalize_gbs": 6 * N / (fin_ms * 1e-3) / 1e9,
+            "note": "SURVEY 8(f4b): phx_grads_finalize_async (fp32 main grads -> bf16 + fp64 sum of squares, ONE pass, "
+                    "in the gradient producer) + phx_set_clip_partials(count=1): the step runs no a1 pass"}
+    extras = {"launches": int(launches), "per_step": per, "rig": rig}
 
-    kern_ms = rig.time_fused_kernel_alone(K) if wl.hyper.max_grad_norm > 0 else ms_per_step
-    off_ms = rig.time_steps_off(min(K, 50))
-    peak, peak_src = measured_peaks()
-    achieved = BPE * N / (kern_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": committed_traffic(args.config + ("" if rig.source_name == "staged" else "-direct")
-                                             + ("-fp32" if rig.fp32 else "") + ("-groups" if args.decay_groups else "")),
-                "peak_source": peak_src, "frac_of_nominal_8TBps": achieved / NOMINAL_HBM_GBS,
-                "kernel": rig.kernel_name(),
-                "kernel_ms": kern_ms, "algorithmic_bytes_per_launch": BPE * N, "bytes_per_element": BPE,
-                "snapshot_off_step_ms": off_ms,
-                "snapshot_off_gbs": BYTES_PER_ELEM_OFF * N / (off_ms * 1e-3) / 1e9}
-    if rank == 0 and not args.no_mix_ceiling:
-        # context, not the denominator: what a kernel with NO arithmetic reaches with this read:write mix
-        ceil = measure_hbm_mix_ceiling(torch, rig.B, device, N)
-        roofline["mix_ceiling_gbs"] = ceil
-        roofline["frac_of_mix_ceiling"] = achieved / ceil["off_mix_3r3w" if rig.source_name == "direct" else "step_mix_3r6w"]
+    # ---- e2e: host buffers through the same C-ABI calls --------------------------------------------------
+    d2h_bytes = int(rig.s.info.host_snapshot_bytes)
+    h2d_bytes = int(rig.grad_bytes * N)
+    est = (d2h_bytes / (link["d2h_gbs"] * 1e9) if link else 0.05) * 1e3
+    Ke = args.e2e_steps or max(10, int(math.ceil(1500.0 / est)))
+    with clk.leg(f"{tag}.e2e"):
+        e2e_ms = max_over_ranks(rig.e2e(Ke, world), world, device)
+    rec["e2e"] = {"ms_per_step": e2e_ms, "steps": Ke, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
+                  "link_gbs": (h2d_bytes + d2h_bytes) / (e2e_ms * 1e-3) / 1e9,
+                  "metric_gbs": step_bpe * N / (e2e_ms * 1e-3) / 1e9}
+    if rank != 0:
+        return rec, extras
 
-    # ---- e2e -----------------------------------------------------------------------------------------
-    e2e_ms = max_over_ranks(rig.e2e(args.e2e_steps, world), world, device)
-    d2h_bytes = int(rig.s.info.host_snapshot_bytes)          # = snapshot_bytes unless --payload full
-    e2e = {"value": BPE * units / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
-           "h2d_bytes_per_step": int(rig.grad_bytes * N), "d2h_bytes_per_step": d2h_bytes, "ms_per_step": e2e_ms,
-           "steps": args.e2e_steps,
-           "note": "H2D grads from pinned host + fused step + chunked D2H of the packed snapshot + commit, per step"}
+    # ---- flush alone (a4+a5) against the measured pinned-copy peak -------------------------------------
+    with clk.leg(f"{tag}.flush"):
+        flush_ms = min(rig.time_flush() for _ in range(3))
+    ach = d2h_bytes / (flush_ms * 1e-3) / 1e9
+    rec["flush"] = {"ms": flush_ms, "gbs": ach, "frac_of_d2h_peak": ach / link["d2h_gbs"], "chunk_mib": rig.chunk_mib,
+                    "bytes": d2h_bytes}
 
-    # ---- §8(f1): ring peers (real NVLink ring at N > 1; opt-in loopback stand-in at N = 1) -------------
-    k_peers = args.peers if args.peers >= 0 else (1 if world > 1 else 0)
-    k_peers = min(k_peers, max(world - 1, 0)) if world > 1 else k_peers
-    peer = None
-    if k_peers > 0:
-        try:
-            peer = {"k": k_peers, "link": rig.setup_peers(k_peers, rank, world)}
-            rig.peers_in_overlap = world > 1      # the loopback copy is not NVLink traffic: keep it out of the overlap arm
-        except Exception as e:  # noqa: BLE001  (PeerRing makes every rank fail together)
-            peer = {"k": k_peers, "error": str(e)[:300]}
-            rig.k_peers = 0
-    if peer and "error" not in peer:
-        pf_ms = max_over_ranks(rig.time_peer_flush(), world, device)
-        pbytes = k_peers * int(rig.s.info.snapshot_bytes)
-        peer.update(flush_ms=pf_ms, bytes_per_step=pbytes, gbs_per_gpu=pbytes / (pf_ms * 1e-3) / 1e9,
-                    note="replication of one packed snapshot to all k peers, copy engine, alone; max over ranks, "
-                         "all ranks sending at once")
+    # ---- exposed checkpoint ms/iteration (PAPER.md:283 protocol) ----------------------------------------
+    if not args.no_overlap:
+        ov = {}
+        for wname, factor, pow2 in (("headline_window", 4.0, True), ("tight_window", 1.25, False)):
+            G = args.gemms if (args.gemms > 0 and pow2) else rig.gemms_for(flush_ms, factor, pow2)
+            iters = rig.iters_for(G)
+            with clk.leg(f"{tag}.overlap.{wname}.eager"):
+                o = rig.overlap(G, iters)
+            w = {"rule": ("G = smallest power of two with T_c >= 4 x T_D2H" if pow2 else "G = round(1.25 x T_D2H / T_gemm)")
+                 if args.gemms <= 0 or not pow2 else "G given", "gemms_per_iter": G,
+                 "compute_window_ms": G * rig.gemm_ms, "flush_ms": flush_ms, "iter_ms_off": o["iter_ms_off"],
+                 "exposed_ms_eager": o["exposed_ms"], "exposed_pct_eager": 100.0 * o["exposed_frac_of_compute_step"],
+                 "iter_ms_on_eager": o["iter_ms_on"], "iters_per_arm": o["iters_per_arm"]}
+            if not args.no_graph_step and not rig.full:
+                with clk.leg(f"{tag}.overlap.{wname}.graph_step"):
+                    og = rig.overlap_graph_step(G, iters)
+                w.update(iter_ms_off_graph_step=og["iter_ms_off"], iter_ms_on_graph_step=og["iter_ms_on"],
+                         exposed_ms_graph_step=og["exposed_ms"],
+                         exposed_pct_graph_step=100.0 * og["exposed_frac_of_compute_step"])
+            ov[wname] = w
+        rec["overlap"] = ov
+        rec["exposed_ckpt_ms_per_iter"] = ov["headline_window"]["exposed_ms_eager"]
+        rec["exposed_pct"] = ov["headline_window"]["exposed_pct_eager"]
 
-    # ---- §8(f3): parameter publication (opt-in) --------------------------------------------------------
-    publication = None
-    if args.publish != "none":
-        from paper_2607_01646_b200 import ring as PR
-        pmode = B.PHX_PUBLISH_FUSED if args.publish == "fused" else B.PHX_PUBLISH_COPY_ENGINE
-        pub_stream = torch.cuda.Stream(device=device)
-        try:
-            if world > 1:
-                pg, npeers = PR.ParamGroup(rig.s, pmode, ring_size=world, ring_rank=rank), world
-                plink = "NVLink/NVSwitch P2P into every rank's parameter buffer (CUDA IPC), own buffer included"
-            else:
-                npeers = min(wl.dp_size - 1, B.PHX_MAX_PARAM_PEERS)
-                lbufs = [torch.zeros(wl.dp_size * N, dtype=torch.float32 if rig.fp32 else torch.bfloat16, device=device)
-                         for _ in range(npeers)]
-                B.phx_shard_bind_param_peers(rig.s.h, lbufs, pmode)
-                pg = None
-                plink = "loopback stand-in: dp_size-1 parameter buffers on the SAME GPU (HBM writes, not NVLink)"
-            for _ in range(3):
-                rig.do_step()
-            torch.cuda.synchronize()
-            barrier(world)
-            q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            q0.record(rig.cur)
-            for _ in range(20):
-                rig.do_step()
-                if pmode == B.PHX_PUBLISH_COPY_ENGINE:
-                    B.phx_publish_params_async(rig.s.h, pub_stream)
-                    rig.cur.wait_stream(pub_stream)      # the next forward pass needs the published parameters
-            q1.record(rig.cur)
-            torch.cuda.synchronize()
-            barrier(world)
-            pms = max_over_ranks(q0.elapsed_time(q1) / 20, world, device)
-            publication = {"mode": args.publish, "buffers_written": npeers, "link": plink, "step_plus_publish_ms": pms,
-                           "bytes_published_per_step": int(npeers * N * (4 if rig.fp32 else 2))}
-            B.phx_shard_bind_param_peers(rig.s.h, [])
-            if pg is not None:
-                pg.close()
-        except Exception as e:  # noqa: BLE001
-            publication = {"mode": args.publish, "error": str(e)[:300]}
-
-    host_link = overlap = restore = cpu = None
-    if rank == 0:
-        # flush alone (a4+a5) against the measured pinned-copy peak
-        flush_ms = rig.time_flush()
-        ach = d2h_bytes / (flush_ms * 1e-3) / 1e9
-        host_link = {"bound": "host_link", "achieved": ach, "peak": link["d2h_gbs"], "unit": "GB/s",
-                     "frac": ach / link["d2h_gbs"], "flush_ms": flush_ms, "chunk_mib": rig.chunk_mib,
-                     "h2d_peak_gbs": link["h2d_gbs"]}
-        # overlap: exposed checkpoint ms/iteration (PAPER.md:283 protocol)
-        if not args.no_overlap:
-            G = args.gemms if args.gemms > 0 else rig.headline_gemms(flush_ms)
-            overlap = rig.overlap(G, args.overlap_iters, args.overlap_reps)
-            if args.window == "eager" and not args.no_graph_arm:
-                # the same experiment with the GEMM window replayed from a CUDA graph: separates the part of the
-                # exposed time that is kernel-LAUNCH interference (PCIe busy with the D2H) from real contention
-                og = rig.overlap(G, args.overlap_iters, args.overlap_reps, arms=("off", "on"), window="graph")
-                overlap["graph_window"] = {k: og[k] for k in ("iter_ms_off", "iter_ms_on", "exposed_ms",
-                                                              "exposed_frac_of_compute_step", "window_launch")}
-            overlap["flush_ms"] = flush_ms
-            overlap["rule"] = "G = smallest power of two with T_c >= 4 x T_D2H" if args.gemms <= 0 else "G given"
-        # restore + recompute (a6, a7)
+    # ---- restore + recompute (a6, a7); the c4 hot-swap scenario ----------------------------------------
+    with clk.leg(f"{tag}.restore"):
         back, rms, cms = rig.restore_timing()
-        restore = {"restore_ms": rms, "recompute_ms": cms, "mode": rig.restore_mode_name, "restored_step": back,
-                   "host_link_gbs": (d2h_bytes - 256) / (rms * 1e-3) / 1e9,
-                   "frac_of_h2d_peak": (d2h_bytes - 256) / (rms * 1e-3) / 1e9 / link["h2d_gbs"]}
-        # restore from the ring successor's received buffer (recovery stage 3 over NVLink)
-        if peer and "error" not in peer:
+        rec["restore"] = {"restore_ms": rms, "recompute_ms": cms, "restore_plus_recompute_ms": rms + cms,
+                          "mode": rig.restore_mode_name, "restored_step": int(back),
+                          "host_link_gbs": (d2h_bytes - 256) / (rms * 1e-3) / 1e9,
+                          "frac_of_h2d_peak": (d2h_bytes - 256) / (rms * 1e-3) / 1e9 / link["h2d_gbs"]}
+        if key in ("c4a", "c4b"):
+            rec["hotswap"] = rig.hotswap(rig.gemms_for(flush_ms, 1.25, False))
+    return rec, extras
+
+
+def measure_c5_grid(args, link, clk, replica, flush_ref):
+    """BASELINE.json:configs[4]: D2H chunk size x staging depth at the TIGHT window (T_c = 1.25 x T_D2H, where
+    depth and chunking can matter): exposed checkpoint ms/iteration and host-link GB/s per cell; reduced grid in the
+    default line (the full 7 x 4 x 2 grid is `--mode sweep`)."""
+    import torch
+    cells = []
+    base = None
+    for sync, depth, chunk in [("strict", 2, 4), ("strict", 2, 16), ("strict", 2, 64), ("strict", 2, 256),
+                               ("strict", 1, 8), ("relaxed", 4, 8), ("relaxed", 4, 64), ("relaxed", 3, 256)]:
+        rig = Rig(args, "c5", depth=depth, chunk_mib=chunk, sync=sync, replica=replica, host_grads=False)
+        rig.gemm_setup()
+        G = max(1, int(round(1.25 * flush_ref / rig.gemm_ms)))
+        iters = max(8, min(16, rig.iters_for(G)))
+        if base is None:
+            base = rig.overlap(G, iters, arms=("off",))["iter_ms_off"]
+        fl = rig.time_flush()
+        o = rig.overlap(G, iters, arms=("on",))
+        cells.append({"sync_mode": sync, "depth": depth, "chunk_mib": chunk, "flush_ms": fl,
+                      "host_link_gbs": (256 + 12 * rig.N) / (fl * 1e-3) / 1e9, "gemms_per_iter": G,
+                      "iter_ms_on": o["iter_ms_on"], "iter_ms_off": base, "exposed_ms": o["iter_ms_on"] - base,
+                      "exposed_pct": 100.0 * (o["iter_ms_on"] - base) / base})
+        rig.close()
+        del rig
+        torch.cuda.empty_cache()
+    best = min(cells, key=lambda c: c["exposed_ms"])
+    worst = max(cells, key=lambda c: c["exposed_ms"])
+    return {"window": "tight: T_c = 1.25 x T_D2H", "d2h_peak_gbs": link["d2h_gbs"], "best": best, "worst": worst,
+            "cells": cells, "note": "reduced grid; the full chunk {4..256} x depth {1..4} x sync grid is --mode sweep"}
+
+
+def multi_gpu_legs(args, rig, rank, world, clk):
+    """The N > 1 rows on the headline config: the ring send over real CUDA-IPC peers
+    (k = 1 and 2), restore from the holder, the parameter publication fused vs copy engine, the DP-global clip."""
+    import torch
+    from paper_2607_01646_b200 import ring as PR
+    B, device, N, wl = rig.B, rig.device, rig.N, rig.wl
+    out = {}
+    # ---- f1: ring replication ---------------------------------------------------------------------------
+    ks = [args.peers] if args.peers > 0 else ([1, 2] if world > 1 and args.peers < 0 else [])
+    ks = [k for k in ks if world == 1 or k <= world - 1]
+    peer_rows = []
+    for k in ks:
+        row = {"k": k}
+        try:
+            row["link"] = rig.setup_peers(k, rank, world)
+            with clk.leg(f"peers.k{k}"):
+                pf_ms = max_over_ranks(min(rig.time_peer_flush() for _ in range(3)), world, device)
+            pbytes = k * int(rig.s.info.snapshot_bytes)
+            row.update(flush_ms=pf_ms, bytes_per_step=pbytes, gbs_per_gpu=pbytes / (pf_ms * 1e-3) / 1e9,
+                       streams="one copy stream per peer" if k > 1 else "caller's stream",
+                       note="replication of one packed snapshot to all k peers, copy engine, alone; max over ranks, "
+                            "all ranks sending at once")
+            # the flush to the peers INSIDE the overlap arm (with the host flush): does NVLink traffic expose anything?
+            if not args.no_overlap and world > 1:
+                rig.peers_in_overlap = True
+                fl = rig.time_flush()
+                G = rig.gemms_for(fl, 4.0, True)
+                with clk.leg(f"peers.k{k}.overlap"):
+                    o = rig.overlap(G, rig.iters_for(G))
+                row["overlap_with_host_and_peer_flush"] = {
+                    "gemms_per_iter": G, "iter_ms_off": o["iter_ms_off"], "iter_ms_on": o["iter_ms_on"],
+                    "exposed_ms": max_over_ranks(o["exposed_ms"], world, device)}
+                rig.peers_in_overlap = False
+            # recovery stage 3 (PAPER.md:171): restore from the ring successor's received buffer
             src = rig.ring.opened[0] if world > 1 else rig.recv.ptrs[0]
             rig.s.drop_live()
             torch.cuda.synchronize()
             p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             p0.record(rig.cur)
-            back_p = B.phx_restore_from(rig.s.h, src, rig.cur)
+            back = B.phx_restore_from(rig.s.h, src, rig.cur)
             p1.record(rig.cur)
             torch.cuda.synchronize()
-            rig.step = back_p
-            pms = p0.elapsed_time(p1)
-            peer.update(restore_from_peer_ms=pms, restore_from_peer_gbs=12 * N / (pms * 1e-3) / 1e9,
-                        restored_step=back_p)
-        # cpu baseline: the oracle on the host cores (rank 0, N == 1 only)
+            rig.step = back
+            pms = max_over_ranks(p0.elapsed_time(p1), world, device)
+            row.update(restore_from_holder_ms=pms, restore_from_holder_gbs=12 * N / (pms * 1e-3) / 1e9,
+                       restored_step=int(back))
+        except Exception as e:  # noqa: BLE001  (PeerRing makes every rank fail together)
+            row["error"] = str(e)[:300]
+        barrier(world)
+        rig.close_peers()
+        peer_rows.append(row)
+    if peer_rows:
+        out["peer_replication"] = peer_rows
+
+    # ---- f3: parameter publication ------------------------------------------------------------------------
+    pmodes = {"auto": (["fused", "copy"] if world > 1 else []), "none": [], "both": ["fused", "copy"],
+              "fused": ["fused"], "copy": ["copy"]}[args.publish]
+    pubs = []
+    for name in pmodes:
+        pmode = B.PHX_PUBLISH_FUSED if name == "fused" else B.PHX_PUBLISH_COPY_ENGINE
+        pub_stream = torch.cuda.Stream(device=device)
+        row = {"mode": name}
+        try:
+            lbufs = None
+            if world > 1:
+                pg, nb = PR.ParamGroup(rig.s, pmode, ring_size=world, ring_rank=rank), world
+                row["link"] = "P2P into every rank's parameter buffer (CUDA IPC), own buffer included"
+            else:
+                nb = min(wl.dp_size - 1, B.PHX_MAX_PARAM_PEERS)
+                lbufs = [torch.zeros(wl.dp_size * N, dtype=torch.float32 if rig.fp32 else torch.bfloat16, device=device)
+                         for _ in range(nb)]
+                B.phx_shard_bind_param_peers(rig.s.h, lbufs, pmode)
+                pg = None
+                row["link"] = "loopback stand-in: dp_size-1 parameter buffers on the SAME GPU (HBM writes, not NVLink)"
+            for _ in range(3):
+                rig.do_step()
+            torch.cuda.synchronize()
+            barrier(world)
+            q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with clk.leg(f"publish.{name}"):
+                q0.record(rig.cur)
+                for _ in range(20):
+                    rig.do_step()
+                    if pmode == B.PHX_PUBLISH_COPY_ENGINE:
+                        B.phx_publish_params_async(rig.s.h, pub_stream)
+                        rig.cur.wait_stream(pub_stream)      # the next forward pass needs the published parameters
+                q1.record(rig.cur)
+                torch.cuda.synchronize()
+            barrier(world)
+            pms = max_over_ranks(q0.elapsed_time(q1) / 20, world, device)
+            row.update(buffers_written=nb, step_plus_publish_ms=pms,
+                       bytes_published_per_step=int(nb * N * (4 if rig.fp32 else 2)))
+            B.phx_shard_bind_param_peers(rig.s.h, [])
+            if pg is not None:
+                pg.close()
+            del lbufs
+        except Exception as e:  # noqa: BLE001
+            row["error"] = str(e)[:300]
+        barrier(world)
+        pubs.append(row)
+    if pubs:
+        out["publication"] = pubs
+
+    # ---- (e): the DP-global clip on a config that has one -----------------------------------------------------
+    scope = args.clip_scope
+    if rig.clip and (scope == "global" or (scope == "auto" and world > 1)):
+        from paper_2607_01646_b200.clip import GlobalClip
+        gc = GlobalClip(rig.s)
+        rig.gclip = gc
+        for _ in range(3):
+            rig.do_step()
+        torch.cuda.synchronize()
+        barrier(world)
+        with clk.leg("global_clip"):
+            tot, _, l = rig.time_steps(50, 0)
+        barrier(world)
+        rig.gclip = None
+        out["global_clip"] = {"step_ms": max_over_ranks(tot, world, device) / 50, "kernels_per_step": l / 50,
+                              "exchange": "all-gather of one fp64 sum per rank (8 x %d bytes), then the fixed-tree sum "
+                                          "inside the step" % world,
+                              "backend": "nccl" if not args.debug_shared_gpu and world > 1 else
+                                         ("gloo via host staging (debug)" if world > 1 else "single rank")}
+    return out
+
+
+def run_headline(args):
+    torch, rank, world, local_rank = gpu_setup(args)
+    device = torch.device(f"cuda:{local_rank}")
+    K, Wm = args.steps, max(args.warmup, 3)
+    keys = [k for k in (args.configs.split(",") if args.configs else (ALL_CONFIGS if world == 1 else [args.headline])) if k]
+    if args.headline not in keys:
+        keys.append(args.headline)
+    clk = ClockLog(local_rank) if rank == 0 else contextlib.nullcontext()
+    if rank != 0:
+        clk = type("NoClk", (), {"leg": staticmethod(lambda name: contextlib.nullcontext())})()
+    link = measure_host_link(torch, device) if rank == 0 else {}
+    if world > 1:   # every rank needs an estimate for its e2e step count; rank 0's measurement is the one reported
+        link0 = [link]
+        import torch.distributed as dist
+        dist.broadcast_object_list(link0, src=0)
+        link_all = link0[0]
+    else:
+        link_all = link
+    peak, peak_src = measured_peaks()
+
+    records, head, head_extras = [], None, None
+    grid = None
+    for key in keys:
+        is_head = key == args.headline
+        rec, extras = measure_config(args, key, link_all, clk, rank, world, local_rank, K, Wm, peak, is_head)
+        rig = extras.pop("rig")
+        if is_head:
+            head, head_extras = rec, extras
+            # ---- roofline of the dominant kernel, on the headline config ------------------------------------
+            BPE, N = rig.bytes_per_elem, rig.N
+            tkey = key + ("" if rig.source_name == "staged" else "-direct") + ("-fp32" if rig.fp32 else "") + \
+                ("-groups" if args.decay_groups else "")
+            roofline = {"bound": "hbm", "achieved": rec["kernel_gbs"], "peak": peak, "unit": "GB/s",
+                        "frac": rec["kernel_gbs"] / peak, "traffic": committed_traffic(tkey), "peak_source": peak_src,
+                        "frac_of_nominal_8TBps": rec["kernel_gbs"] / NOMINAL_HBM_GBS, "kernel": rig.kernel_name(),
+                        "kernel_ms": rec["kernel_ms"], "step_ms": rec["step_ms"],
+                        "algorithmic_bytes_per_launch": BPE * N, "bytes_per_element": BPE,
+                        "note": "kernel_ms: the fused kernel alone (a second handle with the clip off on the same memory); "
+                                "step_ms: the whole device-side hot path incl. the a1 pass where the config has one"}
+            if rank == 0 and not args.no_mix_ceiling:
+                with clk.leg("mix_ceiling"):
+                    ceil = measure_hbm_mix_ceiling(torch, device, N)
+                roofline["mix_ceiling_gbs"] = ceil
+                roofline["frac_of_mix_ceiling"] = rec["kernel_gbs"] / ceil["off_mix_3r3w" if rig.source_name == "direct"
+                                                                          else "step_mix_3r6w"]
+            head_extras["roofline"] = roofline
+            head_extras["rig_desc"] = dict(depth=rig.depth, chunk_mib=rig.chunk_mib, sync=rig.sync_name,
+                                           source=rig.source_name, fp32=rig.fp32, full=rig.full, N=int(rig.N),
+                                           title=f"{rig.wl.key}: {rig.wl.title}", clip=rig.clip)
+            head_extras["multi"] = multi_gpu_legs(args, rig, rank, world, clk)
+        if key == "c5" and rank == 0 and world == 1 and not args.no_grid and not args.no_overlap and "flush" in rec:
+            replica, flush_ref = rig.s.replica, rec["flush"]["ms"]
+            barrier(world)
+            rig.close()
+            del rig
+            torch.cuda.empty_cache()
+            with clk.leg("c5.grid"):
+                rec["chunk_depth_grid"] = measure_c5_grid(args, link, clk, replica, flush_ref)
+            del replica
+        else:
+            barrier(world)      # peers' received buffers stay mapped until every rank is done with them
+            rig.close()
+            del rig
+        records.append(rec)
+        torch.cuda.empty_cache()
+
+    if rank == 0:
+        cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            cores = len(os.sched_getaffinity(0))
-            sample = args.cpu_sample or min(N, 1 << 28)
-            n_s, times = time_oracle(wl, sample, 3, 1, cores)
-            t = sum(times) / len(times)
-            n_1, times1 = time_oracle(wl, min(sample, 1 << 25), 2, 1, 1)
-            t1 = sum(times1) / len(times1)
-            cpu = {"value": BYTES_PER_ELEM * n_s / t / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
-                   "sample": f"first {n_s} of {N} elements of the shard, 3 steps after 1 warm-up",
-                   "elements_per_s": n_s / t, "single_thread_elements_per_s": n_1 / t1}
+            wl = workload_of(args, args.headline)
+            with clk.leg("cpu_baseline"):
+                cpu = cpu_baseline(wl, args.cpu_sample or ORACLE_SAMPLE, 5, 1)
+        clocks_all, clocks_legs = clk.stop()
+        d = head_extras["rig_desc"]
+        units = sum_over_ranks(float(d["N"]), 1, device) * world     # weak scaling: every rank owns a shard of the same size
+        step_bpe = head["step_bytes_per_element"]
+        value = step_bpe * units / (head["step_ms"] * 1e-3) / 1e9
+        he = head["e2e"]
+        worst_exposed = None
+        if all("exposed_pct" in r for r in records):
+            w = max(records, key=lambda r: r["exposed_pct"])
+            worst_exposed = {"config": w["config"], "exposed_pct": w["exposed_pct"], "exposed_ms": w["exposed_ckpt_ms_per_iter"]}
+        slowest = min(records, key=lambda r: r["step_gbs"])
+        hl_clock = clocks_legs.get(f"{args.headline}.step", clocks_all)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": head["step_ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"{wl.key}: {wl.title}", "elements_per_shard": int(N),
-                       "state_bytes": int(12 * N), "staging_depth": rig.depth, "chunk_mib": rig.chunk_mib,
-                       "sync_mode": rig.sync_name, "kernel_variant": args.variant, "snapshot_source": rig.source_name,
-                       "bytes_per_element": BPE,
-                       "precision": ("fp32 state + fp32 grads, no bf16 copy (PAPER.md:270): 16 B read + 24 B written"
-                                     if rig.fp32 else "fp32 state + bf16 grads + bf16 copy (north_star): 14 B read + 26 B written"),
+            "config": {"workload": d["title"] + " — the largest single-GPU configuration of BASELINE.json:configs; "
+                                   "every other bandwidth-sized config is in `configs`",
+                       "configs_measured": keys, "elements_per_shard": d["N"], "state_bytes": 12 * d["N"],
+                       "staging_depth": d["depth"], "chunk_mib": d["chunk_mib"], "sync_mode": d["sync"],
+                       "snapshot_source": d["source"], "bytes_per_element": step_bpe,
+                       "bytes_per_element_note": "42 = a1 pass (2 read) + a3 (14 read + 26 written); 40 without the clip pass",
+                       "precision": ("fp32 state + fp32 grads, no bf16 copy (PAPER.md:270)" if d["fp32"] else
+                                     "fp32 state + bf16 grads + bf16 copy (north_star)"),
                        "decay_groups": bool(args.decay_groups),
-                       "l2": "inputs larger than L2 (working set %.2f GB per step >> 126 MB)" % (BYTES_PER_ELEM * N / 1e9),
-                       "timed_region": "K x phx_step_and_snapshot (a1 clip if configured, a2 sync-point wait, a3 fused "
-                                       "AdamW+bf16 copy+packed snapshot); a4/a5 host flush is in e2e and overlap",
-                       "host_payload": ("full rank state: envelope + p,m,v + model-parameter buffer W (SURVEY 8(f4))"
-                                        if rig.full else "optimizer shard: envelope + p,m,v"),
-                       "clip_scope": ("global: all-gather of one fp64 sum per rank (SURVEY 8(e))" if rig.gclip is not None
-                                      else ("local" if wl.hyper.max_grad_norm > 0 else "none")),
-                       "parallelism": (f"dp{world} shards, one 8-byte-per-rank all-gather per step (global clip)"
-                                       if rig.gclip is not None else
-                                       f"dp{world} independent shards, no data-path collective")},
-            "elements_per_s": units / (ms_per_step * 1e-3),
-            "exposed_ckpt_ms_per_iter": overlap["exposed_ms"] if overlap else None,
-            "roofline": roofline, "host_link": host_link, "e2e": e2e, "overlap": overlap, "restore": restore,
-            "peer_replication": peer, "publication": publication, "cpu_baseline": cpu, "gpu_launches": int(launches), "clocks": clk,
-            "step_ms_min_max": [min(per), max(per)],
+                       "l2": "inputs larger than L2 (working set %.2f GB per step >> 126 MB)" % (step_bpe * d["N"] / 1e9),
+                       "timed_region": "K x phx_step_and_snapshot (a1 clip pass, a2 sync-point wait, a3 fused AdamW + bf16 "
+                                       "copy + packed snapshot); a4/a5 host flush is in e2e and overlap",
+                       "host_payload": "full rank state (SURVEY 8(f4))" if d["full"] else "optimizer shard: envelope + p,m,v",
+                       "parallelism": f"dp{world} independent shards, no data-path collective in the timed region",
+                       "shared_gpu_debug": bool(args.debug_shared_gpu)},
+            "elements_per_s": units / (head["step_ms"] * 1e-3),
+            "value_min_over_configs": {"config": slowest["config"], "step_gbs": slowest["step_gbs"]},
+            "exposed_ckpt_ms_per_iter": head.get("exposed_ckpt_ms_per_iter"),
+            "exposed_pct_worst_config": worst_exposed,
+            "roofline": head_extras["roofline"],
+            "host_link": ({"bound": "host_link", "achieved": head["flush"]["gbs"], "peak": link["d2h_gbs"], "unit": "GB/s",
+                           "frac": head["flush"]["frac_of_d2h_peak"], "flush_ms": head["flush"]["ms"],
+                           "chunk_mib": d["chunk_mib"], "h2d_peak_gbs": link["h2d_gbs"]} if "flush" in head else None),
+            "e2e": {"value": he["metric_gbs"] * world, "unit": UNIT, "h2d_bytes_per_step": he["h2d_bytes_per_step"],
+                    "d2h_bytes_per_step": he["d2h_bytes_per_step"], "ms_per_step": he["ms_per_step"], "steps": he["steps"],
+                    "link_gbs": he["link_gbs"],
+                    "note": "H2D grads from pinned host + fused step + chunked D2H of the packed snapshot + commit, per step; "
+                            "host-link bound by construction (14 N bytes must cross PCIe): ms_per_step and link_gbs are "
+                            "the physical numbers, `value` restates them in the metric's unit"},
+            "configs": records,
+            "cpu_baseline": cpu, "gpu_launches": head_extras["launches"],
+            "clocks": hl_clock, "clocks_all_legs": clocks_all, "clocks_legs": clocks_legs,
+            "step_ms_min_max": [min(head_extras["per_step"]), max(head_extras["per_step"])],
         }
+        line.update(head_extras["multi"])
+        if world > 1:
+            import torch.distributed as dist
+            line["process_group"] = {"backend": dist.get_backend(), "nranks": dist.get_world_size(),
+                                     "nccl_version": ".".join(map(str, torch.cuda.nccl.version())) if dist.get_backend() == "nccl" else None}
         print(json.dumps(line), flush=True)
-    barrier(world)      # peers' received buffers stay mapped until rank 0 has finished writing into them
-    rig.close()
+    barrier(world)
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
@@ -909,7 +1319,7 @@ def run_headline(args):
 
 
 # ----------------------------------------------------------------------------------------------
-# the other measurement rows of SURVEY.md §8(d): one JSON line per measurement
+# the deeper measurement rows of SURVEY.md §8(d): one JSON line per measurement
 # ----------------------------------------------------------------------------------------------
 
 
@@ -917,66 +1327,25 @@ def emit(**kw):
     print(json.dumps(kw), flush=True)
 
 
-def run_configs(args):
-    """Every config's kernel, snapshot-off kernel, clip pass, flush, both restore modes."""
-    torch, rank, world, local_rank = gpu_setup()
-    keys = [args.config] if args.config != "c2" else ["c1", "c2", "c3", "c4a", "c4b", "c5"]
-    link = measure_host_link(torch, torch.device(f"cuda:{local_rank}"))
-    peak, _ = measured_peaks()
-    for key in keys:
-        rig = Rig(args, key, host_grads=False)
-        N = rig.N
-        total_ms, per, _ = rig.time_steps(args.steps, max(args.warmup, 3))
-        step_ms = total_ms / args.steps
-        kern_ms = rig.time_fused_kernel_alone(args.steps) if rig.wl.hyper.max_grad_norm > 0 else step_ms
-        off_ms = rig.time_steps_off(args.steps)
-        flush_ms = rig.time_flush()
-        _, r_bulk, rec = rig.restore_timing()
-        B = rig.B
-        replica, back_step = rig.s.replica, rig.step
-        rig.close()
-        # copy-engine restore on a fresh handle bound to the same replica (a replacement rank)
-        r2 = rig.Shard(rig.wl, device=rig.device, restore_mode=B.PHX_RESTORE_COPY_ENGINE, replica=replica)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        r2.restore()
-        e1.record()
-        torch.cuda.synchronize()
-        r_ce = e0.elapsed_time(e1)
-        r2.close()
-        gbs = BYTES_PER_ELEM * N / (kern_ms * 1e-3) / 1e9
-        emit(mode="configs", config=key, elements=int(N), step_ms=step_ms, fused_kernel_ms=kern_ms,
-             fused_gbs=gbs, frac_of_measured_peak=gbs / peak, frac_of_nominal=gbs / NOMINAL_HBM_GBS,
-             elements_per_s=N / (step_ms * 1e-3), snapshot_off_step_ms=off_ms,
-             snapshot_extra_ms=step_ms - off_ms, flush_ms=flush_ms,
-             flush_gbs=rig_bytes(N) / (flush_ms * 1e-3) / 1e9, d2h_peak_gbs=link["d2h_gbs"],
-             restore_bulk_ms=r_bulk, restore_bulk_gbs=12 * N / (r_bulk * 1e-3) / 1e9,
-             restore_copy_engine_ms=r_ce, restore_copy_engine_gbs=12 * N / (r_ce * 1e-3) / 1e9,
-             h2d_peak_gbs=link["h2d_gbs"], recompute_ms=rec,
-             note="c1 fits in L2: reported, not an HBM figure" if key == "c1" else "")
-        del rig, r2, replica
-        torch.cuda.empty_cache()
-    return 0
-
-
 def rig_bytes(N):
     return 256 + 12 * N
 
 
 def run_overlap_curve(args):
-    """Exposed checkpoint ms/iteration against the length of the compute window (R21)."""
-    torch, rank, world, local_rank = gpu_setup()
-    rig = Rig(args, args.config, host_grads=False)
+    """Exposed checkpoint ms/iteration against the length of the compute window (R21), eager and graph-captured."""
+    torch, rank, world, local_rank = gpu_setup(args)
+    rig = Rig(args, args.headline, host_grads=False)
     flush_ms = rig.time_flush()
     gm = rig.gemm_setup()
-    Gs = [int(x) for x in str(args.gemms).split(",")] if args.gemms > 0 else [64, 256, 1024, 4096, 16384]
-    head = rig.headline_gemms(flush_ms)
+    Gs = [args.gemms] if args.gemms > 0 else [64, 256, 1024, 4096, 16384]
+    head = rig.gemms_for(flush_ms)
     for G in sorted(set(Gs + [head])):
-        t_iter = G * gm * 1.2 + 1.0
-        iters = max(5, min(20, int(3000.0 / t_iter)))
-        o = rig.overlap(G, iters, args.overlap_reps)
-        emit(mode="overlap-curve", config=args.config, elements=int(rig.N), flush_ms=flush_ms, headline=(G == head),
+        iters = rig.iters_for(G)
+        o = rig.overlap(G, iters, arms=("off", "staged", "on"), reps=2)
+        if not args.no_graph_step:
+            og = rig.overlap_graph_step(G, iters)
+            o["graph_step"] = {k: og[k] for k in ("iter_ms_off", "iter_ms_on", "exposed_ms", "exposed_frac_of_compute_step")}
+        emit(mode="overlap-curve", config=args.headline, elements=int(rig.N), flush_ms=flush_ms, headline=(G == head),
              knee_gemms=flush_ms / gm, sync_mode=rig.sync_name, depth=rig.depth, chunk_mib=rig.chunk_mib, **o)
     rig.close()
     return 0
@@ -986,18 +1355,17 @@ def run_timeline(args):
     """Copy/compute overlap as a timeline from CUDA events (nsys is not on the image): per iteration, when the
     GEMM window, the hot path (a1-a3) and the side-stream flush (a4+a5) of that iteration's snapshot start and end,
     all in ms since the first iteration's start.  One JSON line per iteration plus a summary."""
-    torch, rank, world, local_rank = gpu_setup()
-    rig = Rig(args, args.config, host_grads=False)
+    torch, rank, world, local_rank = gpu_setup(args)
+    rig = Rig(args, args.headline, host_grads=False)
     flush_ms = rig.time_flush()
     rig.gemm_setup()
     a, b, c = rig._gemm
-    G = args.gemms if args.gemms > 0 else rig.headline_gemms(flush_ms)
+    G = args.gemms if args.gemms > 0 else rig.gemms_for(flush_ms)
     iters, marks = 6, 8
-    E = lambda: torch.cuda.Event(enable_timing=True)
+    E = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
     rows = []
     for _ in range(2):                       # warm-up iterations (not recorded)
-        for _ in range(G):
-            torch.matmul(a, b, out=c)
+        rig.gemm_window(G)
         rig.do_step()
         rig.flush()
     torch.cuda.synchronize()
@@ -1007,8 +1375,7 @@ def run_timeline(args):
         ev = {"gemm": [E()], "k0": E(), "k1": E(), "f0": E(), "f1": E()}
         ev["gemm"][0].record(rig.cur)
         for part in range(marks):
-            for _ in range(G // marks):
-                torch.matmul(a, b, out=c)
+            rig.gemm_window(G // marks)
             e = E()
             e.record(rig.cur)
             ev["gemm"].append(e)
@@ -1021,22 +1388,21 @@ def run_timeline(args):
         rows.append(ev)
     torch.cuda.synchronize()
     rig.s.wait(rig.step)
-    t = lambda e: base.elapsed_time(e)
+    t = lambda e: base.elapsed_time(e)  # noqa: E731
     for it, ev in enumerate(rows):
         # the flush is enqueued behind an event of the step kernel: its real start is max(f0, k1)
-        emit(mode="timeline", config=args.config, iteration=it, gemms=G,
+        emit(mode="timeline", config=args.headline, iteration=it, gemms=G,
              gemm_window_ms=[t(ev["gemm"][0]), t(ev["gemm"][-1])],
              gemm_marks_ms=[t(e) for e in ev["gemm"]],
              hot_path_ms=[t(ev["k0"]), t(ev["k1"])],
              flush_ms=[max(t(ev["f0"]), t(ev["k1"])), t(ev["f1"])])
-    # summary: how much of each flush lies under the NEXT iteration's GEMM window, and the wait at the sync point
     under, waits = [], []
     for it in range(iters - 1):
         f0, f1 = max(t(rows[it]["f0"]), t(rows[it]["k1"])), t(rows[it]["f1"])
         g0, g1 = t(rows[it + 1]["gemm"][0]), t(rows[it + 1]["gemm"][-1])
         under.append(max(0.0, min(f1, g1) - max(f0, g0)) / (f1 - f0))
         waits.append(max(0.0, f1 - t(rows[it + 1]["k0"])))
-    emit(mode="timeline-summary", config=args.config, gemms=G, flush_alone_ms=flush_ms,
+    emit(mode="timeline-summary", config=args.headline, gemms=G, flush_alone_ms=flush_ms,
          flush_fraction_under_next_gemm_window=under, commit_after_next_step_enqueued_ms=waits,
          note="commit_after_next_step_enqueued_ms > 0 would be a stall at the single sync point (PAPER.md:226)")
     rig.close()
@@ -1047,8 +1413,8 @@ def run_sweep(args):
     """BASELINE.json:configs[4]: D2H chunk size 4..256 MiB x staging depth 1..4 (x sync mode), reporting exposed
     checkpoint ms/iteration and host-link GB/s.  Run at a TIGHT compute window (T_c = 1.25 x T_D2H, where depth and
     chunking can matter) and, on a reduced grid, at the headline window (T_c >= 4 x T_D2H)."""
-    torch, rank, world, local_rank = gpu_setup()
-    key = args.config if args.config != "c2" else "c5"
+    torch, rank, world, local_rank = gpu_setup(args)
+    key = args.headline if args.config else "c5"
     device = torch.device(f"cuda:{local_rank}")
     link = measure_host_link(torch, device)
     probe = Rig(args, key, host_grads=False)
@@ -1056,9 +1422,10 @@ def run_sweep(args):
     flush_ref = probe.time_flush()
     gm = probe.gemm_setup()
     G_tight = max(1, int(round(1.25 * flush_ref / gm)))
-    G_head = probe.headline_gemms(flush_ref)
-    base = probe.overlap(G_tight, args.overlap_iters, 1, arms=("off",))
-    base_head = probe.overlap(G_head, max(5, args.overlap_iters // 2), 1, arms=("off",))
+    G_head = probe.gemms_for(flush_ref)
+    it_t, it_h = probe.iters_for(G_tight), max(5, probe.iters_for(G_head) // 2)
+    base = probe.overlap(G_tight, it_t, arms=("off",))
+    base_head = probe.overlap(G_head, it_h, arms=("off",))
     probe.close()
     del probe
     torch.cuda.empty_cache()
@@ -1068,17 +1435,16 @@ def run_sweep(args):
             for chunk in chunks:
                 rig = Rig(args, key, depth=depth, chunk_mib=chunk, sync=sync, replica=replica, host_grads=False)
                 flush_ms = rig.time_flush()
-                o = rig.overlap(G_tight, args.overlap_iters, 1, arms=("on",))
-                row = dict(mode="sweep", window="tight(1.25xT_D2H)", config=key, elements=int(rig.N), sync_mode=sync,
-                           depth=depth, chunk_mib=chunk, flush_ms=flush_ms,
-                           host_link_gbs=rig_bytes(rig.N) / (flush_ms * 1e-3) / 1e9, d2h_peak_gbs=link["d2h_gbs"],
-                           gemms_per_iter=G_tight, iter_ms_on=o["iter_ms_on"], iter_ms_off=base["iter_ms_off"],
-                           exposed_ms=o["iter_ms_on"] - base["iter_ms_off"],
-                           exposed_frac=(o["iter_ms_on"] - base["iter_ms_off"]) / base["iter_ms_off"],
-                           hot_path_ms_in_loop_on=o["hot_path_ms_in_loop_on"])
-                emit(**row)
+                o = rig.overlap(G_tight, it_t, arms=("on",))
+                emit(mode="sweep", window="tight(1.25xT_D2H)", config=key, elements=int(rig.N), sync_mode=sync,
+                     depth=depth, chunk_mib=chunk, flush_ms=flush_ms,
+                     host_link_gbs=rig_bytes(rig.N) / (flush_ms * 1e-3) / 1e9, d2h_peak_gbs=link["d2h_gbs"],
+                     gemms_per_iter=G_tight, iter_ms_on=o["iter_ms_on"], iter_ms_off=base["iter_ms_off"],
+                     exposed_ms=o["iter_ms_on"] - base["iter_ms_off"],
+                     exposed_frac=(o["iter_ms_on"] - base["iter_ms_off"]) / base["iter_ms_off"],
+                     hot_path_ms_in_loop_on=o["hot_path_ms_in_loop_on"])
                 if depth in (1, 2) and chunk in (chunks[0], 64, 256):
-                    o = rig.overlap(G_head, max(5, args.overlap_iters // 2), 1, arms=("on",))
+                    o = rig.overlap(G_head, it_h, arms=("on",))
                     emit(mode="sweep", window="headline(>=4xT_D2H)", config=key, elements=int(rig.N), sync_mode=sync,
                          depth=depth, chunk_mib=chunk, flush_ms=flush_ms, gemms_per_iter=G_head,
                          iter_ms_on=o["iter_ms_on"], iter_ms_off=base_head["iter_ms_off"],
@@ -1091,76 +1457,14 @@ def run_sweep(args):
     return 0
 
 
-def run_hotswap(args):
-    """BASELINE.json:configs[3]: 20 steps with snapshots, drop the live shard while step 21 is in flight, restore
-    from the pinned host replica, recompute step 21, run 22..25; time restore + recompute and check the trajectory
-    bit-exactly against an uninterrupted run (GPU vs GPU; GPU vs oracle is in tests/)."""
-    torch, rank, world, local_rank = gpu_setup()
-    keys = [args.config] if args.config != "c2" else ["c4a", "c4b"]
-    for key in keys:
-        for rmode_name in ("bulk_kernel", "copy_engine"):
-            from paper_2607_01646_b200 import binding as B
-            rmode = B.PHX_RESTORE_BULK_KERNEL if rmode_name == "bulk_kernel" else B.PHX_RESTORE_COPY_ENGINE
-            rig = Rig(args, key, host_grads=False, restore_mode=rmode)
-            W, wl, N = rig.W, rig.wl, rig.N
-            G = rig.headline_gemms(rig.time_flush(), factor=1.25)
-            rig.s.p.copy_(W.init_params(rig.s.n, N, wl.seed, device=rig.device))
-            rig.s.m.zero_(); rig.s.v.zero_()
-            rig.s.set_state(0)
-            rig.step = 0
-            a, b, c = rig._gemm
-            # uninterrupted reference trajectory first (snapshot-off handle on its own arrays)
-            ref = rig.Shard(wl, device=rig.device, snapshot=False)
-            ref.p.copy_(rig.s.p); ref.set_state(0)
-            for t in range(1, 26):
-                ref.step_and_snapshot(rig.grads[t & 1], t)
-            torch.cuda.synchronize()
-            for t in range(1, 21):                       # 20 steps, snapshot + flush every step, overlapped
-                for _ in range(G):
-                    torch.matmul(a, b, out=c)
-                rig.do_step()
-                rig.s.flush_async(rig.side)
-            rig.do_step()                                # step 21 launched: in flight when the fault hits
-            torch.cuda.synchronize()
-            rig.s.drop_live()
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            r0, r1, r2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
-            r0.record(rig.cur)
-            back = rig.s.restore()
-            r1.record(rig.cur)
-            rig.step = back
-            rig.do_step()                                # recompute of the in-flight step (a7)
-            r2.record(rig.cur)
-            torch.cuda.synchronize()
-            wall_ms = (time.perf_counter() - t0) * 1e3
-            for t in range(22, 26):
-                rig.do_step()
-                rig.s.flush_async(rig.side)
-            rig.s.wait(25)
-            torch.cuda.synchronize()
-            same = all(torch.equal(x, y) for x, y in ((rig.s.p, ref.p), (rig.s.m, ref.m), (rig.s.v, ref.v),
-                                                      (rig.s.p16, ref.p16)))
-            rms = r0.elapsed_time(r1)
-            emit(mode="hotswap", config=key, elements=int(N), restore_mode=rmode_name, restored_step=int(back),
-                 restore_ms=rms, recompute_ms=r1.elapsed_time(r2), restore_plus_recompute_wall_ms=wall_ms,
-                 host_link_gbs=12 * N / (rms * 1e-3) / 1e9, trajectory_bit_exact_vs_uninterrupted=bool(same),
-                 steps_before_fault=20, steps_after=5, gemms_per_iter=G)
-            ref.close()
-            rig.close()
-            del rig, ref
-            torch.cuda.empty_cache()
-            if not same:
-                return 1
-    return 0
-
-
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return self_spawn(args)
     if args.impl == "reference":
         return run_reference(args)
-    return {"headline": run_headline, "configs": run_configs, "overlap-curve": run_overlap_curve,
-            "sweep": run_sweep, "hotswap": run_hotswap, "timeline": run_timeline}[args.mode](args)
+    return {"headline": run_headline, "overlap-curve": run_overlap_curve, "sweep": run_sweep,
+            "timeline": run_timeline}[args.mode](args)
 
 
 if __name__ == "__main__":

@@ -29,6 +29,13 @@ def gather_partials(local, group=None):
     if not (dist.is_available() and dist.is_initialized()):
         return local.reshape(1).clone()
     world = dist.get_world_size(group)
+    if local.is_cuda and dist.get_backend(group) != "nccl":
+        # a gloo control plane (CPU tests; bench.py --debug-shared-gpu) cannot all-gather device tensors: stage
+        # the 8 bytes through the host.  This synchronises the host with the stream — a functional path only;
+        # on a GPU box the group is NCCL and the exchange is enqueued on the step's stream.
+        host = torch.empty(world, dtype=torch.float64)
+        dist.all_gather_into_tensor(host, local.reshape(1).cpu(), group=group)
+        return host.to(local.device)
     out = torch.empty(world, dtype=torch.float64, device=local.device)
     dist.all_gather_into_tensor(out, local.reshape(1), group=group)
     return out

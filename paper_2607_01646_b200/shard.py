@@ -98,6 +98,35 @@ class Shard:
         k = step % 2
         return self.replica[k * self.info.host_slot_stride: k * self.info.host_slot_stride + self.info.host_snapshot_bytes]
 
+    # -- the graph-capturable form (include/phx.h "graph") --------------------------------
+    def graph_begin(self, stream=None, hyper: Optional[Hyper] = None):
+        hp = hyper or self.hyper
+        B.phx_graph_begin(self.h, hp.lr, hp.beta1, hp.beta2, hp.eps, hp.wd,
+                          stream or torch.cuda.current_stream(self.device))
+
+    def graph_set_hyper(self, hyper: Hyper, stream=None):
+        B.phx_graph_set_hyper(self.h, hyper.lr, hyper.beta1, hyper.beta2, hyper.eps, hyper.wd,
+                              stream or torch.cuda.current_stream(self.device))
+
+    def graph_step(self, grads: torch.Tensor, stream=None):
+        assert grads.numel() == self.n_padded and grads.is_cuda
+        B.phx_graph_step_and_snapshot(self.h, grads, stream or torch.cuda.current_stream(self.device))
+
+    def graph_flush(self, side_stream):
+        B.phx_graph_flush_async(self.h, side_stream)
+
+    def graph_end(self) -> int:
+        return B.phx_graph_end(self.h)
+
+    # -- SURVEY 8(f4) second half: the gradient producer's epilogue -------------------------
+    def grads_finalize(self, main_grads_fp32: torch.Tensor, scale: float, grads_bf16_out: torch.Tensor,
+                       sumsq_out: torch.Tensor, stream=None):
+        assert main_grads_fp32.dtype == torch.float32 and grads_bf16_out.dtype == torch.bfloat16
+        assert main_grads_fp32.numel() == self.n_padded == grads_bf16_out.numel()
+        assert sumsq_out.dtype == torch.float64 and sumsq_out.is_cuda
+        B.phx_grads_finalize_async(self.h, main_grads_fp32, scale, grads_bf16_out, sumsq_out,
+                                   stream or torch.cuda.current_stream(self.device))
+
     def params_ready(self, stream=None):
         B.phx_params_ready(self.h, stream or torch.cuda.current_stream(self.device))
 

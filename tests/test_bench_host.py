@@ -42,7 +42,57 @@ def test_reference_arm_prints_one_valid_json_line():
     assert d["impl"] == "reference" and d["metric"] == bench.METRIC and d["unit"] == "GB/s"
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"] > 0
-    assert d["config"]["workload"].startswith("c2") and d["steps"] == 2
+    assert d["config"]["workload"].startswith("c3") and d["steps"] == 2      # the headline config (largest single-GPU)
+    # the oracle runs the WHOLE step of that config: a1 (clip) + a3 => 42 algorithmic bytes per element
+    assert d["cpu_baseline"]["bytes_per_element"] == 42 and d["cpu_baseline"]["sample_elements"] == 200000
+    assert d["cpu_baseline"]["value"] == d["value"]
+
+
+def test_plain_launch_with_gpus_2_starts_two_ranks_and_prints_one_line():
+    """`python bench.py --gpus 2` launched PLAINLY (no torchrun) must start 2 ranks by itself and
+    yield exactly one line with n_gpus = 2 (reference arm: rank 0 alone works, the other rank exits 0)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference", "--steps", "1",
+                        "--warmup", "1", "--cpu-sample", "100000"], capture_output=True, text=True, timeout=900, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.strip().startswith("{")]
+    assert len(lines) == 1, r.stdout
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["impl"] == "reference"
+
+
+def test_plain_launch_refuses_more_gpus_than_the_box_has():
+    if torch.cuda.is_available() and torch.cuda.device_count() >= 64:
+        pytest.skip("a box with 64 GPUs")
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "64"], capture_output=True, text=True,
+                       timeout=300, env=env)
+    assert r.returncode != 0 and "CUDA device" in (r.stderr + r.stdout)
+    assert not [l for l in r.stdout.splitlines() if l.strip().startswith("{")]        # no line, no silent 1-GPU run
+
+
+def test_step_bytes_per_element_counts_the_clip_pass():
+    import argparse
+    a = argparse.Namespace(precision="bf16", decay_groups=False)
+    assert bench.step_bytes_per_elem(bench.workload_of(a, "c3")) == 42          # a1 (2) + a3 (40)
+    assert bench.step_bytes_per_elem(bench.workload_of(a, "c2")) == 40
+    assert bench.step_bytes_per_elem(bench.workload_of(a, "c3"), clip_pass=False) == 40
+    assert bench.step_bytes_per_elem(bench.workload_of(a, "c2"), source="direct") == 28
+    a32 = argparse.Namespace(precision="fp32", decay_groups=False)
+    assert bench.step_bytes_per_elem(bench.workload_of(a32, "c3")) == 44        # fp32 gradients: 4-byte a1 read
+
+
+def test_clock_log_cuts_samples_into_legs(tmp_path):
+    f = tmp_path / "smi.csv"
+    f.write_text("2026/11/04 10:00:00.000, 1965, 1965, 400.1, Not Active, Not Active, Not Active, Not Active\n"
+                 "2026/11/04 10:00:00.050, 1700, 1965, 900.5, Not Active, Not Active, Not Active, Active\n"
+                 "garbage line\n"
+                 "2026/11/04 10:00:01.000, 1500, 1965, 950.0, Active, Not Active, Not Active, Not Active\n")
+    rows = bench.ClockLog._parse(str(f))
+    assert len(rows) == 3 and rows[1][1] == 1700.0 and rows[1][4] == [False, False, False, True]
+    s = bench.ClockLog._summary(rows[:2])
+    assert s["samples"] == 2 and s["reasons"] == ["sw_power_cap"] and s["sm_max_mhz"] == 1965.0 and s["sm_min_mhz"] == 1700.0
+    assert bench.ClockLog._summary([])["samples"] == 0
 
 
 def test_reference_arm_under_two_ranks_only_rank0_prints():

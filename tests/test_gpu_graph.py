@@ -1,0 +1,167 @@
+"""GPU parity for the graph-capturable form (include/phx.h "graph"): the device-side derivation
+of the per-step scalars equals the oracle's bitwise, and a CAPTURED (compute window + flush + step) graph
+replayed for many iterations leaves exactly the oracle's state, staging bytes and committed host slots."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2607_01646_b200 import binding as B
+from paper_2607_01646_b200 import workloads as W
+
+from gpu_util import DEV, assert_state_equal, hp_of, make_pair
+
+pytestmark = pytest.mark.gpu
+
+
+def test_device_derived_scalars_equal_the_oracle_for_steps_up_to_a_million():
+    rng = np.random.default_rng(3)
+    steps = sorted(set([1, 2, 3, 4, 5, 7, 10, 100, 1000, 65535, 65536, 10**6, 2**40 + 3]
+                       + [int(x) for x in rng.integers(1, 10**6, 4000)]))
+    for lr, b1, b2, wd in ((3e-4, 0.9, 0.95, 0.1), (1e-3, 0.9, 0.999, 0.01), (6e-4, 0.8, 0.98, 0.0)):
+        got = np.array(B.phx_derived_scalars_device(lr, b1, b2, wd, steps), np.float32).view(np.uint32)
+        for i, t in enumerate(steps):
+            exp = O.scalars(lr, b1, b2, 1e-8, wd, t).view(np.uint32)
+            assert np.array_equal(got[i], exp), (lr, b1, b2, wd, t)
+            host = np.array(B.phx_derived_scalars_host(lr, b1, b2, wd, t), np.float32).view(np.uint32)
+            assert np.array_equal(host, exp)
+
+
+@pytest.mark.parametrize("source", [B.PHX_SNAPSHOT_STAGED, B.PHX_SNAPSHOT_DIRECT])
+@pytest.mark.parametrize("clip", [0.0, 0.02])
+def test_eager_calls_of_the_graph_form_match_the_oracle(source, clip):
+    wl = W.tiny_workload([300_000, 77, 12_345], dp_size=1, hyper=W.Hyper(max_grad_norm=clip))
+    s, o, gdev, gbits = make_pair(wl, steps=6, chunk_bytes=256 << 10, snapshot_source=source, user=b"graph-user")
+    side = torch.cuda.Stream(device=DEV)
+    hp = hp_of(wl)
+    s.step_and_snapshot(gdev[0], 1)                   # eager step; its snapshot becomes the graph form's first flush
+    o.step(gbits[0], **hp, step=1); o.snapshot()
+    s.graph_begin()
+    with pytest.raises(B.PhxError) as e:
+        s.step_and_snapshot(gdev[1], 2)
+    assert e.value.code == B.PHX_ERR_GRAPH_MODE
+    for t in range(2, 6):
+        s.graph_flush(side)                           # flush of snapshot t-1
+        s.graph_step(gdev[t - 1])
+        o.step(gbits[t - 1], **hp, step=t); o.snapshot()
+    assert s.graph_end() == 5
+    assert_state_equal(s, o, "graph form, eager")
+    assert np.array_equal(s.replica_slot(4).numpy(), o.replica[0])
+    assert np.array_equal(s.replica_slot(3).numpy(), o.replica[1])     # slot 1 holds step 3 (step 5 not flushed yet)
+    if source == B.PHX_SNAPSHOT_STAGED:
+        assert np.array_equal(s.staging_slot(5).cpu().numpy(), o.packed_snapshot())
+    s.flush_async(side)                               # back in the eager form: the still-staged newest snapshot
+    s.wait(5)
+    assert np.array_equal(s.replica_slot(5).numpy(), o.replica[1])
+    s.step_and_snapshot(gdev[5], 6)                   # and the eager step continues at last_step + 1
+    o.step(gbits[5], **hp, step=6)
+    assert_state_equal(s, o, "eager after graph_end")
+    s.drop_live()
+    assert s.restore() == 5 and B.phx_restored_user_metadata(s.h) == b"graph-user"
+    s.close()
+
+
+@pytest.mark.parametrize("mode,depth", [(B.PHX_SYNC_STRICT, 2), (B.PHX_SYNC_RELAXED, 2), (B.PHX_SYNC_STRICT, 1),
+                                        (B.PHX_SYNC_RELAXED, 4)])
+def test_captured_graph_replayed_ten_iterations_is_bit_exact(mode, depth):
+    """a captured (GEMM window + flush(k-1) + step k) x L graph, L = lcm(depth, 2) iterations,
+    replayed until 10+ iterations have run, against the oracle stepping 10+ times."""
+    wl = W.CONFIGS["c1"]
+    L = {1: 2, 2: 2, 4: 4}[depth]
+    reps = (10 + L - 1) // L
+    s, o, _, _ = make_pair(wl, steps=0, chunk_bytes=1 << 20, staging_depth=depth, sync_mode=mode)
+    hp = hp_of(wl)
+    # the graph reads the gradients of iteration i from a fixed buffer: L buffers, refilled between replays
+    gbuf = [torch.zeros(s.n_padded, dtype=torch.bfloat16, device=DEV) for _ in range(L)]
+    a = torch.randn(512, 512, device=DEV, dtype=torch.bfloat16)
+    c = torch.empty_like(a)
+    cap = torch.cuda.Stream(device=DEV)
+    side = torch.cuda.Stream(device=DEV)
+    # one eager step of the graph form first, so that the first captured flush has a snapshot to send
+    osegs = [(tid, off, ln) for tid, _, off, ln in o.segments]
+    g1 = W.gen_grads(wl, osegs, s.n_padded, 1, wl.seed)
+    s.graph_begin(stream=cap)
+    gbuf[1 % L].copy_(g1)
+    torch.cuda.synchronize()
+    s.graph_step(gbuf[1 % L], stream=cap)
+    o.step(g1.view(torch.int16).numpy().view(np.uint16).copy(), **hp, step=1); o.snapshot()
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=cap):
+        for i in range(L):
+            t = 2 + i                                  # issue index at capture: 2 .. L+1
+            side.wait_stream(cap)                      # fork: the flush of snapshot t-1 runs beside the window
+            s.graph_flush(side)
+            for _ in range(4):
+                torch.matmul(a, a, out=c)              # the stand-in compute window
+            s.graph_step(gbuf[t % L], stream=cap)      # a2 joins the side stream back, then prologue + fused kernel
+        cap.wait_stream(side)                          # relaxed mode: the last flush may not be joined by any a2
+    t = 1
+    for _ in range(reps):
+        for i in range(L):
+            t += 1
+            g = W.gen_grads(wl, osegs, s.n_padded, t, wl.seed)
+            gbuf[t % L].copy_(g)
+            o.step(g.view(torch.int16).numpy().view(np.uint16).copy(), **hp, step=t)
+            o.snapshot()
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert_state_equal_live(s, o, f"after replay ending at step {t}")
+    assert s.graph_end() == t and t >= 11
+    assert_state_equal(s, o, "graph replays")
+    # every flush inside the graph committed: host slots hold steps t-1 (newest flushed) and t-2
+    assert np.array_equal(s.replica_slot(t - 1).numpy(), o_slot_of(o, wl, hp, t - 1))
+    s.flush_async(side)
+    s.wait(t)
+    assert np.array_equal(s.replica_slot(t).numpy(), o.replica[t % 2])
+    s.close()
+
+
+def assert_state_equal_live(s, o, what):
+    for name, dev, ref in (("p", s.p, o.p), ("m", s.m, o.m), ("v", s.v, o.v)):
+        assert np.array_equal(dev.cpu().numpy().view(np.uint32), ref.view(np.uint32)), (what, name)
+
+
+def o_slot_of(o, wl, hp, step):
+    """The oracle's replica slot of `step` — still intact in slot step % 2 because the oracle snapshotted every step
+    and only step+1 (other parity) came after it."""
+    h = O.parse_header(o.replica[step % 2][:256].tobytes())
+    assert h is not None and h["step"] == step
+    return o.replica[step % 2]
+
+
+def test_misaligned_replay_is_reported():
+    wl = W.tiny_workload([8192], dp_size=1)
+    s, o, gdev, _ = make_pair(wl, steps=3)
+    cap = torch.cuda.Stream(device=DEV)
+    s.graph_begin(stream=cap)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=cap):
+        s.graph_step(gdev[0], stream=cap)              # ONE step captured with depth 2: every second replay is misaligned
+    graph.replay(); graph.replay()
+    with pytest.raises(B.PhxError) as e:
+        s.graph_end()
+    assert e.value.code == B.PHX_ERR_STEP_ORDER
+    assert B.phx_last_step(s.h) == 2                   # the device counter is still the truth
+    s.close()
+
+
+def test_graph_form_protocol_errors():
+    wl = W.tiny_workload([8192], dp_size=1)
+    s, _, gdev, _ = make_pair(wl, steps=1)
+    L = B.lib()
+    assert L.phx_graph_step_and_snapshot(s.h, gdev[0].data_ptr(), None) == B.PHX_ERR_GRAPH_MODE
+    assert L.phx_graph_flush_async(s.h, None) == B.PHX_ERR_GRAPH_MODE
+    assert L.phx_graph_end(s.h, None) == B.PHX_ERR_GRAPH_MODE
+    s.graph_begin()
+    assert L.phx_graph_begin(s.h, 1e-3, 0.9, 0.95, 1e-8, 0.0, None) == B.PHX_ERR_GRAPH_MODE
+    assert L.phx_graph_flush_async(s.h, None) == B.PHX_ERR_NO_FLUSH_PENDING
+    assert L.phx_restore(s.h, None, None) == B.PHX_ERR_GRAPH_MODE
+    assert L.phx_graph_step_and_snapshot(s.h, gdev[0].data_ptr() + 2, None) == B.PHX_ERR_ALIGNMENT
+    assert s.graph_end() == 0
+    s.close()
+    full = B.phx_shard_create([(8192, 0)], 1, 0, payload=B.PHX_PAYLOAD_FULL_RANK_STATE)
+    assert L.phx_graph_begin(full, 1e-3, 0.9, 0.95, 1e-8, 0.0, None) == B.PHX_ERR_NOT_BOUND
+    B.phx_shard_destroy(full)

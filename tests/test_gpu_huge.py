@@ -1,6 +1,7 @@
 """Maximum-size edge case: a shard with MORE THAN 2^32 elements (64-bit element indexing everywhere: the fused
-kernel, the staging planes, the sum of squares) — sampled element-by-element parity with the oracle around the
-2^31 and 2^32 boundaries and the ragged tail, plus whole-array properties.  ~122 GB of the 180 GB HBM; no host
+kernel, the staging planes, the sum of squares) — element-by-element parity with the oracle on sampled windows
+around the 2^31 and 2^32 boundaries and the ragged tail AND on a dense block of 2^28 elements straddling element
+2^32 (every element of p, m, v, bf16 copy and staging planes), plus whole-array properties.  ~122 GB of the 180 GB HBM; no host
 replica (2 x 52 GB of pinned memory is not a test-box assumption), so the snapshot is checked in the staging slot."""
 import numpy as np
 import pytest
@@ -54,6 +55,13 @@ def test_more_than_2_pow_32_elements_sampled_parity():
     idx = torch.cat([torch.arange(a, b, device=DEV) for a, b in wins])
     ref = dict(p=p[idx].cpu().numpy().copy(), m=np.zeros(idx.numel(), np.float32),
                v=np.zeros(idx.numel(), np.float32), h=np.zeros(idx.numel(), np.uint16))
+    # dense block: the last 2^28 elements, [N - 2^28, N), which straddle element 2^32
+    import os
+    cores = len(os.sched_getaffinity(0))
+    dlo = N - (1 << 28)
+    assert dlo < (1 << 32) < N
+    dense = dict(p=p[dlo:].cpu().numpy().copy(), m=np.zeros(1 << 28, np.float32), v=np.zeros(1 << 28, np.float32),
+                 h=np.zeros(1 << 28, np.uint16))
     hp = dict(lr=3e-4, beta1=0.9, beta2=0.95, eps=1e-8, wd=0.1)
     for t in (1, 2):
         _fill_normal(g, 1e-3, 100 + t)
@@ -73,6 +81,15 @@ def test_more_than_2_pow_32_elements_sampled_parity():
         assert np.array_equal(m[idx].cpu().numpy().view(np.uint32), ref["m"].view(np.uint32)), t
         assert np.array_equal(v[idx].cpu().numpy().view(np.uint32), ref["v"].view(np.uint32)), t
         assert np.array_equal(bits16(p16[idx]), ref["h"]), t
+        # the dense block, every element (byte offsets of the staging planes beyond 2^34)
+        O.adamw_step(dense["p"], dense["m"], dense["v"], bits16(g[dlo:]).copy(), dense["h"], **hp, step=t,
+                     coef=float(coef), nthreads=cores)
+        for name, dev in (("p", p), ("m", m), ("v", v)):
+            assert torch.equal(dev[dlo:].view(torch.int32).cpu(), torch.from_numpy(dense[name].view(np.int32))), (t, name)
+        assert torch.equal(p16[dlo:].view(torch.int16).cpu(), torch.from_numpy(dense["h"].view(np.int16))), t
+        for k, name in enumerate("pmv"):
+            st = staging[256 + 4 * (k * N + dlo):256 + 4 * (k + 1) * N].view(torch.int32).cpu()
+            assert torch.equal(st, torch.from_numpy(dense[name].view(np.int32))), (t, "staging", name)
         # whole-array properties: staging planes == live planes, bf16 copy == RNE(p), header describes the shard
         CH = 1 << 28
         for o in range(0, N, CH):

@@ -233,10 +233,13 @@ def test_depth_and_sync_modes(mode, depth):
 
 
 @pytest.mark.parametrize("rmode", [B.PHX_RESTORE_BULK_KERNEL, B.PHX_RESTORE_COPY_ENGINE])
-def test_torn_flush_is_never_chosen(rmode):
+@pytest.mark.parametrize("depth", [2, 3, 4])
+@pytest.mark.parametrize("j", [0, 1, 5, 27, 28])     # 28 payload chunks: nothing, one, some, all but one, ALL (no header)
+def test_torn_flush_is_never_chosen(rmode, depth, j):
     wl = W.tiny_workload([300_000], dp_size=1)
     s, o, gdev, gbits = make_pair(wl, steps=4, chunk_bytes=128 << 10, restore_mode=rmode,
-                                  sync_mode=B.PHX_SYNC_RELAXED)
+                                  sync_mode=B.PHX_SYNC_RELAXED, staging_depth=depth)
+    assert -(-(s.info.snapshot_bytes - 256) // (128 << 10)) == 28
     side = side_stream()
     hp = hp_of(wl)
     for t in (1, 2):
@@ -244,9 +247,9 @@ def test_torn_flush_is_never_chosen(rmode):
         o.step(gbits[t - 1], **hp, step=t); o.snapshot()
     s.step_and_snapshot(gdev[2], 3)
     o.step(gbits[2], **hp, step=3)
-    B.phx_fault_inject_torn_flush(s.h, 5)        # flush(3) dies after 5 of 28 payload chunks
+    B.phx_fault_inject_torn_flush(s.h, j)        # flush(3) dies after j of 28 payload chunks
     s.flush_async(side)
-    o.snapshot(abort_after_chunks=5)
+    o.snapshot(abort_after_chunks=j)
     with pytest.raises(B.PhxError) as e:
         s.wait(3)
     assert e.value.code == B.PHX_ERR_CORRUPT_SLOT

@@ -253,3 +253,30 @@ def test_ring_peers_still_receive_the_optimizer_only_payload():
     for rb in recv:
         rb.free()
     close_all(shards)
+
+
+def test_full_payload_under_relaxed_sync_never_commits_a_W_of_the_next_step():
+    """the full-rank-state flush reads the LIVE W, and the rank's own range of W is d_p_bf16,
+    which step k+1's kernel rewrites.  Under PHX_SYNC_RELAXED (depth 3) with a slow flush (4 KiB chunks) and steps
+    issued back to back WITHOUT phx_params_guard, every committed host slot must still hold the W of exactly its
+    own step: the step waits until the newest flush has finished reading W."""
+    wls, shards, ranks = build_group([600_000, 77], 1, chunk=4096, sync_mode=B.PHX_SYNC_RELAXED, staging_depth=3)
+    wl, s, fr = wls[0], shards[0], ranks[0]
+    side = torch.cuda.Stream(device=DEV)
+    snaps = {}
+    grads = [W.gen_grads(wl, s.segments, s.n_padded, t, seed=11).to(DEV) for t in range(1, 7)]
+    torch.cuda.synchronize()
+    for t in range(1, 7):
+        s.step_and_snapshot(grads[t - 1], t)          # no guard, no host sync: the hazard window is wide open
+        s.params_ready()
+        s.flush_async(side)                           # ~2300 small copies, W first
+        fr.o.step(grad_record(grads[t - 1]), **hp_of(wl), step=t)
+        fr.W[:] = R.publish([fr.o])
+        fr.snapshot()
+        snaps[t] = fr.slots[t % 2].copy()
+    s.wait(6)
+    torch.cuda.synchronize()
+    for t in (5, 6):
+        assert np.array_equal(s.replica_slot(t).numpy(), snaps[t]), t
+    assert_state_equal(s, fr.o, "full + relaxed")
+    close_all(shards)
