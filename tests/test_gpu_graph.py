@@ -40,14 +40,16 @@ def test_eager_calls_of_the_graph_form_match_the_oracle(source, clip):
     with pytest.raises(B.PhxError) as e:
         s.step_and_snapshot(gdev[1], 2)
     assert e.value.code == B.PHX_ERR_GRAPH_MODE
+    snaps = {1: o.replica[1].copy()}
     for t in range(2, 6):
         s.graph_flush(side)                           # flush of snapshot t-1
         s.graph_step(gdev[t - 1])
         o.step(gbits[t - 1], **hp, step=t); o.snapshot()
+        snaps[t] = o.replica[t % 2].copy()
     assert s.graph_end() == 5
     assert_state_equal(s, o, "graph form, eager")
-    assert np.array_equal(s.replica_slot(4).numpy(), o.replica[0])
-    assert np.array_equal(s.replica_slot(3).numpy(), o.replica[1])     # slot 1 holds step 3 (step 5 not flushed yet)
+    assert np.array_equal(s.replica_slot(4).numpy(), snaps[4])
+    assert np.array_equal(s.replica_slot(3).numpy(), snaps[3])         # slot 1 holds step 3 (step 5 not flushed yet)
     if source == B.PHX_SNAPSHOT_STAGED:
         assert np.array_equal(s.staging_slot(5).cpu().numpy(), o.packed_snapshot())
     s.flush_async(side)                               # back in the eager form: the still-staged newest snapshot
@@ -77,6 +79,9 @@ def test_captured_graph_replayed_ten_iterations_is_bit_exact(mode, depth):
     c = torch.empty_like(a)
     cap = torch.cuda.Stream(device=DEV)
     side = torch.cuda.Stream(device=DEV)
+    with torch.cuda.stream(cap):
+        torch.matmul(a, a, out=c)                      # cuBLAS must be initialised on this stream before a capture
+    torch.cuda.synchronize()
     # one eager step of the graph form first, so that the first captured flush has a snapshot to send
     osegs = [(tid, off, ln) for tid, _, off, ln in o.segments]
     g1 = W.gen_grads(wl, osegs, s.n_padded, 1, wl.seed)
