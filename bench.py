@@ -818,7 +818,7 @@ class Rig:
             out["exposed_ms_kernel_only"] = t["staged"] - t["off"]
         return out
 
-    def overlap_graph_step(self, G, iters, warm=1):
+    def overlap_graph_step(self, G, iters, warm=1, arms=("off", "on")):
         """The same experiment with the WHOLE iteration captured in a CUDA graph — the B200-native launch form
         (DESIGN.md §12): [flush of snapshot k-1 on the side stream ‖ G GEMMs] -> step k, two iterations per graph
         (staging / host slot ping-pong), through the graph-capturable form of the step (phx_graph_*).  Arms:
@@ -830,7 +830,7 @@ class Rig:
         cap = torch.cuda.Stream(device=self.device)
         res = {}
         nrep = max(4, (iters + 1) // 2)
-        for arm in ("off", "on"):
+        for arm in arms:
             h = self.off_shard() if arm == "off" else self.s.h
             with torch.cuda.stream(cap):
                 self.gemm_window(2)                                      # cuBLAS handle / workspace of this stream exist before capture
@@ -867,9 +867,14 @@ class Rig:
             else:
                 self.off_step = last
             del graph
-        return {"gemms_per_iter": G, "compute_window_ms": G * self.gemm_ms, "launch": "cuda graph (2 iterations per graph)",
-                "iters_per_arm": 2 * nrep, "iter_ms_off": res["off"], "iter_ms_on": res["on"],
-                "exposed_ms": res["on"] - res["off"], "exposed_frac_of_compute_step": (res["on"] - res["off"]) / res["off"]}
+        out = {"gemms_per_iter": G, "compute_window_ms": G * self.gemm_ms, "launch": "cuda graph (2 iterations per graph)",
+               "iters_per_arm": 2 * nrep}
+        for arm in arms:
+            out[f"iter_ms_{arm}"] = res[arm]
+        if "on" in res and "off" in res:
+            out["exposed_ms"] = res["on"] - res["off"]
+            out["exposed_frac_of_compute_step"] = (res["on"] - res["off"]) / res["off"]
+        return out
 
     def close(self):
         self.close_peers()
@@ -898,7 +903,7 @@ def measure_host_link(torch, device, nbytes=1 << 30, reps=5):
     return out
 
 
-def measure_hbm_mix_ceiling(torch, device, plane_elems, reps=60):
+def measure_hbm_mix_ceiling(torch, device, plane_elems, reps=150):
     """No-arithmetic streaming passes with the fused kernel's access pattern (libphx_probe.so, bench-only): the HBM
     ceiling for a read:write mix.  Returns GB/s per mix; planes of `plane_elems` fp32 each (larger than L2)."""
     from paper_2607_01646_b200 import probe as PB
@@ -1057,7 +1062,7 @@ def measure_c5_grid(args, link, clk, replica, flush_ref):
     default line (the full 7 x 4 x 2 grid is `--mode sweep`)."""
     import torch
     cells = []
-    base = None
+    base = base_g = None
     for sync, depth, chunk in [("strict", 2, 4), ("strict", 2, 16), ("strict", 2, 64), ("strict", 2, 256),
                                ("strict", 1, 8), ("relaxed", 4, 8), ("relaxed", 4, 64), ("relaxed", 3, 256)]:
         rig = Rig(args, "c5", depth=depth, chunk_mib=chunk, sync=sync, replica=replica, host_grads=False)
@@ -1066,12 +1071,20 @@ def measure_c5_grid(args, link, clk, replica, flush_ref):
         iters = max(8, min(16, rig.iters_for(G)))
         if base is None:
             base = rig.overlap(G, iters, arms=("off",))["iter_ms_off"]
+            if not args.no_graph_step:
+                base_g = rig.overlap_graph_step(G, 8, arms=("off",))["iter_ms_off"]
         fl = rig.time_flush()
         o = rig.overlap(G, iters, arms=("on",))
-        cells.append({"sync_mode": sync, "depth": depth, "chunk_mib": chunk, "flush_ms": fl,
-                      "host_link_gbs": (256 + 12 * rig.N) / (fl * 1e-3) / 1e9, "gemms_per_iter": G,
-                      "iter_ms_on": o["iter_ms_on"], "iter_ms_off": base, "exposed_ms": o["iter_ms_on"] - base,
-                      "exposed_pct": 100.0 * (o["iter_ms_on"] - base) / base})
+        cell = {"sync_mode": sync, "depth": depth, "chunk_mib": chunk, "flush_ms": fl,
+                "host_link_gbs": (256 + 12 * rig.N) / (fl * 1e-3) / 1e9, "gemms_per_iter": G,
+                "iter_ms_on": o["iter_ms_on"], "iter_ms_off": base, "exposed_ms": o["iter_ms_on"] - base,
+                "exposed_pct": 100.0 * (o["iter_ms_on"] - base) / base}
+        if base_g is not None and depth in (1, 2):          # the captured sequence here spans 2 steps = lcm(depth, 2)
+            og = rig.overlap_graph_step(G, 8, arms=("on",))
+            cell.update(iter_ms_on_graph_step=og["iter_ms_on"], iter_ms_off_graph_step=base_g,
+                        exposed_ms_graph_step=og["iter_ms_on"] - base_g,
+                        exposed_pct_graph_step=100.0 * (og["iter_ms_on"] - base_g) / base_g)
+        cells.append(cell)
         rig.close()
         del rig
         torch.cuda.empty_cache()
