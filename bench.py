@@ -65,7 +65,7 @@ def parse_args(argv=None):
     ap.add_argument("--config", default="", help="shorthand for --configs X --headline X")
     ap.add_argument("--headline", default=HEADLINE, help="config `value` / `roofline` / `e2e` are quoted on")
     ap.add_argument("--depth", type=int, default=2)
-    ap.add_argument("--chunk-mib", type=int, default=8)
+    ap.add_argument("--chunk-mib", type=int, default=32)
     ap.add_argument("--sync", default="strict", choices=["strict", "relaxed"])
     ap.add_argument("--gemms", type=int, default=0, help="GEMMs per overlapped iteration (0 = auto: T_c >= 4 T_D2H)")
     ap.add_argument("--overlap-secs", type=float, default=4.5, help="time budget per overlap arm (sets the iteration count)")
@@ -76,8 +76,9 @@ def parse_args(argv=None):
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-mix-ceiling", action="store_true", help="skip the no-arithmetic HBM mix-ceiling probe")
     ap.add_argument("--no-grid", action="store_true", help="skip the c5 chunk x depth grid")
+    ap.add_argument("--no-direct", action="store_true", help="skip the PHX_SNAPSHOT_DIRECT repeat on the headline config")
     ap.add_argument("--cpu-sample", type=int, default=0, help="elements the oracle is timed on (0 = %d)" % ORACLE_SAMPLE)
-    ap.add_argument("--mode", default="headline", choices=["headline", "overlap-curve", "sweep", "timeline"],
+    ap.add_argument("--mode", default="headline", choices=["headline", "overlap-curve", "sweep", "timeline", "probe"],
                     help="headline: the ONE contract line (default).  The others print one JSON line per measurement: "
                          "overlap-curve = exposed ms vs G; sweep = the full chunk x depth x sync-mode grid "
                          "(BASELINE.json:configs[4]); timeline = copy/compute overlap from CUDA events")
@@ -1056,6 +1057,43 @@ def measure_config(args, key, link, clk, rank, world, local_rank, K, Wm, peak, h
     return rec, extras
 
 
+def measure_direct_source(args, key, link, clk, replica, K):
+    """The same config with PHX_SNAPSHOT_DIRECT: no staging ring and no staging stores — under the paper's own sync
+    point the flush DMAs the live planes themselves, the kernel moves 28 B/element.  Kernel, flush and
+    the exposed checkpoint time in both windows and both launch forms."""
+    import torch
+    rig = Rig(args, key, source="direct", replica=replica, host_grads=False)
+    N = rig.N
+    for _ in range(3):
+        rig.do_step()
+    with clk.leg(f"{key}.direct.step"):
+        tot, _, _ = rig.time_steps(K, 0)
+        kern_ms = rig.time_fused_kernel_alone(K) if rig.clip else tot / K
+    with clk.leg(f"{key}.direct.flush"):
+        fl = sorted(rig.time_flush() for _ in range(5))
+    flush_ms = fl[0]
+    out = {"snapshot_source": "direct", "step_ms": tot / K, "kernel_ms": kern_ms, "kernel_bytes_per_element": BYTES_PER_ELEM_OFF,
+           "kernel_gbs": BYTES_PER_ELEM_OFF * N / (kern_ms * 1e-3) / 1e9, "flush_ms": flush_ms,
+           "flush_gbs": (256 + 12 * N) / (flush_ms * 1e-3) / 1e9,
+           "flush_frac_of_d2h_peak": (256 + 12 * N) / (flush_ms * 1e-3) / 1e9 / link["d2h_gbs"], "overlap": {}}
+    for wname, factor, pow2 in (("headline_window", 4.0, True), ("tight_window", 1.25, False)):
+        G = rig.gemms_for(flush_ms, factor, pow2)
+        iters = rig.iters_for(G)
+        with clk.leg(f"{key}.direct.overlap.{wname}"):
+            o = rig.overlap(G, iters)
+            w = {"gemms_per_iter": G, "iter_ms_off": o["iter_ms_off"], "exposed_ms_eager": o["exposed_ms"],
+                 "exposed_pct_eager": 100.0 * o["exposed_frac_of_compute_step"]}
+            if not args.no_graph_step:
+                og = rig.overlap_graph_step(G, iters)
+                w.update(iter_ms_off_graph_step=og["iter_ms_off"], exposed_ms_graph_step=og["exposed_ms"],
+                         exposed_pct_graph_step=100.0 * og["exposed_frac_of_compute_step"])
+        out["overlap"][wname] = w
+    rig.close()
+    del rig
+    torch.cuda.empty_cache()
+    return out
+
+
 def measure_c5_grid(args, link, clk, replica, flush_ref):
     """BASELINE.json:configs[4]: D2H chunk size x staging depth at the TIGHT window (T_c = 1.25 x T_D2H, where
     depth and chunking can matter): exposed checkpoint ms/iteration and host-link GB/s per cell; reduced grid in the
@@ -1269,6 +1307,9 @@ def run_headline(args):
                                            source=rig.source_name, fp32=rig.fp32, full=rig.full, N=int(rig.N),
                                            title=f"{rig.wl.key}: {rig.wl.title}", clip=rig.clip)
             head_extras["multi"] = multi_gpu_legs(args, rig, rank, world, clk)
+            if (rank == 0 and world == 1 and rig.source_name == "staged" and not args.no_overlap and not args.no_direct
+                    and not rig.full and "flush" in rec):
+                rec["direct_source"] = measure_direct_source(args, key, link, clk, rig.s.replica, max(50, K // 2))
         if key == "c5" and rank == 0 and world == 1 and not args.no_grid and not args.no_overlap and "flush" in rec:
             replica, flush_ref = rig.s.replica, rec["flush"]["ms"]
             barrier(world)
@@ -1493,6 +1534,40 @@ def run_sweep(args):
     return 0
 
 
+def run_probe(args):
+    """Structure evidence for the fused kernel: the no-arithmetic streaming pass of the bench-only probe
+    library for several read:write mixes, in the ONE-SHOT structure the step uses (one 8-element group per thread,
+    short-lived CTAs) and in the PERSISTENT structure (148 x c CTAs with a grid stride).  One JSON line per cell."""
+    torch, rank, world, local_rank = gpu_setup(args)
+    from paper_2607_01646_b200 import probe as PB
+    device = torch.device(f"cuda:{local_rank}")
+    N = shard_elements(args, args.headline)
+    plane_bytes = 4 * N
+    buf = torch.empty(9 * plane_bytes, dtype=torch.uint8, device=device)
+    buf.zero_()
+    st = torch.cuda.current_stream(device)
+    sms = torch.cuda.get_device_properties(device).multi_processor_count
+    for name, (r, w) in {"step_mix_3r6w": (3, 6), "off_mix_3r3w": (3, 3), "copy_1r1w": (1, 1), "finalize_mix_2r1w": (2, 1),
+                         "write_only_4w": (0, 4)}.items():
+        for label, grid in [("one-shot", 0)] + [(f"persistent {c} CTAs/SM", sms * c) for c in (2, 4, 8)]:
+            def go():
+                if grid:
+                    return PB.phx_hbm_probe_persistent_async(buf, plane_bytes, r, w, grid, st)
+                return PB.phx_hbm_probe_async(buf, plane_bytes, r, w, st)
+            for _ in range(3):
+                assert go() == 0
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            for _ in range(20):
+                go()
+            e1.record(st)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / 20
+            emit(mode="probe", mix=name, planes_read=r, planes_written=w, structure=label, plane_elements=int(N), ms=ms,
+                 gbs=(r + w) * plane_bytes / (ms * 1e-3) / 1e9)
+    return 0
+
+
 def main():
     args = parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
@@ -1500,7 +1575,7 @@ def main():
     if args.impl == "reference":
         return run_reference(args)
     return {"headline": run_headline, "overlap-curve": run_overlap_curve, "sweep": run_sweep,
-            "timeline": run_timeline}[args.mode](args)
+            "timeline": run_timeline, "probe": run_probe}[args.mode](args)
 
 
 if __name__ == "__main__":

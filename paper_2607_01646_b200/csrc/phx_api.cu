@@ -391,7 +391,7 @@ int phx_shard_create(const phx_tensor_desc_t *layout, size_t n_tensors, uint32_t
     if (c.tp_size == 0) c.tp_size = 1;
     if (c.pp_size == 0) c.pp_size = 1;
     if (c.staging_depth == 0) c.staging_depth = 2;
-    if (c.chunk_bytes == 0) c.chunk_bytes = 8ull << 20;
+    if (c.chunk_bytes == 0) c.chunk_bytes = 32ull << 20;
     c.chunk_bytes = (c.chunk_bytes + 255) & ~255ull;
     if (c.tp_rank >= c.tp_size || c.pp_rank >= c.pp_size || c.staging_depth > kMaxDepth ||
         c.sync_mode > PHX_SYNC_RELAXED || c.restore_mode > PHX_RESTORE_BULK_KERNEL || !(c.max_grad_norm == c.max_grad_norm) ||

@@ -18,6 +18,11 @@ extern "C" {
 #endif
 __attribute__((visibility("default"))) int phx_hbm_probe_async(void *d_buf, uint64_t plane_bytes, uint32_t n_read,
                                                                uint32_t n_write, void *stream);
+/* The same pass with a PERSISTENT structure: `grid` CTAs of 256 threads walking the groups with a grid stride
+ * (e.g. 148 x 4) instead of one short-lived CTA per 256 groups — the structural alternative the fused step was
+ * measured against (profiles/r02_structure_probe.md). */
+__attribute__((visibility("default"))) int phx_hbm_probe_persistent_async(void *d_buf, uint64_t plane_bytes, uint32_t n_read,
+                                                                          uint32_t n_write, uint32_t grid, void *stream);
 #ifdef __cplusplus
 }
 #endif

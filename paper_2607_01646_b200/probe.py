@@ -22,6 +22,8 @@ def lib() -> C.CDLL:
         L = C.CDLL(LIB_PATH)
         L.phx_hbm_probe_async.restype = C.c_int
         L.phx_hbm_probe_async.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
+        L.phx_hbm_probe_persistent_async.restype = C.c_int
+        L.phx_hbm_probe_persistent_async.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p]
         _lib = L
     return _lib
 
@@ -29,3 +31,8 @@ def lib() -> C.CDLL:
 def phx_hbm_probe_async(d_buf, plane_bytes: int, n_read: int, n_write: int, stream=None) -> int:
     """Returns the probe's status code (0 ok, -1 invalid argument, -2 alignment, -9 CUDA error)."""
     return lib().phx_hbm_probe_async(_ptr(d_buf), plane_bytes, n_read, n_write, _ptr(stream))
+
+
+def phx_hbm_probe_persistent_async(d_buf, plane_bytes: int, n_read: int, n_write: int, grid: int, stream=None) -> int:
+    """The same pass with `grid` persistent CTAs walking the groups with a grid stride."""
+    return lib().phx_hbm_probe_persistent_async(_ptr(d_buf), plane_bytes, n_read, n_write, grid, _ptr(stream))

@@ -4,12 +4,14 @@
  * and runs it): it reads the initial p and the gradients of each step from files, runs
  *     create -> bind -> set_state -> [step_and_snapshot -> flush_async] x steps -> wait
  *     -> (in-flight step) -> zero the live shard -> restore -> recompute the in-flight step
+ *     -> the gradient producer's epilogue (phx_grads_finalize_async) feeding one step
+ *     -> two steps through the graph-capturable form (phx_graph_begin / flush / step / end), called eagerly
  * and writes p, m, v, the bf16 copy and the two host replica slots to an output file that the test
  * compares byte for byte with the CPU oracle.
  *
  * usage: phx_c_client <in.bin> <out.bin>
  *   in.bin : u64 n_tensors, u64 numel[n_tensors], u32 dp_size, u32 dp_rank, u32 steps, f32 max_grad_norm,
- *            u64 chunk_bytes, f32 p0[n_padded], then (steps + 1) x bf16 g[n_padded]
+ *            u64 chunk_bytes, f32 p0[n_padded], then (steps + 1) x bf16 g[n_padded], f32 scale, f32 g32[n_padded]
  *   out.bin: u64 n_padded, u64 restored_step, f32 p, m, v [n_padded] each, u16 p16[n_padded],
  *            u8 replica[2 * slot_stride]
  */
@@ -83,7 +85,9 @@ int main(int argc, char **argv)
 
     float *h_f = (float *)malloc(4 * N);
     uint16_t *h_g = (uint16_t *)malloc(2 * N * (steps + 1));
-    if (rd(in, h_f, 4 * N) || rd(in, h_g, 2 * N * (steps + 1))) return 1;
+    float scale = 1.0f;
+    float *h_g32 = (float *)malloc(4 * N);
+    if (rd(in, h_f, 4 * N) || rd(in, h_g, 2 * N * (steps + 1)) || rd(in, &scale, 4) || rd(in, h_g32, 4 * N)) return 1;
     fclose(in);
     CU(cudaMemcpy(d_p, h_f, 4 * N, cudaMemcpyHostToDevice));
     CU(cudaMemset(d_m, 0, 4 * N));
@@ -121,6 +125,36 @@ int main(int argc, char **argv)
     }
     /* recompute of the in-flight step ("at most one step of re-execution") */
     CK(phx_step_and_snapshot(s, d_g, lr, b1, b2, eps, wd, back + 1, compute));
+    CK(phx_snapshot_flush_async(s, side));
+
+    /* SURVEY 8(f4), second half: the gradients of the next step come out of the producer's epilogue (fp32 main
+     * gradients x scale -> bf16 + sum of squares, one pass); the step then needs no pass of its own over them */
+    float *d_g32;
+    double *d_sum;
+    CU(cudaMalloc((void **)&d_g32, 4 * N));
+    CU(cudaMalloc((void **)&d_sum, 8));
+    CU(cudaMemcpyAsync(d_g32, h_g32, 4 * N, cudaMemcpyHostToDevice, compute));
+    CK(phx_grads_finalize_async(s, d_g32, scale, d_g, d_sum, compute));
+    if (max_norm > 0.0f) CK(phx_set_clip_partials(s, d_sum, 1));
+    CK(phx_step_and_snapshot(s, d_g, lr, b1, b2, eps, wd, back + 2, compute));
+
+    /* the graph-capturable form, called eagerly: flush of the pending snapshot, then step, twice */
+    void *d_ga, *d_gb;
+    CU(cudaMalloc(&d_ga, 2 * N));
+    CU(cudaMalloc(&d_gb, 2 * N));
+    CU(cudaMemcpyAsync(d_ga, h_g, 2 * N, cudaMemcpyHostToDevice, compute));
+    CU(cudaMemcpyAsync(d_gb, h_g + N, 2 * N, cudaMemcpyHostToDevice, compute));
+    CK(phx_graph_begin(s, lr, b1, b2, eps, wd, compute));
+    CK(phx_graph_flush_async(s, side));
+    CK(phx_graph_step_and_snapshot(s, d_ga, compute));
+    CK(phx_graph_flush_async(s, side));
+    CK(phx_graph_step_and_snapshot(s, d_gb, compute));
+    uint64_t last = 0;
+    CK(phx_graph_end(s, &last));
+    if (last != back + 4) {
+        fprintf(stderr, "graph form ended at step %llu, expected %llu\n", (unsigned long long)last, (unsigned long long)(back + 4));
+        return 5;
+    }
     CU(cudaStreamSynchronize(compute));
 
     FILE *out = fopen(argv[2], "wb");

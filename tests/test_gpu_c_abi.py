@@ -1,6 +1,7 @@
 """The C-ABI boundary used from plain C (tests/c_abi/phx_c_client.c: cudaMalloc/cudaHostAlloc buffers, no Python,
-no torch in the process that runs the hot path): step + snapshot + flush, loss of the live shard, restore, recompute —
-its output file compared byte for byte with the CPU oracle.  The header also has to compile as strict C99."""
+no torch in the process that runs the hot path): step + snapshot + flush, loss of the live shard, restore, recompute,
+the gradient producer's epilogue feeding a step, two steps through the graph-capturable form — its output file
+compared byte for byte with the CPU oracle.  The header also has to compile as strict C99."""
 import os
 import struct
 import subprocess
@@ -10,6 +11,7 @@ import numpy as np
 import pytest
 import torch
 
+from oracle import grad_finalize as GF
 from oracle import oracle as O
 from paper_2607_01646_b200 import binding as B
 from paper_2607_01646_b200 import workloads as W
@@ -60,6 +62,12 @@ def test_c_client_matches_the_oracle(tmp_path, numels, dp, rank, max_norm):
         f.write(p0.tobytes())
         for g in grads:
             f.write(g.tobytes())
+        rng = np.random.default_rng(4)
+        g32 = (rng.standard_t(3, N) * 2e-3).astype(np.float32)
+        g32[o.n:] = 0
+        scale = np.float32(1.0 / 3.0)
+        f.write(struct.pack("<f", scale))
+        f.write(g32.tobytes())
     r = subprocess.run([exe, str(inp), str(outp)], capture_output=True, text=True, timeout=120)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "phx_c_client ok" in r.stdout
@@ -69,11 +77,17 @@ def test_c_client_matches_the_oracle(tmp_path, numels, dp, rank, max_norm):
     for t in range(1, steps + 1):
         o.step(grads[t - 1], **hp, step=t)
         o.snapshot()
-    replica = [x.copy() for x in o.replica]
     o.step(grads[steps], **hp, step=steps + 1)            # in flight, lost
     o.drop_live()
     assert o.restore() == steps
     o.step(grads[steps], **hp, step=steps + 1)            # recompute
+    o.snapshot()                                          # ... and its flush
+    gbits, _ = GF.grads_finalize(g32, scale)              # producer epilogue -> the next step's gradients
+    o.step(gbits, **hp, step=steps + 2)
+    for k in (0, 1):                                      # graph form: flush of the pending snapshot, then step
+        o.snapshot()
+        o.step(grads[k], **hp, step=steps + 3 + k)
+    replica = [x.copy() for x in o.replica]               # slots now hold steps+2 and steps+3
     raw = open(outp, "rb").read()
     n_padded, back = struct.unpack_from("<QQ", raw, 0)
     assert (n_padded, back) == (N, steps)

@@ -53,10 +53,10 @@ def assert_replica_is_oracle_snapshot(s: Shard, o: O.OracleShard, step: int, wha
 
 def run_config(wl, steps=3, **shard_kw):
     fp32 = wl.precision == "fp32"
-    s = Shard(wl, device=DEV, **shard_kw)
+    s = Shard(wl, device=DEV, **shard_kw)              # library defaults = the launch configuration bench.py times
     N = s.n_padded
     o = O.OracleShard(wl.layout(), wl.dp_size, wl.dp_rank, (wl.tp_size, wl.tp_rank), (wl.pp_size, wl.pp_rank),
-                      chunk_bytes=8 << 20, max_grad_norm=wl.hyper.max_grad_norm, flags=wl.flags(),
+                      chunk_bytes=32 << 20, max_grad_norm=wl.hyper.max_grad_norm, flags=wl.flags(),
                       precision=wl.precision)
     assert (o.n, o.n_padded) == (s.n, N) and o.n == wl.n_expected
     p0 = W.init_params(s.n, N, wl.seed, device=DEV)

@@ -37,3 +37,16 @@ def test_probe_argument_errors():
     assert L.phx_hbm_probe_async(buf.data_ptr(), 256, 9, 0, None) == -1
     assert L.phx_hbm_probe_async(buf.data_ptr(), 256, 0, 0, None) == -1
     assert L.phx_hbm_probe_async(buf.data_ptr() + 16, 256, 1, 1, None) == -2
+
+
+def test_persistent_structure_writes_the_same_bytes_as_the_one_shot_structure():
+    plane = 256 * 1000 + 256 * 3
+    a = torch.zeros(9 * plane, dtype=torch.uint8, device=DEV)
+    a[:3 * plane].view(torch.float32).fill_(0.5)
+    b = a.clone()
+    st = torch.cuda.current_stream()
+    assert PB.phx_hbm_probe_async(a, plane, 3, 6, st) == 0
+    assert PB.phx_hbm_probe_persistent_async(b, plane, 3, 6, 148 * 4, st) == 0
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    assert PB.lib().phx_hbm_probe_persistent_async(b.data_ptr(), plane, 3, 6, 0, None) == -1
