@@ -821,16 +821,17 @@ class Rig:
 
     def overlap_graph_step(self, G, iters, warm=1, arms=("off", "on")):
         """The same experiment with the WHOLE iteration captured in a CUDA graph — the B200-native launch form
-        (DESIGN.md §12): [flush of snapshot k-1 on the side stream ‖ G GEMMs] -> step k, two iterations per graph
-        (staging / host slot ping-pong), through the graph-capturable form of the step (phx_graph_*).  Arms:
-        off = snapshot-disabled handle, no flush; on = snapshots + flush.  One eager event pair per replay:
-        iteration time = replay time / 2."""
+        (DESIGN.md §12): [flush of snapshot k-1 on the side stream ‖ G GEMMs] -> step k, L = lcm(staging depth, 2)
+        iterations per graph (staging / host slot ping-pong), through the graph-capturable form of the step
+        (phx_graph_*).  Arms: off = snapshot-disabled handle, no flush; on = snapshots + flush.  One eager event pair
+        per replay: iteration time = replay time / L."""
         torch, B = self.torch, self.B
         self.gemm_setup()
         hp = self.wl.hyper
         cap = torch.cuda.Stream(device=self.device)
         res = {}
-        nrep = max(4, (iters + 1) // 2)
+        L = {1: 2, 2: 2, 3: 6, 4: 4}[self.depth] if self.source_name == "staged" else 2
+        nrep = max(3, (iters + L - 1) // L)
         for arm in arms:
             h = self.off_shard() if arm == "off" else self.s.h
             with torch.cuda.stream(cap):
@@ -841,7 +842,7 @@ class Rig:
             torch.cuda.synchronize()
             graph = torch.cuda.CUDAGraph()
             with torch.cuda.graph(graph, stream=cap):
-                for i in range(2):
+                for i in range(L):
                     if arm == "on":
                         self.side.wait_stream(cap)                       # fork: the flush runs beside the window
                         B.phx_graph_flush_async(h, self.side)
@@ -858,7 +859,7 @@ class Rig:
                     e1.record(cap)
                     times.append((e0, e1))
             torch.cuda.synchronize()
-            ms = [a.elapsed_time(b) / 2 for a, b in times[warm:]]
+            ms = [a.elapsed_time(b) / L for a, b in times[warm:]]
             res[arm] = trimmed_mean(ms)
             last = B.phx_graph_end(h)
             if arm == "on":
@@ -868,8 +869,8 @@ class Rig:
             else:
                 self.off_step = last
             del graph
-        out = {"gemms_per_iter": G, "compute_window_ms": G * self.gemm_ms, "launch": "cuda graph (2 iterations per graph)",
-               "iters_per_arm": 2 * nrep}
+        out = {"gemms_per_iter": G, "compute_window_ms": G * self.gemm_ms, "launch": f"cuda graph ({L} iterations per graph)",
+               "iters_per_arm": L * nrep}
         for arm in arms:
             out[f"iter_ms_{arm}"] = res[arm]
         if "on" in res and "off" in res:
@@ -1070,7 +1071,7 @@ def measure_direct_source(args, key, link, clk, replica, K):
         tot, _, _ = rig.time_steps(K, 0)
         kern_ms = rig.time_fused_kernel_alone(K) if rig.clip else tot / K
     with clk.leg(f"{key}.direct.flush"):
-        fl = sorted(rig.time_flush() for _ in range(5))
+        fl = sorted(rig.time_flush() for _ in range(9))
     flush_ms = fl[0]
     out = {"snapshot_source": "direct", "step_ms": tot / K, "kernel_ms": kern_ms, "kernel_bytes_per_element": BYTES_PER_ELEM_OFF,
            "kernel_gbs": BYTES_PER_ELEM_OFF * N / (kern_ms * 1e-3) / 1e9, "flush_ms": flush_ms,
@@ -1117,7 +1118,7 @@ def measure_c5_grid(args, link, clk, replica, flush_ref):
                 "host_link_gbs": (256 + 12 * rig.N) / (fl * 1e-3) / 1e9, "gemms_per_iter": G,
                 "iter_ms_on": o["iter_ms_on"], "iter_ms_off": base, "exposed_ms": o["iter_ms_on"] - base,
                 "exposed_pct": 100.0 * (o["iter_ms_on"] - base) / base}
-        if base_g is not None and depth in (1, 2):          # the captured sequence here spans 2 steps = lcm(depth, 2)
+        if base_g is not None:
             og = rig.overlap_graph_step(G, 8, arms=("on",))
             cell.update(iter_ms_on_graph_step=og["iter_ms_on"], iter_ms_off_graph_step=base_g,
                         exposed_ms_graph_step=og["iter_ms_on"] - base_g,
@@ -1503,6 +1504,7 @@ def run_sweep(args):
     it_t, it_h = probe.iters_for(G_tight), max(5, probe.iters_for(G_head) // 2)
     base = probe.overlap(G_tight, it_t, arms=("off",))
     base_head = probe.overlap(G_head, it_h, arms=("off",))
+    base_g = None if args.no_graph_step else probe.overlap_graph_step(G_tight, it_t, arms=("off",))["iter_ms_off"]
     probe.close()
     del probe
     torch.cuda.empty_cache()
@@ -1513,8 +1515,14 @@ def run_sweep(args):
                 rig = Rig(args, key, depth=depth, chunk_mib=chunk, sync=sync, replica=replica, host_grads=False)
                 flush_ms = rig.time_flush()
                 o = rig.overlap(G_tight, it_t, arms=("on",))
+                gx = {}
+                if base_g is not None:
+                    og = rig.overlap_graph_step(G_tight, it_t, arms=("on",))
+                    gx = dict(iter_ms_on_graph_step=og["iter_ms_on"], iter_ms_off_graph_step=base_g,
+                              exposed_ms_graph_step=og["iter_ms_on"] - base_g,
+                              exposed_frac_graph_step=(og["iter_ms_on"] - base_g) / base_g)
                 emit(mode="sweep", window="tight(1.25xT_D2H)", config=key, elements=int(rig.N), sync_mode=sync,
-                     depth=depth, chunk_mib=chunk, flush_ms=flush_ms,
+                     depth=depth, chunk_mib=chunk, flush_ms=flush_ms, **gx,
                      host_link_gbs=rig_bytes(rig.N) / (flush_ms * 1e-3) / 1e9, d2h_peak_gbs=link["d2h_gbs"],
                      gemms_per_iter=G_tight, iter_ms_on=o["iter_ms_on"], iter_ms_off=base["iter_ms_off"],
                      exposed_ms=o["iter_ms_on"] - base["iter_ms_off"],

@@ -444,6 +444,10 @@ PHX_API int phx_graph_begin(phx_shard_t *s, float lr, float beta1, float beta2, 
 PHX_API int phx_graph_set_hyper(phx_shard_t *s, float lr, float beta1, float beta2, float eps, float wd, void *stream);
 PHX_API int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *stream);
 PHX_API int phx_graph_flush_async(phx_shard_t *s, void *side_stream);
+/* §8(f1) in the graph form: replication of the last issued step's snapshot to the k bound ring peers, capturable
+ * like phx_graph_flush_async (fork `peer_stream` from the capturing stream first; k > 1 fans out over the
+ * library-owned per-peer streams inside the capture).  The sync point of the next step covers it. */
+PHX_API int phx_graph_flush_peers_async(phx_shard_t *s, void *peer_stream);
 PHX_API int phx_graph_end(phx_shard_t *s, uint64_t *last_step);
 
 /* ---- introspection ---------------------------------------------------------------------- */

@@ -125,6 +125,7 @@ PROTOTYPES = {
     "phx_graph_set_hyper": (C.c_int, [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float, C.c_void_p]),
     "phx_graph_step_and_snapshot": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "phx_graph_flush_async": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "phx_graph_flush_peers_async": (C.c_int, [C.c_void_p, C.c_void_p]),
     "phx_graph_end": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_ring_peer": (C.c_int, [C.c_uint32, C.c_uint32, C.c_int32, C.POINTER(C.c_uint32)]),
     "phx_peer_buffer_alloc": (C.c_int, [C.c_uint64, C.POINTER(C.c_void_p)]),
@@ -354,6 +355,10 @@ def phx_graph_step_and_snapshot(h: int, d_grads, stream=None) -> None:
 
 def phx_graph_flush_async(h: int, side_stream=None) -> None:
     _ck(lib().phx_graph_flush_async(h, _ptr(side_stream)), "phx_graph_flush_async", h)
+
+
+def phx_graph_flush_peers_async(h: int, peer_stream=None) -> None:
+    _ck(lib().phx_graph_flush_peers_async(h, _ptr(peer_stream)), "phx_graph_flush_peers_async", h)
 
 
 def phx_graph_end(h: int) -> int:

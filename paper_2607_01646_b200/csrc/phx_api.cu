@@ -154,7 +154,10 @@ struct phx_shard {
     int g_pending_slot = -1;
     uint64_t g_pending_step = 0;
     int g_last_flush_slot = -1;
-    GraphEvent gev_step[kMaxDepth], gev_flush[kMaxDepth];
+    int g_pending_peer_slot = -1;
+    uint64_t g_pending_peer_step = 0;
+    int g_last_pflush_slot = -1;
+    GraphEvent gev_step[kMaxDepth], gev_flush[kMaxDepth], gev_pflush[kMaxDepth];
 };
 
 #define PHX_CK(call)                                  \
@@ -476,6 +479,7 @@ int phx_shard_destroy(phx_shard_t *s)
         for (int k = 0; k < kMaxDepth; ++k) {
             if (s->gev_step[k].ev) cudaEventDestroy(s->gev_step[k].ev);
             if (s->gev_flush[k].ev) cudaEventDestroy(s->gev_flush[k].ev);
+            if (s->gev_pflush[k].ev) cudaEventDestroy(s->gev_pflush[k].ev);
         }
         if (s->ev_params) cudaEventDestroy(s->ev_params);
         if (s->ev_wflush) cudaEventDestroy(s->ev_wflush);
@@ -549,6 +553,7 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
     for (int k = 0; k < kMaxDepth; ++k) {
         PHX_CK(cudaEventCreateWithFlags(&s->gev_step[k].ev, cudaEventDisableTiming));
         PHX_CK(cudaEventCreateWithFlags(&s->gev_flush[k].ev, cudaEventDisableTiming));
+        PHX_CK(cudaEventCreateWithFlags(&s->gev_pflush[k].ev, cudaEventDisableTiming));
     }
     PHX_CK(cudaEventCreateWithFlags(&s->ev_params, cudaEventDisableTiming));
     PHX_CK(cudaEventCreateWithFlags(&s->ev_wflush, cudaEventDisableTiming));
@@ -1372,7 +1377,10 @@ int phx_graph_begin(phx_shard_t *s, float lr, float beta1, float beta2, float ep
     s->g_pending_slot = s->pending_slot;   // an eager step's un-flushed snapshot becomes the graph's first flush
     s->g_pending_step = s->pending_step;
     s->g_last_flush_slot = -1;
-    for (int k = 0; k < kMaxDepth; ++k) s->gev_step[k].valid = s->gev_flush[k].valid = false;
+    s->g_pending_peer_slot = s->n_peers ? s->pending_peer_slot : -1;
+    s->g_pending_peer_step = s->pending_peer_step;
+    s->g_last_pflush_slot = -1;
+    for (int k = 0; k < kMaxDepth; ++k) s->gev_step[k].valid = s->gev_flush[k].valid = s->gev_pflush[k].valid = false;
     return PHX_OK;
 }
 
@@ -1409,10 +1417,13 @@ int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *strea
         // a2, the single sync point: a dependency edge inside a captured graph, a stream wait outside
         if (s->cfg.sync_mode == PHX_SYNC_STRICT) {
             if (s->g_last_flush_slot >= 0 && (rc = gev_wait(s, s->gev_flush[s->g_last_flush_slot], st)) != PHX_OK) return rc;
-        } else if ((rc = gev_wait(s, s->gev_flush[slot], st)) != PHX_OK) {
-            return rc;
+            if (s->g_last_pflush_slot >= 0 && (rc = gev_wait(s, s->gev_pflush[s->g_last_pflush_slot], st)) != PHX_OK) return rc;
+        } else {
+            if ((rc = gev_wait(s, s->gev_flush[slot], st)) != PHX_OK) return rc;
+            if ((rc = gev_wait(s, s->gev_pflush[slot], st)) != PHX_OK) return rc;
         }
         if (s->g_pending_slot >= 0 && s->h_replica) s->dropped_host += 1;
+        if (s->g_pending_peer_slot >= 0 && s->n_peers) s->dropped_peers += 1;
     }
     fill_common_args(s, d_grads, slot, a);
     void *shdr = a.shdr;
@@ -1425,6 +1436,10 @@ int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *strea
         if ((rc = gev_record(s, s->gev_step[slot], st)) != PHX_OK) return rc;
         s->g_pending_slot = slot;
         s->g_pending_step = step;
+        if (s->n_peers) {
+            s->g_pending_peer_slot = slot;
+            s->g_pending_peer_step = step;
+        }
     }
     s->g_issue = step;
     return PHX_OK;
@@ -1449,6 +1464,38 @@ int phx_graph_flush_async(phx_shard_t *s, void *side_stream)
     if ((rc = gev_record(s, s->gev_flush[slot], st)) != PHX_OK) return rc;
     s->g_last_flush_slot = slot;
     s->g_pending_slot = -1;
+    return PHX_OK;
+}
+
+// §8(f1) in the graph form: the replication of the last issued step's snapshot to the k ring peers, capturable
+int phx_graph_flush_peers_async(phx_shard_t *s, void *peer_stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound || s->n_peers == 0) return PHX_ERR_NOT_BOUND;
+    if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
+    if (!s->graph) return PHX_ERR_GRAPH_MODE;
+    if (s->g_pending_peer_slot < 0) return PHX_ERR_NO_FLUSH_PENDING;
+    cudaStream_t st = static_cast<cudaStream_t>(peer_stream);
+    const int slot = s->g_pending_peer_slot;
+    const int ps = (int)(s->g_pending_peer_step & 1);
+    int rc;
+    if ((rc = gev_wait(s, s->gev_step[slot], st)) != PHX_OK) return rc;
+    if (s->g_last_pflush_slot >= 0 && (rc = gev_wait(s, s->gev_pflush[s->g_last_pflush_slot], st)) != PHX_OK) return rc;
+    const bool fan = s->n_peers > 1;  // one library-owned copy stream per peer, forked from and joined into `st`
+    if (fan) PHX_CK(cudaEventRecord(s->ev_peer_fork, st));
+    for (uint32_t j = 0; j < s->n_peers; ++j) {
+        cudaStream_t pst = fan ? s->peer_st[j] : st;
+        if (fan) PHX_CK(cudaStreamWaitEvent(pst, s->ev_peer_fork, 0));
+        rc = enqueue_snapshot_copy(s, pst, s->d_peer[j] + (uint64_t)ps * s->info.slot_stride, cudaMemcpyDefault, slot, -1);
+        if (rc != PHX_OK) return rc;
+        if (fan) {
+            PHX_CK(cudaEventRecord(s->ev_peer_join[j], pst));
+            PHX_CK(cudaStreamWaitEvent(st, s->ev_peer_join[j], 0));
+        }
+    }
+    if ((rc = gev_record(s, s->gev_pflush[slot], st)) != PHX_OK) return rc;
+    s->g_last_pflush_slot = slot;
+    s->g_pending_peer_slot = -1;
     return PHX_OK;
 }
 
@@ -1477,8 +1524,24 @@ int phx_graph_end(phx_shard_t *s, uint64_t *last_step)
         if (ok && h.step > newest) newest = h.step;
     }
     if (snapshots_on(s) && s->last_step > 0 && newest != s->last_step) {  // the newest step's snapshot is still staged
-        s->pending_slot = s->pending_peer_slot = (int)(s->last_step % ring_depth(s));
-        s->pending_step = s->pending_peer_step = s->last_step;
+        s->pending_slot = (int)(s->last_step % ring_depth(s));
+        s->pending_step = s->last_step;
+    }
+    // the peers' slots are self-describing too: the first peer's two envelopes (all k peers are written as one unit)
+    uint64_t newest_peer = 0;
+    for (int i = 0; i < 2; ++i) {
+        s->peer[i].state = SLOT_EMPTY;
+        if (!s->n_peers) continue;
+        phx_snapshot_header_t h;
+        PHX_CK(cudaMemcpy(&h, s->d_peer[0] + (uint64_t)i * s->info.slot_stride, sizeof(h), cudaMemcpyDefault));
+        if (!(header_valid(&h) && header_matches(s, &h) && h.payload == 0u)) continue;
+        s->peer[i].state = SLOT_COMMITTED;
+        s->peer[i].step = h.step;
+        if (h.step > newest_peer) newest_peer = h.step;
+    }
+    if (snapshots_on(s) && s->n_peers && s->last_step > 0 && newest_peer != s->last_step) {
+        s->pending_peer_slot = (int)(s->last_step % ring_depth(s));
+        s->pending_peer_step = s->last_step;
     }
     if (last_step) *last_step = s->last_step;
     return blk.misaligned ? PHX_ERR_STEP_ORDER : PHX_OK;

@@ -170,3 +170,76 @@ def test_graph_form_protocol_errors():
     full = B.phx_shard_create([(8192, 0)], 1, 0, payload=B.PHX_PAYLOAD_FULL_RANK_STATE)
     assert L.phx_graph_begin(full, 1e-3, 0.9, 0.95, 1e-8, 0.0, None) == B.PHX_ERR_NOT_BOUND
     B.phx_shard_destroy(full)
+
+
+@pytest.mark.parametrize("k", [1, 2])
+def test_captured_graph_with_host_flush_and_ring_peer_flush(k):
+    """The graph form covers §8(f1) too: [flush(k-1) to the host ‖ flush(k-1) to the k ring peers ‖ window] -> step k,
+    captured once, replayed; the peers' received slots are byte-identical to the host slots and to the oracle's."""
+    from paper_2607_01646_b200 import ring as PR
+    wl = W.tiny_workload([200_000, 77], dp_size=3, dp_rank=0)
+    s, o, _, _ = make_pair(wl, steps=0, chunk_bytes=256 << 10)
+    recv = PR.ReceivedBuffers(s.info.slot_stride, k)
+    B.phx_shard_bind_peers(s.h, recv.ptrs)
+    hp = hp_of(wl)
+    osegs = [(tid, off, ln) for tid, _, off, ln in o.segments]
+    gbuf = [torch.zeros(s.n_padded, dtype=torch.bfloat16, device=DEV) for _ in range(2)]
+    a = torch.randn(256, 256, device=DEV, dtype=torch.bfloat16)
+    c = torch.empty_like(a)
+    cap, side, peer = (torch.cuda.Stream(device=DEV) for _ in range(3))
+    with torch.cuda.stream(cap):
+        torch.matmul(a, a, out=c)
+    torch.cuda.synchronize()
+
+    def grads_of(t):
+        return W.gen_grads(wl, osegs, s.n_padded, t, wl.seed)
+
+    s.graph_begin(stream=cap)
+    g1 = grads_of(1)
+    gbuf[1].copy_(g1)
+    torch.cuda.synchronize()
+    s.graph_step(gbuf[1], stream=cap)
+    o.step(g1.view(torch.int16).numpy().view(np.uint16).copy(), **hp, step=1); o.snapshot()
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=cap):
+        for i in range(2):
+            side.wait_stream(cap); s.graph_flush(side)
+            peer.wait_stream(cap); B.phx_graph_flush_peers_async(s.h, peer)
+            torch.matmul(a, a, out=c)
+            s.graph_step(gbuf[i & 1], stream=cap)
+        cap.wait_stream(side); cap.wait_stream(peer)
+    t = 1
+    snaps = {}
+    for _ in range(3):
+        for i in range(2):
+            t += 1
+            g = grads_of(t)
+            gbuf[t & 1].copy_(g)
+            o.step(g.view(torch.int16).numpy().view(np.uint16).copy(), **hp, step=t); o.snapshot()
+            snaps[t] = o.replica[t % 2].copy()
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+    assert s.graph_end() == t == 7
+    assert_state_equal(s, o, "graph with peers")
+    for step in (5, 6):
+        host = s.replica_slot(step).numpy()
+        assert np.array_equal(host, snaps[step]), step
+        for j in range(1, k + 1):
+            got = recv.view(j)[(step % 2) * s.info.slot_stride:(step % 2) * s.info.slot_stride + s.info.snapshot_bytes]
+            assert np.array_equal(got.cpu().numpy(), snaps[step]), (step, j)
+    # back in the eager form: the newest snapshot is still pending for both destinations
+    s.flush_async(side)
+    B.phx_snapshot_flush_peers_async(s.h, peer)
+    s.wait(7)
+    B.phx_snapshot_wait_peers(s.h, 7)
+    for j in range(1, k + 1):
+        got = recv.view(j)[s.info.slot_stride:s.info.slot_stride + s.info.snapshot_bytes]
+        assert np.array_equal(got.cpu().numpy(), snaps[7])
+    s.drop_live()
+    assert B.phx_restore_from(s.h, recv.ptrs[0], torch.cuda.current_stream()) == 7
+    assert_state_equal(s, o, "restored from the ring peer after graph replays")
+    B.phx_shard_bind_peers(s.h, [])
+    recv.free()
+    s.close()
