@@ -138,24 +138,68 @@ def committed_traffic(config):
     return None
 
 
+# the sampler process: NVML (the library nvidia-smi prints from) polled every ~2 ms, one CSV row per sample in the
+# same columns as the nvidia-smi query below, so that even a K = 20 step leg (tens of ms) gets >= 10 samples
+_NVML_SAMPLER = r"""
+import sys, time
+import pynvml as N
+N.nvmlInit()
+uuid, index, period = sys.argv[1], int(sys.argv[2]), float(sys.argv[3])
+h = None
+if uuid:
+    for u in (uuid, uuid.encode()):
+        try:
+            h = N.nvmlDeviceGetHandleByUUID(u); break
+        except Exception:
+            pass
+if h is None:
+    h = N.nvmlDeviceGetHandleByIndex(index)
+reasons = getattr(N, "nvmlDeviceGetCurrentClocksEventReasons", None) or N.nvmlDeviceGetCurrentClocksThrottleReasons
+mx = N.nvmlDeviceGetMaxClockInfo(h, N.NVML_CLOCK_SM)
+out = sys.stdout
+while True:
+    t = time.time()
+    r = reasons(h)
+    out.write("%.6f,%d,%d,%.2f,%d,%d,%d,%d\n" % (t, N.nvmlDeviceGetClockInfo(h, N.NVML_CLOCK_SM), mx,
+              N.nvmlDeviceGetPowerUsage(h) / 1000.0, bool(r & 0x8), bool(r & 0x40), bool(r & 0x20), bool(r & 0x4)))
+    out.flush()
+    time.sleep(period)
+"""
+
+
 class ClockLog:
-    """nvidia-smi clocks / throttle reasons sampled over the WHOLE run with timestamps (one process, 50 ms), cut
-    into the timed legs afterwards — every leg gets its own record (B200_PROFILING.md clocks line)."""
+    """SM clocks / throttle reasons sampled over the WHOLE run with timestamps by ONE side process, cut into the
+    timed legs afterwards — every leg gets its own record (B200_PROFILING.md clocks line).  The sampler polls NVML
+    (what nvidia-smi itself reads) every ~2 ms; if pynvml is missing it falls back to `nvidia-smi -lms 50`."""
     Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
     NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
-    def __init__(self, index=0, period_ms=50):
+    def __init__(self, index=0, period_ms=2, uuid=""):
         self.legs = []
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         self.p = None
+        self.source = None
         try:
-            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", str(period_ms)],
+            import pynvml  # noqa: F401  (only to learn whether the sampler can run)
+            self.p = subprocess.Popen([sys.executable, "-c", _NVML_SAMPLER, uuid, str(index), str(period_ms / 1e3)],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
+            time.sleep(0.3)
+            if self.p.poll() is not None:
+                self.p = None
+            else:
+                self.source = f"nvml, {period_ms} ms period"
         except Exception:
             self.p = None
+        if self.p is None:
+            try:
+                self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                           "--format=csv,noheader,nounits", "-lms", "50"],
+                                          stdout=self.f, stderr=subprocess.DEVNULL)
+                self.source = "nvidia-smi -lms 50"
+            except Exception:
+                self.p = None
 
     @contextlib.contextmanager
     def leg(self, name):
@@ -173,8 +217,9 @@ class ClockLog:
             if len(w) < 8:
                 continue
             try:
-                ts = datetime.datetime.strptime(w[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
-                rows.append((ts, float(w[1]), float(w[2]), float(w[3]), [x.lower().startswith("active") for x in w[4:8]]))
+                ts = float(w[0]) if "/" not in w[0] else datetime.datetime.strptime(w[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                rows.append((ts, float(w[1]), float(w[2]), float(w[3]),
+                             [x == "1" or x.lower().startswith("active") for x in w[4:8]]))
             except Exception:
                 continue
         return rows
@@ -1265,7 +1310,11 @@ def run_headline(args):
     keys = [k for k in (args.configs.split(",") if args.configs else (ALL_CONFIGS if world == 1 else [args.headline])) if k]
     if args.headline not in keys:
         keys.append(args.headline)
-    clk = ClockLog(local_rank) if rank == 0 else contextlib.nullcontext()
+    try:
+        uuid = "GPU-" + str(torch.cuda.get_device_properties(local_rank).uuid)
+    except Exception:
+        uuid = ""
+    clk = ClockLog(local_rank, uuid=uuid) if rank == 0 else contextlib.nullcontext()
     if rank != 0:
         clk = type("NoClk", (), {"leg": staticmethod(lambda name: contextlib.nullcontext())})()
     link = measure_host_link(torch, device) if rank == 0 else {}
@@ -1344,7 +1393,7 @@ def run_headline(args):
             w = max(records, key=lambda r: r["exposed_pct"])
             worst_exposed = {"config": w["config"], "exposed_pct": w["exposed_pct"], "exposed_ms": w["exposed_ckpt_ms_per_iter"]}
         slowest = min(records, key=lambda r: r["step_gbs"])
-        hl_clock = clocks_legs.get(f"{args.headline}.step", clocks_all)
+        hl_clock = dict(clocks_legs.get(f"{args.headline}.step", clocks_all), sampler=clk.source)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": head["step_ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

@@ -16,7 +16,7 @@
  *     pointers.  Replica memory must be pinned (page-locked) and mapped: the restore kernel
  *     reads it directly over the host link.  All buffers are owned by the caller (allocate
  *     them with any CUDA allocator, e.g. torch); the library never frees them and only owns
- *     small internals (events, a few hundred bytes of device scratch).
+ *     small internals (events, a few KB of device scratch, one fp64 reduction partial per 16384 elements).
  *   - Streams are cudaStream_t passed as void*.  Calls that take a stream only ENQUEUE work;
  *     they never block the host on the device unless stated.  The three hot calls
  *     (phx_step_and_snapshot, phx_snapshot_flush_async, phx_restore) never do.  Host-blocking by
@@ -198,7 +198,7 @@ PHX_API int phx_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len
 
 /* ---- a1+a2+a3: fused AdamW step + snapshot -------------------------------------------------
  * Enqueues on `stream`:
- *   a1 (only if max_grad_norm > 0): S = sum g^2 in fp64 by a fixed two-stage tree, clip
+ *   a1 (only if max_grad_norm > 0): S = sum g^2 in fp64 by a fixed tree whose shape depends on n alone, clip
  *      coefficient c = fp32(min(1, max_grad_norm / (sqrt(S) + 1e-6))) left in device memory;
  *   a2: wait (stream-side, not host-side) until the previous snapshot is committed (strict) or
  *      the staging slot about to be written has been drained (relaxed) — PAPER.md:226;
@@ -378,9 +378,9 @@ PHX_API int phx_params_guard(phx_shard_t *s, void *stream);
  * caller's exchange of D doubles (NCCL all-gather on the same stream; 8*D bytes):
  *
  *   phx_grad_sumsq_async(s, d_grads, d_out, stream)   S_r of this rank's gradient shard (same kernels, same
- *        fixed two-stage fp64 tree as the local a1) written to the caller-owned device double *d_out
+ *        fixed fp64 tree as the local a1) written to the caller-owned device double *d_out
  *        (8-byte aligned).  Needs a bound shard; does not touch the optimizer state or the step counter.
- *        It uses the handle's reduction scratch: enqueue it on the SAME stream as the step that follows.
+ *        It uses the handle's a1 reduction scratch: enqueue it on the SAME stream as the step that follows.
  *   [caller: all-gather the D values into a device array ordered by dp_rank]
  *   phx_set_clip_partials(s, d_partials, count)       ONE-SHOT: the next phx_step_and_snapshot skips its own
  *        sum-of-squares pass and takes S = d_partials[0] + ... + d_partials[count-1] (fixed tree, so every
@@ -402,13 +402,14 @@ PHX_API int phx_set_clip_partials(phx_shard_t *s, const double *d_partials, uint
  * one pass (4 B read + 2 B written per element; reading R34):
  *     g16_i = RNE_bf16(g32_i * scale)      one binary32 multiply (scale: gradient averaging; 1.0f exact), then
  *                                          the same rounding as the bf16 model-param copy
- *     *d_sumsq_out = sum_i widen(g16_i)^2  fp64, fixed two-stage tree, of the ROUNDED values — the very number
- *                                          a1 would compute from g16
+ *     *d_sumsq_out = sum_i widen(g16_i)^2  fp64, of the ROUNDED values, by the SAME fixed tree as a1 — the very
+ *                                          number, bit for bit, a1 would compute from g16
  * d_main_grads_fp32: float[n_padded] (pad lanes zero), d_grads_bf16_out: bf16[n_padded], both 256-byte
  * aligned, not overlapping; d_sumsq_out: device double, 8-byte aligned.  Then
  *     phx_set_clip_partials(s, d_sumsq_out, 1);  phx_step_and_snapshot(s, d_grads_bf16_out, ...)
- * runs the step with NO sum-of-squares pass (40 instead of 42 B/element on the critical path).  Uses the
- * handle's reduction scratch: same stream as the step.  PHX_PRECISION_BF16_GRADS only. */
+ * runs the step with NO sum-of-squares pass (40 instead of 42 B/element on the critical path).  It has a
+ * reduction scratch of its own inside the handle (it may run on the producer's stream while a step with its own
+ * a1 pass runs on another); two epilogues of one handle must be stream-ordered.  PHX_PRECISION_BF16_GRADS only. */
 PHX_API int phx_grads_finalize_async(phx_shard_t *s, const float *d_main_grads_fp32, float scale,
                                      void *d_grads_bf16_out, double *d_sumsq_out, void *stream);
 
@@ -424,7 +425,11 @@ PHX_API int phx_grads_finalize_async(phx_shard_t *s, const float *d_main_grads_f
  *
  *   phx_graph_begin(s, lr, beta1, beta2, eps, wd, stream)   mode switch (host-blocking: lands this handle's eager
  *        flushes), initialises the step block at last_step on `stream`.  An un-flushed eager snapshot becomes
- *        the first phx_graph_flush_async's work.  Not available with PHX_PAYLOAD_FULL_RANK_STATE.
+ *        the first phx_graph_flush_async's work.  With PHX_PAYLOAD_FULL_RANK_STATE (§8(f4)) the protocol is
+ *        the eager one with the same two calls, which become edges of the captured graph between begin and end:
+ *        phx_params_ready(stream) before the flush of that step (else PHX_ERR_PARAMS_NOT_READY),
+ *        phx_params_guard(stream) ahead of whatever overwrites W; a declaration made eagerly for a still
+ *        pending snapshot carries over in both directions.
  *   phx_graph_set_hyper(...)                                 stream-ordered update of the hyperparameters (learning-
  *        rate schedules) between replays; not captured itself.
  *   phx_graph_step_and_snapshot(s, d_grads, stream)          a1 (if configured) + a2 + prologue + a3, capturable.  The

@@ -45,8 +45,7 @@ constexpr size_t kScrZeroHdr = 0;      // 256 zero bytes: invalidates a host slo
 constexpr size_t kScrOne = 256;        // float 1.0f: clip coefficient when clipping is off
 constexpr size_t kScrCoef = 260;       // float: clip coefficient of the current step
 constexpr size_t kScrSumsq = 264;      // double
-constexpr size_t kScrPartials = 512;   // kSumsqMaxBlocks doubles
-constexpr size_t kScrHdr = kScrPartials + phx::kSumsqMaxBlocks * sizeof(double);  // 2 x 256 B headers (direct mode)
+constexpr size_t kScrHdr = 512;        // 2 x 256 B headers (direct mode)
 constexpr size_t kScrHdrFull = kScrHdr + 2 * 256;  // kMaxDepth x 256 B full-rank-state headers (§8(f4))
 constexpr size_t kScrBlock = kScrHdrFull + 4 * 256;  // phx::StepBlock of the graph-capturable form
 constexpr size_t kScrBytes = kScrBlock + 1024;
@@ -91,6 +90,7 @@ struct phx_shard {
     uint8_t *h_replica = nullptr;
     uint8_t *d_replica = nullptr;  // device view of h_replica
     uint8_t *d_scratch = nullptr;
+    double *d_partials = nullptr;  // 2 x sumsq_partials_count(n_padded): [a1 / phx_grad_sumsq_async | producer epilogue]
     int sm_count = 148;
     // decay groups: class per 2048-element tile and the offsets where the flag toggles
     std::vector<uint8_t> decay_cls;
@@ -158,6 +158,9 @@ struct phx_shard {
     uint64_t g_pending_peer_step = 0;
     int g_last_pflush_slot = -1;
     GraphEvent gev_step[kMaxDepth], gev_flush[kMaxDepth], gev_pflush[kMaxDepth];
+    GraphEvent gev_params, gev_wflush;  // §8(f4) in the graph form: W complete for g_params_step / newest flush done reading W
+    uint64_t g_params_step = 0;
+    bool g_params_ready = false;
 };
 
 #define PHX_CK(call)                                  \
@@ -296,8 +299,32 @@ int settle_peer_slots(phx_shard *s, bool block) { return settle_slots(s, s->peer
 // chunks and never commit (fault injection).
 // full = true (§8(f4), local slot only): the model-parameter buffer W goes first, behind the optimizer part,
 // and the committed header is the full-rank-state one; ev_wflush marks the end of the reads of W.
+// graph-form events: a dependency edge inside a capture, a plain stream wait outside
+unsigned long long capture_id(cudaStream_t st)
+{
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    unsigned long long id = 0;
+    if (cudaStreamGetCaptureInfo(st, &cs, &id) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 0;
+    }
+    return cs == cudaStreamCaptureStatusActive ? id : 0;
+}
+int gev_record(phx_shard *s, GraphEvent &g, cudaStream_t st)
+{
+    PHX_CK(cudaEventRecord(g.ev, st));
+    g.cap = capture_id(st);
+    g.valid = true;
+    return PHX_OK;
+}
+int gev_wait(phx_shard *s, const GraphEvent &g, cudaStream_t st)
+{
+    if (g.valid && g.cap == capture_id(st)) PHX_CK(cudaStreamWaitEvent(st, g.ev, 0));
+    return PHX_OK;
+}
+
 int enqueue_snapshot_copy(phx_shard *s, cudaStream_t st, uint8_t *dst, cudaMemcpyKind kind, int slot, int64_t torn_chunks,
-                          bool full = false)
+                          bool full = false, GraphEvent *gev_w = nullptr)
 {
     const bool direct = direct_mode(s);
     const uint8_t *src = direct ? nullptr : s->d_staging + (uint64_t)slot * s->info.slot_stride;
@@ -321,8 +348,13 @@ int enqueue_snapshot_copy(phx_shard *s, cudaStream_t st, uint8_t *dst, cudaMemcp
             const uint64_t len = s->info.param_bytes - off < chunk ? s->info.param_bytes - off : chunk;
             PHX_CK(cudaMemcpyAsync(wdst + off, s->d_W + off, len, kind, st));
         }
-        PHX_CK(cudaEventRecord(s->ev_wflush, st));
-        s->wflush_valid = true;
+        if (gev_w) {  // graph form: an edge of the captured graph, not the eager event
+            const int rcw = gev_record(s, *gev_w, st);
+            if (rcw != PHX_OK) return rcw;
+        } else {
+            PHX_CK(cudaEventRecord(s->ev_wflush, st));
+            s->wflush_valid = true;
+        }
     }
     for (uint64_t off = 0; off < payload && !stopped; off += chunk, ++done_chunks) {
         if (torn && (int64_t)done_chunks >= torn_chunks) break;
@@ -481,9 +513,12 @@ int phx_shard_destroy(phx_shard_t *s)
             if (s->gev_flush[k].ev) cudaEventDestroy(s->gev_flush[k].ev);
             if (s->gev_pflush[k].ev) cudaEventDestroy(s->gev_pflush[k].ev);
         }
+        if (s->gev_params.ev) cudaEventDestroy(s->gev_params.ev);
+        if (s->gev_wflush.ev) cudaEventDestroy(s->gev_wflush.ev);
         if (s->ev_params) cudaEventDestroy(s->ev_params);
         if (s->ev_wflush) cudaEventDestroy(s->ev_wflush);
         if (s->d_scratch) cudaFree(s->d_scratch);
+        if (s->d_partials) cudaFree(s->d_partials);
         if (s->d_decay) cudaFree(s->d_decay);
     }
     delete s;
@@ -540,6 +575,7 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
     }
     PHX_CK(cudaMalloc(reinterpret_cast<void **>(&s->d_scratch), kScrBytes));
     PHX_CK(cudaMemset(s->d_scratch, 0, kScrBytes));
+    PHX_CK(cudaMalloc(reinterpret_cast<void **>(&s->d_partials), 2 * phx::sumsq_partials_count(s->info.n_padded) * sizeof(double)));
     const float one = 1.0f;
     PHX_CK(cudaMemcpy(s->d_scratch + kScrOne, &one, 4, cudaMemcpyHostToDevice));
     PHX_CK(cudaMemcpy(s->d_scratch + kScrCoef, &one, 4, cudaMemcpyHostToDevice));
@@ -555,6 +591,8 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
         PHX_CK(cudaEventCreateWithFlags(&s->gev_flush[k].ev, cudaEventDisableTiming));
         PHX_CK(cudaEventCreateWithFlags(&s->gev_pflush[k].ev, cudaEventDisableTiming));
     }
+    PHX_CK(cudaEventCreateWithFlags(&s->gev_params.ev, cudaEventDisableTiming));
+    PHX_CK(cudaEventCreateWithFlags(&s->gev_wflush.ev, cudaEventDisableTiming));
     PHX_CK(cudaEventCreateWithFlags(&s->ev_params, cudaEventDisableTiming));
     PHX_CK(cudaEventCreateWithFlags(&s->ev_wflush, cudaEventDisableTiming));
     for (int k = 0; k < 2; ++k) {
@@ -621,29 +659,6 @@ void derive_scalars_host(float lr, float beta1, float beta2, float eps, float wd
     sc->sbc2 = (float)std::sqrt(1.0 - b2t);
 }
 
-unsigned long long capture_id(cudaStream_t st)
-{
-    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-    unsigned long long id = 0;
-    if (cudaStreamGetCaptureInfo(st, &cs, &id) != cudaSuccess) {
-        (void)cudaGetLastError();
-        return 0;
-    }
-    return cs == cudaStreamCaptureStatusActive ? id : 0;
-}
-int gev_record(phx_shard *s, GraphEvent &g, cudaStream_t st)
-{
-    PHX_CK(cudaEventRecord(g.ev, st));
-    g.cap = capture_id(st);
-    g.valid = true;
-    return PHX_OK;
-}
-int gev_wait(phx_shard *s, const GraphEvent &g, cudaStream_t st)
-{
-    if (g.valid && g.cap == capture_id(st)) PHX_CK(cudaStreamWaitEvent(st, g.ev, 0));
-    return PHX_OK;
-}
-
 // a1: optional clip — from the one-shot partials the caller exchanged (§8(e), §8(f4b)) or by the shard's own pass
 int enqueue_clip(phx_shard *s, const void *d_grads, phx::StepArgs &a, cudaStream_t st)
 {
@@ -659,8 +674,7 @@ int enqueue_clip(phx_shard *s, const void *d_grads, phx::StepArgs &a, cudaStream
         s->clip_count = 0;
     } else {
         int nl = 0;
-        PHX_CK(phx::launch_sumsq_clip(d_grads, fp32_mode(s), s->info.n_padded, s->cfg.max_grad_norm,
-                                      reinterpret_cast<double *>(s->d_scratch + kScrPartials),
+        PHX_CK(phx::launch_sumsq_clip(d_grads, fp32_mode(s), s->info.n_padded, s->cfg.max_grad_norm, s->d_partials,
                                       reinterpret_cast<double *>(s->d_scratch + kScrSumsq),
                                       reinterpret_cast<float *>(s->d_scratch + kScrCoef), st, &nl));
         s->launches += nl;
@@ -1215,6 +1229,13 @@ int phx_params_ready(phx_shard_t *s, void *stream)
 {
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound || !s->d_W) return PHX_ERR_NOT_BOUND;
+    if (s->graph) {  // graph form: the declaration is an edge of the captured graph
+        const int rc = gev_record(s, s->gev_params, static_cast<cudaStream_t>(stream));
+        if (rc != PHX_OK) return rc;
+        s->g_params_ready = true;
+        s->g_params_step = s->g_issue;
+        return PHX_OK;
+    }
     PHX_CK(cudaEventRecord(s->ev_params, static_cast<cudaStream_t>(stream)));
     s->params_ready = true;
     s->params_ready_step = s->last_step;
@@ -1225,6 +1246,7 @@ int phx_params_guard(phx_shard_t *s, void *stream)
 {
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound || !s->d_W) return PHX_ERR_NOT_BOUND;
+    if (s->graph) return gev_wait(s, s->gev_wflush, static_cast<cudaStream_t>(stream));
     if (s->wflush_valid) PHX_CK(cudaStreamWaitEvent(static_cast<cudaStream_t>(stream), s->ev_wflush, 0));
     return PHX_OK;
 }
@@ -1244,8 +1266,7 @@ int phx_grad_sumsq_async(phx_shard_t *s, const void *d_grads, double *d_out, voi
     if (!s->bound) return PHX_ERR_NOT_BOUND;
     if (!aligned256(d_grads) || (reinterpret_cast<uintptr_t>(d_out) & 7u)) return PHX_ERR_ALIGNMENT;
     int nl = 0;
-    PHX_CK(phx::launch_sumsq(d_grads, fp32_mode(s), s->info.n_padded,
-                             reinterpret_cast<double *>(s->d_scratch + kScrPartials), d_out,
+    PHX_CK(phx::launch_sumsq(d_grads, fp32_mode(s), s->info.n_padded, s->d_partials, d_out,
                              static_cast<cudaStream_t>(stream), &nl));
     s->launches += nl;
     return PHX_OK;
@@ -1311,7 +1332,7 @@ int phx_grads_finalize_async(phx_shard_t *s, const float *d_main_grads_fp32, flo
     if (in0 < out0 + 2 * N && out0 < in0 + 4 * N) return PHX_ERR_INVALID_ARG;  // the two arrays must not overlap
     int nl = 0;
     PHX_CK(phx::launch_grads_finalize(d_main_grads_fp32, scale, d_grads_bf16_out, N,
-                                      reinterpret_cast<double *>(s->d_scratch + kScrPartials), d_sumsq_out,
+                                      s->d_partials + phx::sumsq_partials_count(N), d_sumsq_out,
                                       static_cast<cudaStream_t>(stream), &nl));
     s->launches += nl;
     return PHX_OK;
@@ -1358,7 +1379,7 @@ int phx_graph_begin(phx_shard_t *s, float lr, float beta1, float beta2, float ep
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound) return PHX_ERR_NOT_BOUND;
     if (s->graph) return PHX_ERR_GRAPH_MODE;
-    if (full_payload(s)) return PHX_ERR_INVALID_ARG;  // the params_ready protocol of §8(f4) is eager-only
+    if (full_payload(s) && !s->d_W) return PHX_ERR_NOT_BOUND;
     // a mode switch, not a hot call: every eager flush of this handle lands before the first captured / replayed
     // step may touch what it reads
     int rc = settle_host_slots(s, true);
@@ -1381,6 +1402,10 @@ int phx_graph_begin(phx_shard_t *s, float lr, float beta1, float beta2, float ep
     s->g_pending_peer_step = s->pending_peer_step;
     s->g_last_pflush_slot = -1;
     for (int k = 0; k < kMaxDepth; ++k) s->gev_step[k].valid = s->gev_flush[k].valid = s->gev_pflush[k].valid = false;
+    s->gev_params.valid = s->gev_wflush.valid = false;
+    // an eager declaration for the pending snapshot carries over (the eager events have all been settled above)
+    s->g_params_ready = s->params_ready;
+    s->g_params_step = s->params_ready_step;
     return PHX_OK;
 }
 
@@ -1421,6 +1446,8 @@ int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *strea
         } else {
             if ((rc = gev_wait(s, s->gev_flush[slot], st)) != PHX_OK) return rc;
             if ((rc = gev_wait(s, s->gev_pflush[slot], st)) != PHX_OK) return rc;
+            // §8(f4): the kernel rewrites this rank's range of W, which the newest full-rank-state flush reads
+            if (full_payload(s) && (rc = gev_wait(s, s->gev_wflush, st)) != PHX_OK) return rc;
         }
         if (s->g_pending_slot >= 0 && s->h_replica) s->dropped_host += 1;
         if (s->g_pending_peer_slot >= 0 && s->n_peers) s->dropped_peers += 1;
@@ -1429,7 +1456,14 @@ int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *strea
     void *shdr = a.shdr;
     a.shdr = nullptr;  // the prologue writes the envelope; the fused kernel only moves elements
     a.dsc = &step_block(s)->sc;
-    PHX_CK(phx::launch_step_prologue(step_block(s), shdr, nullptr, 0u, snap ? (uint32_t)slot : 0u, snap ? depth : 0u, st));
+    void *shdr_full = nullptr;
+    uint32_t full_word = 0u;
+    if (snap && full_payload(s)) {  // §8(f4): the local slot's envelope differs in the payload word and the hash
+        shdr_full = s->d_scratch + kScrHdrFull + (size_t)slot * kHeaderBytes;
+        full_word = full_payload_word(s);
+    }
+    PHX_CK(phx::launch_step_prologue(step_block(s), shdr, shdr_full, full_word, snap ? (uint32_t)slot : 0u,
+                                     snap ? depth : 0u, st));
     PHX_CK(phx::launch_step(a, snap && !direct_mode(s), step_mode(s), true, st));
     s->launches += 1 + (s->info.n_padded ? 1 : 0);
     if (snap) {
@@ -1442,6 +1476,7 @@ int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *strea
         }
     }
     s->g_issue = step;
+    s->g_params_ready = false;
     return PHX_OK;
 }
 
@@ -1457,9 +1492,15 @@ int phx_graph_flush_async(phx_shard_t *s, void *side_stream)
     const int hs = (int)(s->g_pending_step & 1);  // ping-pong; kept on a replay by the alignment rule
     uint8_t *dst = s->h_replica + (uint64_t)hs * s->info.host_slot_stride;
     int rc;
+    const bool full = full_payload(s);
+    if (full) {
+        if (!s->d_W) return PHX_ERR_NOT_BOUND;
+        if (!s->g_params_ready || s->g_params_step != s->g_pending_step) return PHX_ERR_PARAMS_NOT_READY;
+        if ((rc = gev_wait(s, s->gev_params, st)) != PHX_OK) return rc;  // the all-gather of this step has landed in W
+    }
     if ((rc = gev_wait(s, s->gev_step[slot], st)) != PHX_OK) return rc;  // the step's kernel has written the slot
     if (s->g_last_flush_slot >= 0 && (rc = gev_wait(s, s->gev_flush[s->g_last_flush_slot], st)) != PHX_OK) return rc;
-    rc = enqueue_snapshot_copy(s, st, dst, cudaMemcpyDeviceToHost, slot, -1, false);
+    rc = enqueue_snapshot_copy(s, st, dst, cudaMemcpyDeviceToHost, slot, -1, full, full ? &s->gev_wflush : nullptr);
     if (rc != PHX_OK) return rc;
     if ((rc = gev_record(s, s->gev_flush[slot], st)) != PHX_OK) return rc;
     s->g_last_flush_slot = slot;
@@ -1511,13 +1552,16 @@ int phx_graph_end(phx_shard_t *s, uint64_t *last_step)
     s->last_step = blk.step;
     // the eager bookkeeping restarts from what is self-describing: the envelopes in the host slots
     for (int k = 0; k < kMaxDepth; ++k) s->flush_valid[k] = s->pflush_valid[k] = false;
+    s->wflush_valid = false;  // nothing is reading W any more (device synchronised above)
+    s->params_ready = s->g_params_ready && s->g_params_step == blk.step;
+    s->params_ready_step = s->g_params_step;
     s->last_flush_slot = s->last_pflush_slot = -1;
     s->pending_slot = s->pending_peer_slot = -1;
     uint64_t newest = 0;
     for (int i = 0; i < 2 && s->h_replica; ++i) {
         phx_snapshot_header_t h;
         std::memcpy(&h, s->h_replica + (uint64_t)i * s->info.host_slot_stride, sizeof(h));
-        const bool ok = header_valid(&h) && header_matches(s, &h) && h.payload == 0u;
+        const bool ok = header_valid(&h) && header_matches(s, &h) && h.payload == (full_payload(s) ? full_payload_word(s) : 0u);
         s->host[i].state = ok ? SLOT_COMMITTED : SLOT_EMPTY;
         s->host[i].step = ok ? h.step : 0;
         if (ok) s->host[i].hdr = h;

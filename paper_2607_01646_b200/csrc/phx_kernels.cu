@@ -462,29 +462,17 @@ __device__ __forceinline__ void sq_acc4(double &a0, double &a1, const uint4 &w)
     }
 }
 
-// 256-bit loads (LDG.E.256, 16 gradients each), four in flight per thread: 128 B per thread, 128 KB per SM.
-__global__ void __launch_bounds__(256) k_sumsq_partial(const float *__restrict__ g, uint64_t nunits,
-                                                       double *__restrict__ partials)
+// The three reduction kernels below share ONE shape (profiles/r02_structure_probe.md: short-lived CTAs stream
+// 8-12 % faster than a persistent grid-stride loop on every read:write mix):
+//   one-shot CTAs of 256 threads; thread t of CTA b takes the kSumsqK groups (b*kSumsqK + j)*256 + t, j = 0..K-1,
+//   of 8 consecutive elements each, issues all its loads at once, accumulates in TWO fixed chains (low halves /
+//   even elements, high halves / odd elements, groups in order j), adds the chains, and the CTA reduces
+//   (xor-shuffle tree, then the 8 warp sums in order) to partials[b].  k_sumsq_final folds the
+//   ceil(ngroups / (256 K)) partials: thread t sums partials[t], partials[t + 1024], ... in order, then a
+//   1024-wide tree.  The shape depends on n alone => deterministic run to run, and IDENTICAL between a1 over
+//   bf16 gradients and the producer epilogue over the same (rounded) values: the two sums are equal bit for bit.
+__device__ __forceinline__ void block_reduce_to_partial(double acc, double *__restrict__ partials)
 {
-    double acc = 0.0, acc1 = 0.0;  // two chains: low halves, high halves (fixed association => deterministic)
-    const uint64_t stride = (uint64_t)gridDim.x * 256;
-    uint64_t gi = (uint64_t)blockIdx.x * 256 + threadIdx.x;
-    auto add = [&](const F8 &f) {
-        uint4 a, b;
-        a.x = __float_as_uint(f.x[0]); a.y = __float_as_uint(f.x[1]); a.z = __float_as_uint(f.x[2]); a.w = __float_as_uint(f.x[3]);
-        b.x = __float_as_uint(f.x[4]); b.y = __float_as_uint(f.x[5]); b.z = __float_as_uint(f.x[6]); b.w = __float_as_uint(f.x[7]);
-        sq_acc4(acc, acc1, a);
-        sq_acc4(acc, acc1, b);
-    };
-    for (; gi + 3 * stride < nunits; gi += 4 * stride) {
-        F8 w[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) w[k] = ldg256_stream(g + ((gi + k * stride) << 3));
-#pragma unroll
-        for (int k = 0; k < 4; ++k) add(w[k]);
-    }
-    for (; gi < nunits; gi += stride) add(ldg256_stream(g + (gi << 3)));
-    acc += acc1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
     __shared__ double wsum[8];
@@ -496,6 +484,27 @@ __global__ void __launch_bounds__(256) k_sumsq_partial(const float *__restrict__
         for (int k = 1; k < 8; ++k) s += wsum[k];
         partials[blockIdx.x] = s;
     }
+}
+
+// a1 over bf16 gradients: 128-bit loads (8 gradients each), kSumsqBatchA1 in flight per thread.
+__global__ void __launch_bounds__(256) k_sumsq_partial(const uint16_t *__restrict__ g, uint64_t ngroups,
+                                                       double *__restrict__ partials)
+{
+    double acc = 0.0, acc1 = 0.0;
+    const uint64_t g0 = (uint64_t)blockIdx.x * (256 * kSumsqK) + threadIdx.x;
+#pragma unroll 1
+    for (int b = 0; b < kSumsqK; b += kSumsqBatchA1) {
+        uint4 w[kSumsqBatchA1];
+#pragma unroll
+        for (int j = 0; j < kSumsqBatchA1; ++j) {
+            const uint64_t gi = g0 + (uint64_t)(b + j) * 256;
+            w[j] = gi < ngroups ? ldg128_stream(g + (gi << 3)) : make_uint4(0u, 0u, 0u, 0u);
+        }
+#pragma unroll
+        for (int j = 0; j < kSumsqBatchA1; ++j)
+            if (g0 + (uint64_t)(b + j) * 256 < ngroups) sq_acc4(acc, acc1, w[j]);
+    }
+    block_reduce_to_partial(acc + acc1, partials);
 }
 
 // binary32 gradients: the square of a widened fp32 value is exact in fp64 (48 bits),
@@ -509,42 +518,38 @@ __device__ __forceinline__ double sq_acc_f32(double acc, float g)
 __global__ void __launch_bounds__(256) k_sumsq_partial_f32(const float *__restrict__ g, uint64_t ngroups,
                                                            double *__restrict__ partials)
 {
-    double acc = 0.0;
-    const uint64_t stride = (uint64_t)gridDim.x * 256;
-    uint64_t gi = (uint64_t)blockIdx.x * 256 + threadIdx.x;
-    for (; gi + stride < ngroups; gi += 2 * stride) {
-        F8 w[2];
+    double acc = 0.0, acc1 = 0.0;
+    const uint64_t g0 = (uint64_t)blockIdx.x * (256 * kSumsqK) + threadIdx.x;
+#pragma unroll 1
+    for (int b = 0; b < kSumsqK; b += kSumsqBatchG32) {
+        F8 w[kSumsqBatchG32];
 #pragma unroll
-        for (int k = 0; k < 2; ++k) w[k] = ldg256_stream(g + ((gi + k * stride) << 3));
+        for (int j = 0; j < kSumsqBatchG32; ++j) {
+            const uint64_t gi = g0 + (uint64_t)(b + j) * 256;
+            if (gi < ngroups) w[j] = ldg256_stream(g + (gi << 3));
+        }
 #pragma unroll
-        for (int k = 0; k < 2; ++k)
+        for (int j = 0; j < kSumsqBatchG32; ++j)
+            if (g0 + (uint64_t)(b + j) * 256 < ngroups) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) acc = sq_acc_f32(acc, w[k].x[j]);
+                for (int e = 0; e < 8; e += 2) {
+                    acc = sq_acc_f32(acc, w[j].x[e]);
+                    acc1 = sq_acc_f32(acc1, w[j].x[e + 1]);
+                }
+            }
     }
-    for (; gi < ngroups; gi += stride) {
-        const F8 w = ldg256_stream(g + (gi << 3));
-#pragma unroll
-        for (int j = 0; j < 8; ++j) acc = sq_acc_f32(acc, w.x[j]);
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
-    __shared__ double wsum[8];
-    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double s = wsum[0];
-#pragma unroll
-        for (int k = 1; k < 8; ++k) s += wsum[k];
-        partials[blockIdx.x] = s;
-    }
+    block_reduce_to_partial(acc + acc1, partials);
 }
 
-__global__ void __launch_bounds__(kSumsqMaxBlocks) k_sumsq_final(const double *__restrict__ partials, int nblocks,
+__global__ void __launch_bounds__(kSumsqMaxBlocks) k_sumsq_final(const double *__restrict__ partials, uint64_t count,
                                                                  float max_norm, double *__restrict__ out_sumsq,
                                                                  float *__restrict__ out_coef)
 {
     __shared__ double sh[kSumsqMaxBlocks];
-    sh[threadIdx.x] = (int)threadIdx.x < nblocks ? partials[threadIdx.x] : 0.0;
+    double a = 0.0;  // 0.0 + x == x: for count <= 1024 this is the plain 1024-wide tree over the partials
+#pragma unroll 8
+    for (uint64_t i = threadIdx.x; i < count; i += kSumsqMaxBlocks) a += partials[i];
+    sh[threadIdx.x] = a;
     __syncthreads();
     for (int o = kSumsqMaxBlocks / 2; o > 0; o >>= 1) {
         if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
@@ -559,17 +564,20 @@ __global__ void __launch_bounds__(kSumsqMaxBlocks) k_sumsq_final(const double *_
     }
 }
 
+uint64_t sumsq_partials_count(uint64_t n_padded)
+{
+    const uint64_t ngroups = n_padded >> 3, per = 256ull * kSumsqK;
+    const uint64_t c = (ngroups + per - 1) / per;
+    return c < 1 ? 1 : c;
+}
+
 cudaError_t launch_sumsq_clip(const void *g, bool grads_f32, uint64_t n_padded, float max_norm, double *partials,
                               double *out_sumsq, float *out_coef, cudaStream_t st, int *n_launches)
 {
-    const uint64_t ngroups = n_padded >> 3;
-    uint64_t want = (ngroups + 255) / 256;
-    // 148 SMs x 4 resident CTAs; fixed by n alone, so the summation tree is the same run to run.  (444-1024
-    // blocks and 128- vs 256-bit loads time within 1 % of each other: 130 us for 0.84 GB at c3.)
-    int nblocks = (int)(want < 592 ? want : 592);
-    if (nblocks < 1) nblocks = 1;
-    if (grads_f32) k_sumsq_partial_f32<<<nblocks, 256, 0, st>>>(reinterpret_cast<const float *>(g), ngroups, partials);
-    else k_sumsq_partial<<<nblocks, 256, 0, st>>>(reinterpret_cast<const float *>(g), n_padded >> 4, partials);
+    const uint64_t ngroups = n_padded >> 3, nblocks = sumsq_partials_count(n_padded);
+    if (nblocks > 0x7FFFFFFFull) return cudaErrorInvalidValue;
+    if (grads_f32) k_sumsq_partial_f32<<<(unsigned)nblocks, 256, 0, st>>>(reinterpret_cast<const float *>(g), ngroups, partials);
+    else k_sumsq_partial<<<(unsigned)nblocks, 256, 0, st>>>(reinterpret_cast<const uint16_t *>(g), ngroups, partials);
     k_sumsq_final<<<1, kSumsqMaxBlocks, 0, st>>>(partials, nblocks, max_norm, out_sumsq, out_coef);
     if (n_launches) *n_launches = 2;
     return cudaGetLastError();
@@ -587,7 +595,7 @@ cudaError_t launch_clip_from_partials(const double *partials, uint32_t count, fl
                                       float *out_coef, cudaStream_t st)
 {
     if (count < 1 || count > (uint32_t)kSumsqMaxBlocks) return cudaErrorInvalidValue;
-    k_sumsq_final<<<1, kSumsqMaxBlocks, 0, st>>>(partials, (int)count, max_norm, out_sumsq, out_coef);
+    k_sumsq_final<<<1, kSumsqMaxBlocks, 0, st>>>(partials, count, max_norm, out_sumsq, out_coef);
     return cudaGetLastError();
 }
 
@@ -597,53 +605,45 @@ cudaError_t launch_clip_from_partials(const double *partials, uint32_t count, fl
 // writes the optimizer's bf16 gradients  g16 = RNE_bf16(g32 * scale)  and leaves the fp64 per-block sums
 // of widen(g16)^2 — the squares of the ROUNDED values, i.e. exactly what a1 would compute from g16 — so
 // that the step needs no pass of its own over the gradients (phx_set_clip_partials, count = 1).
-// 4 B read + 2 B written per element; same fixed two-stage tree as a1 (deterministic run to run).
+// 4 B read + 2 B written per element; the same one-shot shape and tree as a1 => the same sum, bit for bit.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_grads_finalize(const float *__restrict__ g32, float scale, void *__restrict__ g16,
                                                         uint64_t ngroups, double *__restrict__ partials)
 {
     double acc = 0.0, acc1 = 0.0;
-    const uint64_t stride = (uint64_t)gridDim.x * 256;
-    uint64_t gi = (uint64_t)blockIdx.x * 256 + threadIdx.x;
-    auto one = [&](const F8 &f, uint64_t g) {
-        uint4 h;  // cvt.rn.bf16x2.f32 of the individually rounded products
-        h.x = pack_bf16x2(__fmul_rn(f.x[0], scale), __fmul_rn(f.x[1], scale));
-        h.y = pack_bf16x2(__fmul_rn(f.x[2], scale), __fmul_rn(f.x[3], scale));
-        h.z = pack_bf16x2(__fmul_rn(f.x[4], scale), __fmul_rn(f.x[5], scale));
-        h.w = pack_bf16x2(__fmul_rn(f.x[6], scale), __fmul_rn(f.x[7], scale));
-        st128u(reinterpret_cast<uint16_t *>(g16) + (g << 3), h);
-        sq_acc4(acc, acc1, h);
-    };
-    for (; gi + 3 * stride < ngroups; gi += 4 * stride) {
-        F8 w[4];
+    const uint64_t g0 = (uint64_t)blockIdx.x * (256 * kSumsqK) + threadIdx.x;
+#pragma unroll 1
+    for (int b = 0; b < kSumsqK; b += kSumsqBatchF32) {
+        F8 w[kSumsqBatchF32];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) w[k] = ldg256_stream(g32 + ((gi + k * stride) << 3));
+        for (int j = 0; j < kSumsqBatchF32; ++j) {
+            const uint64_t gi = g0 + (uint64_t)(b + j) * 256;
+            if (gi < ngroups) w[j] = ldg256_stream(g32 + (gi << 3));
+        }
 #pragma unroll
-        for (int k = 0; k < 4; ++k) one(w[k], gi + k * stride);
+        for (int j = 0; j < kSumsqBatchF32; ++j) {
+            const uint64_t gi = g0 + (uint64_t)(b + j) * 256;
+            if (gi < ngroups) {
+                const F8 &f = w[j];
+                uint4 h;  // cvt.rn.bf16x2.f32 of the individually rounded products
+                h.x = pack_bf16x2(__fmul_rn(f.x[0], scale), __fmul_rn(f.x[1], scale));
+                h.y = pack_bf16x2(__fmul_rn(f.x[2], scale), __fmul_rn(f.x[3], scale));
+                h.z = pack_bf16x2(__fmul_rn(f.x[4], scale), __fmul_rn(f.x[5], scale));
+                h.w = pack_bf16x2(__fmul_rn(f.x[6], scale), __fmul_rn(f.x[7], scale));
+                st128u(reinterpret_cast<uint16_t *>(g16) + (gi << 3), h);
+                sq_acc4(acc, acc1, h);
+            }
+        }
     }
-    for (; gi < ngroups; gi += stride) one(ldg256_stream(g32 + (gi << 3)), gi);
-    acc += acc1;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
-    __shared__ double wsum[8];
-    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double s = wsum[0];
-#pragma unroll
-        for (int k = 1; k < 8; ++k) s += wsum[k];
-        partials[blockIdx.x] = s;
-    }
+    block_reduce_to_partial(acc + acc1, partials);
 }
 
 cudaError_t launch_grads_finalize(const float *g32, float scale, void *g16, uint64_t n_padded, double *partials,
                                   double *out_sumsq, cudaStream_t st, int *n_launches)
 {
-    const uint64_t ngroups = n_padded >> 3;
-    uint64_t want = (ngroups + 255) / 256;
-    int nblocks = (int)(want < 592 ? want : 592);  // 148 SMs x 4 resident CTAs; fixed by n alone
-    if (nblocks < 1) nblocks = 1;
-    k_grads_finalize<<<nblocks, 256, 0, st>>>(g32, scale, g16, ngroups, partials);
+    const uint64_t ngroups = n_padded >> 3, nblocks = sumsq_partials_count(n_padded);
+    if (nblocks > 0x7FFFFFFFull) return cudaErrorInvalidValue;
+    k_grads_finalize<<<(unsigned)nblocks, 256, 0, st>>>(g32, scale, g16, ngroups, partials);
     k_sumsq_final<<<1, kSumsqMaxBlocks, 0, st>>>(partials, nblocks, 0.0f, out_sumsq, nullptr);
     if (n_launches) *n_launches = 2;
     return cudaGetLastError();

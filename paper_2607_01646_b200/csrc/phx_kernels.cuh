@@ -74,8 +74,22 @@ cudaError_t launch_step_block_init(StepBlock *blk, float lr, float beta1, float 
 cudaError_t launch_derive_scalars(float lr, float beta1, float beta2, float wd, const uint64_t *d_steps, uint32_t n,
                                   float *d_out, cudaStream_t st);
 
-// a1.  partials: >= kSumsqMaxBlocks doubles of device scratch; out_sumsq/out_coef device scalars.
+// a1.  partials: >= sumsq_partials_count(n_padded) doubles of device scratch; out_sumsq/out_coef device scalars.
 enum { kSumsqMaxBlocks = 1024 };
+#ifndef PHX_SUMSQ_K
+#define PHX_SUMSQ_K 8
+#endif
+#ifndef PHX_SUMSQ_BATCH_A1
+#define PHX_SUMSQ_BATCH_A1 8
+#endif
+#ifndef PHX_SUMSQ_BATCH_F32
+#define PHX_SUMSQ_BATCH_F32 8
+#endif
+// kSumsqK: 8-element groups per thread of the short-lived reduction CTAs (part of the tree's shape);
+// kSumsqBatch*: how many of them a thread has in flight at once (loads issued together) — not part of the shape
+enum { kSumsqK = PHX_SUMSQ_K, kSumsqBatchA1 = PHX_SUMSQ_BATCH_A1, kSumsqBatchF32 = PHX_SUMSQ_BATCH_F32, kSumsqBatchG32 = 4 };
+static_assert(kSumsqK % kSumsqBatchA1 == 0 && kSumsqK % kSumsqBatchF32 == 0, "batches must tile the per-thread groups");
+uint64_t sumsq_partials_count(uint64_t n_padded);
 cudaError_t launch_sumsq_clip(const void *g, bool grads_f32, uint64_t n_padded, float max_norm, double *partials,
                               double *out_sumsq, float *out_coef, cudaStream_t st, int *n_launches);
 

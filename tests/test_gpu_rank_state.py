@@ -280,3 +280,86 @@ def test_full_payload_under_relaxed_sync_never_commits_a_W_of_the_next_step():
         assert np.array_equal(s.replica_slot(t).numpy(), snaps[t]), t
     assert_state_equal(s, fr.o, "full + relaxed")
     close_all(shards)
+
+
+@pytest.mark.parametrize("sync", [B.PHX_SYNC_STRICT, B.PHX_SYNC_RELAXED])
+def test_graph_form_with_full_rank_state_payload(sync):
+    """The graph-capturable form covers §8(f4) too: per iteration, for the D ranks of one DP group,
+    [params_ready -> full-rank-state flush(k-1) ‖ window] -> params_guard -> step k (fused publication), captured
+    once (two iterations per graph) and replayed; host slots byte-identical to oracle/rank_state.py, then an
+    in-place recovery from them back in the eager form."""
+    D, numels = 2, [60_000, 4097, 64]
+    wls, shards, ranks = build_group(numels, D, chunk=64 << 10, sync_mode=sync)
+    cap, side = torch.cuda.Stream(device=DEV), torch.cuda.Stream(device=DEV)
+    a = torch.randn(256, 256, device=DEV, dtype=torch.bfloat16)
+    c = torch.empty_like(a)
+    with torch.cuda.stream(cap):
+        torch.matmul(a, a, out=c)
+    torch.cuda.synchronize()
+    gbuf = [[torch.zeros(s.n_padded, dtype=torch.bfloat16, device=DEV) for _ in range(2)] for s in shards]
+
+    def load_grads(t):
+        for r, (wl, s, fr) in enumerate(zip(wls, shards, ranks)):
+            g = W.gen_grads(wl, s.segments, s.n_padded, t, seed=11 + r)
+            gbuf[r][t & 1].copy_(g)
+            fr.o.step(grad_record(g), **hp_of(wl), step=t)
+        Wo = R.publish([fr.o for fr in ranks])
+        for fr in ranks:
+            fr.W[:] = Wo
+            fr.snapshot()
+
+    for s in shards:
+        s.graph_begin(stream=cap)
+    # a full payload flush without the declaration is refused in the graph form as well
+    load_grads(1)
+    torch.cuda.synchronize()
+    for r, s in enumerate(shards):
+        s.graph_step(gbuf[r][1], stream=cap)
+    torch.cuda.synchronize()
+    assert B.lib().phx_graph_flush_async(shards[0].h, side.cuda_stream) == B.PHX_ERR_PARAMS_NOT_READY
+    snaps = {1: [fr.slots[1].copy() for fr in ranks]}
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=cap):
+        for i in range(2):
+            for s in shards:
+                s.params_ready(cap)                 # every rank's step k-1 (same capture stream) has published into W
+            side.wait_stream(cap)
+            for s in shards:
+                s.graph_flush(side)
+            torch.matmul(a, a, out=c)
+            for s in shards:
+                s.params_guard(cap)                 # no rank publishes step k into a W a flush still reads
+            for r, s in enumerate(shards):
+                s.graph_step(gbuf[r][i & 1], stream=cap)
+        cap.wait_stream(side)
+    t = 1
+    for _ in range(3):
+        for i in range(2):
+            t += 1
+            load_grads(t)
+            snaps[t] = [fr.slots[t % 2].copy() for fr in ranks]
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+    assert t == 7
+    for r, (s, fr) in enumerate(zip(shards, ranks)):
+        assert s.graph_end() == 7
+        assert_state_equal(s, fr.o, f"rank {r} after graph replays")
+        assert np.array_equal(w_bits(s), fr.W.view(np.uint8))
+        for step in (5, 6):
+            assert np.array_equal(s.replica_slot(step).numpy(), snaps[step][r]), (r, step)
+    # eager again: the newest snapshot (7) is still pending; declare, flush, then recover rank 1 in place
+    for s in shards:
+        s.params_ready()
+        s.flush_async(side)
+    for r, s in enumerate(shards):
+        s.wait(7)
+        assert np.array_equal(s.replica_slot(7).numpy(), snaps[7][r])
+    victim, vfr = shards[1], ranks[1]
+    victim.drop_live()
+    victim.W.zero_()
+    assert victim.restore() == 7
+    torch.cuda.synchronize()
+    assert_state_equal(victim, vfr.o, "in-place recovery after the graph form")
+    assert np.array_equal(w_bits(victim), vfr.W.view(np.uint8))
+    close_all(shards)
