@@ -206,3 +206,55 @@ def test_sum_of_squares_over_zeros_subnormals_and_extreme_exponents(n):
     torch.cuda.synchronize()
     assert np.isnan(out.item())
     s.close()
+
+
+_NCCL_CHILD = r"""
+import os, sys
+sys.path.insert(0, sys.argv[1]); sys.path.insert(0, os.path.join(sys.argv[1], "tests"))
+import numpy as np, torch, torch.distributed as dist
+from oracle import oracle as O
+from paper_2607_01646_b200 import binding as B, workloads as W
+from paper_2607_01646_b200.clip import GlobalClip
+from paper_2607_01646_b200.shard import Shard
+from gpu_util import DEV, assert_state_equal, grad_record, hp_of
+torch.cuda.set_device(0)
+dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device(DEV))
+assert dist.get_backend() == "nccl"
+wl = W.tiny_workload([300_000, 1234, 77], dp_size=1, grad_kind="heavy_tail", hyper=W.Hyper(max_grad_norm=0.01))
+s = Shard(wl, device=DEV, chunk_bytes=1 << 16)
+o = O.OracleShard(wl.layout(), 1, 0, chunk_bytes=1 << 16, max_grad_norm=0.01)
+p0 = W.init_params(s.n, s.n_padded, 5)
+s.p.copy_(p0); s.set_state(0); o.set_state(p0.numpy())
+gc = GlobalClip(s)                                   # default group = the NCCL world
+st = torch.cuda.Stream(device=DEV)                   # not the default stream: the exchange must follow `st`
+for t in range(1, 5):
+    g = W.gen_grads(wl, s.segments, s.n_padded, t, 11)
+    gd = g.to(DEV)
+    torch.cuda.synchronize()
+    gc.step_and_snapshot(gd, t, stream=st)           # sumsq -> NCCL all-gather -> coefficient -> fused step, no host sync
+    coef = o.step(grad_record(g), **hp_of(wl), step=t)
+    torch.cuda.synchronize()
+    c, S = B.phx_last_clip(s.h)
+    assert np.float32(c).view(np.uint32) == np.float32(o.last_coef).view(np.uint32), (t, c, o.last_coef)
+    assert_state_equal(s, o, f"nccl world-1 step {t}")
+s.close()
+dist.destroy_process_group()
+print("NCCL_CLIP_OK")
+"""
+
+
+def test_global_clip_through_a_real_nccl_all_gather():
+    """The branch of clip.gather_partials a GPU box takes — a CUDA-tensor all-gather on an NCCL group, enqueued on the
+    step's (non-default) stream — run on the one GPU there is (world of ONE rank: D = 1 is the local clip, so the
+    oracle is the pinned dp = 1 rule).  In a child process so that the NCCL communicator does not outlive the test."""
+    import os
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    r = subprocess.run([sys.executable, "-c", _NCCL_CHILD, root], capture_output=True, text=True, timeout=600, env=env)
+    assert r.returncode == 0 and "NCCL_CLIP_OK" in r.stdout, r.stdout[-2000:] + r.stderr[-4000:]
