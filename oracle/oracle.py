@@ -361,6 +361,37 @@ class OracleShard:
         self.restored_user = h["user"]
         return self.last_step
 
+    # -- a6 in two phases (reading R37) ---------------------------------
+    # "Execution resumes from the last completed step": the recomputed iteration's
+    # forward/backward reads only the model parameters; the moments are first read by its optimizer
+    # step.  Phase 1 brings back p and regenerates p16 ("parameters ready"); phase 2 brings back m, v.
+    # The state after both phases is the state after restore(); step() refuses to run in between.
+    def restore_params_first(self) -> int:
+        best = self.newest_committed()
+        if best is None:
+            raise OracleError("no committed snapshot")
+        s, h = best
+        if (h["layout_hash"] != self.layout_hash or h["dp"] != self.dp or h["tp"] != self.tp
+                or h["pp"] != self.pp or h["n_padded"] != self.n_padded or h["n"] != self.n):
+            raise OracleError("layout mismatch")
+        N4 = 4 * self.n_padded
+        self.p[:] = self.replica[s][HEADER_BYTES:HEADER_BYTES + N4].view(np.float32)
+        self.p16[:] = rne_bf16(self.p) if self.precision == "bf16" else 0
+        self._restoring = (s, h)
+        self.last_step = -1          # no optimizer step may run until restore_finish()
+        return h["step"]
+
+    def restore_finish(self) -> int:
+        s, h = self._restoring
+        N4 = 4 * self.n_padded
+        raw = self.replica[s]
+        self.m[:] = raw[HEADER_BYTES + N4:HEADER_BYTES + 2 * N4].view(np.float32)
+        self.v[:] = raw[HEADER_BYTES + 2 * N4:].view(np.float32)
+        self.last_step = h["step"]
+        self.restored_user = h["user"]
+        self._restoring = None
+        return self.last_step
+
     def drop_live(self):
         """'Drop the live shard' (BASELINE.json:configs[3], reading R16)."""
         self.p[:] = 0

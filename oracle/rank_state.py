@@ -151,3 +151,31 @@ class FullRankState:
         o.last_step = h["step"]
         o.restored_user = h["user"]
         return o.last_step
+
+    # -- R33 in two phases (reading R37): parameters (p, the bf16 copy, W) first, moments second ---
+    def restore_in_place_params_first(self) -> int:
+        best = self.newest_committed()
+        if best is None:
+            raise O.OracleError("no committed full rank state in the local slots")
+        s, h = best
+        o = self.o
+        raw = self.slots[s]
+        H, N4 = O.HEADER_BYTES, 4 * o.n_padded
+        o.p[:] = raw[H:H + N4].view(np.float32)
+        self.W[:] = raw[H + 3 * N4:].view(self.wdtype)
+        o.p16[:] = O.rne_bf16(o.p) if o.precision == "bf16" else 0
+        self._restoring = (s, h)
+        o.last_step = -1
+        return h["step"]
+
+    def restore_in_place_finish(self) -> int:
+        s, h = self._restoring
+        o = self.o
+        raw = self.slots[s]
+        H, N4 = O.HEADER_BYTES, 4 * o.n_padded
+        o.m[:] = raw[H + N4:H + 2 * N4].view(np.float32)
+        o.v[:] = raw[H + 2 * N4:H + 3 * N4].view(np.float32)
+        o.last_step = h["step"]
+        o.restored_user = h["user"]
+        self._restoring = None
+        return o.last_step
