@@ -719,6 +719,79 @@ class Rig:
         torch.cuda.synchronize()
         return back, r0.elapsed_time(r1), r1.elapsed_time(r2)
 
+    def restore_two_phase(self, G, reps=3):
+        """a6 in two phases (phx_restore_async, R37) and what it buys: the recomputed iteration (G GEMMs of
+        forward/backward + the optimizer step) after a fault, three arms on the same stream —
+          no_fault   : G GEMMs -> step                                   (the iteration itself)
+          serial     : phx_restore -> G GEMMs -> step                     (one-phase restore, everything exposed)
+          overlapped : phx_restore_async on the side stream, the compute stream waits for "parameters ready" only,
+                       G GEMMs -> step (the step waits for the moments by itself).
+        Exposed recovery time = arm - no_fault; median of `reps`."""
+        torch = self.torch
+        self.gemm_setup()
+
+        def fresh_fault():
+            self.do_step()
+            self.flush()
+            self.s.wait(self.step)
+            torch.cuda.synchronize()
+            self.s.drop_live()
+            torch.cuda.synchronize()
+
+        def timed(body):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(self.cur)
+            body()
+            e1.record(self.cur)
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1)
+
+        def iteration():
+            self.gemm_window(G)
+            self.do_step()
+
+        def serial():
+            self.step = self.s.restore()
+            iteration()
+
+        def overlapped():
+            self.side.wait_stream(self.cur)
+            self.step = self.s.restore_async(self.side)
+            self.s.restore_wait_params(self.cur)
+            iteration()
+
+        pr, sr = [], []
+        for _ in range(reps):                      # latency to "parameters ready" / "state ready", nothing else running
+            fresh_fault()
+            r0, r1, r2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            r0.record(self.cur)
+            self.side.wait_stream(self.cur)
+            self.step = self.s.restore_async(self.side)
+            r2.record(self.side)
+            self.s.restore_wait_params(self.cur)
+            r1.record(self.cur)
+            torch.cuda.synchronize()
+            pr.append(r0.elapsed_time(r1))
+            sr.append(r0.elapsed_time(r2))
+        arms = {"no_fault": [], "serial": [], "overlapped": []}
+        for _ in range(reps):
+            self.do_step()
+            torch.cuda.synchronize()
+            arms["no_fault"].append(timed(iteration))
+            fresh_fault()
+            arms["serial"].append(timed(serial))
+            fresh_fault()
+            arms["overlapped"].append(timed(overlapped))
+        med = {k: sorted(v)[len(v) // 2] for k, v in arms.items()}
+        return {"params_ready_ms": sorted(pr)[len(pr) // 2], "state_ready_ms": sorted(sr)[len(sr) // 2],
+                "recomputed_iteration": {"gemms_per_iter": G, "compute_window_ms": G * self.gemm_ms,
+                                         "no_fault_ms": med["no_fault"], "serial_restore_ms": med["serial"],
+                                         "two_phase_restore_ms": med["overlapped"]},
+                "exposed_recovery_ms_serial": med["serial"] - med["no_fault"],
+                "exposed_recovery_ms_two_phase": med["overlapped"] - med["no_fault"], "repeats": reps,
+                "note": "phx_restore_async: p + bf16 copy first on the side stream, m and v behind the recomputed "
+                        "iteration's forward/backward (stand-in GEMMs); the step waits for them by itself"}
+
     def hotswap(self, G):
         """BASELINE.json:configs[3]: 20 steps with snapshots (overlapped with G GEMMs each), the live shard is dropped
         while step 21 is in flight, restore from the pinned host replica, recompute 21, run 22..25; timed, and the
@@ -1098,6 +1171,8 @@ def measure_config(args, key, link, clk, rank, world, local_rank, K, Wm, peak, h
                           "mode": rig.restore_mode_name, "restored_step": int(back),
                           "host_link_gbs": (d2h_bytes - 256) / (rms * 1e-3) / 1e9,
                           "frac_of_h2d_peak": (d2h_bytes - 256) / (rms * 1e-3) / 1e9 / link["h2d_gbs"]}
+        if not args.no_overlap:
+            rec["restore"]["two_phase"] = rig.restore_two_phase(rig.gemms_for(flush_ms, 1.25, False))
         if key in ("c4a", "c4b"):
             rec["hotswap"] = rig.hotswap(rig.gemms_for(flush_ms, 1.25, False))
     return rec, extras

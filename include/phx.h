@@ -259,6 +259,21 @@ PHX_API int phx_fault_inject_torn_flush(phx_shard_t *s, int64_t payload_chunks);
  * A fresh handle created with the same layout/coordinates and bound to the same replica can
  * restore too (a replacement rank assuming the failed rank's role). */
 PHX_API int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step);
+/* a6 in TWO PHASES (reading R37).  "Model parameters are reconstructed ... while optimizer state is
+ * restored from in-memory replicas ... Finally, execution resumes from the last completed step" (PAPER.md:171,
+ * §V-C): the recomputed iteration's forward/backward reads only the model parameters; the moments are first read
+ * by its optimizer step.  phx_restore_async makes the same choice of slot, identity check and hazard ordering as
+ * phx_restore (and only enqueues), but runs everything on `side_stream` in the order
+ *     p -> model-param copy (bf16 regeneration) [-> W, full rank state]   == "parameters ready"
+ *     m -> v                                                              == "state ready"
+ * (PHX_RESTORE_BULK_KERNEL: two launches of the bulk kernel, planes {p} then {m, v}).
+ * phx_restore_wait_params makes `stream` wait (stream-side) until the parameters are in place, after which the
+ * forward/backward of the recomputed iteration may be enqueued on it; two thirds of the host-link transfer then
+ * hide behind that compute.  The next phx_step_and_snapshot (any stream) waits for "state ready" by itself, and so do
+ * phx_restore*, phx_graph_begin and the publication calls; the final state is bit-identical to phx_restore's.
+ * On return last_step = header.step.  A no-op wait when no two-phase restore is outstanding. */
+PHX_API int phx_restore_async(phx_shard_t *s, void *side_stream, uint64_t *restored_step);
+PHX_API int phx_restore_wait_params(phx_shard_t *s, void *stream);
 /* Copies the user blob of the slot the last phx_restore used. */
 PHX_API int phx_restored_user_metadata(const phx_shard_t *s, void *blob, uint32_t cap, uint32_t *len);
 

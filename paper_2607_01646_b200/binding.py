@@ -109,6 +109,8 @@ PROTOTYPES = {
     "phx_snapshot_query": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64), C.POINTER(C.c_int)]),
     "phx_fault_inject_torn_flush": (C.c_int, [C.c_void_p, C.c_int64]),
     "phx_restore": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(C.c_uint64)]),
+    "phx_restore_async": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(C.c_uint64)]),
+    "phx_restore_wait_params": (C.c_int, [C.c_void_p, C.c_void_p]),
     "phx_restored_user_metadata": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(C.c_uint32)]),
     "phx_last_step": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_last_clip": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)]),
@@ -272,6 +274,16 @@ def phx_restore(h: int, stream=None) -> int:
     st = C.c_uint64()
     _ck(lib().phx_restore(h, _ptr(stream), C.byref(st)), "phx_restore", h)
     return st.value
+
+
+def phx_restore_async(h: int, side_stream=None) -> int:
+    st = C.c_uint64()
+    _ck(lib().phx_restore_async(h, _ptr(side_stream), C.byref(st)), "phx_restore_async", h)
+    return st.value
+
+
+def phx_restore_wait_params(h: int, stream=None) -> None:
+    _ck(lib().phx_restore_wait_params(h, _ptr(stream)), "phx_restore_wait_params", h)
 
 
 def phx_restored_user_metadata(h: int) -> bytes:

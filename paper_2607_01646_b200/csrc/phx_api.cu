@@ -141,6 +141,9 @@ struct phx_shard {
     cudaEvent_t ev_wflush = nullptr;   // the newest local flush has finished reading W
     uint64_t params_ready_step = 0;
     bool params_ready = false, wflush_valid = false;
+    // a6 in two phases (phx_restore_async): parameters (p, the model-param copy, W) in place / moments in place
+    cudaEvent_t ev_rparams = nullptr, ev_rstate = nullptr;
+    bool rparams_valid = false, rstate_valid = false;
     // misc
     int last_cuda_error = 0;
     uint64_t launches = 0;
@@ -515,6 +518,8 @@ int phx_shard_destroy(phx_shard_t *s)
         }
         if (s->gev_params.ev) cudaEventDestroy(s->gev_params.ev);
         if (s->gev_wflush.ev) cudaEventDestroy(s->gev_wflush.ev);
+        if (s->ev_rparams) cudaEventDestroy(s->ev_rparams);
+        if (s->ev_rstate) cudaEventSynchronize(s->ev_rstate), cudaEventDestroy(s->ev_rstate);
         if (s->ev_params) cudaEventDestroy(s->ev_params);
         if (s->ev_wflush) cudaEventDestroy(s->ev_wflush);
         if (s->d_scratch) cudaFree(s->d_scratch);
@@ -593,6 +598,8 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
     }
     PHX_CK(cudaEventCreateWithFlags(&s->gev_params.ev, cudaEventDisableTiming));
     PHX_CK(cudaEventCreateWithFlags(&s->gev_wflush.ev, cudaEventDisableTiming));
+    PHX_CK(cudaEventCreateWithFlags(&s->ev_rparams, cudaEventDisableTiming));
+    PHX_CK(cudaEventCreateWithFlags(&s->ev_rstate, cudaEventDisableTiming));
     PHX_CK(cudaEventCreateWithFlags(&s->ev_params, cudaEventDisableTiming));
     PHX_CK(cudaEventCreateWithFlags(&s->ev_wflush, cudaEventDisableTiming));
     for (int k = 0; k < 2; ++k) {
@@ -769,6 +776,11 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
     if (s->pub_valid) PHX_CK(cudaStreamWaitEvent(st, s->ev_pub, 0));
     fill_common_args(s, d_grads, slot, a);
 
+    // a two-phase restore (phx_restore_async) may still be bringing m and v back on its side stream
+    if (s->rstate_valid) {
+        PHX_CK(cudaStreamWaitEvent(st, s->ev_rstate, 0));
+        s->rstate_valid = false;  // later steps follow this one in the caller's stream order
+    }
     // a3: one kernel, one pass
     PHX_CK(phx::launch_step(a, snap && !direct_mode(s), step_mode(s), false, st));
     s->launches += s->info.n_padded ? 1 : 0;
@@ -880,36 +892,61 @@ int choose_slot(const phx_shard *s, const phx_snapshot_header_t hdr[2], const bo
 
 // Enqueue the rebuild of the live shard from slot `best` of a replica (two slots `stride` apart).
 // copy_src: address for copy-engine copies; kern_src: device-visible address for the bulk kernel.
+// two_phase (phx_restore_async, reading R37): p -> model-param copy [-> W] -> ev_rparams -> m, v -> ev_rstate
+// on the one stream `st`; the recomputed iteration's forward/backward may start at ev_rparams, the next optimizer
+// step waits for ev_rstate by itself.
 int enqueue_restore(phx_shard *s, int best, const phx_snapshot_header_t &hdr, const uint8_t *copy_src,
-                    const uint8_t *kern_src, cudaStream_t st, uint64_t stride, uint32_t want_payload)
+                    const uint8_t *kern_src, cudaStream_t st, uint64_t stride, uint32_t want_payload, bool two_phase = false)
 {
     // The copies overwrite the live planes (and W): order them behind everything of THIS handle that may still be
     // reading or writing them — the newest step's kernel, a direct-source flush to the host or to the peers, a
-    // full-rank-state flush reading W, a copy-engine publication.
+    // full-rank-state flush reading W, a copy-engine publication, an earlier two-phase restore.
     if (s->last_step > 0 || s->ev_last_step) PHX_CK(cudaStreamWaitEvent(st, s->ev_last_step, 0));
     if (s->last_flush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_flush[s->last_flush_slot], 0));
     if (s->last_pflush_slot >= 0) PHX_CK(cudaStreamWaitEvent(st, s->ev_pflush[s->last_pflush_slot], 0));
     if (s->wflush_valid) PHX_CK(cudaStreamWaitEvent(st, s->ev_wflush, 0));
     if (s->pub_valid) PHX_CK(cudaStreamWaitEvent(st, s->ev_pub, 0));
+    if (s->rstate_valid) PHX_CK(cudaStreamWaitEvent(st, s->ev_rstate, 0));
+    s->rparams_valid = s->rstate_valid = false;
 
     const uint64_t N = s->info.n_padded;
     const uint64_t off = (uint64_t)best * stride + kHeaderBytes;
-    if (s->cfg.restore_mode == PHX_RESTORE_BULK_KERNEL) {
-        PHX_CK(phx::launch_restore_bulk(kern_src + off, s->d_p, s->d_m, s->d_v, fp32_mode(s) ? nullptr : s->d_p16, N,
-                                        s->sm_count, st));
+    const bool bulk = s->cfg.restore_mode == PHX_RESTORE_BULK_KERNEL;
+    void *p16 = fp32_mode(s) ? nullptr : s->d_p16;
+    const float *ksrc = reinterpret_cast<const float *>(kern_src + off);
+    const uint8_t *src = copy_src + off;
+    // phase 1 (or, one-phase, everything): p and the model-param copy
+    if (bulk) {
+        phx::RestorePlanes pl{{ksrc, ksrc + N, ksrc + 2 * N}, {s->d_p, s->d_m, s->d_v}, two_phase ? 1 : 3};
+        PHX_CK(phx::launch_restore_bulk(pl, p16, N, s->sm_count, st));
         s->launches += N ? 1 : 0;
     } else {
-        const uint8_t *src = copy_src + off;
         PHX_CK(cudaMemcpyAsync(s->d_p, src, 4 * N, cudaMemcpyDefault, st));
-        PHX_CK(cudaMemcpyAsync(s->d_m, src + 4 * N, 4 * N, cudaMemcpyDefault, st));
-        PHX_CK(cudaMemcpyAsync(s->d_v, src + 8 * N, 4 * N, cudaMemcpyDefault, st));
-        if (!fp32_mode(s)) {
+        if (!two_phase) {
+            PHX_CK(cudaMemcpyAsync(s->d_m, src + 4 * N, 4 * N, cudaMemcpyDefault, st));
+            PHX_CK(cudaMemcpyAsync(s->d_v, src + 8 * N, 4 * N, cudaMemcpyDefault, st));
+        }
+        if (p16) {
             PHX_CK(phx::launch_regen_bf16(s->d_p, s->d_p16, N, st));
             s->launches += N ? 1 : 0;
         }
     }
     if (want_payload != 0)  // §8(f4) in-place recovery: W comes back from the same slot, no other rank is read
         PHX_CK(cudaMemcpyAsync(s->d_W, copy_src + off + 12 * N, s->info.param_bytes, cudaMemcpyDefault, st));
+    if (two_phase) {  // phase 2: the moments
+        PHX_CK(cudaEventRecord(s->ev_rparams, st));
+        s->rparams_valid = true;
+        if (bulk) {
+            phx::RestorePlanes pl{{ksrc + N, ksrc + 2 * N, nullptr}, {s->d_m, s->d_v, nullptr}, 2};
+            PHX_CK(phx::launch_restore_bulk(pl, nullptr, N, s->sm_count, st));
+            s->launches += N ? 1 : 0;
+        } else {
+            PHX_CK(cudaMemcpyAsync(s->d_m, src + 4 * N, 4 * N, cudaMemcpyDefault, st));
+            PHX_CK(cudaMemcpyAsync(s->d_v, src + 8 * N, 4 * N, cudaMemcpyDefault, st));
+        }
+        PHX_CK(cudaEventRecord(s->ev_rstate, st));
+        s->rstate_valid = true;
+    }
     PHX_CK(cudaEventRecord(s->ev_last_step, st));  // later flushes / publications order behind the restore
     s->last_step = hdr.step;
     s->pending_slot = -1;
@@ -930,7 +967,8 @@ int enqueue_restore(phx_shard *s, int best, const phx_snapshot_header_t &hdr, co
 //   - the handle's own commit bookkeeping for a slot whose flush is still in flight: the envelope it sent is
 //     known, the flush cannot tear (a torn flush is known as such and skipped), and `stream` is made to wait
 //     for the flush event before the copies, so the payload has landed when it is read.
-int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
+namespace {
+int restore_own(phx_shard *s, void *stream, uint64_t *restored_step, bool two_phase)
 {
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound || (snapshots_on(s) && !s->h_replica)) return PHX_ERR_NOT_BOUND;
@@ -952,7 +990,7 @@ int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
     const int best = choose_slot(s, hdr, usable, want, ok);
     if (best < 0) return best;
     if (inflight[best]) PHX_CK(cudaStreamWaitEvent(st, s->ev_host[best], 0));
-    rc = enqueue_restore(s, best, hdr[best], s->h_replica, s->d_replica, st, s->info.host_slot_stride, want);
+    rc = enqueue_restore(s, best, hdr[best], s->h_replica, s->d_replica, st, s->info.host_slot_stride, want, two_phase);
     if (rc != PHX_OK) return rc;
     for (int i = 0; i < 2; ++i) {  // adopt what the replica shows (a replacement handle starts with EMPTY slots)
         if (inflight[i] || s->host[i].state == SLOT_TORN_INFLIGHT) continue;
@@ -963,6 +1001,23 @@ int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step)
         }
     }
     if (restored_step) *restored_step = s->last_step;
+    return PHX_OK;
+}
+}  // namespace
+
+int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step) { return restore_own(s, stream, restored_step, false); }
+
+// a6 in two phases: everything on `side_stream`, parameters first; see include/phx.h
+int phx_restore_async(phx_shard_t *s, void *side_stream, uint64_t *restored_step)
+{
+    return restore_own(s, side_stream, restored_step, true);
+}
+
+int phx_restore_wait_params(phx_shard_t *s, void *stream)
+{
+    if (!s) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (s->rparams_valid) PHX_CK(cudaStreamWaitEvent(static_cast<cudaStream_t>(stream), s->ev_rparams, 0));
     return PHX_OK;
 }
 
@@ -1386,6 +1441,10 @@ int phx_graph_begin(phx_shard_t *s, float lr, float beta1, float beta2, float ep
     if (rc != PHX_OK) return rc;
     rc = settle_peer_slots(s, true);
     if (rc != PHX_OK) return rc;
+    if (s->rstate_valid) {  // a two-phase restore still bringing the moments back
+        PHX_CK(cudaEventSynchronize(s->ev_rstate));
+        s->rstate_valid = false;
+    }
     phx_snapshot_header_t tmpl;
     build_header(s, 0, true, &tmpl);
     phx::HeaderBlob blob;

@@ -686,14 +686,14 @@ constexpr int kTile = 2048;  // elements per plane per tile (8 KB)
 constexpr int kStages = 4;
 constexpr int kRestoreThreads = 256;
 
-__global__ void __launch_bounds__(kRestoreThreads) k_restore_bulk(const float *__restrict__ src, float *__restrict__ p,
-                                                                  float *__restrict__ m, float *__restrict__ v,
+__global__ void __launch_bounds__(kRestoreThreads) k_restore_bulk(const __grid_constant__ RestorePlanes pl,
                                                                   void *__restrict__ p16, uint64_t n_padded)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float *tiles = reinterpret_cast<float *>(smem_raw);  // [kStages][3][kTile]
     __shared__ __align__(8) uint64_t full[kStages];
 
+    const int np = pl.n;  // 1..3 planes: {p, m, v}, {p} (parameters first) or {m, v} (two-phase restore)
     const uint64_t ntiles = (n_padded + kTile - 1) / kTile;
     const uint64_t my_first = blockIdx.x;
     const uint64_t stride = gridDim.x;
@@ -712,10 +712,8 @@ __global__ void __launch_bounds__(kRestoreThreads) k_restore_bulk(const float *_
         const uint32_t cnt = (uint32_t)((n_padded - e0) < (uint64_t)kTile ? (n_padded - e0) : kTile);
         const uint32_t bytes = cnt * 4u;
         float *dst = tiles + (size_t)s * 3 * kTile;
-        mbar_expect_tx(&full[s], 3u * bytes);
-        bulk_g2s(dst, src + e0, bytes, &full[s]);
-        bulk_g2s(dst + kTile, src + n_padded + e0, bytes, &full[s]);
-        bulk_g2s(dst + 2 * kTile, src + 2 * n_padded + e0, bytes, &full[s]);
+        mbar_expect_tx(&full[s], (uint32_t)np * bytes);
+        for (int k = 0; k < np; ++k) bulk_g2s(dst + k * kTile, pl.src[k] + e0, bytes, &full[s]);
     };
 
     if (threadIdx.x == 0)
@@ -730,12 +728,10 @@ __global__ void __launch_bounds__(kRestoreThreads) k_restore_bulk(const float *_
         float *tp = tiles + (size_t)s * 3 * kTile;
         mbar_wait(&full[s], parity);
         if (threadIdx.x == 0) {
-            bulk_s2g(p + e0, tp, cnt * 4u);
-            bulk_s2g(m + e0, tp + kTile, cnt * 4u);
-            bulk_s2g(v + e0, tp + 2 * kTile, cnt * 4u);
+            for (int k = 0; k < np; ++k) bulk_s2g(pl.dst[k] + e0, tp + k * kTile, cnt * 4u);
             bulk_commit();
         }
-        // bf16 copy: 8 elements per thread, conflict-free 128-bit shared loads
+        // bf16 copy of plane 0 (p): 8 elements per thread, conflict-free 128-bit shared loads
         const uint32_t e = threadIdx.x * 8;
         if (p16 != nullptr && e < cnt) {
             const float4 a = *reinterpret_cast<const float4 *>(tp + e);
@@ -756,10 +752,10 @@ __global__ void __launch_bounds__(kRestoreThreads) k_restore_bulk(const float *_
     if (threadIdx.x == 0) bulk_wait_all0();  // stores globally complete before the CTA exits
 }
 
-cudaError_t launch_restore_bulk(const void *src_payload, float *p, float *m, float *v, void *p16,
-                                uint64_t n_padded, int sm_count, cudaStream_t st)
+cudaError_t launch_restore_bulk(const RestorePlanes &pl, void *p16, uint64_t n_padded, int sm_count, cudaStream_t st)
 {
     if (n_padded == 0) return cudaSuccess;
+    if (pl.n < 1 || pl.n > 3) return cudaErrorInvalidValue;
     const size_t smem = (size_t)kStages * 3 * kTile * sizeof(float);  // 96 KB
     static bool attr_set = false;
     if (!attr_set) {
@@ -770,8 +766,7 @@ cudaError_t launch_restore_bulk(const void *src_payload, float *p, float *m, flo
     const uint64_t ntiles = (n_padded + kTile - 1) / kTile;
     uint64_t grid = (uint64_t)sm_count * 2;
     if (grid > ntiles) grid = ntiles;
-    k_restore_bulk<<<(unsigned)grid, kRestoreThreads, smem, st>>>(reinterpret_cast<const float *>(src_payload), p, m, v,
-                                                                   p16, n_padded);
+    k_restore_bulk<<<(unsigned)grid, kRestoreThreads, smem, st>>>(pl, p16, n_padded);
     return cudaGetLastError();
 }
 

@@ -106,9 +106,14 @@ cudaError_t launch_grads_finalize(const float *g32, float scale, void *g16, uint
 // p16 = RNE_bf16(p)
 cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cudaStream_t st);
 
-// a6, bulk-kernel mode: src_payload = device-visible address of the host slot's payload (p ‖ m ‖ v);
-// p16 == nullptr skips the bf16 regeneration (kModeF32 shards have no bf16 copy).
-cudaError_t launch_restore_bulk(const void *src_payload, float *p, float *m, float *v, void *p16,
-                                uint64_t n_padded, int sm_count, cudaStream_t st);
+// a6, bulk-kernel mode: src[k] = device-visible address of plane k inside the host slot's payload (p ‖ m ‖ v),
+// dst[k] the live plane it restores; n = 3 for the one-phase restore, {p} then {m, v} for the two-phase one.
+// p16 != nullptr: the bf16 copy is regenerated from plane 0 (must be p); kModeF32 shards have no bf16 copy.
+struct RestorePlanes {
+    const float *src[3];
+    float *dst[3];
+    int n;
+};
+cudaError_t launch_restore_bulk(const RestorePlanes &pl, void *p16, uint64_t n_padded, int sm_count, cudaStream_t st);
 
 }  // namespace phx

@@ -90,6 +90,13 @@ class Shard:
     def restore(self, stream=None) -> int:
         return B.phx_restore(self.h, stream or torch.cuda.current_stream(self.device))
 
+    def restore_async(self, side_stream) -> int:
+        """a6 in two phases (include/phx.h): parameters first, moments behind the recomputed forward/backward."""
+        return B.phx_restore_async(self.h, side_stream)
+
+    def restore_wait_params(self, stream=None):
+        B.phx_restore_wait_params(self.h, stream or torch.cuda.current_stream(self.device))
+
     def staging_slot(self, step: int) -> torch.Tensor:
         k = step % self.info.staging_depth
         return self.staging[k * self.info.slot_stride: k * self.info.slot_stride + self.info.snapshot_bytes]

@@ -82,6 +82,8 @@ def test_no_byte_outside_the_bound_buffers_is_touched(numels, rmode):
     for x in (p, m, v):
         x.zero_()
     assert B.phx_restore(h, cur) == 5
+    assert B.phx_restore_async(h, side) == 5                  # two phases on the side stream: {p, bf16 copy} then {m, v}
+    B.phx_restore_wait_params(h, cur)
     assert B.phx_restore_from(h, bufs["recv"].body, cur) == 4
     # graph-form steps (prologue writes the envelope into the staging slot) + flushes
     B.phx_graph_begin(h, *hp, cur)
