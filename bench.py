@@ -792,10 +792,12 @@ class Rig:
                 "note": "phx_restore_async: p + bf16 copy first on the side stream, m and v behind the recomputed "
                         "iteration's forward/backward (stand-in GEMMs); the step waits for them by itself"}
 
-    def hotswap(self, G):
+    def hotswap(self, G, two_phase=False):
         """BASELINE.json:configs[3]: 20 steps with snapshots (overlapped with G GEMMs each), the live shard is dropped
         while step 21 is in flight, restore from the pinned host replica, recompute 21, run 22..25; timed, and the
-        trajectory compared bit for bit with an uninterrupted run (GPU vs GPU; GPU vs oracle is in tests/)."""
+        trajectory compared bit for bit with an uninterrupted run (GPU vs GPU; GPU vs oracle is in tests/).
+        two_phase: the recovery is phx_restore_async (parameters first, moments behind the recomputed iteration's G
+        GEMMs of forward/backward); the timed region then holds that compute window too."""
         torch, W, wl, N = self.torch, self.W, self.wl, self.N
         torch.cuda.synchronize()
         self.s.p.copy_(W.init_params(self.s.n, N, wl.seed, device=self.device))
@@ -819,8 +821,15 @@ class Rig:
         t0 = time.perf_counter()
         r0, r1, r2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         r0.record(self.cur)
-        back = self.s.restore()
-        r1.record(self.cur)
+        if two_phase:
+            self.side.wait_stream(self.cur)
+            back = self.s.restore_async(self.side)
+            self.s.restore_wait_params(self.cur)      # forward/backward may start: the parameters are back
+            r1.record(self.cur)
+            self.gemm_window(G)
+        else:
+            back = self.s.restore()
+            r1.record(self.cur)
         self.step = back
         self.do_step()                                # recompute of the in-flight step (a7)
         r2.record(self.cur)
@@ -836,6 +845,12 @@ class Rig:
         ref.close()
         del ref
         rms = r0.elapsed_time(r1)
+        if two_phase:
+            return {"restored_step": int(back), "params_ready_ms": rms, "recomputed_iteration_ms": r1.elapsed_time(r2),
+                    "compute_window_ms": G * self.gemm_ms, "recovery_plus_recomputed_iteration_ms": r0.elapsed_time(r2),
+                    "trajectory_bit_exact_vs_uninterrupted": bool(same), "gemms_per_iter": G, "mode": self.restore_mode_name,
+                    "note": "phx_restore_async: the timed region holds the recomputed iteration's G GEMMs; m and v "
+                            "come back behind them"}
         return {"restored_step": int(back), "restore_ms": rms, "recompute_ms": r1.elapsed_time(r2),
                 "restore_plus_recompute_ms": r0.elapsed_time(r2), "restore_plus_recompute_wall_ms": wall_ms,
                 "host_link_gbs": 12 * N / (rms * 1e-3) / 1e9, "trajectory_bit_exact_vs_uninterrupted": bool(same),
@@ -1156,6 +1171,12 @@ def measure_config(args, key, link, clk, rank, world, local_rank, K, Wm, peak, h
                 w.update(iter_ms_off_graph_step=og["iter_ms_off"], iter_ms_on_graph_step=og["iter_ms_on"],
                          exposed_ms_graph_step=og["exposed_ms"],
                          exposed_pct_graph_step=100.0 * og["exposed_frac_of_compute_step"])
+            # SURVEY 8(d) decomposition: the kernel's own share (12 B/element of staging stores, from the isolated
+            # step timings above) vs everything else (sync-point stall + slowdown of the window under copy traffic)
+            kd = step_ms - off_ms
+            w["exposed_decomposition_ms"] = {"kernel_delta_isolated": kd, "rest_eager": o["exposed_ms"] - kd}
+            if "exposed_ms_graph_step" in w:
+                w["exposed_decomposition_ms"]["rest_graph_step"] = w["exposed_ms_graph_step"] - kd
             ov[wname] = w
         rec["overlap"] = ov
         rec["exposed_ckpt_ms_per_iter"] = ov["headline_window"]["exposed_ms_eager"]
@@ -1175,6 +1196,8 @@ def measure_config(args, key, link, clk, rank, world, local_rank, K, Wm, peak, h
             rec["restore"]["two_phase"] = rig.restore_two_phase(rig.gemms_for(flush_ms, 1.25, False))
         if key in ("c4a", "c4b"):
             rec["hotswap"] = rig.hotswap(rig.gemms_for(flush_ms, 1.25, False))
+            if not args.no_overlap:
+                rec["hotswap"]["two_phase"] = rig.hotswap(rig.gemms_for(flush_ms, 1.25, False), two_phase=True)
     return rec, extras
 
 

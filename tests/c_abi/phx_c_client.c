@@ -6,6 +6,7 @@
  *     -> (in-flight step) -> zero the live shard -> restore -> recompute the in-flight step
  *     -> the gradient producer's epilogue (phx_grads_finalize_async) feeding one step
  *     -> two steps through the graph-capturable form (phx_graph_begin / flush / step / end), called eagerly
+ *     -> a second fault recovered in two phases (phx_restore_async / phx_restore_wait_params) and one more step
  * and writes p, m, v, the bf16 copy and the two host replica slots to an output file that the test
  * compares byte for byte with the CPU oracle.
  *
@@ -155,7 +156,26 @@ int main(int argc, char **argv)
         fprintf(stderr, "graph form ended at step %llu, expected %llu\n", (unsigned long long)last, (unsigned long long)(back + 4));
         return 5;
     }
+    /* a second fault, recovered in TWO PHASES (phx_restore_async): the newest snapshot is flushed, the live shard is
+     * lost, the parameters come back first on the side stream, the compute stream waits for them only, and the next
+     * step waits for the moments by itself */
+    CK(phx_snapshot_flush_async(s, side));
+    CK(phx_snapshot_wait(s, last));
     CU(cudaStreamSynchronize(compute));
+    CU(cudaMemset(d_p, 0, 4 * N));
+    CU(cudaMemset(d_m, 0, 4 * N));
+    CU(cudaMemset(d_v, 0, 4 * N));
+    CU(cudaMemset(d_p16, 0, 2 * N));
+    uint64_t back2 = 0;
+    CK(phx_restore_async(s, side, &back2));
+    CK(phx_restore_wait_params(s, compute));
+    if (back2 != last) {
+        fprintf(stderr, "two-phase restore came back at step %llu, expected %llu\n", (unsigned long long)back2, (unsigned long long)last);
+        return 6;
+    }
+    CK(phx_step_and_snapshot(s, d_ga, lr, b1, b2, eps, wd, back2 + 1, compute));
+    CU(cudaStreamSynchronize(compute));
+    CU(cudaStreamSynchronize(side));
 
     FILE *out = fopen(argv[2], "wb");
     if (!out) return 1;

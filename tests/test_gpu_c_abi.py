@@ -87,7 +87,11 @@ def test_c_client_matches_the_oracle(tmp_path, numels, dp, rank, max_norm):
     for k in (0, 1):                                      # graph form: flush of the pending snapshot, then step
         o.snapshot()
         o.step(grads[k], **hp, step=steps + 3 + k)
-    replica = [x.copy() for x in o.replica]               # slots now hold steps+2 and steps+3
+    o.snapshot()                                          # second fault: newest snapshot flushed, live shard lost,
+    o.drop_live()                                         # two-phase restore, one more step
+    assert o.restore_params_first() == steps + 4 and o.restore_finish() == steps + 4
+    o.step(grads[0], **hp, step=steps + 5)
+    replica = [x.copy() for x in o.replica]               # slots now hold steps+3 and steps+4
     raw = open(outp, "rb").read()
     n_padded, back = struct.unpack_from("<QQ", raw, 0)
     assert (n_padded, back) == (N, steps)
