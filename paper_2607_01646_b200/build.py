@@ -38,6 +38,13 @@ NVCC_FLAGS = [
 ]
 
 
+# Tuning experiments only (profiles/ name the macro they set, e.g. PHX_NVCC_EXTRA=-DPHX_RESTORE_P2_CTAS=8): extra nvcc
+# flags for the product library; unset in every build the tests, smoke() and bench.py's numbers come from.
+def extra_flags():
+    import shlex
+    return shlex.split(os.environ.get("PHX_NVCC_EXTRA", ""))
+
+
 def nvcc() -> str:
     for c in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
         if c and (os.path.sep not in c or os.path.exists(c)):
@@ -67,7 +74,7 @@ def _link(lib, sources, extra, verbose):
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or not _fresh(LIB, DEPS):
         # the version script exports phx_* only (no leaked template instantiations of the C++ runtime)
-        _link(LIB, SOURCES, ["-Xlinker", f"--version-script={MAP}"], verbose)
+        _link(LIB, SOURCES, ["-Xlinker", f"--version-script={MAP}", *extra_flags()], verbose)
     if force or not _fresh(PROBE_LIB, PROBE_DEPS):
         _link(PROBE_LIB, PROBE_SOURCES, [], verbose)
     return LIB

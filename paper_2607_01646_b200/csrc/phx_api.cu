@@ -15,6 +15,10 @@ constexpr uint64_t kPadUnit = 64;      // elements; every rank's range is a mult
 constexpr uint64_t kHeaderBytes = 256;
 constexpr uint32_t kVersion = 1;
 constexpr int kMaxDepth = 4;
+#ifndef PHX_RESTORE_P2_CTAS
+#define PHX_RESTORE_P2_CTAS 4
+#endif
+constexpr int kRestorePhase2Ctas = PHX_RESTORE_P2_CTAS;  // bulk-kernel CTAs of the second phase of phx_restore_async
 
 struct Segment {
     uint32_t tensor_id;
@@ -918,7 +922,7 @@ int enqueue_restore(phx_shard *s, int best, const phx_snapshot_header_t &hdr, co
     // phase 1 (or, one-phase, everything): p and the model-param copy
     if (bulk) {
         phx::RestorePlanes pl{{ksrc, ksrc + N, ksrc + 2 * N}, {s->d_p, s->d_m, s->d_v}, two_phase ? 1 : 3};
-        PHX_CK(phx::launch_restore_bulk(pl, p16, N, s->sm_count, st));
+        PHX_CK(phx::launch_restore_bulk(pl, p16, N, 2 * s->sm_count, st));
         s->launches += N ? 1 : 0;
     } else {
         PHX_CK(cudaMemcpyAsync(s->d_p, src, 4 * N, cudaMemcpyDefault, st));
@@ -938,7 +942,10 @@ int enqueue_restore(phx_shard *s, int best, const phx_snapshot_header_t &hdr, co
         s->rparams_valid = true;
         if (bulk) {
             phx::RestorePlanes pl{{ksrc + N, ksrc + 2 * N, nullptr}, {s->d_m, s->d_v, nullptr}, 2};
-            PHX_CK(phx::launch_restore_bulk(pl, nullptr, N, s->sm_count, st));
+            // the moments come back BESIDE the recomputed iteration's kernels: FOUR persistent CTAs already saturate the
+            // host link (2: 86 %; 8-37: the same rate, but each CTA's 96 KB of shared memory takes an SM away from the
+            // forward/backward — profiles/r02c_restore_bulk.md), the other 144 SMs stay with the compute
+            PHX_CK(phx::launch_restore_bulk(pl, nullptr, N, kRestorePhase2Ctas, st));
             s->launches += N ? 1 : 0;
         } else {
             PHX_CK(cudaMemcpyAsync(s->d_m, src + 4 * N, 4 * N, cudaMemcpyDefault, st));

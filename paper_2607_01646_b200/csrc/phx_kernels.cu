@@ -752,7 +752,7 @@ __global__ void __launch_bounds__(kRestoreThreads) k_restore_bulk(const __grid_c
     if (threadIdx.x == 0) bulk_wait_all0();  // stores globally complete before the CTA exits
 }
 
-cudaError_t launch_restore_bulk(const RestorePlanes &pl, void *p16, uint64_t n_padded, int sm_count, cudaStream_t st)
+cudaError_t launch_restore_bulk(const RestorePlanes &pl, void *p16, uint64_t n_padded, int max_ctas, cudaStream_t st)
 {
     if (n_padded == 0) return cudaSuccess;
     if (pl.n < 1 || pl.n > 3) return cudaErrorInvalidValue;
@@ -764,7 +764,7 @@ cudaError_t launch_restore_bulk(const RestorePlanes &pl, void *p16, uint64_t n_p
         attr_set = true;
     }
     const uint64_t ntiles = (n_padded + kTile - 1) / kTile;
-    uint64_t grid = (uint64_t)sm_count * 2;
+    uint64_t grid = max_ctas > 0 ? (uint64_t)max_ctas : 1;
     if (grid > ntiles) grid = ntiles;
     k_restore_bulk<<<(unsigned)grid, kRestoreThreads, smem, st>>>(pl, p16, n_padded);
     return cudaGetLastError();

@@ -114,6 +114,8 @@ struct RestorePlanes {
     float *dst[3];
     int n;
 };
-cudaError_t launch_restore_bulk(const RestorePlanes &pl, void *p16, uint64_t n_padded, int sm_count, cudaStream_t st);
+// max_ctas: persistent CTAs (96 KB of shared memory each).  The link, not the SMs, is the bound, so a handful keeps it
+// busy; the two-phase restore runs its second phase on few CTAs so that the recomputed iteration's kernels keep the SMs.
+cudaError_t launch_restore_bulk(const RestorePlanes &pl, void *p16, uint64_t n_padded, int max_ctas, cudaStream_t st);
 
 }  // namespace phx
