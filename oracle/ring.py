@@ -29,7 +29,7 @@ and resume invariants of the single-rank oracle carried over to the ring.
 """
 from __future__ import annotations
 
-from typing import Dict, Iterable, List, Optional, Tuple
+from typing import Dict, Iterable, List, Optional, Sequence, Tuple
 
 import numpy as np
 
@@ -54,47 +54,102 @@ def recoverable(dp_size: int, k: int, failed: Iterable[int]) -> bool:
     return all(any(h not in f for h in holders(dp_size, r, k)) for r in f)
 
 
+# ---- topology-aware placement (reading R38) ------------------------------------------------------
+# "PHOENIX can leverage cluster topology information to place the k replicas on nodes under k distinct
+# switches or racks, ensuring that a single infrastructure event affects at most one copy of any given
+# shard".  A shard has k + 1 copies (the owner's and the k replicas), so all k + 1 must sit
+# in pairwise distinct failure domains.  The paper does not say WHICH ranks are taken; R38: walk the DP
+# ring from the owner (r+1, r+2, ...) and take a rank iff its domain differs from the owner's and from the
+# domain of every rank already taken — the nearest admissible ranks in ring order.
+
+
+def holders_topology_aware(domains: Sequence[int], dp_rank: int, k: int) -> List[int]:
+    D = len(domains)
+    assert 0 <= dp_rank < D and 0 <= k <= D - 1
+    used = {domains[dp_rank]}
+    out: List[int] = []
+    for j in range(1, D):
+        if len(out) == k:
+            break
+        q = (dp_rank + j) % D
+        if domains[q] not in used:
+            used.add(domains[q])
+            out.append(q)
+    if len(out) < k:
+        raise O.OracleError("fewer than k + 1 distinct failure domains")
+    return out
+
+
+def placement(dp_size: int, k: int, domains: Optional[Sequence[int]] = None) -> List[List[int]]:
+    """place[r] = the ranks that hold rank r's replicas: the plain ring (R25) or, with failure domains, R38."""
+    if domains is None:
+        return [holders(dp_size, r, k) for r in range(dp_size)]
+    assert len(domains) == dp_size
+    return [holders_topology_aware(domains, r, k) for r in range(dp_size)]
+
+
+def recoverable_with(place: Sequence[Sequence[int]], failed: Iterable[int]) -> bool:
+    """R28 for an arbitrary placement."""
+    f = set(failed)
+    return all(any(h not in f for h in place[r]) for r in f)
+
+
+def max_copies_in_one_domain(domains: Sequence[int], place: Sequence[Sequence[int]]) -> int:
+    """The largest number of copies (owner's + replicas) of any one shard that share a failure domain."""
+    worst = 0
+    for r, hs in enumerate(place):
+        doms = [domains[r]] + [domains[h] for h in hs]
+        worst = max(worst, max(doms.count(d) for d in set(doms)))
+    return worst
+
+
 class OracleRing:
-    """D OracleShards of one DP group (same layout, tp/pp coordinates; dp_rank = 0..D-1) plus,
-    on every rank, the k received buffers it holds for its ring predecessors."""
+    """D OracleShards of one DP group (same layout, tp/pp coordinates; dp_rank = 0..D-1) plus, on every
+    rank, the received buffers it holds for the ranks whose replicas are placed on it: the k ring
+    predecessors (plain ring), or whoever the topology-aware placement R38 sends there (`domains`)."""
 
     def __init__(self, layout, dp_size: int, k: int, *, tp=(1, 0), pp=(1, 0), chunk_bytes=64 << 20,
-                 flags=None, precision="bf16", max_grad_norm=0.0):
+                 flags=None, precision="bf16", max_grad_norm=0.0, domains: Optional[Sequence[int]] = None):
         assert 1 <= k <= dp_size - 1
         self.D, self.k = dp_size, k
+        self.domains = None if domains is None else list(domains)
+        self.place = placement(dp_size, k, self.domains)
         self.shards = [O.OracleShard(layout, dp_size, r, tp, pp, chunk_bytes=chunk_bytes, flags=flags,
                                      precision=precision, max_grad_norm=max_grad_norm) for r in range(dp_size)]
         nbytes = self.shards[0].snapshot_bytes
-        # received[h][j-1][slot]: what rank h holds for its j-th predecessor (h - j) mod D
-        self.received: List[List[List[np.ndarray]]] = [
-            [[np.zeros(nbytes, np.uint8) for _ in range(2)] for _ in range(k)] for _ in range(dp_size)]
+        # recv[(h, r)][slot]: what rank h holds for owner r
+        self.recv: Dict[Tuple[int, int], List[np.ndarray]] = {
+            (h, r): [np.zeros(nbytes, np.uint8) for _ in range(2)] for r in range(dp_size) for h in self.place[r]}
         self.alive = [True] * dp_size
 
-    # -- H2H phase: owner r -> its k ring successors (R26, R27) -------------------------------
+    @property
+    def received(self) -> List[List[List[np.ndarray]]]:
+        """Plain ring only: received[h][j-1][slot] = what rank h holds for its j-th predecessor (h - j) mod D."""
+        assert self.domains is None
+        return [[self.recv[(h, ring_peer(self.D, h, -j))] for j in range(1, self.k + 1)] for h in range(self.D)]
+
+    # -- H2H phase: owner r -> its k holders (R26, R27) ---------------------------------------
     def replicate(self, r: int, abort_after_chunks: Optional[Dict[int, int]] = None):
         """Send rank r's packed snapshot of its last step to every holder.  abort_after_chunks[j]
-        = c tears the transfer to peer j after c payload chunks (never commits)."""
+        = c tears the transfer to holder number j (1-based) after c payload chunks (never commits)."""
         o = self.shards[r]
         src = o.packed_snapshot()
         slot = o.last_step % 2
         cb = o.chunk_bytes
         payload = o.snapshot_bytes - O.HEADER_BYTES
         nchunks = (payload + cb - 1) // cb
-        for j in range(1, self.k + 1):
-            h = ring_peer(self.D, r, j)
+        for j, h in enumerate(self.place[r], 1):
             if not self.alive[h]:
                 continue
-            dst = self.received[h][j - 1][slot]
+            dst = self.recv[(h, r)][slot]
             stop = None if abort_after_chunks is None else abort_after_chunks.get(j)
             dst[:O.HEADER_BYTES] = 0
-            done = 0
             for c in range(nchunks):
                 if stop is not None and c >= stop:
                     break
                 lo = O.HEADER_BYTES + c * cb
                 hi = min(lo + cb, o.snapshot_bytes)
                 dst[lo:hi] = src[lo:hi]
-                done += 1
             if stop is None:
                 dst[:O.HEADER_BYTES] = src[:O.HEADER_BYTES]
 
@@ -106,22 +161,22 @@ class OracleRing:
             o.drop_live()
             for s in range(2):
                 o.replica[s][:] = 0
-            for j in range(self.k):
-                for s in range(2):
-                    self.received[r][j][s][:] = 0xA5
+            for (h, _), bufs in self.recv.items():
+                if h == r:
+                    for s in range(2):
+                        bufs[s][:] = 0xA5
 
     # -- recovery stage 3 for one lost shard (R28) ---------------------
     def newest_replica_of(self, r: int) -> Optional[Tuple[int, int, int, dict]]:
         """(holder, j, slot, header) of the valid, identity-matching slot with the largest step
-        among surviving holders of rank r's shard, or None."""
+        among surviving holders of rank r's shard (j = the holder's 1-based number), or None."""
         o = self.shards[r]
         best = None
-        for j in range(1, self.k + 1):
-            h = ring_peer(self.D, r, j)
+        for j, h in enumerate(self.place[r], 1):
             if not self.alive[h]:
                 continue
             for s in range(2):
-                hd = O.parse_header(self.received[h][j - 1][s][:O.HEADER_BYTES].tobytes())
+                hd = O.parse_header(self.recv[(h, r)][s][:O.HEADER_BYTES].tobytes())
                 if hd is None:
                     continue
                 if (hd["layout_hash"] != o.layout_hash or hd["dp"] != o.dp or hd["tp"] != o.tp
@@ -140,12 +195,13 @@ class OracleRing:
             raise O.OracleError("shard lost: owner and all holders failed (PAPER.md:175)")
         h, j, s, hd = best
         o = self.shards[r]
-        o.replica[hd["step"] % 2][:] = self.received[h][j - 1][s]   # same bytes, then the plain restore
+        o.replica[hd["step"] % 2][:] = self.recv[(h, r)][s]   # same bytes, then the plain restore
         o.replica[1 - hd["step"] % 2][:] = 0
         step = o.restore()
-        for jj in range(self.k):
-            for ss in range(2):
-                self.received[r][jj][ss][:] = 0
+        for (hh, _), bufs in self.recv.items():
+            if hh == r:
+                for ss in range(2):
+                    bufs[ss][:] = 0
         self.alive[r] = True
         return step
 
