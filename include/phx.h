@@ -297,6 +297,15 @@ PHX_API int phx_restored_user_metadata(const phx_shard_t *s, void *blob, uint32_
 /* Ring peer j of rank r: (r + j) mod dp_size; j = 1..k are the ranks that hold r's replicas, j = -1..-k the
  * ranks whose replicas r holds.  |j| must be in [1, dp_size - 1] (k distinct peers need k <= D - 1). */
 PHX_API int phx_ring_peer(uint32_t dp_size, uint32_t dp_rank, int32_t j, uint32_t *peer);
+/* Topology-aware placement ("place the k replicas on nodes under k distinct switches or racks, ensuring
+ * that a single infrastructure event affects at most one copy of any given shard"; reading R38): with
+ * domain_of_rank[q] = the failure domain (switch, rack, node, ...) of DP rank q, peers[0..k) receives the k nearest
+ * ranks in ring order (dp_rank + 1, dp_rank + 2, ...) whose domains differ from the owner's and from one another, so
+ * that the k + 1 copies of the shard sit under k + 1 distinct domains.  k <= min(PHX_MAX_PEERS, dp_size - 1);
+ * PHX_ERR_INVALID_ARG when fewer than k + 1 distinct domains exist.  One rank per domain gives phx_ring_peer's ring.
+ * Host arithmetic only; the buffers of whichever ranks are chosen are bound with phx_shard_bind_peers as before. */
+PHX_API int phx_ring_peers_topology_aware(uint32_t dp_size, uint32_t dp_rank, uint32_t k, const uint32_t *domain_of_rank,
+                                          uint32_t *peers);
 /* Received-buffer memory: a zeroed device allocation of its own (cudaMalloc), so that it can be exported
  * over CUDA IPC; owned by the caller, freed with phx_peer_buffer_free. */
 PHX_API int phx_peer_buffer_alloc(uint64_t bytes, void **d_buf);

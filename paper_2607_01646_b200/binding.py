@@ -130,6 +130,8 @@ PROTOTYPES = {
     "phx_graph_flush_peers_async": (C.c_int, [C.c_void_p, C.c_void_p]),
     "phx_graph_end": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_ring_peer": (C.c_int, [C.c_uint32, C.c_uint32, C.c_int32, C.POINTER(C.c_uint32)]),
+    "phx_ring_peers_topology_aware": (C.c_int, [C.c_uint32, C.c_uint32, C.c_uint32, C.POINTER(C.c_uint32),
+                                                C.POINTER(C.c_uint32)]),
     "phx_peer_buffer_alloc": (C.c_int, [C.c_uint64, C.POINTER(C.c_void_p)]),
     "phx_peer_buffer_free": (C.c_int, [C.c_void_p]),
     "phx_ipc_export": (C.c_int, [C.c_void_p, C.c_char_p]),
@@ -385,6 +387,13 @@ def phx_version() -> int:
 
 
 # ---- peer replication ------------------------------------------------------
+
+
+def phx_ring_peers_topology_aware(dp_size: int, dp_rank: int, k: int, domains) -> list:
+    dom = (C.c_uint32 * dp_size)(*[int(d) for d in domains])
+    out = (C.c_uint32 * max(k, 1))()
+    _ck(lib().phx_ring_peers_topology_aware(dp_size, dp_rank, k, dom, out), "phx_ring_peers_topology_aware")
+    return [int(out[j]) for j in range(k)]
 
 
 def phx_ring_peer(dp_size: int, dp_rank: int, j: int) -> int:

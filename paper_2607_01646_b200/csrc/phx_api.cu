@@ -1078,6 +1078,27 @@ int phx_ring_peer(uint32_t dp_size, uint32_t dp_rank, int32_t j, uint32_t *peer)
     return PHX_OK;
 }
 
+// Topology-aware placement (include/phx.h): the k holders of rank r's replicas are the nearest ranks
+// in ring order whose failure domains differ from the owner's and from one another.
+int phx_ring_peers_topology_aware(uint32_t dp_size, uint32_t dp_rank, uint32_t k, const uint32_t *domain_of_rank,
+                                  uint32_t *peers)
+{
+    if (!domain_of_rank || (k && !peers) || dp_size == 0 || dp_rank >= dp_size || k > dp_size - 1 || k > PHX_MAX_PEERS)
+        return PHX_ERR_INVALID_ARG;
+    uint32_t used[PHX_MAX_PEERS + 1];
+    uint32_t n_used = 0, found = 0;
+    used[n_used++] = domain_of_rank[dp_rank];
+    for (uint32_t j = 1; j < dp_size && found < k; ++j) {
+        const uint32_t q = (dp_rank + j) % dp_size;
+        bool taken = false;
+        for (uint32_t u = 0; u < n_used; ++u) taken = taken || used[u] == domain_of_rank[q];
+        if (taken) continue;
+        used[n_used++] = domain_of_rank[q];
+        peers[found++] = q;
+    }
+    return found == k ? PHX_OK : PHX_ERR_INVALID_ARG;  // fewer than k + 1 distinct failure domains
+}
+
 int phx_peer_buffer_alloc(uint64_t bytes, void **d_buf)
 {
     if (!d_buf || bytes == 0) return PHX_ERR_INVALID_ARG;

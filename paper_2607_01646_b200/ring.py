@@ -30,10 +30,26 @@ def predecessors(dp_size: int, dp_rank: int, k: int) -> List[int]:
     return [B.phx_ring_peer(dp_size, dp_rank, -j) for j in range(1, k + 1)]
 
 
-def route_handles(table: Sequence[Sequence[bytes]], dp_size: int, dp_rank: int, k: int) -> List[bytes]:
-    """table[h][j-1] = handle of the buffer rank h keeps for ITS j-th predecessor (gathered from all
-    ranks).  Returns the k handles this rank must open: its j-th successor's buffer number j-1."""
-    return [table[h][j] for j, h in enumerate(successors(dp_size, dp_rank, k))]
+def placement(dp_size: int, k: int, domains: Optional[Sequence[int]] = None) -> List[List[int]]:
+    """place[r] = the ranks that hold rank r's replicas: the plain ring (phx_ring_peer), or — `domains[q]` = the
+    failure domain of rank q — the topology-aware placement of PAPER.md:187 (phx_ring_peers_topology_aware)."""
+    if domains is None:
+        return [successors(dp_size, r, k) for r in range(dp_size)]
+    assert len(domains) == dp_size
+    return [B.phx_ring_peers_topology_aware(dp_size, r, k, domains) for r in range(dp_size)]
+
+
+def held_for(place: Sequence[Sequence[int]], h: int) -> List[int]:
+    """The owners whose replicas rank h holds, in the order of h's received buffers: by ring distance from the
+    owner to h (on the plain ring: predecessor 1, 2, .. k — buffer j-1 belongs to the j-th predecessor)."""
+    D = len(place)
+    return sorted((r for r in range(D) if h in place[r]), key=lambda r: (h - r) % D)
+
+
+def route_handles(table: Sequence[Sequence[bytes]], place: Sequence[Sequence[int]], dp_rank: int) -> List[bytes]:
+    """table[h][i] = handle of the buffer rank h keeps for held_for(place, h)[i] (gathered from all ranks).
+    Returns the handles this rank must open, one per holder in place[dp_rank]."""
+    return [table[h][held_for(place, h).index(dp_rank)] for h in place[dp_rank]]
 
 
 class _Raw:
@@ -48,7 +64,8 @@ def device_view(ptr: int, nbytes: int):
 
 
 class ReceivedBuffers:
-    """The k received buffers (two snapshot slots each) a rank keeps for its ring predecessors."""
+    """The received buffers (two snapshot slots each) a rank keeps for the owners whose replicas it holds: its k ring
+    predecessors, or held_for(place, rank) under a topology-aware placement (possibly none, possibly more than k)."""
 
     def __init__(self, slot_stride: int, k: int):
         self.slot_stride, self.k = slot_stride, k
@@ -74,10 +91,12 @@ class ReceivedBuffers:
 class PeerRing:
     """One rank's end of the ring: its received buffers + its successors' buffers opened over IPC."""
 
-    def __init__(self, shard, k: int, group=None, ring_size: Optional[int] = None, ring_rank: Optional[int] = None):
+    def __init__(self, shard, k: int, group=None, ring_size: Optional[int] = None, ring_rank: Optional[int] = None,
+                 domains: Optional[Sequence[int]] = None):
         """group: the DP group of this shard.  ring_size / ring_rank override the ring the handles are routed
         on when only some of the D data-parallel ranks are present (e.g. N < D GPUs of one node in a
-        benchmark): the ring then closes among the ranks of `group`."""
+        benchmark): the ring then closes among the ranks of `group`.  domains[q] = failure domain of ring
+        position q: the replicas go to the topology-aware placement instead of the ring successors."""
         import torch.distributed as dist
         self.shard, self.k = shard, k
         D = shard.info.dp_size if ring_size is None else ring_size
@@ -89,7 +108,9 @@ class PeerRing:
         # a rank whose allocation / IPC open failed must not leave the others waiting
         self.received, self.opened, err = None, [], None
         try:
-            self.received = ReceivedBuffers(shard.info.slot_stride, k)
+            self.place = placement(D, k, domains)          # same inputs on every rank => the same table everywhere
+            self.holds = held_for(self.place, r)
+            self.received = ReceivedBuffers(shard.info.slot_stride, len(self.holds))
             mine = self.received.handles()
         except Exception as e:  # noqa: BLE001
             mine, err = None, repr(e)
@@ -97,7 +118,7 @@ class PeerRing:
         dist.all_gather_object(table, mine, group=group)
         if err is None and all(t is not None for t in table):
             try:
-                self.opened = [B.phx_ipc_open(h) for h in route_handles(table, D, r, k)]
+                self.opened = [B.phx_ipc_open(h) for h in route_handles(table, self.place, r)]
                 B.phx_shard_bind_peers(shard.h, self.opened)
             except Exception as e:  # noqa: BLE001
                 err = repr(e)
@@ -229,12 +250,15 @@ class ParamGroup:
         self.own = None
 
 
-def connect_in_process(shards: Sequence, k: int) -> List[ReceivedBuffers]:
-    """D logical ranks in one process on one device: rank r's peer j is rank (r + j) mod D's received
-    buffer number j-1, bound by plain device pointer (no IPC inside one process)."""
+def connect_in_process(shards: Sequence, k: int, domains: Optional[Sequence[int]] = None) -> List[ReceivedBuffers]:
+    """D logical ranks in one process on one device: every rank gets a received buffer per owner it holds replicas
+    for (held_for order; on the plain ring buffer j-1 belongs to the j-th predecessor), bound by plain device
+    pointer (no IPC inside one process)."""
     D = len(shards)
     assert all(s.info.dp_size == D and s.info.dp_rank == r for r, s in enumerate(shards))
-    recv = [ReceivedBuffers(s.info.slot_stride, k) for s in shards]
+    place = placement(D, k, domains)
+    holds = [held_for(place, h) for h in range(D)]
+    recv = [ReceivedBuffers(s.info.slot_stride, len(holds[h])) for h, s in enumerate(shards)]
     for r, s in enumerate(shards):
-        B.phx_shard_bind_peers(s.h, [recv[h].ptrs[j] for j, h in enumerate(successors(D, r, k))])
+        B.phx_shard_bind_peers(s.h, [recv[h].ptrs[holds[h].index(r)] for h in place[r]])
     return recv

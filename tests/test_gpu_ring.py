@@ -22,12 +22,12 @@ from gpu_util import DEV, assert_state_equal, bits16, grad_record, hp_of
 pytestmark = pytest.mark.gpu
 
 
-def build_ring(numels, D, k, *, chunk=8192, **shard_kw):
+def build_ring(numels, D, k, *, chunk=8192, domains=None, **shard_kw):
     """D Shards (one per DP rank) wired in process + the ring oracle, equal initial state, per-rank grads."""
     wls = [W.tiny_workload(numels, dp_size=D, dp_rank=r) for r in range(D)]
     shards = [Shard(wl, device=DEV, chunk_bytes=chunk, **shard_kw) for wl in wls]
-    recv = PR.connect_in_process(shards, k)
-    oring = R.OracleRing(wls[0].layout(), D, k, chunk_bytes=(chunk + 255) & ~255)
+    recv = PR.connect_in_process(shards, k, domains)
+    oring = R.OracleRing(wls[0].layout(), D, k, chunk_bytes=(chunk + 255) & ~255, domains=domains)
     for r, (s, o) in enumerate(zip(shards, oring.shards)):
         p0 = W.init_params(s.n, s.n_padded, seed=100 + r)
         s.p.copy_(p0)
@@ -123,6 +123,61 @@ def test_recovery_from_a_surviving_holder_resumes_bit_exactly(failed, rmode):
     for r, (s, o) in enumerate(zip(shards, oring.shards)):
         assert_state_equal(s, o, f"resumed rank {r}")
         B.phx_snapshot_wait_peers(s.h, 7)
+        s.close()
+    for rb in recv + recv2:
+        rb.free()
+
+
+@pytest.mark.parametrize("D,k,domains,dead", [(4, 1, [0, 0, 1, 1], 0), (6, 2, [0, 0, 1, 1, 2, 2], 1),
+                                              (5, 2, [7, 3, 3, 7, 9], 3)])
+def test_topology_aware_placement_survives_a_whole_failed_domain(D, k, domains, dead):
+    """PAPER.md:187 (R38): the k + 1 copies of every shard sit under distinct failure domains; the received
+    buffers — irregular now: some ranks hold for several owners, some for none — are byte-identical to the oracle's,
+    and after ALL ranks of one domain die every lost shard comes back from a surviving holder and resumes bit-exactly."""
+    wls, shards, recv, oring = build_ring([20_000, 77], D, k, domains=domains)
+    place = PR.placement(D, k, domains)
+    assert place == oring.place and R.max_copies_in_one_domain(domains, place) == 1
+    holds = [PR.held_for(place, h) for h in range(D)]
+    assert [len(rb.ptrs) for rb in recv] == [len(x) for x in holds]
+    streams = (torch.cuda.Stream(device=DEV), torch.cuda.Stream(device=DEV))
+    for t in range(1, 5):
+        step_all(wls, shards, oring, t, streams)
+    for s in shards:
+        B.phx_snapshot_wait_peers(s.h, 4)
+    for r, s in enumerate(shards):
+        for h in place[r]:
+            j = holds[h].index(r) + 1
+            for slot in (0, 1):
+                assert np.array_equal(received_bytes(recv, h, j, slot, s), oring.recv[(h, r)][slot]), (r, h, slot)
+    failed = [q for q in range(D) if domains[q] == domains[dead]]
+    g5 = grads_for(wls, shards, 5)
+    for r in failed:                                     # step 5 in flight on the nodes that die with their switch
+        shards[r].step_and_snapshot(g5[r].to(DEV), 5)
+        oring.shards[r].step(grad_record(g5[r]), **hp_of(wls[r]), step=5)
+    torch.cuda.synchronize()
+    oring.fail(failed)
+    for r in failed:
+        shards[r].close()
+        for j in range(1, len(holds[r]) + 1):
+            recv[r].view(j).fill_(0xA5)
+    for r in failed:
+        fresh = Shard(wls[r], device=DEV, chunk_bytes=8192)
+        holder, _, _, hd = oring.newest_replica_of(r)
+        assert holder not in failed
+        assert B.phx_restore_from(fresh.h, recv[holder].ptrs[holds[holder].index(r)]) == 4 == oring.recover(r)
+        shards[r] = fresh
+        assert_state_equal(fresh, oring.shards[r], f"restored rank {r}")
+    recv2 = PR.connect_in_process(shards, k, domains)    # topology re-established (PAPER.md:171 stage 2)
+    for t in (5, 6):
+        gs = grads_for(wls, shards, t)
+        for r, (s, o) in enumerate(zip(shards, oring.shards)):
+            if o.last_step == t - 1:
+                s.step_and_snapshot(gs[r].to(DEV), t)
+                B.phx_snapshot_flush_peers_async(s.h, streams[1])
+                o.step(grad_record(gs[r]), **hp_of(wls[r]), step=t)
+    for r, (s, o) in enumerate(zip(shards, oring.shards)):
+        assert_state_equal(s, o, f"resumed rank {r}")
+        B.phx_snapshot_wait_peers(s.h, 6)
         s.close()
     for rb in recv + recv2:
         rb.free()

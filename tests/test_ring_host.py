@@ -55,14 +55,46 @@ def test_peer_entry_points_fail_loudly_without_binding_or_gpu():
     B.phx_shard_destroy(h)
 
 
-def _worker(rank, world, k, port, q):
+def test_topology_aware_placement_matches_the_oracle_on_every_domain_map():
+    import ctypes as C
+    import itertools
+    from oracle import oracle as O
+    L = B.lib()
+    for D in range(2, 7):
+        for domains in itertools.product(range(min(D, 4)), repeat=D):
+            for k in range(1, min(D, 5)):
+                for r in range(D):
+                    try:
+                        want = R.holders_topology_aware(domains, r, k)
+                    except O.OracleError:
+                        want = None
+                    if want is None:
+                        dom = (C.c_uint32 * D)(*domains)
+                        out = (C.c_uint32 * k)()
+                        assert L.phx_ring_peers_topology_aware(D, r, k, dom, out) == B.PHX_ERR_INVALID_ARG
+                    else:
+                        assert B.phx_ring_peers_topology_aware(D, r, k, domains) == want, (domains, r, k)
+    # one rank per domain: the plain ring; held_for on the plain ring: predecessor 1, 2, .. k
+    for D, k in ((3, 1), (5, 2), (6, 4)):
+        assert PR.placement(D, k, list(range(D))) == PR.placement(D, k) == R.placement(D, k)
+        for h in range(D):
+            assert PR.held_for(PR.placement(D, k), h) == PR.predecessors(D, h, k)
+    dom = (C.c_uint32 * 4)(0, 0, 1, 1)
+    out = (C.c_uint32 * 4)()
+    for args in ((0, 0, 1, dom, out), (4, 4, 1, dom, out), (4, 0, 4, dom, out), (4, 0, 1, None, out), (4, 0, 1, dom, None)):
+        assert L.phx_ring_peers_topology_aware(*args) == B.PHX_ERR_INVALID_ARG, args[:3]
+    assert L.phx_ring_peers_topology_aware(4, 0, 0, dom, None) == B.PHX_OK
+
+
+def _worker(rank, world, k, port, q, domains=None):
     os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     dist.init_process_group("gloo")
-    # stand-in handles: 64 bytes that name (holder, buffer index)
-    mine = [bytes([rank, j]) + b"\0" * 62 for j in range(k)]
+    place = PR.placement(world, k, domains)
+    # stand-in handles: 64 bytes that name (holder, buffer index); one buffer per owner this rank holds replicas for
+    mine = [bytes([rank, j]) + b"\0" * 62 for j in range(len(PR.held_for(place, rank)))]
     table = [None] * world
     dist.all_gather_object(table, mine)
-    got = PR.route_handles(table, world, rank, k)
+    got = PR.route_handles(table, place, rank)
     q.put((rank, [(h[0], h[1]) for h in got]))
     dist.barrier()
     dist.destroy_process_group()
@@ -84,3 +116,21 @@ def test_handle_exchange_on_gloo(world, k):
         # rank r must open, for j = 1..k, the buffer number j-1 of its j-th ring successor — exactly the
         # buffers the ring oracle's replicate() writes
         assert res[r] == [(R.ring_peer(world, r, j), j - 1) for j in range(1, k + 1)]
+
+
+def test_handle_exchange_with_a_topology_aware_placement_on_gloo():
+    world, k, domains = 4, 1, [0, 0, 1, 1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29960 + os.getpid() % 30
+    ps = [ctx.Process(target=_worker, args=(r, world, k, port, q, domains)) for r in range(world)]
+    for p in ps:
+        p.start()
+    res = dict(q.get(timeout=120) for _ in ps)
+    for p in ps:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    place = R.placement(world, k, domains)
+    assert place == [[2], [2], [0], [0]]
+    # rank 2 holds for owners 1 (distance 1) and 0 (distance 2) in that order; rank 0 for owners 3 and 2
+    assert res == {0: [(2, 1)], 1: [(2, 0)], 2: [(0, 1)], 3: [(0, 0)]}
