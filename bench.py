@@ -572,9 +572,11 @@ class Rig:
         l0 = B.phx_kernel_launches(self.s.h)
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
         ev[0].record(self.cur)
+        h0 = time.perf_counter()
         for k in range(K):
             self.do_step()
             ev[k + 1].record(self.cur)
+        self.host_enqueue_us = (time.perf_counter() - h0) * 1e6 / K      # the calls only enqueue: host time per step
         torch.cuda.synchronize()
         per = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
         return ev[0].elapsed_time(ev[K]), per, B.phx_kernel_launches(self.s.h) - l0
@@ -1117,6 +1119,7 @@ def measure_config(args, key, link, clk, rank, world, local_rank, K, Wm, peak, h
                kernel_ms=kern_ms, kernel_bytes_per_element=BPE, kernel_gbs=kern_gbs,
                kernel_frac_of_measured_peak=kern_gbs / peak, kernel_frac_of_nominal_8TBps=kern_gbs / NOMINAL_HBM_GBS,
                elements_per_s=N / (step_ms * 1e-3), snapshot_off_step_ms=off_ms,
+               host_enqueue_us_per_step=rig.host_enqueue_us,
                snapshot_off_gbs=(step_bpe - 12) * N / (off_ms * 1e-3) / 1e9, steps_timed=K)
     if rig.clip and not rig.fp32 and rank == 0:
         with clk.leg(f"{tag}.producer_clip"):

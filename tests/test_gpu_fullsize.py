@@ -121,6 +121,15 @@ def test_whole_array_parity_full_size(key):
     assert s.restore() == last
     for name, dev, ref in (("p", s.p, o.p), ("m", s.m, o.m), ("v", s.v, o.v), ("p16", s.p16, o.p16)):
         assert_whole_equal(dev, ref, f"{key} restored {name}")
+    # ... and through the two-phase restore (parameters first on the side stream, moments behind them)
+    s.drop_live()
+    side.wait_stream(torch.cuda.current_stream())
+    assert s.restore_async(side) == last
+    s.restore_wait_params()
+    assert_whole_equal(s.p16, o.p16, f"{key} two-phase restore, p16 at 'parameters ready'")
+    torch.cuda.synchronize()
+    for name, dev, ref in (("p", s.p, o.p), ("m", s.m, o.m), ("v", s.v, o.v), ("p16", s.p16, o.p16)):
+        assert_whole_equal(dev, ref, f"{key} two-phase restored {name}")
     s.close()
 
 
