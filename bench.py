@@ -573,10 +573,12 @@ class Rig:
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
         ev[0].record(self.cur)
         h0 = time.perf_counter()
+        kh = min(K, 48)          # host cost of the calls: a short burst, before the driver's launch queue can fill up
         for k in range(K):
             self.do_step()
             ev[k + 1].record(self.cur)
-        self.host_enqueue_us = (time.perf_counter() - h0) * 1e6 / K      # the calls only enqueue: host time per step
+            if k + 1 == kh:
+                self.host_enqueue_us = (time.perf_counter() - h0) * 1e6 / kh   # the calls only enqueue
         torch.cuda.synchronize()
         per = [ev[k].elapsed_time(ev[k + 1]) for k in range(K)]
         return ev[0].elapsed_time(ev[K]), per, B.phx_kernel_launches(self.s.h) - l0
@@ -1021,7 +1023,7 @@ class Rig:
         self.s.close()
 
 
-def measure_host_link(torch, device, nbytes=1 << 30, reps=5):
+def measure_host_link(torch, device, nbytes=1 << 30, reps=10):
     """Measured pinned-copy peak of the host link, each direction (north_star)."""
     h = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
     d = torch.empty(nbytes, dtype=torch.uint8, device=device)
@@ -1119,7 +1121,7 @@ def measure_config(args, key, link, clk, rank, world, local_rank, K, Wm, peak, h
                kernel_ms=kern_ms, kernel_bytes_per_element=BPE, kernel_gbs=kern_gbs,
                kernel_frac_of_measured_peak=kern_gbs / peak, kernel_frac_of_nominal_8TBps=kern_gbs / NOMINAL_HBM_GBS,
                elements_per_s=N / (step_ms * 1e-3), snapshot_off_step_ms=off_ms,
-               host_enqueue_us_per_step=rig.host_enqueue_us,
+               host_enqueue_us_per_step=rig.host_enqueue_us,   # Python binding + C call + launches, first 48 steps
                snapshot_off_gbs=(step_bpe - 12) * N / (off_ms * 1e-3) / 1e9, steps_timed=K)
     if rig.clip and not rig.fp32 and rank == 0:
         with clk.leg(f"{tag}.producer_clip"):
@@ -1635,6 +1637,43 @@ def run_timeline(args):
     emit(mode="timeline-summary", config=args.headline, gemms=G, flush_alone_ms=flush_ms,
          flush_fraction_under_next_gemm_window=under, commit_after_next_step_enqueued_ms=waits,
          note="commit_after_next_step_enqueued_ms > 0 would be a stall at the single sync point (PAPER.md:226)")
+
+    # ---- recovery timeline: fault, two-phase restore (phx_restore_async) beside the recomputed iteration ---------
+    Gr = rig.gemms_for(flush_ms, 1.25, False)
+    for form in ("one_phase", "two_phase"):
+        rig.do_step()
+        rig.flush()
+        rig.s.wait(rig.step)
+        torch.cuda.synchronize()
+        rig.s.drop_live()
+        torch.cuda.synchronize()
+        r0, rp, rs, k0, k1 = E(), E(), E(), E(), E()
+        gm = []
+        r0.record(rig.cur)
+        if form == "two_phase":
+            rig.side.wait_stream(rig.cur)
+            rig.step = rig.s.restore_async(rig.side)      # side stream: p -> bf16 copy -> m -> v
+            rs.record(rig.side)
+            rig.s.restore_wait_params(rig.cur)            # compute stream: waits for "parameters ready" only
+        else:
+            rig.step = rig.s.restore()
+            rs.record(rig.cur)
+        rp.record(rig.cur)
+        for part in range(marks):
+            rig.gemm_window(Gr // marks)
+            e = E()
+            e.record(rig.cur)
+            gm.append(e)
+        k0.record(rig.cur)
+        rig.do_step()                                     # waits (stream-side) for the moments
+        k1.record(rig.cur)
+        torch.cuda.synchronize()
+        tr = lambda e: r0.elapsed_time(e)  # noqa: E731
+        emit(mode="timeline-recovery", config=args.headline, form=form, gemms=Gr // marks * marks,
+             params_ready_ms=tr(rp), state_ready_ms=tr(rs), gemm_window_ms=[tr(rp), tr(gm[-1])],
+             gemm_marks_ms=[tr(e) for e in gm], step_ms=[tr(k0), tr(k1)],
+             note="ms since the fault was detected; two_phase: the moments (state_ready) arrive on the side stream "
+                  "while the recomputed iteration's GEMMs run on the compute stream")
     rig.close()
     return 0
 
