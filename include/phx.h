@@ -19,7 +19,7 @@
  *     small internals (events, a few KB of device scratch, one fp64 reduction partial per 16384 elements).
  *   - Streams are cudaStream_t passed as void*.  Calls that take a stream only ENQUEUE work;
  *     they never block the host on the device unless stated.  The three hot calls
- *     (phx_step_and_snapshot, phx_snapshot_flush_async, phx_restore) never do.  Host-blocking by
+ *     (phx_step_and_snapshot, phx_snapshot_flush_async, phx_restore / phx_restore_async) never do.  Host-blocking by
  *     contract: phx_snapshot_wait*, phx_restore_from / phx_replica_inspect (a blocking 512-byte read
  *     of a FOREIGN replica's envelopes), phx_last_clip, phx_graph_begin / phx_graph_end (mode
  *     switches), phx_shard_destroy.  Ordering between the compute stream and the flush stream
