@@ -16,11 +16,12 @@ The one line covers EVERY bandwidth-sized config of BASELINE.json (c2, c3, c4a, 
   configs    per config: step / kernel / snapshot-off ms and GB/s, flush GB/s against the pinned-copy peak measured
              in the same run, exposed checkpoint ms/iteration at T_c >= 4 T_D2H and at the tight 1.25 T_D2H window,
              with eagerly launched iterations and with the whole iteration captured in a CUDA graph (the
-             graph-capturable form of the step), e2e through host buffers, restore + recompute, the c4 hot-swap
-             scenario (bit-exact trajectory flag), the c5 chunk x depth grid, the c3 producer-side clip.
+             graph-capturable form of the step), e2e through host buffers, restore + recompute (one phase, and the
+             two-phase restore beside the recomputed iteration), the c4 hot-swap scenario (bit-exact trajectory
+             flag), the c5 chunk x depth grid, the c3 producer-side clip.
   e2e        the headline config through the same C-ABI calls with HOST buffers (H2D grads, D2H snapshot + commit).
   cpu_baseline  the oracle as it stands on the box's host cores, on the SAME bounded sample `--impl reference` times.
-  clocks     nvidia-smi sampled over the whole run (50 ms), reported per timed leg.
+  clocks     NVML (what nvidia-smi prints from) sampled over the whole run every 2 ms, reported per timed leg.
 `--impl reference` times the oracle instead (the reference arm of this tier).
 """
 from __future__ import annotations
