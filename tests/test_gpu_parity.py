@@ -155,6 +155,54 @@ def test_extreme_values_denormals_and_zeros():
     s.close()
 
 
+@pytest.mark.parametrize("seed", range(10))
+def test_random_hyperparameters_and_late_step_indices_bit_exact(seed):
+    """The arithmetic contract (every operation individually rounded, derived scalars in binary64) over the whole
+    hyperparameter domain, not only the configs' defaults: random lr / betas / eps / wd incl. the corners beta = 0,
+    a vanishing eps, wd = 0, a start deep into training (bias corrections close to 1, beta^t underflowing to 0), a different
+    hyperparameter set at EVERY step (a schedule), warm moments — eager form and graph-capturable form."""
+    rng = np.random.default_rng(1000 + seed)
+
+    def draw():
+        return W.Hyper(lr=float(10.0 ** rng.uniform(-6, -1)),
+                       beta1=float(rng.choice([0.0, 0.5, 0.9, 0.99, rng.uniform(0, 1)])),
+                       beta2=float(rng.choice([0.0, 0.95, 0.999, 0.9999, rng.uniform(0, 1)])),
+                       eps=float(rng.choice([1e-30, 1e-8, 1e-5, 1e-12])),   # eps = 0 makes 0/0 in the pad lanes (R8)
+                       wd=float(rng.choice([0.0, 0.01, 0.1, rng.uniform(0, 1)])))
+    t0 = int(rng.choice([0, 1, 7, 999, 10**5, 2**20 - 3, 2**31 + 5]))
+    wl = W.tiny_workload([int(rng.integers(1, 200_000)), 77], dp_size=2, dp_rank=int(rng.integers(0, 2)),
+                         grad_kind="heavy_tail", hyper=W.Hyper(max_grad_norm=float(rng.choice([0.0, 0.01]))))
+    s, o, gdev, gbits = make_pair(wl, steps=6, init_mv=True)
+    s.set_state(t0)
+    o.last_step = t0
+    side = torch.cuda.Stream(device=DEV)
+    hps = [draw() for _ in range(6)]
+    for i in range(3):                                   # eager form, a new hyperparameter set every step
+        hp = hps[i]
+        s.step_and_snapshot(gdev[i], t0 + i + 1, hyper=hp)
+        s.flush_async(side)
+        o.step(gbits[i], lr=hp.lr, beta1=hp.beta1, beta2=hp.beta2, eps=hp.eps, wd=hp.wd, step=t0 + i + 1)
+        o.snapshot()
+        assert_state_equal(s, o, f"seed {seed} t0 {t0} eager step {i} {hp}")
+    s.graph_begin(hyper=hps[3])                          # graph form: scalars derived on the device
+    for i in range(3, 6):
+        hp = hps[i]
+        s.graph_set_hyper(hp)
+        s.graph_step(gdev[i])
+        s.graph_flush(side)
+        o.step(gbits[i], lr=hp.lr, beta1=hp.beta1, beta2=hp.beta2, eps=hp.eps, wd=hp.wd, step=t0 + i + 1)
+        torch.cuda.synchronize()                         # (phx_last_step follows the device counter at graph_end only)
+        for name, dev, ref in (("p", s.p, o.p), ("m", s.m, o.m), ("v", s.v, o.v)):
+            assert np.array_equal(dev.cpu().numpy().view(np.uint32), ref.view(np.uint32)), (seed, t0, i, name, hp)
+        assert np.array_equal(bits16(s.p16), o.p16), (seed, t0, i, hp)
+        o.snapshot()
+    assert s.graph_end() == t0 + 6
+    assert_state_equal(s, o, f"seed {seed} t0 {t0} after the graph form")
+    s.wait(t0 + 6)
+    assert np.array_equal(s.replica_slot(t0 + 6).numpy(), o.replica[(t0 + 6) % 2])
+    s.close()
+
+
 def test_snapshot_off_variant_gives_identical_live_bits():
     wl = W.tiny_workload([100_000, 31], dp_size=2, dp_rank=0)
     a, o, gdev, gbits = make_pair(wl, steps=3)
