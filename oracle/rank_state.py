@@ -152,7 +152,10 @@ class FullRankState:
         o.restored_user = h["user"]
         return o.last_step
 
-    # -- R33 in two phases (reading R37): parameters (p, the bf16 copy, W) first, moments second ---
+    # -- R33 in two phases (reading R37): the parameters first, the optimizer state second.  For a full
+    # rank state "the parameters" are W itself — the forward/backward of the recomputed iteration reads W and nothing
+    # else; the rank's own range of W (its model-param copy, R29) is part of the snapshot's W — so phase 1 is W
+    # ALONE and the fp32 master p comes back in phase 2 with the moments.
     def restore_in_place_params_first(self) -> int:
         best = self.newest_committed()
         if best is None:
@@ -161,9 +164,9 @@ class FullRankState:
         o = self.o
         raw = self.slots[s]
         H, N4 = O.HEADER_BYTES, 4 * o.n_padded
-        o.p[:] = raw[H:H + N4].view(np.float32)
         self.W[:] = raw[H + 3 * N4:].view(self.wdtype)
-        o.p16[:] = O.rne_bf16(o.p) if o.precision == "bf16" else 0
+        if o.precision == "bf16":
+            o.p16[:] = self.own_range()            # the model-param copy IS the rank's range of W
         self._restoring = (s, h)
         o.last_step = -1
         return h["step"]
@@ -173,6 +176,7 @@ class FullRankState:
         o = self.o
         raw = self.slots[s]
         H, N4 = O.HEADER_BYTES, 4 * o.n_padded
+        o.p[:] = raw[H:H + N4].view(np.float32)
         o.m[:] = raw[H + N4:H + 2 * N4].view(np.float32)
         o.v[:] = raw[H + 2 * N4:H + 3 * N4].view(np.float32)
         o.last_step = h["step"]

@@ -101,8 +101,16 @@ def test_full_rank_state_two_phases(precision, torn):
     want = a.restore_in_place()
     assert want == (3 if torn is None else 2)
     b.o.m[:] = 9.0
+    b.o.p[:] = -7.0
     assert b.restore_in_place_params_first() == want
-    assert np.array_equal(b.W, a.W) and b.o.p.tobytes() == a.o.p.tobytes() and np.array_equal(b.o.p16, a.o.p16)
-    assert np.all(b.o.m == 9.0)                          # phase 1 left the moments alone
+    # for a full rank state the parameters ARE W: phase 1 brings back W alone (the own range of it = the model-param
+    # copy, which must equal torch's bf16 cast of the p that arrives in phase 2)
+    assert np.array_equal(b.W, a.W) and np.array_equal(b.o.p16, a.o.p16)
+    assert np.all(b.o.m == 9.0) and np.all(b.o.p == -7.0)          # phase 1 left p and the moments alone
     assert b.restore_in_place_finish() == want
     assert state_bytes(a.o) == state_bytes(b.o) and np.array_equal(a.W, b.W)
+    if precision == "bf16":
+        cast = torch.from_numpy(b.o.p.copy()).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+        assert np.array_equal(b.own_range(), cast)       # R31: the own range of the restored W == RNE_bf16(restored p)
+    else:
+        assert np.array_equal(b.own_range(), b.o.p)
