@@ -264,9 +264,11 @@ PHX_API int phx_restore(phx_shard_t *s, void *stream, uint64_t *restored_step);
  * §V-C): the recomputed iteration's forward/backward reads only the model parameters; the moments are first read
  * by its optimizer step.  phx_restore_async makes the same choice of slot, identity check and hazard ordering as
  * phx_restore (and only enqueues), but runs everything on `side_stream` in the order
- *     p -> model-param copy (bf16 regeneration) [-> W, full rank state]   == "parameters ready"
- *     m -> v                                                              == "state ready"
- * (PHX_RESTORE_BULK_KERNEL: two launches of the bulk kernel, planes {p} then {m, v}).
+ *     optimizer-only payload:  p -> model-param copy (bf16 regeneration)  == "parameters ready";   m -> v  == "state ready"
+ *     full rank state:         W (alone: the rank's own range of W IS its model-param copy, and the forward/backward
+ *                              reads nothing else)                          == "parameters ready";   p -> m -> v  == "state ready"
+ * (PHX_RESTORE_BULK_KERNEL: two launches of the bulk kernel, the second — beside the recomputed iteration — on four
+ * persistent CTAs, which already saturate the host link and leave the other SMs to the compute).
  * phx_restore_wait_params makes `stream` wait (stream-side) until the parameters are in place, after which the
  * forward/backward of the recomputed iteration may be enqueued on it; two thirds of the host-link transfer then
  * hide behind that compute.  The next phx_step_and_snapshot (any stream) waits for "state ready" by itself, and so do

@@ -919,38 +919,49 @@ int enqueue_restore(phx_shard *s, int best, const phx_snapshot_header_t &hdr, co
     void *p16 = fp32_mode(s) ? nullptr : s->d_p16;
     const float *ksrc = reinterpret_cast<const float *>(kern_src + off);
     const uint8_t *src = copy_src + off;
-    // phase 1 (or, one-phase, everything): p and the model-param copy
-    if (bulk) {
-        phx::RestorePlanes pl{{ksrc, ksrc + N, ksrc + 2 * N}, {s->d_p, s->d_m, s->d_v}, two_phase ? 1 : 3};
-        PHX_CK(phx::launch_restore_bulk(pl, p16, N, 2 * s->sm_count, st));
-        s->launches += N ? 1 : 0;
-    } else {
-        PHX_CK(cudaMemcpyAsync(s->d_p, src, 4 * N, cudaMemcpyDefault, st));
-        if (!two_phase) {
-            PHX_CK(cudaMemcpyAsync(s->d_m, src + 4 * N, 4 * N, cudaMemcpyDefault, st));
-            PHX_CK(cudaMemcpyAsync(s->d_v, src + 8 * N, 4 * N, cudaMemcpyDefault, st));
-        }
-        if (p16) {
-            PHX_CK(phx::launch_regen_bf16(s->d_p, s->d_p16, N, st));
-            s->launches += N ? 1 : 0;
-        }
-    }
-    if (want_payload != 0)  // §8(f4) in-place recovery: W comes back from the same slot, no other rank is read
-        PHX_CK(cudaMemcpyAsync(s->d_W, copy_src + off + 12 * N, s->info.param_bytes, cudaMemcpyDefault, st));
-    if (two_phase) {  // phase 2: the moments
-        PHX_CK(cudaEventRecord(s->ev_rparams, st));
-        s->rparams_valid = true;
+    // planes [first, first + count) of p ‖ m ‖ v -> the live planes; with_p16: regenerate the model-param copy from p
+    auto planes = [&](int first, int count, bool with_p16, int ctas) -> int {
+        float *dst[3] = {s->d_p, s->d_m, s->d_v};
         if (bulk) {
-            phx::RestorePlanes pl{{ksrc + N, ksrc + 2 * N, nullptr}, {s->d_m, s->d_v, nullptr}, 2};
-            // the moments come back BESIDE the recomputed iteration's kernels: FOUR persistent CTAs already saturate the
-            // host link (2: 86 %; 8-37: the same rate, but each CTA's 96 KB of shared memory takes an SM away from the
-            // forward/backward — profiles/r02c_restore_bulk.md), the other 144 SMs stay with the compute
-            PHX_CK(phx::launch_restore_bulk(pl, nullptr, N, kRestorePhase2Ctas, st));
+            phx::RestorePlanes pl{{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}, count};
+            for (int k = 0; k < count; ++k) {
+                pl.src[k] = ksrc + (uint64_t)(first + k) * N;
+                pl.dst[k] = dst[first + k];
+            }
+            PHX_CK(phx::launch_restore_bulk(pl, with_p16 ? p16 : nullptr, N, ctas, st));
             s->launches += N ? 1 : 0;
         } else {
-            PHX_CK(cudaMemcpyAsync(s->d_m, src + 4 * N, 4 * N, cudaMemcpyDefault, st));
-            PHX_CK(cudaMemcpyAsync(s->d_v, src + 8 * N, 4 * N, cudaMemcpyDefault, st));
+            for (int k = first; k < first + count; ++k)
+                PHX_CK(cudaMemcpyAsync(dst[k], src + (uint64_t)k * 4 * N, 4 * N, cudaMemcpyDefault, st));
+            if (with_p16 && p16) {
+                PHX_CK(phx::launch_regen_bf16(s->d_p, s->d_p16, N, st));
+                s->launches += N ? 1 : 0;
+            }
         }
+        return PHX_OK;
+    };
+    const uint8_t *wsrc = copy_src + off + 12 * N;  // §8(f4): W sits behind the optimizer part of the same slot
+    int rc = PHX_OK;
+    if (!two_phase) {
+        if ((rc = planes(0, 3, true, 2 * s->sm_count)) != PHX_OK) return rc;
+        if (want_payload != 0)  // in-place recovery: W comes back from the same slot, no other rank is read
+            PHX_CK(cudaMemcpyAsync(s->d_W, wsrc, s->info.param_bytes, cudaMemcpyDefault, st));
+    } else {
+        // phase 1 = what the recomputed iteration's forward/backward reads.  Optimizer-only payload: p, from which the
+        // model-param copy is regenerated.  Full rank state: W ALONE — the rank's own range of it (d_p_bf16, enforced
+        // by phx_shard_bind_params) is part of the snapshot's W, so p can wait for phase 2 with the moments.
+        if (want_payload != 0) {
+            PHX_CK(cudaMemcpyAsync(s->d_W, wsrc, s->info.param_bytes, cudaMemcpyDefault, st));
+        } else if ((rc = planes(0, 1, true, 2 * s->sm_count)) != PHX_OK) {
+            return rc;
+        }
+        PHX_CK(cudaEventRecord(s->ev_rparams, st));
+        s->rparams_valid = true;
+        // phase 2 runs BESIDE the recomputed iteration's kernels: FOUR persistent CTAs of the bulk kernel already
+        // saturate the host link (2: 86 %; 8-37: the same rate, but each CTA's 96 KB of shared memory takes an SM away
+        // from the forward/backward — profiles/r02c_restore_bulk.md), the other 144 SMs stay with the compute
+        rc = want_payload != 0 ? planes(0, 3, false, kRestorePhase2Ctas) : planes(1, 2, false, kRestorePhase2Ctas);
+        if (rc != PHX_OK) return rc;
         PHX_CK(cudaEventRecord(s->ev_rstate, st));
         s->rstate_valid = true;
     }
