@@ -794,8 +794,9 @@ class Rig:
                                          "two_phase_restore_ms": med["overlapped"]},
                 "exposed_recovery_ms_serial": med["serial"] - med["no_fault"],
                 "exposed_recovery_ms_two_phase": med["overlapped"] - med["no_fault"], "repeats": reps,
-                "note": "phx_restore_async: p + bf16 copy first on the side stream, m and v behind the recomputed "
-                        "iteration's forward/backward (stand-in GEMMs); the step waits for them by itself"}
+                "note": "phx_restore_async: the parameters first on the side stream (p + bf16 copy; W alone for a full "
+                        "rank state), the rest behind the recomputed iteration's forward/backward (stand-in GEMMs); the "
+                        "step waits for it by itself"}
 
     def hotswap(self, G, two_phase=False):
         """BASELINE.json:configs[3]: 20 steps with snapshots (overlapped with G GEMMs each), the live shard is dropped
