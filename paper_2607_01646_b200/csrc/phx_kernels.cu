@@ -15,9 +15,9 @@
 //   k_grads_finalize  : SURVEY §8(f4) second half: the gradient producer's epilogue — fp32 main gradients
 //                       x scale -> RNE bf16 gradients AND the fp64 sum of squares of the rounded values, one pass.
 //   k_regen_bf16      : p16 = RNE_bf16(p).
-//   k_restore_bulk    : a6, pulls the replica from mapped pinned host memory with 1-D bulk
-//                       async copies (TMA, cp.async.bulk + mbarrier) into shared memory, writes
-//                       p, m, v back with bulk stores and regenerates the bf16 copy.
+//   k_restore_bulk    : a6, pulls the replica (a list of 1..3 of its planes) from mapped pinned host memory
+//                       with 1-D bulk async copies (TMA, cp.async.bulk + mbarrier) into shared memory, writes
+//                       the live planes back with bulk stores and regenerates the bf16 copy from p.
 //
 // The other flavours tried in round 1 (128-bit vectors, two/four groups per thread, .cs hints, a TMA tile
 // pipeline: 5.8-6.4 TB/s against 6.65 for this one) are recorded in profiles/r01_step8_c2_full.md.
@@ -675,12 +675,15 @@ cudaError_t launch_regen_bf16(const float *p, void *p16, uint64_t n_padded, cuda
 
 // ------------------------------------------------------------------------------------------
 // a6: restore from the mapped pinned host replica with 1-D bulk async copies (TMA).
-//   Per CTA: kStages shared-memory stages of 3 x kTile fp32 (p, m, v tiles).  One elected
-//   thread arms an mbarrier with the byte count and issues three cp.async.bulk loads
-//   host -> smem per tile; when they land it issues three cp.async.bulk stores smem -> live
-//   p, m, v (no register traffic), while all threads read the p tile from smem, convert to
-//   bf16 and store the copy.  The host link (PCIe) is the bound; the deep pipeline keeps
-//   148 x 2 x kStages x 24 KB of reads in flight.
+//   Takes a PLANE LIST (1..3 of p, m, v): all three for the one-phase restore; {p} and then {m, v} (or, full rank
+//   state, {p, m, v} behind W) for the two-phase restore of phx_restore_async.
+//   Per CTA: kStages shared-memory stages of 3 x kTile fp32 (one tile per plane).  One elected
+//   thread arms an mbarrier with the byte count and issues one cp.async.bulk load
+//   host -> smem per plane and tile; when they land it issues the cp.async.bulk stores smem -> live
+//   planes (no register traffic), while all threads read the tile of plane 0 (p) from smem, convert to
+//   bf16 and store the copy (p16 != nullptr).  The host link (PCIe) is the bound: 148 x 2 CTAs keep
+//   296 x kStages x 24 KB of reads in flight, but FOUR CTAs already saturate it (profiles/r02c_restore_bulk.md),
+//   which is what the second phase runs on so that the recomputed iteration keeps the other SMs.
 // ------------------------------------------------------------------------------------------
 constexpr int kTile = 2048;  // elements per plane per tile (8 KB)
 constexpr int kStages = 4;
