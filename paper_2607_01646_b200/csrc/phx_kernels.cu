@@ -427,14 +427,24 @@ cudaError_t launch_derive_scalars(float lr, float beta1, float beta2, float wd, 
 //              (sign dropped: only squares are taken); zeros, subnormals, Inf and NaN (e8 = 0 or 255) fall
 //              back to the conversion so that they keep their IEEE meaning.
 // x*x is exact in binary64 (16 significant bits), so fma(x, x, acc) is ONE rounding of acc + g^2.
-// non-zero iff the high half of w has exponent field 0 or 255: (field + 1) mod 256 < 2
-__device__ __forceinline__ uint32_t hi_special(uint32_t w)
+// non-zero iff the high half of ANY of the four words has exponent field E = 0 or 255.  (w + 0x00800000) adds one to
+// E (carry into the sign bit, nothing below bit 23 moves), so bits 30..24 of the sum — the low 7 bits of its top
+// byte — are all zero iff E + 1 is 0 or 1 mod 256.  The four top bytes are gathered into one word (PRMT) and tested
+// with the zero-byte trick: 11 integer operations per 8-element group instead of a compare per word.
+__device__ __forceinline__ uint32_t any_hi_special(const uint4 &w)
 {
-    return (((w & 0x7F800000u) + 0x00800000u) & 0x7F000000u) == 0u;
+    const uint32_t c = 0x00800000u;
+    const uint32_t t01 = __byte_perm(w.x + c, w.y + c, 0x0073);   // byte 0 = top byte of x, byte 1 = top byte of y
+    const uint32_t t23 = __byte_perm(w.z + c, w.w + c, 0x0073);
+    const uint32_t u = __byte_perm(t01, t23, 0x5410) & 0x7F7F7F7Fu;
+    return (u - 0x01010101u) & ~u & 0x80808080u;                    // some byte of u is zero
 }
 __device__ __forceinline__ double widen_hi_int(uint32_t w)
 {
-    return __hiloint2double((int)(((w >> 3) & 0x0FFFE000u) + 0x38000000u), 0);
+    // high word = ((w & 0x7FFF0000) >> 3) + 0x38000000, the shift and the add as ONE multiply-add-high by 2^29
+    uint32_t hi;
+    asm("mad.hi.u32 %0, %1, 0x20000000, 0x38000000;" : "=r"(hi) : "r"(w & 0x7FFF0000u));
+    return __hiloint2double((int)hi, 0);
 }
 __device__ __forceinline__ void sq_acc4(double &a0, double &a1, const uint4 &w)
 {
@@ -445,7 +455,7 @@ __device__ __forceinline__ void sq_acc4(double &a0, double &a1, const uint4 &w)
         a0 = fma(lo, lo, a0);
     }
     // one branch per 8-element group keeps the conversions of the fallback off the XU pipe in the common case
-    if ((hi_special(w.x) | hi_special(w.y) | hi_special(w.z) | hi_special(w.w)) == 0u) {
+    if (any_hi_special(w) == 0u) {
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             const double hi = widen_hi_int(ww[k]);
