@@ -914,8 +914,11 @@ class Rig:
         self.gemm_setup()
         it_ms = {k: [] for k in arms}
         hp_ms = {k: [] for k in arms}
-        for _ in range(reps):
-            for arm in arms:
+        for rep in range(reps):
+            # the arms alternate AND swap their order from one repetition to the next (off, on | on, off | ...), so
+            # that a drift of the GEMM rate over the leg (the board warming up to its power limit) does not always
+            # land on the same arm
+            for arm in (arms if rep % 2 == 0 else tuple(reversed(arms))):
                 evs, kevs = [], []
                 for it in range(warm + iters):
                     e0 = torch.cuda.Event(enable_timing=True)
@@ -1166,7 +1169,7 @@ def measure_config(args, key, link, clk, rank, world, local_rank, K, Wm, peak, h
             G = args.gemms if (args.gemms > 0 and pow2) else rig.gemms_for(flush_ms, factor, pow2)
             iters = rig.iters_for(G)
             with clk.leg(f"{tag}.overlap.{wname}.eager"):
-                o = rig.overlap(G, iters)
+                o = rig.overlap(G, max(4, (iters + 1) // 2), reps=2)
             w = {"rule": ("G = smallest power of two with T_c >= 4 x T_D2H" if pow2 else "G = round(1.25 x T_D2H / T_gemm)")
                  if args.gemms <= 0 or not pow2 else "G given", "gemms_per_iter": G,
                  "compute_window_ms": G * rig.gemm_ms, "flush_ms": flush_ms, "iter_ms_off": o["iter_ms_off"],
