@@ -971,14 +971,14 @@ class Rig:
         self.gemm_setup()
         hp = self.wl.hyper
         cap = torch.cuda.Stream(device=self.device)
-        res = {}
         L = {1: 2, 2: 2, 3: 6, 4: 4}[self.depth] if self.source_name == "staged" else 2
         nrep = max(3, (iters + L - 1) // L)
-        for arm in arms:
+        with torch.cuda.stream(cap):
+            self.gemm_window(2)                                          # cuBLAS handle / workspace of this stream exist before capture
+        torch.cuda.synchronize()
+        graphs = {}
+        for arm in arms:                                                 # capture every arm once; the handles differ, the live memory is shared
             h = self.off_shard() if arm == "off" else self.s.h
-            with torch.cuda.stream(cap):
-                self.gemm_window(2)                                      # cuBLAS handle / workspace of this stream exist before capture
-            torch.cuda.synchronize()
             B.phx_graph_begin(h, hp.lr, hp.beta1, hp.beta2, hp.eps, hp.wd, cap)
             B.phx_graph_step_and_snapshot(h, self.grads[1], cap)         # a snapshot for the first captured flush
             torch.cuda.synchronize()
@@ -992,17 +992,26 @@ class Rig:
                     B.phx_graph_step_and_snapshot(h, self.grads[i & 1], cap)   # a2 joins the flush back
                 if arm == "on":
                     cap.wait_stream(self.side)
+            graphs[arm] = (h, graph)
+        # timed blocks in swapped order (off, on | on, off) like the eager arms, one warm-up replay per block
+        order = list(arms) + list(reversed(arms)) if len(arms) > 1 else list(arms)
+        per_block = max(2, (nrep + 1) // 2) if len(arms) > 1 else nrep
+        ms = {arm: [] for arm in arms}
+        for arm in order:
+            graph = graphs[arm][1]
             times = []
             with torch.cuda.stream(cap):                                 # replay() launches on the current stream
-                for r in range(warm + nrep):
+                for r in range(warm + per_block):
                     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                     e0.record(cap)
                     graph.replay()
                     e1.record(cap)
                     times.append((e0, e1))
             torch.cuda.synchronize()
-            ms = [a.elapsed_time(b) / L for a, b in times[warm:]]
-            res[arm] = trimmed_mean(ms)
+            ms[arm] += [a.elapsed_time(b) / L for a, b in times[warm:]]
+        res = {arm: trimmed_mean(v) for arm, v in ms.items()}
+        for arm in arms:
+            h, graph = graphs[arm]
             last = B.phx_graph_end(h)
             if arm == "on":
                 self.step = last
@@ -1011,6 +1020,7 @@ class Rig:
             else:
                 self.off_step = last
             del graph
+        nrep = per_block * (2 if len(arms) > 1 else 1)
         out = {"gemms_per_iter": G, "compute_window_ms": G * self.gemm_ms, "launch": f"cuda graph ({L} iterations per graph)",
                "iters_per_arm": L * nrep}
         for arm in arms:
