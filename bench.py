@@ -1266,12 +1266,13 @@ def measure_c5_grid(args, link, clk, replica, flush_ref):
     default line (the full 7 x 4 x 2 grid is `--mode sweep`)."""
     import torch
     cells = []
-    base = base_g = None
+    base = base_g = G = None
     for sync, depth, chunk in [("strict", 2, 4), ("strict", 2, 16), ("strict", 2, 64), ("strict", 2, 256),
                                ("strict", 1, 8), ("relaxed", 4, 8), ("relaxed", 4, 64), ("relaxed", 3, 256)]:
         rig = Rig(args, "c5", depth=depth, chunk_mib=chunk, sync=sync, replica=replica, host_grads=False)
         rig.gemm_setup()
-        G = max(1, int(round(1.25 * flush_ref / rig.gemm_ms)))
+        if G is None:       # ONE window for the baseline and every cell (the per-rig GEMM timing moves by a few per cent)
+            G = max(1, int(round(1.25 * flush_ref / rig.gemm_ms)))
         iters = max(8, min(16, rig.iters_for(G)))
         if base is None:
             base = rig.overlap(G, iters, arms=("off",))["iter_ms_off"]
