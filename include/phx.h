@@ -69,7 +69,8 @@ enum {
     PHX_ERR_SNAPSHOT_DISABLED = -11,  /* flush/restore asked of a shard created with snapshots off */
     PHX_ERR_NOMEM = -12,
     PHX_ERR_PARAMS_NOT_READY = -13,   /* full-rank-state flush before phx_params_ready for that step  */
-    PHX_ERR_GRAPH_MODE = -14          /* eager call between phx_graph_begin/end, or a phx_graph_* call outside them */
+    PHX_ERR_GRAPH_MODE = -14,         /* eager call between phx_graph_begin/end, or a phx_graph_* call outside them */
+    PHX_ERR_TOO_LARGE = -15           /* phx_grad_sumsq_no_alloc: more elements than its built-in scratch serves */
 };
 
 /* ---- types ----------------------------------------------------------------------------- */
@@ -418,6 +419,43 @@ PHX_API int phx_params_guard(phx_shard_t *s, void *stream);
  * With count = 1 and d_partials = the rank's own S_r the coefficient is bit-identical to the local a1. */
 PHX_API int phx_grad_sumsq_async(phx_shard_t *s, const void *d_grads, double *d_out, void *stream);
 PHX_API int phx_set_clip_partials(phx_shard_t *s, const double *d_partials, uint32_t count);
+
+/* ---- a1 for callers that must not allocate device memory -------------------------------------------
+ * phx_grad_sumsq_no_alloc: the same S_r = sum_i g_i^2 as phx_grad_sumsq_async (same kernels, same fixed fp64
+ * tree, hence the same bits on the same gradients), but without a handle and without a single allocation:
+ * it calls neither cudaMalloc nor cudaFree nor any routine that does.
+ *
+ * Who needs it.  phx_grad_sumsq_async wants a bound shard, and phx_shard_bind gets the reduction scratch from
+ * cudaMalloc.  That is no option for (i) a trainer whose framework allocator already holds all of the GPU's
+ * memory — an allocation made beside it fails, or robs the framework and surfaces as its out-of-memory error
+ * later; (ii) code on the iteration's critical path — cudaMalloc and cudaFree synchronise the device, so one
+ * call from a monitoring thread stalls the very flush/compute overlap this library exists for (PAPER.md:128,
+ * 143); (iii) the fault-handling side, which wants a rank's gradient norm at the moment the
+ * allocator is least to be relied on.  For these callers the scratch is built into the library image.
+ *
+ * The limit.  The scratch is one statically declared device array of 65536 doubles = 512 KiB; EVERY GPU on
+ * which the process uses libphx.so holds it from module load until the process exits, whether or not this call is
+ * ever made.  It serves n_elems <= PHX_NO_ALLOC_MAX_ELEMS = 2^30 elements (one partial per 16384); a larger
+ * n_elems returns PHX_ERR_TOO_LARGE and enqueues nothing.
+ *
+ * Arguments.  d_grads: device, read-only, 256-byte aligned; bf16[n_elems] if grads_fp32 == 0, float[n_elems]
+ * if grads_fp32 == 1 (any other value: PHX_ERR_INVALID_ARG).  n_elems: > 0 and a multiple of 8 (a shard's
+ * n_padded always is); padding lanes must be zero.  d_out: device double, 8-byte aligned, caller-owned, written in
+ * `stream` order.  stream: cudaStream_t; the call only enqueues two kernels.  cuda_error: optional (may be NULL);
+ * receives the cudaError_t when the result is PHX_ERR_CUDA, else 0.  Works on the CURRENT device, which must be
+ * compute capability 10.x (PHX_ERR_UNSUPPORTED_DEVICE otherwise) and the one d_grads and d_out live on.
+ *
+ * Sharing.  There is ONE array per GPU for all callers and threads.  It keeps the previous call's contents; no
+ * clearing is needed, because each call first overwrites exactly the entries it then reads.  Calls whose kernels
+ * can overlap on one GPU (unordered streams) RACE on the array and return garbage: keep them on one stream or
+ * order them with events.  The handle-based calls use their own scratch and are unaffected.
+ *
+ * First call.  The first call on each device looks up the array's device address (and thereby makes the driver
+ * load the library's module on that device); it takes a process-wide mutex and is slower than the rest.  Make it
+ * once per device BEFORE any stream capture begins. */
+#define PHX_NO_ALLOC_MAX_ELEMS (1ull << 30)
+PHX_API int phx_grad_sumsq_no_alloc(const void *d_grads, int grads_fp32, uint64_t n_elems, double *d_out,
+                                    void *stream, int *cuda_error);
 
 /* ---- SURVEY.md §8(f4), second half: the gradient producer's epilogue -------------------------------
  * "single-pass fusion of the sum-of-squares with the previous step's epilogue".  The

@@ -32,6 +32,8 @@ PHX_ERR_SNAPSHOT_DISABLED = -11
 PHX_ERR_NOMEM = -12
 PHX_ERR_PARAMS_NOT_READY = -13
 PHX_ERR_GRAPH_MODE = -14
+PHX_ERR_TOO_LARGE = -15
+PHX_NO_ALLOC_MAX_ELEMS = 1 << 30
 
 PHX_SYNC_STRICT, PHX_SYNC_RELAXED = 0, 1
 PHX_RESTORE_COPY_ENGINE, PHX_RESTORE_BULK_KERNEL = 0, 1
@@ -115,6 +117,8 @@ PROTOTYPES = {
     "phx_last_step": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_last_clip": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_double)]),
     "phx_grad_sumsq_async": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "phx_grad_sumsq_no_alloc": (C.c_int, [C.c_void_p, C.c_int, C.c_uint64, C.c_void_p, C.c_void_p,
+                                          C.POINTER(C.c_int)]),
     "phx_set_clip_partials": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint32]),
     "phx_kernel_launches": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64)]),
     "phx_dropped_snapshots": (C.c_int, [C.c_void_p, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]),
@@ -310,6 +314,18 @@ def phx_last_clip(h: int) -> Tuple[float, float]:
 def phx_grad_sumsq_async(h: int, d_grads, d_out, stream=None) -> None:
     """this rank's sum of squared gradients into a caller-owned device double."""
     _ck(lib().phx_grad_sumsq_async(h, _ptr(d_grads), _ptr(d_out), _ptr(stream)), "phx_grad_sumsq_async", h)
+
+
+def phx_grad_sumsq_no_alloc(d_grads, grads_fp32: bool, n_elems: int, d_out, stream=None) -> None:
+    """Sum of squared gradients into a caller-owned device double, for callers that must not allocate device
+    memory (no handle, no cudaMalloc: the reduction scratch is a 512 KiB array built into libphx.so).  Same bits as
+    phx_grad_sumsq_async.  n_elems <= PHX_NO_ALLOC_MAX_ELEMS (PHX_ERR_TOO_LARGE beyond).  One scratch per GPU: do not
+    let two calls overlap on the device; make the first call on a device before any stream capture (phx.h)."""
+    err = C.c_int(0)
+    rc = lib().phx_grad_sumsq_no_alloc(_ptr(d_grads), 1 if grads_fp32 else 0, int(n_elems), _ptr(d_out), _ptr(stream),
+                                       C.byref(err))
+    if rc != PHX_OK:
+        raise PhxError(rc, "phx_grad_sumsq_no_alloc", err.value)
 
 
 def phx_set_clip_partials(h: int, d_partials, count: int) -> None:

@@ -18,7 +18,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libphx.so")
-SOURCES = [os.path.join(CSRC, f) for f in ("phx_api.cu", "phx_kernels.cu")]
+SOURCES = [os.path.join(CSRC, f) for f in ("phx_api.cu", "phx_kernels.cu", "phx_no_alloc.cu")]
 MAP = os.path.join(CSRC, "phx.map")
 DEPS = SOURCES + [os.path.join(CSRC, "phx_kernels.cuh"), MAP,
                   os.path.join(os.path.dirname(HERE), "include", "phx.h")]

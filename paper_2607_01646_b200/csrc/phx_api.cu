@@ -413,6 +413,7 @@ const char *phx_strerror(int err)
     case PHX_ERR_NOMEM: return "out of memory";
     case PHX_ERR_PARAMS_NOT_READY: return "model-parameter buffer not declared ready for this step";
     case PHX_ERR_GRAPH_MODE: return "call not available between phx_graph_begin and phx_graph_end (or outside them)";
+    case PHX_ERR_TOO_LARGE: return "more elements than the built-in scratch of the no-alloc entry point serves";
     default: return "unknown error";
     }
 }
