@@ -26,6 +26,11 @@
  *     is by library-owned events.  One host thread uses a handle at a time.
  *   - There is deliberately no fallback: a device that is not compute capability 10.x gives
  *     PHX_ERR_UNSUPPORTED_DEVICE at phx_shard_bind.
+ *   - A shard belongs to the device that is current at phx_shard_bind.  Bind checks with
+ *     cudaPointerGetAttributes that every d_* pointer is device (or managed) memory of THAT device
+ *     (PHX_ERR_INVALID_ARG otherwise: a host pointer would fault asynchronously, far from the call) and that
+ *     h_replica is pinned, mapped host memory.  The hot calls (step, flush, restore, their graph forms) return
+ *     PHX_ERR_WRONG_DEVICE when another device is current.
  *
  * Memory layout (all little-endian, unit-stride)
  *   live state   d_p, d_m, d_v : float[n_padded]; d_p_bf16 : bf16[n_padded];
@@ -70,7 +75,8 @@ enum {
     PHX_ERR_NOMEM = -12,
     PHX_ERR_PARAMS_NOT_READY = -13,   /* full-rank-state flush before phx_params_ready for that step  */
     PHX_ERR_GRAPH_MODE = -14,         /* eager call between phx_graph_begin/end, or a phx_graph_* call outside them */
-    PHX_ERR_TOO_LARGE = -15           /* phx_grad_sumsq_no_alloc: more elements than its built-in scratch serves */
+    PHX_ERR_TOO_LARGE = -15,          /* phx_grad_sumsq_no_alloc: more elements than its built-in scratch serves */
+    PHX_ERR_WRONG_DEVICE = -16        /* the current CUDA device is not the one the shard was bound on         */
 };
 
 /* ---- types ----------------------------------------------------------------------------- */
@@ -194,7 +200,9 @@ PHX_API int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, v
 /* Declare the bound p, m, v to be the state after optimizer step `step` (0 at initialisation)
  * and regenerate d_p_bf16 = RNE_bf16(p) on `stream`. */
 PHX_API int phx_shard_set_state(phx_shard_t *s, uint64_t step, void *stream);
-/* Opaque blob (<= 128 bytes) copied into the header of every later snapshot. */
+/* Opaque blob (<= 128 bytes) copied into the header of every later snapshot.  PHX_ERR_GRAPH_MODE between
+ * phx_graph_begin and phx_graph_end (the envelope template then lives on the device): use
+ * phx_graph_set_user_metadata there. */
 PHX_API int phx_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len);
 
 /* ---- a1+a2+a3: fused AdamW step + snapshot -------------------------------------------------
@@ -496,6 +504,11 @@ PHX_API int phx_grads_finalize_async(phx_shard_t *s, const float *d_main_grads_f
  *        pending snapshot carries over in both directions.
  *   phx_graph_set_hyper(...)                                 stream-ordered update of the hyperparameters (learning-
  *        rate schedules) between replays; not captured itself.
+ *        PHX_ERR_INVALID_ARG if `stream` is being captured (its source is host memory of the call).
+ *   phx_graph_set_user_metadata(s, blob, len, stream)        the same for the caller blob of the envelope (RNG states,
+ *        PAPER.md:145): stream-ordered update of the device-resident envelope template; every snapshot whose
+ *        prologue runs after it on `stream` carries the new blob (and so do the eager calls after
+ *        phx_graph_end).  Call it between replays; not capturable (PHX_ERR_INVALID_ARG on a capturing stream).
  *   phx_graph_step_and_snapshot(s, d_grads, stream)          a1 (if configured) + a2 + prologue + a3, capturable.  The
  *        staging slot (issue index mod depth) and the host slot parity are fixed when the call is CAPTURED:
  *        a captured sequence must span a multiple of lcm(depth, 2) steps and be replayed from the step
@@ -508,9 +521,11 @@ PHX_API int phx_grads_finalize_async(phx_shard_t *s, const float *d_main_grads_f
  *   phx_graph_end(s, &last_step)                             mode switch (cudaDeviceSynchronize): reads the device step
  *        counter, rebuilds the commit bookkeeping from the self-describing host slots; afterwards the eager
  *        calls continue at last_step + 1 and a still-staged newest snapshot can be flushed eagerly.
- * Eager calls (step, flush, restore) return PHX_ERR_GRAPH_MODE in between, phx_graph_* outside. */
+ * Eager calls (step, flush, restore, phx_set_user_metadata, phx_publish_params_async, phx_last_clip) return
+ * PHX_ERR_GRAPH_MODE in between, phx_graph_* outside. */
 PHX_API int phx_graph_begin(phx_shard_t *s, float lr, float beta1, float beta2, float eps, float wd, void *stream);
 PHX_API int phx_graph_set_hyper(phx_shard_t *s, float lr, float beta1, float beta2, float eps, float wd, void *stream);
+PHX_API int phx_graph_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len, void *stream);
 PHX_API int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *stream);
 PHX_API int phx_graph_flush_async(phx_shard_t *s, void *side_stream);
 /* §8(f1) in the graph form: replication of the last issued step's snapshot to the k bound ring peers, capturable

@@ -33,6 +33,7 @@ PHX_ERR_NOMEM = -12
 PHX_ERR_PARAMS_NOT_READY = -13
 PHX_ERR_GRAPH_MODE = -14
 PHX_ERR_TOO_LARGE = -15
+PHX_ERR_WRONG_DEVICE = -16
 PHX_NO_ALLOC_MAX_ELEMS = 1 << 30
 
 PHX_SYNC_STRICT, PHX_SYNC_RELAXED = 0, 1
@@ -129,6 +130,7 @@ PROTOTYPES = {
     "phx_grads_finalize_async": (C.c_int, [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]),
     "phx_graph_begin": (C.c_int, [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float, C.c_void_p]),
     "phx_graph_set_hyper": (C.c_int, [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float, C.c_void_p]),
+    "phx_graph_set_user_metadata": (C.c_int, [C.c_void_p, C.c_char_p, C.c_uint32, C.c_void_p]),
     "phx_graph_step_and_snapshot": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "phx_graph_flush_async": (C.c_int, [C.c_void_p, C.c_void_p]),
     "phx_graph_flush_peers_async": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -377,6 +379,10 @@ def phx_graph_begin(h: int, lr: float, beta1: float, beta2: float, eps: float, w
 
 def phx_graph_set_hyper(h: int, lr: float, beta1: float, beta2: float, eps: float, wd: float, stream=None) -> None:
     _ck(lib().phx_graph_set_hyper(h, lr, beta1, beta2, eps, wd, _ptr(stream)), "phx_graph_set_hyper", h)
+
+
+def phx_graph_set_user_metadata(h: int, blob: bytes, stream=None) -> None:
+    _ck(lib().phx_graph_set_user_metadata(h, blob, len(blob), _ptr(stream)), "phx_graph_set_user_metadata", h)
 
 
 def phx_graph_step_and_snapshot(h: int, d_grads, stream=None) -> None:

@@ -96,6 +96,7 @@ struct phx_shard {
     uint8_t *d_scratch = nullptr;
     double *d_partials = nullptr;  // 2 x sumsq_partials_count(n_padded): [a1 / phx_grad_sumsq_async | producer epilogue]
     int sm_count = 148;
+    int device = -1;  // ordinal of the device that was current at phx_shard_bind; the hot calls check it
     // decay groups: class per 2048-element tile and the offsets where the flag toggles
     std::vector<uint8_t> decay_cls;
     std::vector<uint64_t> decay_bnd;
@@ -278,6 +279,27 @@ void build_decay_groups(phx_shard *s)
     }
 }
 bool direct_mode(const phx_shard *s) { return s->cfg.snapshot_source == PHX_SNAPSHOT_DIRECT; }
+// SURVEY §8(b) "Ownership": a d_* pointer must be device (or managed) memory of the device the shard is bound on.
+// A host pointer would be accepted by the launch and fault asynchronously, far from the call that caused it.
+bool device_memory_on(const void *p, int dev)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    return (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged) && at.device == dev;
+}
+
+// The handle's events, scratch and function attributes belong to the device it was bound on; every later call
+// assumes that device is current.  Checked in the hot calls (one thread-local read).
+int check_device(phx_shard *s)
+{
+    int dev = -1;
+    PHX_CK(cudaGetDevice(&dev));
+    return dev == s->device ? PHX_OK : PHX_ERR_WRONG_DEVICE;
+}
+
 // number of ring positions the bookkeeping cycles through (direct mode: two header slots)
 uint32_t ring_depth(const phx_shard *s) { return direct_mode(s) ? 2u : s->cfg.staging_depth; }
 
@@ -413,6 +435,7 @@ const char *phx_strerror(int err)
     case PHX_ERR_NOMEM: return "out of memory";
     case PHX_ERR_PARAMS_NOT_READY: return "model-parameter buffer not declared ready for this step";
     case PHX_ERR_GRAPH_MODE: return "call not available between phx_graph_begin and phx_graph_end (or outside them)";
+    case PHX_ERR_WRONG_DEVICE: return "the current CUDA device is not the one the shard was bound on";
     case PHX_ERR_TOO_LARGE: return "more elements than the built-in scratch of the no-alloc entry point serves";
     default: return "unknown error";
     }
@@ -572,6 +595,10 @@ int phx_shard_bind(phx_shard_t *s, float *d_p, float *d_m, float *d_v, void *d_p
     PHX_CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
     if (major != 10) return PHX_ERR_UNSUPPORTED_DEVICE;  // sm_100a only; deliberately no fallback
     PHX_CK(cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    for (const void *p : {static_cast<const void *>(d_p), static_cast<const void *>(d_m), static_cast<const void *>(d_v),
+                          static_cast<const void *>(d_p_bf16), static_cast<const void *>(d_staging)})
+        if (p != nullptr && !device_memory_on(p, dev)) return PHX_ERR_INVALID_ARG;
+    s->device = dev;
 
     if (snapshots_on(s) && h_replica) {
         void *dview = nullptr;
@@ -645,6 +672,8 @@ int phx_shard_set_state(phx_shard_t *s, uint64_t step, void *stream)
 int phx_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len)
 {
     if (!s || len > 128 || (len && !blob)) return PHX_ERR_INVALID_ARG;
+    // the graph form keeps the envelope template on the device: phx_graph_set_user_metadata updates it in stream order
+    if (s->graph) return PHX_ERR_GRAPH_MODE;
     std::memset(s->user, 0, sizeof(s->user));
     if (len) std::memcpy(s->user, blob, len);
     s->user_len = len;
@@ -736,6 +765,7 @@ int phx_step_and_snapshot(phx_shard_t *s, const void *d_grads, float lr, float b
     if (!s || !d_grads) return PHX_ERR_INVALID_ARG;
     if (!s->bound) return PHX_ERR_NOT_BOUND;
     if (s->graph) return PHX_ERR_GRAPH_MODE;
+    if (int rcd = check_device(s)) return rcd;
     if (!aligned256(d_grads)) return PHX_ERR_ALIGNMENT;
     if (step != s->last_step + 1) return PHX_ERR_STEP_ORDER;  // I4 step atomicity
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -809,6 +839,7 @@ int phx_snapshot_flush_async(phx_shard_t *s, void *side_stream)
     if (!s->bound || (snapshots_on(s) && !s->h_replica)) return PHX_ERR_NOT_BOUND;
     if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
     if (s->graph) return PHX_ERR_GRAPH_MODE;
+    if (int rcd = check_device(s)) return rcd;
     if (s->pending_slot < 0) return PHX_ERR_NO_FLUSH_PENDING;
     cudaStream_t st = static_cast<cudaStream_t>(side_stream);
     const int slot = s->pending_slot;
@@ -994,6 +1025,7 @@ int restore_own(phx_shard *s, void *stream, uint64_t *restored_step, bool two_ph
     if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
     if (s->graph) return PHX_ERR_GRAPH_MODE;
     if (full_payload(s) && !s->d_W) return PHX_ERR_NOT_BOUND;
+    if (int rcd = check_device(s)) return rcd;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int rc = settle_host_slots(s, false);
     if (rc != PHX_OK) return rc;
@@ -1286,6 +1318,9 @@ int phx_publish_params_async(phx_shard_t *s, void *stream)
 {
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound || s->n_pub == 0) return PHX_ERR_NOT_BOUND;
+    // ev_last_step / ev_pub are the EAGER step's events; the graph form neither records the first nor waits on the
+    // second, so a publication there would wait on a stale event and race the step
+    if (s->graph) return PHX_ERR_GRAPH_MODE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const uint64_t bytes = s->info.n_padded * model_elem_bytes(s);
     const uint8_t *src = fp32_mode(s) ? reinterpret_cast<const uint8_t *>(s->d_p) : static_cast<const uint8_t *>(s->d_p16);
@@ -1386,6 +1421,7 @@ int phx_last_clip(phx_shard_t *s, float *coef, double *sumsq)
 {
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (s->graph) return PHX_ERR_GRAPH_MODE;  // it would synchronise on the last EAGER step's event, not on the replay
     float c = 1.0f;
     double q = 0.0;
     if (s->clip_valid) {
@@ -1513,10 +1549,36 @@ int phx_graph_set_hyper(phx_shard_t *s, float lr, float beta1, float beta2, floa
     if (!s) return PHX_ERR_INVALID_ARG;
     if (!s->bound) return PHX_ERR_NOT_BOUND;
     if (!s->graph) return PHX_ERR_GRAPH_MODE;
+    // Not capturable: the source is a host stack array.  Outside a capture cudaMemcpyAsync stages a pageable source
+    // before it returns; a captured memcpy node would keep the dangling pointer and read it at every replay.
+    if (capture_id(static_cast<cudaStream_t>(stream)) != 0) return PHX_ERR_INVALID_ARG;
     // five floats at the front of the block's hyperparameter area, stream-ordered; the step counter stays
     const float h[5] = {lr, beta1, beta2, eps, wd};
     PHX_CK(cudaMemcpyAsync(reinterpret_cast<uint8_t *>(step_block(s)) + offsetof(phx::StepBlock, lr), h, sizeof(h),
                            cudaMemcpyHostToDevice, static_cast<cudaStream_t>(stream)));
+    return PHX_OK;
+}
+
+// The caller blob of the envelope (RNG states) changes every iteration; in the graph form the envelope
+// template lives in the device step block, so the update is a stream-ordered copy into it (user_len ‖ payload ‖
+// user[128] are contiguous in phx_snapshot_header_t; the prologue rewrites the payload word per slot anyway).
+int phx_graph_set_user_metadata(phx_shard_t *s, const void *blob, uint32_t len, void *stream)
+{
+    if (!s || len > 128 || (len && !blob)) return PHX_ERR_INVALID_ARG;
+    if (!s->bound) return PHX_ERR_NOT_BOUND;
+    if (!s->graph) return PHX_ERR_GRAPH_MODE;
+    if (capture_id(static_cast<cudaStream_t>(stream)) != 0) return PHX_ERR_INVALID_ARG;  // pageable source, see set_hyper
+    std::memset(s->user, 0, sizeof(s->user));
+    if (len) std::memcpy(s->user, blob, len);
+    s->user_len = len;  // the eager calls after phx_graph_end carry the same blob on
+    phx_snapshot_header_t tmpl;
+    build_header(s, 0, true, &tmpl);
+    constexpr size_t off = offsetof(phx_snapshot_header_t, user_len);
+    constexpr size_t bytes = offsetof(phx_snapshot_header_t, user) + sizeof(tmpl.user) - off;
+    static_assert(bytes == 136, "user_len, payload and user[] are contiguous");
+    PHX_CK(cudaMemcpyAsync(reinterpret_cast<uint8_t *>(step_block(s)) + offsetof(phx::StepBlock, hdr_tmpl) + off,
+                           reinterpret_cast<const uint8_t *>(&tmpl) + off, bytes, cudaMemcpyHostToDevice,
+                           static_cast<cudaStream_t>(stream)));
     return PHX_OK;
 }
 
@@ -1525,6 +1587,7 @@ int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *strea
     if (!s || !d_grads) return PHX_ERR_INVALID_ARG;
     if (!s->bound) return PHX_ERR_NOT_BOUND;
     if (!s->graph) return PHX_ERR_GRAPH_MODE;
+    if (int rcd = check_device(s)) return rcd;
     if (!aligned256(d_grads)) return PHX_ERR_ALIGNMENT;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const bool snap = snapshots_on(s);
@@ -1561,8 +1624,13 @@ int phx_graph_step_and_snapshot(phx_shard_t *s, const void *d_grads, void *strea
         shdr_full = s->d_scratch + kScrHdrFull + (size_t)slot * kHeaderBytes;
         full_word = full_payload_word(s);
     }
-    PHX_CK(phx::launch_step_prologue(step_block(s), shdr, shdr_full, full_word, snap ? (uint32_t)slot : 0u,
-                                     snap ? depth : 0u, st));
+    // What a captured call bakes in: the staging slot (step mod depth) AND the host / peer ping-pong slot (step mod 2,
+    // phx_graph_flush_async).  The device check therefore runs modulo lcm(depth, 2): with depth 1 or 3 a replay can land
+    // on the right staging slot and still on the wrong host slot (it would invalidate and rewrite the newest committed
+    // replica), which the staging-slot test alone let through.
+    const uint32_t period = (depth & 1u) ? 2u * depth : depth;
+    PHX_CK(phx::launch_step_prologue(step_block(s), shdr, shdr_full, full_word, snap ? (uint32_t)(step % period) : 0u,
+                                     snap ? period : 0u, st));
     PHX_CK(phx::launch_step(a, snap && !direct_mode(s), step_mode(s), true, st));
     s->launches += 1 + (s->info.n_padded ? 1 : 0);
     if (snap) {
@@ -1585,6 +1653,7 @@ int phx_graph_flush_async(phx_shard_t *s, void *side_stream)
     if (!s->bound || (snapshots_on(s) && !s->h_replica)) return PHX_ERR_NOT_BOUND;
     if (!snapshots_on(s)) return PHX_ERR_SNAPSHOT_DISABLED;
     if (!s->graph) return PHX_ERR_GRAPH_MODE;
+    if (int rcd = check_device(s)) return rcd;
     if (s->g_pending_slot < 0) return PHX_ERR_NO_FLUSH_PENDING;
     cudaStream_t st = static_cast<cudaStream_t>(side_stream);
     const int slot = s->g_pending_slot;
@@ -1652,8 +1721,11 @@ int phx_graph_end(phx_shard_t *s, uint64_t *last_step)
     // the eager bookkeeping restarts from what is self-describing: the envelopes in the host slots
     for (int k = 0; k < kMaxDepth; ++k) s->flush_valid[k] = s->pflush_valid[k] = false;
     s->wflush_valid = false;  // nothing is reading W any more (device synchronised above)
-    s->params_ready = s->g_params_ready && s->g_params_step == blk.step;
-    s->params_ready_step = s->g_params_step;
+    // g_params_step counts ISSUED calls (the host mirror), blk.step is the device counter, which runs ahead of it
+    // after any replay: a declaration made for the last issued step holds for the step the device finished last
+    // (in a replayed graph the declaration is an edge behind that step's kernel), so it carries over.
+    s->params_ready = s->g_params_ready && s->g_params_step == s->g_issue;
+    s->params_ready_step = s->params_ready ? blk.step : 0;
     s->last_flush_slot = s->last_pflush_slot = -1;
     s->pending_slot = s->pending_peer_slot = -1;
     uint64_t newest = 0;

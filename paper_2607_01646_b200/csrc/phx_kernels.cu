@@ -334,8 +334,9 @@ __device__ __forceinline__ uint64_t fnv1a64_dev(const uint8_t *b, int len)
 }
 
 // blk->step += 1; scalars of that step -> blk->sc; envelope of that step (template + step + hash) -> shdr
-// and, §8(f4), the full-rank-state flavour -> shdr_full.  expect_slot/expect_depth: the staging slot the
-// host baked into the captured kernel node; a replay whose device step does not land on it is counted in
+// and, §8(f4), the full-rank-state flavour -> shdr_full.  expect_slot/expect_depth: the step index the host
+// issued this call at, modulo expect_depth = lcm(staging depth, 2) — which fixes both the staging slot and the host
+// ping-pong slot baked into the captured nodes; a replay whose device step does not land on it is counted in
 // blk->misaligned (phx_graph_end reports it) instead of silently writing the wrong slot.
 __global__ void __launch_bounds__(32) k_step_prologue(StepBlock *blk, uint8_t *shdr, uint8_t *shdr_full,
                                                       uint32_t full_payload, uint32_t expect_slot, uint32_t expect_depth)
@@ -770,12 +771,10 @@ cudaError_t launch_restore_bulk(const RestorePlanes &pl, void *p16, uint64_t n_p
     if (n_padded == 0) return cudaSuccess;
     if (pl.n < 1 || pl.n > 3) return cudaErrorInvalidValue;
     const size_t smem = (size_t)kStages * 3 * kTile * sizeof(float);  // 96 KB
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_restore_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    // function attributes are per DEVICE: set it on every launch (a cheap host-side call) rather than behind a
+    // process-wide flag, which left the second GPU of a one-process-many-GPUs caller without the opt-in
+    cudaError_t e = cudaFuncSetAttribute(k_restore_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     const uint64_t ntiles = (n_padded + kTile - 1) / kTile;
     uint64_t grid = max_ctas > 0 ? (uint64_t)max_ctas : 1;
     if (grid > ntiles) grid = ntiles;

@@ -153,6 +153,91 @@ def test_misaligned_replay_is_reported():
     s.close()
 
 
+@pytest.mark.parametrize("depth,captured,replays,ok", [(1, 1, 2, False), (3, 3, 2, False), (1, 2, 3, True),
+                                                       (3, 6, 2, True), (2, 2, 3, True)])
+def test_replay_alignment_covers_the_host_ping_pong_parity(depth, captured, replays, ok):
+    """a captured sequence of `depth` steps keeps the STAGING slot aligned on every replay, but with an odd
+    depth it flips the host ping-pong parity baked into the captured flush (step & 1): every second replay would
+    invalidate and rewrite the newest committed host slot.  phx.h asks for a multiple of lcm(depth, 2) steps; the
+    device check must report anything else (PHX_ERR_STEP_ORDER at phx_graph_end)."""
+    wl = W.tiny_workload([8192], dp_size=1)
+    s, o, gdev, _ = make_pair(wl, steps=6, staging_depth=depth)
+    cap, side = torch.cuda.Stream(device=DEV), torch.cuda.Stream(device=DEV)
+    s.graph_begin(stream=cap)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=cap):
+        for i in range(captured):
+            s.graph_step(gdev[i], stream=cap)
+            side.wait_stream(cap)
+            s.graph_flush(side)
+            cap.wait_stream(side)
+    for _ in range(replays):
+        graph.replay()
+    torch.cuda.synchronize()
+    if ok:
+        assert s.graph_end() == captured * replays
+    else:
+        with pytest.raises(B.PhxError) as e:
+            s.graph_end()
+        assert e.value.code == B.PHX_ERR_STEP_ORDER
+        assert B.phx_last_step(s.h) == captured * replays
+    s.close()
+
+
+def test_user_metadata_changed_between_replays_reaches_the_committed_envelope():
+    """the caller blob (RNG states) changes every iteration, but the graph form's envelope
+    template was frozen at phx_graph_begin, so every replayed snapshot committed the blob of begin and a restore
+    handed back stale RNG state.  phx_graph_set_user_metadata updates the device-resident template in stream order;
+    the eager setter refuses in graph mode instead of silently doing nothing.  Replica slots vs the oracle's, byte
+    for byte, and the restored blob."""
+    wl = W.tiny_workload([50_000, 77], dp_size=1)
+    blob0, blob1, blob2 = b"rng-state-at-begin", bytes(range(1, 129)), b"x"
+    s, o, gdev, gbits = make_pair(wl, steps=7, chunk_bytes=64 << 10, user=blob0)
+    hp = hp_of(wl)
+    cap, side = torch.cuda.Stream(device=DEV), torch.cuda.Stream(device=DEV)
+    gbuf = [torch.zeros_like(gdev[0]) for _ in range(2)]
+    s.graph_begin(stream=cap)
+    assert B.lib().phx_set_user_metadata(s.h, blob1, len(blob1)) == B.PHX_ERR_GRAPH_MODE
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=cap):
+        for i in range(2):
+            s.graph_step(gbuf[(1 + i) % 2], stream=cap)     # issue indices 1, 2
+            side.wait_stream(cap)
+            s.graph_flush(side)
+            cap.wait_stream(side)
+        assert B.lib().phx_graph_set_user_metadata(s.h, blob1, len(blob1), cap.cuda_stream) == B.PHX_ERR_INVALID_ARG
+        assert B.lib().phx_graph_set_hyper(s.h, 1e-3, 0.9, 0.95, 1e-8, 0.0, cap.cuda_stream) == B.PHX_ERR_INVALID_ARG
+    t = 0
+    for blob in (None, blob1, blob2):                       # replay 1 keeps the blob of begin
+        if blob is not None:
+            B.phx_graph_set_user_metadata(s.h, blob, cap)
+            o.user = blob
+        for i in range(2):
+            t += 1
+            with torch.cuda.stream(cap):
+                gbuf[t % 2].copy_(gdev[t - 1])
+            o.step(gbits[t - 1], **hp, step=t)
+            o.snapshot()
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        for k in (t - 1, t):
+            assert np.array_equal(s.replica_slot(k).numpy(), o.replica[k % 2]), (t, k)
+        hdr = O.parse_header(s.replica_slot(t).numpy()[:256].tobytes())
+        assert hdr["user"] == (blob0 if blob is None else blob)
+    assert s.graph_end() == 6
+    # the eager calls carry the last blob on, and a restore hands it back
+    s.step_and_snapshot(gdev[6], 7); s.flush_async(side); s.wait(7)
+    o.step(gbits[6], **hp, step=7); o.snapshot()
+    assert np.array_equal(s.replica_slot(7).numpy(), o.replica[1])
+    s.drop_live()
+    assert s.restore() == 7
+    assert B.phx_restored_user_metadata(s.h) == blob2
+    s.close()
+
+
 def test_graph_form_protocol_errors():
     wl = W.tiny_workload([8192], dp_size=1)
     s, _, gdev, _ = make_pair(wl, steps=1)

@@ -100,3 +100,39 @@ def test_no_byte_outside_the_bound_buffers_is_touched(numels, rmode):
     B.phx_shard_bind_param_peers(h, [])
     B.phx_shard_bind_peers(h, [])
     B.phx_shard_destroy(h)
+
+
+def test_bind_rejects_pointers_that_are_not_device_memory_of_the_current_device():
+    """SURVEY §8(b) "Ownership" / VERDICT r2 item 4: phx_shard_bind validates the KIND of every d_* pointer with
+    cudaPointerGetAttributes.  A pinned host pointer (which the GPU could even reach) or plain pageable memory passed
+    as d_p used to be accepted and fault — or silently train on host memory — at the first step."""
+    h = B.phx_shard_create([(4096, 0)], 1, 0, chunk_bytes=64 << 10)
+    info = B.phx_shard_info(h)
+    N = info.n_padded
+    dev = {k: torch.zeros(N, dtype=torch.float32, device=DEV) for k in ("p", "m", "v")}
+    p16 = torch.zeros(N, dtype=torch.bfloat16, device=DEV)
+    staging = torch.zeros(2 * info.slot_stride, dtype=torch.uint8, device=DEV)
+    replica = torch.zeros(2 * info.host_slot_stride, dtype=torch.uint8).pin_memory()
+    pinned = torch.zeros(N + 64, dtype=torch.float32).pin_memory()
+    pageable = torch.zeros(N + 64, dtype=torch.float32)
+    L = B.lib()
+
+    def bind(p=None, m=None, v=None, b16=None, st=None):
+        return L.phx_shard_bind(h, (p if p is not None else dev["p"]).data_ptr(), (m if m is not None else dev["m"]).data_ptr(),
+                                (v if v is not None else dev["v"]).data_ptr(), (b16 if b16 is not None else p16).data_ptr(),
+                                (st if st is not None else staging).data_ptr(), replica.data_ptr())
+
+    def aligned(t):
+        off = (-t.data_ptr() % 256) // t.element_size()
+        return t[off:]
+
+    assert bind(p=aligned(pinned)) == B.PHX_ERR_INVALID_ARG
+    assert bind(m=aligned(pageable)) == B.PHX_ERR_INVALID_ARG
+    assert bind(v=aligned(pinned)) == B.PHX_ERR_INVALID_ARG
+    assert bind(st=aligned(pinned.view(torch.uint8))) == B.PHX_ERR_INVALID_ARG
+    # a device pointer as the host replica is refused as before (not pinned, mapped host memory)
+    assert L.phx_shard_bind(h, dev["p"].data_ptr(), dev["m"].data_ptr(), dev["v"].data_ptr(), p16.data_ptr(),
+                            staging.data_ptr(), staging.data_ptr()) == B.PHX_ERR_INVALID_ARG
+    assert bind() == B.PHX_OK                              # nothing above left the handle half-bound
+    assert b"bound on" in L.phx_strerror(B.PHX_ERR_WRONG_DEVICE)
+    B.phx_shard_destroy(h)
