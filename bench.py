@@ -978,7 +978,8 @@ class Rig:
                 "restore_plus_recompute_ms": r0.elapsed_time(r2), "restore_plus_recompute_wall_ms": wall_ms,
                 "host_link_gbs": 12 * N / (rms * 1e-3) / 1e9, "trajectory_bit_exact_vs_uninterrupted": bool(same),
                 "steps_before_fault": 20, "steps_after": 5, "gemms_per_iter": G, "mode": self.restore_mode_name,
-                "fault": "second stream, no host sync: flush(20) and step 21 in flight; restore_ms includes the rest of flush(20)"}
+                "fault": "second stream, no host sync: lands while flush(20) is in flight and step 21 is queued or running; the timed "
+                         "region starts on the compute stream behind step 21"}
 
     # -- the stand-in compute window ----------------------------------------------------------------
     def gemm_setup(self):
