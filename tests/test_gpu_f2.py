@@ -165,43 +165,3 @@ def test_f2_fp32_shard_needs_no_bf16_buffer_but_bf16_precision_does():
                          torch.zeros(2 * (256 + 12 * 4096), dtype=torch.uint8).pin_memory())
     assert e.value.code == B.PHX_ERR_INVALID_ARG
     B.phx_shard_destroy(h)
-
-
-def test_c2_full_size_fp32_with_groups_sampled_parity():
-    """The 1.3B-style shard in the paper's precision with GPT parameter groups, in the launch configuration
-    bench.py times: sampled windows against the oracle element by element (including windows that straddle a
-    bias / LayerNorm tensor), full-size properties for the rest."""
-    wl = dataclasses.replace(W.CONFIGS["c2"], decay_groups=True, precision="fp32")
-    s = Shard(wl, device=DEV)
-    N = s.n_padded
-    s.p.copy_(W.init_params(s.n, N, wl.seed, device=DEV))
-    s.set_state(0)
-    rng = np.random.default_rng(12)
-    flags = wl.flags()
-    starts = [0, N - 4096]
-    for tid, off, ln in s.segments:                       # windows around no-decay tensors
-        if flags[tid] and len(starts) < 40:
-            starts.append(max(0, (off - 1000) // 64 * 64))
-    starts += [int(x) // 64 * 64 for x in rng.integers(0, N - 4096, 16)]
-    wins = [(a, min(a + 4096, N)) for a in starts]
-    idx = torch.cat([torch.arange(a, b) for a, b in wins]).to(DEV)
-    o = O.OracleShard(wl.layout(), wl.dp_size, wl.dp_rank, flags=flags, precision="fp32")
-    mask = np.ascontiguousarray(o.no_decay[idx.cpu().numpy()])
-    assert 0 < mask.sum() < mask.size
-    ref = dict(p=s.p[idx].cpu().numpy().copy(), m=np.zeros(idx.numel(), np.float32), v=np.zeros(idx.numel(), np.float32))
-    hp = hp_of(wl)
-    for t in range(1, 4):
-        g = W.gen_grads(wl, s.segments, N, t, wl.seed, device=DEV, dtype=torch.float32)
-        s.step_and_snapshot(g, t)
-        gs = g[idx].cpu().numpy().copy()
-        O.adamw_step_ex(ref["p"], ref["m"], ref["v"], gs, None, mask, hp["lr"], hp["beta1"], hp["beta2"], hp["eps"],
-                        hp["wd"], t, 1.0, 4)
-        torch.cuda.synchronize()
-        for name, dev in (("p", s.p), ("m", s.m), ("v", s.v)):
-            assert np.array_equal(dev[idx].cpu().numpy().view(np.uint32), ref[name].view(np.uint32)), (name, t)
-        st = s.staging_slot(t)
-        assert torch.equal(st[256:256 + 4 * N].view(torch.float32), s.p)
-        assert torch.equal(st[256 + 4 * N:256 + 8 * N].view(torch.float32), s.m)
-        assert torch.equal(st[256 + 8 * N:].view(torch.float32), s.v)
-        del g
-    s.close()

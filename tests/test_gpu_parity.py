@@ -366,73 +366,15 @@ def test_protocol_errors_on_device():
 
 
 # ------------------------------------------------------------------------------------------------
-# full size, in the launch configuration bench.py times: sampled element-by-element parity and
-# properties that hold at any size
+# full size, in the launch configuration bench.py times.  Every element of c2, c3, c4a, c4b and c5 is compared with
+# the oracle in tests/test_gpu_fullsize.py (the sampled-window tests that stood here were superseded by it and
+# removed in round 3); what remains here is the configs[3] hot-swap trajectory.
 # ------------------------------------------------------------------------------------------------
 
 
 def _sample_windows(n_padded, rng, k=48, w=4096):
     starts = [0, max(0, n_padded - w)] + [int(x) // 64 * 64 for x in rng.integers(0, max(1, n_padded - w), k)]
     return [(a, min(a + w, n_padded)) for a in starts]
-
-
-@pytest.mark.parametrize("key", ["c2", "c3"])
-def test_full_size_sampled_parity(key):
-    wl = W.CONFIGS[key]
-    free, _ = torch.cuda.mem_get_info()
-    s = Shard(wl, device=DEV)
-    N = s.n_padded
-    s.p.copy_(W.init_params(s.n, N, wl.seed, device=DEV))
-    s.set_state(0)
-    rng = np.random.default_rng(11)
-    wins = _sample_windows(N, rng)
-    idx = torch.cat([torch.arange(a, b) for a, b in wins]).to(DEV)
-    ref = dict(p=s.p[idx].cpu().numpy().copy(), m=np.zeros(idx.numel(), np.float32),
-               v=np.zeros(idx.numel(), np.float32), h=np.zeros(idx.numel(), np.uint16))
-    side = side_stream()
-    hp = hp_of(wl)
-    for t in range(1, 4):
-        g = W.gen_grads(wl, s.segments, N, t, wl.seed, device=DEV)
-        s.step_and_snapshot(g, t)
-        s.flush_async(side)
-        coef = 1.0
-        if wl.hyper.max_grad_norm > 0:
-            coef, S = B.phx_last_clip(s.h)
-            # full-size sum of squares against an independent fp64 reduction (torch), then the
-            # oracle's coefficient formula on the oracle's own sum over the full gradient
-            gb = bits16(g)
-            So = O.sumsq(gb)
-            assert abs(S - So) <= 1e-13 * So
-            assert np.float32(coef) == O.clip_coef(So, wl.hyper.max_grad_norm)
-            assert 0.02 < coef < 0.2          # clip always active at c3 statistics (~0.048)
-        gs = bits16(g[idx]).copy()
-        O.adamw_step(ref["p"], ref["m"], ref["v"], gs, ref["h"], **hp, step=t, coef=float(coef), nthreads=4)
-        torch.cuda.synchronize()
-        assert np.array_equal(s.p[idx].cpu().numpy().view(np.uint32), ref["p"].view(np.uint32)), t
-        assert np.array_equal(s.m[idx].cpu().numpy().view(np.uint32), ref["m"].view(np.uint32)), t
-        assert np.array_equal(s.v[idx].cpu().numpy().view(np.uint32), ref["v"].view(np.uint32)), t
-        assert np.array_equal(bits16(s.p16[idx]), ref["h"]), t
-        # properties at full size: staging planes == live planes; bf16 copy == RNE(p); replica == staging
-        st = s.staging_slot(t)
-        assert torch.equal(st[256:256 + 4 * N].view(torch.float32), s.p)
-        assert torch.equal(st[256 + 4 * N:256 + 8 * N].view(torch.float32), s.m)
-        assert torch.equal(st[256 + 8 * N:].view(torch.float32), s.v)
-        assert torch.equal(s.p.to(torch.bfloat16), s.p16)
-        del g
-    s.wait(3)
-    rep = s.replica_slot(3)
-    CH = 1 << 28
-    for off in range(0, rep.numel(), CH):
-        assert torch.equal(rep[off:off + CH].to(DEV), s.staging_slot(3)[off:off + CH])
-    hdr = O.parse_header(rep[:256].numpy().tobytes())
-    assert hdr is not None and hdr["step"] == 3 and hdr["n"] == wl.n_expected
-    before = [x.clone() for x in (s.p, s.m, s.v, s.p16)]
-    s.drop_live()
-    assert s.restore() == 3
-    torch.cuda.synchronize()
-    for a, b in zip((s.p, s.m, s.v, s.p16), before):
-        assert torch.equal(a, b)
-    s.close()
 
 
 def test_c4a_hot_swap_recovery_trajectory_bit_exact():
